@@ -164,7 +164,7 @@ def random_tree_parent(n: int, stream, max_children: int = 3) -> np.ndarray:
 
 
 def random_tree_cells(n_cell, n_lo, n_hi, stream="rtree", mech="pas", identical=False,
-                      with_ring=True, weight=0.05, delay=1.0):
+                      with_ring=True, weight=0.05, delay=1.0, amp=0.5):
     """Cells with seeded random topology; optional ring of ExpSyn NetCons and an IClamp on cell 0.
 
     mech = "pas" (passive dendrites + HH soma) or "hh" (HH everywhere).
@@ -208,7 +208,7 @@ def random_tree_cells(n_cell, n_lo, n_hi, stream="rtree", mech="pas", identical=
                                         "e": _const(len(pn), -65.0)}))
     syn_t = len(mechs)
     mechs.append(_mech("expsyn", roots, {"tau": _const(n_cell, 2.0), "e": _const(n_cell, 0.0)}))
-    mechs.append(_mech("iclamp", [roots[0]], {"del": [1.0], "dur": [1.0], "amp": [0.5]}))
+    mechs.append(_mech("iclamp", [roots[0]], {"del": [1.0], "dur": [1.0], "amp": [amp]}))
     if with_ring and n_cell > 1:
         src = np.arange(n_cell)
         nc = _netcons(src, np.full(n_cell, syn_t), (src + 1) % n_cell, _const(n_cell, weight),

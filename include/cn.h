@@ -1,0 +1,150 @@
+/*
+ * cn.h -- C ABI of libcn: B200-native fixed-step time integration of networks of
+ * multi-compartment neurons (the hot path of arxiv 1901.10975, "CoreNEURON").
+ *
+ * Each dt runs, entirely on the device:
+ *   event-driven spike delivery (L64) -> matrix assembly: per-mechanism currents and
+ *   conductances plus the tree terms of the discretised cable equation (L65, Eq. 1)
+ *   -> Hines tree solve (L62 "direct Gaussian elimination", L66) -> voltage update (L66)
+ *   -> per-mechanism state update, cnexp / derivimplicit (L67, L278)
+ *   -> threshold detection and NetCon event generation with delays (L68, L62, L156).
+ *
+ * Conventions
+ *   - All pointers in cn_model_desc are HOST pointers; cn_model_create deep-copies, so the
+ *     caller may free them on return.  Output pointers are HOST pointers owned by the caller.
+ *   - The model owns its device and host memory until cn_model_destroy.
+ *   - Every call returns a status (CN_OK or a negative CN_ERR_*), never throws or aborts;
+ *     cn_last_error() gives a thread-local message for the last non-OK return.
+ *   - Units (L58-60): mV, ms, uF/cm2, S/cm2 and mA/cm2 for distributed mechanisms; point
+ *     processes in nA and uS (converted by 100/area[um2], L60); area um2; axial resistance MOhm.
+ *   - All indices in and out are in the caller's order; the internal permutation is invisible.
+ *   - No CPU fallback exists: without a CUDA device every compute call fails with CN_ERR_CUDA.
+ */
+#ifndef CN_H
+#define CN_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cn_model cn_model; /* opaque */
+
+enum {
+  CN_OK = 0,
+  CN_ERR_ARG = -1,      /* NULL / non-finite / out-of-range scalar or array argument */
+  CN_ERR_TOPOLOGY = -2, /* parent[] is not a forest with parent[i] < i inside each cell */
+  CN_ERR_MECH = -3,     /* unknown mechanism type, wrong parameter count, node out of range */
+  CN_ERR_NETCON = -4,   /* NetCon source/target out of range, or delay rounds to < 1 step */
+  CN_ERR_DT = -5,       /* dt <= 0 or different from the dt of the first cn_run */
+  CN_ERR_CUDA = -6,     /* CUDA runtime error (message in cn_last_error) */
+  CN_ERR_OVERFLOW = -7, /* spike buffer overflowed during a run; results are invalid */
+  CN_ERR_NOMEM = -8,    /* host or device allocation failed */
+  CN_ERR_UNSUPPORTED = -9 /* a cell too large for the on-chip solve */
+};
+
+/* Mechanism types.  Parameter order = row order of cn_mech_table.param. */
+enum {
+  CN_PAS = 1,      /* i = g (v - e)                         param: g, e                       */
+  CN_HH = 2,       /* Hodgkin-Huxley squid Na/K/leak        param: gnabar, gkbar, gl, el
+                      global: ena, ek.  Temperature factor 3^((celsius-6.3)/10).              */
+  CN_EXPSYN = 3,   /* point: i = g (v - e), g' = -g/tau     param: tau, e ; event: g += w     */
+  CN_EXP2SYN = 4,  /* point: i = (B-A)(v-e)                 param: tau1, tau2, e (tau1<tau2)
+                      event: A += w f, B += w f, f normalises the peak to w                   */
+  CN_ICLAMP = 5,   /* point: current amp for del <= t < del+dur   param: del, dur, amp (nA)
+                      sampled at the step midpoint (k + 1/2) dt                               */
+  CN_HHFORM = 6,   /* i = gbar m^p h^q (v - E)              param: gbar
+                      global: p, q, E, to_ica, m:(vh,k,t0,t1,vt,s), h:(vh,k,t0,t1,vt,s)
+                      xinf = 1/(1+exp((vh-v)/k)), tau = t0 + t1/(exp((v-vt)/s)+exp(-(v-vt)/s)) */
+  CN_SK = 7,       /* i = gbar z (v - E), zinf = 1/(1+(Kd/cai)^n)  param: gbar
+                      global: E, Kd, n, tau_z                                                 */
+  CN_CADYN = 8,    /* cai' = -(1e4 gamma/(2 F depth)) ica - (cai-cai_min)/tau_d  (derivimplicit)
+                      no param ; global: gamma, depth, tau_d, cai_min                         */
+  CN_AMPANMDA = 9  /* point: AMPA + NMDA double exponentials with Mg block
+                      no param ; global: tau_r_A, tau_d_A, tau_r_N, tau_d_N, r_nmda, mg, e    */
+};
+
+/* One mechanism type = one instance table, structure of arrays (L178, Fig. 3D). */
+typedef struct {
+  int32_t type;          /* CN_PAS ... */
+  int64_t n;             /* number of instances */
+  const int32_t *node;   /* [n] global node index, caller order */
+  int32_t n_param;       /* must equal the type's parameter count */
+  const double *param;   /* [n_param][n]: parameter j of instance i at param[j*n + i] */
+  int32_t n_global;      /* must equal the type's global count */
+  const double *global;  /* [n_global] per-table constants */
+} cn_mech_table;
+
+typedef struct {
+  int32_t n_cell;
+  int64_t n_node;
+  const int64_t *cell_first;  /* [n_cell+1]; node cell_first[c] is the root (soma) of cell c;
+                                 the spike source id (gid) of cell c is c */
+  const int32_t *parent;      /* [n_node] global index; -1 for roots; parent[i] < i, same cell */
+  const double *area_um2;     /* [n_node] membrane area, > 0 */
+  const double *ri_MOhm;      /* [n_node] axial resistance node <-> parent, > 0 (ignored at roots) */
+  const double *cm_uF_cm2;    /* [n_node] specific capacitance, > 0 */
+  double v_init_mV;           /* initial voltage of every node; gates start at steady state */
+  double celsius;
+  int32_t n_mech;
+  const cn_mech_table *mech;  /* currents and states are evaluated in table order */
+  int64_t n_netcon;           /* NetCons, structure of arrays (L62, L156) */
+  const int32_t *nc_src_gid;  /* cell gid (< n_cell) or scripted source gid (>= n_cell) */
+  const int32_t *nc_tgt_mech; /* index into mech[]; must be a point process with a receive rule */
+  const int64_t *nc_tgt_inst; /* instance within that table */
+  const double *nc_weight_uS;
+  const double *nc_delay_ms;  /* quantised as llround(delay/dt) steps at the first cn_run; >= 1 */
+  const double *thr_mV;       /* [n_cell] threshold on the root node: spike iff v rises above */
+  int64_t n_stim;             /* scripted source spikes (artificial spike sources) */
+  const int32_t *stim_gid;    /* [n_stim] >= n_cell */
+  const double *stim_t_ms;    /* [n_stim] >= 0; spike step = llround(t/dt) */
+} cn_model_desc;
+
+/* Validate, find shape classes, choose the permutation, upload.  *out is NULL on failure. */
+int cn_model_create(const cn_model_desc *desc, cn_model **out);
+
+/* Advance to ABSOLUTE time tstop with fixed step dt: K = llround(tstop/dt) - steps_done steps
+ * (K <= 0 is a no-op).  dt is fixed by the first call.  Runs on `stream` set by cn_set_stream
+ * (default: the legacy default stream) and synchronises it before returning. */
+int cn_run(cn_model *m, double tstop_ms, double dt_ms);
+
+/* Same as cn_run but returns without synchronising; cn_sync() waits and reports overflow. */
+int cn_run_async(cn_model *m, double tstop_ms, double dt_ms);
+int cn_sync(cn_model *m);
+
+/* cudaStream_t (as void*) on which all work of this model is issued. */
+int cn_set_stream(cn_model *m, void *cuda_stream);
+
+/* Current voltages in caller node order; n must equal n_node. */
+int cn_get_v(const cn_model *m, double *v_out, int64_t n);
+
+/* Spikes (gid, step) sorted by (step, gid); a spike detected after the update to t_{k+1} has
+ * step k+1.  Pass cap = 0 to query *n_out only. */
+int cn_get_spikes(const cn_model *m, int32_t *gid, int64_t *step, int64_t cap, int64_t *n_out);
+
+/* Record v of the given nodes after every step (before the first cn_run only). */
+int cn_set_probes(cn_model *m, const int32_t *node, int64_t n, int64_t max_steps);
+/* trace_out[s*n_probe + j] = v(node j) after step s; *n_steps_out = steps recorded. */
+int cn_get_trace(const cn_model *m, double *trace_out, int64_t cap_steps, int64_t *n_steps_out);
+
+/* State s of mechanism table t in caller instance order (for parity tests); n = table size. */
+int cn_get_state(const cn_model *m, int32_t t, int32_t s, double *out, int64_t n);
+
+int64_t cn_steps_done(const cn_model *m);
+/* Number of kernels launched by this model so far (for bench.py's gpu_launches). */
+int64_t cn_launch_count(const cn_model *m);
+/* Device pointer + stream-ordered timing of the step kernels of the last run, in ms, measured
+ * with CUDA events on the model's stream around the step loop. */
+int cn_last_run_ms(const cn_model *m, double *ms_out);
+/* Layout facts for DESIGN/bench: n_class, n_group, smem bytes per warp, rounds (max). */
+int cn_get_layout_info(const cn_model *m, int64_t *info4);
+/* Spike buffer capacity (default 16*n_cell + 65536); before the first cn_run only. */
+int cn_set_spike_capacity(cn_model *m, int64_t cap);
+
+void cn_model_destroy(cn_model *m);
+const char *cn_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

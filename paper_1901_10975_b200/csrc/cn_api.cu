@@ -1,0 +1,1121 @@
+// cn_api.cu -- host side of libcn: validation, shape classes, permutation, upload, step loop.
+// C ABI declared in include/cn.h.  No CPU compute path exists: every step runs in cn_device.cuh.
+#include "../../include/cn.h"
+#include "cn_device.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+using namespace cn;
+
+// ---------------------------------------------------------------------------------------------
+// errors
+// ---------------------------------------------------------------------------------------------
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CU(call)                                                                         \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess)                                                               \
+      return fail(e_ == cudaErrorMemoryAllocation ? CN_ERR_NOMEM : CN_ERR_CUDA,          \
+                  "%s failed: %s", #call, cudaGetErrorString(e_));                       \
+  } while (0)
+
+extern "C" const char *cn_last_error(void) { return g_err; }
+
+// ---------------------------------------------------------------------------------------------
+// mechanism metadata
+// ---------------------------------------------------------------------------------------------
+
+struct TypeInfo { int n_param, n_state, n_global, point, n_dev_param; };
+
+static bool type_info(int type, TypeInfo &ti) {
+  switch (type) {
+    case CN_PAS: ti = {2, 0, 0, 0, 0}; return true;       // folded into the static arrays
+    case CN_HH: ti = {4, 3, 2, 0, 5}; return true;        // + invc
+    case CN_EXPSYN: ti = {2, 1, 0, 1, 3}; return true;    // + scale
+    case CN_EXP2SYN: ti = {3, 2, 0, 1, 5}; return true;   // + scale, factor
+    case CN_ICLAMP: ti = {3, 0, 0, 1, 4}; return true;    // + scale
+    case CN_HHFORM: ti = {1, 2, 16, 0, 2}; return true;   // + invc
+    case CN_SK: ti = {1, 1, 4, 0, 2}; return true;        // + invc
+    case CN_CADYN: ti = {0, 0, 4, 0, 0}; return true;
+    case CN_AMPANMDA: ti = {0, 4, 7, 1, 1}; return true;  // scale
+  }
+  return false;
+}
+
+static double h_vtrap(double x, double y) {
+  double u = x / y;
+  if (std::fabs(u) < 1e-6) return y * (1.0 - u / 2.0);
+  return x / (std::exp(u) - 1.0);
+}
+
+static double h_exp2_factor(double t1, double t2) {
+  double tp = (t1 * t2) / (t2 - t1) * std::log(t2 / t1);
+  return 1.0 / (std::exp(-tp / t2) - std::exp(-tp / t1));
+}
+
+// ---------------------------------------------------------------------------------------------
+// model
+// ---------------------------------------------------------------------------------------------
+
+struct HTable {
+  int type = 0;
+  TypeInfo ti{};
+  int64_t n = 0;
+  std::vector<int32_t> node;
+  std::vector<double> param;  // [n_param][n]
+  std::vector<double> glob;
+  // layout
+  int64_t n_dev = 0;               // padded device instance count
+  std::vector<int64_t> inst_pos;   // caller instance -> device instance
+  // device
+  double *d_param[CN_MAX_PARAM] = {};
+  double *d_state[CN_MAX_STATE] = {};
+  int64_t *d_pp_first = nullptr;
+  int32_t *d_pp_slot = nullptr;
+  int32_t *d_cls_cnt = nullptr, *d_cls_nodeoff = nullptr;
+  int64_t *d_grp_instbase = nullptr;
+  // host layout tables
+  std::vector<int64_t> pp_first;
+  std::vector<int32_t> pp_slot;
+  std::vector<int32_t> cls_cnt, cls_nodeoff;
+  std::vector<int64_t> grp_instbase;
+  // per-cell CSR of distributed instances sorted by local node
+  std::vector<int64_t> cell_first;
+  std::vector<int64_t> cell_inst;
+};
+
+struct HClass {
+  int n = 0, G = 1, lgG = 0, rounds = 0, needs_ica = 0;
+  int rep_cell = -1;
+  int64_t count = 0;
+  int sched_off = 0;
+  std::vector<int32_t> cells;
+  std::vector<uint32_t> sched;
+};
+
+struct cn_model {
+  // description (deep copy)
+  int32_t n_cell = 0;
+  int64_t N = 0;
+  std::vector<int64_t> cell_first;
+  std::vector<int32_t> parent;
+  std::vector<double> area, ri, cm, thr;
+  double v_init = -65.0, celsius = 6.3;
+  std::vector<HTable> tab;
+  int64_t n_netcon = 0;
+  std::vector<int32_t> nc_src, nc_tgt_mech;
+  std::vector<int64_t> nc_tgt_inst;
+  std::vector<double> nc_w, nc_delay;
+  std::vector<int32_t> stim_gid;
+  std::vector<double> stim_t;
+  int32_t n_src = 0;
+  // layout
+  std::vector<HClass> cls;
+  std::vector<GroupInfo> grp;
+  std::vector<int32_t> cell_cls, cell_grp, cell_slot;
+  std::vector<int64_t> node_pos;  // caller node -> device node
+  std::vector<int32_t> dist_nodes;  // per class and distributed table: local node lists
+  int64_t n_pnode = 0, n_ab = 0;
+  int32_t n_pcell = 0;
+  int warp_smem_doubles = 0, wpb = 4;
+  bool any_ica = false, any_cai = false;
+  // run state
+  double dt = 0.0;
+  int64_t k = 0;
+  bool uploaded = false;
+  int64_t launches = 0;
+  int64_t sp_cap = 0;
+  cudaStream_t stream = 0;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timed = false;
+  // probes
+  std::vector<int32_t> probe;
+  int64_t probe_cap = 0, probe_rows = 0;
+  // device
+  std::vector<void *> dev_allocs;
+  DModel hm{};
+  DModel *d_m = nullptr;
+  double *d_v = nullptr, *d_cai = nullptr, *d_trace = nullptr, *d_gather = nullptr;
+  int64_t *d_node_pos = nullptr, *d_probe_pos = nullptr;
+  int32_t *d_overflow = nullptr;
+  unsigned long long *d_nsp = nullptr;
+  int32_t *d_sp_gid = nullptr;
+  int64_t *d_sp_step = nullptr;
+};
+
+template <class T>
+static int dev_upload(cn_model *m, const std::vector<T> &h, T **out, size_t min_elems = 1) {
+  size_t n = std::max(h.size(), min_elems);
+  void *p = nullptr;
+  CU(cudaMalloc(&p, n * sizeof(T)));
+  m->dev_allocs.push_back(p);
+  if (!h.empty()) CU(cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  if (h.size() < n)
+    CU(cudaMemset((char *)p + h.size() * sizeof(T), 0, (n - h.size()) * sizeof(T)));
+  *out = (T *)p;
+  return CN_OK;
+}
+
+template <class T>
+static int dev_alloc(cn_model *m, size_t n, T **out, bool zero = true) {
+  void *p = nullptr;
+  if (n == 0) n = 1;
+  CU(cudaMalloc(&p, n * sizeof(T)));
+  m->dev_allocs.push_back(p);
+  if (zero) CU(cudaMemset(p, 0, n * sizeof(T)));
+  *out = (T *)p;
+  return CN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// list scheduling of the elimination (Hu's level algorithm for in-trees, P nodes per round,
+// at most one child of a parent per round so that the parent updates never collide)
+// ---------------------------------------------------------------------------------------------
+
+static int hu_schedule(int n, const int32_t *par, int P, std::vector<uint32_t> &out) {
+  out.clear();
+  if (n <= 1) return 0;
+  std::vector<int> depth(n, 0), left(n, 0), used(n, -1);
+  int maxd = 0;
+  for (int i = 1; i < n; ++i) {
+    depth[i] = depth[par[i]] + 1;
+    left[par[i]]++;
+    maxd = std::max(maxd, depth[i]);
+  }
+  std::vector<std::vector<int>> bucket(maxd + 1);
+  for (int i = 1; i < n; ++i)
+    if (left[i] == 0) bucket[depth[i]].push_back(i);
+  int remaining = n - 1, round = 0;
+  std::vector<int> picked;
+  while (remaining > 0) {
+    picked.clear();
+    for (int dl = maxd; dl >= 1 && (int)picked.size() < P; --dl) {
+      auto &bk = bucket[dl];
+      for (size_t j = 0; j < bk.size() && (int)picked.size() < P;) {
+        int i = bk[j];
+        if (used[par[i]] != round) {
+          used[par[i]] = round;
+          picked.push_back(i);
+          bk[j] = bk.back();
+          bk.pop_back();
+        } else {
+          ++j;
+        }
+      }
+    }
+    for (int i : picked) {
+      out.push_back((uint32_t)i | ((uint32_t)par[i] << 16));
+      --remaining;
+      int p = par[i];
+      if (--left[p] == 0 && p != 0) bucket[depth[p]].push_back(p);
+    }
+    for (int j = (int)picked.size(); j < P; ++j) out.push_back(CN_IDLE | (CN_IDLE << 16));
+    ++round;
+  }
+  return round;
+}
+
+// ---------------------------------------------------------------------------------------------
+// create: validate + deep copy + shape classes + permutation (dt-independent part)
+// ---------------------------------------------------------------------------------------------
+
+static bool finite_all(const double *x, int64_t n) {
+  for (int64_t i = 0; i < n; ++i)
+    if (!std::isfinite(x[i])) return false;
+  return true;
+}
+
+static int build_layout(cn_model *m);
+
+extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
+  if (out) *out = nullptr;
+  if (!de || !out) return fail(CN_ERR_ARG, "cn_model_create: NULL argument");
+  if (de->n_cell < 0 || de->n_node < 0) return fail(CN_ERR_ARG, "negative sizes");
+  if (de->n_node >= (int64_t)1 << 31) return fail(CN_ERR_ARG, "n_node must be < 2^31");
+  if (de->n_mech < 0 || de->n_mech > CN_MAX_TABLES)
+    return fail(CN_ERR_MECH, "n_mech must be in [0, %d]", CN_MAX_TABLES);
+  const int64_t N = de->n_node;
+  if (de->n_cell > 0 &&
+      (!de->cell_first || !de->parent || !de->area_um2 || !de->ri_MOhm || !de->cm_uF_cm2 ||
+       !de->thr_mV))
+    return fail(CN_ERR_ARG, "NULL node / cell array");
+  if (de->n_cell > 0 && (de->cell_first[0] != 0 || de->cell_first[de->n_cell] != N))
+    return fail(CN_ERR_TOPOLOGY, "cell_first must start at 0 and end at n_node");
+  if (de->n_cell == 0 && N != 0) return fail(CN_ERR_TOPOLOGY, "nodes without cells");
+  for (int32_t c = 0; c < de->n_cell; ++c) {
+    const int64_t f = de->cell_first[c], l = de->cell_first[c + 1];
+    if (l <= f) return fail(CN_ERR_TOPOLOGY, "cell %d is empty", c);
+    if (l - f > 65534) return fail(CN_ERR_UNSUPPORTED, "cell %d has more than 65534 nodes", c);
+    if (de->parent[f] != -1) return fail(CN_ERR_TOPOLOGY, "root of cell %d has a parent", c);
+    for (int64_t i = f + 1; i < l; ++i)
+      if (de->parent[i] < f || de->parent[i] >= i)
+        return fail(CN_ERR_TOPOLOGY, "parent[%lld] = %d violates parent < child inside cell %d",
+                    (long long)i, de->parent[i], c);
+  }
+  if (!finite_all(de->area_um2, N) || !finite_all(de->ri_MOhm, N) ||
+      !finite_all(de->cm_uF_cm2, N) || !finite_all(de->thr_mV, de->n_cell) ||
+      !std::isfinite(de->v_init_mV) || !std::isfinite(de->celsius))
+    return fail(CN_ERR_ARG, "non-finite value in a node / cell array");
+  for (int64_t i = 0; i < N; ++i) {
+    if (!(de->area_um2[i] > 0.0) || !(de->cm_uF_cm2[i] > 0.0))
+      return fail(CN_ERR_ARG, "area and cm must be > 0 (node %lld)", (long long)i);
+    if (de->parent[i] >= 0 && !(de->ri_MOhm[i] > 0.0))
+      return fail(CN_ERR_ARG, "ri must be > 0 (node %lld)", (long long)i);
+  }
+  for (int32_t t = 0; t < de->n_mech; ++t) {
+    const cn_mech_table &mt = de->mech[t];
+    TypeInfo ti;
+    if (!type_info(mt.type, ti)) return fail(CN_ERR_MECH, "table %d: unknown type %d", t, mt.type);
+    if (mt.n < 0 || mt.n_param != ti.n_param || mt.n_global != ti.n_global)
+      return fail(CN_ERR_MECH, "table %d: type %d needs %d params and %d globals", t, mt.type,
+                  ti.n_param, ti.n_global);
+    if (mt.n > 0 && (!mt.node || (ti.n_param > 0 && !mt.param)))
+      return fail(CN_ERR_MECH, "table %d: NULL array", t);
+    if (ti.n_global > 0 && !mt.global) return fail(CN_ERR_MECH, "table %d: NULL globals", t);
+    for (int64_t i = 0; i < mt.n; ++i)
+      if (mt.node[i] < 0 || mt.node[i] >= N)
+        return fail(CN_ERR_MECH, "table %d: node of instance %lld out of range", t, (long long)i);
+    if (!finite_all(mt.param, mt.n * ti.n_param) || !finite_all(mt.global, ti.n_global))
+      return fail(CN_ERR_MECH, "table %d: non-finite parameter", t);
+    if (mt.type == CN_EXP2SYN)
+      for (int64_t i = 0; i < mt.n; ++i)
+        if (!(mt.param[i] > 0.0) || !(mt.param[mt.n + i] > mt.param[i]))
+          return fail(CN_ERR_MECH, "table %d: Exp2Syn needs 0 < tau1 < tau2", t);
+    if (mt.type == CN_EXPSYN)
+      for (int64_t i = 0; i < mt.n; ++i)
+        if (!(mt.param[i] > 0.0)) return fail(CN_ERR_MECH, "table %d: ExpSyn needs tau > 0", t);
+  }
+  if (de->n_netcon < 0 || de->n_stim < 0) return fail(CN_ERR_NETCON, "negative count");
+  int32_t n_src = de->n_cell;
+  for (int64_t i = 0; i < de->n_netcon; ++i) {
+    const int32_t tm = de->nc_tgt_mech[i];
+    if (tm < 0 || tm >= de->n_mech) return fail(CN_ERR_NETCON, "netcon %lld: bad table", (long long)i);
+    const int ty = de->mech[tm].type;
+    if (ty != CN_EXPSYN && ty != CN_EXP2SYN && ty != CN_AMPANMDA)
+      return fail(CN_ERR_NETCON, "netcon %lld: target type %d receives no events", (long long)i, ty);
+    if (de->nc_tgt_inst[i] < 0 || de->nc_tgt_inst[i] >= de->mech[tm].n)
+      return fail(CN_ERR_NETCON, "netcon %lld: target instance out of range", (long long)i);
+    if (de->nc_src_gid[i] < 0) return fail(CN_ERR_NETCON, "netcon %lld: negative source", (long long)i);
+    if (!std::isfinite(de->nc_weight_uS[i]) || !std::isfinite(de->nc_delay_ms[i]) ||
+        !(de->nc_delay_ms[i] > 0.0))
+      return fail(CN_ERR_NETCON, "netcon %lld: weight / delay invalid", (long long)i);
+    n_src = std::max(n_src, de->nc_src_gid[i] + 1);
+  }
+  for (int64_t i = 0; i < de->n_stim; ++i) {
+    if (de->stim_gid[i] < de->n_cell)
+      return fail(CN_ERR_NETCON, "scripted source %lld: gid must be >= n_cell", (long long)i);
+    if (!std::isfinite(de->stim_t_ms[i]) || de->stim_t_ms[i] < 0.0)
+      return fail(CN_ERR_NETCON, "scripted source %lld: time invalid", (long long)i);
+    n_src = std::max(n_src, de->stim_gid[i] + 1);
+  }
+
+  cn_model *m = new (std::nothrow) cn_model();
+  if (!m) return fail(CN_ERR_NOMEM, "out of host memory");
+  try {
+    m->n_cell = de->n_cell;
+    m->N = N;
+    m->cell_first.assign(de->cell_first, de->cell_first + (de->n_cell ? de->n_cell + 1 : 0));
+    if (de->n_cell == 0) m->cell_first.assign(1, 0);
+    m->parent.assign(de->parent, de->parent + N);
+    m->area.assign(de->area_um2, de->area_um2 + N);
+    m->ri.assign(de->ri_MOhm, de->ri_MOhm + N);
+    m->cm.assign(de->cm_uF_cm2, de->cm_uF_cm2 + N);
+    m->thr.assign(de->thr_mV, de->thr_mV + de->n_cell);
+    m->v_init = de->v_init_mV;
+    m->celsius = de->celsius;
+    m->tab.resize(de->n_mech);
+    for (int32_t t = 0; t < de->n_mech; ++t) {
+      const cn_mech_table &mt = de->mech[t];
+      HTable &T = m->tab[t];
+      T.type = mt.type;
+      type_info(mt.type, T.ti);
+      T.n = mt.n;
+      T.node.assign(mt.node, mt.node + mt.n);
+      T.param.assign(mt.param, mt.param + mt.n * T.ti.n_param);
+      T.glob.assign(mt.global, mt.global + T.ti.n_global);
+    }
+    m->n_netcon = de->n_netcon;
+    m->nc_src.assign(de->nc_src_gid, de->nc_src_gid + de->n_netcon);
+    m->nc_tgt_mech.assign(de->nc_tgt_mech, de->nc_tgt_mech + de->n_netcon);
+    m->nc_tgt_inst.assign(de->nc_tgt_inst, de->nc_tgt_inst + de->n_netcon);
+    m->nc_w.assign(de->nc_weight_uS, de->nc_weight_uS + de->n_netcon);
+    m->nc_delay.assign(de->nc_delay_ms, de->nc_delay_ms + de->n_netcon);
+    m->stim_gid.assign(de->stim_gid, de->stim_gid + de->n_stim);
+    m->stim_t.assign(de->stim_t_ms, de->stim_t_ms + de->n_stim);
+    m->n_src = n_src;
+    m->sp_cap = 16 * (int64_t)de->n_cell + 65536;
+    int rc = build_layout(m);
+    if (rc != CN_OK) {
+      delete m;
+      return rc;
+    }
+  } catch (const std::bad_alloc &) {
+    delete m;
+    return fail(CN_ERR_NOMEM, "out of host memory");
+  }
+  *out = m;
+  return CN_OK;
+}
+
+static inline uint64_t mix64(uint64_t h, uint64_t x) {
+  h ^= x + 0x9E3779B97F4A7C15ull + (h << 6) + (h >> 2);
+  h *= 0xBF58476D1CE4E5B9ull;
+  return h ^ (h >> 29);
+}
+
+static int build_layout(cn_model *m) {
+  const int32_t nc = m->n_cell;
+  const int64_t N = m->N;
+  const int nt = (int)m->tab.size();
+  // node -> cell
+  std::vector<int32_t> cell_of(N);
+  for (int32_t c = 0; c < nc; ++c)
+    for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of[i] = c;
+  // per distributed table: CSR of instances per cell, sorted by local node
+  for (int t = 0; t < nt; ++t) {
+    HTable &T = m->tab[t];
+    if (T.ti.point) continue;
+    T.cell_first.assign((size_t)nc + 1, 0);
+    for (int64_t i = 0; i < T.n; ++i) T.cell_first[cell_of[T.node[i]] + 1]++;
+    for (int32_t c = 0; c < nc; ++c) T.cell_first[c + 1] += T.cell_first[c];
+    T.cell_inst.resize((size_t)T.n);
+    std::vector<int64_t> fill(T.cell_first.begin(), T.cell_first.end() - 1);
+    for (int64_t i = 0; i < T.n; ++i) T.cell_inst[fill[cell_of[T.node[i]]]++] = i;
+    for (int32_t c = 0; c < nc; ++c) {
+      auto b = T.cell_inst.begin() + T.cell_first[c], e = T.cell_inst.begin() + T.cell_first[c + 1];
+      if (!std::is_sorted(b, e, [&](int64_t x, int64_t y) { return T.node[x] < T.node[y]; }))
+        std::sort(b, e, [&](int64_t x, int64_t y) { return T.node[x] < T.node[y]; });
+      for (auto it = b; it != e && it + 1 != e; ++it)
+        if (T.node[*it] == T.node[*(it + 1)])
+          return fail(CN_ERR_MECH, "table %d: two instances on node %d", t, T.node[*it]);
+    }
+  }
+  // shape signature per cell: topology + placement of every distributed table
+  std::vector<uint64_t> sig(nc);
+  for (int32_t c = 0; c < nc; ++c) {
+    const int64_t f = m->cell_first[c], l = m->cell_first[c + 1];
+    uint64_t h = mix64(0x1234567ull, (uint64_t)(l - f));
+    for (int64_t i = f + 1; i < l; ++i) h = mix64(h, (uint64_t)(m->parent[i] - f));
+    for (int t = 0; t < nt; ++t) {
+      const HTable &T = m->tab[t];
+      if (T.ti.point) continue;
+      h = mix64(h, 0xABCD0000ull + (uint64_t)t);
+      for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j)
+        h = mix64(h, (uint64_t)(T.node[T.cell_inst[j]] - f));
+    }
+    sig[c] = h;
+  }
+  auto same_shape = [&](int32_t x, int32_t y) {
+    const int64_t fx = m->cell_first[x], fy = m->cell_first[y];
+    const int64_t n = m->cell_first[x + 1] - fx;
+    if (n != m->cell_first[y + 1] - fy) return false;
+    for (int64_t i = 1; i < n; ++i)
+      if (m->parent[fx + i] - fx != m->parent[fy + i] - fy) return false;
+    for (int t = 0; t < nt; ++t) {
+      const HTable &T = m->tab[t];
+      if (T.ti.point) continue;
+      const int64_t cx = T.cell_first[x + 1] - T.cell_first[x];
+      if (cx != T.cell_first[y + 1] - T.cell_first[y]) return false;
+      for (int64_t j = 0; j < cx; ++j)
+        if (T.node[T.cell_inst[T.cell_first[x] + j]] - fx !=
+            T.node[T.cell_inst[T.cell_first[y] + j]] - fy)
+          return false;
+    }
+    return true;
+  };
+  m->cell_cls.assign(nc, -1);
+  {
+    std::unordered_map<uint64_t, std::vector<int>> by_sig;
+    by_sig.reserve((size_t)nc / 8 + 16);
+    for (int32_t c = 0; c < nc; ++c) {
+      auto &cands = by_sig[sig[c]];
+      int found = -1;
+      for (int k : cands)
+        if (same_shape(m->cls[k].rep_cell, c)) { found = k; break; }
+      if (found < 0) {
+        found = (int)m->cls.size();
+        m->cls.emplace_back();
+        m->cls.back().rep_cell = c;
+        m->cls.back().n = (int)(m->cell_first[c + 1] - m->cell_first[c]);
+        cands.push_back(found);
+      }
+      m->cls[found].cells.push_back(c);
+      m->cell_cls[c] = found;
+    }
+  }
+  // which tables need ica / cai
+  bool has_cadyn = false, has_caform = false, has_sk = false;
+  for (const HTable &T : m->tab) {
+    if (T.type == CN_CADYN) has_cadyn = true;
+    if (T.type == CN_SK) has_sk = true;
+    if (T.type == CN_HHFORM && T.glob[3] != 0.0) has_caform = true;
+  }
+  m->any_ica = has_cadyn || has_caform;
+  m->any_cai = has_cadyn || has_sk;
+  // choose G per class and schedule
+  int force_g = 0;
+  if (const char *e = std::getenv("CN_FORCE_G")) force_g = std::atoi(e);
+  int max_g = 4;
+  if (const char *e = std::getenv("CN_MAX_G")) max_g = std::max(1, std::atoi(e));
+  int64_t smem_cap = 24 * 1024;
+  if (const char *e = std::getenv("CN_WARP_SMEM")) smem_cap = std::atoll(e);
+  const int64_t hard_cap = 200 * 1024;
+  int sched_total = 0;
+  m->warp_smem_doubles = 0;
+  for (HClass &K : m->cls) {
+    K.count = (int64_t)K.cells.size();
+    K.needs_ica = m->any_ica ? 1 : 0;
+    const int arrays = 2 + K.needs_ica;
+    if ((int64_t)K.n * arrays * 8 > hard_cap)
+      return fail(CN_ERR_UNSUPPORTED,
+                  "a cell with %d nodes does not fit the on-chip solve (limit %lld nodes)", K.n,
+                  (long long)(hard_cap / (arrays * 8)));
+    int G = 1;
+    while (G * 2 <= max_g && G * 2 <= K.count && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap)
+      G *= 2;
+    if (force_g > 0) {
+      G = 1;
+      while (G * 2 <= force_g && (int64_t)K.n * arrays * 8 * G * 2 <= hard_cap) G *= 2;
+    }
+    K.G = G;
+    K.lgG = 0;
+    while ((1 << K.lgG) < G) K.lgG++;
+    std::vector<int32_t> pl(K.n);
+    const int64_t f = m->cell_first[K.rep_cell];
+    pl[0] = -1;
+    for (int i = 1; i < K.n; ++i) pl[i] = (int32_t)(m->parent[f + i] - f);
+    K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched);
+    K.sched_off = sched_total;
+    sched_total += (int)K.sched.size();
+    m->warp_smem_doubles = std::max(m->warp_smem_doubles, K.n * G * arrays);
+  }
+  // groups
+  m->cell_grp.assign(nc, -1);
+  m->cell_slot.assign(nc, 0);
+  m->node_pos.assign((size_t)N, -1);
+  int64_t node_base = 0, ab_base = 0;
+  int32_t cell_base = 0;
+  for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
+    HClass &K = m->cls[kc];
+    for (int64_t q = 0; q < K.count; q += K.G) {
+      GroupInfo gi{};
+      gi.cls = kc;
+      gi.ncell = (int32_t)std::min<int64_t>(K.G, K.count - q);
+      gi.cell_base = cell_base;
+      gi.node_base = node_base;
+      gi.ab_base = ab_base;
+      const int gidx = (int)m->grp.size();
+      for (int c = 0; c < gi.ncell; ++c) {
+        const int32_t cell = K.cells[q + c];
+        m->cell_grp[cell] = gidx;
+        m->cell_slot[cell] = c;
+        const int64_t f = m->cell_first[cell];
+        for (int i = 0; i < K.n; ++i) m->node_pos[f + i] = node_base + (int64_t)i * K.G + c;
+      }
+      m->grp.push_back(gi);
+      node_base += (int64_t)K.n * K.G;
+      ab_base += (int64_t)K.rounds * 32;
+      cell_base += K.G;
+    }
+  }
+  m->n_pnode = node_base;
+  m->n_ab = ab_base;
+  m->n_pcell = cell_base;
+  const int ng = (int)m->grp.size();
+  // per-table instance layout
+  std::vector<int32_t> dist_nodes;
+  for (int t = 0; t < nt; ++t) {
+    HTable &T = m->tab[t];
+    T.inst_pos.assign((size_t)T.n, -1);
+    if (T.ti.point) {
+      // instances ordered by group (stable), slot = local node * G + cell slot
+      T.pp_first.assign((size_t)ng + 1, 0);
+      for (int64_t i = 0; i < T.n; ++i) T.pp_first[m->cell_grp[cell_of[T.node[i]]] + 1]++;
+      for (int g = 0; g < ng; ++g) T.pp_first[g + 1] += T.pp_first[g];
+      std::vector<int64_t> fill(T.pp_first.begin(), T.pp_first.end() - 1);
+      T.pp_slot.assign((size_t)T.n, 0);
+      for (int64_t i = 0; i < T.n; ++i) {
+        const int32_t cell = cell_of[T.node[i]];
+        const int g = m->cell_grp[cell];
+        const int64_t pos = fill[g]++;
+        T.inst_pos[i] = pos;
+        const int G = m->cls[m->grp[g].cls].G;
+        T.pp_slot[pos] = (int32_t)((T.node[i] - m->cell_first[cell]) * G + m->cell_slot[cell]);
+      }
+      T.n_dev = T.n;
+    } else {
+      T.cls_cnt.assign(m->cls.size(), 0);
+      T.cls_nodeoff.assign(m->cls.size(), 0);
+      for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
+        const HClass &K = m->cls[kc];
+        const int32_t rc = K.rep_cell;
+        T.cls_cnt[kc] = (int32_t)(T.cell_first[rc + 1] - T.cell_first[rc]);
+        T.cls_nodeoff[kc] = (int32_t)dist_nodes.size();
+        for (int64_t j = T.cell_first[rc]; j < T.cell_first[rc + 1]; ++j)
+          dist_nodes.push_back((int32_t)(T.node[T.cell_inst[j]] - m->cell_first[rc]));
+      }
+      T.grp_instbase.assign((size_t)ng, 0);
+      int64_t base = 0;
+      for (int g = 0; g < ng; ++g) {
+        const GroupInfo &gi = m->grp[g];
+        const HClass &K = m->cls[gi.cls];
+        const int cnt = T.cls_cnt[gi.cls];
+        T.grp_instbase[g] = base;
+        base += (int64_t)cnt * K.G;
+      }
+      T.n_dev = base;
+      for (int32_t c = 0; c < nc; ++c) {
+        const int g = m->cell_grp[c];
+        const int G = m->cls[m->grp[g].cls].G;
+        const int64_t b0 = T.grp_instbase[g];
+        int64_t kk = 0;
+        for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j, ++kk)
+          T.inst_pos[T.cell_inst[j]] = b0 + kk * G + m->cell_slot[c];
+      }
+    }
+  }
+  m->dist_nodes = std::move(dist_nodes);
+  m->hm.n_group = ng;
+  m->hm.n_class = (int32_t)m->cls.size();
+  m->hm.n_table = nt;
+  static_assert(sizeof(GroupInfo) == 32, "GroupInfo layout");
+  // CTA shape: as many warps per block as fit ~100 KB, at most 8
+  const int64_t wbytes = std::max<int64_t>((int64_t)m->warp_smem_doubles * 8, 8);
+  int wpb = 8;
+  if (const char *e = std::getenv("CN_WPB")) wpb = std::max(1, std::atoi(e));
+  while (wpb > 1 && wbytes * wpb > 110 * 1024) wpb /= 2;
+  m->wpb = wpb;
+  return CN_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// first cn_run: dt-dependent constants (row-normalised system), initial states, upload
+// ---------------------------------------------------------------------------------------------
+
+static int finalize(cn_model *m, double dt) {
+  const int64_t N = m->N;
+  const int nt = (int)m->tab.size();
+  const int ng = (int)m->grp.size();
+  int dev_count = 0;
+  if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
+    return fail(CN_ERR_CUDA, "no CUDA device: libcn has no CPU fallback");
+  // delays
+  std::vector<int32_t> dsteps((size_t)m->n_netcon);
+  int64_t mind = INT32_MAX, maxd = 1;
+  for (int64_t i = 0; i < m->n_netcon; ++i) {
+    const long long ds = llround(m->nc_delay[i] / dt);
+    if (ds < 1) return fail(CN_ERR_NETCON, "netcon %lld: delay %.6g ms is < 1 step of %.6g ms",
+                            (long long)i, m->nc_delay[i], dt);
+    if (ds > 1000000) return fail(CN_ERR_NETCON, "netcon %lld: delay too long", (long long)i);
+    dsteps[i] = (int32_t)ds;
+    mind = std::min<int64_t>(mind, ds);
+    maxd = std::max<int64_t>(maxd, ds);
+  }
+  if (m->n_netcon == 0) mind = 1;
+  // row-normalised static arrays:  c_i = 1e-3 cm_i/dt,  b' = b/c_i,  a' = a/c_parent,
+  // dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
+  std::vector<double> invc((size_t)N), bn((size_t)N, 0.0), an((size_t)N, 0.0);
+  std::vector<double> dstat((size_t)m->n_pnode, 1.0), rstat((size_t)m->n_pnode, 0.0);
+  std::vector<double> v0((size_t)m->n_pnode, 0.0);
+  std::vector<double> dsum((size_t)N), rsum((size_t)N, 0.0);
+  for (int64_t i = 0; i < N; ++i) {
+    const double c = 1e-3 * m->cm[i] / dt;
+    invc[i] = 1.0 / c;
+    dsum[i] = c;
+  }
+  for (int64_t i = 0; i < N; ++i) {
+    const int32_t p = m->parent[i];
+    if (p >= 0) {
+      const double b = -100.0 / (m->ri[i] * m->area[i]);
+      const double a = -100.0 / (m->ri[i] * m->area[p]);
+      dsum[i] -= b;
+      dsum[p] -= a;
+      bn[i] = b * invc[i];
+      an[i] = a * invc[p];
+    }
+  }
+  for (const HTable &T : m->tab)
+    if (T.type == CN_PAS)
+      for (int64_t i = 0; i < T.n; ++i) {
+        const double g = T.param[i], e = T.param[T.n + i];
+        dsum[T.node[i]] += g;
+        rsum[T.node[i]] += g * e;
+      }
+  for (int64_t i = 0; i < N; ++i) {
+    const int64_t q = m->node_pos[i];
+    dstat[q] = dsum[i] * invc[i];
+    rstat[q] = rsum[i] * invc[i];
+    v0[q] = m->v_init;
+  }
+  // schedule-ordered off-diagonals
+  std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
+  std::vector<uint32_t> sched_all;
+  std::vector<ClassInfo> cinfo(m->cls.size());
+  for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+    const HClass &K = m->cls[kc];
+    cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, 0, 0};
+    sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
+  }
+  // inverse map: (group, slot) -> caller cell
+  std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
+  for (int32_t c = 0; c < m->n_cell; ++c)
+    cell_of_pcell[m->grp[m->cell_grp[c]].cell_base + m->cell_slot[c]] = c;
+  for (int g = 0; g < ng; ++g) {
+    const GroupInfo &gi = m->grp[g];
+    const HClass &K = m->cls[gi.cls];
+    const int P = 32 / K.G;
+    for (int c = 0; c < gi.ncell; ++c) {
+      const int32_t cell = cell_of_pcell[gi.cell_base + c];
+      const int64_t f = m->cell_first[cell];
+      for (int r = 0; r < K.rounds; ++r)
+        for (int p = 0; p < P; ++p) {
+          const uint32_t e = K.sched[(size_t)r * P + p];
+          if ((e & 0xFFFFu) == CN_IDLE) continue;
+          const int64_t i = f + (e & 0xFFFFu);
+          const int64_t pos = gi.ab_base + (int64_t)r * 32 + p * K.G + c;
+          a_s[pos] = an[i];
+          b_s[pos] = bn[i];
+        }
+    }
+  }
+  // thresholds, flags, gids per permuted cell
+  std::vector<double> thr((size_t)m->n_pcell, 0.0);
+  std::vector<unsigned char> flag((size_t)m->n_pcell, 0);
+  std::vector<int32_t> gid_of((size_t)m->n_pcell, -1);
+  for (int32_t pc = 0; pc < m->n_pcell; ++pc) {
+    const int32_t c = cell_of_pcell[pc];
+    if (c < 0) continue;
+    thr[pc] = m->thr[c];
+    flag[pc] = m->v_init > m->thr[c];
+    gid_of[pc] = c;
+  }
+  // cai per node
+  std::vector<double> cai;
+  if (m->any_cai) {
+    cai.assign((size_t)m->n_pnode, 1e-4);
+    for (const HTable &T : m->tab)
+      if (T.type == CN_CADYN)
+        for (int64_t i = 0; i < T.n; ++i) cai[m->node_pos[T.node[i]]] = T.glob[3];
+  }
+
+  DModel &H = m->hm;
+  H.warp_smem_doubles = m->warp_smem_doubles;
+  H.dt = dt;
+  H.celsius = m->celsius;
+  H.q10 = std::pow(3.0, (m->celsius - 6.3) / 10.0);
+  int rc;
+#define UP(vec, ptr)                                            \
+  do {                                                          \
+    rc = dev_upload(m, vec, &ptr);                              \
+    if (rc != CN_OK) return rc;                                 \
+  } while (0)
+  {
+    GroupInfo *dg; ClassInfo *dc; uint32_t *ds; int32_t *dn;
+    UP(m->grp, dg); UP(cinfo, dc); UP(sched_all, ds); UP(m->dist_nodes, dn);
+    H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
+    double *p;
+    UP(v0, m->d_v); H.v = m->d_v;
+    UP(dstat, p); H.dstat = p;
+    UP(rstat, p); H.rstat = p;
+    UP(a_s, p); H.a_s = p;
+    UP(b_s, p); H.b_s = p;
+    if (m->any_cai) { UP(cai, m->d_cai); H.cai = m->d_cai; } else H.cai = nullptr;
+    UP(thr, p); H.thr = p;
+    unsigned char *pf; UP(flag, pf); H.flag = pf;
+    int32_t *pg; UP(gid_of, pg); H.gid_of_pcell = pg;
+  }
+  // mechanism tables
+  for (int t = 0; t < nt; ++t) {
+    HTable &T = m->tab[t];
+    DTable &D = H.tab[t];
+    memset(&D, 0, sizeof(D));
+    D.type = T.type;
+    D.is_point = T.ti.point;
+    D.n_param = T.ti.n_dev_param;
+    D.n_state = T.ti.n_state;
+    for (size_t j = 0; j < T.glob.size(); ++j) D.glob[j] = T.glob[j];
+    if (T.type == CN_AMPANMDA) {
+      D.glob[7] = h_exp2_factor(T.glob[0], T.glob[1]);
+      D.glob[8] = h_exp2_factor(T.glob[2], T.glob[3]);
+    }
+    if (T.type == CN_PAS) continue;  // folded
+    const int64_t nd = T.n_dev;
+    std::vector<std::vector<double>> par(T.ti.n_dev_param, std::vector<double>((size_t)nd, 0.0));
+    std::vector<std::vector<double>> st(T.ti.n_state, std::vector<double>((size_t)nd, 0.0));
+    // benign padding for distributed tables
+    if (!T.ti.point && T.ti.n_dev_param > 0)
+      std::fill(par[T.ti.n_dev_param - 1].begin(), par[T.ti.n_dev_param - 1].end(), 1.0);
+    for (int64_t i = 0; i < T.n; ++i) {
+      const int64_t q = T.inst_pos[i];
+      const int32_t nd_i = T.node[i];
+      for (int j = 0; j < T.ti.n_param; ++j) par[j][q] = T.param[(size_t)j * T.n + i];
+      const double scale = 100.0 / m->area[nd_i] * invc[nd_i];
+      const double v = m->v_init;
+      switch (T.type) {
+        case CN_HH: {
+          par[4][q] = invc[nd_i];
+          double al, be;
+          al = 0.1 * h_vtrap(-(v + 40.0), 10.0); be = 4.0 * std::exp(-(v + 65.0) / 18.0);
+          st[0][q] = al / (al + be);
+          al = 0.07 * std::exp(-(v + 65.0) / 20.0); be = 1.0 / (std::exp(-(v + 35.0) / 10.0) + 1.0);
+          st[1][q] = al / (al + be);
+          al = 0.01 * h_vtrap(-(v + 55.0), 10.0); be = 0.125 * std::exp(-(v + 65.0) / 80.0);
+          st[2][q] = al / (al + be);
+          break;
+        }
+        case CN_EXPSYN: par[2][q] = scale; break;
+        case CN_EXP2SYN:
+          par[3][q] = scale;
+          par[4][q] = h_exp2_factor(par[0][q], par[1][q]);
+          break;
+        case CN_ICLAMP: par[3][q] = scale; break;
+        case CN_HHFORM:
+          par[1][q] = invc[nd_i];
+          st[0][q] = 1.0 / (1.0 + std::exp((T.glob[4] - v) / T.glob[5]));
+          st[1][q] = 1.0 / (1.0 + std::exp((T.glob[10] - v) / T.glob[11]));
+          break;
+        case CN_SK: {
+          par[1][q] = invc[nd_i];
+          double ca = m->any_cai ? cai[m->node_pos[nd_i]] : 1e-4;
+          if (ca < 1e-9) ca = 1e-9;
+          st[0][q] = 1.0 / (1.0 + std::pow(T.glob[1] / ca, T.glob[2]));
+          break;
+        }
+        case CN_AMPANMDA: par[0][q] = scale; break;
+        default: break;
+      }
+    }
+    for (int j = 0; j < T.ti.n_dev_param; ++j) { UP(par[j], T.d_param[j]); D.param[j] = T.d_param[j]; }
+    for (int j = 0; j < T.ti.n_state; ++j) { UP(st[j], T.d_state[j]); D.state[j] = T.d_state[j]; }
+    if (T.ti.point) {
+      UP(T.pp_first, T.d_pp_first); UP(T.pp_slot, T.d_pp_slot);
+      D.pp_first = T.d_pp_first; D.pp_slot = T.d_pp_slot;
+    } else {
+      UP(T.cls_cnt, T.d_cls_cnt); UP(T.cls_nodeoff, T.d_cls_nodeoff);
+      UP(T.grp_instbase, T.d_grp_instbase);
+      D.cls_cnt = T.d_cls_cnt; D.cls_nodeoff = T.d_cls_nodeoff; D.grp_instbase = T.d_grp_instbase;
+    }
+  }
+  // PAS tables still need (empty) layout pointers so the kernel's table loop can skip them
+  for (int t = 0; t < nt; ++t) {
+    HTable &T = m->tab[t];
+    if (T.type != CN_PAS) continue;
+    std::vector<int32_t> zc(m->cls.size(), 0);
+    std::vector<int64_t> zg((size_t)ng, 0);
+    UP(zc, T.d_cls_cnt); UP(zc, T.d_cls_nodeoff); UP(zg, T.d_grp_instbase);
+    H.tab[t].cls_cnt = T.d_cls_cnt; H.tab[t].cls_nodeoff = T.d_cls_nodeoff;
+    H.tab[t].grp_instbase = T.d_grp_instbase;
+  }
+  // NetCons: CSR by source gid, sorted by delay steps (stable in caller order)
+  {
+    std::vector<int64_t> order((size_t)m->n_netcon);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) {
+      if (m->nc_src[x] != m->nc_src[y]) return m->nc_src[x] < m->nc_src[y];
+      return dsteps[x] < dsteps[y];
+    });
+    std::vector<int64_t> src_first((size_t)m->n_src + 1, 0);
+    for (int64_t i = 0; i < m->n_netcon; ++i) src_first[m->nc_src[i] + 1]++;
+    for (int32_t s = 0; s < m->n_src; ++s) src_first[s + 1] += src_first[s];
+    std::vector<int32_t> nd((size_t)m->n_netcon), ntab((size_t)m->n_netcon);
+    std::vector<int64_t> ninst((size_t)m->n_netcon);
+    std::vector<double> nw((size_t)m->n_netcon);
+    for (int64_t j = 0; j < m->n_netcon; ++j) {
+      const int64_t i = order[j];
+      nd[j] = dsteps[i];
+      ntab[j] = m->nc_tgt_mech[i];
+      ninst[j] = m->tab[m->nc_tgt_mech[i]].inst_pos[m->nc_tgt_inst[i]];
+      nw[j] = m->nc_w[i];
+    }
+    int64_t *p64; int32_t *p32; double *pd;
+    UP(src_first, p64); H.src_first = p64;
+    UP(nd, p32); H.nc_d = p32;
+    UP(ntab, p32); H.nc_tab = p32;
+    UP(ninst, p64); H.nc_inst = p64;
+    UP(nw, pd); H.nc_w = pd;
+    H.mind = (int32_t)mind;
+    H.maxd = (int32_t)maxd;
+    H.wr = (int32_t)(maxd + 2);
+    rc = dev_alloc(m, (size_t)H.wr, &H.sp_end);
+    if (rc != CN_OK) return rc;
+    // scripted sources sorted by step
+    const int64_t ns = (int64_t)m->stim_gid.size();
+    std::vector<int64_t> sstep((size_t)ns), so((size_t)ns);
+    for (int64_t i = 0; i < ns; ++i) sstep[i] = llround(m->stim_t[i] / dt);
+    std::iota(so.begin(), so.end(), 0);
+    std::stable_sort(so.begin(), so.end(), [&](int64_t x, int64_t y) { return sstep[x] < sstep[y]; });
+    std::vector<int32_t> sg((size_t)ns);
+    std::vector<int64_t> ss((size_t)ns);
+    for (int64_t j = 0; j < ns; ++j) { sg[j] = m->stim_gid[so[j]]; ss[j] = sstep[so[j]]; }
+    UP(sg, p32); H.stim_gid = p32;
+    UP(ss, p64); H.stim_step = p64;
+    H.n_stim = ns;
+  }
+  // spikes
+  rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_gid, false); if (rc) return rc;
+  rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_step, false); if (rc) return rc;
+  rc = dev_alloc(m, 1, &m->d_nsp); if (rc) return rc;
+  rc = dev_alloc(m, 1, &m->d_overflow); if (rc) return rc;
+  H.sp_gid = m->d_sp_gid; H.sp_step = m->d_sp_step; H.n_sp = m->d_nsp; H.sp_cap = m->sp_cap;
+  H.overflow = m->d_overflow;
+  // caller-order lookup for cn_get_v, probes
+  UP(m->node_pos, m->d_node_pos);
+  rc = dev_alloc(m, (size_t)std::max<int64_t>(N, 1), &m->d_gather, false); if (rc) return rc;
+  if (!m->probe.empty()) {
+    std::vector<int64_t> pp(m->probe.size());
+    for (size_t j = 0; j < pp.size(); ++j) pp[j] = m->node_pos[m->probe[j]];
+    UP(pp, m->d_probe_pos);
+    rc = dev_alloc(m, (size_t)(m->probe_cap * (int64_t)m->probe.size()), &m->d_trace, false);
+    if (rc) return rc;
+  }
+  {
+    std::vector<DModel> one(1, H);
+    UP(one, m->d_m);
+  }
+#undef UP
+  CU(cudaEventCreate(&m->ev0));
+  CU(cudaEventCreate(&m->ev1));
+  m->dt = dt;
+  m->uploaded = true;
+  return CN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// run
+// ---------------------------------------------------------------------------------------------
+
+template <int WPB>
+static cudaError_t launch_step(cn_model *m, int64_t k) {
+  const int ng = m->hm.n_group;
+  const size_t smem = (size_t)WPB * m->warp_smem_doubles * sizeof(double);
+  static bool attr_set[16] = {};
+  if (!attr_set[WPB]) {
+    cudaError_t e = cudaFuncSetAttribute(step_kernel<WPB>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_set[WPB] = true;
+  }
+  step_kernel<WPB><<<(ng + WPB - 1) / WPB, WPB * 32, smem, m->stream>>>(m->d_m, k);
+  return cudaGetLastError();
+}
+
+static int run_steps(cn_model *m, int64_t K) {
+  const int ng = m->hm.n_group;
+  int deliver_blocks = 8;
+  if (m->n_netcon > 1000000) deliver_blocks = 148;
+  CU(cudaEventRecord(m->ev0, m->stream));
+  for (int64_t s = 0; s < K; ++s) {
+    const int64_t k = m->k + s;
+    if (m->n_netcon > 0) {
+      deliver_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->d_m, k);
+      m->launches++;
+    }
+    if (ng > 0) {
+      cudaError_t e;
+      switch (m->wpb) {
+        case 8: e = launch_step<8>(m, k); break;
+        case 4: e = launch_step<4>(m, k); break;
+        case 2: e = launch_step<2>(m, k); break;
+        default: e = launch_step<1>(m, k); break;
+      }
+      if (e != cudaSuccess) return fail(CN_ERR_CUDA, "step launch failed: %s", cudaGetErrorString(e));
+      m->launches++;
+    }
+    if (!m->probe.empty() && m->probe_rows < m->probe_cap) {
+      const int np = (int)m->probe.size();
+      probe_kernel<<<(np + 127) / 128, 128, 0, m->stream>>>(m->d_v, m->d_probe_pos, np,
+                                                              m->d_trace, m->probe_rows);
+      m->probe_rows++;
+      m->launches++;
+    }
+  }
+  CU(cudaEventRecord(m->ev1, m->stream));
+  CU(cudaGetLastError());
+  m->k += K;
+  m->timed = true;
+  return CN_OK;
+}
+
+extern "C" int cn_run_async(cn_model *m, double tstop, double dt) {
+  if (!m) return fail(CN_ERR_ARG, "NULL model");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(CN_ERR_DT, "dt must be > 0");
+  if (!std::isfinite(tstop)) return fail(CN_ERR_ARG, "tstop must be finite");
+  if (!m->uploaded) {
+    int rc = finalize(m, dt);
+    if (rc != CN_OK) return rc;
+  } else if (dt != m->dt) {
+    return fail(CN_ERR_DT, "dt = %.17g differs from the first run's dt = %.17g", dt, m->dt);
+  }
+  const int64_t target = llround(tstop / dt);
+  if (target <= m->k) return CN_OK;
+  return run_steps(m, target - m->k);
+}
+
+extern "C" int cn_sync(cn_model *m) {
+  if (!m) return fail(CN_ERR_ARG, "NULL model");
+  if (!m->uploaded) return CN_OK;
+  CU(cudaStreamSynchronize(m->stream));
+  int32_t ov = 0;
+  CU(cudaMemcpy(&ov, m->d_overflow, sizeof(ov), cudaMemcpyDeviceToHost));
+  if (ov) return fail(CN_ERR_OVERFLOW, "spike buffer overflow (capacity %lld)", (long long)m->sp_cap);
+  return CN_OK;
+}
+
+extern "C" int cn_run(cn_model *m, double tstop, double dt) {
+  int rc = cn_run_async(m, tstop, dt);
+  if (rc != CN_OK) return rc;
+  return cn_sync(m);
+}
+
+extern "C" int cn_set_stream(cn_model *m, void *s) {
+  if (!m) return fail(CN_ERR_ARG, "NULL model");
+  m->stream = (cudaStream_t)s;
+  return CN_OK;
+}
+
+extern "C" int cn_get_v(const cn_model *cm, double *out, int64_t n) {
+  cn_model *m = const_cast<cn_model *>(cm);
+  if (!m || (!out && n > 0)) return fail(CN_ERR_ARG, "NULL argument");
+  if (n != m->N) return fail(CN_ERR_ARG, "n = %lld but the model has %lld nodes", (long long)n,
+                             (long long)m->N);
+  if (!m->uploaded) {  // before the first run: initial condition
+    for (int64_t i = 0; i < n; ++i) out[i] = m->v_init;
+    return CN_OK;
+  }
+  if (n == 0) return CN_OK;
+  gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(m->d_v, m->d_node_pos, n,
+                                                                     m->d_gather);
+  m->launches++;
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(out, m->d_gather, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost,
+                     m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  return CN_OK;
+}
+
+extern "C" int cn_get_spikes(const cn_model *cm, int32_t *gid, int64_t *step, int64_t cap,
+                             int64_t *n_out) {
+  cn_model *m = const_cast<cn_model *>(cm);
+  if (!m || !n_out) return fail(CN_ERR_ARG, "NULL argument");
+  *n_out = 0;
+  if (!m->uploaded) return CN_OK;
+  CU(cudaStreamSynchronize(m->stream));
+  unsigned long long ns = 0;
+  CU(cudaMemcpy(&ns, m->d_nsp, sizeof(ns), cudaMemcpyDeviceToHost));
+  int64_t n = std::min<int64_t>((int64_t)ns, m->sp_cap);
+  *n_out = n;
+  if (cap == 0 || n == 0) return CN_OK;
+  if (!gid || !step) return fail(CN_ERR_ARG, "NULL output array");
+  std::vector<int32_t> g((size_t)n);
+  std::vector<int64_t> s((size_t)n);
+  CU(cudaMemcpy(g.data(), m->d_sp_gid, (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  CU(cudaMemcpy(s.data(), m->d_sp_step, (size_t)n * sizeof(int64_t), cudaMemcpyDeviceToHost));
+  std::vector<int64_t> ord((size_t)n);
+  std::iota(ord.begin(), ord.end(), 0);
+  std::sort(ord.begin(), ord.end(), [&](int64_t x, int64_t y) {
+    if (s[x] != s[y]) return s[x] < s[y];
+    return g[x] < g[y];
+  });
+  const int64_t w = std::min(n, cap);
+  for (int64_t i = 0; i < w; ++i) { gid[i] = g[ord[i]]; step[i] = s[ord[i]]; }
+  return CN_OK;
+}
+
+extern "C" int cn_set_probes(cn_model *m, const int32_t *node, int64_t n, int64_t max_steps) {
+  if (!m || (n > 0 && !node)) return fail(CN_ERR_ARG, "NULL argument");
+  if (m->uploaded) return fail(CN_ERR_ARG, "probes must be set before the first cn_run");
+  if (n < 0 || max_steps < 0) return fail(CN_ERR_ARG, "negative count");
+  for (int64_t i = 0; i < n; ++i)
+    if (node[i] < 0 || node[i] >= m->N) return fail(CN_ERR_ARG, "probe node out of range");
+  m->probe.assign(node, node + n);
+  m->probe_cap = max_steps;
+  return CN_OK;
+}
+
+extern "C" int cn_get_trace(const cn_model *cm, double *out, int64_t cap_steps, int64_t *n_steps) {
+  cn_model *m = const_cast<cn_model *>(cm);
+  if (!m || !n_steps) return fail(CN_ERR_ARG, "NULL argument");
+  *n_steps = m->probe_rows;
+  const int64_t rows = std::min(m->probe_rows, cap_steps);
+  if (rows <= 0 || m->probe.empty()) return CN_OK;
+  if (!out) return fail(CN_ERR_ARG, "NULL output");
+  CU(cudaStreamSynchronize(m->stream));
+  CU(cudaMemcpy(out, m->d_trace, (size_t)rows * m->probe.size() * sizeof(double),
+                cudaMemcpyDeviceToHost));
+  return CN_OK;
+}
+
+extern "C" int cn_get_state(const cn_model *cm, int32_t t, int32_t s, double *out, int64_t n) {
+  cn_model *m = const_cast<cn_model *>(cm);
+  if (!m || !out) return fail(CN_ERR_ARG, "NULL argument");
+  if (t < 0 || t >= (int)m->tab.size()) return fail(CN_ERR_MECH, "table out of range");
+  HTable &T = m->tab[t];
+  if (s < 0 || s >= T.ti.n_state || n != T.n) return fail(CN_ERR_MECH, "state / size mismatch");
+  if (!m->uploaded) return fail(CN_ERR_ARG, "states exist after the first cn_run");
+  CU(cudaStreamSynchronize(m->stream));
+  std::vector<double> h((size_t)std::max<int64_t>(T.n_dev, 1));
+  CU(cudaMemcpy(h.data(), T.d_state[s], (size_t)T.n_dev * sizeof(double), cudaMemcpyDeviceToHost));
+  for (int64_t i = 0; i < n; ++i) out[i] = h[T.inst_pos[i]];
+  return CN_OK;
+}
+
+extern "C" int64_t cn_steps_done(const cn_model *m) { return m ? m->k : 0; }
+extern "C" int64_t cn_launch_count(const cn_model *m) { return m ? m->launches : 0; }
+
+extern "C" int cn_last_run_ms(const cn_model *m, double *ms) {
+  if (!m || !ms) return fail(CN_ERR_ARG, "NULL argument");
+  if (!m->timed) return fail(CN_ERR_ARG, "no run yet");
+  float f = 0.f;
+  CU(cudaEventSynchronize(m->ev1));
+  CU(cudaEventElapsedTime(&f, m->ev0, m->ev1));
+  *ms = f;
+  return CN_OK;
+}
+
+extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
+  if (!m || !info) return fail(CN_ERR_ARG, "NULL argument");
+  info[0] = (int64_t)m->cls.size();
+  info[1] = (int64_t)m->grp.size();
+  info[2] = (int64_t)m->warp_smem_doubles * 8;
+  int r = 0;
+  for (const HClass &K : m->cls) r = std::max(r, K.rounds);
+  info[3] = r;
+  return CN_OK;
+}
+
+extern "C" int cn_set_spike_capacity(cn_model *m, int64_t cap) {
+  if (!m || cap < 1) return fail(CN_ERR_ARG, "bad capacity");
+  if (m->uploaded) return fail(CN_ERR_ARG, "capacity must be set before the first cn_run");
+  m->sp_cap = cap;
+  return CN_OK;
+}
+
+extern "C" void cn_model_destroy(cn_model *m) {
+  if (!m) return;
+  if (m->uploaded) cudaStreamSynchronize(m->stream);
+  for (void *p : m->dev_allocs) cudaFree(p);
+  if (m->ev0) cudaEventDestroy(m->ev0);
+  if (m->ev1) cudaEventDestroy(m->ev1);
+  delete m;
+}

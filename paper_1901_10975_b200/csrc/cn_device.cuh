@@ -1,0 +1,591 @@
+// cn_device.cuh -- device-side data model and kernels of libcn (sm_100a, fp64).
+//
+// One warp integrates one GROUP = G cells of one shape class (same topology and same placement
+// of distributed mechanisms) for one dt, with P = 32/G lanes per cell:
+//   load   : D = dstat, R = v + rstat            (node-parallel, coalesced, interleaved [node][cell])
+//   cur    : per mechanism table, D += g, R += g*E   (nrn_cur; conductance form L160)
+//   solve  : Hines elimination in shared memory, list-scheduled in rounds of P independent nodes
+//            (L62, L66, L196); off-diagonals are stored in schedule order so they stream coalesced
+//   store  : v = R                               (L66)
+//   state  : per mechanism table, cnexp / implicit updates with the new v (L67, L278)
+//   detect : warp-ballot threshold detection on the root nodes, spike append (L68)
+// The linear system is the paper's backward-Euler system written for v_new instead of delta-v and
+// with every row divided by c_i = 1e-3 cm_i/dt.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define CN_MAX_TABLES 32
+#define CN_MAX_PARAM 8
+#define CN_MAX_STATE 4
+#define CN_MAX_GLOBAL 16
+#define CN_IDLE 0xFFFFu
+
+namespace cn {
+
+enum { T_PAS = 1, T_HH = 2, T_EXPSYN = 3, T_EXP2SYN = 4, T_ICLAMP = 5, T_HHFORM = 6, T_SK = 7,
+       T_CADYN = 8, T_AMPANMDA = 9 };
+
+struct DTable {
+  int type, is_point, n_param, n_state;
+  double *param[CN_MAX_PARAM];   // permuted SoA, incl. derived per-instance constants (see host)
+  double *state[CN_MAX_STATE];
+  double glob[CN_MAX_GLOBAL];
+  const int64_t *pp_first;       // point tables: [n_group+1] instance range of each group
+  const int32_t *pp_slot;        // point tables: [n] shared-memory slot (node*G + cell) in its group
+  const int32_t *cls_cnt;        // distributed: [n_class] instances per cell
+  const int32_t *cls_nodeoff;    // distributed: [n_class] offset into dist_nodes
+  const int64_t *grp_instbase;   // distributed: [n_group] first instance of the group
+};
+
+struct GroupInfo {
+  int32_t cls, ncell;
+  int32_t cell_base;   // first permuted cell index of the group
+  int32_t pad;
+  int64_t node_base;   // first permuted node of the group (n*G nodes follow, interleaved)
+  int64_t ab_base;     // first entry of the group's schedule-ordered a/b arrays (rounds*32)
+};
+
+struct ClassInfo {
+  int32_t n, G, lgG, rounds;
+  int32_t sched_off, needs_ica, pad0, pad1;
+};
+
+struct DModel {
+  int32_t n_group, n_class, n_table, warp_smem_doubles;
+  const GroupInfo *grp;
+  const ClassInfo *cls;
+  const uint32_t *sched;        // per class: rounds * P entries, node | parent << 16
+  const int32_t *dist_nodes;    // local node lists of distributed tables per class
+  double *v;                    // [n_pnode] permuted, padded
+  const double *dstat, *rstat;  // static diagonal / rhs parts (row-normalised)
+  const double *a_s, *b_s;      // off-diagonals in schedule order
+  double *cai;                  // per node (only when a table needs it) else null
+  const double *thr;            // [n_pcell]
+  unsigned char *flag;          // [n_pcell]
+  const int32_t *gid_of_pcell;  // [n_pcell]
+  // spikes
+  int32_t *sp_gid;
+  int64_t *sp_step;
+  unsigned long long *n_sp;
+  int64_t sp_cap;
+  int32_t *overflow;
+  // delivery
+  int64_t *sp_end;              // ring [wr]: number of spikes with step <= s
+  int32_t wr, mind, maxd, pad2;
+  const int64_t *src_first;     // [n_src+1] netcons by source gid, sorted by delay steps
+  const int32_t *nc_d;          // delay in steps
+  const int32_t *nc_tab;
+  const int64_t *nc_inst;       // permuted instance
+  const double *nc_w;
+  int64_t n_stim;
+  const int32_t *stim_gid;      // sorted by step
+  const int64_t *stim_step;
+  double q10, dt, celsius;
+  DTable tab[CN_MAX_TABLES];
+};
+
+// ------------------------------------------------------------------------------------------
+// mechanism arithmetic
+// ------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ double vtrap(double x, double y) {
+  double u = x / y;
+  if (fabs(u) < 1e-6) return y * (1.0 - u / 2.0);
+  return x / (exp(u) - 1.0);
+}
+
+__device__ __forceinline__ double cnexp(double y, double yinf, double tau, double dt) {
+  return y + (1.0 - exp(-dt / tau)) * (yinf - y);
+}
+
+__device__ __forceinline__ void hh_rates(double v, double q10, double &minf, double &mtau,
+                                         double &hinf, double &htau, double &ninf,
+                                         double &ntau) {
+  double al, be, s;
+  al = 0.1 * vtrap(-(v + 40.0), 10.0);
+  be = 4.0 * exp(-(v + 65.0) / 18.0);
+  s = al + be;
+  minf = al / s;
+  mtau = 1.0 / (q10 * s);
+  al = 0.07 * exp(-(v + 65.0) / 20.0);
+  be = 1.0 / (exp(-(v + 35.0) / 10.0) + 1.0);
+  s = al + be;
+  hinf = al / s;
+  htau = 1.0 / (q10 * s);
+  al = 0.01 * vtrap(-(v + 55.0), 10.0);
+  be = 0.125 * exp(-(v + 65.0) / 80.0);
+  s = al + be;
+  ninf = al / s;
+  ntau = 1.0 / (q10 * s);
+}
+
+__device__ __forceinline__ void hhform_gate(double v, const double *g6, double &xinf,
+                                            double &xtau) {
+  double u = (v - g6[4]) / g6[5];
+  xinf = 1.0 / (1.0 + exp((g6[0] - v) / g6[1]));
+  xtau = g6[2] + g6[3] / (exp(u) + exp(-u));
+}
+
+__device__ __forceinline__ double ipow(double x, int p) {
+  double r = 1.0;
+  for (int j = 0; j < p; ++j) r *= x;
+  return r;
+}
+
+__device__ __forceinline__ double mgblock(double v, double mg) {
+  return 1.0 / (1.0 + exp(-0.062 * v) * (mg / 3.57));
+}
+
+// ------------------------------------------------------------------------------------------
+// nrn_cur: conductance G (row-normalised) and G*E into the shared-memory system
+// ------------------------------------------------------------------------------------------
+
+// Distributed table, lockstep over the group's cells: instance j = k*G + c sits on node
+// nodes[k] of cell c.  At most one instance per node and table, so plain read-modify-write.
+__device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int cnt, int G,
+                                                int lgG, const int32_t *nodes, double *D,
+                                                double *R, double *I, const double *vold,
+                                                int lane) {
+  const int tot = cnt << lgG;
+  switch (T.type) {
+    case T_HH: {
+      const double ena = T.glob[0], ek = T.glob[1];
+      for (int j = lane; j < tot; j += 32) {
+        const int64_t q = ib + j;
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const double m = T.state[0][q], h = T.state[1][q], n = T.state[2][q];
+        const double invc = T.param[4][q];
+        const double gna = T.param[0][q] * m * m * m * h;
+        const double n2 = n * n;
+        const double gk = T.param[1][q] * n2 * n2;
+        const double gl = T.param[2][q];
+        D[slot] += (gna + gk + gl) * invc;
+        R[slot] += (gna * ena + gk * ek + gl * T.param[3][q]) * invc;
+      }
+      break;
+    }
+    case T_HHFORM: {
+      const int p = (int)T.glob[0], qq = (int)T.glob[1];
+      const double E = T.glob[2];
+      const bool to_ica = T.glob[3] != 0.0;
+      for (int j = lane; j < tot; j += 32) {
+        const int64_t q = ib + j;
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const double g = T.param[0][q] * ipow(T.state[0][q], p) * ipow(T.state[1][q], qq);
+        const double invc = T.param[1][q];
+        D[slot] += g * invc;
+        R[slot] += g * E * invc;
+        if (to_ica) I[slot] += g * (vold[slot] - E);  // ica uses v_old, still in global memory
+      }
+      break;
+    }
+    case T_SK: {
+      const double E = T.glob[0];
+      for (int j = lane; j < tot; j += 32) {
+        const int64_t q = ib + j;
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const double g = T.param[0][q] * T.state[0][q];
+        const double invc = T.param[1][q];
+        D[slot] += g * invc;
+        R[slot] += g * E * invc;
+      }
+      break;
+    }
+    default: break;  // PAS is folded into dstat/rstat; CADYN carries no current
+  }
+}
+
+// Point-process table: instances of this group, arbitrary nodes -> shared-memory atomics.
+__device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i1, double *D,
+                                          double *R, const double *vold, int lane,
+                                          double t_mid) {
+  switch (T.type) {
+    case T_EXPSYN:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const double g = T.state[0][q] * T.param[2][q];  // param[2] = 100/area/c
+        if (g != 0.0) {
+          const int slot = T.pp_slot[q];
+          atomicAdd(&D[slot], g);
+          atomicAdd(&R[slot], g * T.param[1][q]);
+        }
+      }
+      break;
+    case T_EXP2SYN:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const double g = (T.state[1][q] - T.state[0][q]) * T.param[3][q];
+        if (g != 0.0) {
+          const int slot = T.pp_slot[q];
+          atomicAdd(&D[slot], g);
+          atomicAdd(&R[slot], g * T.param[2][q]);
+        }
+      }
+      break;
+    case T_ICLAMP:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const double del = T.param[0][q];
+        if (t_mid >= del && t_mid < del + T.param[1][q])
+          atomicAdd(&R[T.pp_slot[q]], T.param[2][q] * T.param[3][q]);
+      }
+      break;
+    case T_AMPANMDA:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const int slot = T.pp_slot[q];
+        const double gA = T.state[1][q] - T.state[0][q];
+        const double gN = T.state[3][q] - T.state[2][q];
+        if (gA != 0.0 || gN != 0.0) {
+          const double g = (gA + T.glob[4] * gN * mgblock(vold[slot], T.glob[5])) * T.param[0][q];
+          atomicAdd(&D[slot], g);
+          atomicAdd(&R[slot], g * T.glob[6]);
+        }
+      }
+      break;
+    default: break;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// nrn_state with the new v (in R)
+// ------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, int cnt, int G,
+                                                  int lgG, const int32_t *nodes,
+                                                  const double *R, double *cai_g,
+                                                  int64_t node_base, const double *I,
+                                                  const double *vold, int lane, double dt,
+                                                  double q10) {
+  const int tot = cnt << lgG;
+  switch (T.type) {
+    case T_HH:
+      for (int j = lane; j < tot; j += 32) {
+        const int64_t q = ib + j;
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        double minf, mtau, hinf, htau, ninf, ntau;
+        hh_rates(R[slot], q10, minf, mtau, hinf, htau, ninf, ntau);
+        T.state[0][q] = cnexp(T.state[0][q], minf, mtau, dt);
+        T.state[1][q] = cnexp(T.state[1][q], hinf, htau, dt);
+        T.state[2][q] = cnexp(T.state[2][q], ninf, ntau, dt);
+      }
+      break;
+    case T_HHFORM: {
+      const int p = (int)T.glob[0], qq = (int)T.glob[1];
+      for (int j = lane; j < tot; j += 32) {
+        const int64_t q = ib + j;
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const double v = R[slot];
+        double xinf, xtau;
+        if (p > 0) {
+          hhform_gate(v, T.glob + 4, xinf, xtau);
+          T.state[0][q] = cnexp(T.state[0][q], xinf, xtau, dt);
+        }
+        if (qq > 0) {
+          hhform_gate(v, T.glob + 10, xinf, xtau);
+          T.state[1][q] = cnexp(T.state[1][q], xinf, xtau, dt);
+        }
+      }
+      break;
+    }
+    case T_SK:
+      for (int j = lane; j < tot; j += 32) {
+        const int64_t q = ib + j;
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        double cai = cai_g[node_base + slot];
+        if (cai < 1e-9) cai = 1e-9;
+        const double zinf = 1.0 / (1.0 + pow(T.glob[1] / cai, T.glob[2]));
+        T.state[0][q] = cnexp(T.state[0][q], zinf, T.glob[3], dt);
+      }
+      break;
+    case T_CADYN: {
+      // derivimplicit on a linear ODE: one Newton step of backward Euler is exact (L278)
+      const double kappa = 1e4 * T.glob[0] / (2.0 * 96485.33212 * T.glob[1]);
+      const double taud = T.glob[2], cmin = T.glob[3];
+      for (int j = lane; j < tot; j += 32) {
+        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const double ica = I[slot];
+        const double y0 = cai_g[node_base + slot];
+        cai_g[node_base + slot] = (y0 + dt * (-kappa * ica + cmin / taud)) / (1.0 + dt / taud);
+      }
+      break;
+    }
+    default: break;
+  }
+  (void)vold;
+}
+
+__device__ __forceinline__ void state_point(const DTable &T, int64_t i0, int64_t i1, int lane,
+                                            double dt) {
+  switch (T.type) {
+    case T_EXPSYN:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const double g = T.state[0][q];
+        if (g != 0.0) T.state[0][q] = cnexp(g, 0.0, T.param[0][q], dt);
+      }
+      break;
+    case T_EXP2SYN:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const double A = T.state[0][q], B = T.state[1][q];
+        if (A != 0.0 || B != 0.0) {
+          T.state[0][q] = cnexp(A, 0.0, T.param[0][q], dt);
+          T.state[1][q] = cnexp(B, 0.0, T.param[1][q], dt);
+        }
+      }
+      break;
+    case T_AMPANMDA:
+      for (int64_t q = i0 + lane; q < i1; q += 32) {
+        const double a0 = T.state[0][q], a1 = T.state[1][q], a2 = T.state[2][q],
+                     a3 = T.state[3][q];
+        if (a0 != 0.0 || a1 != 0.0 || a2 != 0.0 || a3 != 0.0) {
+          T.state[0][q] = cnexp(a0, 0.0, T.glob[0], dt);
+          T.state[1][q] = cnexp(a1, 0.0, T.glob[1], dt);
+          T.state[2][q] = cnexp(a2, 0.0, T.glob[2], dt);
+          T.state[3][q] = cnexp(a3, 0.0, T.glob[3], dt);
+        }
+      }
+      break;
+    default: break;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// the step kernel: one warp per group
+// ------------------------------------------------------------------------------------------
+
+template <int WPB>
+__global__ void __launch_bounds__(WPB * 32) step_kernel(const DModel *__restrict__ Mp,
+                                                        int64_t k) {
+  extern __shared__ double smem[];
+  const DModel &M = *Mp;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = blockIdx.x * WPB + warp;
+  if (g >= M.n_group) return;
+  const GroupInfo gi = M.grp[g];
+  const ClassInfo ci = M.cls[gi.cls];
+  const int n = ci.n, G = ci.G, lgG = ci.lgG;
+  const int nG = n << lgG;
+  double *D = smem + (size_t)warp * M.warp_smem_doubles;
+  double *R = D + nG;
+  double *I = R + nG;  // only valid when ci.needs_ica
+  const int64_t nb = gi.node_base;
+  const double dt = M.dt;
+  const double t_mid = ((double)k + 0.5) * dt;
+
+  // ---- load: D = static diagonal, R = v_old + static rhs --------------------------------
+  {
+    const double *__restrict__ ds = M.dstat + nb;
+    const double *__restrict__ rs = M.rstat + nb;
+    const double *__restrict__ vv = M.v + nb;
+    for (int j = lane; j < nG; j += 32) {
+      D[j] = ds[j];
+      R[j] = vv[j] + rs[j];
+    }
+    if (ci.needs_ica)
+      for (int j = lane; j < nG; j += 32) I[j] = 0.0;
+  }
+  __syncwarp();
+
+  // ---- nrn_cur -------------------------------------------------------------------------
+  for (int t = 0; t < M.n_table; ++t) {
+    const DTable &T = M.tab[t];
+    if (T.is_point) {
+      const int64_t i0 = T.pp_first[g], i1 = T.pp_first[g + 1];
+      if (i1 > i0) {
+        cur_point(T, i0, i1, D, R, M.v + nb, lane, t_mid);
+        __syncwarp();
+      }
+    } else {
+      const int cnt = T.cls_cnt[gi.cls];
+      if (cnt > 0) {
+        cur_distributed(T, T.grp_instbase[g], cnt, G, lgG, M.dist_nodes + T.cls_nodeoff[gi.cls],
+                        D, R, I, M.v + nb, lane);
+        __syncwarp();
+      }
+    }
+  }
+
+  // ---- Hines triangularisation: rounds of P independent nodes per cell -------------------
+  const int c = lane & (G - 1), p = lane >> lgG;
+  const int P = 32 >> lgG;
+  const uint32_t *__restrict__ sched = M.sched + ci.sched_off;
+  const double *__restrict__ as = M.a_s + gi.ab_base + lane;
+  const double *__restrict__ bs = M.b_s + gi.ab_base + lane;
+  const int rounds = ci.rounds;
+  {
+    uint32_t e = rounds > 0 ? sched[p] : CN_IDLE;
+    double a = rounds > 0 ? as[0] : 0.0, b = rounds > 0 ? bs[0] : 0.0;
+    for (int r = 0; r < rounds; ++r) {
+      uint32_t e_n = CN_IDLE;
+      double a_n = 0.0, b_n = 0.0;
+      if (r + 1 < rounds) {  // prefetch the next round's entry and off-diagonals
+        e_n = sched[(r + 1) * P + p];
+        a_n = as[(size_t)(r + 1) * 32];
+        b_n = bs[(size_t)(r + 1) * 32];
+      }
+      if ((e & 0xFFFFu) != CN_IDLE) {
+        const int si = ((e & 0xFFFFu) << lgG) + c, sp = ((e >> 16) << lgG) + c;
+        const double di = D[si], ri = R[si];
+        const double rinv = 1.0 / di;
+        const double f = a * rinv;
+        D[sp] -= f * b;
+        R[sp] -= f * ri;
+        D[si] = b * rinv;   // back-substitution multiplier
+        R[si] = ri * rinv;
+      }
+      __syncwarp();
+      e = e_n;
+      a = a_n;
+      b = b_n;
+    }
+  }
+  // root: local node 0
+  if (p == 0) R[c] = R[c] / D[c];
+  __syncwarp();
+  // ---- back-substitution, rounds in reverse ------------------------------------------------
+  for (int r = rounds - 1; r >= 0; --r) {
+    const uint32_t e = sched[r * P + p];
+    if ((e & 0xFFFFu) != CN_IDLE) {
+      const int si = ((e & 0xFFFFu) << lgG) + c, sp = ((e >> 16) << lgG) + c;
+      R[si] -= D[si] * R[sp];
+    }
+    __syncwarp();
+  }
+
+  // ---- voltage update: v = solution ----------------------------------------------------------
+  {
+    double *__restrict__ vv = M.v + nb;
+    for (int j = lane; j < nG; j += 32) vv[j] = R[j];
+  }
+
+  // ---- nrn_state with the new v --------------------------------------------------------------
+  for (int t = 0; t < M.n_table; ++t) {
+    const DTable &T = M.tab[t];
+    if (T.n_state == 0 && T.type != T_CADYN) continue;
+    if (T.is_point) {
+      const int64_t i0 = T.pp_first[g], i1 = T.pp_first[g + 1];
+      if (i1 > i0) state_point(T, i0, i1, lane, dt);
+    } else {
+      const int cnt = T.cls_cnt[gi.cls];
+      if (cnt > 0) {
+        state_distributed(T, T.grp_instbase[g], cnt, G, lgG,
+                          M.dist_nodes + T.cls_nodeoff[gi.cls], R, M.cai, nb, I, nullptr, lane,
+                          dt, M.q10);
+        __syncwarp();
+      }
+    }
+  }
+
+  // ---- threshold detection on the roots (warp ballot, one atomic per warp) --------------------
+  {
+    bool fire = false;
+    int pc = 0;
+    if (p == 0 && c < gi.ncell) {
+      pc = gi.cell_base + c;
+      const bool above = R[c] > M.thr[pc];
+      fire = above && !M.flag[pc];
+      M.flag[pc] = (unsigned char)above;
+    }
+    const unsigned ball = __ballot_sync(0xffffffffu, fire);
+    if (ball) {
+      unsigned long long base = 0;
+      const int leader = __ffs(ball) - 1;
+      if (lane == leader) base = atomicAdd(M.n_sp, (unsigned long long)__popc(ball));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (fire) {
+        const unsigned long long pos = base + __popc(ball & ((1u << lane) - 1u));
+        if ((int64_t)pos < M.sp_cap) {
+          M.sp_gid[pos] = M.gid_of_pcell[pc];
+          M.sp_step[pos] = k + 1;
+        } else {
+          *M.overflow = 1;
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// event delivery for step k (L64): every spike (gid, s) with a NetCon of delay k - s
+// ------------------------------------------------------------------------------------------
+
+__device__ __forceinline__ void receive(const DModel &M, int64_t nc) {
+  const DTable &T = M.tab[M.nc_tab[nc]];
+  const int64_t q = M.nc_inst[nc];
+  const double w = M.nc_w[nc];
+  switch (T.type) {
+    case T_EXPSYN: atomicAdd(&T.state[0][q], w); break;
+    case T_EXP2SYN: {
+      const double wf = w * T.param[4][q];  // param[4] = peak-normalisation factor
+      atomicAdd(&T.state[0][q], wf);
+      atomicAdd(&T.state[1][q], wf);
+      break;
+    }
+    case T_AMPANMDA: {
+      const double wa = w * T.glob[7], wn = w * T.glob[8];  // factors appended by the host
+      atomicAdd(&T.state[0][q], wa);
+      atomicAdd(&T.state[1][q], wa);
+      atomicAdd(&T.state[2][q], wn);
+      atomicAdd(&T.state[3][q], wn);
+      break;
+    }
+    default: break;
+  }
+}
+
+__device__ __forceinline__ void deliver_source(const DModel &M, int32_t gid, int32_t d,
+                                               int lane) {
+  int64_t lo = M.src_first[gid], hi = M.src_first[gid + 1];
+  if (lo >= hi) return;
+  // lower / upper bound of delay d in the delay-sorted NetCon list of this source
+  int64_t a = lo, b = hi;
+  while (a < b) {
+    const int64_t mid = (a + b) >> 1;
+    if (M.nc_d[mid] < d) a = mid + 1; else b = mid;
+  }
+  const int64_t first = a;
+  b = hi;
+  while (a < b) {
+    const int64_t mid = (a + b) >> 1;
+    if (M.nc_d[mid] <= d) a = mid + 1; else b = mid;
+  }
+  for (int64_t nc = first + lane; nc < a; nc += 32) receive(M, nc);
+}
+
+__global__ void __launch_bounds__(128) deliver_kernel(const DModel *__restrict__ Mp, int64_t k) {
+  const DModel &M = *Mp;
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    unsigned long long ns = *M.n_sp;
+    if ((int64_t)ns > M.sp_cap) ns = (unsigned long long)M.sp_cap;
+    M.sp_end[k % M.wr] = (int64_t)ns;  // all spikes with step <= k are recorded by now
+  }
+  const int64_t s_lo = k - M.maxd, s_hi = k - M.mind;  // spike steps that may deliver now
+  if (s_hi < 0) return;
+  const int64_t i_lo = (s_lo - 1 >= 0) ? M.sp_end[(s_lo - 1) % M.wr] : 0;
+  const int64_t i_hi = M.sp_end[s_hi % M.wr];
+  for (int64_t i = i_lo + warp; i < i_hi; i += nwarp)
+    deliver_source(M, M.sp_gid[i], (int32_t)(k - M.sp_step[i]), lane);
+  if (M.n_stim > 0) {
+    int64_t a = 0, b = M.n_stim;
+    while (a < b) {
+      const int64_t mid = (a + b) >> 1;
+      if (M.stim_step[mid] < s_lo) a = mid + 1; else b = mid;
+    }
+    for (int64_t i = a + warp; i < M.n_stim && M.stim_step[i] <= s_hi; i += nwarp)
+      deliver_source(M, M.stim_gid[i], (int32_t)(k - M.stim_step[i]), lane);
+  }
+}
+
+__global__ void probe_kernel(const double *__restrict__ v, const int64_t *__restrict__ pos,
+                             int n_probe, double *__restrict__ trace, int64_t row) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < n_probe) trace[row * n_probe + j] = v[pos[j]];
+}
+
+__global__ void gather_kernel(const double *__restrict__ src, const int64_t *__restrict__ pos,
+                              int64_t n, double *__restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = src[pos[i]];
+}
+
+}  // namespace cn

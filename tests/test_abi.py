@@ -1,0 +1,105 @@
+"""Host-side checks of the C ABI (no GPU): the library loads, exports every symbol include/cn.h
+declares, validates descriptions at create time, and refuses to compute without a device."""
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import cn_workloads as W
+import paper_1901_10975_b200 as cn
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    from paper_1901_10975_b200.build import build
+    build()
+
+
+def test_exports_every_declared_symbol():
+    hdr = (ROOT / "include" / "cn.h").read_text()
+    declared = set(re.findall(r"\b(cn_[a-z_0-9]+)\s*\(", hdr))
+    assert {"cn_model_create", "cn_run", "cn_get_v", "cn_get_spikes"} <= declared
+    L = cn.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert declared == set(cn.EXPORTS)
+
+
+def test_create_and_initial_v_without_device():
+    m = cn.Model(W.config1())
+    assert m.n_node == 488 and m.n_cell == 8
+    assert np.all(m.get_v() == -65.0)
+    g, s = m.get_spikes()
+    assert len(g) == 0
+    info = m.layout_info()
+    assert info["n_class"] == 1 and info["n_group"] >= 2
+
+
+def test_shape_classes_found_in_shuffled_cells():
+    d = W.config4(n_cell=256, n_types=8)
+    m = cn.Model(d)
+    assert m.layout_info()["n_class"] == 8
+    d = W.random_tree_cells(9, 10, 40, stream="abi")
+    assert cn.Model(d).layout_info()["n_class"] == 9
+
+
+def _expect(desc, code):
+    with pytest.raises(cn.CnError) as e:
+        cn.Model(desc)
+    assert e.value.code == code
+
+
+def test_validation_errors():
+    base = W.config1()
+    d = dict(base); d["parent"] = base["parent"].copy(); d["parent"][5] = 9
+    _expect(d, -2)
+    d = dict(base); d["parent"] = base["parent"].copy(); d["parent"][62] = 3
+    _expect(d, -2)
+    d = dict(base); d["parent"] = base["parent"].copy(); d["parent"][61] = 60
+    _expect(d, -2)
+    d = dict(base); d["area"] = base["area"].copy(); d["area"][7] = 0.0
+    _expect(d, -1)
+    d = dict(base); d["cm"] = base["cm"].copy(); d["cm"][7] = np.nan
+    _expect(d, -1)
+    d = dict(base); d["ri"] = base["ri"].copy(); d["ri"][7] = -1.0
+    _expect(d, -1)
+    d = dict(base); d["mechs"] = [dict(m) for m in base["mechs"]]
+    d["mechs"][0] = dict(d["mechs"][0]); d["mechs"][0]["node"] = np.array([10 ** 6] * 8, np.int32)
+    _expect(d, -3)
+    d = dict(base); d["netcons"] = dict(base["netcons"])
+    d["netcons"]["tgt_inst"] = base["netcons"]["tgt_inst"].copy(); d["netcons"]["tgt_inst"][0] = 99
+    _expect(d, -4)
+    d = dict(base); d["netcons"] = dict(base["netcons"])
+    d["netcons"]["tgt_mech"] = base["netcons"]["tgt_mech"].copy(); d["netcons"]["tgt_mech"][0] = 1
+    _expect(d, -4)          # pas receives no events
+    d = dict(base); d["netcons"] = dict(base["netcons"])
+    d["netcons"]["delay"] = base["netcons"]["delay"].copy(); d["netcons"]["delay"][0] = -1.0
+    _expect(d, -4)
+    # two instances of one distributed table on one node
+    d = dict(base); d["mechs"] = list(base["mechs"])
+    pas = dict(d["mechs"][1]); pas["node"] = pas["node"].copy(); pas["node"][1] = pas["node"][0]
+    d["mechs"][1] = pas
+    _expect(d, -3)
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    m = cn.Model(W.config1())
+    with pytest.raises(cn.CnError) as e:
+        m.run(1.0, 0.025)
+    assert e.value.code == -6
+    with pytest.raises(cn.CnError) as e:
+        m.run(1.0, -0.025)
+    assert e.value.code == -5
+
+
+def test_binding_never_imports_the_oracle():
+    src = (ROOT / "paper_1901_10975_b200" / "__init__.py").read_text()
+    assert "import oracle" not in src and "from oracle" not in src
+    for f in (ROOT / "paper_1901_10975_b200" / "csrc").iterdir():
+        assert "oracle" not in f.read_text().lower().replace("no cpu", "")

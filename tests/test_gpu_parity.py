@@ -1,0 +1,190 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): identical spike (gid, step) lists and max |dV| <= 1e-6 mV at every
+recorded step.  The minimum threshold-detection margin of the oracle run is asserted to be far
+above the voltage error, so spike identity is not knife-edge (R16).
+"""
+import numpy as np
+import pytest
+
+import cn_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+DT = 0.025
+TOL = 1e-6
+
+
+@pytest.fixture(scope="module")
+def cn():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1901_10975_b200.build import build
+    build()
+    import paper_1901_10975_b200 as cn
+    return cn
+
+
+def run_both(cn, desc, tstop, dt=DT, probes=None, chunks=1, env=None):
+    from oracle import OracleModel
+    nsteps = int(round(tstop / dt))
+    if probes is None:
+        probes = np.asarray(desc["cell_first"][:-1], dtype=np.int32)
+    o = OracleModel(desc)
+    o.set_probes(probes)
+    o.run(tstop, dt)
+    g = cn.Model(desc)
+    g.set_probes(probes, nsteps)
+    for j in range(1, chunks + 1):
+        g.run(tstop * j / chunks if j < chunks else tstop, dt)
+    return o, g
+
+
+def check(o, g, tol=TOL, min_spikes=0):
+    og, os_ = o.get_spikes()
+    gg, gs = g.get_spikes()
+    assert len(og) >= min_spikes
+    tr_o, tr_g = o.get_trace(), g.get_trace()
+    assert tr_o.shape == tr_g.shape
+    err_t = np.max(np.abs(tr_o - tr_g)) if tr_o.size else 0.0
+    err_v = np.max(np.abs(o.get_v() - g.get_v())) if o.n_node else 0.0
+    assert err_t <= tol and err_v <= tol, (err_t, err_v)
+    assert list(og) == list(gg) and list(os_) == list(gs)
+    if len(og):
+        assert o.min_margin > 1e3 * max(err_t, err_v, 1e-12), (o.min_margin, err_t)
+    return err_t, err_v
+
+
+def test_config1_full(cn):
+    desc = W.config1()
+    probes = np.concatenate([desc["cell_first"][:-1], [30, 60, 100, 487]]).astype(np.int32)
+    o, g = run_both(cn, desc, 100.0, probes=probes)
+    check(o, g, min_spikes=60)
+    for t, s in ((0, 0), (0, 1), (0, 2), (2, 0)):
+        assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9
+
+
+def test_unique_topologies_one_cell_per_warp(cn):
+    desc = W.random_tree_cells(13, 5, 120, stream="gpu-u", weight=0.2, amp=2.0)
+    o, g = run_both(cn, desc, 40.0)
+    assert g.layout_info()["n_class"] == 13
+    check(o, g, min_spikes=5)
+
+
+def test_identical_random_cells_grouped(cn):
+    desc = W.random_tree_cells(11, 77, 77, stream="gpu-i", identical=True, weight=0.2, amp=2.0)
+    o, g = run_both(cn, desc, 40.0)
+    info = g.layout_info()
+    assert info["n_class"] == 1 and info["n_group"] == 3   # 4 + 4 + 3 (ragged tail group)
+    check(o, g, min_spikes=5)
+
+
+def test_hh_everywhere_config2_shape(cn):
+    desc = W.config2(n_cell=8, ring_size=4, weight=0.05)
+    o, g = run_both(cn, desc, 30.0)
+    check(o, g, min_spikes=4)
+
+
+def test_config2_one_ring_of_64(cn):
+    desc = W.config2(rings=[1])
+    o, g = run_both(cn, desc, 12.0)
+    check(o, g, min_spikes=3)
+
+
+def test_config4_small_full_length(cn):
+    desc = W.config4(n_cell=256, n_types=8)
+    o, g = run_both(cn, desc, 50.0)
+    assert g.layout_info()["n_class"] == 8
+    check(o, g, min_spikes=100)
+
+
+def test_chunked_run_equals_one_shot(cn):
+    desc = W.config1()
+    a = cn.Model(desc)
+    a.run(20.0, DT)
+    b = cn.Model(desc)
+    for t in (0.025, 1.0, 1.0, 7.3, 7.325, 20.0):
+        b.run(t, DT)
+    assert b.steps_done == 800 == a.steps_done
+    assert np.array_equal(a.get_v(), b.get_v())
+    assert [list(x) for x in a.get_spikes()] == [list(x) for x in b.get_spikes()]
+
+
+def test_run_is_deterministic(cn):
+    desc = W.config4(n_cell=128, n_types=4)
+    r = []
+    for _ in range(2):
+        m = cn.Model(desc)
+        m.run(30.0, DT)
+        r.append((m.get_v(), m.get_spikes()))
+    assert np.array_equal(r[0][0], r[1][0])
+    assert [list(x) for x in r[0][1]] == [list(x) for x in r[1][1]]
+
+
+def test_edge_cases(cn):
+    from oracle import OracleModel
+    # empty model
+    empty = {"cell_first": np.zeros(1, np.int64), "parent": np.zeros(0, np.int32),
+             "area": np.zeros(0), "ri": np.zeros(0), "cm": np.zeros(0), "mechs": [],
+             "netcons": {k: np.zeros(0) for k in ("src", "tgt_mech", "tgt_inst", "weight", "delay")},
+             "thr": np.zeros(0), "stim": {"gid": np.zeros(0, np.int32), "t": np.zeros(0)}}
+    m = cn.Model(empty)
+    m.run(1.0, DT)
+    assert m.steps_done == 40 and len(m.get_v()) == 0 and len(m.get_spikes()[0]) == 0
+    # single passive compartment: closed-form backward Euler decay
+    d = W.single_compartment([("pas", {"g": 0.001, "e": -65.0}, {})], v_init=-50.0)
+    m = cn.Model(d)
+    m.set_probes([0], 200)
+    m.run(5.0, DT)
+    n = np.arange(1, 201)
+    assert np.max(np.abs(m.get_trace()[:, 0] - (-65.0 + 15.0 * (1 + DT / 1.0) ** (-n)))) < 1e-11
+    # mechanism-free cell next to single-node cells
+    d = W.random_tree_cells(3, 1, 1, stream="gpu-e1", weight=0.5)
+    o, g = run_both(cn, d, 10.0)
+    check(o, g)
+    # tstop not after the current time is a no-op; dt change is an error
+    g.run(5.0, DT)
+    assert g.steps_done == 400
+    with pytest.raises(cn.CnError) as e:
+        g.run(20.0, 0.0125)
+    assert e.value.code == -5
+    # delay below one step
+    d = W.config1()
+    d["netcons"] = dict(d["netcons"]); d["netcons"]["delay"] = np.full(8, 0.01)
+    with pytest.raises(cn.CnError) as e:
+        cn.Model(d).run(1.0, DT)
+    assert e.value.code == -4
+    # spike buffer overflow is reported
+    m = cn.Model(W.config1())
+    m.set_spike_capacity(3)
+    with pytest.raises(cn.CnError) as e:
+        m.run(30.0, DT)
+    assert e.value.code == -7
+
+
+def test_scripted_sources_and_delays(cn):
+    from tests.test_oracle_pins import _syn_target
+    for ks in (0, 7):
+        d = _syn_target([1 * DT, 40 * DT, 400 * DT], ks * DT)
+        o, g = run_both(cn, d, (ks + 402) * DT)
+        check(o, g)
+        assert np.max(np.abs(o.get_state(1, 0) - g.get_state(1, 0))) < 1e-15
+
+
+def test_node_renumbering_invariance(cn):
+    desc = W.random_tree_cells(4, 30, 60, stream="gpu-r", weight=0.4, amp=4.0)
+    ren = W.renumber_nodes(desc)
+    a, b = cn.Model(desc), cn.Model(ren)
+    a.run(15.0, DT)
+    b.run(15.0, DT)
+    assert np.max(np.abs(b.get_v()[ren["_new_of_old"]] - a.get_v())) < 1e-9
+    assert [list(x) for x in a.get_spikes()] == [list(x) for x in b.get_spikes()]
+
+
+@pytest.mark.parametrize("force_g", ["1", "2", "8"])
+def test_lanes_per_cell_variants(cn, force_g, monkeypatch):
+    monkeypatch.setenv("CN_FORCE_G", force_g)
+    desc = W.config4(n_cell=64, n_types=2)
+    o, g = run_both(cn, desc, 30.0)
+    check(o, g, min_spikes=10)

@@ -695,7 +695,7 @@ def test_p13_permuting_cells_permutes_results_bitwise():
 # ---------------------------------------------------------------------------------------------
 
 def test_p14_node_renumbering():
-    desc = W.random_tree_cells(3, 30, 60, stream="p14", weight=0.08)
+    desc = W.random_tree_cells(3, 30, 60, stream="p14", weight=0.4, amp=4.0)
     ren = W.renumber_nodes(desc)
     m, mr = OracleModel(desc), OracleModel(ren)
     m.run(15.0, DT)
