@@ -136,6 +136,11 @@ int64_t cn_launch_count(const cn_model *m);
 /* Device pointer + stream-ordered timing of the step kernels of the last run, in ms, measured
  * with CUDA events on the model's stream around the step loop. */
 int cn_last_run_ms(const cn_model *m, double *ms_out);
+/* Sample the duration of the step kernel (the dominant kernel) with CUDA event pairs on the
+ * model's stream around every `every`-th launch (0 = off), at most max_samples between reads.
+ * cn_get_kernel_timing returns the summed duration and the number of samples, and resets. */
+int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samples);
+int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
 /* Layout facts for DESIGN/bench: n_class, n_group, smem bytes per warp, rounds (max). */
 int cn_get_layout_info(const cn_model *m, int64_t *info4);
 /* Spike buffer capacity (default 16*n_cell + 65536); before the first cn_run only. */

@@ -37,7 +37,7 @@ MECH = {
 
 EXPORTS = ("cn_model_create", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
            "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_steps_done",
-           "cn_launch_count", "cn_last_run_ms", "cn_get_layout_info", "cn_set_spike_capacity",
+           "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_get_kernel_timing", "cn_get_layout_info", "cn_set_spike_capacity",
            "cn_model_destroy", "cn_last_error")
 
 
@@ -91,6 +91,8 @@ def lib():
         L.cn_launch_count.restype = C.c_int64
         L.cn_launch_count.argtypes = [vp]
         L.cn_last_run_ms.argtypes = [vp, C.POINTER(C.c_double)]
+        L.cn_set_kernel_timing.argtypes = [vp, C.c_int32, C.c_int32]
+        L.cn_get_kernel_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cn_get_layout_info.argtypes = [vp, vp]
         L.cn_set_spike_capacity.argtypes = [vp, C.c_int64]
         L.cn_model_destroy.restype = None
@@ -248,6 +250,14 @@ class Model:
         ms = C.c_double()
         _check(lib().cn_last_run_ms(self._h, C.byref(ms)))
         return ms.value
+
+    def set_kernel_timing(self, every, max_samples=4096):
+        _check(lib().cn_set_kernel_timing(self._h, int(every), int(max_samples)))
+
+    def get_kernel_timing(self):
+        ms, n = C.c_double(), C.c_int64()
+        _check(lib().cn_get_kernel_timing(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     def layout_info(self):
         a = np.zeros(4, dtype=np.int64)

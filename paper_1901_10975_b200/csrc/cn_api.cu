@@ -148,6 +148,9 @@ struct cn_model {
   cudaStream_t stream = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
+  int ktime_every = 0;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ktime_ev;
+  size_t ktime_used = 0;
   // probes
   std::vector<int32_t> probe;
   int64_t probe_cap = 0, probe_rows = 0;
@@ -933,6 +936,9 @@ static int run_steps(cn_model *m, int64_t K) {
     }
     if (ng > 0) {
       cudaError_t e;
+      const bool timeit = m->ktime_every > 0 && (k % m->ktime_every) == 0 &&
+                          m->ktime_used < m->ktime_ev.size();
+      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
       switch (m->wpb) {
         case 8: e = launch_step<8>(m, k); break;
         case 4: e = launch_step<4>(m, k); break;
@@ -940,6 +946,7 @@ static int run_steps(cn_model *m, int64_t K) {
         default: e = launch_step<1>(m, k); break;
       }
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "step launch failed: %s", cudaGetErrorString(e));
+      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
       m->launches++;
     }
     if (!m->probe.empty() && m->probe_rows < m->probe_cap) {
@@ -1111,9 +1118,41 @@ extern "C" int cn_set_spike_capacity(cn_model *m, int64_t cap) {
   return CN_OK;
 }
 
+extern "C" int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samples) {
+  if (!m || every < 0 || max_samples < 0) return fail(CN_ERR_ARG, "bad argument");
+  for (auto &pr : m->ktime_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  m->ktime_ev.clear();
+  m->ktime_used = 0;
+  m->ktime_every = every;
+  if (every > 0)
+    for (int i = 0; i < max_samples; ++i) {
+      cudaEvent_t a, b;
+      CU(cudaEventCreate(&a));
+      CU(cudaEventCreate(&b));
+      m->ktime_ev.emplace_back(a, b);
+    }
+  return CN_OK;
+}
+
+extern "C" int cn_get_kernel_timing(cn_model *m, double *sum_ms, int64_t *count) {
+  if (!m || !sum_ms || !count) return fail(CN_ERR_ARG, "NULL argument");
+  double tot = 0.0;
+  for (size_t i = 0; i < m->ktime_used; ++i) {
+    float f = 0.f;
+    CU(cudaEventSynchronize(m->ktime_ev[i].second));
+    CU(cudaEventElapsedTime(&f, m->ktime_ev[i].first, m->ktime_ev[i].second));
+    tot += f;
+  }
+  *sum_ms = tot;
+  *count = (int64_t)m->ktime_used;
+  m->ktime_used = 0;
+  return CN_OK;
+}
+
 extern "C" void cn_model_destroy(cn_model *m) {
   if (!m) return;
   if (m->uploaded) cudaStreamSynchronize(m->stream);
+  for (auto &pr : m->ktime_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   for (void *p : m->dev_allocs) cudaFree(p);
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);
