@@ -111,6 +111,8 @@ struct HClass {
   int sched_off = 0;
   std::vector<int32_t> cells;
   std::vector<uint32_t> sched;
+  std::vector<int32_t> node_off;  // local node -> slot offset round*32 + p*G (root: rounds*32)
+  int nodeoff_off = 0;
 };
 
 struct cn_model {
@@ -483,7 +485,7 @@ static int build_layout(cn_model *m) {
   int64_t smem_cap = 24 * 1024;
   if (const char *e = std::getenv("CN_WARP_SMEM")) smem_cap = std::atoll(e);
   const int64_t hard_cap = 200 * 1024;
-  int sched_total = 0;
+  int sched_total = 0, nodeoff_total = 0;
   m->warp_smem_doubles = 0;
   for (HClass &K : m->cls) {
     K.count = (int64_t)K.cells.size();
@@ -510,6 +512,15 @@ static int build_layout(cn_model *m) {
     K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched);
     K.sched_off = sched_total;
     sched_total += (int)K.sched.size();
+    K.node_off.assign(K.n, 0);
+    K.node_off[0] = K.rounds * 32;
+    for (int r = 0; r < K.rounds; ++r)
+      for (int p = 0; p < 32 / G; ++p) {
+        const uint32_t e = K.sched[(size_t)r * (32 / G) + p];
+        if ((e & 0xFFFFu) != CN_IDLE) K.node_off[e & 0xFFFFu] = r * 32 + p * G;
+      }
+    K.nodeoff_off = nodeoff_total;
+    nodeoff_total += K.n;
     m->warp_smem_doubles = std::max(m->warp_smem_doubles, K.n * G * arrays);
   }
   // groups
@@ -533,15 +544,15 @@ static int build_layout(cn_model *m) {
         m->cell_grp[cell] = gidx;
         m->cell_slot[cell] = c;
         const int64_t f = m->cell_first[cell];
-        for (int i = 0; i < K.n; ++i) m->node_pos[f + i] = node_base + (int64_t)i * K.G + c;
+        for (int i = 0; i < K.n; ++i) m->node_pos[f + i] = ab_base + K.node_off[i] + c;
       }
       m->grp.push_back(gi);
       node_base += (int64_t)K.n * K.G;
-      ab_base += (int64_t)K.rounds * 32;
+      ab_base += (int64_t)(K.rounds + 1) * 32;
       cell_base += K.G;
     }
   }
-  m->n_pnode = node_base;
+  m->n_pnode = ab_base;  // all node arrays live in schedule order
   m->n_ab = ab_base;
   m->n_pcell = cell_base;
   const int ng = (int)m->grp.size();
@@ -674,11 +685,13 @@ static int finalize(cn_model *m, double dt) {
   // schedule-ordered off-diagonals
   std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
   std::vector<uint32_t> sched_all;
+  std::vector<int32_t> nodeoff_all;
   std::vector<ClassInfo> cinfo(m->cls.size());
   for (size_t kc = 0; kc < m->cls.size(); ++kc) {
     const HClass &K = m->cls[kc];
-    cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, 0, 0};
+    cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, K.nodeoff_off, 0};
     sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
+    nodeoff_all.insert(nodeoff_all.end(), K.node_off.begin(), K.node_off.end());
   }
   // inverse map: (group, slot) -> caller cell
   std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
@@ -737,6 +750,7 @@ static int finalize(cn_model *m, double dt) {
     GroupInfo *dg; ClassInfo *dc; uint32_t *ds; int32_t *dn;
     UP(m->grp, dg); UP(cinfo, dc); UP(sched_all, ds); UP(m->dist_nodes, dn);
     H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
+    int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
     double *p;
     UP(v0, m->d_v); H.v = m->d_v;
     UP(dstat, p); H.dstat = p;
@@ -892,10 +906,6 @@ static int finalize(cn_model *m, double dt) {
     rc = dev_alloc(m, (size_t)(m->probe_cap * (int64_t)m->probe.size()), &m->d_trace, false);
     if (rc) return rc;
   }
-  {
-    std::vector<DModel> one(1, H);
-    UP(one, m->d_m);
-  }
 #undef UP
   CU(cudaEventCreate(&m->ev0));
   CU(cudaEventCreate(&m->ev1));
@@ -919,7 +929,7 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
     if (e != cudaSuccess) return e;
     attr_set[WPB] = true;
   }
-  step_kernel<WPB><<<(ng + WPB - 1) / WPB, WPB * 32, smem, m->stream>>>(m->d_m, k);
+  step_kernel<WPB><<<(ng + WPB - 1) / WPB, WPB * 32, smem, m->stream>>>(m->hm, k);
   return cudaGetLastError();
 }
 
@@ -931,7 +941,7 @@ static int run_steps(cn_model *m, int64_t K) {
   for (int64_t s = 0; s < K; ++s) {
     const int64_t k = m->k + s;
     if (m->n_netcon > 0) {
-      deliver_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->d_m, k);
+      deliver_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->hm, k);
       m->launches++;
     }
     if (ng > 0) {

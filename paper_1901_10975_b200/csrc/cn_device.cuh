@@ -2,11 +2,14 @@
 //
 // One warp integrates one GROUP = G cells of one shape class (same topology and same placement
 // of distributed mechanisms) for one dt, with P = 32/G lanes per cell:
-//   load   : D = dstat, R = v + rstat            (node-parallel, coalesced, interleaved [node][cell])
-//   cur    : per mechanism table, D += g, R += g*E   (nrn_cur; conductance form L160)
+//   cur    : per mechanism table, D += g, R += g*E into a zeroed shared-memory system
+//            (nrn_cur; conductance form L160)
 //   solve  : Hines elimination in shared memory, list-scheduled in rounds of P independent nodes
-//            (L62, L66, L196); off-diagonals are stored in schedule order so they stream coalesced
-//   store  : v = R                               (L66)
+//            (L62, L66, L196).  EVERY per-node array (v, static diagonal / rhs, off-diagonals) is
+//            stored in schedule order [round][lane], so each round is one coalesced 256 B load per
+//            array, prefetched several rounds ahead in registers; a node's static terms and old v
+//            are added when the node is eliminated, and v_new is stored from the back-substitution
+//            round (L66).  There is no separate load or store pass over the nodes.
 //   state  : per mechanism table, cnexp / implicit updates with the new v (L67, L278)
 //   detect : warp-ballot threshold detection on the root nodes, spike append (L68)
 // The linear system is the paper's backward-Euler system written for v_new instead of delta-v and
@@ -15,7 +18,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define CN_MAX_TABLES 32
+#define CN_MAX_TABLES 24
 #define CN_MAX_PARAM 8
 #define CN_MAX_STATE 4
 #define CN_MAX_GLOBAL 16
@@ -42,13 +45,13 @@ struct GroupInfo {
   int32_t cls, ncell;
   int32_t cell_base;   // first permuted cell index of the group
   int32_t pad;
-  int64_t node_base;   // first permuted node of the group (n*G nodes follow, interleaved)
-  int64_t ab_base;     // first entry of the group's schedule-ordered a/b arrays (rounds*32)
+  int64_t node_base;   // unused (kept for layout stability)
+  int64_t ab_base;     // first slot of the group's schedule-ordered node arrays ((rounds+1)*32)
 };
 
 struct ClassInfo {
   int32_t n, G, lgG, rounds;
-  int32_t sched_off, needs_ica, pad0, pad1;
+  int32_t sched_off, needs_ica, nodeoff_off, pad1;
 };
 
 struct DModel {
@@ -57,9 +60,10 @@ struct DModel {
   const ClassInfo *cls;
   const uint32_t *sched;        // per class: rounds * P entries, node | parent << 16
   const int32_t *dist_nodes;    // local node lists of distributed tables per class
-  double *v;                    // [n_pnode] permuted, padded
-  const double *dstat, *rstat;  // static diagonal / rhs parts (row-normalised)
-  const double *a_s, *b_s;      // off-diagonals in schedule order
+  const int32_t *node_off;      // per class: slot offset (round*32 + p*G) of every local node
+  double *v;                    // [n_slot] schedule order, padded
+  const double *dstat, *rstat;  // static diagonal / rhs parts (row-normalised), schedule order
+  const double *a_s, *b_s;      // off-diagonals, schedule order
   double *cai;                  // per node (only when a table needs it) else null
   const double *thr;            // [n_pcell]
   unsigned char *flag;          // [n_pcell]
@@ -141,12 +145,23 @@ __device__ __forceinline__ double mgblock(double v, double mg) {
 // nrn_cur: conductance G (row-normalised) and G*E into the shared-memory system
 // ------------------------------------------------------------------------------------------
 
+// Where a group's node (shared-memory slot = node*G + cell) lives in the schedule-ordered arrays.
+struct GroupView {
+  int64_t ab;             // first slot of the group
+  const int32_t *noff;    // class table: node -> round*32 + p*G
+  int G, lgG;
+  __device__ __forceinline__ int64_t gpos(int slot) const {
+    return ab + noff[slot >> lgG] + (slot & (G - 1));
+  }
+};
+
 // Distributed table, lockstep over the group's cells: instance j = k*G + c sits on node
 // nodes[k] of cell c.  At most one instance per node and table, so plain read-modify-write.
-__device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int cnt, int G,
-                                                int lgG, const int32_t *nodes, double *D,
-                                                double *R, double *I, const double *vold,
-                                                int lane) {
+__device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int cnt,
+                                                const GroupView &gv, const int32_t *nodes,
+                                                double *D, double *R, double *I,
+                                                const double *v_g, int lane) {
+  const int G = gv.G, lgG = gv.lgG;
   const int tot = cnt << lgG;
   switch (T.type) {
     case T_HH: {
@@ -176,7 +191,7 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
         const double invc = T.param[1][q];
         D[slot] += g * invc;
         R[slot] += g * E * invc;
-        if (to_ica) I[slot] += g * (vold[slot] - E);  // ica uses v_old, still in global memory
+        if (to_ica) I[slot] += g * (v_g[gv.gpos(slot)] - E);  // ica uses v_old (still in HBM)
       }
       break;
     }
@@ -198,8 +213,8 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
 
 // Point-process table: instances of this group, arbitrary nodes -> shared-memory atomics.
 __device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i1, double *D,
-                                          double *R, const double *vold, int lane,
-                                          double t_mid) {
+                                          double *R, const GroupView &gv, const double *v_g,
+                                          int lane, double t_mid) {
   switch (T.type) {
     case T_EXPSYN:
       for (int64_t q = i0 + lane; q < i1; q += 32) {
@@ -230,11 +245,12 @@ __device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i
       break;
     case T_AMPANMDA:
       for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const int slot = T.pp_slot[q];
         const double gA = T.state[1][q] - T.state[0][q];
         const double gN = T.state[3][q] - T.state[2][q];
         if (gA != 0.0 || gN != 0.0) {
-          const double g = (gA + T.glob[4] * gN * mgblock(vold[slot], T.glob[5])) * T.param[0][q];
+          const int slot = T.pp_slot[q];
+          const double g =
+              (gA + T.glob[4] * gN * mgblock(v_g[gv.gpos(slot)], T.glob[5])) * T.param[0][q];
           atomicAdd(&D[slot], g);
           atomicAdd(&R[slot], g * T.glob[6]);
         }
@@ -248,12 +264,12 @@ __device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i
 // nrn_state with the new v (in R)
 // ------------------------------------------------------------------------------------------
 
-__device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, int cnt, int G,
-                                                  int lgG, const int32_t *nodes,
+__device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, int cnt,
+                                                  const GroupView &gv, const int32_t *nodes,
                                                   const double *R, double *cai_g,
-                                                  int64_t node_base, const double *I,
-                                                  const double *vold, int lane, double dt,
+                                                  const double *I, int lane, double dt,
                                                   double q10) {
+  const int G = gv.G, lgG = gv.lgG;
   const int tot = cnt << lgG;
   switch (T.type) {
     case T_HH:
@@ -289,7 +305,7 @@ __device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, i
       for (int j = lane; j < tot; j += 32) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
-        double cai = cai_g[node_base + slot];
+        double cai = cai_g[gv.gpos(slot)];
         if (cai < 1e-9) cai = 1e-9;
         const double zinf = 1.0 / (1.0 + pow(T.glob[1] / cai, T.glob[2]));
         T.state[0][q] = cnexp(T.state[0][q], zinf, T.glob[3], dt);
@@ -301,15 +317,14 @@ __device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, i
       const double taud = T.glob[2], cmin = T.glob[3];
       for (int j = lane; j < tot; j += 32) {
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
-        const double ica = I[slot];
-        const double y0 = cai_g[node_base + slot];
-        cai_g[node_base + slot] = (y0 + dt * (-kappa * ica + cmin / taud)) / (1.0 + dt / taud);
+        const int64_t gp = gv.gpos(slot);
+        const double y0 = cai_g[gp];
+        cai_g[gp] = (y0 + dt * (-kappa * I[slot] + cmin / taud)) / (1.0 + dt / taud);
       }
       break;
     }
     default: break;
   }
-  (void)vold;
 }
 
 __device__ __forceinline__ void state_point(const DTable &T, int64_t i0, int64_t i1, int lane,
@@ -350,11 +365,12 @@ __device__ __forceinline__ void state_point(const DTable &T, int64_t i0, int64_t
 // the step kernel: one warp per group
 // ------------------------------------------------------------------------------------------
 
+#define CN_PF 4  // rounds of prefetch distance for the schedule-ordered streams
+
 template <int WPB>
-__global__ void __launch_bounds__(WPB * 32) step_kernel(const DModel *__restrict__ Mp,
+__global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ DModel M,
                                                         int64_t k) {
   extern __shared__ double smem[];
-  const DModel &M = *Mp;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = blockIdx.x * WPB + warp;
   if (g >= M.n_group) return;
@@ -365,22 +381,56 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const DModel *__restrict
   double *D = smem + (size_t)warp * M.warp_smem_doubles;
   double *R = D + nG;
   double *I = R + nG;  // only valid when ci.needs_ica
-  const int64_t nb = gi.node_base;
+  const int64_t ab = gi.ab_base;
   const double dt = M.dt;
   const double t_mid = ((double)k + 0.5) * dt;
+  const int c = lane & (G - 1), p = lane >> lgG;
+  const int P = 32 >> lgG;
+  const int rounds = ci.rounds;
+  GroupView gv;
+  gv.ab = ab;
+  gv.noff = M.node_off + ci.nodeoff_off;
+  gv.G = G;
+  gv.lgG = lgG;
 
-  // ---- load: D = static diagonal, R = v_old + static rhs --------------------------------
-  {
-    const double *__restrict__ ds = M.dstat + nb;
-    const double *__restrict__ rs = M.rstat + nb;
-    const double *__restrict__ vv = M.v + nb;
-    for (int j = lane; j < nG; j += 32) {
-      D[j] = ds[j];
-      R[j] = vv[j] + rs[j];
+  // schedule-ordered streams of this lane: slot (round r, lane) = ab + r*32 + lane
+  const uint32_t *__restrict__ sched = M.sched + ci.sched_off + p;
+  const double *__restrict__ as = M.a_s + ab + lane;
+  const double *__restrict__ bs = M.b_s + ab + lane;
+  const double *__restrict__ dss = M.dstat + ab + lane;
+  const double *__restrict__ rss = M.rstat + ab + lane;
+  double *__restrict__ vs = M.v + ab + lane;
+
+  // issue the first CN_PF rounds of loads and the root's terms before anything else
+  uint32_t e_[CN_PF];
+  double a_[CN_PF], b_[CN_PF], d_[CN_PF], r_[CN_PF];
+#pragma unroll
+  for (int u = 0; u < CN_PF; ++u) {
+    e_[u] = CN_IDLE;
+    a_[u] = b_[u] = d_[u] = r_[u] = 0.0;
+    if (u < rounds) {
+      e_[u] = sched[u * P];
+      if ((e_[u] & 0xFFFFu) != CN_IDLE) {
+        a_[u] = as[(size_t)u * 32];
+        b_[u] = bs[(size_t)u * 32];
+        d_[u] = dss[(size_t)u * 32];
+        r_[u] = vs[(size_t)u * 32] + rss[(size_t)u * 32];
+      }
     }
-    if (ci.needs_ica)
-      for (int j = lane; j < nG; j += 32) I[j] = 0.0;
   }
+  double d_root = 1.0, r_root = 0.0;
+  if (p == 0) {
+    d_root = dss[(size_t)rounds * 32];
+    r_root = vs[(size_t)rounds * 32] + rss[(size_t)rounds * 32];
+  }
+
+  // ---- zero the system -------------------------------------------------------------------
+  for (int j = lane; j < nG; j += 32) {
+    D[j] = 0.0;
+    R[j] = 0.0;
+  }
+  if (ci.needs_ica)
+    for (int j = lane; j < nG; j += 32) I[j] = 0.0;
   __syncwarp();
 
   // ---- nrn_cur -------------------------------------------------------------------------
@@ -389,70 +439,72 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const DModel *__restrict
     if (T.is_point) {
       const int64_t i0 = T.pp_first[g], i1 = T.pp_first[g + 1];
       if (i1 > i0) {
-        cur_point(T, i0, i1, D, R, M.v + nb, lane, t_mid);
+        cur_point(T, i0, i1, D, R, gv, M.v, lane, t_mid);
         __syncwarp();
       }
     } else {
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
-        cur_distributed(T, T.grp_instbase[g], cnt, G, lgG, M.dist_nodes + T.cls_nodeoff[gi.cls],
-                        D, R, I, M.v + nb, lane);
+        cur_distributed(T, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls], D,
+                        R, I, M.v, lane);
         __syncwarp();
       }
     }
   }
 
   // ---- Hines triangularisation: rounds of P independent nodes per cell -------------------
-  const int c = lane & (G - 1), p = lane >> lgG;
-  const int P = 32 >> lgG;
-  const uint32_t *__restrict__ sched = M.sched + ci.sched_off;
-  const double *__restrict__ as = M.a_s + gi.ab_base + lane;
-  const double *__restrict__ bs = M.b_s + gi.ab_base + lane;
-  const int rounds = ci.rounds;
-  {
-    uint32_t e = rounds > 0 ? sched[p] : CN_IDLE;
-    double a = rounds > 0 ? as[0] : 0.0, b = rounds > 0 ? bs[0] : 0.0;
-    for (int r = 0; r < rounds; ++r) {
-      uint32_t e_n = CN_IDLE;
-      double a_n = 0.0, b_n = 0.0;
-      if (r + 1 < rounds) {  // prefetch the next round's entry and off-diagonals
-        e_n = sched[(r + 1) * P + p];
-        a_n = as[(size_t)(r + 1) * 32];
-        b_n = bs[(size_t)(r + 1) * 32];
+  for (int r0 = 0; r0 < rounds; r0 += CN_PF) {
+#pragma unroll
+    for (int u = 0; u < CN_PF; ++u) {
+      const int r = r0 + u;
+      if (r < rounds) {
+        const uint32_t e = e_[u];
+        if ((e & 0xFFFFu) != CN_IDLE) {
+          const int si = ((e & 0xFFFFu) << lgG) + c, sp = ((e >> 16) << lgG) + c;
+          const double di = D[si] + d_[u], ri = R[si] + r_[u];
+          const double rinv = 1.0 / di;
+          const double f = a_[u] * rinv;
+          D[sp] -= f * b_[u];
+          R[sp] -= f * ri;
+          D[si] = b_[u] * rinv;   // back-substitution multiplier
+          R[si] = ri * rinv;
+        }
+        __syncwarp();
+        const int rn = r + CN_PF;  // refill this ring slot
+        e_[u] = CN_IDLE;
+        if (rn < rounds) {
+          e_[u] = sched[rn * P];
+          if ((e_[u] & 0xFFFFu) != CN_IDLE) {
+            a_[u] = as[(size_t)rn * 32];
+            b_[u] = bs[(size_t)rn * 32];
+            d_[u] = dss[(size_t)rn * 32];
+            r_[u] = vs[(size_t)rn * 32] + rss[(size_t)rn * 32];
+          }
+        }
       }
+    }
+  }
+  // root: local node 0, stored in the extra round
+  if (p == 0) {
+    const double u0 = (R[c] + r_root) / (D[c] + d_root);
+    R[c] = u0;
+    vs[(size_t)rounds * 32] = u0;
+  }
+  __syncwarp();
+  // ---- back-substitution, rounds in reverse; v_new is stored in schedule order ---------------
+  {
+    uint32_t en = rounds > 0 ? sched[(rounds - 1) * P] : CN_IDLE;
+    for (int r = rounds - 1; r >= 0; --r) {
+      const uint32_t e = en;
+      if (r > 0) en = sched[(r - 1) * P];
       if ((e & 0xFFFFu) != CN_IDLE) {
         const int si = ((e & 0xFFFFu) << lgG) + c, sp = ((e >> 16) << lgG) + c;
-        const double di = D[si], ri = R[si];
-        const double rinv = 1.0 / di;
-        const double f = a * rinv;
-        D[sp] -= f * b;
-        R[sp] -= f * ri;
-        D[si] = b * rinv;   // back-substitution multiplier
-        R[si] = ri * rinv;
+        const double u = R[si] - D[si] * R[sp];
+        R[si] = u;
+        vs[(size_t)r * 32] = u;
       }
       __syncwarp();
-      e = e_n;
-      a = a_n;
-      b = b_n;
     }
-  }
-  // root: local node 0
-  if (p == 0) R[c] = R[c] / D[c];
-  __syncwarp();
-  // ---- back-substitution, rounds in reverse ------------------------------------------------
-  for (int r = rounds - 1; r >= 0; --r) {
-    const uint32_t e = sched[r * P + p];
-    if ((e & 0xFFFFu) != CN_IDLE) {
-      const int si = ((e & 0xFFFFu) << lgG) + c, sp = ((e >> 16) << lgG) + c;
-      R[si] -= D[si] * R[sp];
-    }
-    __syncwarp();
-  }
-
-  // ---- voltage update: v = solution ----------------------------------------------------------
-  {
-    double *__restrict__ vv = M.v + nb;
-    for (int j = lane; j < nG; j += 32) vv[j] = R[j];
   }
 
   // ---- nrn_state with the new v --------------------------------------------------------------
@@ -465,9 +517,8 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const DModel *__restrict
     } else {
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
-        state_distributed(T, T.grp_instbase[g], cnt, G, lgG,
-                          M.dist_nodes + T.cls_nodeoff[gi.cls], R, M.cai, nb, I, nullptr, lane,
-                          dt, M.q10);
+        state_distributed(T, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls],
+                          R, M.cai, I, lane, dt, M.q10);
         __syncwarp();
       }
     }
@@ -549,8 +600,8 @@ __device__ __forceinline__ void deliver_source(const DModel &M, int32_t gid, int
   for (int64_t nc = first + lane; nc < a; nc += 32) receive(M, nc);
 }
 
-__global__ void __launch_bounds__(128) deliver_kernel(const DModel *__restrict__ Mp, int64_t k) {
-  const DModel &M = *Mp;
+__global__ void __launch_bounds__(128) deliver_kernel(const __grid_constant__ DModel M,
+                                                      int64_t k) {
   const int lane = threadIdx.x & 31;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
