@@ -2,6 +2,7 @@
 // C ABI declared in include/cn.h.  No CPU compute path exists: every step runs in cn_device.cuh.
 #include "../../include/cn.h"
 #include "cn_device.cuh"
+#include "cn_tape.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -86,7 +87,10 @@ struct HTable {
   std::vector<double> glob;
   // layout
   int64_t n_dev = 0;               // padded device instance count
-  std::vector<int64_t> inst_pos;   // caller instance -> device instance
+  std::vector<int64_t> inst_pos;   // caller instance -> device instance (table arrays)
+  std::vector<int64_t> tape_loc;   // distributed: tape element of the first PARAMETER row of an
+                                   // instance on a tape cell, else -1
+  int64_t pp_tape_begin = 0;       // point: instances [pp_tape_begin, n) sit on tape cells
   // device
   double *d_param[CN_MAX_PARAM] = {};
   double *d_state[CN_MAX_STATE] = {};
@@ -104,7 +108,19 @@ struct HTable {
   std::vector<int64_t> cell_inst;
 };
 
+struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh)
+  int n_groups = 0;
+  int64_t n_cells = 0;                       // the first n_cells of HClass::cells are tape cells
+  std::vector<int32_t> order, pos_of;        // position -> local node, local node -> position
+  std::vector<uint32_t> row, srow, flags, mask;
+  std::vector<uint8_t> has_pp;               // per local node
+  std::vector<std::vector<int32_t>> tab_row; // [table][local node]: first row of its block or -1
+  std::vector<int32_t> cai_row, pp_row;      // per local node or -1
+  int n_rows = 0, n_srows = 0, depth = 0, prog_off = 0;
+};
+
 struct HClass {
+  HTape tp;
   int n = 0, G = 1, lgG = 0, rounds = 0, needs_ica = 0;
   int rep_cell = -1;
   int64_t count = 0;
@@ -139,6 +155,13 @@ struct cn_model {
   std::vector<int32_t> dist_nodes;  // per class and distributed table: local node lists
   int64_t n_pnode = 0, n_ab = 0;
   int32_t n_pcell = 0;
+  // interleaved (tape) groups
+  std::vector<TapeGroup> tgrp;
+  std::vector<uint8_t> cell_tape;   // per caller cell
+  int64_t n_tape = 0, n_scratch = 0;  // doubles
+  int tape_prog_cap = 0, tape_stack_cap = 0, tape_max_len = 0;
+  int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
+  std::vector<double> cai0;         // initial cai per caller node (when any table needs it)
   int warp_smem_doubles = 0, wpb = 4;
   bool any_ica = false, any_cai = false;
   // run state
@@ -388,6 +411,142 @@ static inline uint64_t mix64(uint64_t h, uint64_t x) {
   return h ^ (h >> 29);
 }
 
+// dev parameter / state rows of a distributed type on the tape (same order as the table arrays)
+static int tape_rows_of(const TypeInfo &ti, int type) {
+  if (type == CN_PAS || type == CN_CADYN) return 0;
+  return ti.n_dev_param + ti.n_state;
+}
+
+// Program of the interleaved kernel for one class: depth-first post-order (children before
+// parents, L196), the child visited last hands its contribution to the parent in registers, the
+// others through a stack; row offsets of every node's record on the tape and the scratch tape.
+static int build_tape_program(cn_model *m, HClass &K) {
+  HTape &P = K.tp;
+  const int n = K.n;
+  const int nt = (int)m->tab.size();
+  const int64_t f = m->cell_first[K.rep_cell];
+  std::vector<int32_t> par(n, -1);
+  std::vector<std::vector<int32_t>> ch(n);
+  for (int i = 1; i < n; ++i) {
+    par[i] = (int32_t)(m->parent[f + i] - f);
+    ch[par[i]].push_back(i);
+  }
+  // stack need of every subtree; visit the child with the largest need first
+  std::vector<int32_t> need(n, 0);
+  for (int x = n - 1; x >= 0; --x) {
+    auto &c = ch[x];
+    std::stable_sort(c.begin(), c.end(), [&](int p, int q) { return need[p] > need[q]; });
+    if (c.size() == 1) need[x] = need[c[0]];
+    else if (c.size() >= 2) need[x] = std::max(need[c[0]], 1 + need[c[1]]);
+  }
+  P.order.clear();
+  P.order.reserve(n);
+  {
+    std::vector<std::pair<int32_t, uint32_t>> st;  // node, next child
+    st.emplace_back(0, 0u);
+    while (!st.empty()) {
+      auto &top = st.back();
+      if (top.second < ch[top.first].size()) {
+        const int32_t c = ch[top.first][top.second++];
+        st.emplace_back(c, 0u);
+      } else {
+        P.order.push_back(top.first);
+        st.pop_back();
+      }
+    }
+  }
+  P.pos_of.assign(n, 0);
+  for (int j = 0; j < n; ++j) P.pos_of[P.order[j]] = j;
+  // which local nodes carry which distributed table (from the representative cell)
+  P.tab_row.assign(nt, std::vector<int32_t>());
+  std::vector<uint32_t> node_mask(n, 0);
+  std::vector<uint8_t> has_cai(n, 0), need_ica(n, 0);
+  for (int t = 0; t < nt; ++t) {
+    const HTable &T = m->tab[t];
+    if (T.ti.point) continue;
+    P.tab_row[t].assign(n, -1);
+    for (int64_t q = T.cell_first[K.rep_cell]; q < T.cell_first[K.rep_cell + 1]; ++q) {
+      const int x = (int)(T.node[T.cell_inst[q]] - f);
+      if (T.type == CN_PAS) continue;  // folded into the static rows
+      node_mask[x] |= 1u << t;
+      if (T.type == CN_CADYN) has_cai[x] = need_ica[x] = 1;
+      if (T.type == CN_SK) has_cai[x] = 1;
+    }
+  }
+  P.row.assign(n, 0);
+  P.srow.assign(n, 0);
+  P.flags.assign(n, 0);
+  P.mask.assign(n, 0);
+  P.cai_row.assign(n, -1);
+  P.pp_row.assign(n, -1);
+  uint32_t row = 0;
+  int max_len = 0;
+  std::vector<uint32_t> slen(n, 0);
+  for (int j = 0; j < n; ++j) {
+    const int x = P.order[j];
+    uint32_t fl = 0, r = row + 5, sl = 2;
+    if (x == 0) {
+      fl |= PG_ROOT;
+    } else {
+      const auto &sib = ch[par[x]];
+      if (sib.back() == x) fl |= PG_FWD;
+      else if (sib.front() == x) fl |= PG_PUSH;
+      else fl |= PG_ADD;
+    }
+    if (!ch[x].empty()) fl |= PG_FWD_IN;
+    if (ch[x].size() >= 2) fl |= PG_POP;
+    if (P.has_pp[x]) {
+      fl |= PG_HAS_PP;
+      P.pp_row[x] = (int32_t)r;
+      r += 2;
+    }
+    if (need_ica[x]) {
+      fl |= PG_NEED_ICA;
+      sl += 1;
+    }
+    if (has_cai[x]) {
+      fl |= PG_HAS_CAI;
+      P.cai_row[x] = (int32_t)r;
+      r += 1;
+      sl += 1;
+    }
+    for (int t = 0; t < nt; ++t)
+      if (node_mask[x] & (1u << t)) {
+        const HTable &T = m->tab[t];
+        P.tab_row[t][x] = (int32_t)r;
+        r += (uint32_t)tape_rows_of(T.ti, T.type);
+        sl += (uint32_t)T.ti.n_state;
+      }
+    const uint32_t len = r - row;
+    if (len > 255 || sl > 255)
+      return fail(CN_ERR_UNSUPPORTED, "too many mechanism rows on one node for the tape kernel");
+    max_len = std::max(max_len, (int)std::max(len, sl));
+    P.row[j] = row;
+    P.flags[j] = fl | (len << 8) | (sl << 16);
+    P.mask[j] = node_mask[x];
+    slen[j] = sl;
+    row = r;
+  }
+  P.n_rows = (int)row;
+  uint32_t srow = 0;
+  for (int j = n - 1; j >= 0; --j) {  // the scratch tape is written back to front
+    P.srow[j] = srow;
+    srow += slen[j];
+  }
+  P.n_srows = (int)srow;
+  // stack depth by simulation of the forward pass
+  int sp = 0, depth = 0;
+  for (int j = 0; j < n; ++j) {
+    const uint32_t fl = P.flags[j];
+    if (fl & PG_POP) --sp;
+    if ((fl & PG_KIND) == PG_PUSH && !(fl & PG_ROOT)) depth = std::max(depth, ++sp);
+  }
+  if (sp != 0) return fail(CN_ERR_TOPOLOGY, "internal: unbalanced tape program");
+  P.depth = std::max(depth, 1);
+  m->tape_max_len = std::max(m->tape_max_len, max_len);
+  return CN_OK;
+}
+
 static int build_layout(cn_model *m) {
   const int32_t nc = m->n_cell;
   const int64_t N = m->N;
@@ -477,7 +636,58 @@ static int build_layout(cn_model *m) {
   }
   m->any_ica = has_cadyn || has_caform;
   m->any_cai = has_cadyn || has_sk;
-  // choose G per class and schedule
+  if (m->any_cai) {
+    m->cai0.assign((size_t)N, 1e-4);
+    for (const HTable &T : m->tab)
+      if (T.type == CN_CADYN)
+        for (int64_t i = 0; i < T.n; ++i) m->cai0[T.node[i]] = T.glob[3];
+  }
+
+  // ---- strategy per class (north_star: interleaved one-lane-per-cell versus warp-cooperative) --
+  // A class with >= 32 same-shape cells is integrated 32 cells per warp by the tape kernel when
+  // the model is large enough to fill the GPU that way; everything else (small classes, small
+  // models, the ragged remainder of a class) goes to the warp-cooperative kernel.
+  int tape_mode = -1;  // -1 auto, 0 off, 1 on
+  if (const char *e = std::getenv("CN_TAPE")) tape_mode = std::atoi(e);
+  int64_t tape_min_cells = 8192;
+  if (const char *e = std::getenv("CN_TAPE_MIN_CELLS")) tape_min_cells = std::atoll(e);
+  int tape_min_group = 16;  // a ragged last group needs at least this many cells
+  if (const char *e = std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = std::max(1, std::atoi(e));
+  const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells);
+  m->cell_tape.assign(nc, 0);
+  for (HClass &K : m->cls) {
+    K.count = (int64_t)K.cells.size();
+    K.tp.n_groups = 0;
+    K.tp.n_cells = 0;
+    if (!tape_on || nt > 32) continue;
+    const int64_t full = K.count / 32, rem = K.count % 32;
+    K.tp.n_groups = (int)(full + (rem >= tape_min_group ? 1 : 0));
+    K.tp.n_cells = std::min<int64_t>(K.count, (int64_t)K.tp.n_groups * 32);
+    for (int64_t q = 0; q < K.tp.n_cells; ++q) m->cell_tape[K.cells[q]] = 1;
+  }
+  // point processes on tape cells mark their local node in the class
+  for (HClass &K : m->cls)
+    if (K.tp.n_groups > 0) K.tp.has_pp.assign(K.n, 0);
+  for (int t = 0; t < nt; ++t) {
+    const HTable &T = m->tab[t];
+    if (!T.ti.point) continue;
+    for (int64_t i = 0; i < T.n; ++i) {
+      const int32_t c = cell_of[T.node[i]];
+      if (m->cell_tape[c]) m->cls[m->cell_cls[c]].tp.has_pp[T.node[i] - m->cell_first[c]] = 1;
+    }
+  }
+  int prog_total = 0;
+  for (HClass &K : m->cls) {
+    if (K.tp.n_groups == 0) continue;
+    int rc = build_tape_program(m, K);
+    if (rc != CN_OK) return rc;
+    K.tp.prog_off = prog_total;
+    prog_total += K.n;
+    m->tape_prog_cap = std::max(m->tape_prog_cap, K.n);
+    m->tape_stack_cap = std::max(m->tape_stack_cap, K.tp.depth);
+  }
+
+  // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
   int force_g = 0;
   if (const char *e = std::getenv("CN_FORCE_G")) force_g = std::atoi(e);
   int max_g = 4;
@@ -488,15 +698,24 @@ static int build_layout(cn_model *m) {
   int sched_total = 0, nodeoff_total = 0;
   m->warp_smem_doubles = 0;
   for (HClass &K : m->cls) {
-    K.count = (int64_t)K.cells.size();
     K.needs_ica = m->any_ica ? 1 : 0;
+    const int64_t ccount = K.count - K.tp.n_cells;  // cells left for the cooperative kernel
+    K.sched.clear();
+    K.node_off.assign(K.n, 0);
+    if (ccount == 0) {
+      K.G = 1; K.lgG = 0; K.rounds = 0;
+      K.sched_off = sched_total;
+      K.nodeoff_off = nodeoff_total;
+      nodeoff_total += K.n;
+      continue;
+    }
     const int arrays = 2 + K.needs_ica;
     if ((int64_t)K.n * arrays * 8 > hard_cap)
       return fail(CN_ERR_UNSUPPORTED,
                   "a cell with %d nodes does not fit the on-chip solve (limit %lld nodes)", K.n,
                   (long long)(hard_cap / (arrays * 8)));
     int G = 1;
-    while (G * 2 <= max_g && G * 2 <= K.count && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap)
+    while (G * 2 <= max_g && G * 2 <= ccount && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap)
       G *= 2;
     if (force_g > 0) {
       G = 1;
@@ -512,7 +731,6 @@ static int build_layout(cn_model *m) {
     K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched);
     K.sched_off = sched_total;
     sched_total += (int)K.sched.size();
-    K.node_off.assign(K.n, 0);
     K.node_off[0] = K.rounds * 32;
     for (int r = 0; r < K.rounds; ++r)
       for (int p = 0; p < 32 / G; ++p) {
@@ -523,7 +741,7 @@ static int build_layout(cn_model *m) {
     nodeoff_total += K.n;
     m->warp_smem_doubles = std::max(m->warp_smem_doubles, K.n * G * arrays);
   }
-  // groups
+  // groups: cooperative groups first, then tape groups
   m->cell_grp.assign(nc, -1);
   m->cell_slot.assign(nc, 0);
   m->node_pos.assign((size_t)N, -1);
@@ -531,7 +749,7 @@ static int build_layout(cn_model *m) {
   int32_t cell_base = 0;
   for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
     HClass &K = m->cls[kc];
-    for (int64_t q = 0; q < K.count; q += K.G) {
+    for (int64_t q = K.tp.n_cells; q < K.count; q += K.G) {
       GroupInfo gi{};
       gi.cls = kc;
       gi.ncell = (int32_t)std::min<int64_t>(K.G, K.count - q);
@@ -552,17 +770,50 @@ static int build_layout(cn_model *m) {
       cell_base += K.G;
     }
   }
-  m->n_pnode = ab_base;  // all node arrays live in schedule order
+  m->n_pnode = ab_base;  // all node arrays of the cooperative kernel live in schedule order
   m->n_ab = ab_base;
+  m->n_cgroup = (int)m->grp.size();
+  const int ngc = m->n_cgroup;
+  int64_t tape_base = 0, scratch_base = 0;
+  for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
+    HClass &K = m->cls[kc];
+    for (int gq = 0; gq < K.tp.n_groups; ++gq) {
+      TapeGroup tg{};
+      tg.cls = kc;
+      tg.tape_base = tape_base;
+      tg.scratch_base = scratch_base;
+      tg.cell_base = cell_base;
+      tg.ncell = (int32_t)std::min<int64_t>(32, K.tp.n_cells - (int64_t)gq * 32);
+      const int gidx = ngc + (int)m->tgrp.size();
+      for (int c = 0; c < tg.ncell; ++c) {
+        const int32_t cell = K.cells[(int64_t)gq * 32 + c];
+        m->cell_grp[cell] = gidx;
+        m->cell_slot[cell] = c;
+        const int64_t f = m->cell_first[cell];
+        for (int i = 0; i < K.n; ++i)
+          m->node_pos[f + i] =
+              m->n_ab + tape_base + ((int64_t)K.tp.row[K.tp.pos_of[i]] + 4) * 32 + c;
+      }
+      m->tgrp.push_back(tg);
+      tape_base += (int64_t)K.tp.n_rows * 32;
+      scratch_base += (int64_t)K.tp.n_srows * 32;
+      cell_base += 32;
+    }
+  }
+  m->n_tape = tape_base;
+  m->n_scratch = scratch_base;
+  if (m->n_tape >= ((int64_t)1 << 32))
+    return fail(CN_ERR_UNSUPPORTED, "tape larger than 2^32 doubles");
   m->n_pcell = cell_base;
-  const int ng = (int)m->grp.size();
+  const int ng = ngc + (int)m->tgrp.size();
   // per-table instance layout
   std::vector<int32_t> dist_nodes;
   for (int t = 0; t < nt; ++t) {
     HTable &T = m->tab[t];
     T.inst_pos.assign((size_t)T.n, -1);
     if (T.ti.point) {
-      // instances ordered by group (stable), slot = local node * G + cell slot
+      // instances ordered by group (stable); cooperative groups: slot = local node * G + cell
+      // slot in shared memory; tape groups: element of the node's conductance row on the tape
       T.pp_first.assign((size_t)ng + 1, 0);
       for (int64_t i = 0; i < T.n; ++i) T.pp_first[m->cell_grp[cell_of[T.node[i]]] + 1]++;
       for (int g = 0; g < ng; ++g) T.pp_first[g + 1] += T.pp_first[g];
@@ -573,11 +824,21 @@ static int build_layout(cn_model *m) {
         const int g = m->cell_grp[cell];
         const int64_t pos = fill[g]++;
         T.inst_pos[i] = pos;
-        const int G = m->cls[m->grp[g].cls].G;
-        T.pp_slot[pos] = (int32_t)((T.node[i] - m->cell_first[cell]) * G + m->cell_slot[cell]);
+        const int32_t local = (int32_t)(T.node[i] - m->cell_first[cell]);
+        if (g < ngc) {
+          const int G = m->cls[m->grp[g].cls].G;
+          T.pp_slot[pos] = (int32_t)(local * G + m->cell_slot[cell]);
+        } else {
+          const TapeGroup &tg = m->tgrp[g - ngc];
+          const int64_t el = tg.tape_base + (int64_t)m->cls[tg.cls].tp.pp_row[local] * 32 +
+                             m->cell_slot[cell];
+          T.pp_slot[pos] = (int32_t)(uint32_t)el;
+        }
       }
+      T.pp_tape_begin = T.pp_first[ngc];
       T.n_dev = T.n;
     } else {
+      T.tape_loc.assign((size_t)T.n, -1);
       T.cls_cnt.assign(m->cls.size(), 0);
       T.cls_nodeoff.assign(m->cls.size(), 0);
       for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
@@ -588,9 +849,9 @@ static int build_layout(cn_model *m) {
         for (int64_t j = T.cell_first[rc]; j < T.cell_first[rc + 1]; ++j)
           dist_nodes.push_back((int32_t)(T.node[T.cell_inst[j]] - m->cell_first[rc]));
       }
-      T.grp_instbase.assign((size_t)ng, 0);
+      T.grp_instbase.assign((size_t)std::max(ngc, 1), 0);
       int64_t base = 0;
-      for (int g = 0; g < ng; ++g) {
+      for (int g = 0; g < ngc; ++g) {
         const GroupInfo &gi = m->grp[g];
         const HClass &K = m->cls[gi.cls];
         const int cnt = T.cls_cnt[gi.cls];
@@ -600,20 +861,32 @@ static int build_layout(cn_model *m) {
       T.n_dev = base;
       for (int32_t c = 0; c < nc; ++c) {
         const int g = m->cell_grp[c];
-        const int G = m->cls[m->grp[g].cls].G;
-        const int64_t b0 = T.grp_instbase[g];
-        int64_t kk = 0;
-        for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j, ++kk)
-          T.inst_pos[T.cell_inst[j]] = b0 + kk * G + m->cell_slot[c];
+        if (g < ngc) {
+          const int G = m->cls[m->grp[g].cls].G;
+          const int64_t b0 = T.grp_instbase[g];
+          int64_t kk = 0;
+          for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j, ++kk)
+            T.inst_pos[T.cell_inst[j]] = b0 + kk * G + m->cell_slot[c];
+        } else if (T.type != CN_PAS && T.type != CN_CADYN) {
+          const TapeGroup &tg = m->tgrp[g - ngc];
+          const HTape &P = m->cls[tg.cls].tp;
+          for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j) {
+            const int64_t i = T.cell_inst[j];
+            const int32_t local = (int32_t)(T.node[i] - m->cell_first[c]);
+            T.tape_loc[i] = tg.tape_base + (int64_t)P.tab_row[t][local] * 32 + m->cell_slot[c];
+          }
+        }
       }
     }
   }
   m->dist_nodes = std::move(dist_nodes);
-  m->hm.n_group = ng;
+  m->hm.n_group = ngc;
+  m->hm.n_tgroup = (int32_t)m->tgrp.size();
   m->hm.n_class = (int32_t)m->cls.size();
   m->hm.n_table = nt;
   static_assert(sizeof(GroupInfo) == 32, "GroupInfo layout");
-  // CTA shape: as many warps per block as fit ~100 KB, at most 8
+  static_assert(sizeof(TapeGroup) == 32, "TapeGroup layout");
+  // CTA shape of the cooperative kernel: as many warps per block as fit ~100 KB, at most 8
   const int64_t wbytes = std::max<int64_t>((int64_t)m->warp_smem_doubles * 8, 8);
   int wpb = 8;
   if (const char *e = std::getenv("CN_WPB")) wpb = std::max(1, std::atoi(e));
@@ -651,8 +924,13 @@ static int finalize(cn_model *m, double dt) {
   // dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
   std::vector<double> invc((size_t)N), bn((size_t)N, 0.0), an((size_t)N, 0.0);
   std::vector<double> dstat((size_t)m->n_pnode, 1.0), rstat((size_t)m->n_pnode, 0.0);
-  std::vector<double> v0((size_t)m->n_pnode, 0.0);
+  // one arena: [schedule-ordered v of the cooperative groups | tapes of the interleaved groups]
+  std::vector<double> v0((size_t)(m->n_ab + m->n_tape), 0.0);
+  double *tape = v0.data() + m->n_ab;
   std::vector<double> dsum((size_t)N), rsum((size_t)N, 0.0);
+  std::vector<int32_t> cell_of_node((size_t)N);
+  for (int32_t c = 0; c < m->n_cell; ++c)
+    for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of_node[i] = c;
   for (int64_t i = 0; i < N; ++i) {
     const double c = 1e-3 * m->cm[i] / dt;
     invc[i] = 1.0 / c;
@@ -678,10 +956,35 @@ static int finalize(cn_model *m, double dt) {
       }
   for (int64_t i = 0; i < N; ++i) {
     const int64_t q = m->node_pos[i];
-    dstat[q] = dsum[i] * invc[i];
-    rstat[q] = rsum[i] * invc[i];
-    v0[q] = m->v_init;
+    if (m->cell_tape[cell_of_node[i]]) {  // q is the node's v element; a, b, d, r precede it
+      double *rec = v0.data() + q;
+      rec[-4 * 32] = an[i];
+      rec[-3 * 32] = bn[i];
+      rec[-2 * 32] = dsum[i] * invc[i];
+      rec[-1 * 32] = rsum[i] * invc[i];
+      rec[0] = m->v_init;
+    } else {
+      dstat[q] = dsum[i] * invc[i];
+      rstat[q] = rsum[i] * invc[i];
+      v0[q] = m->v_init;
+    }
   }
+  // idle lanes of a ragged tape group: unit diagonal, everything else zero; cai rows
+  for (const TapeGroup &tg : m->tgrp) {
+    const HTape &P = m->cls[tg.cls].tp;
+    for (int j = 0; j < m->cls[tg.cls].n; ++j)
+      for (int l = tg.ncell; l < 32; ++l) tape[tg.tape_base + ((int64_t)P.row[j] + 2) * 32 + l] = 1.0;
+  }
+  if (m->any_cai)
+    for (int32_t c = 0; c < m->n_cell; ++c) {
+      if (!m->cell_tape[c]) continue;
+      const TapeGroup &tg = m->tgrp[m->cell_grp[c] - m->n_cgroup];
+      const HTape &P = m->cls[tg.cls].tp;
+      const int64_t f = m->cell_first[c];
+      for (int i = 0; i < m->cls[tg.cls].n; ++i)
+        if (P.cai_row[i] >= 0)
+          tape[tg.tape_base + (int64_t)P.cai_row[i] * 32 + m->cell_slot[c]] = m->cai0[f + i];
+    }
   // schedule-ordered off-diagonals
   std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
   std::vector<uint32_t> sched_all;
@@ -695,8 +998,11 @@ static int finalize(cn_model *m, double dt) {
   }
   // inverse map: (group, slot) -> caller cell
   std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
-  for (int32_t c = 0; c < m->n_cell; ++c)
-    cell_of_pcell[m->grp[m->cell_grp[c]].cell_base + m->cell_slot[c]] = c;
+  for (int32_t c = 0; c < m->n_cell; ++c) {
+    const int g = m->cell_grp[c];
+    const int32_t cb = g < m->n_cgroup ? m->grp[g].cell_base : m->tgrp[g - m->n_cgroup].cell_base;
+    cell_of_pcell[cb + m->cell_slot[c]] = c;
+  }
   for (int g = 0; g < ng; ++g) {
     const GroupInfo &gi = m->grp[g];
     const HClass &K = m->cls[gi.cls];
@@ -726,13 +1032,12 @@ static int finalize(cn_model *m, double dt) {
     flag[pc] = m->v_init > m->thr[c];
     gid_of[pc] = c;
   }
-  // cai per node
+  // cai per node of the cooperative groups
   std::vector<double> cai;
   if (m->any_cai) {
     cai.assign((size_t)m->n_pnode, 1e-4);
-    for (const HTable &T : m->tab)
-      if (T.type == CN_CADYN)
-        for (int64_t i = 0; i < T.n; ++i) cai[m->node_pos[T.node[i]]] = T.glob[3];
+    for (int64_t i = 0; i < N; ++i)
+      if (!m->cell_tape[cell_of_node[i]]) cai[m->node_pos[i]] = m->cai0[i];
   }
 
   DModel &H = m->hm;
@@ -752,7 +1057,6 @@ static int finalize(cn_model *m, double dt) {
     H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
     int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
     double *p;
-    UP(v0, m->d_v); H.v = m->d_v;
     UP(dstat, p); H.dstat = p;
     UP(rstat, p); H.rstat = p;
     UP(a_s, p); H.a_s = p;
@@ -784,43 +1088,52 @@ static int finalize(cn_model *m, double dt) {
     if (!T.ti.point && T.ti.n_dev_param > 0)
       std::fill(par[T.ti.n_dev_param - 1].begin(), par[T.ti.n_dev_param - 1].end(), 1.0);
     for (int64_t i = 0; i < T.n; ++i) {
-      const int64_t q = T.inst_pos[i];
       const int32_t nd_i = T.node[i];
-      for (int j = 0; j < T.ti.n_param; ++j) par[j][q] = T.param[(size_t)j * T.n + i];
+      double P[CN_MAX_PARAM] = {0.0}, S[CN_MAX_STATE] = {0.0};
+      for (int j = 0; j < T.ti.n_param; ++j) P[j] = T.param[(size_t)j * T.n + i];
       const double scale = 100.0 / m->area[nd_i] * invc[nd_i];
       const double v = m->v_init;
       switch (T.type) {
         case CN_HH: {
-          par[4][q] = invc[nd_i];
+          P[4] = invc[nd_i];
           double al, be;
           al = 0.1 * h_vtrap(-(v + 40.0), 10.0); be = 4.0 * std::exp(-(v + 65.0) / 18.0);
-          st[0][q] = al / (al + be);
+          S[0] = al / (al + be);
           al = 0.07 * std::exp(-(v + 65.0) / 20.0); be = 1.0 / (std::exp(-(v + 35.0) / 10.0) + 1.0);
-          st[1][q] = al / (al + be);
+          S[1] = al / (al + be);
           al = 0.01 * h_vtrap(-(v + 55.0), 10.0); be = 0.125 * std::exp(-(v + 65.0) / 80.0);
-          st[2][q] = al / (al + be);
+          S[2] = al / (al + be);
           break;
         }
-        case CN_EXPSYN: par[2][q] = scale; break;
+        case CN_EXPSYN: P[2] = scale; break;
         case CN_EXP2SYN:
-          par[3][q] = scale;
-          par[4][q] = h_exp2_factor(par[0][q], par[1][q]);
+          P[3] = scale;
+          P[4] = h_exp2_factor(P[0], P[1]);
           break;
-        case CN_ICLAMP: par[3][q] = scale; break;
+        case CN_ICLAMP: P[3] = scale; break;
         case CN_HHFORM:
-          par[1][q] = invc[nd_i];
-          st[0][q] = 1.0 / (1.0 + std::exp((T.glob[4] - v) / T.glob[5]));
-          st[1][q] = 1.0 / (1.0 + std::exp((T.glob[10] - v) / T.glob[11]));
+          P[1] = invc[nd_i];
+          S[0] = 1.0 / (1.0 + std::exp((T.glob[4] - v) / T.glob[5]));
+          S[1] = 1.0 / (1.0 + std::exp((T.glob[10] - v) / T.glob[11]));
           break;
         case CN_SK: {
-          par[1][q] = invc[nd_i];
-          double ca = m->any_cai ? cai[m->node_pos[nd_i]] : 1e-4;
+          P[1] = invc[nd_i];
+          double ca = m->any_cai ? m->cai0[nd_i] : 1e-4;
           if (ca < 1e-9) ca = 1e-9;
-          st[0][q] = 1.0 / (1.0 + std::pow(T.glob[1] / ca, T.glob[2]));
+          S[0] = 1.0 / (1.0 + std::pow(T.glob[1] / ca, T.glob[2]));
           break;
         }
-        case CN_AMPANMDA: par[0][q] = scale; break;
+        case CN_AMPANMDA: P[0] = scale; break;
         default: break;
+      }
+      if (!T.ti.point && T.tape_loc[i] >= 0) {  // the instance lives on a tape
+        double *rec = tape + T.tape_loc[i];
+        for (int j = 0; j < T.ti.n_dev_param; ++j) rec[(size_t)j * 32] = P[j];
+        for (int j = 0; j < T.ti.n_state; ++j) rec[(size_t)(T.ti.n_dev_param + j) * 32] = S[j];
+      } else if (T.inst_pos[i] >= 0) {
+        const int64_t q = T.inst_pos[i];
+        for (int j = 0; j < T.ti.n_dev_param; ++j) par[j][q] = P[j];
+        for (int j = 0; j < T.ti.n_state; ++j) st[j][q] = S[j];
       }
     }
     for (int j = 0; j < T.ti.n_dev_param; ++j) { UP(par[j], T.d_param[j]); D.param[j] = T.d_param[j]; }
@@ -832,6 +1145,32 @@ static int finalize(cn_model *m, double dt) {
       UP(T.cls_cnt, T.d_cls_cnt); UP(T.cls_nodeoff, T.d_cls_nodeoff);
       UP(T.grp_instbase, T.d_grp_instbase);
       D.cls_cnt = T.d_cls_cnt; D.cls_nodeoff = T.d_cls_nodeoff; D.grp_instbase = T.d_grp_instbase;
+    }
+  }
+  // the arena (filled above, including the mechanism rows of the tapes), scratch, programs
+  {
+    UP(v0, m->d_v);
+    H.v = m->d_v;
+    H.tape = m->d_v + m->n_ab;
+    rc = dev_alloc(m, (size_t)std::max<int64_t>(m->n_scratch, 1), &H.scratch, false);
+    if (rc != CN_OK) return rc;
+    std::vector<TapeClass> tcls(m->cls.size());
+    std::vector<uint4> prog;
+    for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+      const HClass &K = m->cls[kc];
+      const HTape &P = K.tp;
+      tcls[kc] = TapeClass{K.n, P.prog_off, P.n_rows, P.n_srows, P.depth, 0, 0, 0};
+      if (P.n_groups == 0) continue;
+      for (int j = 0; j < K.n; ++j) prog.push_back(make_uint4(P.row[j], P.srow[j], P.flags[j], P.mask[j]));
+    }
+    TapeGroup *dtg; TapeClass *dtc; uint4 *dpg;
+    UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg);
+    H.tgrp = dtg; H.tcls = dtc; H.prog = dpg;
+    H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
+    H.tape_stack_cap = std::max(m->tape_stack_cap, 1);
+    for (int t = 0; t < nt; ++t) {
+      H.tab[t].pp_tape_begin = m->tab[t].pp_tape_begin;
+      H.tab[t].pp_tape_end = m->tab[t].ti.point ? m->tab[t].n : 0;
     }
   }
   // PAS tables still need (empty) layout pointers so the kernel's table loop can skip them
@@ -933,10 +1272,36 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
   return cudaGetLastError();
 }
 
+// ring geometry of the tape kernel: S stages of CH rows of 256 B
+#define CN_TAPE_S 8
+#define CN_TAPE_CH 8
+
+static size_t tape_smem_bytes(const cn_model *m) {
+  return (size_t)CN_TAPE_S * CN_TAPE_CH * 256 + (size_t)m->hm.tape_prog_cap * 16 +
+         (size_t)m->hm.tape_stack_cap * 512 + (CN_TAPE_S + 1) * 8;
+}
+
+static cudaError_t launch_tape(cn_model *m, int64_t k) {
+  const size_t smem = tape_smem_bytes(m);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(tape_step_kernel<CN_TAPE_S, CN_TAPE_CH>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  tape_step_kernel<CN_TAPE_S, CN_TAPE_CH><<<m->hm.n_tgroup, 32, smem, m->stream>>>(m->hm, k);
+  return cudaGetLastError();
+}
+
 static int run_steps(cn_model *m, int64_t K) {
-  const int ng = m->hm.n_group;
+  const int ng = m->hm.n_group, ntg = m->hm.n_tgroup;
   int deliver_blocks = 8;
   if (m->n_netcon > 1000000) deliver_blocks = 148;
+  int64_t pp_tape = 0;
+  for (const HTable &T : m->tab)
+    if (T.ti.point) pp_tape = std::max(pp_tape, T.n - T.pp_tape_begin);
+  const int pp_blocks = (int)std::min<int64_t>((pp_tape + 255) / 256, 148 * 8);
   CU(cudaEventRecord(m->ev0, m->stream));
   for (int64_t s = 0; s < K; ++s) {
     const int64_t k = m->k + s;
@@ -944,11 +1309,16 @@ static int run_steps(cn_model *m, int64_t K) {
       deliver_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->hm, k);
       m->launches++;
     }
+    if (ntg > 0 && pp_tape > 0) {
+      pp_tape_kernel<<<pp_blocks, 256, 0, m->stream>>>(m->hm, k);
+      m->launches++;
+    }
+    const bool timeit = m->ktime_every > 0 && (k % m->ktime_every) == 0 &&
+                        m->ktime_used < m->ktime_ev.size();
+    const bool time_tape = ntg > 0;  // the dominant kernel is the tape kernel when it runs
     if (ng > 0) {
       cudaError_t e;
-      const bool timeit = m->ktime_every > 0 && (k % m->ktime_every) == 0 &&
-                          m->ktime_used < m->ktime_ev.size();
-      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
+      if (timeit && !time_tape) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
       switch (m->wpb) {
         case 8: e = launch_step<8>(m, k); break;
         case 4: e = launch_step<4>(m, k); break;
@@ -956,6 +1326,13 @@ static int run_steps(cn_model *m, int64_t K) {
         default: e = launch_step<1>(m, k); break;
       }
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "step launch failed: %s", cudaGetErrorString(e));
+      if (timeit && !time_tape) cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+      m->launches++;
+    }
+    if (ntg > 0) {
+      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
+      cudaError_t e = launch_tape(m, k);
+      if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
       if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
       m->launches++;
     }
@@ -1090,10 +1467,29 @@ extern "C" int cn_get_state(const cn_model *cm, int32_t t, int32_t s, double *ou
   HTable &T = m->tab[t];
   if (s < 0 || s >= T.ti.n_state || n != T.n) return fail(CN_ERR_MECH, "state / size mismatch");
   if (!m->uploaded) return fail(CN_ERR_ARG, "states exist after the first cn_run");
-  CU(cudaStreamSynchronize(m->stream));
-  std::vector<double> h((size_t)std::max<int64_t>(T.n_dev, 1));
-  CU(cudaMemcpy(h.data(), T.d_state[s], (size_t)T.n_dev * sizeof(double), cudaMemcpyDeviceToHost));
-  for (int64_t i = 0; i < n; ++i) out[i] = h[T.inst_pos[i]];
+  if (n == 0) return CN_OK;
+  // instances live in the table arrays (cooperative groups) or on a tape (interleaved groups)
+  std::vector<int64_t> loc((size_t)n);
+  for (int64_t i = 0; i < n; ++i) {
+    const bool on_tape = !T.ti.point && T.tape_loc[i] >= 0;
+    loc[i] = on_tape ? -(T.tape_loc[i] + (int64_t)T.ti.n_dev_param * 32 + 1) : T.inst_pos[i];
+  }
+  int64_t *d_loc = nullptr;
+  double *d_out = nullptr;
+  CU(cudaMalloc(&d_loc, (size_t)n * sizeof(int64_t)));
+  if (cudaMalloc(&d_out, (size_t)n * sizeof(double)) != cudaSuccess) {
+    cudaFree(d_loc);
+    return fail(CN_ERR_NOMEM, "out of device memory");
+  }
+  cudaMemcpyAsync(d_loc, loc.data(), (size_t)n * sizeof(int64_t), cudaMemcpyHostToDevice, m->stream);
+  gather_state_kernel<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(
+      m->hm.tape, T.d_state[s], d_loc, n, s, d_out);
+  m->launches++;
+  cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, m->stream);
+  cudaError_t e = cudaStreamSynchronize(m->stream);
+  cudaFree(d_loc);
+  cudaFree(d_out);
+  if (e != cudaSuccess) return fail(CN_ERR_CUDA, "cn_get_state: %s", cudaGetErrorString(e));
   return CN_OK;
 }
 
@@ -1113,11 +1509,15 @@ extern "C" int cn_last_run_ms(const cn_model *m, double *ms) {
 extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
   if (!m || !info) return fail(CN_ERR_ARG, "NULL argument");
   info[0] = (int64_t)m->cls.size();
-  info[1] = (int64_t)m->grp.size();
+  info[1] = (int64_t)m->grp.size() + (int64_t)m->tgrp.size();
   info[2] = (int64_t)m->warp_smem_doubles * 8;
   int r = 0;
   for (const HClass &K : m->cls) r = std::max(r, K.rounds);
   info[3] = r;
+  info[4] = (int64_t)m->tgrp.size();
+  info[5] = m->n_tape * 8;
+  info[6] = m->n_scratch * 8;
+  info[7] = m->tape_stack_cap;
   return CN_OK;
 }
 

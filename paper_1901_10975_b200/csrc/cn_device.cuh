@@ -31,6 +31,7 @@ enum { T_PAS = 1, T_HH = 2, T_EXPSYN = 3, T_EXP2SYN = 4, T_ICLAMP = 5, T_HHFORM 
 
 struct DTable {
   int type, is_point, n_param, n_state;
+  int64_t pp_tape_begin, pp_tape_end;  // point tables: instance range that sits on tape groups
   double *param[CN_MAX_PARAM];   // permuted SoA, incl. derived per-instance constants (see host)
   double *state[CN_MAX_STATE];
   double glob[CN_MAX_GLOBAL];
@@ -54,8 +55,31 @@ struct ClassInfo {
   int32_t sched_off, needs_ica, nodeoff_off, pad1;
 };
 
+// ---- interleaved ("tape") groups: 32 same-shape cells, one lane per cell (cn_tape.cuh) ----------
+struct TapeGroup {
+  int64_t tape_base;     // first element of the group's tape (multiple of 32 doubles)
+  int64_t scratch_base;  // first element of the group's scratch tape
+  int32_t cls, cell_base, ncell, pad;
+};
+
+struct TapeClass {
+  int32_t n, prog_off, n_rows, n_srows;
+  int32_t depth, pad0, pad1, pad2;
+};
+
+// program entry flags (uint4: x = first tape row, y = first scratch row (reversed order),
+// z = flags | rows << 8 | scratch rows << 16, w = mask of distributed tables on this node)
+enum { PG_FWD = 1, PG_PUSH = 2, PG_ADD = 3, PG_KIND = 3, PG_FWD_IN = 4, PG_POP = 8, PG_ROOT = 16,
+       PG_HAS_PP = 32, PG_HAS_CAI = 64, PG_NEED_ICA = 128 };
+
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
+  int32_t n_tgroup, tape_prog_cap, tape_stack_cap, pad_t;
+  const TapeGroup *tgrp;
+  const TapeClass *tcls;
+  const uint4 *prog;
+  double *tape;                 // == v + n_ab: one arena, so node positions index both
+  double *scratch;
   const GroupInfo *grp;
   const ClassInfo *cls;
   const uint32_t *sched;        // per class: rounds * P entries, node | parent << 16

@@ -26,6 +26,18 @@ def cn():
     return cn
 
 
+@pytest.fixture(params=["coop", "tape"])
+def strategy(request, monkeypatch):
+    """Both kernels on the same inputs: warp-cooperative groups, or every cell on the interleaved
+    (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1)."""
+    if request.param == "tape":
+        monkeypatch.setenv("CN_TAPE", "1")
+        monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+    else:
+        monkeypatch.setenv("CN_TAPE", "0")
+    return request.param
+
+
 def run_both(cn, desc, tstop, dt=DT, probes=None, chunks=1, env=None):
     from oracle import OracleModel
     nsteps = int(round(tstop / dt))
@@ -56,7 +68,7 @@ def check(o, g, tol=TOL, min_spikes=0):
     return err_t, err_v
 
 
-def test_config1_full(cn):
+def test_config1_full(cn, strategy):
     desc = W.config1()
     probes = np.concatenate([desc["cell_first"][:-1], [30, 60, 100, 487]]).astype(np.int32)
     o, g = run_both(cn, desc, 100.0, probes=probes)
@@ -65,41 +77,54 @@ def test_config1_full(cn):
         assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9
 
 
-def test_unique_topologies_one_cell_per_warp(cn):
+def test_unique_topologies_one_cell_per_warp(cn, strategy):
     desc = W.random_tree_cells(13, 5, 120, stream="gpu-u", weight=0.2, amp=2.0)
     o, g = run_both(cn, desc, 40.0)
     assert g.layout_info()["n_class"] == 13
+    assert g.layout_info()["n_tape_group"] == (13 if strategy == "tape" else 0)
     check(o, g, min_spikes=5)
 
 
-def test_identical_random_cells_grouped(cn):
+def test_identical_random_cells_grouped(cn, strategy):
     desc = W.random_tree_cells(11, 77, 77, stream="gpu-i", identical=True, weight=0.2, amp=2.0)
     o, g = run_both(cn, desc, 40.0)
     info = g.layout_info()
-    assert info["n_class"] == 1 and info["n_group"] == 3   # 4 + 4 + 3 (ragged tail group)
+    # coop: 4 + 4 + 3 (ragged tail group); tape: one ragged group of 11 lanes
+    assert info["n_class"] == 1 and info["n_group"] == (3 if strategy == "coop" else 1)
     check(o, g, min_spikes=5)
 
 
-def test_hh_everywhere_config2_shape(cn):
+def test_hh_everywhere_config2_shape(cn, strategy):
     desc = W.config2(n_cell=8, ring_size=4, weight=0.05)
     o, g = run_both(cn, desc, 30.0)
     check(o, g, min_spikes=4)
 
 
-def test_config2_one_ring_of_64(cn):
+def test_config2_one_ring_of_64(cn, strategy):
     desc = W.config2(rings=[1])
     o, g = run_both(cn, desc, 12.0)
     check(o, g, min_spikes=3)
 
 
-def test_config4_small_full_length(cn):
+def test_config4_small_full_length(cn, strategy):
     desc = W.config4(n_cell=256, n_types=8)
     o, g = run_both(cn, desc, 50.0)
     assert g.layout_info()["n_class"] == 8
+    assert g.layout_info()["n_tape_group"] == (8 if strategy == "tape" else 0)
     check(o, g, min_spikes=100)
 
 
-def test_chunked_run_equals_one_shot(cn):
+def test_mixed_strategies_in_one_model(cn, monkeypatch):
+    """Classes of 40 cells: 32 go to one tape group, the ragged 8 to warp-cooperative groups."""
+    monkeypatch.setenv("CN_TAPE", "1")
+    desc = W.config4(n_cell=320, n_types=8, ring_size=64)
+    o, g = run_both(cn, desc, 30.0)
+    info = g.layout_info()
+    assert info["n_tape_group"] == 8 and info["n_group"] == 8 + 8 * 2
+    check(o, g, min_spikes=50)
+
+
+def test_chunked_run_equals_one_shot(cn, strategy):
     desc = W.config1()
     a = cn.Model(desc)
     a.run(20.0, DT)
@@ -111,7 +136,7 @@ def test_chunked_run_equals_one_shot(cn):
     assert [list(x) for x in a.get_spikes()] == [list(x) for x in b.get_spikes()]
 
 
-def test_run_is_deterministic(cn):
+def test_run_is_deterministic(cn, strategy):
     desc = W.config4(n_cell=128, n_types=4)
     r = []
     for _ in range(2):
@@ -122,7 +147,7 @@ def test_run_is_deterministic(cn):
     assert [list(x) for x in r[0][1]] == [list(x) for x in r[1][1]]
 
 
-def test_edge_cases(cn):
+def test_edge_cases(cn, strategy):
     from oracle import OracleModel
     # empty model
     empty = {"cell_first": np.zeros(1, np.int64), "parent": np.zeros(0, np.int32),
@@ -163,7 +188,7 @@ def test_edge_cases(cn):
     assert e.value.code == -7
 
 
-def test_scripted_sources_and_delays(cn):
+def test_scripted_sources_and_delays(cn, strategy):
     from tests.test_oracle_pins import _syn_target
     for ks in (0, 7):
         d = _syn_target([1 * DT, 40 * DT, 400 * DT], ks * DT)
@@ -172,7 +197,7 @@ def test_scripted_sources_and_delays(cn):
         assert np.max(np.abs(o.get_state(1, 0) - g.get_state(1, 0))) < 1e-15
 
 
-def test_node_renumbering_invariance(cn):
+def test_node_renumbering_invariance(cn, strategy):
     desc = W.random_tree_cells(4, 30, 60, stream="gpu-r", weight=0.4, amp=4.0)
     ren = W.renumber_nodes(desc)
     a, b = cn.Model(desc), cn.Model(ren)
