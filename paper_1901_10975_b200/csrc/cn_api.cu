@@ -18,6 +18,10 @@
 
 using namespace cn;
 
+// ring geometry of the tape kernel: S stages of CH rows of 256 B
+#define CN_TAPE_S 8
+#define CN_TAPE_CH 8
+
 // ---------------------------------------------------------------------------------------------
 // errors
 // ---------------------------------------------------------------------------------------------
@@ -518,11 +522,14 @@ static int build_tape_program(cn_model *m, HClass &K) {
         sl += (uint32_t)T.ti.n_state;
       }
     const uint32_t len = r - row;
-    if (len > 255 || sl > 255)
-      return fail(CN_ERR_UNSUPPORTED, "too many mechanism rows on one node for the tape kernel");
+    if (len > (CN_TAPE_S - 1) * CN_TAPE_CH || sl > (CN_TAPE_S - 1) * CN_TAPE_CH) {
+      P.n_groups = 0;  // a record must fit the ring: this class stays on the cooperative kernel
+      P.n_cells = 0;
+      return CN_OK;
+    }
     max_len = std::max(max_len, (int)std::max(len, sl));
     P.row[j] = row;
-    P.flags[j] = fl | (len << 8) | (sl << 16);
+    P.flags[j] = fl | (len << 24);
     P.mask[j] = node_mask[x];
     slen[j] = sl;
     row = r;
@@ -534,6 +541,27 @@ static int build_tape_program(cn_model *m, HClass &K) {
     srow += slen[j];
   }
   P.n_srows = (int)srow;
+  // chunk bookkeeping of the ring, precomputed: how many chunks a node must wait for before its
+  // rows are complete and how many are fully consumed after it, in both directions
+  {
+    const int CH = CN_TAPE_CH;
+    int last = -1, next = 0;
+    for (int j = 0; j < n; ++j) {
+      const uint32_t len = P.flags[j] >> 24;
+      const int cl = (int)((P.row[j] + len - 1) / CH), cn = (int)((P.row[j] + len) / CH);
+      P.flags[j] |= (uint32_t)(cl - last) << 8 | (uint32_t)(cn - next) << 12;
+      last = cl;
+      next = cn;
+    }
+    last = -1;
+    next = 0;
+    for (int j = n - 1; j >= 0; --j) {
+      const int cl = (int)((P.srow[j] + slen[j] - 1) / CH), cn = (int)((P.srow[j] + slen[j]) / CH);
+      P.flags[j] |= (uint32_t)(cl - last) << 16 | (uint32_t)(cn - next) << 20;
+      last = cl;
+      next = cn;
+    }
+  }
   // stack depth by simulation of the forward pass
   int sp = 0, depth = 0;
   for (int j = 0; j < n; ++j) {
@@ -663,17 +691,16 @@ static int build_layout(cn_model *m) {
     const int64_t full = K.count / 32, rem = K.count % 32;
     K.tp.n_groups = (int)(full + (rem >= tape_min_group ? 1 : 0));
     K.tp.n_cells = std::min<int64_t>(K.count, (int64_t)K.tp.n_groups * 32);
-    for (int64_t q = 0; q < K.tp.n_cells; ++q) m->cell_tape[K.cells[q]] = 1;
-  }
-  // point processes on tape cells mark their local node in the class
-  for (HClass &K : m->cls)
     if (K.tp.n_groups > 0) K.tp.has_pp.assign(K.n, 0);
+  }
+  // a point process on any cell of the class marks its local node (two dynamic rows there)
   for (int t = 0; t < nt; ++t) {
     const HTable &T = m->tab[t];
     if (!T.ti.point) continue;
     for (int64_t i = 0; i < T.n; ++i) {
       const int32_t c = cell_of[T.node[i]];
-      if (m->cell_tape[c]) m->cls[m->cell_cls[c]].tp.has_pp[T.node[i] - m->cell_first[c]] = 1;
+      HTape &P = m->cls[m->cell_cls[c]].tp;
+      if (P.n_groups > 0) P.has_pp[T.node[i] - m->cell_first[c]] = 1;
     }
   }
   int prog_total = 0;
@@ -681,6 +708,8 @@ static int build_layout(cn_model *m) {
     if (K.tp.n_groups == 0) continue;
     int rc = build_tape_program(m, K);
     if (rc != CN_OK) return rc;
+    if (K.tp.n_groups == 0) continue;
+    for (int64_t q = 0; q < K.tp.n_cells; ++q) m->cell_tape[K.cells[q]] = 1;
     K.tp.prog_off = prog_total;
     prog_total += K.n;
     m->tape_prog_cap = std::max(m->tape_prog_cap, K.n);
@@ -1161,7 +1190,10 @@ static int finalize(cn_model *m, double dt) {
       const HTape &P = K.tp;
       tcls[kc] = TapeClass{K.n, P.prog_off, P.n_rows, P.n_srows, P.depth, 0, 0, 0};
       if (P.n_groups == 0) continue;
-      for (int j = 0; j < K.n; ++j) prog.push_back(make_uint4(P.row[j], P.srow[j], P.flags[j], P.mask[j]));
+      const uint32_t R = CN_TAPE_S * CN_TAPE_CH;
+      for (int j = 0; j < K.n; ++j)
+        prog.push_back(make_uint4((P.row[j] % R) * 256u | ((P.srow[j] % R) * 256u) << 16,
+                                  P.srow[j] * 32u, P.flags[j], P.mask[j]));
     }
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg;
     UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg);
@@ -1271,10 +1303,6 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
   step_kernel<WPB><<<(ng + WPB - 1) / WPB, WPB * 32, smem, m->stream>>>(m->hm, k);
   return cudaGetLastError();
 }
-
-// ring geometry of the tape kernel: S stages of CH rows of 256 B
-#define CN_TAPE_S 8
-#define CN_TAPE_CH 8
 
 static size_t tape_smem_bytes(const cn_model *m) {
   return (size_t)CN_TAPE_S * CN_TAPE_CH * 256 + (size_t)m->hm.tape_prog_cap * 16 +

@@ -56,35 +56,88 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       : "memory");
 }
 
+// Reciprocal to ~1 ulp without the special-case handling of an IEEE division: MUFU.RCP64H seed
+// plus two Newton steps.  Every argument here is a positive, finite, O(1)..O(1e3) quantity
+// (pivots of a diagonally dominant row-normalised matrix, sums of rate constants).
+__device__ __forceinline__ double rcp_fast(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+
+// x / (exp(x/y) - 1) for y = 10 (both HH uses), removable singularity as in vtrap()
+__device__ __forceinline__ double vtrap10(double x) {
+  const double u = x * 0.1;
+  if (fabs(u) < 1e-6) return 10.0 * (1.0 - 0.5 * u);
+  return x * rcp_fast(exp(u) - 1.0);
+}
+
+// HH gates advanced over dt with cnexp at the new v: y += (1 - exp(-dt*q10*(a+b))) * (a/(a+b) - y).
+// Same formulas as hh_rates() + cnexp(); divisions by constants are multiplications by their
+// reciprocals and 1/tau is never formed (differences of a few ulp).
+__device__ __forceinline__ void hh_advance(double v, double q10dt, double &m, double &h,
+                                           double &n) {
+  double al, be, s;
+  al = 0.1 * vtrap10(-(v + 40.0));
+  be = 4.0 * exp(-(v + 65.0) * (1.0 / 18.0));
+  s = al + be;
+  m += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - m);
+  al = 0.07 * exp(-(v + 65.0) * 0.05);
+  be = rcp_fast(exp(-(v + 35.0) * 0.1) + 1.0);
+  s = al + be;
+  h += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - h);
+  al = 0.01 * vtrap10(-(v + 55.0));
+  be = 0.125 * exp(-(v + 65.0) * 0.0125);
+  s = al + be;
+  n += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - n);
+}
+
 // S stages of CH rows; S * CH must be a power of two.
+//
+// Program entry (uint4, one per node in elimination order; built by the host, uniform per class):
+//   x = byte offset in the ring of the node's first tape row (low 16 bits) and of its first
+//       scratch row (high 16 bits)
+//   y = element offset of the node's scratch record on the group's scratch tape
+//   z = flags (8 bits) | chunks to wait for, forward (4) | chunks freed, forward (4)
+//       | chunks to wait for, backward (4) | chunks freed, backward (4) | tape rows (8)
+//   w = mask of the distributed mechanism tables with an instance on this node
 template <int S, int CH>
 __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ DModel M,
                                                        int64_t k) {
   extern __shared__ __align__(128) unsigned char sm_raw[];
-  constexpr int RING_ROWS = S * CH;
-  static_assert((RING_ROWS & (RING_ROWS - 1)) == 0, "ring rows must be a power of two");
+  constexpr uint32_t RB = S * CH * 256u;  // ring bytes
+  static_assert((RB & (RB - 1)) == 0 && RB <= 65536u, "ring must be a power of two <= 64 KB");
+  static_assert((S & (S - 1)) == 0, "stages must be a power of two");
   const int lane = threadIdx.x;
+  const uint32_t lane8 = (uint32_t)lane * 8u;
   const TapeGroup tg = M.tgrp[blockIdx.x];
   const TapeClass tc = M.tcls[tg.cls];
-  double *ring = reinterpret_cast<double *>(sm_raw);
-  uint4 *prog = reinterpret_cast<uint4 *>(ring + RING_ROWS * 32);
+  const unsigned char *ringc = sm_raw;
+  uint4 *prog = reinterpret_cast<uint4 *>(sm_raw + RB);
   double *stk = reinterpret_cast<double *>(prog + M.tape_prog_cap);
   uint64_t *mbar = reinterpret_cast<uint64_t *>(stk + M.tape_stack_cap * 64);
-  const uint32_t ring_s = smem_u32(ring), bar_s = smem_u32(mbar);
+  const uint32_t ring_s = smem_u32(sm_raw), bar_s = smem_u32(mbar);
   double *__restrict__ tape = M.tape + tg.tape_base;
   double *__restrict__ scr = M.scratch + tg.scratch_base;
+  double *__restrict__ tape_l = tape + lane;
+  double *__restrict__ scr_l = scr + lane;
   const int n = tc.n;
   const int nchunk = (tc.n_rows + CH - 1) / CH;
   const int nsch = (tc.n_srows + CH - 1) / CH;
   const double dt = M.dt;
+  const double q10dt = M.q10 * dt;
 
-#define CN_ROW(r) ring[((((uint32_t)(r)) & (RING_ROWS - 1)) << 5) + lane]
+#define CN_RD(base, i) \
+  (*reinterpret_cast<const double *>(ringc + (((base) + (uint32_t)(i) * 256u) & (RB - 1u))))
 
   // chunk c of a row stream goes to stage c % S
   auto issue = [&](const double *base, int c, int total_rows) {
     const int rows = min(CH, total_rows - c * CH);
     const uint32_t bytes = (uint32_t)rows * 256u;
-    const int s = c % S;
+    const int s = c & (S - 1);
     mbar_expect_tx(bar_s + 8 * s, bytes);
     bulk_g2s(ring_s + (uint32_t)s * (CH * 256), base + (size_t)c * (CH * 32), bytes,
              bar_s + 8 * s);
@@ -101,23 +154,31 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
   __syncwarp();
   mbar_wait(bar_s + 8 * S, 0);
 
+  uint32_t phase = 0;  // bit s: parity the next wait on stage s looks for
+  uint32_t ws = 0;     // stage of the next chunk to wait for
+  int ci = S;          // next chunk to issue
+
   // ------------------------------------------------------------------------------------------
   // forward: nrn_cur + tree terms + triangularisation, children before parents
   // ------------------------------------------------------------------------------------------
-  int c_wait = -1, c_free = 0, sp = 0;
-  double accD = 0.0, accR = 0.0, v_root = 0.0;
+  int sp = 0;
+  uint32_t grow = 0;  // element offset of the current node's record on the group's tape
+  double accD = 0.0, accR = 0.0;
   for (int j = 0; j < n; ++j) {
     const uint4 e = prog[j];
-    const uint32_t row = e.x, sr = e.y, fl = e.z, len = (e.z >> 8) & 0xFFu;
-    const int c_last = (int)((row + len - 1) / CH);
-    while (c_wait < c_last) {
-      ++c_wait;
-      mbar_wait(bar_s + 8 * (c_wait % S), (uint32_t)(c_wait / S) & 1u);
+    const uint32_t fl = e.z;
+    for (uint32_t nw = (fl >> 8) & 15u; nw; --nw) {
+      mbar_wait(bar_s + 8 * ws, (phase >> ws) & 1u);
+      phase ^= 1u << ws;
+      ws = (ws + 1) & (S - 1);
     }
-    const double a = CN_ROW(row), b = CN_ROW(row + 1);
-    const double v_old = CN_ROW(row + 4);
-    double D = CN_ROW(row + 2), R = v_old + CN_ROW(row + 3);
-    uint32_t cur = row + 5, scur = sr + 2;
+    const uint32_t rb = (e.x & 0xFFFFu) + lane8;
+    double *__restrict__ srec = scr_l + e.y;
+    double *__restrict__ trec = tape_l + grow;
+    const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
+    const double v_old = CN_RD(rb, 4);
+    double D = CN_RD(rb, 2), R = v_old + CN_RD(rb, 3);
+    uint32_t cur = 5, scur = 2;
     if (fl & PG_FWD_IN) {
       D += accD;
       R += accR;
@@ -128,19 +189,19 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
       R += stk[sp * 64 + 32 + lane];
     }
     if (fl & PG_HAS_PP) {  // conductance / current of the point processes (pp_tape_kernel)
-      const double pd = CN_ROW(cur), pr = CN_ROW(cur + 1);
+      const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
       D += pd;
       R += pr;
       if (pd != 0.0 || pr != 0.0) {
-        tape[(size_t)cur * 32 + lane] = 0.0;
-        tape[(size_t)(cur + 1) * 32 + lane] = 0.0;
+        trec[5 * 32] = 0.0;
+        trec[6 * 32] = 0.0;
       }
-      cur += 2;
+      cur = 7;
     }
     double ica = 0.0;
     if (fl & PG_NEED_ICA) ++scur;
     if (fl & PG_HAS_CAI) {
-      scr[(size_t)scur * 32 + lane] = CN_ROW(cur);
+      srec[scur * 32] = CN_RD(rb, cur);
       ++cur;
       ++scur;
     }
@@ -148,41 +209,41 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
       const DTable &T = M.tab[__ffs(mk) - 1];
       switch (T.type) {
         case T_HH: {
-          const double m = CN_ROW(cur + 5), h = CN_ROW(cur + 6), nn = CN_ROW(cur + 7);
-          const double invc = CN_ROW(cur + 4);
-          const double gna = CN_ROW(cur) * m * m * m * h;
+          const double m = CN_RD(rb, cur + 5), h = CN_RD(rb, cur + 6), nn = CN_RD(rb, cur + 7);
+          const double invc = CN_RD(rb, cur + 4);
+          const double gna = CN_RD(rb, cur) * m * m * m * h;
           const double n2 = nn * nn;
-          const double gk = CN_ROW(cur + 1) * n2 * n2;
-          const double gl = CN_ROW(cur + 2);
+          const double gk = CN_RD(rb, cur + 1) * n2 * n2;
+          const double gl = CN_RD(rb, cur + 2);
           D += (gna + gk + gl) * invc;
-          R += (gna * T.glob[0] + gk * T.glob[1] + gl * CN_ROW(cur + 3)) * invc;
-          scr[(size_t)scur * 32 + lane] = m;
-          scr[(size_t)(scur + 1) * 32 + lane] = h;
-          scr[(size_t)(scur + 2) * 32 + lane] = nn;
+          R += (gna * T.glob[0] + gk * T.glob[1] + gl * CN_RD(rb, cur + 3)) * invc;
+          srec[scur * 32] = m;
+          srec[(scur + 1) * 32] = h;
+          srec[(scur + 2) * 32] = nn;
           cur += 8;
           scur += 3;
           break;
         }
         case T_HHFORM: {
-          const double ms = CN_ROW(cur + 2), hs = CN_ROW(cur + 3);
-          const double g = CN_ROW(cur) * ipow(ms, (int)T.glob[0]) * ipow(hs, (int)T.glob[1]);
-          const double invc = CN_ROW(cur + 1);
+          const double ms = CN_RD(rb, cur + 2), hs = CN_RD(rb, cur + 3);
+          const double g = CN_RD(rb, cur) * ipow(ms, (int)T.glob[0]) * ipow(hs, (int)T.glob[1]);
+          const double invc = CN_RD(rb, cur + 1);
           D += g * invc;
           R += g * T.glob[2] * invc;
           if (T.glob[3] != 0.0) ica += g * (v_old - T.glob[2]);
-          scr[(size_t)scur * 32 + lane] = ms;
-          scr[(size_t)(scur + 1) * 32 + lane] = hs;
+          srec[scur * 32] = ms;
+          srec[(scur + 1) * 32] = hs;
           cur += 4;
           scur += 2;
           break;
         }
         case T_SK: {
-          const double z = CN_ROW(cur + 2);
-          const double g = CN_ROW(cur) * z;
-          const double invc = CN_ROW(cur + 1);
+          const double z = CN_RD(rb, cur + 2);
+          const double g = CN_RD(rb, cur) * z;
+          const double invc = CN_RD(rb, cur + 1);
           D += g * invc;
           R += g * T.glob[0] * invc;
-          scr[(size_t)scur * 32 + lane] = z;
+          srec[scur * 32] = z;
           cur += 3;
           scur += 1;
           break;
@@ -190,17 +251,14 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
         default: break;  // PAS is folded into the static rows; CADYN carries no current
       }
     }
-    if (fl & PG_NEED_ICA) scr[(size_t)(sr + 2) * 32 + lane] = ica;
-    double mult = 0.0, rp;
-    if (fl & PG_ROOT) {
-      rp = R / D;
-      v_root = rp;
-    } else {
-      const double rinv = 1.0 / D;
+    if (fl & PG_NEED_ICA) srec[2 * 32] = ica;
+    const double rinv = rcp_fast(D);
+    const double rp = R * rinv;
+    double mult = 0.0;
+    if (!(fl & PG_ROOT)) {
       const double f = a * rinv;
       const double cD = -(f * b), cR = -(f * R);
       mult = b * rinv;  // back-substitution multiplier
-      rp = R * rinv;
       const uint32_t kind = fl & PG_KIND;
       if (kind == PG_FWD) {
         accD = cD;
@@ -214,16 +272,17 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
         stk[(sp - 1) * 64 + 32 + lane] += cR;
       }
     }
-    scr[(size_t)sr * 32 + lane] = mult;
-    scr[(size_t)(sr + 1) * 32 + lane] = rp;
+    srec[0] = mult;
+    srec[32] = rp;
+    grow += (fl >> 24) * 32u;
     // stages whose rows are all consumed are refilled S chunks ahead
-    const int c_next = (int)((row + len) / CH);
-    if (c_free < c_next) {
+    uint32_t nf = (fl >> 12) & 15u;
+    if (nf) {
       __syncwarp();
       if (lane == 0)
-        for (int c = c_free; c < c_next; ++c)
-          if (c + S < nchunk) issue(tape, c + S, tc.n_rows);
-      c_free = c_next;
+        for (; nf; --nf, ++ci)
+          if (ci < nchunk) issue(tape, ci, tc.n_rows);
+      ci = __shfl_sync(0xffffffffu, ci, 0);
     }
   }
 
@@ -234,45 +293,46 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
   __syncwarp();
   if (lane == 0)
     for (int c = 0; c < S && c < nsch; ++c) issue(scr, c, tc.n_srows);
-  int b_wait = -1, b_free = 0;
+  ws = 0;
+  ci = S;
   double v_prev = 0.0;
   sp = 0;
   for (int j = n - 1; j >= 0; --j) {
     const uint4 e = prog[j];
-    const uint32_t row = e.x, sr = e.y, fl = e.z, slen = (e.z >> 16) & 0xFFu;
-    const int c_last = (int)((sr + slen - 1) / CH);
-    while (b_wait < c_last) {
-      ++b_wait;
-      const int s = b_wait % S;
-      const int used = (nchunk > s ? (nchunk - s + S - 1) / S : 0) + b_wait / S;
-      mbar_wait(bar_s + 8 * s, (uint32_t)used & 1u);
+    const uint32_t fl = e.z;
+    grow -= (fl >> 24) * 32u;
+    for (uint32_t nw = (fl >> 16) & 15u; nw; --nw) {
+      mbar_wait(bar_s + 8 * ws, (phase >> ws) & 1u);
+      phase ^= 1u << ws;
+      ws = (ws + 1) & (S - 1);
     }
+    const uint32_t sb = (e.x >> 16) + lane8;
+    double *__restrict__ trec = tape_l + grow;
     const uint32_t kind = fl & PG_KIND;
     double vp = v_prev;
     if (kind == PG_ADD) vp = stk[(sp - 1) * 32 + lane];
     if (kind == PG_PUSH) vp = stk[(--sp) * 32 + lane];
-    double v = CN_ROW(sr + 1);
-    if (!(fl & PG_ROOT)) v -= CN_ROW(sr) * vp;
+    const double v = fma(-CN_RD(sb, 0), vp, CN_RD(sb, 1));  // the root's multiplier is 0
     if (fl & PG_POP) stk[(sp++) * 32 + lane] = v;
     v_prev = v;
-    tape[(size_t)(row + 4) * 32 + lane] = v;
-    uint32_t cur = row + 5 + ((fl & PG_HAS_PP) ? 2u : 0u), scur = sr + 2;
+    trec[4 * 32] = v;
+    uint32_t cur = 5 + ((fl & PG_HAS_PP) ? 2u : 0u), scur = 2;
     double ica = 0.0, cai = 0.0;
     uint32_t cai_row = 0;
-    if (fl & PG_NEED_ICA) ica = CN_ROW(scur++);
+    if (fl & PG_NEED_ICA) ica = CN_RD(sb, scur++);
     if (fl & PG_HAS_CAI) {
-      cai = CN_ROW(scur++);
+      cai = CN_RD(sb, scur++);
       cai_row = cur++;
     }
     for (uint32_t mk = e.w; mk; mk &= mk - 1) {
       const DTable &T = M.tab[__ffs(mk) - 1];
       switch (T.type) {
         case T_HH: {
-          double minf, mtau, hinf, htau, ninf, ntau;
-          hh_rates(v, M.q10, minf, mtau, hinf, htau, ninf, ntau);
-          tape[(size_t)(cur + 5) * 32 + lane] = cnexp(CN_ROW(scur), minf, mtau, dt);
-          tape[(size_t)(cur + 6) * 32 + lane] = cnexp(CN_ROW(scur + 1), hinf, htau, dt);
-          tape[(size_t)(cur + 7) * 32 + lane] = cnexp(CN_ROW(scur + 2), ninf, ntau, dt);
+          double m = CN_RD(sb, scur), h = CN_RD(sb, scur + 1), nn = CN_RD(sb, scur + 2);
+          hh_advance(v, q10dt, m, h, nn);
+          trec[(cur + 5) * 32] = m;
+          trec[(cur + 6) * 32] = h;
+          trec[(cur + 7) * 32] = nn;
           cur += 8;
           scur += 3;
           break;
@@ -281,11 +341,11 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
           double xinf, xtau;
           if ((int)T.glob[0] > 0) {
             hhform_gate(v, T.glob + 4, xinf, xtau);
-            tape[(size_t)(cur + 2) * 32 + lane] = cnexp(CN_ROW(scur), xinf, xtau, dt);
+            trec[(cur + 2) * 32] = cnexp(CN_RD(sb, scur), xinf, xtau, dt);
           }
           if ((int)T.glob[1] > 0) {
             hhform_gate(v, T.glob + 10, xinf, xtau);
-            tape[(size_t)(cur + 3) * 32 + lane] = cnexp(CN_ROW(scur + 1), xinf, xtau, dt);
+            trec[(cur + 3) * 32] = cnexp(CN_RD(sb, scur + 1), xinf, xtau, dt);
           }
           cur += 4;
           scur += 2;
@@ -294,7 +354,7 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
         case T_SK: {
           const double ca = cai < 1e-9 ? 1e-9 : cai;
           const double zinf = 1.0 / (1.0 + pow(T.glob[1] / ca, T.glob[2]));
-          tape[(size_t)(cur + 2) * 32 + lane] = cnexp(CN_ROW(scur), zinf, T.glob[3], dt);
+          trec[(cur + 2) * 32] = cnexp(CN_RD(sb, scur), zinf, T.glob[3], dt);
           cur += 3;
           scur += 1;
           break;
@@ -303,7 +363,7 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
           // derivimplicit on a linear ODE: one Newton step of backward Euler is exact (L278)
           const double kappa = 1e4 * T.glob[0] / (2.0 * 96485.33212 * T.glob[1]);
           cai = (cai + dt * (-kappa * ica + T.glob[3] / T.glob[2])) / (1.0 + dt / T.glob[2]);
-          tape[(size_t)cai_row * 32 + lane] = cai;
+          trec[cai_row * 32] = cai;
           break;
         }
         default: break;
@@ -334,17 +394,16 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
         }
       }
     }
-    const int c_next = (int)((sr + slen) / CH);
-    if (b_free < c_next) {
+    uint32_t nf = (fl >> 20) & 15u;
+    if (nf) {
       __syncwarp();
       if (lane == 0)
-        for (int c = b_free; c < c_next; ++c)
-          if (c + S < nsch) issue(scr, c + S, tc.n_srows);
-      b_free = c_next;
+        for (; nf; --nf, ++ci)
+          if (ci < nsch) issue(scr, ci, tc.n_srows);
+      ci = __shfl_sync(0xffffffffu, ci, 0);
     }
   }
-  (void)v_root;
-#undef CN_ROW
+#undef CN_RD
 }
 
 // ------------------------------------------------------------------------------------------------
