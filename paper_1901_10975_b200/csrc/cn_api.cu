@@ -521,11 +521,24 @@ static int build_tape_program(cn_model *m, HClass &K) {
         r += (uint32_t)tape_rows_of(T.ti, T.type);
         sl += (uint32_t)T.ti.n_state;
       }
-    const uint32_t len = r - row;
+    uint32_t len = r - row;
     if (len > (CN_TAPE_S - 1) * CN_TAPE_CH || sl > (CN_TAPE_S - 1) * CN_TAPE_CH) {
       P.n_groups = 0;  // a record must fit the ring: this class stays on the cooperative kernel
       P.n_cells = 0;
       return CN_OK;
+    }
+    {  // a record never wraps around the ring: pad to the next lap when it would
+      const uint32_t R = CN_TAPE_S * CN_TAPE_CH;
+      if (row % R + len > R) {
+        const uint32_t pad = R - row % R;
+        if (j > 0) P.flags[j - 1] += pad << 24;  // the pad rows ride with the previous record
+        for (int t = 0; t < nt; ++t)
+          if (P.tab_row[t].size() && P.tab_row[t][x] >= 0) P.tab_row[t][x] += (int32_t)pad;
+        if (P.cai_row[x] >= 0) P.cai_row[x] += (int32_t)pad;
+        if (P.pp_row[x] >= 0) P.pp_row[x] += (int32_t)pad;
+        row += pad;
+        r += pad;
+      }
     }
     max_len = std::max(max_len, (int)std::max(len, sl));
     P.row[j] = row;
@@ -537,6 +550,12 @@ static int build_tape_program(cn_model *m, HClass &K) {
   P.n_rows = (int)row;
   uint32_t srow = 0;
   for (int j = n - 1; j >= 0; --j) {  // the scratch tape is written back to front
+    const uint32_t R = CN_TAPE_S * CN_TAPE_CH;
+    if (srow % R + slen[j] > R) {
+      const uint32_t pad = R - srow % R;
+      slen[j + 1] += pad;  // (j < n-1 here: the first record starts at 0)
+      srow += pad;
+    }
     P.srow[j] = srow;
     srow += slen[j];
   }

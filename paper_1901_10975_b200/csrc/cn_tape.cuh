@@ -130,8 +130,9 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
   const double dt = M.dt;
   const double q10dt = M.q10 * dt;
 
-#define CN_RD(base, i) \
-  (*reinterpret_cast<const double *>(ringc + (((base) + (uint32_t)(i) * 256u) & (RB - 1u))))
+  // the host pads the tapes so that no record wraps around the ring: row i of a record is at a
+  // fixed distance from its first row
+#define CN_RD(base, i) (*reinterpret_cast<const double *>((base) + (uint32_t)(i) * 256u))
 
   // chunk c of a row stream goes to stage c % S
   auto issue = [&](const double *base, int c, int total_rows) {
@@ -172,7 +173,7 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
       phase ^= 1u << ws;
       ws = (ws + 1) & (S - 1);
     }
-    const uint32_t rb = (e.x & 0xFFFFu) + lane8;
+    const unsigned char *rb = ringc + ((e.x & 0xFFFFu) + lane8);
     double *__restrict__ srec = scr_l + e.y;
     double *__restrict__ trec = tape_l + grow;
     const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
@@ -306,7 +307,7 @@ __global__ void __launch_bounds__(32) tape_step_kernel(const __grid_constant__ D
       phase ^= 1u << ws;
       ws = (ws + 1) & (S - 1);
     }
-    const uint32_t sb = (e.x >> 16) + lane8;
+    const unsigned char *sb = ringc + ((e.x >> 16) + lane8);
     double *__restrict__ trec = tape_l + grow;
     const uint32_t kind = fl & PG_KIND;
     double vp = v_prev;
