@@ -18,9 +18,6 @@
 
 using namespace cn;
 
-// ring geometry of the tape kernel: S stages of CH rows of 256 B
-#define CN_TAPE_S 8
-#define CN_TAPE_CH 8
 
 // ---------------------------------------------------------------------------------------------
 // errors
@@ -112,7 +109,12 @@ struct HTable {
   std::vector<int64_t> cell_inst;
 };
 
+struct HTask { int p0 = 0, p1 = 0; uint32_t row0 = 0, nrows = 0, srow0 = 0, nsrows = 0; };
+
 struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh)
+  std::vector<HTask> task;                   // W leaf tasks + the top task
+  std::vector<uint32_t> ring;                // per position: ring byte offsets (tape | scratch<<16)
+  int n_xs = 0;                              // exchange slots (cut subtree roots)
   int n_groups = 0;
   int64_t n_cells = 0;                       // the first n_cells of HClass::cells are tape cells
   std::vector<int32_t> order, pos_of;        // position -> local node, local node -> position
@@ -163,7 +165,8 @@ struct cn_model {
   std::vector<TapeGroup> tgrp;
   std::vector<uint8_t> cell_tape;   // per caller cell
   int64_t n_tape = 0, n_scratch = 0;  // doubles
-  int tape_prog_cap = 0, tape_stack_cap = 0, tape_max_len = 0;
+  int tape_prog_cap = 0, tape_stack_cap = 0, tape_max_len = 0, tape_xs_cap = 0;
+  int tape_W = 1, tape_S = 8, tape_CH = 8;  // warps per group, ring stages, rows per chunk
   int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
   std::vector<double> cai0;         // initial cai per caller node (when any table needs it)
   int warp_smem_doubles = 0, wpb = 4;
@@ -421,50 +424,35 @@ static int tape_rows_of(const TypeInfo &ti, int type) {
   return ti.n_dev_param + ti.n_state;
 }
 
-// Program of the interleaved kernel for one class: depth-first post-order (children before
-// parents, L196), the child visited last hands its contribution to the parent in registers, the
-// others through a stack; row offsets of every node's record on the tape and the scratch tape.
+// Program of the interleaved kernel for one class.  The cell's tree is cut into W sets of whole
+// subtrees (one LEAF TASK per warp, balanced by estimated cost) and the TOP part that holds the
+// root; every task visits its nodes in depth-first post-order (children before parents, L196):
+// the child visited last hands its contribution to the parent in registers, the others through a
+// stack, the root of a cut subtree through an exchange slot read by the top task.  Each task has
+// its own segment of the group's tape and scratch tape; row offsets are relative to the segment.
 static int build_tape_program(cn_model *m, HClass &K) {
   HTape &P = K.tp;
   const int n = K.n;
   const int nt = (int)m->tab.size();
+  const int W = m->tape_W;
+  const uint32_t CH = (uint32_t)m->tape_CH, R = (uint32_t)(m->tape_S * m->tape_CH);
   const int64_t f = m->cell_first[K.rep_cell];
+  auto give_up = [&]() {  // this class stays on the cooperative kernel
+    P.n_groups = 0;
+    P.n_cells = 0;
+    return CN_OK;
+  };
   std::vector<int32_t> par(n, -1);
   std::vector<std::vector<int32_t>> ch(n);
   for (int i = 1; i < n; ++i) {
     par[i] = (int32_t)(m->parent[f + i] - f);
     ch[par[i]].push_back(i);
   }
-  // stack need of every subtree; visit the child with the largest need first
-  std::vector<int32_t> need(n, 0);
-  for (int x = n - 1; x >= 0; --x) {
-    auto &c = ch[x];
-    std::stable_sort(c.begin(), c.end(), [&](int p, int q) { return need[p] > need[q]; });
-    if (c.size() == 1) need[x] = need[c[0]];
-    else if (c.size() >= 2) need[x] = std::max(need[c[0]], 1 + need[c[1]]);
-  }
-  P.order.clear();
-  P.order.reserve(n);
-  {
-    std::vector<std::pair<int32_t, uint32_t>> st;  // node, next child
-    st.emplace_back(0, 0u);
-    while (!st.empty()) {
-      auto &top = st.back();
-      if (top.second < ch[top.first].size()) {
-        const int32_t c = ch[top.first][top.second++];
-        st.emplace_back(c, 0u);
-      } else {
-        P.order.push_back(top.first);
-        st.pop_back();
-      }
-    }
-  }
-  P.pos_of.assign(n, 0);
-  for (int j = 0; j < n; ++j) P.pos_of[P.order[j]] = j;
-  // which local nodes carry which distributed table (from the representative cell)
+  // which local nodes carry which distributed table (from the representative cell), cost weights
   P.tab_row.assign(nt, std::vector<int32_t>());
   std::vector<uint32_t> node_mask(n, 0);
   std::vector<uint8_t> has_cai(n, 0), need_ica(n, 0);
+  std::vector<double> wgt(n, 1.0), sw(n, 0.0);
   for (int t = 0; t < nt; ++t) {
     const HTable &T = m->tab[t];
     if (T.ti.point) continue;
@@ -475,63 +463,200 @@ static int build_tape_program(cn_model *m, HClass &K) {
       node_mask[x] |= 1u << t;
       if (T.type == CN_CADYN) has_cai[x] = need_ica[x] = 1;
       if (T.type == CN_SK) has_cai[x] = 1;
+      wgt[x] += T.type == CN_HH ? 4.0 : T.type == CN_CADYN ? 0.3 : 2.5;
     }
   }
+  for (int x = 0; x < n; ++x)
+    if (P.has_pp[x]) wgt[x] += 0.2;
+  for (int x = n - 1; x >= 0; --x) {
+    sw[x] += wgt[x];
+    if (x > 0) sw[par[x]] += sw[x];
+  }
+  // ---- cut: top set + frontier of subtree roots, refined while the estimated time improves ----
+  std::vector<uint8_t> in_top(n, 0), is_cut(n, 0);
+  std::vector<int32_t> frontier;
+  std::vector<int> owner(n, -1);  // warp of a cut subtree root
+  if (W <= 1) {
+    for (int x = 0; x < n; ++x) in_top[x] = 1;
+  } else {
+    double top_w = 0.0;
+    auto lpt = [&](const std::vector<int32_t> &F, std::vector<int> *assign) {
+      std::vector<int32_t> s(F);
+      std::sort(s.begin(), s.end(), [&](int a, int b) { return sw[a] > sw[b]; });
+      std::vector<double> load(W, 0.0);
+      for (int32_t x : s) {
+        const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+        load[w] += sw[x];
+        if (assign) (*assign)[x] = w;
+      }
+      return *std::max_element(load.begin(), load.end());
+    };
+    // moving x into the top set: x and its single-child chain down to the first branch point
+    auto split = [&](int32_t x, std::vector<int32_t> &F, double &tw, std::vector<int32_t> *moved) {
+      F.erase(std::find(F.begin(), F.end(), x));
+      int32_t y = x;
+      for (;;) {
+        tw += wgt[y];
+        if (moved) moved->push_back(y);
+        if (ch[y].size() == 1) { y = ch[y][0]; continue; }
+        for (int32_t c : ch[y]) F.push_back(c);
+        break;
+      }
+    };
+    frontier.push_back(0);
+    {
+      std::vector<int32_t> moved;
+      split(0, frontier, top_w, &moved);
+      for (int32_t y : moved) in_top[y] = 1;
+    }
+    double est = lpt(frontier, nullptr) + top_w;
+    std::vector<uint8_t> frozen(n, 0);
+    while ((int)frontier.size() < 6 * W && (int)frontier.size() < 200) {
+      int32_t best = -1;
+      for (int32_t x : frontier)
+        if (!frozen[x] && (best < 0 || sw[x] > sw[best])) best = x;
+      if (best < 0) break;
+      std::vector<int32_t> F2(frontier), moved;
+      double tw2 = top_w;
+      split(best, F2, tw2, &moved);
+      size_t max_cut_children = 0;
+      {
+        const int32_t last = moved.back();
+        max_cut_children = ch[last].size();
+      }
+      const double est2 = lpt(F2, nullptr) + tw2;
+      if (est2 < est * 0.999 && max_cut_children <= 15) {
+        frontier.swap(F2);
+        top_w = tw2;
+        est = est2;
+        for (int32_t y : moved) in_top[y] = 1;
+      } else {
+        frozen[best] = 1;
+      }
+    }
+    for (int32_t x : frontier) is_cut[x] = 1;
+    lpt(frontier, &owner);
+  }
+  // cut children of a top node must fit the 4-bit import count
+  for (int x = 0; x < n; ++x) {
+    if (!in_top[x]) continue;
+    int cnt = 0;
+    for (int32_t c : ch[x]) cnt += is_cut[c];
+    if (cnt > 15) return give_up();
+  }
+  if (frontier.size() > 255) return give_up();
+  // ---- visiting order inside a task: stack need of every subtree, largest need first ----------
+  // (children that belong to another task -- cut subtree roots under a top node -- do not count)
+  std::vector<std::vector<int32_t>> tch(n);  // same-task children
+  for (int x = 1; x < n; ++x)
+    if (!is_cut[x]) tch[par[x]].push_back(x);
+  std::vector<int32_t> need(n, 0);
+  for (int x = n - 1; x >= 0; --x) {
+    auto &c = tch[x];
+    std::stable_sort(c.begin(), c.end(), [&](int p, int q) { return need[p] > need[q]; });
+    if (c.size() == 1) need[x] = need[c[0]];
+    else if (c.size() >= 2) need[x] = std::max(need[c[0]], 1 + need[c[1]]);
+  }
+  auto post_order = [&](int32_t root, std::vector<int32_t> &out) {
+    std::vector<std::pair<int32_t, uint32_t>> st;
+    st.emplace_back(root, 0u);
+    while (!st.empty()) {
+      auto &top = st.back();
+      if (top.second < tch[top.first].size()) {
+        const int32_t c = tch[top.first][top.second++];
+        st.emplace_back(c, 0u);
+      } else {
+        out.push_back(top.first);
+        st.pop_back();
+      }
+    }
+  };
+  P.order.clear();
+  P.order.reserve(n);
+  P.task.assign(W + 1, HTask());
+  for (int w = 0; w < W; ++w) {
+    P.task[w].p0 = (int)P.order.size();
+    for (int32_t x : frontier)
+      if (owner[x] == w) post_order(x, P.order);
+    P.task[w].p1 = (int)P.order.size();
+  }
+  P.task[W].p0 = (int)P.order.size();
+  post_order(0, P.order);
+  P.task[W].p1 = (int)P.order.size();
+  if ((int)P.order.size() != n) return fail(CN_ERR_TOPOLOGY, "internal: tape order incomplete");
+  P.pos_of.assign(n, 0);
+  for (int j = 0; j < n; ++j) P.pos_of[P.order[j]] = j;
+  // exchange slots: the cut children of a top node get consecutive slots, in top visiting order
+  std::vector<int32_t> slot_of(n, -1), imp_first(n, 0), imp_cnt(n, 0);
+  {
+    int ns = 0;
+    for (int j = P.task[W].p0; j < P.task[W].p1; ++j) {
+      const int x = P.order[j];
+      imp_first[x] = ns;
+      for (int32_t c : ch[x])
+        if (is_cut[c]) {
+          slot_of[c] = ns++;
+          imp_cnt[x]++;
+        }
+    }
+    P.n_xs = ns;
+  }
+  // ---- records: rows of every node on the tape / scratch tape, per task -----------------------
   P.row.assign(n, 0);
   P.srow.assign(n, 0);
   P.flags.assign(n, 0);
   P.mask.assign(n, 0);
+  P.ring.assign(n, 0);
   P.cai_row.assign(n, -1);
   P.pp_row.assign(n, -1);
-  uint32_t row = 0;
-  int max_len = 0;
-  std::vector<uint32_t> slen(n, 0);
-  for (int j = 0; j < n; ++j) {
-    const int x = P.order[j];
-    uint32_t fl = 0, r = row + 5, sl = 2;
-    if (x == 0) {
-      fl |= PG_ROOT;
-    } else {
-      const auto &sib = ch[par[x]];
-      if (sib.back() == x) fl |= PG_FWD;
-      else if (sib.front() == x) fl |= PG_PUSH;
-      else fl |= PG_ADD;
-    }
-    if (!ch[x].empty()) fl |= PG_FWD_IN;
-    if (ch[x].size() >= 2) fl |= PG_POP;
-    if (P.has_pp[x]) {
-      fl |= PG_HAS_PP;
-      P.pp_row[x] = (int32_t)r;
-      r += 2;
-    }
-    if (need_ica[x]) {
-      fl |= PG_NEED_ICA;
-      sl += 1;
-    }
-    if (has_cai[x]) {
-      fl |= PG_HAS_CAI;
-      P.cai_row[x] = (int32_t)r;
-      r += 1;
-      sl += 1;
-    }
-    for (int t = 0; t < nt; ++t)
-      if (node_mask[x] & (1u << t)) {
-        const HTable &T = m->tab[t];
-        P.tab_row[t][x] = (int32_t)r;
-        r += (uint32_t)tape_rows_of(T.ti, T.type);
-        sl += (uint32_t)T.ti.n_state;
+  std::vector<uint32_t> len(n, 0), slen(n, 0);
+  uint32_t row = 0, srow_base = 0;
+  int max_len = 0, depth = 1;
+  for (int w = 0; w <= W; ++w) {
+    HTask &Tk = P.task[w];
+    Tk.row0 = row;
+    for (int j = Tk.p0; j < Tk.p1; ++j) {
+      const int x = P.order[j];
+      uint32_t fl = 0, r = row + 5, sl = 2;
+      if (x == 0) {
+        fl |= PG_ROOT;
+      } else if (!is_cut[x]) {
+        const auto &sib = tch[par[x]];
+        if (sib.back() == x) fl |= PG_FWD;
+        else if (sib.front() == x) fl |= PG_PUSH;
+        else fl |= PG_ADD;
+      }  // a cut subtree root has kind 0 without PG_ROOT: it exports to its slot
+      if (!tch[x].empty()) fl |= PG_FWD_IN;
+      if (tch[x].size() >= 2) fl |= PG_POP;
+      if (P.has_pp[x]) {
+        fl |= PG_HAS_PP;
+        P.pp_row[x] = (int32_t)r;
+        r += 2;
       }
-    uint32_t len = r - row;
-    if (len > (CN_TAPE_S - 1) * CN_TAPE_CH || sl > (CN_TAPE_S - 1) * CN_TAPE_CH) {
-      P.n_groups = 0;  // a record must fit the ring: this class stays on the cooperative kernel
-      P.n_cells = 0;
-      return CN_OK;
-    }
-    {  // a record never wraps around the ring: pad to the next lap when it would
-      const uint32_t R = CN_TAPE_S * CN_TAPE_CH;
-      if (row % R + len > R) {
-        const uint32_t pad = R - row % R;
-        if (j > 0) P.flags[j - 1] += pad << 24;  // the pad rows ride with the previous record
+      if (need_ica[x]) {
+        fl |= PG_NEED_ICA;
+        sl += 1;
+      }
+      if (has_cai[x]) {
+        fl |= PG_HAS_CAI;
+        P.cai_row[x] = (int32_t)r;
+        r += 1;
+        sl += 1;
+      }
+      for (int t = 0; t < nt; ++t)
+        if (node_mask[x] & (1u << t)) {
+          const HTable &T = m->tab[t];
+          P.tab_row[t][x] = (int32_t)r;
+          r += (uint32_t)tape_rows_of(T.ti, T.type);
+          sl += (uint32_t)T.ti.n_state;
+        }
+      uint32_t ln = r - row;
+      if (ln > R - CH || sl > R - CH) return give_up();  // a record must fit the ring
+      const uint32_t rel = row - Tk.row0;
+      if (rel % R + ln > R) {  // a record never wraps around the ring: pad to the next lap
+        const uint32_t pad = R - rel % R;
+        len[j - 1] += pad;     // the pad rows ride with the previous record (j > p0 here)
+        if (len[j - 1] > R - CH) return give_up();
         for (int t = 0; t < nt; ++t)
           if (P.tab_row[t].size() && P.tab_row[t][x] >= 0) P.tab_row[t][x] += (int32_t)pad;
         if (P.cai_row[x] >= 0) P.cai_row[x] += (int32_t)pad;
@@ -539,57 +664,63 @@ static int build_tape_program(cn_model *m, HClass &K) {
         row += pad;
         r += pad;
       }
+      max_len = std::max(max_len, (int)std::max(ln, sl));
+      P.row[j] = row;
+      P.flags[j] = fl;
+      P.mask[j] = node_mask[x] | (uint32_t)(is_cut[x] ? slot_of[x] : imp_first[x]) << 20 |
+                  (uint32_t)imp_cnt[x] << 28;
+      len[j] = ln;
+      slen[j] = sl;
+      row = r;
     }
-    max_len = std::max(max_len, (int)std::max(len, sl));
-    P.row[j] = row;
-    P.flags[j] = fl | (len << 24);
-    P.mask[j] = node_mask[x];
-    slen[j] = sl;
-    row = r;
-  }
-  P.n_rows = (int)row;
-  uint32_t srow = 0;
-  for (int j = n - 1; j >= 0; --j) {  // the scratch tape is written back to front
-    const uint32_t R = CN_TAPE_S * CN_TAPE_CH;
-    if (srow % R + slen[j] > R) {
-      const uint32_t pad = R - srow % R;
-      slen[j + 1] += pad;  // (j < n-1 here: the first record starts at 0)
-      srow += pad;
+    Tk.nrows = row - Tk.row0;
+    // the scratch segment of the task is written back to front
+    Tk.srow0 = srow_base;
+    uint32_t sr = 0;
+    for (int j = Tk.p1 - 1; j >= Tk.p0; --j) {
+      if (sr % R + slen[j] > R) {
+        const uint32_t pad = R - sr % R;
+        slen[j + 1] += pad;
+        if (slen[j + 1] > R - CH) return give_up();
+        sr += pad;
+      }
+      P.srow[j] = srow_base + sr;
+      P.ring[j] = ((P.row[j] - Tk.row0) % R) * 256u | ((sr % R) * 256u) << 16;
+      sr += slen[j];
     }
-    P.srow[j] = srow;
-    srow += slen[j];
-  }
-  P.n_srows = (int)srow;
-  // chunk bookkeeping of the ring, precomputed: how many chunks a node must wait for before its
-  // rows are complete and how many are fully consumed after it, in both directions
-  {
-    const int CH = CN_TAPE_CH;
+    Tk.nsrows = sr;
+    srow_base += sr;
+    // chunk bookkeeping of the ring, precomputed: how many chunks a node must wait for before
+    // its rows are complete and how many are fully consumed after it, in both directions
     int last = -1, next = 0;
-    for (int j = 0; j < n; ++j) {
-      const uint32_t len = P.flags[j] >> 24;
-      const int cl = (int)((P.row[j] + len - 1) / CH), cn = (int)((P.row[j] + len) / CH);
-      P.flags[j] |= (uint32_t)(cl - last) << 8 | (uint32_t)(cn - next) << 12;
+    for (int j = Tk.p0; j < Tk.p1; ++j) {
+      const uint32_t rel = P.row[j] - Tk.row0;
+      const int cl = (int)((rel + len[j] - 1) / CH), cn = (int)((rel + len[j]) / CH);
+      P.flags[j] |= (uint32_t)(cl - last) << 8 | (uint32_t)(cn - next) << 12 | len[j] << 24;
       last = cl;
       next = cn;
     }
     last = -1;
     next = 0;
-    for (int j = n - 1; j >= 0; --j) {
-      const int cl = (int)((P.srow[j] + slen[j] - 1) / CH), cn = (int)((P.srow[j] + slen[j]) / CH);
+    for (int j = Tk.p1 - 1; j >= Tk.p0; --j) {
+      const uint32_t rel = P.srow[j] - Tk.srow0;
+      const int cl = (int)((rel + slen[j] - 1) / CH), cn = (int)((rel + slen[j]) / CH);
       P.flags[j] |= (uint32_t)(cl - last) << 16 | (uint32_t)(cn - next) << 20;
       last = cl;
       next = cn;
     }
+    // stack depth by simulation of the forward pass
+    int sp = 0;
+    for (int j = Tk.p0; j < Tk.p1; ++j) {
+      const uint32_t fl = P.flags[j];
+      if (fl & PG_POP) --sp;
+      if ((fl & PG_KIND) == PG_PUSH) depth = std::max(depth, ++sp);
+    }
+    if (sp != 0) return fail(CN_ERR_TOPOLOGY, "internal: unbalanced tape program");
   }
-  // stack depth by simulation of the forward pass
-  int sp = 0, depth = 0;
-  for (int j = 0; j < n; ++j) {
-    const uint32_t fl = P.flags[j];
-    if (fl & PG_POP) --sp;
-    if ((fl & PG_KIND) == PG_PUSH && !(fl & PG_ROOT)) depth = std::max(depth, ++sp);
-  }
-  if (sp != 0) return fail(CN_ERR_TOPOLOGY, "internal: unbalanced tape program");
-  P.depth = std::max(depth, 1);
+  P.n_rows = (int)row;
+  P.n_srows = (int)srow_base;
+  P.depth = depth;
   m->tape_max_len = std::max(m->tape_max_len, max_len);
   return CN_OK;
 }
@@ -701,12 +832,25 @@ static int build_layout(cn_model *m) {
   int tape_min_group = 16;  // a ragged last group needs at least this many cells
   if (const char *e = std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = std::max(1, std::atoi(e));
   const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells);
+  m->tape_W = 2;
+  if (const char *e = std::getenv("CN_TAPE_W")) m->tape_W = std::min(4, std::max(1, std::atoi(e)));
+  m->tape_S = m->tape_W == 1 ? 8 : 4;
+  m->tape_CH = 8;
+  if (const char *e = std::getenv("CN_TAPE_S")) {
+    const int v = std::atoi(e);
+    if (v == 4 || v == 8 || v == 16) m->tape_S = v;
+  }
+  if (const char *e = std::getenv("CN_TAPE_CH")) {
+    const int v = std::atoi(e);
+    if (v == 8 || v == 16) m->tape_CH = v;
+  }
+  if (m->tape_S * m->tape_CH > 128) m->tape_S = 128 / m->tape_CH;
   m->cell_tape.assign(nc, 0);
   for (HClass &K : m->cls) {
     K.count = (int64_t)K.cells.size();
     K.tp.n_groups = 0;
     K.tp.n_cells = 0;
-    if (!tape_on || nt > 32) continue;
+    if (!tape_on || nt > 20) continue;
     const int64_t full = K.count / 32, rem = K.count % 32;
     K.tp.n_groups = (int)(full + (rem >= tape_min_group ? 1 : 0));
     K.tp.n_cells = std::min<int64_t>(K.count, (int64_t)K.tp.n_groups * 32);
@@ -733,6 +877,7 @@ static int build_layout(cn_model *m) {
     prog_total += K.n;
     m->tape_prog_cap = std::max(m->tape_prog_cap, K.n);
     m->tape_stack_cap = std::max(m->tape_stack_cap, K.tp.depth);
+    m->tape_xs_cap = std::max(m->tape_xs_cap, K.tp.n_xs);
   }
 
   // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
@@ -1203,20 +1348,26 @@ static int finalize(cn_model *m, double dt) {
     rc = dev_alloc(m, (size_t)std::max<int64_t>(m->n_scratch, 1), &H.scratch, false);
     if (rc != CN_OK) return rc;
     std::vector<TapeClass> tcls(m->cls.size());
+    std::vector<TapeTask> ttask(m->cls.size() * (size_t)(m->tape_W + 1));
     std::vector<uint4> prog;
     for (size_t kc = 0; kc < m->cls.size(); ++kc) {
       const HClass &K = m->cls[kc];
       const HTape &P = K.tp;
-      tcls[kc] = TapeClass{K.n, P.prog_off, P.n_rows, P.n_srows, P.depth, 0, 0, 0};
+      tcls[kc] = TapeClass{K.n, P.prog_off, P.n_rows, P.n_srows, P.depth, P.n_xs, 0, 0};
       if (P.n_groups == 0) continue;
-      const uint32_t R = CN_TAPE_S * CN_TAPE_CH;
       for (int j = 0; j < K.n; ++j)
-        prog.push_back(make_uint4((P.row[j] % R) * 256u | ((P.srow[j] % R) * 256u) << 16,
-                                  P.srow[j] * 32u, P.flags[j], P.mask[j]));
+        prog.push_back(make_uint4(P.ring[j], P.srow[j] * 32u, P.flags[j], P.mask[j]));
+      for (int w = 0; w <= m->tape_W; ++w) {
+        const HTask &Tk = P.task[w];
+        ttask[kc * (size_t)(m->tape_W + 1) + w] =
+            TapeTask{Tk.p0, Tk.p1, Tk.row0, Tk.nrows, Tk.srow0, Tk.nsrows, 0, 0};
+      }
     }
-    TapeGroup *dtg; TapeClass *dtc; uint4 *dpg;
-    UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg);
-    H.tgrp = dtg; H.tcls = dtc; H.prog = dpg;
+    TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
+    UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg); UP(ttask, dtt);
+    H.tgrp = dtg; H.tcls = dtc; H.prog = dpg; H.ttask = dtt;
+    H.tape_W = m->tape_W;
+    H.tape_xs_cap = std::max(m->tape_xs_cap, 1);
     H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
     H.tape_stack_cap = std::max(m->tape_stack_cap, 1);
     for (int t = 0; t < nt; ++t) {
@@ -1324,21 +1475,34 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
 }
 
 static size_t tape_smem_bytes(const cn_model *m) {
-  return (size_t)CN_TAPE_S * CN_TAPE_CH * 256 + (size_t)m->hm.tape_prog_cap * 16 +
-         (size_t)m->hm.tape_stack_cap * 512 + (CN_TAPE_S + 1) * 8;
+  const size_t W = (size_t)m->tape_W;
+  return W * m->tape_S * m->tape_CH * 256 + (size_t)m->hm.tape_prog_cap * 16 +
+         W * m->hm.tape_stack_cap * 512 + (size_t)m->hm.tape_xs_cap * 512 +
+         W * (m->tape_S + 1) * 8;
 }
 
-static cudaError_t launch_tape(cn_model *m, int64_t k) {
+template <int S, int CH>
+static cudaError_t launch_tape_t(cn_model *m, int64_t k) {
   const size_t smem = tape_smem_bytes(m);
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(tape_step_kernel<CN_TAPE_S, CN_TAPE_CH>,
+    cudaError_t e = cudaFuncSetAttribute(tape_step_kernel<S, CH>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tape_step_kernel<S, CH>,
+                             cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  tape_step_kernel<CN_TAPE_S, CN_TAPE_CH><<<m->hm.n_tgroup, 32, smem, m->stream>>>(m->hm, k);
+  tape_step_kernel<S, CH><<<m->hm.n_tgroup, 32 * m->tape_W, smem, m->stream>>>(m->hm, k);
   return cudaGetLastError();
+}
+
+static cudaError_t launch_tape(cn_model *m, int64_t k) {
+  if (m->tape_CH == 16) return m->tape_S == 8 ? launch_tape_t<8, 16>(m, k) : launch_tape_t<4, 16>(m, k);
+  if (m->tape_S == 16) return launch_tape_t<16, 8>(m, k);
+  return m->tape_S == 8 ? launch_tape_t<8, 8>(m, k) : launch_tape_t<4, 8>(m, k);
 }
 
 static int run_steps(cn_model *m, int64_t K) {
@@ -1614,4 +1778,17 @@ extern "C" void cn_model_destroy(cn_model *m) {
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);
   delete m;
+}
+
+// debugging aid for DESIGN/bench: positions per task of the first tape class
+extern "C" int cn_debug_tasks(const cn_model *m, int32_t *out, int32_t cap) {
+  for (const HClass &K : m->cls) {
+    if (K.tp.n_groups == 0) continue;
+    int n = 0;
+    for (const HTask &t : K.tp.task) {
+      if (n + 2 <= cap) { out[n++] = t.p1 - t.p0; out[n++] = (int32_t)t.nrows; }
+    }
+    return n;
+  }
+  return 0;
 }

@@ -64,19 +64,28 @@ struct TapeGroup {
 
 struct TapeClass {
   int32_t n, prog_off, n_rows, n_srows;
-  int32_t depth, pad0, pad1, pad2;
+  int32_t depth, n_xs, pad1, pad2;
 };
 
-// program entry flags (uint4: x = first tape row, y = first scratch row (reversed order),
-// z = flags | rows << 8 | scratch rows << 16, w = mask of distributed tables on this node)
+// one task of a class: a range of program positions with its own tape / scratch-tape segment
+struct TapeTask {
+  int32_t p0, p1;
+  uint32_t row0, nrows, srow0, nsrows;
+  int32_t pad0, pad1;
+};
+
+// program entry flags (layout of the uint4 entry: see tape_step_kernel).  Kind 0 without PG_ROOT
+// is the root of a cut subtree: it exports its contribution to an exchange slot.
 enum { PG_FWD = 1, PG_PUSH = 2, PG_ADD = 3, PG_KIND = 3, PG_FWD_IN = 4, PG_POP = 8, PG_ROOT = 16,
        PG_HAS_PP = 32, PG_HAS_CAI = 64, PG_NEED_ICA = 128 };
 
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
-  int32_t n_tgroup, tape_prog_cap, tape_stack_cap, pad_t;
+  int32_t n_tgroup, tape_prog_cap, tape_stack_cap, tape_xs_cap;
+  int32_t tape_W, pad_t0, pad_t1, pad_t2;
   const TapeGroup *tgrp;
   const TapeClass *tcls;
+  const TapeTask *ttask;        // [n_class][tape_W + 1]: leaf task of every warp, then the top task
   const uint4 *prog;
   double *tape;                 // == v + n_ab: one arena, so node positions index both
   double *scratch;

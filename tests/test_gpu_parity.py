@@ -26,16 +26,19 @@ def cn():
     return cn
 
 
-@pytest.fixture(params=["coop", "tape"])
+@pytest.fixture(params=["coop", "tape", "tape-w1", "tape-w4"])
 def strategy(request, monkeypatch):
     """Both kernels on the same inputs: warp-cooperative groups, or every cell on the interleaved
-    (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1)."""
-    if request.param == "tape":
+    (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1), with 2 (default), 1 or 4 warps
+    (subtree tasks) per group of 32 cells."""
+    if request.param.startswith("tape"):
         monkeypatch.setenv("CN_TAPE", "1")
         monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+        if "-w" in request.param:
+            monkeypatch.setenv("CN_TAPE_W", request.param[-1])
     else:
         monkeypatch.setenv("CN_TAPE", "0")
-    return request.param
+    return "tape" if request.param.startswith("tape") else "coop"
 
 
 def run_both(cn, desc, tstop, dt=DT, probes=None, chunks=1, env=None):
