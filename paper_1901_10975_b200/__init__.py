@@ -264,7 +264,7 @@ class Model:
         _check(lib().cn_get_layout_info(self._h, _ptr(a)))
         return {"n_class": int(a[0]), "n_group": int(a[1]), "warp_smem_bytes": int(a[2]),
                 "max_rounds": int(a[3]), "n_tape_group": int(a[4]), "tape_bytes": int(a[5]),
-                "scratch_bytes": int(a[6]), "tape_stack_depth": int(a[7])}
+                "scratch_bytes": int(a[6]), "tape_warps": int(a[7])}
 
     def set_spike_capacity(self, cap):
         _check(lib().cn_set_spike_capacity(self._h, int(cap)))

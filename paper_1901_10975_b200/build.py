@@ -8,7 +8,8 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 SO = HERE / "libcn.so"
 SRCS = [HERE / "csrc" / "cn_api.cu"]
-DEPS = SRCS + [HERE / "csrc" / "cn_device.cuh", HERE.parent / "include" / "cn.h"]
+DEPS = SRCS + [HERE / "csrc" / "cn_device.cuh", HERE / "csrc" / "cn_tape.cuh",
+               HERE.parent / "include" / "cn.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

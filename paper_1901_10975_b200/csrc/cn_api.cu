@@ -109,20 +109,20 @@ struct HTable {
   std::vector<int64_t> cell_inst;
 };
 
-struct HTask { int p0 = 0, p1 = 0; uint32_t row0 = 0, nrows = 0, srow0 = 0, nsrows = 0; };
+struct HTask { int p0 = 0, p1 = 0, pm = 0; uint32_t row0 = 0, nrows = 0, mrows = 0; };
 
 struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh)
-  std::vector<HTask> task;                   // W leaf tasks + the top task
-  std::vector<uint32_t> ring;                // per position: ring byte offsets (tape | scratch<<16)
-  int n_xs = 0;                              // exchange slots (cut subtree roots)
+  std::vector<HTask> task;                   // one per warp
+  std::vector<uint4> prog;                   // records of all warps, warp after warp
   int n_groups = 0;
   int64_t n_cells = 0;                       // the first n_cells of HClass::cells are tape cells
-  std::vector<int32_t> order, pos_of;        // position -> local node, local node -> position
-  std::vector<uint32_t> row, srow, flags, mask;
+  std::vector<int32_t> order, pos_of;        // system row -> local node, local node -> system row
+  std::vector<uint32_t> row;                 // per system row: first tape row of the node's record
   std::vector<uint8_t> has_pp;               // per local node
   std::vector<std::vector<int32_t>> tab_row; // [table][local node]: first row of its block or -1
-  std::vector<int32_t> cai_row, pp_row;      // per local node or -1
-  int n_rows = 0, n_srows = 0, depth = 0, prog_off = 0;
+  std::vector<int32_t> cai_row, ica_row, pp_row, vcopy_row;  // per local node or -1
+  int n_rows = 0, prog_off = 0;
+  double sim_makespan = 0.0, sim_work = 0.0; // schedule quality (cn_debug_tasks)
 };
 
 struct HClass {
@@ -164,9 +164,11 @@ struct cn_model {
   // interleaved (tape) groups
   std::vector<TapeGroup> tgrp;
   std::vector<uint8_t> cell_tape;   // per caller cell
-  int64_t n_tape = 0, n_scratch = 0;  // doubles
-  int tape_prog_cap = 0, tape_stack_cap = 0, tape_max_len = 0, tape_xs_cap = 0;
-  int tape_W = 1, tape_S = 8, tape_CH = 8;  // warps per group, ring stages, rows per chunk
+  int64_t n_tape = 0;               // doubles
+  int tape_prog_cap = 0, tape_sys_cap = 0;
+  int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
+  int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
+  bool state_pending = false;       // nrn_state of the last step has not been applied yet
   int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
   std::vector<double> cai0;         // initial cai per caller node (when any table needs it)
   int warp_smem_doubles = 0, wpb = 4;
@@ -424,12 +426,23 @@ static int tape_rows_of(const TypeInfo &ti, int type) {
   return ti.n_dev_param + ti.n_state;
 }
 
-// Program of the interleaved kernel for one class.  The cell's tree is cut into W sets of whole
-// subtrees (one LEAF TASK per warp, balanced by estimated cost) and the TOP part that holds the
-// root; every task visits its nodes in depth-first post-order (children before parents, L196):
-// the child visited last hands its contribution to the parent in registers, the others through a
-// stack, the root of a cut subtree through an exchange slot read by the top task.  Each task has
-// its own segment of the group's tape and scratch tape; row offsets are relative to the segment.
+// Program of the interleaved kernel for one class: a static schedule of the cell's elimination
+// over W warps (children before parents, L196).
+//   1. The tree is cut into tasks: whole subtrees small enough to balance (visited depth-first,
+//      the heaviest child last so that it hands over to the parent in registers) and, above them,
+//      single nodes.  The tasks are list-scheduled on W warps, deepest first; a warp that
+//      completes the last child of a node continues with that node.
+//   2. Every node with distributed mechanisms gets a MECH record (nrn_state of the previous step,
+//      nrn_cur); these come first on every warp, spread evenly in the order the elimination
+//      needs them.
+//   3. Contributions that are not handed over in registers meet in the parent's row of the
+//      shared-memory system: the first contributor stores, the others add, one after the other
+//      in the order of the simulated schedule.  Dependencies between warps become WAIT records /
+//      signal flags on per-warp progress counters.  All dependencies point backwards in simulated
+//      time (MECH records depend on nothing), so the program cannot deadlock; a host-side dry run
+//      checks that anyway.
+//   4. Each warp's records get consecutive rows of the group's tape, padded so that no record
+//      wraps around the warp's ring; the chunk bookkeeping of the ring is precomputed.
 static int build_tape_program(cn_model *m, HClass &K) {
   HTape &P = K.tp;
   const int n = K.n;
@@ -442,6 +455,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
     P.n_cells = 0;
     return CN_OK;
   };
+  if (n > 1023) return give_up();  // 10-bit system rows
   std::vector<int32_t> par(n, -1);
   std::vector<std::vector<int32_t>> ch(n);
   for (int i = 1; i < n; ++i) {
@@ -452,276 +466,479 @@ static int build_tape_program(cn_model *m, HClass &K) {
   P.tab_row.assign(nt, std::vector<int32_t>());
   std::vector<uint32_t> node_mask(n, 0);
   std::vector<uint8_t> has_cai(n, 0), need_ica(n, 0);
-  std::vector<double> wgt(n, 1.0), sw(n, 0.0);
+  std::vector<double> ecost(n, 1.0), mcost(n, 0.0);
   for (int t = 0; t < nt; ++t) {
     const HTable &T = m->tab[t];
     if (T.ti.point) continue;
     P.tab_row[t].assign(n, -1);
+    if (T.type == CN_PAS) continue;  // folded into the static rows
     for (int64_t q = T.cell_first[K.rep_cell]; q < T.cell_first[K.rep_cell + 1]; ++q) {
       const int x = (int)(T.node[T.cell_inst[q]] - f);
-      if (T.type == CN_PAS) continue;  // folded into the static rows
       node_mask[x] |= 1u << t;
       if (T.type == CN_CADYN) has_cai[x] = need_ica[x] = 1;
       if (T.type == CN_SK) has_cai[x] = 1;
-      wgt[x] += T.type == CN_HH ? 4.0 : T.type == CN_CADYN ? 0.3 : 2.5;
+      mcost[x] += T.type == CN_HH ? 12.0 : T.type == CN_HHFORM ? 8.0 : T.type == CN_SK ? 6.0 : 1.0;
     }
   }
   for (int x = 0; x < n; ++x)
-    if (P.has_pp[x]) wgt[x] += 0.2;
-  for (int x = n - 1; x >= 0; --x) {
-    sw[x] += wgt[x];
-    if (x > 0) sw[par[x]] += sw[x];
-  }
-  // ---- cut: top set + frontier of subtree roots, refined while the estimated time improves ----
-  std::vector<uint8_t> in_top(n, 0), is_cut(n, 0);
-  std::vector<int32_t> frontier;
-  std::vector<int> owner(n, -1);  // warp of a cut subtree root
-  if (W <= 1) {
-    for (int x = 0; x < n; ++x) in_top[x] = 1;
-  } else {
-    double top_w = 0.0;
-    auto lpt = [&](const std::vector<int32_t> &F, std::vector<int> *assign) {
-      std::vector<int32_t> s(F);
-      std::sort(s.begin(), s.end(), [&](int a, int b) { return sw[a] > sw[b]; });
-      std::vector<double> load(W, 0.0);
-      for (int32_t x : s) {
-        const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
-        load[w] += sw[x];
-        if (assign) (*assign)[x] = w;
-      }
-      return *std::max_element(load.begin(), load.end());
-    };
-    // moving x into the top set: x and its single-child chain down to the first branch point
-    auto split = [&](int32_t x, std::vector<int32_t> &F, double &tw, std::vector<int32_t> *moved) {
-      F.erase(std::find(F.begin(), F.end(), x));
-      int32_t y = x;
-      for (;;) {
-        tw += wgt[y];
-        if (moved) moved->push_back(y);
-        if (ch[y].size() == 1) { y = ch[y][0]; continue; }
-        for (int32_t c : ch[y]) F.push_back(c);
-        break;
-      }
-    };
-    frontier.push_back(0);
-    {
-      std::vector<int32_t> moved;
-      split(0, frontier, top_w, &moved);
-      for (int32_t y : moved) in_top[y] = 1;
-    }
-    double est = lpt(frontier, nullptr) + top_w;
-    std::vector<uint8_t> frozen(n, 0);
-    while ((int)frontier.size() < 6 * W && (int)frontier.size() < 200) {
-      int32_t best = -1;
-      for (int32_t x : frontier)
-        if (!frozen[x] && (best < 0 || sw[x] > sw[best])) best = x;
-      if (best < 0) break;
-      std::vector<int32_t> F2(frontier), moved;
-      double tw2 = top_w;
-      split(best, F2, tw2, &moved);
-      size_t max_cut_children = 0;
-      {
-        const int32_t last = moved.back();
-        max_cut_children = ch[last].size();
-      }
-      const double est2 = lpt(F2, nullptr) + tw2;
-      if (est2 < est * 0.999 && max_cut_children <= 15) {
-        frontier.swap(F2);
-        top_w = tw2;
-        est = est2;
-        for (int32_t y : moved) in_top[y] = 1;
-      } else {
-        frozen[best] = 1;
-      }
-    }
-    for (int32_t x : frontier) is_cut[x] = 1;
-    lpt(frontier, &owner);
-  }
-  // cut children of a top node must fit the 4-bit import count
-  for (int x = 0; x < n; ++x) {
-    if (!in_top[x]) continue;
-    int cnt = 0;
-    for (int32_t c : ch[x]) cnt += is_cut[c];
-    if (cnt > 15) return give_up();
-  }
-  if (frontier.size() > 255) return give_up();
-  // ---- visiting order inside a task: stack need of every subtree, largest need first ----------
-  // (children that belong to another task -- cut subtree roots under a top node -- do not count)
-  std::vector<std::vector<int32_t>> tch(n);  // same-task children
-  for (int x = 1; x < n; ++x)
-    if (!is_cut[x]) tch[par[x]].push_back(x);
-  std::vector<int32_t> need(n, 0);
-  for (int x = n - 1; x >= 0; --x) {
-    auto &c = tch[x];
-    std::stable_sort(c.begin(), c.end(), [&](int p, int q) { return need[p] > need[q]; });
-    if (c.size() == 1) need[x] = need[c[0]];
-    else if (c.size() >= 2) need[x] = std::max(need[c[0]], 1 + need[c[1]]);
-  }
-  auto post_order = [&](int32_t root, std::vector<int32_t> &out) {
-    std::vector<std::pair<int32_t, uint32_t>> st;
-    st.emplace_back(root, 0u);
-    while (!st.empty()) {
-      auto &top = st.back();
-      if (top.second < tch[top.first].size()) {
-        const int32_t c = tch[top.first][top.second++];
-        st.emplace_back(c, 0u);
-      } else {
-        out.push_back(top.first);
-        st.pop_back();
-      }
-    }
+    if (P.has_pp[x]) ecost[x] += 0.3;
+  std::vector<double> sw(ecost), bl(n, 0.0);
+  for (int x = n - 1; x >= 1; --x) sw[par[x]] += sw[x];
+  for (int x = 0; x < n; ++x) bl[x] = ecost[x] + (x ? bl[par[x]] : 0.0);
+
+  // ---- 1. tasks ---------------------------------------------------------------------------
+  struct Task {
+    std::vector<int32_t> nodes;  // in visiting order, top node last
+    int ptask = -1, pending = 0, warp = -1;
+    double cost = 0.0, ready = 0.0, prio = 0.0, t0 = 0.0;
   };
-  P.order.clear();
-  P.order.reserve(n);
-  P.task.assign(W + 1, HTask());
-  for (int w = 0; w < W; ++w) {
-    P.task[w].p0 = (int)P.order.size();
-    for (int32_t x : frontier)
-      if (owner[x] == w) post_order(x, P.order);
-    P.task[w].p1 = (int)P.order.size();
-  }
-  P.task[W].p0 = (int)P.order.size();
-  post_order(0, P.order);
-  P.task[W].p1 = (int)P.order.size();
-  if ((int)P.order.size() != n) return fail(CN_ERR_TOPOLOGY, "internal: tape order incomplete");
-  P.pos_of.assign(n, 0);
-  for (int j = 0; j < n; ++j) P.pos_of[P.order[j]] = j;
-  // exchange slots: the cut children of a top node get consecutive slots, in top visiting order
-  std::vector<int32_t> slot_of(n, -1), imp_first(n, 0), imp_cnt(n, 0);
-  {
-    int ns = 0;
-    for (int j = P.task[W].p0; j < P.task[W].p1; ++j) {
-      const int x = P.order[j];
-      imp_first[x] = ns;
-      for (int32_t c : ch[x])
-        if (is_cut[c]) {
-          slot_of[c] = ns++;
-          imp_cnt[x]++;
+  std::vector<Task> tasks;
+  std::vector<int32_t> task_of(n, -1);
+  const double gran = W > 1 ? sw[0] / (4.0 * W) : 1e300;
+  for (int x = 0; x < n; ++x) {
+    if (sw[x] > gran) {  // upper node: a task of its own
+      task_of[x] = (int)tasks.size();
+      tasks.emplace_back();
+      tasks.back().nodes.push_back(x);
+    } else if (x == 0 || sw[par[x]] > gran) {  // root of a small subtree: depth-first post-order
+      const int id = (int)tasks.size();
+      tasks.emplace_back();
+      std::vector<std::pair<int32_t, uint32_t>> st;
+      st.emplace_back(x, 0u);
+      while (!st.empty()) {
+        auto &top = st.back();
+        auto &c = ch[top.first];
+        if (top.second == 0 && c.size() > 1)
+          std::stable_sort(c.begin(), c.end(), [&](int p, int q) { return sw[p] < sw[q]; });
+        if (top.second < c.size()) {
+          const int32_t y = c[top.second++];
+          st.emplace_back(y, 0u);
+        } else {
+          tasks[id].nodes.push_back(top.first);
+          task_of[top.first] = id;
+          st.pop_back();
         }
+      }
     }
-    P.n_xs = ns;
   }
-  // ---- records: rows of every node on the tape / scratch tape, per task -----------------------
-  P.row.assign(n, 0);
-  P.srow.assign(n, 0);
-  P.flags.assign(n, 0);
-  P.mask.assign(n, 0);
-  P.ring.assign(n, 0);
-  P.cai_row.assign(n, -1);
-  P.pp_row.assign(n, -1);
-  std::vector<uint32_t> len(n, 0), slen(n, 0);
-  uint32_t row = 0, srow_base = 0;
-  int max_len = 0, depth = 1;
-  for (int w = 0; w <= W; ++w) {
-    HTask &Tk = P.task[w];
-    Tk.row0 = row;
-    for (int j = Tk.p0; j < Tk.p1; ++j) {
-      const int x = P.order[j];
-      uint32_t fl = 0, r = row + 5, sl = 2;
-      if (x == 0) {
-        fl |= PG_ROOT;
-      } else if (!is_cut[x]) {
-        const auto &sib = tch[par[x]];
-        if (sib.back() == x) fl |= PG_FWD;
-        else if (sib.front() == x) fl |= PG_PUSH;
-        else fl |= PG_ADD;
-      }  // a cut subtree root has kind 0 without PG_ROOT: it exports to its slot
-      if (!tch[x].empty()) fl |= PG_FWD_IN;
-      if (tch[x].size() >= 2) fl |= PG_POP;
-      if (P.has_pp[x]) {
-        fl |= PG_HAS_PP;
-        P.pp_row[x] = (int32_t)r;
-        r += 2;
-      }
-      if (need_ica[x]) {
-        fl |= PG_NEED_ICA;
-        sl += 1;
-      }
-      if (has_cai[x]) {
-        fl |= PG_HAS_CAI;
-        P.cai_row[x] = (int32_t)r;
-        r += 1;
-        sl += 1;
-      }
-      for (int t = 0; t < nt; ++t)
-        if (node_mask[x] & (1u << t)) {
-          const HTable &T = m->tab[t];
-          P.tab_row[t][x] = (int32_t)r;
-          r += (uint32_t)tape_rows_of(T.ti, T.type);
-          sl += (uint32_t)T.ti.n_state;
+  const int ntask = (int)tasks.size();
+  for (int id = 0; id < ntask; ++id) {
+    Task &T = tasks[id];
+    const int top = T.nodes.back();
+    for (int32_t x : T.nodes) T.cost += ecost[x];
+    T.prio = bl[top];
+    T.ptask = top ? task_of[par[top]] : -1;
+  }
+  // ---- list scheduling (two passes: the second one knows the mechanism load of each warp) ----
+  std::vector<double> mload(W, 0.0), t_end(n, 0.0), mt_end(n, 0.0);
+  std::vector<int> e_warp(n, 0), m_warp(n, -1);
+  std::vector<std::vector<int32_t>> elist(W), mlist(W);
+  for (int pass = 0; pass < 2; ++pass) {
+    for (Task &T : tasks) { T.pending = 0; T.warp = -1; T.ready = 0.0; }
+    for (const Task &T : tasks)
+      if (T.ptask >= 0) tasks[T.ptask].pending++;
+    std::vector<double> wt(mload);
+    std::vector<int> last(W, -1);
+    for (auto &l : elist) l.clear();
+    for (int done = 0; done < ntask; ++done) {
+      // the earliest free warp; among equals one that can continue with the parent of its last task
+      auto affinity = [&](int w) {
+        if (last[w] < 0) return -1;
+        const int pt = tasks[last[w]].ptask;
+        if (pt >= 0 && tasks[pt].warp < 0 && tasks[pt].pending == 0 &&
+            tasks[pt].ready <= wt[w] + 1e-9)
+          return pt;
+        return -1;
+      };
+      int w = 0;
+      for (int u = 1; u < W; ++u)
+        if (wt[u] < wt[w] - 1e-9 || (std::fabs(wt[u] - wt[w]) <= 1e-9 && affinity(w) < 0 &&
+                                     affinity(u) >= 0))
+          w = u;
+      int cand = affinity(w);
+      if (cand < 0) {
+        int best_now = -1, best_later = -1;
+        for (int id = 0; id < ntask; ++id) {
+          const Task &T = tasks[id];
+          if (T.warp >= 0 || T.pending > 0) continue;
+          if (T.ready <= wt[w] + 1e-9) {
+            if (best_now < 0 || T.prio > tasks[best_now].prio) best_now = id;
+          } else if (best_later < 0 || T.ready < tasks[best_later].ready - 1e-9 ||
+                     (T.ready <= tasks[best_later].ready + 1e-9 &&
+                      T.prio > tasks[best_later].prio)) {
+            best_later = id;
+          }
         }
-      uint32_t ln = r - row;
-      if (ln > R - CH || sl > R - CH) return give_up();  // a record must fit the ring
-      const uint32_t rel = row - Tk.row0;
-      if (rel % R + ln > R) {  // a record never wraps around the ring: pad to the next lap
-        const uint32_t pad = R - rel % R;
-        len[j - 1] += pad;     // the pad rows ride with the previous record (j > p0 here)
-        if (len[j - 1] > R - CH) return give_up();
-        for (int t = 0; t < nt; ++t)
-          if (P.tab_row[t].size() && P.tab_row[t][x] >= 0) P.tab_row[t][x] += (int32_t)pad;
-        if (P.cai_row[x] >= 0) P.cai_row[x] += (int32_t)pad;
-        if (P.pp_row[x] >= 0) P.pp_row[x] += (int32_t)pad;
-        row += pad;
-        r += pad;
+        if (best_now < 0 && best_later >= 0) {
+          // nothing to do yet: wait until the next task becomes ready, then decide again (the warp
+          // that completes its last child may want to continue with it)
+          bool other_busy = false;
+          for (int u = 0; u < W; ++u)
+            if (u != w && wt[u] > wt[w] + 1e-9) other_busy = true;
+          if (other_busy && wt[w] < tasks[best_later].ready - 1e-9) {
+            wt[w] = tasks[best_later].ready;
+            --done;
+            continue;
+          }
+        }
+        cand = best_now >= 0 ? best_now : best_later;
       }
-      max_len = std::max(max_len, (int)std::max(ln, sl));
-      P.row[j] = row;
-      P.flags[j] = fl;
-      P.mask[j] = node_mask[x] | (uint32_t)(is_cut[x] ? slot_of[x] : imp_first[x]) << 20 |
-                  (uint32_t)imp_cnt[x] << 28;
-      len[j] = ln;
-      slen[j] = sl;
-      row = r;
+      if (cand < 0) return fail(CN_ERR_TOPOLOGY, "internal: tape scheduler found no task");
+      Task &T = tasks[cand];
+      T.warp = w;
+      T.t0 = std::max(wt[w], T.ready);
+      double t = T.t0;
+      for (int32_t x : T.nodes) {
+        t += ecost[x];
+        t_end[x] = t;
+        e_warp[x] = w;
+        elist[w].push_back(x);
+      }
+      wt[w] = t;
+      last[w] = cand;
+      if (T.ptask >= 0) {
+        tasks[T.ptask].pending--;
+        tasks[T.ptask].ready = std::max(tasks[T.ptask].ready, t);
+      }
+    }
+    P.sim_makespan = *std::max_element(wt.begin(), wt.end());
+    if (pass == 1) break;
+    // ---- 2. mechanism records: in the order the elimination needs them, to the least loaded ----
+    std::vector<int32_t> mn;
+    for (int x = 0; x < n; ++x)
+      if (node_mask[x]) mn.push_back(x);
+    if (mn.empty()) break;
+    std::stable_sort(mn.begin(), mn.end(), [&](int p, int q) { return t_end[p] < t_end[q]; });
+    for (int32_t x : mn) {
+      const int w = (int)(std::min_element(mload.begin(), mload.end()) - mload.begin());
+      mload[w] += mcost[x];
+      mt_end[x] = mload[w];
+      m_warp[x] = w;
+      mlist[w].push_back(x);
+    }
+  }
+  P.sim_work = sw[0];
+  for (int x = 0; x < n; ++x) P.sim_work += mcost[x];
+
+  // ---- 3. records, hand-over kinds, dependencies ----------------------------------------------
+  struct Rec {
+    int type = 0;      // 0 ELIM, 1 MECH
+    int32_t node = 0;
+    uint32_t flags = 0;
+    std::vector<std::pair<int, int>> deps;  // (warp, pre-index) this record waits for, forward
+    int bw_warp = -1, bw_pre = -1;          // backward: the parent's record on another warp
+    int fidx = 0;                           // index in the final list (WAIT records included)
+    uint32_t row = 0, len = 0;
+    bool padded = false;                    // pad rows precede the record on the tape
+  };
+  std::vector<std::vector<Rec>> recs(W);
+  std::vector<int> e_pre(n, -1), m_pre(n, -1);  // pre-index of a node's records in its warp's list
+  for (int w = 0; w < W; ++w) {
+    for (int32_t x : mlist[w]) {
+      m_pre[x] = (int)recs[w].size();
+      Rec r;
+      r.type = 1;
+      r.node = x;
+      r.flags = RT_MECH | (has_cai[x] ? RM_HAS_CAI : 0) | (need_ica[x] ? RM_NEED_ICA : 0);
+      recs[w].push_back(r);
+    }
+    for (int32_t x : elist[w]) {
+      e_pre[x] = (int)recs[w].size();
+      Rec r;
+      r.node = x;
+      recs[w].push_back(r);
+    }
+  }
+  auto erec = [&](int x) -> Rec & { return recs[e_warp[x]][e_pre[x]]; };
+  std::vector<uint8_t> fwd(n, 0);
+  for (int w = 0; w < W; ++w)
+    for (size_t i = 0; i + 1 < elist[w].size(); ++i)
+      if (par[elist[w][i]] == elist[w][i + 1]) fwd[elist[w][i]] = 1;
+  auto add_dep = [&](Rec &r, int rw, int w2, int pre2) {
+    if (w2 == rw) return;  // program order
+    r.deps.emplace_back(w2, pre2);
+    recs[w2][pre2].flags |= RF_SIG_F;
+  };
+  for (int x = 0; x < n; ++x) {
+    Rec &r = erec(x);
+    if (x == 0) r.flags |= RK_ROOT;
+    else if (fwd[x]) r.flags |= RK_FWD;
+    if (P.has_pp[x]) r.flags |= RF_HAS_PP;
+    if (node_mask[x]) r.flags |= RF_MECHV;
+    // contributors to x's system row: its mechanism record first, then the children that do not
+    // hand over in registers, in the order of the simulated schedule
+    std::vector<int32_t> cs;
+    for (int32_t c : ch[x]) {
+      if (fwd[c]) r.flags |= RF_FWD_IN;
+      else cs.push_back(c);
+    }
+    std::stable_sort(cs.begin(), cs.end(), [&](int p, int q) {
+      if (t_end[p] != t_end[q]) return t_end[p] < t_end[q];
+      if (e_warp[p] != e_warp[q]) return e_warp[p] < e_warp[q];
+      return e_pre[p] < e_pre[q];
+    });
+    int lw = -1, lp = -1;  // last contributor so far
+    if (node_mask[x]) {
+      lw = m_warp[x];
+      lp = m_pre[x];
+    }
+    for (int32_t c : cs) {
+      Rec &rc = erec(c);
+      rc.flags |= lw < 0 ? RK_STORE : RK_ADD;
+      if (lw >= 0) add_dep(rc, e_warp[c], lw, lp);
+      lw = e_warp[c];
+      lp = e_pre[c];
+      // backward: c reads v of x from x's system row
+      if (e_warp[c] != e_warp[x]) {
+        rc.bw_warp = e_warp[x];
+        rc.bw_pre = e_pre[x];
+        rc.flags |= RF_WAIT_B;
+        r.flags |= RF_SIG_B;
+      }
+    }
+    if (lw >= 0) {
+      r.flags |= RF_HAS_ACC;
+      add_dep(r, e_warp[x], lw, lp);
+    }
+  }
+  // ---- 4. tape rows: each warp's records get consecutive rows, padded so that no record wraps
+  // around the warp's ring; system rows in the same order ----------------------------------------
+  P.order.clear();
+  P.pos_of.assign(n, 0);
+  P.row.assign(n, 0);
+  P.cai_row.assign(n, -1);
+  P.ica_row.assign(n, -1);
+  P.pp_row.assign(n, -1);
+  P.vcopy_row.assign(n, -1);
+  P.task.assign(W, HTask());
+  P.prog.clear();
+  for (int w = 0; w < W; ++w)
+    for (int32_t x : elist[w]) {
+      P.pos_of[x] = (int32_t)P.order.size();
+      P.order.push_back(x);
+    }
+  uint32_t row = 0;
+  for (int w = 0; w < W; ++w) {
+    HTask &Tk = P.task[w];
+    Tk.pm = (int)mlist[w].size();
+    Tk.row0 = row;
+    bool m_open = true;
+    Tk.mrows = 0;
+    for (Rec &r : recs[w]) {
+      const int x = r.node;
+      uint32_t ln;
+      if (r.type == 1) {
+        ln = 1 + (has_cai[x] ? 1 : 0) + (need_ica[x] ? 1 : 0);
+        for (int t = 0; t < nt; ++t)
+          if (node_mask[x] & (1u << t)) ln += (uint32_t)tape_rows_of(m->tab[t].ti, m->tab[t].type);
+      } else {
+        ln = 5 + (P.has_pp[x] ? 2 : 0);
+      }
+      if (ln > R - CH || ln > 255) return give_up();  // a record must fit the ring
+      const uint32_t rel = row - Tk.row0;
+      r.padded = false;
+      if (rel % R + ln > R) {  // a record never wraps around the ring: pad to the next lap
+        row += R - rel % R;
+        r.padded = true;
+      }
+      if (r.type == 0 && m_open) {
+        Tk.mrows = row - Tk.row0;
+        m_open = false;
+      }
+      r.row = row;
+      r.len = ln;
+      row += ln;
+      if (r.type == 1) {
+        uint32_t q = r.row;
+        P.vcopy_row[x] = (int32_t)q++;
+        if (has_cai[x]) P.cai_row[x] = (int32_t)q++;
+        if (need_ica[x]) P.ica_row[x] = (int32_t)q++;
+        for (int t = 0; t < nt; ++t)
+          if (node_mask[x] & (1u << t)) {
+            P.tab_row[t][x] = (int32_t)q;
+            q += (uint32_t)tape_rows_of(m->tab[t].ti, m->tab[t].type);
+          }
+      } else {
+        P.row[P.pos_of[x]] = r.row;
+        if (P.has_pp[x]) P.pp_row[x] = (int32_t)(r.row + 5);
+      }
     }
     Tk.nrows = row - Tk.row0;
-    // the scratch segment of the task is written back to front
-    Tk.srow0 = srow_base;
-    uint32_t sr = 0;
-    for (int j = Tk.p1 - 1; j >= Tk.p0; --j) {
-      if (sr % R + slen[j] > R) {
-        const uint32_t pad = R - sr % R;
-        slen[j + 1] += pad;
-        if (slen[j + 1] > R - CH) return give_up();
-        sr += pad;
-      }
-      P.srow[j] = srow_base + sr;
-      P.ring[j] = ((P.row[j] - Tk.row0) % R) * 256u | ((sr % R) * 256u) << 16;
-      sr += slen[j];
-    }
-    Tk.nsrows = sr;
-    srow_base += sr;
-    // chunk bookkeeping of the ring, precomputed: how many chunks a node must wait for before
-    // its rows are complete and how many are fully consumed after it, in both directions
-    int last = -1, next = 0;
-    for (int j = Tk.p0; j < Tk.p1; ++j) {
-      const uint32_t rel = P.row[j] - Tk.row0;
-      const int cl = (int)((rel + len[j] - 1) / CH), cn = (int)((rel + len[j]) / CH);
-      P.flags[j] |= (uint32_t)(cl - last) << 8 | (uint32_t)(cn - next) << 12 | len[j] << 24;
-      last = cl;
-      next = cn;
-    }
-    last = -1;
-    next = 0;
-    for (int j = Tk.p1 - 1; j >= Tk.p0; --j) {
-      const uint32_t rel = P.srow[j] - Tk.srow0;
-      const int cl = (int)((rel + slen[j] - 1) / CH), cn = (int)((rel + slen[j]) / CH);
-      P.flags[j] |= (uint32_t)(cl - last) << 16 | (uint32_t)(cn - next) << 20;
-      last = cl;
-      next = cn;
-    }
-    // stack depth by simulation of the forward pass
-    int sp = 0;
-    for (int j = Tk.p0; j < Tk.p1; ++j) {
-      const uint32_t fl = P.flags[j];
-      if (fl & PG_POP) --sp;
-      if ((fl & PG_KIND) == PG_PUSH) depth = std::max(depth, ++sp);
-    }
-    if (sp != 0) return fail(CN_ERR_TOPOLOGY, "internal: unbalanced tape program");
+    if (m_open) Tk.mrows = Tk.nrows;
+    if (row > 65535) return give_up();  // 16-bit tape rows
   }
   P.n_rows = (int)row;
-  P.n_srows = (int)srow_base;
-  P.depth = depth;
-  m->tape_max_len = std::max(m->tape_max_len, max_len);
+  // final lists: WAIT records go in front of the record that needs them (a wait that an earlier
+  // wait of the same warp already covers is dropped: positions on one warp only grow); plain
+  // chain nodes that follow one another on the tape are merged into RUN records
+  struct Fin { int type; int pre; int cnt; int w2, pre2; };  // type 2 = WAIT, 3 = RUN
+  std::vector<std::vector<Fin>> fin(W);
+  for (int w = 0; w < W; ++w) {
+    std::vector<int> seen(W, -1);
+    for (int i = 0; i < (int)recs[w].size(); ++i) {
+      Rec &r = recs[w][i];
+      bool waited = false;
+      for (auto &d : r.deps) {
+        if (seen[d.first] >= d.second) continue;
+        seen[d.first] = d.second;
+        fin[w].push_back(Fin{2, -1, 0, d.first, d.second});
+        waited = true;
+      }
+      const bool plain = r.type == 0 && (r.flags & ~(uint32_t)RF_FWD_IN) == RK_FWD;
+      if (plain && !waited && !r.padded && !fin[w].empty() && fin[w].back().type == 3 &&
+          fin[w].back().cnt < 255 && (r.flags & RF_FWD_IN)) {
+        const Rec &prev = recs[w][i - 1];
+        if (prev.row + 5 == r.row && (r.row - P.task[w].row0) % R != 0) {  // not at a ring lap
+          r.fidx = (int)fin[w].size() - 1;
+          fin[w].back().cnt++;
+          continue;
+        }
+      }
+      r.fidx = (int)fin[w].size();
+      fin[w].push_back(Fin{plain ? 3 : r.type, i, 1, -1, -1});
+    }
+    if (fin[w].size() > 2047) return give_up();  // 12-bit backward positions
+  }
+  // backward waits: drop those an earlier (in backward order) wait of the same warp covers
+  for (int w = 0; w < W; ++w) {
+    std::vector<int> seen(W, -1);  // largest backward position waited for so far, per warp
+    for (int i = (int)recs[w].size() - 1; i >= 0; --i) {
+      Rec &r = recs[w][i];
+      if (r.bw_warp < 0) continue;
+      const int nrec2 = (int)fin[r.bw_warp].size();
+      const int posb = nrec2 + (nrec2 - recs[r.bw_warp][r.bw_pre].fidx);
+      if (seen[r.bw_warp] >= posb) {
+        r.flags &= ~(uint32_t)RF_WAIT_B;
+        r.bw_warp = -1;
+      } else {
+        seen[r.bw_warp] = posb;
+        r.bw_pre = posb;  // from here on: the position itself
+      }
+    }
+  }
+  // encoding (layout of the records: cn_device.cuh)
+  for (int w = 0; w < W; ++w) {
+    HTask &Tk = P.task[w];
+    Tk.p0 = (int)P.prog.size();
+    for (const Fin &F : fin[w]) {
+      if (F.type == 2) {
+        const int pos = recs[F.w2][F.pre2].fidx + 1;
+        P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)F.w2 | (uint32_t)pos << 16, 0u));
+        continue;
+      }
+      const Rec &r = recs[w][F.pre];
+      const int x = r.node;
+      const uint32_t rel = r.row - Tk.row0;
+      const uint32_t roff = (rel % R) * 256u;
+      if (F.type == 3) {
+        P.prog.push_back(make_uint4(roff | (uint32_t)F.cnt << 16 |
+                                        ((r.flags & RF_FWD_IN) ? 1u << 24 : 0u),
+                                    (uint32_t)RT_RUN, (uint32_t)P.pos_of[x],
+                                    r.row | (rel + r.len) << 16));
+      } else if (r.type == 1) {
+        P.prog.push_back(make_uint4(roff | r.len << 16, r.flags | r.row << 16,
+                                    (uint32_t)P.pos_of[x], node_mask[x]));
+      } else {
+        uint32_t ey = r.flags;
+        if (r.bw_warp >= 0) ey |= (uint32_t)r.bw_pre << 16 | (uint32_t)r.bw_warp << 28;
+        const uint32_t ez = (uint32_t)P.pos_of[x] | (uint32_t)(x ? P.pos_of[par[x]] : 0) << 10;
+        const uint32_t ew = r.row | (uint32_t)(node_mask[x] ? P.vcopy_row[x] : 0) << 16;
+        P.prog.push_back(make_uint4(roff | r.len << 16, ey, ez, ew));
+      }
+    }
+    Tk.p1 = (int)P.prog.size();
+  }
+
+  // ---- dry run: the W record lists with the kernel's wait / signal rules -------------------------
+  {
+    std::vector<int> pc(W), ctrv(W, 0), acc(n, 0);
+    std::vector<uint8_t> done_e(n, 0), done_m(n, 0);
+    for (int w = 0; w < W; ++w) pc[w] = P.task[w].p0;
+    bool progress = true;
+    while (progress) {
+      progress = false;
+      for (int w = 0; w < W; ++w) {
+        while (pc[w] < P.task[w].p1) {
+          const uint4 e = P.prog[pc[w]];
+          const uint32_t fl = e.y & 0xFFFFu;
+          if ((fl & RT_MASK) == RT_WAIT) {
+            if (ctrv[e.z & 0xFFFFu] < (int)(e.z >> 16)) break;
+          } else if ((fl & RT_MASK) == RT_RUN) {
+            for (uint32_t i = 0; i < ((e.x >> 16) & 255u); ++i) {
+              const int x = P.order[e.z + i];
+              if (node_mask[x] || acc[x] != 0 || !fwd[x] || ch[x].size() > 1 ||
+                  (ch[x].size() == 1 && (!done_e[ch[x][0]] || !fwd[ch[x][0]])) ||
+                  (ch[x].size() == 1) != (i > 0 || (e.x >> 24 & 1u)))
+                return fail(CN_ERR_TOPOLOGY, "internal: tape program (run)");
+              done_e[x] = 1;
+            }
+          } else if ((fl & RT_MASK) == RT_MECH) {
+            const int x = P.order[e.z & 1023u];
+            if (acc[x] != 0) return fail(CN_ERR_TOPOLOGY, "internal: tape program (mech order)");
+            acc[x] = 1;
+            done_m[x] = 1;
+          } else {
+            const int x = P.order[e.z & 1023u];
+            int want = node_mask[x] ? 1 : 0;
+            for (int32_t c : ch[x]) {
+              if (!done_e[c]) return fail(CN_ERR_TOPOLOGY, "internal: tape program (child order)");
+              if (!fwd[c]) ++want;
+            }
+            if (acc[x] != want || ((fl & RF_HAS_ACC) != 0) != (want > 0))
+              return fail(CN_ERR_TOPOLOGY, "internal: tape program (contributions)");
+            const uint32_t kind = fl & RK_KIND;
+            if (kind >= RK_STORE) {
+              const int p = P.order[(e.z >> 10) & 1023u];
+              if (p != par[x] || (kind == RK_STORE) != (acc[p] == 0))
+                return fail(CN_ERR_TOPOLOGY, "internal: tape program (store/add)");
+              acc[p]++;
+            }
+            done_e[x] = 1;
+          }
+          if (fl & RF_SIG_F) ctrv[w] = pc[w] - P.task[w].p0 + 1;
+          ++pc[w];
+          progress = true;
+        }
+      }
+    }
+    for (int w = 0; w < W; ++w)
+      if (pc[w] != P.task[w].p1) return fail(CN_ERR_TOPOLOGY, "internal: tape program deadlocks");
+    // backward
+    std::vector<uint8_t> done_b(n, 0);
+    for (int w = 0; w < W; ++w) pc[w] = P.task[w].p1 - 1;
+    std::fill(ctrv.begin(), ctrv.end(), 0);
+    progress = true;
+    while (progress) {
+      progress = false;
+      for (int w = 0; w < W; ++w) {
+        const HTask &Tk = P.task[w];
+        while (pc[w] >= Tk.p0 + Tk.pm) {
+          const uint4 e = P.prog[pc[w]];
+          const uint32_t fl = e.y & 0xFFFFu;
+          if ((fl & RT_MASK) == RT_RUN) {
+            for (int i = (int)((e.x >> 16) & 255u) - 1; i >= 0; --i) {
+              const int x = P.order[e.z + i];
+              if (!done_b[par[x]])
+                return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward run)");
+              done_b[x] = 1;
+            }
+          } else if ((fl & RT_MASK) == RT_ELIM) {
+            if ((fl & RF_WAIT_B) && ctrv[e.y >> 28] < (int)((e.y >> 16) & 0xFFFu)) break;
+            const int x = P.order[e.z & 1023u];
+            if (x && !done_b[par[x]])
+              return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward order)");
+            done_b[x] = 1;
+            if (fl & RF_SIG_B) ctrv[w] = (Tk.p1 - Tk.p0) + (Tk.p1 - pc[w]);
+          }
+          --pc[w];
+          progress = true;
+        }
+      }
+    }
+    for (int w = 0; w < W; ++w)
+      if (pc[w] >= P.task[w].p0 + P.task[w].pm)
+        return fail(CN_ERR_TOPOLOGY, "internal: tape program deadlocks (backward)");
+  }
   return CN_OK;
 }
 
@@ -832,19 +1049,20 @@ static int build_layout(cn_model *m) {
   int tape_min_group = 16;  // a ragged last group needs at least this many cells
   if (const char *e = std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = std::max(1, std::atoi(e));
   const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells);
-  m->tape_W = 2;
-  if (const char *e = std::getenv("CN_TAPE_W")) m->tape_W = std::min(4, std::max(1, std::atoi(e)));
-  m->tape_S = m->tape_W == 1 ? 8 : 4;
+  // W warps per group (CTA), each with a ring of S chunks x CH rows; the whole CTA must fit the
+  // 227 KB of shared memory next to the group's system (512 B per node)
+  m->tape_W = 8;
+  if (const char *e = std::getenv("CN_TAPE_W")) m->tape_W = std::min(16, std::max(1, std::atoi(e)));
+  m->tape_S = 4;
   m->tape_CH = 8;
-  if (const char *e = std::getenv("CN_TAPE_S")) {
-    const int v = std::atoi(e);
-    if (v == 4 || v == 8 || v == 16) m->tape_S = v;
-  }
-  if (const char *e = std::getenv("CN_TAPE_CH")) {
-    const int v = std::atoi(e);
-    if (v == 8 || v == 16) m->tape_CH = v;
-  }
-  if (m->tape_S * m->tape_CH > 128) m->tape_S = 128 / m->tape_CH;
+  auto pow2 = [](int v, int lo, int hi) {
+    int p = lo;
+    while (p * 2 <= v && p * 2 <= hi) p *= 2;
+    return p;
+  };
+  if (const char *e = std::getenv("CN_TAPE_S")) m->tape_S = pow2(std::atoi(e), 2, 16);
+  if (const char *e = std::getenv("CN_TAPE_CH")) m->tape_CH = pow2(std::atoi(e), 4, 32);
+  while (m->tape_S * m->tape_CH > 128) m->tape_S /= 2;  // 16-bit ring offsets
   m->cell_tape.assign(nc, 0);
   for (HClass &K : m->cls) {
     K.count = (int64_t)K.cells.size();
@@ -872,12 +1090,21 @@ static int build_layout(cn_model *m) {
     int rc = build_tape_program(m, K);
     if (rc != CN_OK) return rc;
     if (K.tp.n_groups == 0) continue;
+    // the CTA must fit: rings + system + two program buffers + counters and barriers
+    const size_t sys_cap = (size_t)std::max(m->tape_sys_cap, K.n);
+    const size_t prog_cap = std::max((size_t)m->tape_prog_cap, K.tp.prog.size());
+    const size_t need = (size_t)m->tape_W * m->tape_S * m->tape_CH * 256 + sys_cap * 512 +
+                        2 * prog_cap * 16 + 64 + ((size_t)m->tape_W * m->tape_S + 2) * 8;
+    if (need > 227 * 1024) {
+      K.tp.n_groups = 0;
+      K.tp.n_cells = 0;
+      continue;
+    }
     for (int64_t q = 0; q < K.tp.n_cells; ++q) m->cell_tape[K.cells[q]] = 1;
     K.tp.prog_off = prog_total;
-    prog_total += K.n;
-    m->tape_prog_cap = std::max(m->tape_prog_cap, K.n);
-    m->tape_stack_cap = std::max(m->tape_stack_cap, K.tp.depth);
-    m->tape_xs_cap = std::max(m->tape_xs_cap, K.tp.n_xs);
+    prog_total += (int)K.tp.prog.size();
+    m->tape_prog_cap = std::max(m->tape_prog_cap, (int)K.tp.prog.size());
+    m->tape_sys_cap = std::max(m->tape_sys_cap, K.n);
   }
 
   // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
@@ -967,14 +1194,13 @@ static int build_layout(cn_model *m) {
   m->n_ab = ab_base;
   m->n_cgroup = (int)m->grp.size();
   const int ngc = m->n_cgroup;
-  int64_t tape_base = 0, scratch_base = 0;
+  int64_t tape_base = 0;
   for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
     HClass &K = m->cls[kc];
     for (int gq = 0; gq < K.tp.n_groups; ++gq) {
       TapeGroup tg{};
       tg.cls = kc;
       tg.tape_base = tape_base;
-      tg.scratch_base = scratch_base;
       tg.cell_base = cell_base;
       tg.ncell = (int32_t)std::min<int64_t>(32, K.tp.n_cells - (int64_t)gq * 32);
       const int gidx = ngc + (int)m->tgrp.size();
@@ -989,12 +1215,10 @@ static int build_layout(cn_model *m) {
       }
       m->tgrp.push_back(tg);
       tape_base += (int64_t)K.tp.n_rows * 32;
-      scratch_base += (int64_t)K.tp.n_srows * 32;
       cell_base += 32;
     }
   }
   m->n_tape = tape_base;
-  m->n_scratch = scratch_base;
   if (m->n_tape >= ((int64_t)1 << 32))
     return fail(CN_ERR_UNSUPPORTED, "tape larger than 2^32 doubles");
   m->n_pcell = cell_base;
@@ -1168,6 +1392,13 @@ static int finalize(cn_model *m, double dt) {
     for (int j = 0; j < m->cls[tg.cls].n; ++j)
       for (int l = tg.ncell; l < 32; ++l) tape[tg.tape_base + ((int64_t)P.row[j] + 2) * 32 + l] = 1.0;
   }
+  for (const TapeGroup &tg : m->tgrp) {  // the copy of v at the head of every mechanism record
+    const HTape &P = m->cls[tg.cls].tp;
+    for (int i = 0; i < m->cls[tg.cls].n; ++i)
+      if (P.vcopy_row[i] >= 0)
+        for (int l = 0; l < 32; ++l)
+          tape[tg.tape_base + (int64_t)P.vcopy_row[i] * 32 + l] = m->v_init;
+  }
   if (m->any_cai)
     for (int32_t c = 0; c < m->n_cell; ++c) {
       if (!m->cell_tape[c]) continue;
@@ -1340,36 +1571,37 @@ static int finalize(cn_model *m, double dt) {
       D.cls_cnt = T.d_cls_cnt; D.cls_nodeoff = T.d_cls_nodeoff; D.grp_instbase = T.d_grp_instbase;
     }
   }
-  // the arena (filled above, including the mechanism rows of the tapes), scratch, programs
+  // the arena (filled above, including the mechanism rows of the tapes) and the programs
   {
     UP(v0, m->d_v);
     H.v = m->d_v;
     H.tape = m->d_v + m->n_ab;
-    rc = dev_alloc(m, (size_t)std::max<int64_t>(m->n_scratch, 1), &H.scratch, false);
-    if (rc != CN_OK) return rc;
     std::vector<TapeClass> tcls(m->cls.size());
-    std::vector<TapeTask> ttask(m->cls.size() * (size_t)(m->tape_W + 1));
+    std::vector<TapeTask> ttask(m->cls.size() * (size_t)m->tape_W);
     std::vector<uint4> prog;
     for (size_t kc = 0; kc < m->cls.size(); ++kc) {
       const HClass &K = m->cls[kc];
       const HTape &P = K.tp;
-      tcls[kc] = TapeClass{K.n, P.prog_off, P.n_rows, P.n_srows, P.depth, P.n_xs, 0, 0};
+      tcls[kc] = TapeClass{K.n, P.prog_off, (int32_t)P.prog.size(), P.n_rows};
       if (P.n_groups == 0) continue;
-      for (int j = 0; j < K.n; ++j)
-        prog.push_back(make_uint4(P.ring[j], P.srow[j] * 32u, P.flags[j], P.mask[j]));
-      for (int w = 0; w <= m->tape_W; ++w) {
+      if ((int)prog.size() != P.prog_off) return fail(CN_ERR_ARG, "internal: program offsets");
+      prog.insert(prog.end(), P.prog.begin(), P.prog.end());
+      for (int w = 0; w < m->tape_W; ++w) {
         const HTask &Tk = P.task[w];
-        ttask[kc * (size_t)(m->tape_W + 1) + w] =
-            TapeTask{Tk.p0, Tk.p1, Tk.row0, Tk.nrows, Tk.srow0, Tk.nsrows, 0, 0};
+        // program positions are relative to the class's program (as it sits in shared memory)
+        ttask[kc * (size_t)m->tape_W + w] =
+            TapeTask{Tk.p0, Tk.p1, Tk.pm, 0, Tk.row0, Tk.nrows, Tk.mrows, 0};
       }
     }
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
     UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg); UP(ttask, dtt);
     H.tgrp = dtg; H.tcls = dtc; H.prog = dpg; H.ttask = dtt;
     H.tape_W = m->tape_W;
-    H.tape_xs_cap = std::max(m->tape_xs_cap, 1);
+    H.tape_S = m->tape_S;
+    H.tape_lgCH = 0;
+    while ((1 << H.tape_lgCH) < m->tape_CH) H.tape_lgCH++;
     H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
-    H.tape_stack_cap = std::max(m->tape_stack_cap, 1);
+    H.tape_sys_cap = std::max(m->tape_sys_cap, 1);
     for (int t = 0; t < nt; ++t) {
       H.tab[t].pp_tape_begin = m->tab[t].pp_tape_begin;
       H.tab[t].pp_tape_end = m->tab[t].ti.point ? m->tab[t].n : 0;
@@ -1476,33 +1708,34 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
 
 static size_t tape_smem_bytes(const cn_model *m) {
   const size_t W = (size_t)m->tape_W;
-  return W * m->tape_S * m->tape_CH * 256 + (size_t)m->hm.tape_prog_cap * 16 +
-         W * m->hm.tape_stack_cap * 512 + (size_t)m->hm.tape_xs_cap * 512 +
-         W * (m->tape_S + 1) * 8;
+  return W * m->tape_S * m->tape_CH * 256 + (size_t)m->hm.tape_sys_cap * 512 +
+         2 * (size_t)m->hm.tape_prog_cap * 16 + 64 + (W * m->tape_S + 2) * 8;
 }
 
-template <int S, int CH>
-static cudaError_t launch_tape_t(cn_model *m, int64_t k) {
+// Persistent CTAs: as many as fit the device at once (shared memory decides), each looping over
+// the groups blockIdx.x, blockIdx.x + gridDim.x, ...
+static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
   const size_t smem = tape_smem_bytes(m);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(tape_step_kernel<S, CH>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  auto kern = m->tape_W <= 8 ? tape_step_kernel<256> : tape_step_kernel<512>;
+  if (m->tape_ctas == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         227 * 1024);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(tape_step_kernel<S, CH>,
-                             cudaFuncAttributePreferredSharedMemoryCarveout,
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout,
                              cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    int dev = 0, sms = 0, per_sm = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+      return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * m->tape_W, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    if (const char *s = std::getenv("CN_TAPE_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, std::atoi(s)));
+    m->tape_ctas = std::min(m->hm.n_tgroup, sms * per_sm);
   }
-  tape_step_kernel<S, CH><<<m->hm.n_tgroup, 32 * m->tape_W, smem, m->stream>>>(m->hm, k);
+  kern<<<m->tape_ctas, 32 * m->tape_W, smem, m->stream>>>(m->hm, k, mode);
   return cudaGetLastError();
-}
-
-static cudaError_t launch_tape(cn_model *m, int64_t k) {
-  if (m->tape_CH == 16) return m->tape_S == 8 ? launch_tape_t<8, 16>(m, k) : launch_tape_t<4, 16>(m, k);
-  if (m->tape_S == 16) return launch_tape_t<16, 8>(m, k);
-  return m->tape_S == 8 ? launch_tape_t<8, 8>(m, k) : launch_tape_t<4, 8>(m, k);
 }
 
 static int run_steps(cn_model *m, int64_t K) {
@@ -1542,8 +1775,9 @@ static int run_steps(cn_model *m, int64_t K) {
     }
     if (ntg > 0) {
       if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
-      cudaError_t e = launch_tape(m, k);
+      cudaError_t e = launch_tape(m, k, m->state_pending ? TM_ADVANCE : 0);
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
+      m->state_pending = true;
       if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
       m->launches++;
     }
@@ -1679,6 +1913,13 @@ extern "C" int cn_get_state(const cn_model *cm, int32_t t, int32_t s, double *ou
   if (s < 0 || s >= T.ti.n_state || n != T.n) return fail(CN_ERR_MECH, "state / size mismatch");
   if (!m->uploaded) return fail(CN_ERR_ARG, "states exist after the first cn_run");
   if (n == 0) return CN_OK;
+  if (m->state_pending && !T.ti.point && m->hm.n_tgroup > 0) {
+    // the interleaved kernel applies nrn_state of a step at the start of the next one: do it now
+    cudaError_t e = launch_tape(m, m->k, TM_ADVANCE | TM_FLUSH);
+    if (e != cudaSuccess) return fail(CN_ERR_CUDA, "state flush failed: %s", cudaGetErrorString(e));
+    m->launches++;
+    m->state_pending = false;
+  }
   // instances live in the table arrays (cooperative groups) or on a tape (interleaved groups)
   std::vector<int64_t> loc((size_t)n);
   for (int64_t i = 0; i < n; ++i) {
@@ -1727,8 +1968,8 @@ extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
   info[3] = r;
   info[4] = (int64_t)m->tgrp.size();
   info[5] = m->n_tape * 8;
-  info[6] = m->n_scratch * 8;
-  info[7] = m->tape_stack_cap;
+  info[6] = 0;  // no scratch tape: the system of a group lives in shared memory
+  info[7] = m->tape_W;
   return CN_OK;
 }
 
@@ -1787,6 +2028,10 @@ extern "C" int cn_debug_tasks(const cn_model *m, int32_t *out, int32_t cap) {
     int n = 0;
     for (const HTask &t : K.tp.task) {
       if (n + 2 <= cap) { out[n++] = t.p1 - t.p0; out[n++] = (int32_t)t.nrows; }
+    }
+    if (n + 2 <= cap) {  // simulated makespan and total work of the schedule, x100
+      out[n++] = (int32_t)(K.tp.sim_makespan * 100.0);
+      out[n++] = (int32_t)(K.tp.sim_work * 100.0);
     }
     return n;
   }

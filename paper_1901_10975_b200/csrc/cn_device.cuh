@@ -58,37 +58,59 @@ struct ClassInfo {
 // ---- interleaved ("tape") groups: 32 same-shape cells, one lane per cell (cn_tape.cuh) ----------
 struct TapeGroup {
   int64_t tape_base;     // first element of the group's tape (multiple of 32 doubles)
-  int64_t scratch_base;  // first element of the group's scratch tape
-  int32_t cls, cell_base, ncell, pad;
+  int32_t cls, cell_base, ncell, pad0;
+  int64_t pad1;
 };
 
 struct TapeClass {
-  int32_t n, prog_off, n_rows, n_srows;
-  int32_t depth, n_xs, pad1, pad2;
+  int32_t n, prog_off, prog_len, n_rows;
 };
 
-// one task of a class: a range of program positions with its own tape / scratch-tape segment
+// the part of a class's program that one warp runs: records [p0, p1) (the first pm of them are
+// mechanism records) and its segment of the group's tape (the first mrows rows hold the
+// mechanism records)
 struct TapeTask {
-  int32_t p0, p1;
-  uint32_t row0, nrows, srow0, nsrows;
-  int32_t pad0, pad1;
+  int32_t p0, p1, pm, pad0;
+  uint32_t row0, nrows, mrows, pad1;
 };
 
-// program entry flags (layout of the uint4 entry: see tape_step_kernel).  Kind 0 without PG_ROOT
-// is the root of a cut subtree: it exports its contribution to an exchange slot.
-enum { PG_FWD = 1, PG_PUSH = 2, PG_ADD = 3, PG_KIND = 3, PG_FWD_IN = 4, PG_POP = 8, PG_ROOT = 16,
-       PG_HAS_PP = 32, PG_HAS_CAI = 64, PG_NEED_ICA = 128 };
+// Program record (uint4) of the interleaved kernel: one per run of plain chain nodes (RUN), per
+// other node elimination (ELIM), per node with distributed mechanisms (MECH) and per cross-warp
+// dependency (WAIT).  Rows are counted from the start of the warp's segment of the tape.
+//   RUN   x = ring byte offset of the first node's record (16) | nodes in the run (8) | first
+//             node takes a contribution in registers (bit 24)
+//         y = RT_RUN     z = system row of the first node     w = first tape row of the first
+//             node's record (16, relative to the group) | row count of the segment up to and
+//             including the first node's record (16)
+//   ELIM  x = ring byte offset (16) | rows of the record (8)
+//         y = flags (16) | backward wait: position (12) and warp (4)
+//         z = own system row (10) | parent's system row (10)
+//         w = first tape row of the record (16) | tape row of the v copy in the node's mechanism
+//             record (16)
+//   MECH  x = ring byte offset (16) | rows of the record (8)
+//         y = flags (16) | first tape row of the record (16)
+//         z = system row of the node     w = mask of the distributed tables on the node
+//   WAIT  y = RT_WAIT    z = warp (16) | position (16)
+enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
+       RF_FWD_IN = 4,     // the previous record of this warp handed its contribution in registers
+       RF_HAS_ACC = 8,    // contributions (mechanisms, children) wait in the node's own system row
+       RF_HAS_PP = 16,    // two dynamic rows (conductance, current of point processes)
+       RF_MECHV = 32,     // the node has a mechanism record: v is also stored to its v copy
+       RF_SIG_F = 64,     // publish this warp's position after the record, forward / backward
+       RF_SIG_B = 128,
+       RF_WAIT_B = 256,   // backward: wait for the parent's warp first
+       RM_HAS_CAI = 1, RM_NEED_ICA = 2,
+       RT_ELIM = 0, RT_MECH = 1 << 14, RT_WAIT = 2 << 14, RT_RUN = 3 << 14, RT_MASK = 3 << 14 };
 
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
-  int32_t n_tgroup, tape_prog_cap, tape_stack_cap, tape_xs_cap;
-  int32_t tape_W, pad_t0, pad_t1, pad_t2;
+  int32_t n_tgroup, tape_prog_cap, tape_sys_cap, tape_W;
+  int32_t tape_S, tape_lgCH, pad_t1, pad_t2;  // ring: S stages (power of 2) of 2^lgCH rows
   const TapeGroup *tgrp;
   const TapeClass *tcls;
-  const TapeTask *ttask;        // [n_class][tape_W + 1]: leaf task of every warp, then the top task
+  const TapeTask *ttask;        // [n_class][tape_W]
   const uint4 *prog;
   double *tape;                 // == v + n_ab: one arena, so node positions index both
-  double *scratch;
   const GroupInfo *grp;
   const ClassInfo *cls;
   const uint32_t *sched;        // per class: rounds * P entries, node | parent << 16

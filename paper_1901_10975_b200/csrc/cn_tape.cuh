@@ -1,26 +1,30 @@
-// cn_tape.cuh -- the interleaved step kernel: one warp integrates 32 cells of one shape class for
-// one dt, ONE LANE PER CELL ("one cell per thread", Fig. 5D), re-designed for B200:
+// cn_tape.cuh -- the interleaved step kernel: 32 cells of one shape class are integrated for one
+// dt with ONE LANE PER CELL ("one cell per thread", Fig. 5D), re-designed for B200:
 //
 //   * Every per-node quantity of the 32 cells is a ROW of 32 doubles (256 B).  All rows of a group
-//     are laid out in the order the elimination visits them -- a TAPE: per node a, b, static
-//     diagonal, static rhs, v, then the parameter and state rows of the mechanisms on that node.
-//     The kernel never computes an address from the tree: it reads the tape front to back.
-//   * The tape is staged through a shared-memory ring by 1-D TMA bulk copies
-//     (cp.async.bulk.shared.global + mbarrier complete_tx), S chunks of CH rows in flight per warp,
-//     issued by one lane; HBM latency is hidden by the ring, not by occupancy.
-//   * Nodes are visited in depth-first post-order (children before parents, L196), so a node's
-//     contribution to its parent stays in REGISTERS when the parent is next (chains), and goes
-//     through a small shared-memory stack at branch points (depth <= height in branch points).
-//     No per-node shared-memory system: the shared memory per warp is ring + stack + program.
-//   * Triangularisation (L66) writes the back-substitution multiplier and reduced rhs of every
-//     node to a SCRATCH tape in reverse order; back-substitution streams it back through the same
-//     ring (it is re-read within microseconds: L2-resident), computes v_new, runs nrn_state (L67)
-//     on the mechanisms of the node and detects threshold crossings at the root (L68).
-//   * Control is uniform across the warp: the per-class PROGRAM (one uint4 per node) says where
-//     the node's rows are, how it hands its contribution to the parent, and which mechanisms sit
-//     on it.  Lanes never diverge.
+//     are laid out in the order they are consumed -- a TAPE: per node a, b, static diagonal,
+//     static rhs, v (+ two dynamic rows for point processes); per node with distributed
+//     mechanisms a second record with a copy of v and the parameter / state rows.  The kernel
+//     never computes an address from the tree: it reads the tape front to back.
+//   * One CTA (W warps) owns one group at a time and loops over groups (persistent).  The linear
+//     system of the group lives in SHARED MEMORY for the whole step: triangularisation (L66)
+//     leaves (multiplier, reduced rhs) of every node there, back-substitution reads them back.
+//     Nothing but the tape is read from HBM and nothing but v and the states is written.
+//   * The tree is compiled by the host into W record lists (a static schedule of the elimination
+//     over W warps, children before parents, L196).  A chain hands its contribution to the parent
+//     in REGISTERS; at a branch point the contributions meet in the parent's system row.  Warps
+//     synchronise only through per-warp progress counters in shared memory (WAIT records).
+//   * Each warp streams its own segment of the tape through a shared-memory ring with 1-D TMA bulk
+//     copies (cp.async.bulk.shared.global + mbarrier complete_tx), S chunks of CH rows in flight,
+//     issued by one lane; the ring of a warp that has finished its part of a group already loads
+//     the next group while the back-substitution runs.
+//   * nrn_state (L67) of step k is evaluated at the start of step k+1, in the mechanism record,
+//     just before nrn_cur (L65) needs the states: same arithmetic on the same values (the new v
+//     and the old states), but the states are read and written once per step and the
+//     back-substitution carries no mechanism work.  cn_get_state runs the pending update first.
+//   * Control is uniform across a warp; lanes never diverge.
 // Point processes of these cells are evaluated by pp_tape_kernel (one thread per instance) which
-// adds conductance and current into two dynamic tape rows of the node (L60, L65).
+// adds conductance and current into the two dynamic rows of the node (L60, L65).
 #pragma once
 #include "cn_device.cuh"
 
@@ -54,6 +58,16 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "DONE:\n"
       "}" ::"r"(bar), "r"(parity)
       : "memory");
+}
+// per-warp progress counters (shared memory): release by one lane after __syncwarp, acquire by all
+__device__ __forceinline__ void ctr_publish(uint32_t addr, uint32_t val) {
+  asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(val) : "memory");
+}
+__device__ __forceinline__ void ctr_wait(uint32_t addr, uint32_t target) {
+  uint32_t x;
+  do {
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(x) : "r"(addr) : "memory");
+  } while ((int32_t)(x - target) < 0);
 }
 
 // Reciprocal to ~1 ulp without the special-case handling of an IEEE division: MUFU.RCP64H seed
@@ -95,408 +109,399 @@ __device__ __forceinline__ void hh_advance(double v, double q10dt, double &m, do
   n += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - n);
 }
 
-__device__ __forceinline__ void bar_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-__device__ __forceinline__ void bar_arrive(int id, int nthreads) {
-  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+enum { TM_ADVANCE = 1, TM_FLUSH = 2 };
+
+// One mechanism record: nrn_state of the previous step (if `mode & TM_ADVANCE`: the states on the
+// tape are still those the previous nrn_cur used) followed by nrn_cur of this step with the
+// advanced states.  rb = the record in the ring (this lane's column), trec = the same record on
+// the tape.  Row order: v copy, [cai], [ica of the previous step], then per table its parameter
+// and state rows.  Returns the row-normalised conductance / current sums in gD, gR.
+__device__ __forceinline__ void mech_record(const DModel &M, const unsigned char *rb,
+                                            double *__restrict__ trec, uint32_t fl,
+                                            uint32_t mask, int mode, double dt, double q10dt,
+                                            double &gD, double &gR) {
+#define CN_RD(base, i) (*reinterpret_cast<const double *>((base) + (uint32_t)(i) * 256u))
+  const bool adv = mode & TM_ADVANCE;
+  const double v = CN_RD(rb, 0);
+  uint32_t cur = 1, cai_row = 0, ica_row = 0;
+  double cai = 0.0, ica_prev = 0.0, ica = 0.0;
+  if (fl & RM_HAS_CAI) {
+    cai = CN_RD(rb, cur);
+    cai_row = cur++;
+  }
+  if (fl & RM_NEED_ICA) {
+    ica_prev = CN_RD(rb, cur);
+    ica_row = cur++;
+  }
+  gD = 0.0;
+  gR = 0.0;
+  for (uint32_t mk = mask; mk; mk &= mk - 1) {
+    const DTable &T = M.tab[__ffs(mk) - 1];
+    const unsigned char *mr = rb + cur * 256u;
+    switch (T.type) {
+      case T_HH: {
+        double m = CN_RD(mr, 5), h = CN_RD(mr, 6), nn = CN_RD(mr, 7);
+        if (adv) {
+          hh_advance(v, q10dt, m, h, nn);
+          trec[(cur + 5) * 32] = m;
+          trec[(cur + 6) * 32] = h;
+          trec[(cur + 7) * 32] = nn;
+        }
+        const double invc = CN_RD(mr, 4);
+        const double gna = CN_RD(mr, 0) * m * m * m * h;
+        const double n2 = nn * nn;
+        const double gk = CN_RD(mr, 1) * n2 * n2;
+        const double gl = CN_RD(mr, 2);
+        gD += (gna + gk + gl) * invc;
+        gR += (gna * T.glob[0] + gk * T.glob[1] + gl * CN_RD(mr, 3)) * invc;
+        cur += 8;
+        break;
+      }
+      case T_HHFORM: {
+        double ms = CN_RD(mr, 2), hs = CN_RD(mr, 3);
+        if (adv) {
+          double xinf, xtau;
+          if ((int)T.glob[0] > 0) {
+            hhform_gate(v, T.glob + 4, xinf, xtau);
+            ms = cnexp(ms, xinf, xtau, dt);
+            trec[(cur + 2) * 32] = ms;
+          }
+          if ((int)T.glob[1] > 0) {
+            hhform_gate(v, T.glob + 10, xinf, xtau);
+            hs = cnexp(hs, xinf, xtau, dt);
+            trec[(cur + 3) * 32] = hs;
+          }
+        }
+        const double g = CN_RD(mr, 0) * ipow(ms, (int)T.glob[0]) * ipow(hs, (int)T.glob[1]);
+        const double invc = CN_RD(mr, 1);
+        gD += g * invc;
+        gR += g * T.glob[2] * invc;
+        if (T.glob[3] != 0.0) ica += g * (v - T.glob[2]);
+        cur += 4;
+        break;
+      }
+      case T_SK: {
+        double z = CN_RD(mr, 2);
+        if (adv) {
+          const double ca = cai < 1e-9 ? 1e-9 : cai;
+          const double zinf = 1.0 / (1.0 + pow(T.glob[1] / ca, T.glob[2]));
+          z = cnexp(z, zinf, T.glob[3], dt);
+          trec[(cur + 2) * 32] = z;
+        }
+        const double g = CN_RD(mr, 0) * z;
+        const double invc = CN_RD(mr, 1);
+        gD += g * invc;
+        gR += g * T.glob[0] * invc;
+        cur += 3;
+        break;
+      }
+      case T_CADYN: {
+        // derivimplicit on a linear ODE: one Newton step of backward Euler is exact (L278)
+        if (adv) {
+          const double kappa = 1e4 * T.glob[0] / (2.0 * 96485.33212 * T.glob[1]);
+          cai = (cai + dt * (-kappa * ica_prev + T.glob[3] / T.glob[2])) / (1.0 + dt / T.glob[2]);
+          trec[cai_row * 32] = cai;
+        }
+        break;
+      }
+      default: break;  // PAS is folded into the static rows
+    }
+  }
+  if ((fl & RM_NEED_ICA) && !(mode & TM_FLUSH)) trec[ica_row * 32] = ica;
+#undef CN_RD
 }
 
-// One CTA = one group of 32 cells, W warps.  Warp w runs leaf task w (a set of whole subtrees);
-// warp 0 then runs the top task (the part of the tree above the cut, root included), after which
-// every warp back-substitutes its leaf task.  S stages of CH rows per warp; S * CH is a power of 2.
-//
-// Program entry (uint4, one per node in task order; built by the host, uniform per class):
-//   x = byte offset in the ring of the node's first tape row (low 16 bits) and of its first
-//       scratch row (high 16 bits), relative to the task's segments
-//   y = element offset of the node's scratch record on the group's scratch tape
-//   z = flags (8 bits) | chunks to wait for, forward (4) | chunks freed, forward (4)
-//       | chunks to wait for, backward (4) | chunks freed, backward (4) | tape rows (8)
-//   w = mask of the distributed mechanism tables with an instance on this node (20 bits)
-//       | exchange slot: own slot of a cut subtree root, first import slot of a top node (8 bits)
-//       | number of import slots (4 bits)
-template <int S, int CH>
-__global__ void __launch_bounds__(128, 4) tape_step_kernel(const __grid_constant__ DModel M,
-                                                        int64_t k) {
+// One CTA = W warps = one group of 32 cells at a time (persistent over groups).  See the header
+// of this file and the record layout in cn_device.cuh.
+// Shared memory: W rings of S << lgCH rows | system: tape_sys_cap x (32 + 32) doubles | two
+// program buffers of tape_prog_cap records | 16 progress counters | W*S + 2 mbarriers.
+template <int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constant__ DModel M,
+                                                          int64_t k, int mode) {
   extern __shared__ __align__(128) unsigned char sm_raw[];
-  constexpr uint32_t RB = S * CH * 256u;  // ring bytes per warp
-  static_assert((RB & (RB - 1)) == 0 && RB <= 65536u, "ring must be a power of two <= 64 KB");
-  static_assert((S & (S - 1)) == 0, "stages must be a power of two");
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int W = M.tape_W;
-  const int nthreads = W * 32;
+  const int W = M.tape_W, S = M.tape_S, lgCH = M.tape_lgCH, CH = 1 << lgCH;
+  const uint32_t RB = (uint32_t)(S << lgCH) * 256u;  // ring bytes per warp
   const uint32_t lane8 = (uint32_t)lane * 8u;
-  const TapeGroup tg = M.tgrp[blockIdx.x];
-  const TapeClass tc = M.tcls[tg.cls];
-  // shared memory: rings | program | stacks | exchange slots | mbarriers
-  const unsigned char *ringc = sm_raw + (size_t)warp * RB;
-  uint4 *prog = reinterpret_cast<uint4 *>(sm_raw + (size_t)W * RB);
-  double *stk = reinterpret_cast<double *>(prog + M.tape_prog_cap) +
-                (size_t)warp * M.tape_stack_cap * 64;
-  double *xs = reinterpret_cast<double *>(prog + M.tape_prog_cap) +
-               (size_t)W * M.tape_stack_cap * 64;
-  uint64_t *mbar = reinterpret_cast<uint64_t *>(xs + (size_t)M.tape_xs_cap * 64) +
-                   (size_t)warp * (S + 1);
-  const uint32_t ring_s = smem_u32(ringc), bar_s = smem_u32(mbar);
-  double *__restrict__ tape = M.tape + tg.tape_base;
-  double *__restrict__ scr = M.scratch + tg.scratch_base;
-  double *__restrict__ tape_l = tape + lane;
-  double *__restrict__ scr_l = scr + lane;
+  const unsigned char *ringc = sm_raw + (size_t)warp * RB + lane8;  // this lane's column
+  double *sys_l = reinterpret_cast<double *>(sm_raw + (size_t)W * RB) + lane;
+  uint4 *progbuf = reinterpret_cast<uint4 *>(sm_raw + (size_t)W * RB +
+                                             (size_t)M.tape_sys_cap * 512);
+  uint32_t *ctr = reinterpret_cast<uint32_t *>(progbuf + 2 * (size_t)M.tape_prog_cap);
+  uint64_t *mbar_all = reinterpret_cast<uint64_t *>(ctr + 16);
+  const uint32_t ring_s = smem_u32(sm_raw + (size_t)warp * RB);
+  const uint32_t bar_s = smem_u32(mbar_all + (size_t)warp * S);  // S ring barriers of this warp
+  const uint32_t pbar_s = smem_u32(mbar_all + (size_t)W * S);    // 2 program barriers
+  const uint32_t ctr_s = smem_u32(ctr);
   const double dt = M.dt;
   const double q10dt = M.q10 * dt;
-  const TapeTask *tasks = M.ttask + (size_t)tg.cls * (W + 1);
+  const bool flush = mode & TM_FLUSH;
+  const int ngrp = M.n_tgroup;
 
-  // the host pads the tapes so that no record wraps around the ring: row i of a record is at a
-  // fixed distance from its first row
 #define CN_RD(base, i) (*reinterpret_cast<const double *>((base) + (uint32_t)(i) * 256u))
 
-  // chunk c of a row stream goes to stage c % S
-  auto issue = [&](const double *base, int c, int total_rows) {
-    const int rows = min(CH, total_rows - c * CH);
-    const uint32_t bytes = (uint32_t)rows * 256u;
-    const int s = c & (S - 1);
-    mbar_expect_tx(bar_s + 8 * s, bytes);
-    bulk_g2s(ring_s + (uint32_t)s * (CH * 256), base + (size_t)c * (CH * 32), bytes,
-             bar_s + 8 * s);
-  };
-
-  uint32_t phase = 0;  // bit s: parity the next wait on stage s looks for
-  uint32_t ws = 0;     // stage of the next chunk to wait for
-  int ci = S;          // next chunk to issue
-
-  const TapeTask leaf = tasks[warp];
-  if (lane == 0) {
-    for (int s = 0; s <= S; ++s) mbar_init(bar_s + 8 * s, 1);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < W * S + 2; ++s) mbar_init(smem_u32(mbar_all + s), 1);
+    for (int w = 0; w < 16; ++w) ctr[w] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    // this warp's slice of the program (warp 0: also the top task's, which follows the leaves')
-    const int q0 = leaf.p0, q1 = leaf.p1;
-    uint32_t bytes = 0;
-    if (warp == 0) {
-      bytes = (uint32_t)(leaf.p1 - leaf.p0 + tasks[W].p1 - tasks[W].p0) * 16u;
-      mbar_expect_tx(bar_s + 8 * S, bytes);
-      if (leaf.p1 > leaf.p0)
-        bulk_g2s(smem_u32(prog + leaf.p0), M.prog + tc.prog_off + leaf.p0,
-                 (uint32_t)(leaf.p1 - leaf.p0) * 16u, bar_s + 8 * S);
-      bulk_g2s(smem_u32(prog + tasks[W].p0), M.prog + tc.prog_off + tasks[W].p0,
-               (uint32_t)(tasks[W].p1 - tasks[W].p0) * 16u, bar_s + 8 * S);
-    } else {
-      bytes = (uint32_t)(q1 - q0) * 16u;
-      mbar_expect_tx(bar_s + 8 * S, bytes);
-      if (bytes) bulk_g2s(smem_u32(prog + q0), M.prog + tc.prog_off + q0, bytes, bar_s + 8 * S);
-    }
-    const int nchunk0 = ((int)leaf.nrows + CH - 1) / CH;
-    for (int c = 0; c < S && c < nchunk0; ++c)
-      issue(tape + (size_t)leaf.row0 * 32, c, (int)leaf.nrows);
   }
-  __syncwarp();
-  mbar_wait(bar_s + 8 * S, 0);
+  __syncthreads();
 
-  int sp = 0;
-  // ==========================================================================================
-  // forward: nrn_cur + tree terms + triangularisation, children before parents.
-  // phase 0: the warp's leaf task; phase 1 (warp 0 only, after all leaves): the top task
-  // ==========================================================================================
-  const int n_fwd = warp == 0 ? 2 : 1;
-  for (int ph = 0; ph < n_fwd; ++ph) {
-    const TapeTask tk = ph == 0 ? leaf : tasks[W];
-    const double *tseg = tape + (size_t)tk.row0 * 32;
-    const int nchunk = ((int)tk.nrows + CH - 1) / CH;
-    if (ph == 1) {
-      bar_sync(1, nthreads);  // every leaf task has exported its subtree roots
-      ws = 0;
-      ci = S;
-      if (lane == 0)
-        for (int c = 0; c < S && c < nchunk; ++c) issue(tseg, c, (int)tk.nrows);
+  // ring state (uniform over the warp): chunk c of a segment goes to stage c % S
+  uint32_t phase = 0;      // bit s: parity the next wait on stage s looks for
+  int cw = 0, ci = 0;      // chunks waited for / issued so far in the current segment
+  const double *seg = nullptr;
+  int seg_rows = 0, nchunk = 0;
+  auto issue = [&](int c) {  // lane 0: chunk c of the current segment
+    const int rows = min(CH, seg_rows - (c << lgCH));
+    const uint32_t bytes = (uint32_t)rows * 256u;
+    const uint32_t s = (uint32_t)c & (uint32_t)(S - 1);
+    mbar_expect_tx(bar_s + 8 * s, bytes);
+    bulk_g2s(ring_s + ((s << lgCH) << 8), seg + ((size_t)c << (lgCH + 5)), bytes, bar_s + 8 * s);
+  };
+  // rows [0, e) of the segment must have landed
+  auto ring_need = [&](int e) {
+    const int need = (e + CH - 1) >> lgCH;
+    while (cw < need) {
+      const uint32_t s = (uint32_t)cw & (uint32_t)(S - 1);
+      mbar_wait(bar_s + 8 * s, (phase >> s) & 1u);
+      phase ^= 1u << s;
+      ++cw;
     }
-    uint32_t grow = tk.row0 * 32u;  // element offset of the current record on the group's tape
+  };
+  // rows [0, e) are consumed: refill the stages they occupied, S chunks ahead
+  auto ring_done = [&](int e) {
+    const int lim = min(nchunk, (e >> lgCH) + S);
+    if (ci < lim) {
+      __syncwarp();
+      if (lane == 0)
+        for (int c = ci; c < lim; ++c) issue(c);
+      ci = lim;
+    }
+  };
+  auto start_segment = [&](const TapeGroup &g, const TapeTask &t) {
+    seg = M.tape + g.tape_base + (size_t)t.row0 * 32;
+    seg_rows = (int)(flush ? t.mrows : t.nrows);
+    nchunk = (seg_rows + CH - 1) >> lgCH;
+    cw = 0;
+    ci = min(S, nchunk);
+    if (lane == 0)
+      for (int c = 0; c < ci; ++c) issue(c);
+  };
+  auto load_program = [&](const TapeClass &c, int buf) {  // one thread
+    const uint32_t bytes = (uint32_t)c.prog_len * 16u;
+    mbar_expect_tx(pbar_s + 8 * buf, bytes);
+    bulk_g2s(smem_u32(progbuf + (size_t)buf * M.tape_prog_cap), M.prog + c.prog_off, bytes,
+             pbar_s + 8 * buf);
+  };
+
+  int g = blockIdx.x;
+  if (g >= ngrp) return;
+  TapeGroup tg = M.tgrp[g];
+  TapeClass tc = M.tcls[tg.cls];
+  TapeTask tk = M.ttask[(size_t)tg.cls * W + warp];
+  if (threadIdx.x == 0) load_program(tc, 0);
+  start_segment(tg, tk);
+
+  for (uint32_t it = 0; g < ngrp; g += gridDim.x, ++it) {
+    const uint32_t base = (it + 1) << 13;  // progress counters never run backwards
+    const int gn = g + gridDim.x;
+    const bool has_next = gn < ngrp;
+    TapeGroup tgn = tg;
+    TapeClass tcn = tc;
+    TapeTask tkn = tk;
+    if (has_next) {
+      tgn = M.tgrp[gn];
+      tcn = M.tcls[tgn.cls];
+      tkn = M.ttask[(size_t)tgn.cls * W + warp];
+      if (threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
+    }
+    mbar_wait(pbar_s + 8 * (it & 1), (it >> 1) & 1);
+    const uint4 *prog = progbuf + (size_t)(it & 1) * M.tape_prog_cap;
+    double *__restrict__ tape_l = M.tape + tg.tape_base + lane;
+    const int p0 = tk.p0, p1 = flush ? tk.p0 + tk.pm : tk.p1;
+    const int row0 = (int)tk.row0;
+
+    // ========================================================================================
+    // forward: mechanism records (nrn_state of the previous step, nrn_cur), then tree terms and
+    // triangularisation, children before parents
+    // ========================================================================================
     double accD = 0.0, accR = 0.0;
-    for (int j = tk.p0; j < tk.p1; ++j) {
+    for (int j = p0; j < p1; ++j) {
       const uint4 e = prog[j];
-      const uint32_t fl = e.z;
-      for (uint32_t nw = (fl >> 8) & 15u; nw; --nw) {
-        mbar_wait(bar_s + 8 * ws, (phase >> ws) & 1u);
-        phase ^= 1u << ws;
-        ws = (ws + 1) & (S - 1);
+      const uint32_t ty = e.y & RT_MASK;
+      if (ty == RT_RUN) {
+        // a run of plain chain nodes: each hands its contribution to the next in registers
+        const unsigned char *rb = ringc + (e.x & 0xFFFFu);
+        double *srow = sys_l + e.z * 64u;
+        int rend = (int)(e.w >> 16);
+        if (!(e.x & (1u << 24))) {
+          accD = 0.0;
+          accR = 0.0;
+        }
+        for (int q = (int)((e.x >> 16) & 255u); q; --q) {
+          ring_need(rend);
+          const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
+          const double D = CN_RD(rb, 2) + accD;
+          const double R = (CN_RD(rb, 4) + CN_RD(rb, 3)) + accR;
+          const double rinv = rcp_fast(D);
+          const double f = a * rinv;
+          srow[0] = b * rinv;
+          srow[32] = R * rinv;
+          accD = -(f * b);
+          accR = -(f * R);
+          ring_done(rend);
+          rb += 5 * 256;
+          srow += 64;
+          rend += 5;
+        }
+        continue;
       }
-      const unsigned char *rb = ringc + ((e.x & 0xFFFFu) + lane8);
-      double *__restrict__ srec = scr_l + e.y;
-      const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
-      const double v_old = CN_RD(rb, 4);
-      double D = CN_RD(rb, 2), R = v_old + CN_RD(rb, 3);
-      double mult, rp;
-      if ((fl & (0xFFu & ~PG_FWD_IN)) == PG_FWD && e.w == 0u) {
-        // FAST PATH (most nodes): interior or tip of an unbranched stretch, no mechanism rows;
-        // the contribution to the parent stays in registers
-        if (fl & PG_FWD_IN) {
+      if (ty == RT_WAIT) {
+        ctr_wait(ctr_s + 4 * (e.z & 0xFFFFu), base + (e.z >> 16));
+        continue;
+      }
+      const uint32_t fl = e.y & 0xFFFFu;
+      const unsigned char *rb = ringc + (e.x & 0xFFFFu);
+      double *srow = sys_l + (e.z & 1023u) * 64u;
+      int rend;
+      if (ty == RT_ELIM) {
+        rend = (int)(e.w & 0xFFFFu) - row0 + (int)((e.x >> 16) & 255u);
+        ring_need(rend);
+        const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
+        double D = CN_RD(rb, 2), R = CN_RD(rb, 4) + CN_RD(rb, 3);
+        if (fl & RF_FWD_IN) {
           D += accD;
           R += accR;
         }
+        if (fl & RF_HAS_ACC) {
+          D += srow[0];
+          R += srow[32];
+        }
+        if (fl & RF_HAS_PP) {  // conductance / current of the point processes (pp_tape_kernel)
+          const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
+          D += pd;
+          R += pr;
+          if (pd != 0.0 || pr != 0.0) {
+            double *trec = tape_l + (e.w & 0xFFFFu) * 32u;
+            trec[5 * 32] = 0.0;
+            trec[6 * 32] = 0.0;
+          }
+        }
         const double rinv = rcp_fast(D);
-        const double f = a * rinv;
-        rp = R * rinv;
-        mult = b * rinv;
-        accD = -(f * b);
-        accR = -(f * R);
-      } else {
-      double *__restrict__ trec = tape_l + grow;
-      uint32_t cur = 5, scur = 2;
-      if (fl & PG_FWD_IN) {
-        D += accD;
-        R += accR;
-      }
-      if (fl & PG_POP) {
-        --sp;
-        D += stk[sp * 64 + lane];
-        R += stk[sp * 64 + 32 + lane];
-      }
-      for (uint32_t ni = e.w >> 28, s0 = (e.w >> 20) & 255u; ni; --ni, ++s0) {  // cut subtrees
-        D += xs[s0 * 64 + lane];
-        R += xs[s0 * 64 + 32 + lane];
-      }
-      if (fl & PG_HAS_PP) {  // conductance / current of the point processes (pp_tape_kernel)
-        const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
-        D += pd;
-        R += pr;
-        if (pd != 0.0 || pr != 0.0) {
-          trec[5 * 32] = 0.0;
-          trec[6 * 32] = 0.0;
-        }
-        cur = 7;
-      }
-      double ica = 0.0;
-      if (fl & PG_NEED_ICA) ++scur;
-      if (fl & PG_HAS_CAI) {
-        srec[scur * 32] = CN_RD(rb, cur);
-        ++cur;
-        ++scur;
-      }
-      for (uint32_t mk = e.w & 0xFFFFFu; mk; mk &= mk - 1) {
-        const DTable &T = M.tab[__ffs(mk) - 1];
-        const unsigned char *mr = rb + cur * 256u;
-        switch (T.type) {
-          case T_HH: {
-            const double m = CN_RD(mr, 5), h = CN_RD(mr, 6), nn = CN_RD(mr, 7);
-            const double invc = CN_RD(mr, 4);
-            const double gna = CN_RD(mr, 0) * m * m * m * h;
-            const double n2 = nn * nn;
-            const double gk = CN_RD(mr, 1) * n2 * n2;
-            const double gl = CN_RD(mr, 2);
-            D += (gna + gk + gl) * invc;
-            R += (gna * T.glob[0] + gk * T.glob[1] + gl * CN_RD(mr, 3)) * invc;
-            srec[scur * 32] = m;
-            srec[(scur + 1) * 32] = h;
-            srec[(scur + 2) * 32] = nn;
-            cur += 8;
-            scur += 3;
-            break;
-          }
-          case T_HHFORM: {
-            const double ms = CN_RD(mr, 2), hs = CN_RD(mr, 3);
-            const double g = CN_RD(mr, 0) * ipow(ms, (int)T.glob[0]) * ipow(hs, (int)T.glob[1]);
-            const double invc = CN_RD(mr, 1);
-            D += g * invc;
-            R += g * T.glob[2] * invc;
-            if (T.glob[3] != 0.0) ica += g * (v_old - T.glob[2]);
-            srec[scur * 32] = ms;
-            srec[(scur + 1) * 32] = hs;
-            cur += 4;
-            scur += 2;
-            break;
-          }
-          case T_SK: {
-            const double z = CN_RD(mr, 2);
-            const double g = CN_RD(mr, 0) * z;
-            const double invc = CN_RD(mr, 1);
-            D += g * invc;
-            R += g * T.glob[0] * invc;
-            srec[scur * 32] = z;
-            cur += 3;
-            scur += 1;
-            break;
-          }
-          default: break;  // PAS is folded into the static rows; CADYN carries no current
-        }
-      }
-      if (fl & PG_NEED_ICA) srec[2 * 32] = ica;
-      const double rinv = rcp_fast(D);
-      rp = R * rinv;
-      mult = 0.0;
-      if (!(fl & PG_ROOT)) {
-        const double f = a * rinv;
-        const double cD = -(f * b), cR = -(f * R);
-        mult = b * rinv;  // back-substitution multiplier
-        const uint32_t kind = fl & PG_KIND;
-        if (kind == PG_FWD) {
-          accD = cD;
-          accR = cR;
-        } else if (kind == PG_PUSH) {
-          stk[sp * 64 + lane] = cD;
-          stk[sp * 64 + 32 + lane] = cR;
-          ++sp;
-        } else if (kind == PG_ADD) {
-          stk[(sp - 1) * 64 + lane] += cD;
-          stk[(sp - 1) * 64 + 32 + lane] += cR;
-        } else {  // root of a cut subtree: export to the top task
-          const uint32_t s0 = (e.w >> 20) & 255u;
-          xs[s0 * 64 + lane] = cD;
-          xs[s0 * 64 + 32 + lane] = cR;
-        }
-      }
-      }
-      srec[0] = mult;
-      srec[32] = rp;
-      grow += (fl >> 24) * 32u;
-      // stages whose rows are all consumed are refilled S chunks ahead
-      uint32_t nf = (fl >> 12) & 15u;
-      if (nf) {
-        __syncwarp();
-        if (lane == 0)
-          for (; nf; --nf, ++ci)
-            if (ci < nchunk) issue(tseg, ci, (int)tk.nrows);
-        ci = __shfl_sync(0xffffffffu, ci, 0);
-      }
-    }
-    if (ph == 0 && warp != 0) bar_arrive(1, nthreads);
-  }
-
-  // ==========================================================================================
-  // backward: back-substitution (L66), nrn_state with the new v (L67), threshold at the root
-  // (L68).  phase 0 (warp 0 only): the top task; phase 1 (after it): the warp's leaf task
-  // ==========================================================================================
-  asm volatile("fence.proxy.async;" ::: "memory");  // scratch written above, read by bulk copies
-  __syncwarp();
-  for (int ph = warp == 0 ? 0 : 1; ph < 2; ++ph) {
-    const TapeTask tk = ph == 0 ? tasks[W] : leaf;
-    const double *sseg = scr + (size_t)tk.srow0 * 32;
-    const int nsch = ((int)tk.nsrows + CH - 1) / CH;
-    if (lane == 0)
-      for (int c = 0; c < S && c < nsch; ++c) issue(sseg, c, (int)tk.nsrows);
-    ws = 0;
-    ci = S;
-    if (ph == 1) {  // the top task has written v of every cut subtree's parent
-      if (warp == 0) bar_arrive(2, nthreads);
-      else bar_sync(2, nthreads);
-    }
-    uint32_t grow = (tk.row0 + tk.nrows) * 32u;
-    double v_prev = 0.0;
-    sp = 0;
-    for (int j = tk.p1 - 1; j >= tk.p0; --j) {
-      const uint4 e = prog[j];
-      const uint32_t fl = e.z;
-      grow -= (fl >> 24) * 32u;
-      for (uint32_t nw = (fl >> 16) & 15u; nw; --nw) {
-        mbar_wait(bar_s + 8 * ws, (phase >> ws) & 1u);
-        phase ^= 1u << ws;
-        ws = (ws + 1) & (S - 1);
-      }
-      const unsigned char *sb = ringc + ((e.x >> 16) + lane8);
-      double *__restrict__ trec = tape_l + grow;
-      if ((fl & (0xFFu & ~PG_FWD_IN)) == PG_FWD && e.w == 0u) {
-        // FAST PATH: the parent is the node just solved
-        v_prev = fma(-CN_RD(sb, 0), v_prev, CN_RD(sb, 1));
-        trec[4 * 32] = v_prev;
-      } else {
-      const uint32_t kind = fl & PG_KIND;
-      double vp = v_prev;
-      if (kind == PG_ADD) vp = stk[(sp - 1) * 32 + lane];
-      if (kind == PG_PUSH) vp = stk[(--sp) * 32 + lane];
-      if (kind == 0 && !(fl & PG_ROOT)) vp = xs[((e.w >> 20) & 255u) * 64 + lane];
-      const double v = fma(-CN_RD(sb, 0), vp, CN_RD(sb, 1));  // the root's multiplier is 0
-      if (fl & PG_POP) stk[(sp++) * 32 + lane] = v;
-      for (uint32_t ni = e.w >> 28, s0 = (e.w >> 20) & 255u; ni; --ni, ++s0)
-        xs[s0 * 64 + lane] = v;  // v of the parent of cut subtrees
-      v_prev = v;
-      trec[4 * 32] = v;
-      uint32_t cur = 5 + ((fl & PG_HAS_PP) ? 2u : 0u), scur = 2;
-      double ica = 0.0, cai = 0.0;
-      uint32_t cai_row = 0;
-      if (fl & PG_NEED_ICA) ica = CN_RD(sb, scur++);
-      if (fl & PG_HAS_CAI) {
-        cai = CN_RD(sb, scur++);
-        cai_row = cur++;
-      }
-      for (uint32_t mk = e.w & 0xFFFFFu; mk; mk &= mk - 1) {
-        const DTable &T = M.tab[__ffs(mk) - 1];
-        const unsigned char *ms = sb + scur * 256u;
-        switch (T.type) {
-          case T_HH: {
-            double m = CN_RD(ms, 0), h = CN_RD(ms, 1), nn = CN_RD(ms, 2);
-            hh_advance(v, q10dt, m, h, nn);
-            trec[(cur + 5) * 32] = m;
-            trec[(cur + 6) * 32] = h;
-            trec[(cur + 7) * 32] = nn;
-            cur += 8;
-            scur += 3;
-            break;
-          }
-          case T_HHFORM: {
-            double xinf, xtau;
-            if ((int)T.glob[0] > 0) {
-              hhform_gate(v, T.glob + 4, xinf, xtau);
-              trec[(cur + 2) * 32] = cnexp(CN_RD(ms, 0), xinf, xtau, dt);
-            }
-            if ((int)T.glob[1] > 0) {
-              hhform_gate(v, T.glob + 10, xinf, xtau);
-              trec[(cur + 3) * 32] = cnexp(CN_RD(ms, 1), xinf, xtau, dt);
-            }
-            cur += 4;
-            scur += 2;
-            break;
-          }
-          case T_SK: {
-            const double ca = cai < 1e-9 ? 1e-9 : cai;
-            const double zinf = 1.0 / (1.0 + pow(T.glob[1] / ca, T.glob[2]));
-            trec[(cur + 2) * 32] = cnexp(CN_RD(ms, 0), zinf, T.glob[3], dt);
-            cur += 3;
-            scur += 1;
-            break;
-          }
-          case T_CADYN: {
-            // derivimplicit on a linear ODE: one Newton step of backward Euler is exact (L278)
-            const double kappa = 1e4 * T.glob[0] / (2.0 * 96485.33212 * T.glob[1]);
-            cai = (cai + dt * (-kappa * ica + T.glob[3] / T.glob[2])) / (1.0 + dt / T.glob[2]);
-            trec[cai_row * 32] = cai;
-            break;
-          }
-          default: break;
-        }
-      }
-      if (fl & PG_ROOT) {  // warp-ballot threshold detection, one atomic per warp
-        bool fire = false;
-        const int pc = tg.cell_base + lane;
-        if (lane < tg.ncell) {
-          const bool above = v > M.thr[pc];
-          fire = above && !M.flag[pc];
-          M.flag[pc] = (unsigned char)above;
-        }
-        const unsigned ball = __ballot_sync(0xffffffffu, fire);
-        if (ball) {
-          unsigned long long base = 0;
-          const int leader = __ffs(ball) - 1;
-          if (lane == leader) base = atomicAdd(M.n_sp, (unsigned long long)__popc(ball));
-          base = __shfl_sync(0xffffffffu, base, leader);
-          if (fire) {
-            const unsigned long long pos = base + __popc(ball & ((1u << lane) - 1u));
-            if ((int64_t)pos < M.sp_cap) {
-              M.sp_gid[pos] = M.gid_of_pcell[pc];
-              M.sp_step[pos] = k + 1;
+        const uint32_t kind = fl & RK_KIND;
+        double mult = 0.0;
+        if (kind != RK_ROOT) {
+          const double f = a * rinv;
+          const double cD = -(f * b), cR = -(f * R);
+          mult = b * rinv;  // back-substitution multiplier
+          if (kind == RK_FWD) {
+            accD = cD;
+            accR = cR;
+          } else {
+            double *prow = sys_l + ((e.z >> 10) & 1023u) * 64u;
+            if (kind == RK_STORE) {
+              prow[0] = cD;
+              prow[32] = cR;
             } else {
-              *M.overflow = 1;
+              prow[0] += cD;
+              prow[32] += cR;
+            }
+          }
+        }
+        srow[0] = mult;
+        srow[32] = R * rinv;
+      } else {  // RT_MECH
+        rend = (int)(e.y >> 16) - row0 + (int)((e.x >> 16) & 255u);
+        ring_need(rend);
+        double gD, gR;
+        mech_record(M, rb, tape_l + (e.y >> 16) * 32u, fl, e.w, mode, dt, q10dt, gD, gR);
+        if (!flush) {
+          srow[0] = gD;
+          srow[32] = gR;
+        }
+      }
+      if (fl & RF_SIG_F) {
+        __syncwarp();
+        if (lane == 0) ctr_publish(ctr_s + 4 * warp, base + (uint32_t)(j - p0) + 1u);
+      }
+      ring_done(rend);
+    }
+    // this warp's ring is idle until the next group: start loading it now
+    __syncwarp();
+    if (has_next) start_segment(tgn, tkn);
+
+    // ========================================================================================
+    // backward: back-substitution (L66), v to the tape, threshold at the root (L68)
+    // ========================================================================================
+    if (!flush) {
+      const uint32_t nrec = (uint32_t)(tk.p1 - tk.p0);
+      double v_prev = 0.0;
+      for (int j = tk.p1 - 1; j >= tk.p0 + tk.pm; --j) {
+        const uint4 e = prog[j];
+        const uint32_t ty = e.y & RT_MASK;
+        if (ty == RT_RUN) {
+          // the parent of the run's last node is the node just solved
+          const int q = (int)((e.x >> 16) & 255u);
+          const double *srow = sys_l + (e.z + (uint32_t)q) * 64u;
+          double *trow = tape_l + ((e.w & 0xFFFFu) + 5u * (uint32_t)q + 4u) * 32u;
+          for (int i = q; i; --i) {
+            srow -= 64;
+            trow -= 5 * 32;
+            v_prev = fma(-srow[0], v_prev, srow[32]);
+            *trow = v_prev;
+          }
+          continue;
+        }
+        if (ty != RT_ELIM) continue;
+        const uint32_t fl = e.y & 0xFFFFu;
+        if (fl & RF_WAIT_B) ctr_wait(ctr_s + 4 * (e.y >> 28), base + ((e.y >> 16) & 0xFFFu));
+        double *srow = sys_l + (e.z & 1023u) * 64u;
+        const uint32_t kind = fl & RK_KIND;
+        double vp = v_prev;
+        if (kind >= RK_STORE) vp = sys_l[((e.z >> 10) & 1023u) * 64u + 32];
+        const double v = fma(-srow[0], vp, srow[32]);  // the root's multiplier is 0
+        srow[32] = v;  // children that did not hand over in registers read it here
+        v_prev = v;
+        tape_l[(e.w & 0xFFFFu) * 32u + 4 * 32] = v;
+        if (fl & RF_MECHV) tape_l[(e.w >> 16) * 32u] = v;
+        if (fl & RF_SIG_B) {
+          __syncwarp();
+          if (lane == 0)
+            ctr_publish(ctr_s + 4 * warp, base + nrec + (uint32_t)(tk.p1 - j));
+        }
+        if (kind == RK_ROOT) {  // warp-ballot threshold detection, one atomic per warp
+          bool fire = false;
+          const int pc = tg.cell_base + lane;
+          if (lane < tg.ncell) {
+            const bool above = v > M.thr[pc];
+            fire = above && !M.flag[pc];
+            M.flag[pc] = (unsigned char)above;
+          }
+          const unsigned ball = __ballot_sync(0xffffffffu, fire);
+          if (ball) {
+            unsigned long long sbase = 0;
+            const int leader = __ffs(ball) - 1;
+            if (lane == leader) sbase = atomicAdd(M.n_sp, (unsigned long long)__popc(ball));
+            sbase = __shfl_sync(0xffffffffu, sbase, leader);
+            if (fire) {
+              const unsigned long long pos = sbase + __popc(ball & ((1u << lane) - 1u));
+              if ((int64_t)pos < M.sp_cap) {
+                M.sp_gid[pos] = M.gid_of_pcell[pc];
+                M.sp_step[pos] = k + 1;
+              } else {
+                *M.overflow = 1;
+              }
             }
           }
         }
       }
-      }
-      uint32_t nf = (fl >> 20) & 15u;
-      if (nf) {
-        __syncwarp();
-        if (lane == 0)
-          for (; nf; --nf, ++ci)
-            if (ci < nsch) issue(sseg, ci, (int)tk.nsrows);
-        ci = __shfl_sync(0xffffffffu, ci, 0);
-      }
     }
+    __syncthreads();  // the system rows and counters of this group are dead from here on
+    tg = tgn;
+    tc = tcn;
+    tk = tkn;
   }
 #undef CN_RD
 }
