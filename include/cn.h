@@ -143,7 +143,8 @@ int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samples);
 int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
 /* Layout facts for DESIGN/bench, info8 = { n_class, n_group (all), shared-memory bytes per warp and
  * max elimination rounds of the warp-cooperative kernel, n_group of the interleaved (tape) kernel,
- * tape bytes, scratch-tape bytes, max stack depth }. */
+ * tape bytes, shared-memory bytes per CTA of the interleaved kernel (after the first cn_run),
+ * warps per CTA | persistent CTAs << 8 | shared-memory system rows << 24 }. */
 int cn_get_layout_info(const cn_model *m, int64_t *info8);
 /* Spike buffer capacity (default 16*n_cell + 65536); before the first cn_run only. */
 int cn_set_spike_capacity(cn_model *m, int64_t cap);

@@ -264,7 +264,8 @@ class Model:
         _check(lib().cn_get_layout_info(self._h, _ptr(a)))
         return {"n_class": int(a[0]), "n_group": int(a[1]), "warp_smem_bytes": int(a[2]),
                 "max_rounds": int(a[3]), "n_tape_group": int(a[4]), "tape_bytes": int(a[5]),
-                "scratch_bytes": int(a[6]), "tape_warps": int(a[7])}
+                "tape_smem_bytes": int(a[6]), "tape_warps": int(a[7]) & 255,
+                "tape_ctas": (int(a[7]) >> 8) & 0xFFFF, "tape_sys_rows": int(a[7]) >> 24}
 
     def set_spike_capacity(self, cap):
         _check(lib().cn_set_spike_capacity(self._h, int(cap)))

@@ -11,7 +11,7 @@ SRCS = [HERE / "csrc" / "cn_api.cu"]
 DEPS = SRCS + [HERE / "csrc" / "cn_device.cuh", HERE / "csrc" / "cn_tape.cuh",
                HERE.parent / "include" / "cn.h"]
 
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+NVCC_FLAGS = (["-DCN_TRACE"] if os.environ.get("CN_TRACE") else []) + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
 

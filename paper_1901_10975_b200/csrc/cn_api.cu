@@ -109,7 +109,7 @@ struct HTable {
   std::vector<int64_t> cell_inst;
 };
 
-struct HTask { int p0 = 0, p1 = 0, pm = 0; uint32_t row0 = 0, nrows = 0, mrows = 0; };
+struct HTask { int p0 = 0, p1 = 0, nchunk = 0, tm_base = 0; uint32_t row0 = 0, nrows = 0, head = 0; };
 
 struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh)
   std::vector<HTask> task;                   // one per warp
@@ -122,6 +122,7 @@ struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh
   std::vector<std::vector<int32_t>> tab_row; // [table][local node]: first row of its block or -1
   std::vector<int32_t> cai_row, ica_row, pp_row, vcopy_row;  // per local node or -1
   int n_rows = 0, prog_off = 0;
+  int n_srow = 0;                            // rows of the shared-memory system (the rest: TMEM)
   double sim_makespan = 0.0, sim_work = 0.0; // schedule quality (cn_debug_tasks)
 };
 
@@ -167,6 +168,8 @@ struct cn_model {
   int64_t n_tape = 0;               // doubles
   int tape_prog_cap = 0, tape_sys_cap = 0;
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
+  bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
+  bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
   int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
   bool state_pending = false;       // nrn_state of the last step has not been applied yet
   int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
@@ -540,7 +543,41 @@ static int build_tape_program(cn_model *m, HClass &K) {
     std::vector<double> wt(mload);
     std::vector<int> last(W, -1);
     for (auto &l : elist) l.clear();
-    for (int done = 0; done < ntask; ++done) {
+    int done0 = 0;
+    auto place = [&](int id, int w) {
+      Task &T = tasks[id];
+      T.warp = w;
+      T.t0 = std::max(wt[w], T.ready);
+      double t = T.t0;
+      for (int32_t x : T.nodes) {
+        t += ecost[x];
+        t_end[x] = t;
+        e_warp[x] = w;
+        elist[w].push_back(x);
+      }
+      wt[w] = t;
+      last[w] = id;
+      if (T.ptask >= 0) {
+        tasks[T.ptask].pending--;
+        tasks[T.ptask].ready = std::max(tasks[T.ptask].ready, t);
+      }
+    };
+    // the whole subtrees first, largest first to the least loaded warp: in the backward sweep
+    // (the reverse of each warp's list) the upper nodes, which every warp waits for, then come
+    // before any subtree
+    if (W > 1 && m->tape_leaf_first) {
+      std::vector<int> leafs;
+      for (int id = 0; id < ntask; ++id)
+        if (sw[tasks[id].nodes.back()] <= gran) leafs.push_back(id);
+      std::stable_sort(leafs.begin(), leafs.end(),
+                       [&](int a, int b) { return tasks[a].cost > tasks[b].cost; });
+      for (int id : leafs) {
+        const int w = (int)(std::min_element(wt.begin(), wt.end()) - wt.begin());
+        place(id, w);
+        ++done0;
+      }
+    }
+    for (int done = done0; done < ntask; ++done) {
       // the earliest free warp; among equals one that can continue with the parent of its last task
       auto affinity = [&](int w) {
         if (last[w] < 0) return -1;
@@ -584,22 +621,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
         cand = best_now >= 0 ? best_now : best_later;
       }
       if (cand < 0) return fail(CN_ERR_TOPOLOGY, "internal: tape scheduler found no task");
-      Task &T = tasks[cand];
-      T.warp = w;
-      T.t0 = std::max(wt[w], T.ready);
-      double t = T.t0;
-      for (int32_t x : T.nodes) {
-        t += ecost[x];
-        t_end[x] = t;
-        e_warp[x] = w;
-        elist[w].push_back(x);
-      }
-      wt[w] = t;
-      last[w] = cand;
-      if (T.ptask >= 0) {
-        tasks[T.ptask].pending--;
-        tasks[T.ptask].ready = std::max(tasks[T.ptask].ready, t);
-      }
+      place(cand, w);
     }
     P.sim_makespan = *std::max_element(wt.begin(), wt.end());
     if (pass == 1) break;
@@ -628,8 +650,9 @@ static int build_tape_program(cn_model *m, HClass &K) {
     std::vector<std::pair<int, int>> deps;  // (warp, pre-index) this record waits for, forward
     int bw_warp = -1, bw_pre = -1;          // backward: the parent's record on another warp
     int fidx = 0;                           // index in the final list (WAIT records included)
-    uint32_t row = 0, len = 0;
-    bool padded = false;                    // pad rows precede the record on the tape
+    uint32_t row = 0, len = 0, ring = 0;    // first tape row, rows, byte offset in the ring
+    uint32_t srow = 0;                      // row of the shared-memory system, or TMEM slot
+    bool tm = false;
   };
   std::vector<std::vector<Rec>> recs(W);
   std::vector<int> e_pre(n, -1), m_pre(n, -1);  // pre-index of a node's records in its warp's list
@@ -717,13 +740,53 @@ static int build_tape_program(cn_model *m, HClass &K) {
       P.pos_of[x] = (int32_t)P.order.size();
       P.order.push_back(x);
     }
+  // Where (multiplier, reduced rhs) of a node wait for the back-substitution: a node without
+  // contributions from mechanisms or from children that do not hand over in registers (its row
+  // is written and read by its own warp only) gets a slot of the warp's share of tensor
+  // memory (each quarter of the CTA's 256 TMEM columns = 64 slots, shared by the warps w, w + 4, ...
+  // that can address it); every other node, and what does not fit, a row of the shared-memory
+  // system.
+  {
+    std::vector<int> plain_cnt(W, 0), cap(W, 0);
+    auto is_plain = [&](const Rec &r) {  // nobody else touches the node's row
+      return r.type == 0 && !(r.flags & RF_HAS_ACC);
+    };
+    for (int w = 0; w < W; ++w)
+      for (const Rec &r : recs[w]) plain_cnt[w] += is_plain(r) ? 1 : 0;
+    const int tm_slots = m->tape_tmem ? 64 : 0;
+    for (int q = 0; q < 4 && q < W; ++q) {
+      int tot = 0;
+      for (int w = q; w < W; w += 4) tot += plain_cnt[w];
+      int base = 0;
+      for (int w = q; w < W; w += 4) {
+        cap[w] = tot <= tm_slots ? plain_cnt[w] : (int)((int64_t)plain_cnt[w] * tm_slots / tot);
+        P.task[w].tm_base = base;
+        base += cap[w];
+      }
+    }
+    uint32_t ns = 0;
+    for (int w = 0; w < W; ++w) {
+      int used = 0;
+      for (Rec &r : recs[w]) {
+        if (r.type != 0) continue;
+        if (is_plain(r) && used < cap[w]) {
+          r.tm = true;
+          r.srow = (uint32_t)used++;
+        } else {
+          r.srow = ns++;
+        }
+      }
+    }
+    for (int w = 0; w < W; ++w)
+      for (Rec &r : recs[w])
+        if (r.type == 1) r.srow = erec(r.node).srow;  // a mechanism record writes the node's row
+    if (ns > 1023) return give_up();
+    P.n_srow = (int)ns;
+  }
   uint32_t row = 0;
   for (int w = 0; w < W; ++w) {
     HTask &Tk = P.task[w];
-    Tk.pm = (int)mlist[w].size();
     Tk.row0 = row;
-    bool m_open = true;
-    Tk.mrows = 0;
     for (Rec &r : recs[w]) {
       const int x = r.node;
       uint32_t ln;
@@ -734,17 +797,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
       } else {
         ln = 5 + (P.has_pp[x] ? 2 : 0);
       }
-      if (ln > R - CH || ln > 255) return give_up();  // a record must fit the ring
-      const uint32_t rel = row - Tk.row0;
-      r.padded = false;
-      if (rel % R + ln > R) {  // a record never wraps around the ring: pad to the next lap
-        row += R - rel % R;
-        r.padded = true;
-      }
-      if (r.type == 0 && m_open) {
-        Tk.mrows = row - Tk.row0;
-        m_open = false;
-      }
+      if (ln > CH) return give_up();  // a record must fit a chunk
       r.row = row;
       r.len = ln;
       row += ln;
@@ -764,40 +817,55 @@ static int build_tape_program(cn_model *m, HClass &K) {
       }
     }
     Tk.nrows = row - Tk.row0;
-    if (m_open) Tk.mrows = Tk.nrows;
     if (row > 65535) return give_up();  // 16-bit tape rows
   }
   P.n_rows = (int)row;
-  // final lists: WAIT records go in front of the record that needs them (a wait that an earlier
-  // wait of the same warp already covers is dropped: positions on one warp only grow); plain
-  // chain nodes that follow one another on the tape are merged into RUN records
-  struct Fin { int type; int pre; int cnt; int w2, pre2; };  // type 2 = WAIT, 3 = RUN
+  // final lists.  The records of a warp are packed into chunks of at most CH rows (chunk c goes
+  // to stage c % S of the warp's ring): a CHUNK record precedes the first record of every chunk.
+  // WAIT records go in front of the record that needs them (a wait that an earlier wait of the
+  // same warp already covers is dropped: positions on one warp only grow).  Plain chain nodes
+  // that follow one another inside a chunk are merged into RUN records.
+  struct Fin { int type; int pre; int cnt; int w2, pre2; };  // type 2 = WAIT, 3 = RUN, 4 = CHUNK
   std::vector<std::vector<Fin>> fin(W);
+  std::vector<std::vector<std::pair<uint32_t, uint32_t>>> chunks(W);  // (first row in segment, rows)
+  const uint32_t S = (uint32_t)m->tape_S;
   for (int w = 0; w < W; ++w) {
     std::vector<int> seen(W, -1);
+    uint32_t fill = CH + 1;  // rows used in the current chunk (none open yet)
     for (int i = 0; i < (int)recs[w].size(); ++i) {
       Rec &r = recs[w][i];
-      bool waited = false;
+      bool fresh = false;
+      if (fill + r.len > CH) {
+        fin[w].push_back(Fin{4, (int)chunks[w].size(), 0, -1, -1});
+        chunks[w].emplace_back(r.row - P.task[w].row0, 0u);
+        fill = 0;
+        fresh = true;
+      }
+      r.ring = ((uint32_t)((chunks[w].size() - 1) % S) * CH + fill) * 256u;
+      fill += r.len;
+      chunks[w].back().second = fill;
       for (auto &d : r.deps) {
         if (seen[d.first] >= d.second) continue;
         seen[d.first] = d.second;
         fin[w].push_back(Fin{2, -1, 0, d.first, d.second});
-        waited = true;
+        fresh = true;
       }
       const bool plain = r.type == 0 && (r.flags & ~(uint32_t)RF_FWD_IN) == RK_FWD;
-      if (plain && !waited && !r.padded && !fin[w].empty() && fin[w].back().type == 3 &&
-          fin[w].back().cnt < 255 && (r.flags & RF_FWD_IN)) {
-        const Rec &prev = recs[w][i - 1];
-        if (prev.row + 5 == r.row && (r.row - P.task[w].row0) % R != 0) {  // not at a ring lap
-          r.fidx = (int)fin[w].size() - 1;
-          fin[w].back().cnt++;
-          continue;
-        }
+      if (plain && !fresh && fin[w].back().type == 3 && fin[w].back().cnt < 255 &&
+          (r.flags & RF_FWD_IN) && recs[w][i - 1].tm == r.tm &&
+          recs[w][i - 1].srow + 1 == r.srow) {
+        r.fidx = (int)fin[w].size() - 1;
+        fin[w].back().cnt++;
+        continue;
       }
       r.fidx = (int)fin[w].size();
       fin[w].push_back(Fin{plain ? 3 : r.type, i, 1, -1, -1});
     }
     if (fin[w].size() > 2047) return give_up();  // 12-bit backward positions
+    HTask &Tk = P.task[w];
+    Tk.nchunk = (int)chunks[w].size();
+    Tk.head = 0;
+    for (uint32_t c = 0; c < 4 && c < chunks[w].size(); ++c) Tk.head |= chunks[w][c].second << (8 * c);
   }
   // backward waits: drop those an earlier (in backward order) wait of the same warp covers
   for (int w = 0; w < W; ++w) {
@@ -826,24 +894,32 @@ static int build_tape_program(cn_model *m, HClass &K) {
         P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)F.w2 | (uint32_t)pos << 16, 0u));
         continue;
       }
+      if (F.type == 4) {  // chunk c starts: chunk c-1 is consumed, its stage takes chunk c-1+S
+        const uint32_t c = (uint32_t)F.pre;
+        uint32_t ex = 0, fill_stage = 0;
+        if (c >= 1 && c - 1 + S < chunks[w].size()) {
+          ex = chunks[w][c - 1 + S].first | chunks[w][c - 1 + S].second << 16;
+          fill_stage = (c - 1) % S;
+        }
+        P.prog.push_back(make_uint4(ex, (uint32_t)RT_CHUNK, fill_stage | (c % S) << 16, 0u));
+        continue;
+      }
       const Rec &r = recs[w][F.pre];
       const int x = r.node;
-      const uint32_t rel = r.row - Tk.row0;
-      const uint32_t roff = (rel % R) * 256u;
       if (F.type == 3) {
-        P.prog.push_back(make_uint4(roff | (uint32_t)F.cnt << 16 |
+        P.prog.push_back(make_uint4(r.ring | (uint32_t)F.cnt << 16 |
                                         ((r.flags & RF_FWD_IN) ? 1u << 24 : 0u),
-                                    (uint32_t)RT_RUN, (uint32_t)P.pos_of[x],
-                                    r.row | (rel + r.len) << 16));
+                                    (uint32_t)RT_RUN, r.srow | (r.tm ? 1u << 20 : 0u), r.row));
       } else if (r.type == 1) {
-        P.prog.push_back(make_uint4(roff | r.len << 16, r.flags | r.row << 16,
-                                    (uint32_t)P.pos_of[x], node_mask[x]));
+        P.prog.push_back(make_uint4(r.ring, r.flags | r.row << 16, r.srow, node_mask[x]));
       } else {
-        uint32_t ey = r.flags;
+        uint32_t ey = r.flags | (r.tm ? (uint32_t)RF_TMEM : 0u);
         if (r.bw_warp >= 0) ey |= (uint32_t)r.bw_pre << 16 | (uint32_t)r.bw_warp << 28;
-        const uint32_t ez = (uint32_t)P.pos_of[x] | (uint32_t)(x ? P.pos_of[par[x]] : 0) << 10;
+        // the parent's row is read (v) or written (contribution) only by children that do not
+        // hand over in registers; such a parent is never a plain node, so its row is in shared memory
+        const uint32_t ez = r.srow | (uint32_t)(x && !fwd[x] ? erec(par[x]).srow : 0) << 10;
         const uint32_t ew = r.row | (uint32_t)(node_mask[x] ? P.vcopy_row[x] : 0) << 16;
-        P.prog.push_back(make_uint4(roff | r.len << 16, ey, ez, ew));
+        P.prog.push_back(make_uint4(r.ring, ey, ez, ew));
       }
     }
     Tk.p1 = (int)P.prog.size();
@@ -851,6 +927,18 @@ static int build_tape_program(cn_model *m, HClass &K) {
 
   // ---- dry run: the W record lists with the kernel's wait / signal rules -------------------------
   {
+    std::vector<int32_t> node_of_srow((size_t)P.n_srow + 1, -1);
+    std::vector<std::vector<int32_t>> node_of_slot(W);
+    for (int w = 0; w < W; ++w)
+      for (const Rec &r : recs[w]) {
+        if (r.type != 0) continue;
+        if (r.tm) {
+          if (node_of_slot[w].size() <= r.srow) node_of_slot[w].resize(r.srow + 1, -1);
+          node_of_slot[w][r.srow] = r.node;
+        } else {
+          node_of_srow[r.srow] = r.node;
+        }
+      }
     std::vector<int> pc(W), ctrv(W, 0), acc(n, 0);
     std::vector<uint8_t> done_e(n, 0), done_m(n, 0);
     for (int w = 0; w < W; ++w) pc[w] = P.task[w].p0;
@@ -861,11 +949,13 @@ static int build_tape_program(cn_model *m, HClass &K) {
         while (pc[w] < P.task[w].p1) {
           const uint4 e = P.prog[pc[w]];
           const uint32_t fl = e.y & 0xFFFFu;
-          if ((fl & RT_MASK) == RT_WAIT) {
+          if ((fl & RT_MASK) == RT_CHUNK) {
+          } else if ((fl & RT_MASK) == RT_WAIT) {
             if (ctrv[e.z & 0xFFFFu] < (int)(e.z >> 16)) break;
           } else if ((fl & RT_MASK) == RT_RUN) {
             for (uint32_t i = 0; i < ((e.x >> 16) & 255u); ++i) {
-              const int x = P.order[e.z + i];
+              const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + i]
+                                             : node_of_srow[(e.z & 1023u) + i];
               if (node_mask[x] || acc[x] != 0 || !fwd[x] || ch[x].size() > 1 ||
                   (ch[x].size() == 1 && (!done_e[ch[x][0]] || !fwd[ch[x][0]])) ||
                   (ch[x].size() == 1) != (i > 0 || (e.x >> 24 & 1u)))
@@ -873,12 +963,12 @@ static int build_tape_program(cn_model *m, HClass &K) {
               done_e[x] = 1;
             }
           } else if ((fl & RT_MASK) == RT_MECH) {
-            const int x = P.order[e.z & 1023u];
+            const int x = node_of_srow[e.z & 1023u];
             if (acc[x] != 0) return fail(CN_ERR_TOPOLOGY, "internal: tape program (mech order)");
             acc[x] = 1;
             done_m[x] = 1;
           } else {
-            const int x = P.order[e.z & 1023u];
+            const int x = (fl & RF_TMEM) ? node_of_slot[w][e.z & 1023u] : node_of_srow[e.z & 1023u];
             int want = node_mask[x] ? 1 : 0;
             for (int32_t c : ch[x]) {
               if (!done_e[c]) return fail(CN_ERR_TOPOLOGY, "internal: tape program (child order)");
@@ -888,7 +978,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
               return fail(CN_ERR_TOPOLOGY, "internal: tape program (contributions)");
             const uint32_t kind = fl & RK_KIND;
             if (kind >= RK_STORE) {
-              const int p = P.order[(e.z >> 10) & 1023u];
+              const int p = node_of_srow[(e.z >> 10) & 1023u];
               if (p != par[x] || (kind == RK_STORE) != (acc[p] == 0))
                 return fail(CN_ERR_TOPOLOGY, "internal: tape program (store/add)");
               acc[p]++;
@@ -912,19 +1002,20 @@ static int build_tape_program(cn_model *m, HClass &K) {
       progress = false;
       for (int w = 0; w < W; ++w) {
         const HTask &Tk = P.task[w];
-        while (pc[w] >= Tk.p0 + Tk.pm) {
+        while (pc[w] >= Tk.p0) {
           const uint4 e = P.prog[pc[w]];
           const uint32_t fl = e.y & 0xFFFFu;
           if ((fl & RT_MASK) == RT_RUN) {
             for (int i = (int)((e.x >> 16) & 255u) - 1; i >= 0; --i) {
-              const int x = P.order[e.z + i];
+              const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + (uint32_t)i]
+                                             : node_of_srow[(e.z & 1023u) + (uint32_t)i];
               if (!done_b[par[x]])
                 return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward run)");
               done_b[x] = 1;
             }
           } else if ((fl & RT_MASK) == RT_ELIM) {
             if ((fl & RF_WAIT_B) && ctrv[e.y >> 28] < (int)((e.y >> 16) & 0xFFFu)) break;
-            const int x = P.order[e.z & 1023u];
+            const int x = (fl & RF_TMEM) ? node_of_slot[w][e.z & 1023u] : node_of_srow[e.z & 1023u];
             if (x && !done_b[par[x]])
               return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward order)");
             done_b[x] = 1;
@@ -936,7 +1027,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
       }
     }
     for (int w = 0; w < W; ++w)
-      if (pc[w] >= P.task[w].p0 + P.task[w].pm)
+      if (pc[w] >= P.task[w].p0)
         return fail(CN_ERR_TOPOLOGY, "internal: tape program deadlocks (backward)");
   }
   return CN_OK;
@@ -1053,16 +1144,12 @@ static int build_layout(cn_model *m) {
   // 227 KB of shared memory next to the group's system (512 B per node)
   m->tape_W = 8;
   if (const char *e = std::getenv("CN_TAPE_W")) m->tape_W = std::min(16, std::max(1, std::atoi(e)));
-  m->tape_S = 4;
-  m->tape_CH = 8;
-  auto pow2 = [](int v, int lo, int hi) {
-    int p = lo;
-    while (p * 2 <= v && p * 2 <= hi) p *= 2;
-    return p;
-  };
-  if (const char *e = std::getenv("CN_TAPE_S")) m->tape_S = pow2(std::atoi(e), 2, 16);
-  if (const char *e = std::getenv("CN_TAPE_CH")) m->tape_CH = pow2(std::atoi(e), 4, 32);
-  while (m->tape_S * m->tape_CH > 128) m->tape_S /= 2;  // 16-bit ring offsets
+  m->tape_S = 2;
+  m->tape_CH = 16;
+  if (const char *e = std::getenv("CN_TAPE_S")) m->tape_S = std::min(4, std::max(2, std::atoi(e)));
+  if (const char *e = std::getenv("CN_TAPE_CH")) m->tape_CH = std::min(63, std::max(7, std::atoi(e)));
+  if (const char *e = std::getenv("CN_TAPE_TMEM")) m->tape_tmem = std::atoi(e) != 0;
+  if (const char *e = std::getenv("CN_TAPE_LEAF_FIRST")) m->tape_leaf_first = std::atoi(e) != 0;
   m->cell_tape.assign(nc, 0);
   for (HClass &K : m->cls) {
     K.count = (int64_t)K.cells.size();
@@ -1091,10 +1178,10 @@ static int build_layout(cn_model *m) {
     if (rc != CN_OK) return rc;
     if (K.tp.n_groups == 0) continue;
     // the CTA must fit: rings + system + two program buffers + counters and barriers
-    const size_t sys_cap = (size_t)std::max(m->tape_sys_cap, K.n);
+    const size_t sys_cap = (size_t)std::max(m->tape_sys_cap, K.tp.n_srow);
     const size_t prog_cap = std::max((size_t)m->tape_prog_cap, K.tp.prog.size());
     const size_t need = (size_t)m->tape_W * m->tape_S * m->tape_CH * 256 + sys_cap * 512 +
-                        2 * prog_cap * 16 + 64 + ((size_t)m->tape_W * m->tape_S + 2) * 8;
+                        2 * prog_cap * 16 + 64 + ((size_t)m->tape_W * m->tape_S + 2) * 8 + 16;
     if (need > 227 * 1024) {
       K.tp.n_groups = 0;
       K.tp.n_cells = 0;
@@ -1104,7 +1191,7 @@ static int build_layout(cn_model *m) {
     K.tp.prog_off = prog_total;
     prog_total += (int)K.tp.prog.size();
     m->tape_prog_cap = std::max(m->tape_prog_cap, (int)K.tp.prog.size());
-    m->tape_sys_cap = std::max(m->tape_sys_cap, K.n);
+    m->tape_sys_cap = std::max(m->tape_sys_cap, K.tp.n_srow);
   }
 
   // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
@@ -1590,7 +1677,7 @@ static int finalize(cn_model *m, double dt) {
         const HTask &Tk = P.task[w];
         // program positions are relative to the class's program (as it sits in shared memory)
         ttask[kc * (size_t)m->tape_W + w] =
-            TapeTask{Tk.p0, Tk.p1, Tk.pm, 0, Tk.row0, Tk.nrows, Tk.mrows, 0};
+            TapeTask{Tk.p0, Tk.p1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.nrows, Tk.head, 0};
       }
     }
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
@@ -1598,8 +1685,7 @@ static int finalize(cn_model *m, double dt) {
     H.tgrp = dtg; H.tcls = dtc; H.prog = dpg; H.ttask = dtt;
     H.tape_W = m->tape_W;
     H.tape_S = m->tape_S;
-    H.tape_lgCH = 0;
-    while ((1 << H.tape_lgCH) < m->tape_CH) H.tape_lgCH++;
+    H.tape_CH = m->tape_CH;
     H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
     H.tape_sys_cap = std::max(m->tape_sys_cap, 1);
     for (int t = 0; t < nt; ++t) {
@@ -1709,7 +1795,7 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
 static size_t tape_smem_bytes(const cn_model *m) {
   const size_t W = (size_t)m->tape_W;
   return W * m->tape_S * m->tape_CH * 256 + (size_t)m->hm.tape_sys_cap * 512 +
-         2 * (size_t)m->hm.tape_prog_cap * 16 + 64 + (W * m->tape_S + 2) * 8;
+         2 * (size_t)m->hm.tape_prog_cap * 16 + 64 + (W * m->tape_S + 2) * 8 + 16;
 }
 
 // Persistent CTAs: as many as fit the device at once (shared memory decides), each looping over
@@ -1728,10 +1814,18 @@ static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
       return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * m->tape_W, smem);
+    // Two CTAs per SM when they fit: 2 x 256 threads x 128 registers fill the register file,
+    // each CTA allocates half of the SM's tensor memory, and shared memory decides.  (The
+    // occupancy API answers 1 for this kernel whatever the shared-memory size; the hardware
+    // does run two CTAs side by side -- measured.)
+    int smem_sm = 0;
+    e = cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     if (e != cudaSuccess) return e;
-    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-    if (const char *s = std::getenv("CN_TAPE_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, std::atoi(s)));
+    per_sm = (m->tape_W <= 8 && 2 * (smem + 1024) <= (size_t)smem_sm) ? 2 : 1;
+    if (const char *s = std::getenv("CN_TAPE_CTAS_PER_SM")) per_sm = std::max(1, std::min(2, std::atoi(s)));
+    if (std::getenv("CN_DEBUG"))
+      fprintf(stderr, "[cn] tape kernel: %zu B smem, %d threads, %d CTAs/SM\n", smem,
+              32 * m->tape_W, per_sm);
     m->tape_ctas = std::min(m->hm.n_tgroup, sms * per_sm);
   }
   kern<<<m->tape_ctas, 32 * m->tape_W, smem, m->stream>>>(m->hm, k, mode);
@@ -1968,8 +2062,8 @@ extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
   info[3] = r;
   info[4] = (int64_t)m->tgrp.size();
   info[5] = m->n_tape * 8;
-  info[6] = 0;  // no scratch tape: the system of a group lives in shared memory
-  info[7] = m->tape_W;
+  info[6] = m->hm.n_tgroup > 0 ? (int64_t)tape_smem_bytes(m) : 0;  // valid after the first cn_run
+  info[7] = (int64_t)m->tape_W | (int64_t)m->tape_ctas << 8 | (int64_t)m->tape_sys_cap << 24;
   return CN_OK;
 }
 
@@ -2037,3 +2131,9 @@ extern "C" int cn_debug_tasks(const cn_model *m, int32_t *out, int32_t cap) {
   }
   return 0;
 }
+
+#ifdef CN_TRACE
+extern "C" int cn_debug_trace(long long *out) {
+  return (int)cudaMemcpyFromSymbol(out, cn::g_trace, sizeof(long long) * 148 * 16 * 8 * 8);
+}
+#endif

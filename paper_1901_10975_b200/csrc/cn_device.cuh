@@ -66,30 +66,34 @@ struct TapeClass {
   int32_t n, prog_off, prog_len, n_rows;
 };
 
-// the part of a class's program that one warp runs: records [p0, p1) (the first pm of them are
-// mechanism records) and its segment of the group's tape (the first mrows rows hold the
-// mechanism records)
+// the part of a class's program that one warp runs: records [p0, p1) and its segment of the
+// group's tape, which is cut into chunks of whole records (at most tape_CH rows each); head holds
+// the row counts of the first four chunks (8 bits each), which are requested before the program
+// starts
 struct TapeTask {
-  int32_t p0, p1, pm, pad0;
-  uint32_t row0, nrows, mrows, pad1;
+  int32_t p0, p1, nchunk, tm_base;  // tm_base: first tensor-memory slot of the warp
+  uint32_t row0, nrows, head, pad1;
 };
 
 // Program record (uint4) of the interleaved kernel: one per run of plain chain nodes (RUN), per
-// other node elimination (ELIM), per node with distributed mechanisms (MECH) and per cross-warp
-// dependency (WAIT).  Rows are counted from the start of the warp's segment of the tape.
+// other node elimination (ELIM), per node with distributed mechanisms (MECH), per chunk of the
+// warp's tape segment (CHUNK) and per cross-warp dependency (WAIT).
 //   RUN   x = ring byte offset of the first node's record (16) | nodes in the run (8) | first
 //             node takes a contribution in registers (bit 24)
-//         y = RT_RUN     z = system row of the first node     w = first tape row of the first
-//             node's record (16, relative to the group) | row count of the segment up to and
-//             including the first node's record (16)
-//   ELIM  x = ring byte offset (16) | rows of the record (8)
+//         y = RT_RUN     z = system row of the first node (10), or, with bit 20 set, its slot in
+//             the warp's share of tensor memory     w = first tape row of the first node's record
+//   ELIM  x = ring byte offset (16)
 //         y = flags (16) | backward wait: position (12) and warp (4)
 //         z = own system row (10) | parent's system row (10)
 //         w = first tape row of the record (16) | tape row of the v copy in the node's mechanism
 //             record (16)
-//   MECH  x = ring byte offset (16) | rows of the record (8)
+//   MECH  x = ring byte offset (16)
 //         y = flags (16) | first tape row of the record (16)
 //         z = system row of the node     w = mask of the distributed tables on the node
+//   CHUNK the records that follow sit in the next chunk: the stage of the chunk before it is free
+//         x = first row (relative to the warp's segment) of the chunk to request into that stage
+//             (16) | its rows (8; 0: nothing left to request)
+//         y = RT_CHUNK   z = stage to fill (16) | stage to wait for (16)
 //   WAIT  y = RT_WAIT    z = warp (16) | position (16)
 enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
        RF_FWD_IN = 4,     // the previous record of this warp handed its contribution in registers
@@ -99,13 +103,15 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
        RF_SIG_F = 64,     // publish this warp's position after the record, forward / backward
        RF_SIG_B = 128,
        RF_WAIT_B = 256,   // backward: wait for the parent's warp first
+       RF_TMEM = 512,     // the node's own row is a tensor-memory slot of the warp (z, low 10 bits)
        RM_HAS_CAI = 1, RM_NEED_ICA = 2,
-       RT_ELIM = 0, RT_MECH = 1 << 14, RT_WAIT = 2 << 14, RT_RUN = 3 << 14, RT_MASK = 3 << 14 };
+       RT_ELIM = 0, RT_MECH = 1 << 13, RT_WAIT = 2 << 13, RT_RUN = 3 << 13, RT_CHUNK = 4 << 13,
+       RT_MASK = 7 << 13 };
 
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
   int32_t n_tgroup, tape_prog_cap, tape_sys_cap, tape_W;
-  int32_t tape_S, tape_lgCH, pad_t1, pad_t2;  // ring: S stages (power of 2) of 2^lgCH rows
+  int32_t tape_S, tape_CH, pad_t1, pad_t2;  // ring of a warp: S stages of CH rows
   const TapeGroup *tgrp;
   const TapeClass *tcls;
   const TapeTask *ttask;        // [n_class][tape_W]

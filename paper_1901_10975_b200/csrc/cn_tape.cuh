@@ -59,7 +59,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}" ::"r"(bar), "r"(parity)
       : "memory");
 }
-// per-warp progress counters (shared memory): release by one lane after __syncwarp, acquire by all
+// Per-warp progress counters in shared memory.  Producer: all lanes write their system rows
+// (shared memory), __syncwarp, then one lane stores the counter with release semantics; consumer:
+// every lane polls the counter with acquire semantics, then reads the rows.  (Plain volatile
+// accesses are NOT enough: measured, the rows can be read before they are written.)
 __device__ __forceinline__ void ctr_publish(uint32_t addr, uint32_t val) {
   asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(val) : "memory");
 }
@@ -82,31 +85,60 @@ __device__ __forceinline__ double rcp_fast(double x) {
   return fma(r, e, r);
 }
 
-// x / (exp(x/y) - 1) for y = 10 (both HH uses), removable singularity as in vtrap()
-__device__ __forceinline__ double vtrap10(double x) {
-  const double u = x * 0.1;
-  if (fabs(u) < 1e-6) return 10.0 * (1.0 - 0.5 * u);
-  return x * rcp_fast(exp(u) - 1.0);
+// exp(x) for |x| < 700 to ~1 ulp without the special-case handling of the library routine:
+// x = n ln2 + r with |r| <= ln2/2 (two-part ln2), Taylor polynomial of degree 13 (truncation
+// 4e-18), scaling by 2^n through the exponent field.  Every argument here is a bounded rate
+// exponent (|x| < 50 for |v| < 500 mV).
+__device__ __forceinline__ double exp_lean(double x) {
+  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);  // round to nearest integer
+  const double nf = t - 6755399441055744.0;
+  double r = fma(nf, -6.93147180369123816490e-01, x);
+  r = fma(nf, -1.90821492927058770002e-10, r);
+  double p = 1.6059043836821613e-10;            // 1/13!
+  p = fma(p, r, 2.08767569878681e-09);          // 1/12!
+  p = fma(p, r, 2.505210838544172e-08);         // 1/11!
+  p = fma(p, r, 2.755731922398589e-07);         // 1/10!
+  p = fma(p, r, 2.7557319223985893e-06);        // 1/9!
+  p = fma(p, r, 2.48015873015873e-05);          // 1/8!
+  p = fma(p, r, 1.984126984126984e-04);         // 1/7!
+  p = fma(p, r, 1.3888888888888889e-03);        // 1/6!
+  p = fma(p, r, 8.333333333333333e-03);         // 1/5!
+  p = fma(p, r, 4.1666666666666664e-02);        // 1/4!
+  p = fma(p, r, 1.6666666666666666e-01);        // 1/3!
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);
+  const int n = __double2loint(t);
+  return p * __hiloint2double((n + 1023) << 20, 0);
 }
 
 // HH gates advanced over dt with cnexp at the new v: y += (1 - exp(-dt*q10*(a+b))) * (a/(a+b) - y).
 // Same formulas as hh_rates() + cnexp(); divisions by constants are multiplications by their
-// reciprocals and 1/tau is never formed (differences of a few ulp).
+// reciprocals, 1/tau is never formed, and the three exponentials in v/10 share one evaluation
+// (exp(-(v+40)/10) = exp(-(v+35)/10) e^-0.5, exp(-(v+55)/10) = exp(-(v+35)/10) e^-2): differences
+// of a few ulp in the rates.
 __device__ __forceinline__ void hh_advance(double v, double q10dt, double &m, double &h,
                                            double &n) {
-  double al, be, s;
-  al = 0.1 * vtrap10(-(v + 40.0));
-  be = 4.0 * exp(-(v + 65.0) * (1.0 / 18.0));
+  const double x65 = v + 65.0;
+  const double e10 = exp_lean(-(v + 35.0) * 0.1);
+  double al, be, s, u;
+  // m: alpha = 0.1 vtrap(-(v+40), 10), removable singularity as in vtrap()
+  u = -(v + 40.0) * 0.1;
+  al = fabs(u) < 1e-6 ? 1.0 - 0.5 * u : u * rcp_fast(e10 * 0.60653065971263342 - 1.0);
+  be = 4.0 * exp_lean(x65 * (-1.0 / 18.0));
   s = al + be;
-  m += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - m);
-  al = 0.07 * exp(-(v + 65.0) * 0.05);
-  be = rcp_fast(exp(-(v + 35.0) * 0.1) + 1.0);
+  m += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - m);
+  // h
+  al = 0.07 * exp_lean(x65 * -0.05);
+  be = rcp_fast(e10 + 1.0);
   s = al + be;
-  h += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - h);
-  al = 0.01 * vtrap10(-(v + 55.0));
-  be = 0.125 * exp(-(v + 65.0) * 0.0125);
+  h += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - h);
+  // n: alpha = 0.01 vtrap(-(v+55), 10)
+  u = -(v + 55.0) * 0.1;
+  al = fabs(u) < 1e-6 ? 0.1 * (1.0 - 0.5 * u) : 0.1 * u * rcp_fast(e10 * 0.1353352832366127 - 1.0);
+  be = 0.125 * exp_lean(x65 * -0.0125);
   s = al + be;
-  n += (1.0 - exp(-q10dt * s)) * (al * rcp_fast(s) - n);
+  n += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - n);
 }
 
 enum { TM_ADVANCE = 1, TM_FLUSH = 2 };
@@ -213,15 +245,42 @@ __device__ __forceinline__ void mech_record(const DModel &M, const unsigned char
 
 // One CTA = W warps = one group of 32 cells at a time (persistent over groups).  See the header
 // of this file and the record layout in cn_device.cuh.
-// Shared memory: W rings of S << lgCH rows | system: tape_sys_cap x (32 + 32) doubles | two
-// program buffers of tape_prog_cap records | 16 progress counters | W*S + 2 mbarriers.
+// Shared memory: W rings of S stages x CH rows | system: tape_sys_cap x (32 + 32) doubles | two
+// program buffers of tape_prog_cap records | 16 progress counters | W*S + 2 mbarriers | TMEM base.
+// Tensor memory as a per-lane scratchpad (Blackwell: 512 columns x 128 lanes x 32 bit per SM; a
+// warp addresses the 32 lanes of its quarter, thread i <-> lane i): (multiplier, reduced rhs) of a
+// plain chain node = 4 columns.  SASS: STTM / LDTM.
+__device__ __forceinline__ void tm_store2(uint32_t taddr, double a, double b) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr),
+               "r"(__double2loint(a)), "r"(__double2hiint(a)), "r"(__double2loint(b)),
+               "r"(__double2hiint(b))
+               : "memory");
+}
+__device__ __forceinline__ void tm_load2(uint32_t taddr, double &a, double &b) {
+  uint32_t r0, r1, r2, r3;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+               : "r"(taddr)
+               : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  a = __hiloint2double((int)r1, (int)r0);
+  b = __hiloint2double((int)r3, (int)r2);
+}
+constexpr int CN_TMEM_COLS = 256;  // per CTA: two CTAs share the 512 columns of an SM
+
+#ifdef CN_TRACE
+__device__ long long g_trace[148 * 16 * 8 * 8];
+#define CN_TR(i) if (lane == 0 && it < 8 && blockIdx.x < 148) g_trace[((blockIdx.x * 16 + warp) * 8 + it) * 8 + (i)] = clock64()
+#else
+#define CN_TR(i)
+#endif
 template <int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constant__ DModel M,
+__global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __grid_constant__ DModel M,
                                                           int64_t k, int mode) {
   extern __shared__ __align__(128) unsigned char sm_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int W = M.tape_W, S = M.tape_S, lgCH = M.tape_lgCH, CH = 1 << lgCH;
-  const uint32_t RB = (uint32_t)(S << lgCH) * 256u;  // ring bytes per warp
+  const int W = M.tape_W, S = M.tape_S, CH = M.tape_CH;
+  const uint32_t RB = (uint32_t)(S * CH) * 256u;  // ring bytes per warp
   const uint32_t lane8 = (uint32_t)lane * 8u;
   const unsigned char *ringc = sm_raw + (size_t)warp * RB + lane8;  // this lane's column
   double *sys_l = reinterpret_cast<double *>(sm_raw + (size_t)W * RB) + lane;
@@ -246,48 +305,41 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
+  if (blockIdx.x >= ngrp) return;
+  uint32_t *tm_base_s = reinterpret_cast<uint32_t *>(mbar_all + (size_t)W * S + 2);
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                     smem_u32(tm_base_s)),
+                 "n"(CN_TMEM_COLS)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  // this warp's lanes of tensor memory (quarter warp % 4); its slots start at TapeTask::tm_base
+  const uint32_t tm_warp = *tm_base_s + (((uint32_t)(warp & 3) * 32u) << 16);
 
-  // ring state (uniform over the warp): chunk c of a segment goes to stage c % S
-  uint32_t phase = 0;      // bit s: parity the next wait on stage s looks for
-  int cw = 0, ci = 0;      // chunks waited for / issued so far in the current segment
+  // ring: chunk c of a segment (whole records, at most CH rows) goes to stage c % S; the program's
+  // CHUNK records say when a stage is free again and what to request into it
+  uint32_t phase = 0;  // bit s: parity the next wait on stage s looks for
   const double *seg = nullptr;
-  int seg_rows = 0, nchunk = 0;
-  auto issue = [&](int c) {  // lane 0: chunk c of the current segment
-    const int rows = min(CH, seg_rows - (c << lgCH));
-    const uint32_t bytes = (uint32_t)rows * 256u;
-    const uint32_t s = (uint32_t)c & (uint32_t)(S - 1);
-    mbar_expect_tx(bar_s + 8 * s, bytes);
-    bulk_g2s(ring_s + ((s << lgCH) << 8), seg + ((size_t)c << (lgCH + 5)), bytes, bar_s + 8 * s);
-  };
-  // rows [0, e) of the segment must have landed
-  auto ring_need = [&](int e) {
-    const int need = (e + CH - 1) >> lgCH;
-    while (cw < need) {
-      const uint32_t s = (uint32_t)cw & (uint32_t)(S - 1);
-      mbar_wait(bar_s + 8 * s, (phase >> s) & 1u);
-      phase ^= 1u << s;
-      ++cw;
-    }
-  };
-  // rows [0, e) are consumed: refill the stages they occupied, S chunks ahead
-  auto ring_done = [&](int e) {
-    const int lim = min(nchunk, (e >> lgCH) + S);
-    if (ci < lim) {
-      __syncwarp();
-      if (lane == 0)
-        for (int c = ci; c < lim; ++c) issue(c);
-      ci = lim;
-    }
+  auto issue = [&](uint32_t stage, uint32_t row, uint32_t rows) {  // one lane
+    const uint32_t bytes = rows * 256u;
+    mbar_expect_tx(bar_s + 8 * stage, bytes);
+    bulk_g2s(ring_s + stage * (uint32_t)(CH * 256), seg + (size_t)row * 32, bytes,
+             bar_s + 8 * stage);
   };
   auto start_segment = [&](const TapeGroup &g, const TapeTask &t) {
     seg = M.tape + g.tape_base + (size_t)t.row0 * 32;
-    seg_rows = (int)(flush ? t.mrows : t.nrows);
-    nchunk = (seg_rows + CH - 1) >> lgCH;
-    cw = 0;
-    ci = min(S, nchunk);
-    if (lane == 0)
-      for (int c = 0; c < ci; ++c) issue(c);
+    if (lane == 0) {
+      uint32_t row = 0;
+      for (int c = 0; c < S && c < t.nchunk; ++c) {
+        const uint32_t rows = (t.head >> (8 * c)) & 255u;
+        issue((uint32_t)c, row, rows);
+        row += rows;
+      }
+    }
   };
   auto load_program = [&](const TapeClass &c, int buf) {  // one thread
     const uint32_t bytes = (uint32_t)c.prog_len * 16u;
@@ -297,7 +349,6 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
   };
 
   int g = blockIdx.x;
-  if (g >= ngrp) return;
   TapeGroup tg = M.tgrp[g];
   TapeClass tc = M.tcls[tg.cls];
   TapeTask tk = M.ttask[(size_t)tg.cls * W + warp];
@@ -317,11 +368,12 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
       tkn = M.ttask[(size_t)tgn.cls * W + warp];
       if (threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
     }
+    CN_TR(0);
     mbar_wait(pbar_s + 8 * (it & 1), (it >> 1) & 1);
+    CN_TR(1);
     const uint4 *prog = progbuf + (size_t)(it & 1) * M.tape_prog_cap;
     double *__restrict__ tape_l = M.tape + tg.tape_base + lane;
-    const int p0 = tk.p0, p1 = flush ? tk.p0 + tk.pm : tk.p1;
-    const int row0 = (int)tk.row0;
+    const int p0 = tk.p0, p1 = tk.p1;
 
     // ========================================================================================
     // forward: mechanism records (nrn_state of the previous step, nrn_cur), then tree terms and
@@ -333,15 +385,32 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
       const uint32_t ty = e.y & RT_MASK;
       if (ty == RT_RUN) {
         // a run of plain chain nodes: each hands its contribution to the next in registers
+        if (flush) continue;
         const unsigned char *rb = ringc + (e.x & 0xFFFFu);
-        double *srow = sys_l + e.z * 64u;
-        int rend = (int)(e.w >> 16);
         if (!(e.x & (1u << 24))) {
           accD = 0.0;
           accR = 0.0;
         }
+        if (e.z & (1u << 20)) {  // (multiplier, reduced rhs) to the warp's tensor-memory slots
+          uint32_t ta = tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u)) * 4u;
+#pragma unroll 1
+          for (int q = (int)((e.x >> 16) & 255u); q; --q) {
+            const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
+            const double D = CN_RD(rb, 2) + accD;
+            const double R = (CN_RD(rb, 4) + CN_RD(rb, 3)) + accR;
+            const double rinv = rcp_fast(D);
+            const double f = a * rinv;
+            tm_store2(ta, b * rinv, R * rinv);
+            accD = -(f * b);
+            accR = -(f * R);
+            rb += 5 * 256;
+            ta += 4;
+          }
+          continue;
+        }
+        double *srow = sys_l + (e.z & 1023u) * 64u;
+#pragma unroll 1
         for (int q = (int)((e.x >> 16) & 255u); q; --q) {
-          ring_need(rend);
           const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
           const double D = CN_RD(rb, 2) + accD;
           const double R = (CN_RD(rb, 4) + CN_RD(rb, 3)) + accR;
@@ -351,24 +420,32 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
           srow[32] = R * rinv;
           accD = -(f * b);
           accR = -(f * R);
-          ring_done(rend);
           rb += 5 * 256;
           srow += 64;
-          rend += 5;
         }
         continue;
       }
+      if (ty == RT_CHUNK) {
+        // the previous chunk is consumed: refill its stage, then wait for the next chunk
+        const uint32_t rows = (e.x >> 16) & 255u;
+        if (rows) {
+          __syncwarp();
+          if (lane == 0) issue(e.z & 0xFFFFu, e.x & 0xFFFFu, rows);
+        }
+        const uint32_t s = e.z >> 16;
+        mbar_wait(bar_s + 8 * s, (phase >> s) & 1u);
+        phase ^= 1u << s;
+        continue;
+      }
       if (ty == RT_WAIT) {
-        ctr_wait(ctr_s + 4 * (e.z & 0xFFFFu), base + (e.z >> 16));
+        if (!flush) ctr_wait(ctr_s + 4 * (e.z & 0xFFFFu), base + (e.z >> 16));
         continue;
       }
       const uint32_t fl = e.y & 0xFFFFu;
       const unsigned char *rb = ringc + (e.x & 0xFFFFu);
       double *srow = sys_l + (e.z & 1023u) * 64u;
-      int rend;
       if (ty == RT_ELIM) {
-        rend = (int)(e.w & 0xFFFFu) - row0 + (int)((e.x >> 16) & 255u);
-        ring_need(rend);
+        if (flush) continue;
         const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
         double D = CN_RD(rb, 2), R = CN_RD(rb, 4) + CN_RD(rb, 3);
         if (fl & RF_FWD_IN) {
@@ -410,11 +487,13 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
             }
           }
         }
-        srow[0] = mult;
-        srow[32] = R * rinv;
+        if (fl & RF_TMEM) {
+          tm_store2(tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u)) * 4u, mult, R * rinv);
+        } else {
+          srow[0] = mult;
+          srow[32] = R * rinv;
+        }
       } else {  // RT_MECH
-        rend = (int)(e.y >> 16) - row0 + (int)((e.x >> 16) & 255u);
-        ring_need(rend);
         double gD, gR;
         mech_record(M, rb, tape_l + (e.y >> 16) * 32u, fl, e.w, mode, dt, q10dt, gD, gR);
         if (!flush) {
@@ -426,8 +505,9 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
         __syncwarp();
         if (lane == 0) ctr_publish(ctr_s + 4 * warp, base + (uint32_t)(j - p0) + 1u);
       }
-      ring_done(rend);
     }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    CN_TR(2);
     // this warp's ring is idle until the next group: start loading it now
     __syncwarp();
     if (has_next) start_segment(tgn, tkn);
@@ -438,14 +518,28 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
     if (!flush) {
       const uint32_t nrec = (uint32_t)(tk.p1 - tk.p0);
       double v_prev = 0.0;
-      for (int j = tk.p1 - 1; j >= tk.p0 + tk.pm; --j) {
+      for (int j = tk.p1 - 1; j >= tk.p0; --j) {
         const uint4 e = prog[j];
         const uint32_t ty = e.y & RT_MASK;
         if (ty == RT_RUN) {
           // the parent of the run's last node is the node just solved
           const int q = (int)((e.x >> 16) & 255u);
-          const double *srow = sys_l + (e.z + (uint32_t)q) * 64u;
           double *trow = tape_l + ((e.w & 0xFFFFu) + 5u * (uint32_t)q + 4u) * 32u;
+          if (e.z & (1u << 20)) {
+            uint32_t ta = tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u) + (uint32_t)q) * 4u;
+#pragma unroll 1
+            for (int i = q; i; --i) {
+              ta -= 4;
+              trow -= 5 * 32;
+              double mult, rp;
+              tm_load2(ta, mult, rp);
+              v_prev = fma(-mult, v_prev, rp);
+              *trow = v_prev;
+            }
+            continue;
+          }
+          const double *srow = sys_l + ((e.z & 1023u) + (uint32_t)q) * 64u;
+#pragma unroll 2
           for (int i = q; i; --i) {
             srow -= 64;
             trow -= 5 * 32;
@@ -456,13 +550,23 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
         }
         if (ty != RT_ELIM) continue;
         const uint32_t fl = e.y & 0xFFFFu;
-        if (fl & RF_WAIT_B) ctr_wait(ctr_s + 4 * (e.y >> 28), base + ((e.y >> 16) & 0xFFFu));
+        if (fl & RF_WAIT_B) {
+          ctr_wait(ctr_s + 4 * (e.y >> 28), base + ((e.y >> 16) & 0xFFFu));
+          if (j == tk.p1 - 1) { CN_TR(3); }
+        }
         double *srow = sys_l + (e.z & 1023u) * 64u;
         const uint32_t kind = fl & RK_KIND;
         double vp = v_prev;
         if (kind >= RK_STORE) vp = sys_l[((e.z >> 10) & 1023u) * 64u + 32];
-        const double v = fma(-srow[0], vp, srow[32]);  // the root's multiplier is 0
-        srow[32] = v;  // children that did not hand over in registers read it here
+        double mult, rp;
+        if (fl & RF_TMEM) {
+          tm_load2(tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u)) * 4u, mult, rp);
+        } else {
+          mult = srow[0];
+          rp = srow[32];
+        }
+        const double v = fma(-mult, vp, rp);  // the root's multiplier is 0
+        if (fl & RF_HAS_ACC) srow[32] = v;  // children that did not hand over in registers read it
         v_prev = v;
         tape_l[(e.w & 0xFFFFu) * 32u + 4 * 32] = v;
         if (fl & RF_MECHV) tape_l[(e.w >> 16) * 32u] = v;
@@ -498,11 +602,19 @@ __global__ void __launch_bounds__(MAXT, 1) tape_step_kernel(const __grid_constan
         }
       }
     }
+    CN_TR(4);
     __syncthreads();  // the system rows and counters of this group are dead from here on
+    CN_TR(5);
     tg = tgn;
     tc = tcn;
     tk = tkn;
   }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0)
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tm_base_s),
+                 "n"(CN_TMEM_COLS)
+                 : "memory");
 #undef CN_RD
 }
 
