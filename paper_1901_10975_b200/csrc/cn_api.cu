@@ -109,7 +109,11 @@ struct HTable {
   std::vector<int64_t> cell_inst;
 };
 
-struct HTask { int p0 = 0, p1 = 0, nchunk = 0, tm_base = 0; uint32_t row0 = 0, nrows = 0, head = 0; };
+struct HTask {
+  int p0 = 0, p1 = 0, b0 = 0, b1 = 0;  // forward / backward records in the class's program
+  int nchunk = 0, tm_base = 0;
+  uint32_t row0 = 0, nrows = 0, head = 0;
+};
 
 struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh)
   std::vector<HTask> task;                   // one per warp
@@ -653,6 +657,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
     uint32_t row = 0, len = 0, ring = 0;    // first tape row, rows, byte offset in the ring
     uint32_t srow = 0;                      // row of the shared-memory system, or TMEM slot
     bool tm = false;
+    int unit = -1;                          // backward unit (RUN or single ELIM record) of the node
   };
   std::vector<std::vector<Rec>> recs(W);
   std::vector<int> e_pre(n, -1), m_pre(n, -1);  // pre-index of a node's records in its warp's list
@@ -711,13 +716,6 @@ static int build_tape_program(cn_model *m, HClass &K) {
       if (lw >= 0) add_dep(rc, e_warp[c], lw, lp);
       lw = e_warp[c];
       lp = e_pre[c];
-      // backward: c reads v of x from x's system row
-      if (e_warp[c] != e_warp[x]) {
-        rc.bw_warp = e_warp[x];
-        rc.bw_pre = e_pre[x];
-        rc.flags |= RF_WAIT_B;
-        r.flags |= RF_SIG_B;
-      }
     }
     if (lw >= 0) {
       r.flags |= RF_HAS_ACC;
@@ -867,23 +865,6 @@ static int build_tape_program(cn_model *m, HClass &K) {
     Tk.head = 0;
     for (uint32_t c = 0; c < 4 && c < chunks[w].size(); ++c) Tk.head |= chunks[w][c].second << (8 * c);
   }
-  // backward waits: drop those an earlier (in backward order) wait of the same warp covers
-  for (int w = 0; w < W; ++w) {
-    std::vector<int> seen(W, -1);  // largest backward position waited for so far, per warp
-    for (int i = (int)recs[w].size() - 1; i >= 0; --i) {
-      Rec &r = recs[w][i];
-      if (r.bw_warp < 0) continue;
-      const int nrec2 = (int)fin[r.bw_warp].size();
-      const int posb = nrec2 + (nrec2 - recs[r.bw_warp][r.bw_pre].fidx);
-      if (seen[r.bw_warp] >= posb) {
-        r.flags &= ~(uint32_t)RF_WAIT_B;
-        r.bw_warp = -1;
-      } else {
-        seen[r.bw_warp] = posb;
-        r.bw_pre = posb;  // from here on: the position itself
-      }
-    }
-  }
   // encoding (layout of the records: cn_device.cuh)
   for (int w = 0; w < W; ++w) {
     HTask &Tk = P.task[w];
@@ -913,16 +894,148 @@ static int build_tape_program(cn_model *m, HClass &K) {
       } else if (r.type == 1) {
         P.prog.push_back(make_uint4(r.ring, r.flags | r.row << 16, r.srow, node_mask[x]));
       } else {
-        uint32_t ey = r.flags | (r.tm ? (uint32_t)RF_TMEM : 0u);
-        if (r.bw_warp >= 0) ey |= (uint32_t)r.bw_pre << 16 | (uint32_t)r.bw_warp << 28;
-        // the parent's row is read (v) or written (contribution) only by children that do not
-        // hand over in registers; such a parent is never a plain node, so its row is in shared memory
-        const uint32_t ez = r.srow | (uint32_t)(x && !fwd[x] ? erec(par[x]).srow : 0) << 10;
+        const uint32_t ey = r.flags | (r.tm ? (uint32_t)RF_TMEM : 0u);
+        // the parent's row is written (contribution) or read (v) only if it collects contributions
+        // (RF_HAS_ACC); such a row is always in shared memory
+        const uint32_t ez =
+            r.srow | (uint32_t)(x && (erec(par[x]).flags & RF_HAS_ACC) ? erec(par[x]).srow : 0) << 10;
         const uint32_t ew = r.row | (uint32_t)(node_mask[x] ? P.vcopy_row[x] : 0) << 16;
         P.prog.push_back(make_uint4(r.ring, ey, ez, ew));
       }
     }
     Tk.p1 = (int)P.prog.size();
+  }
+
+  // ---- 5. backward program -----------------------------------------------------------------------
+  // Back-substitution visits parents before children.  Its order is NOT the reverse of the
+  // forward lists: per warp, the units (a RUN or a single ELIM record) whose parent is solved are
+  // taken upper nodes first (every other warp waits for those), then depth-first.  A unit whose
+  // last-solved node does not keep v in its system row (no RF_HAS_ACC) must be followed by its
+  // only child at once (v travels in a register); every other unit reads the parent's v from the
+  // parent's row (RF_BW_ROW) unless it happens to follow its parent directly.
+  {
+    struct Unit { int w; int fin_idx; int top, bottom; bool stores_v; int warp_pos = -1; };
+    std::vector<Unit> units;
+    for (int w = 0; w < W; ++w) {
+      int fi = 0;
+      for (const Fin &F : fin[w]) {
+        if (F.type == 0 || F.type == 3) {
+          Unit u;
+          u.w = w;
+          u.fin_idx = fi;
+          u.bottom = recs[w][F.pre].node;
+          u.top = recs[w][F.pre + F.cnt - 1].node;
+          u.stores_v = F.type == 0 && (recs[w][F.pre].flags & RF_HAS_ACC);
+          for (int i = 0; i < F.cnt; ++i) recs[w][F.pre + i].unit = (int)units.size();
+          units.push_back(u);
+        }
+        ++fi;
+      }
+    }
+    const int nu = (int)units.size();
+    std::vector<std::vector<int>> kids(nu);  // same-warp child units, the register child first
+    std::vector<int> punit(nu, -1);
+    std::vector<int> depth(n, 0);
+    for (int x = 1; x < n; ++x) depth[x] = depth[par[x]] + 1;
+    for (int u = 0; u < nu; ++u) {
+      const int t = units[u].top;
+      if (t == 0) continue;
+      punit[u] = erec(par[t]).unit;
+      if (units[punit[u]].w == units[u].w) {
+        if (fwd[t]) kids[punit[u]].insert(kids[punit[u]].begin(), u);
+        else kids[punit[u]].push_back(u);
+      }
+    }
+    std::vector<std::vector<int>> blist(W);
+    std::vector<uint8_t> bw_row(nu, 0);
+    for (int w = 0; w < W; ++w) {
+      // upper units by depth, others depth-first (a stack)
+      auto upper = [&](int u) { return sw[units[u].top] > gran; };
+      std::vector<int> heap, stack;
+      auto push = [&](int u) { (upper(u) ? heap : stack).push_back(u); };
+      for (int u = nu - 1; u >= 0; --u)
+        if (units[u].w == w && (punit[u] < 0 || units[punit[u]].w != w)) push(u);
+      int forced = -1, last = -1;
+      while (forced >= 0 || !heap.empty() || !stack.empty()) {
+        int u;
+        if (forced >= 0) {
+          u = forced;
+        } else if (!heap.empty()) {
+          auto it = std::min_element(heap.begin(), heap.end(), [&](int a, int b) {
+            return depth[units[a].top] < depth[units[b].top];
+          });
+          u = *it;
+          heap.erase(it);
+        } else {
+          u = stack.back();
+          stack.pop_back();
+        }
+        // v of the parent: register if the parent unit was solved just before, else its row
+        if (punit[u] >= 0 && !(last == punit[u] && fwd[units[u].top])) bw_row[u] = 1;
+        units[u].warp_pos = (int)blist[w].size();
+        blist[w].push_back(u);
+        last = u;
+        forced = -1;
+        if (!units[u].stores_v) {
+          if (kids[u].size() > 1 || (kids[u].size() == 1 && !fwd[units[kids[u][0]].top]))
+            return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward hand-over)");
+          if (!kids[u].empty()) forced = kids[u][0];
+        } else {
+          // push so that the register child is taken first if nothing more urgent waits
+          for (int i = (int)kids[u].size() - 1; i >= 0; --i) push(kids[u][i]);
+        }
+      }
+    }
+    // positions in the backward lists (a run whose parent sits on another warp is preceded by a
+    // WAIT record; a single record carries its wait itself), signals, waits, encoding
+    std::vector<int> idxb(nu, 0);
+    std::vector<uint8_t> sig_b(nu, 0);
+    for (int w = 0; w < W; ++w) {
+      int pos = 0;
+      for (int u : blist[w]) {
+        const bool remote = punit[u] >= 0 && units[punit[u]].w != w;
+        const bool is_run = fin[w][units[u].fin_idx].type == 3;
+        if (remote) sig_b[punit[u]] = 1;
+        if (remote && is_run) ++pos;
+        idxb[u] = pos++;
+      }
+    }
+    for (int w = 0; w < W; ++w) {
+      HTask &Tk = P.task[w];
+      Tk.b0 = (int)P.prog.size();
+      std::vector<int> seen(W, -1);
+      for (int u : blist[w]) {
+        uint4 e = P.prog[Tk.p0 + units[u].fin_idx];
+        const bool is_run = (e.y & RT_MASK) == RT_RUN;
+        const int pu = punit[u];
+        if (pu >= 0 && units[pu].w != w) {
+          const int wp = units[pu].w;
+          const int posb = (P.task[wp].p1 - P.task[wp].p0) + idxb[pu] + 1;
+          if (posb > 4095) return give_up();
+          if (is_run) {
+            P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)wp | (uint32_t)posb << 16, 0u));
+          } else if (seen[wp] < posb) {
+            e.y |= RF_WAIT_B | (uint32_t)posb << 16 | (uint32_t)wp << 28;
+          }
+          seen[wp] = std::max(seen[wp], posb);
+        }
+        if (bw_row[u]) {
+          const Rec &pr = erec(par[units[u].top]);
+          if (!(pr.flags & RF_HAS_ACC) || pr.tm)
+            return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward row of a private parent)");
+          if (is_run) e.x |= 1u << 25, e.z |= pr.srow << 21;  // z bits 21..30: the parent's row
+          else e.y |= RF_BW_ROW;
+        }
+        if (sig_b[u]) {
+          if (is_run) return fail(CN_ERR_TOPOLOGY, "internal: tape program (a run cannot signal)");
+          e.y |= RF_SIG_B;
+        }
+        if ((int)P.prog.size() - Tk.b0 != idxb[u])
+          return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward positions)");
+        P.prog.push_back(e);
+      }
+      Tk.b1 = (int)P.prog.size();
+    }
   }
 
   // ---- dry run: the W record lists with the kernel's wait / signal rules -------------------------
@@ -994,41 +1107,59 @@ static int build_tape_program(cn_model *m, HClass &K) {
     for (int w = 0; w < W; ++w)
       if (pc[w] != P.task[w].p1) return fail(CN_ERR_TOPOLOGY, "internal: tape program deadlocks");
     // backward
-    std::vector<uint8_t> done_b(n, 0);
-    for (int w = 0; w < W; ++w) pc[w] = P.task[w].p1 - 1;
+    std::vector<uint8_t> done_b(n, 0), stored_v(n, 0);
+    for (int w = 0; w < W; ++w) pc[w] = P.task[w].b0;
     std::fill(ctrv.begin(), ctrv.end(), 0);
+    std::vector<int> lastn(W, -1);  // the node whose v is in the warp's register
     progress = true;
     while (progress) {
       progress = false;
       for (int w = 0; w < W; ++w) {
         const HTask &Tk = P.task[w];
-        while (pc[w] >= Tk.p0) {
+        while (pc[w] < Tk.b1) {
           const uint4 e = P.prog[pc[w]];
           const uint32_t fl = e.y & 0xFFFFu;
-          if ((fl & RT_MASK) == RT_RUN) {
+          if ((fl & RT_MASK) == RT_WAIT) {
+            if (ctrv[e.z & 0xFFFFu] < (int)(e.z >> 16)) break;
+          } else if ((fl & RT_MASK) == RT_RUN) {
             for (int i = (int)((e.x >> 16) & 255u) - 1; i >= 0; --i) {
               const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + (uint32_t)i]
                                              : node_of_srow[(e.z & 1023u) + (uint32_t)i];
-              if (!done_b[par[x]])
+              const bool from_row = i == (int)((e.x >> 16) & 255u) - 1 && (e.x >> 25 & 1u);
+              if (!done_b[par[x]] || (from_row ? !stored_v[par[x]] ||
+                                                     node_of_srow[(e.z >> 21) & 1023u] != par[x]
+                                                : lastn[w] != par[x]))
                 return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward run)");
               done_b[x] = 1;
+              lastn[w] = x;
             }
           } else if ((fl & RT_MASK) == RT_ELIM) {
             if ((fl & RF_WAIT_B) && ctrv[e.y >> 28] < (int)((e.y >> 16) & 0xFFFu)) break;
             const int x = (fl & RF_TMEM) ? node_of_slot[w][e.z & 1023u] : node_of_srow[e.z & 1023u];
-            if (x && !done_b[par[x]])
-              return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward order)");
+            if (x) {
+              const bool from_row = fl & RF_BW_ROW;
+              if (!done_b[par[x]] || (from_row ? !stored_v[par[x]] ||
+                                                     node_of_srow[(e.z >> 10) & 1023u] != par[x]
+                                                : lastn[w] != par[x]))
+                return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward order)");
+            }
             done_b[x] = 1;
-            if (fl & RF_SIG_B) ctrv[w] = (Tk.p1 - Tk.p0) + (Tk.p1 - pc[w]);
+            lastn[w] = x;
+            if (fl & RF_HAS_ACC) stored_v[x] = 1;
+            if (fl & RF_SIG_B) ctrv[w] = (Tk.p1 - Tk.p0) + (pc[w] - Tk.b0) + 1;
+          } else {
+            return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward record type)");
           }
-          --pc[w];
+          ++pc[w];
           progress = true;
         }
       }
     }
     for (int w = 0; w < W; ++w)
-      if (pc[w] >= P.task[w].p0)
+      if (pc[w] != P.task[w].b1)
         return fail(CN_ERR_TOPOLOGY, "internal: tape program deadlocks (backward)");
+    for (int x = 0; x < n; ++x)
+      if (!done_b[x]) return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward incomplete)");
   }
   return CN_OK;
 }
@@ -1181,7 +1312,7 @@ static int build_layout(cn_model *m) {
     const size_t sys_cap = (size_t)std::max(m->tape_sys_cap, K.tp.n_srow);
     const size_t prog_cap = std::max((size_t)m->tape_prog_cap, K.tp.prog.size());
     const size_t need = (size_t)m->tape_W * m->tape_S * m->tape_CH * 256 + sys_cap * 512 +
-                        2 * prog_cap * 16 + 64 + ((size_t)m->tape_W * m->tape_S + 2) * 8 + 16;
+                        prog_cap * 16 + 64 + ((size_t)m->tape_W * m->tape_S + 2) * 8 + 16;
     if (need > 227 * 1024) {
       K.tp.n_groups = 0;
       K.tp.n_cells = 0;
@@ -1677,7 +1808,7 @@ static int finalize(cn_model *m, double dt) {
         const HTask &Tk = P.task[w];
         // program positions are relative to the class's program (as it sits in shared memory)
         ttask[kc * (size_t)m->tape_W + w] =
-            TapeTask{Tk.p0, Tk.p1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.nrows, Tk.head, 0};
+            TapeTask{Tk.p0, Tk.p1, Tk.b0, Tk.b1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.head};
       }
     }
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
@@ -1792,16 +1923,15 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
   return cudaGetLastError();
 }
 
-static size_t tape_smem_bytes(const cn_model *m) {
+static size_t tape_smem_bytes(const cn_model *m, int pbuf) {
   const size_t W = (size_t)m->tape_W;
   return W * m->tape_S * m->tape_CH * 256 + (size_t)m->hm.tape_sys_cap * 512 +
-         2 * (size_t)m->hm.tape_prog_cap * 16 + 64 + (W * m->tape_S + 2) * 8 + 16;
+         (size_t)pbuf * m->hm.tape_prog_cap * 16 + 64 + (W * m->tape_S + 2) * 8 + 16;
 }
 
 // Persistent CTAs: as many as fit the device at once (shared memory decides), each looping over
 // the groups blockIdx.x, blockIdx.x + gridDim.x, ...
 static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
-  const size_t smem = tape_smem_bytes(m);
   auto kern = m->tape_W <= 8 ? tape_step_kernel<256> : tape_step_kernel<512>;
   if (m->tape_ctas == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1821,6 +1951,13 @@ static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
     int smem_sm = 0;
     e = cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
     if (e != cudaSuccess) return e;
+    // the next group's program is prefetched into a second buffer unless that costs the second CTA
+    m->hm.tape_pbuf = 2;
+    if (m->tape_W <= 8 && 2 * (tape_smem_bytes(m, 2) + 1024) > (size_t)smem_sm &&
+        2 * (tape_smem_bytes(m, 1) + 1024) <= (size_t)smem_sm)
+      m->hm.tape_pbuf = 1;
+    if (const char *s = std::getenv("CN_TAPE_PBUF")) m->hm.tape_pbuf = std::atoi(s) == 1 ? 1 : 2;
+    const size_t smem = tape_smem_bytes(m, m->hm.tape_pbuf);
     per_sm = (m->tape_W <= 8 && 2 * (smem + 1024) <= (size_t)smem_sm) ? 2 : 1;
     if (const char *s = std::getenv("CN_TAPE_CTAS_PER_SM")) per_sm = std::max(1, std::min(2, std::atoi(s)));
     if (std::getenv("CN_DEBUG"))
@@ -1828,7 +1965,7 @@ static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
               32 * m->tape_W, per_sm);
     m->tape_ctas = std::min(m->hm.n_tgroup, sms * per_sm);
   }
-  kern<<<m->tape_ctas, 32 * m->tape_W, smem, m->stream>>>(m->hm, k, mode);
+  kern<<<m->tape_ctas, 32 * m->tape_W, tape_smem_bytes(m, m->hm.tape_pbuf), m->stream>>>(m->hm, k, mode);
   return cudaGetLastError();
 }
 
@@ -2062,7 +2199,7 @@ extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
   info[3] = r;
   info[4] = (int64_t)m->tgrp.size();
   info[5] = m->n_tape * 8;
-  info[6] = m->hm.n_tgroup > 0 ? (int64_t)tape_smem_bytes(m) : 0;  // valid after the first cn_run
+  info[6] = m->hm.n_tgroup > 0 ? (int64_t)tape_smem_bytes(m, m->hm.tape_pbuf ? m->hm.tape_pbuf : 2) : 0;  // valid after the first cn_run
   info[7] = (int64_t)m->tape_W | (int64_t)m->tape_ctas << 8 | (int64_t)m->tape_sys_cap << 24;
   return CN_OK;
 }

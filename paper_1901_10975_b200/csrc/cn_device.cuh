@@ -66,24 +66,26 @@ struct TapeClass {
   int32_t n, prog_off, prog_len, n_rows;
 };
 
-// the part of a class's program that one warp runs: records [p0, p1) and its segment of the
-// group's tape, which is cut into chunks of whole records (at most tape_CH rows each); head holds
-// the row counts of the first four chunks (8 bits each), which are requested before the program
-// starts
+// the part of a class's program that one warp runs: forward records [p0, p1), backward records
+// [b0, b1) and its segment of the group's tape, which is cut into chunks of whole records (at
+// most tape_CH rows each); head holds the row counts of the first four chunks (8 bits each),
+// which are requested before the program starts
 struct TapeTask {
-  int32_t p0, p1, nchunk, tm_base;  // tm_base: first tensor-memory slot of the warp
-  uint32_t row0, nrows, head, pad1;
+  int32_t p0, p1, b0, b1;
+  int32_t nchunk, tm_base;  // tm_base: first tensor-memory slot of the warp
+  uint32_t row0, head;
 };
 
 // Program record (uint4) of the interleaved kernel: one per run of plain chain nodes (RUN), per
 // other node elimination (ELIM), per node with distributed mechanisms (MECH), per chunk of the
 // warp's tape segment (CHUNK) and per cross-warp dependency (WAIT).
 //   RUN   x = ring byte offset of the first node's record (16) | nodes in the run (8) | first
-//             node takes a contribution in registers (bit 24)
+//             node takes a contribution in registers (bit 24) | backward: v of the run's parent
+//             comes from the parent's system row, z bits 21..30 (bit 25)
 //         y = RT_RUN     z = system row of the first node (10), or, with bit 20 set, its slot in
 //             the warp's share of tensor memory     w = first tape row of the first node's record
 //   ELIM  x = ring byte offset (16)
-//         y = flags (16) | backward wait: position (12) and warp (4)
+//         y = flags (16) | backward copy: wait position (12) and warp (4)
 //         z = own system row (10) | parent's system row (10)
 //         w = first tape row of the record (16) | tape row of the v copy in the node's mechanism
 //             record (16)
@@ -104,6 +106,7 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
        RF_SIG_B = 128,
        RF_WAIT_B = 256,   // backward: wait for the parent's warp first
        RF_TMEM = 512,     // the node's own row is a tensor-memory slot of the warp (z, low 10 bits)
+       RF_BW_ROW = 1024,  // backward: v of the parent comes from the parent's row, not a register
        RM_HAS_CAI = 1, RM_NEED_ICA = 2,
        RT_ELIM = 0, RT_MECH = 1 << 13, RT_WAIT = 2 << 13, RT_RUN = 3 << 13, RT_CHUNK = 4 << 13,
        RT_MASK = 7 << 13 };
@@ -111,7 +114,7 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
   int32_t n_tgroup, tape_prog_cap, tape_sys_cap, tape_W;
-  int32_t tape_S, tape_CH, pad_t1, pad_t2;  // ring of a warp: S stages of CH rows
+  int32_t tape_S, tape_CH, tape_pbuf, pad_t2;  // ring of a warp: S stages of CH rows; program buffers
   const TapeGroup *tgrp;
   const TapeClass *tcls;
   const TapeTask *ttask;        // [n_class][tape_W]

@@ -245,8 +245,8 @@ __device__ __forceinline__ void mech_record(const DModel &M, const unsigned char
 
 // One CTA = W warps = one group of 32 cells at a time (persistent over groups).  See the header
 // of this file and the record layout in cn_device.cuh.
-// Shared memory: W rings of S stages x CH rows | system: tape_sys_cap x (32 + 32) doubles | two
-// program buffers of tape_prog_cap records | 16 progress counters | W*S + 2 mbarriers | TMEM base.
+// Shared memory: W rings of S stages x CH rows | system: tape_sys_cap x (32 + 32) doubles | one
+// or two program buffers of tape_prog_cap records | 16 progress counters | W*S + 2 mbarriers | TMEM base.
 // Tensor memory as a per-lane scratchpad (Blackwell: 512 columns x 128 lanes x 32 bit per SM; a
 // warp addresses the 32 lanes of its quarter, thread i <-> lane i): (multiplier, reduced rhs) of a
 // plain chain node = 4 columns.  SASS: STTM / LDTM.
@@ -286,7 +286,8 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
   double *sys_l = reinterpret_cast<double *>(sm_raw + (size_t)W * RB) + lane;
   uint4 *progbuf = reinterpret_cast<uint4 *>(sm_raw + (size_t)W * RB +
                                              (size_t)M.tape_sys_cap * 512);
-  uint32_t *ctr = reinterpret_cast<uint32_t *>(progbuf + 2 * (size_t)M.tape_prog_cap);
+  const int PB = M.tape_pbuf;  // program buffers: 2 (the next program loads during the group) or 1
+  uint32_t *ctr = reinterpret_cast<uint32_t *>(progbuf + (size_t)PB * M.tape_prog_cap);
   uint64_t *mbar_all = reinterpret_cast<uint64_t *>(ctr + 16);
   const uint32_t ring_s = smem_u32(sm_raw + (size_t)warp * RB);
   const uint32_t bar_s = smem_u32(mbar_all + (size_t)warp * S);  // S ring barriers of this warp
@@ -366,12 +367,13 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
       tgn = M.tgrp[gn];
       tcn = M.tcls[tgn.cls];
       tkn = M.ttask[(size_t)tgn.cls * W + warp];
-      if (threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
+      if (PB == 2 && threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
     }
     CN_TR(0);
-    mbar_wait(pbar_s + 8 * (it & 1), (it >> 1) & 1);
+    const uint32_t pb = PB == 2 ? (it & 1u) : 0u;
+    mbar_wait(pbar_s + 8 * pb, (PB == 2 ? it >> 1 : it) & 1u);
     CN_TR(1);
-    const uint4 *prog = progbuf + (size_t)(it & 1) * M.tape_prog_cap;
+    const uint4 *prog = progbuf + (size_t)pb * M.tape_prog_cap;
     double *__restrict__ tape_l = M.tape + tg.tape_base + lane;
     const int p0 = tk.p0, p1 = tk.p1;
 
@@ -518,12 +520,13 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     if (!flush) {
       const uint32_t nrec = (uint32_t)(tk.p1 - tk.p0);
       double v_prev = 0.0;
-      for (int j = tk.p1 - 1; j >= tk.p0; --j) {
+      for (int j = tk.b0; j < tk.b1; ++j) {
         const uint4 e = prog[j];
         const uint32_t ty = e.y & RT_MASK;
         if (ty == RT_RUN) {
-          // the parent of the run's last node is the node just solved
+          // the parent of the run's last node: the node just solved, or a row that keeps its v
           const int q = (int)((e.x >> 16) & 255u);
+          if (e.x & (1u << 25)) v_prev = sys_l[((e.z >> 21) & 1023u) * 64u + 32];
           double *trow = tape_l + ((e.w & 0xFFFFu) + 5u * (uint32_t)q + 4u) * 32u;
           if (e.z & (1u << 20)) {
             uint32_t ta = tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u) + (uint32_t)q) * 4u;
@@ -548,16 +551,19 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           }
           continue;
         }
-        if (ty != RT_ELIM) continue;
+        if (ty == RT_WAIT) {
+          ctr_wait(ctr_s + 4 * (e.z & 0xFFFFu), base + (e.z >> 16));
+          CN_TR(3);
+          continue;
+        }
         const uint32_t fl = e.y & 0xFFFFu;
         if (fl & RF_WAIT_B) {
           ctr_wait(ctr_s + 4 * (e.y >> 28), base + ((e.y >> 16) & 0xFFFu));
-          if (j == tk.p1 - 1) { CN_TR(3); }
+          CN_TR(3);
         }
         double *srow = sys_l + (e.z & 1023u) * 64u;
-        const uint32_t kind = fl & RK_KIND;
         double vp = v_prev;
-        if (kind >= RK_STORE) vp = sys_l[((e.z >> 10) & 1023u) * 64u + 32];
+        if (fl & RF_BW_ROW) vp = sys_l[((e.z >> 10) & 1023u) * 64u + 32];
         double mult, rp;
         if (fl & RF_TMEM) {
           tm_load2(tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u)) * 4u, mult, rp);
@@ -572,10 +578,9 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         if (fl & RF_MECHV) tape_l[(e.w >> 16) * 32u] = v;
         if (fl & RF_SIG_B) {
           __syncwarp();
-          if (lane == 0)
-            ctr_publish(ctr_s + 4 * warp, base + nrec + (uint32_t)(tk.p1 - j));
+          if (lane == 0) ctr_publish(ctr_s + 4 * warp, base + nrec + (uint32_t)(j - tk.b0) + 1u);
         }
-        if (kind == RK_ROOT) {  // warp-ballot threshold detection, one atomic per warp
+        if ((fl & RK_KIND) == RK_ROOT) {  // warp-ballot threshold detection, one atomic per warp
           bool fire = false;
           const int pc = tg.cell_base + lane;
           if (lane < tg.ncell) {
@@ -604,6 +609,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     }
     CN_TR(4);
     __syncthreads();  // the system rows and counters of this group are dead from here on
+    if (PB == 1 && has_next && threadIdx.x == 0) load_program(tcn, 0);
     CN_TR(5);
     tg = tgn;
     tc = tcn;
