@@ -4,3 +4,4 @@ Holds none of the method's arithmetic (see configs.py).
 """
 from . import rng  # noqa: F401
 from .configs import *  # noqa: F401,F403
+from .networks import *  # noqa: F401,F403

@@ -174,6 +174,7 @@ struct cn_model {
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
   bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
   bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
+  int tape_need_CH = 0;             // longest record that did not fit a chunk (build_layout retries)
   int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
   bool state_pending = false;       // nrn_state of the last step has not been applied yet
   int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
@@ -795,7 +796,10 @@ static int build_tape_program(cn_model *m, HClass &K) {
       } else {
         ln = 5 + (P.has_pp[x] ? 2 : 0);
       }
-      if (ln > CH) return give_up();  // a record must fit a chunk
+      if (ln > CH) {  // a record must fit a chunk
+        m->tape_need_CH = std::max(m->tape_need_CH, (int)ln);
+        return give_up();
+      }
       r.row = row;
       r.len = ln;
       row += ln;
@@ -1301,6 +1305,17 @@ static int build_layout(cn_model *m) {
       HTape &P = m->cls[m->cell_cls[c]].tp;
       if (P.n_groups > 0) P.has_pp[T.node[i] - m->cell_first[c]] = 1;
     }
+  }
+  // chunk size: the default suits plain nodes (three 5-row records); a model whose mechanism
+  // records are longer gets chunks of that length (a dry pass over the classes finds out)
+  if (!std::getenv("CN_TAPE_CH")) {
+    for (HClass &K : m->cls) {
+      if (K.tp.n_groups == 0) continue;
+      HClass probe = K;
+      int rc = build_tape_program(m, probe);
+      if (rc != CN_OK) return rc;
+    }
+    if (m->tape_need_CH > m->tape_CH && m->tape_need_CH <= 63) m->tape_CH = m->tape_need_CH;
   }
   int prog_total = 0;
   for (HClass &K : m->cls) {

@@ -103,6 +103,50 @@ def test_hh_everywhere_config2_shape(cn, strategy):
     check(o, g, min_spikes=4)
 
 
+def test_hh_everywhere_small_cells_on_tape(cn, strategy):
+    """61-node cells with HH on every node: every node has a mechanism record, every system row
+    sits in shared memory (no tensor-memory rows), two rings of 32 cells = two full groups."""
+    desc = W.config2(n_cell=64, ring_size=32, depth=2, ncomp_branch=10, weight=0.05)
+    o, g = run_both(cn, desc, 30.0)
+    assert g.layout_info()["n_tape_group"] == (2 if strategy == "tape" else 0)
+    check(o, g, min_spikes=20)
+    for s in (0, 1, 2):
+        assert np.max(np.abs(o.get_state(0, s) - g.get_state(0, s))) < 1e-9
+
+
+def test_config3_shape(cn, strategy):
+    """Config 3 scaled to 140 cells (14 morphology types x 10): HH + Ca_HVA + SK + cai + pas,
+    Exp2Syn with random presynaptic cells and delays, Poisson IClamp drive."""
+    desc = W.config3(n_cell=140, syn_per_cell=60)
+    o, g = run_both(cn, desc, 40.0)
+    info = g.layout_info()
+    assert info["n_class"] == 14 and info["n_tape_group"] == (14 if strategy == "tape" else 0)
+    check(o, g, min_spikes=100)
+    for t, s in ((0, 0), (0, 2), (1, 0), (1, 1), (2, 0), (5, 0), (5, 1)):
+        assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9, (t, s)
+
+
+def test_config3_full_size_first_wave(cn):
+    """All 3,560 cells / 465,740 compartments / 1.1 M Exp2Syn for 12 ms (the first population
+    wave); default strategy for this size (warp-cooperative kernel)."""
+    desc = W.config3()
+    assert len(desc["parent"]) == 465740 and len(desc["netcons"]["src"]) == 1100040
+    o, g = run_both(cn, desc, 12.0)
+    check(o, g, min_spikes=1000)
+
+
+def test_config5_shape(cn, strategy):
+    """Config 5 scaled to 110 cells (55 types x 2, full-size cells of 330-580 compartments):
+    ten channel types, AMPA+NMDA synapses with Mg block, delays from 0.1 ms (4 steps).  Every
+    node carries a mechanism (Ih), so these cells always run on the warp-cooperative kernel."""
+    desc = W.config5(n_cell=110, syn_per_cell=40)
+    o, g = run_both(cn, desc, 20.0)
+    assert g.layout_info()["n_class"] == 55
+    check(o, g, min_spikes=10)
+    for t, s in ((0, 0), (0, 1), (3, 1), (4, 0), (6, 1), (7, 0), (10, 0), (10, 3)):
+        assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9, (t, s)
+
+
 def test_config2_one_ring_of_64(cn, strategy):
     desc = W.config2(rings=[1])
     o, g = run_both(cn, desc, 12.0)
