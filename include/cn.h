@@ -138,7 +138,8 @@ int64_t cn_launch_count(const cn_model *m);
 int cn_last_run_ms(const cn_model *m, double *ms_out);
 /* Sample the duration of the step kernel (the dominant kernel) with CUDA event pairs on the
  * model's stream around every `every`-th launch (0 = off), at most max_samples between reads.
- * cn_get_kernel_timing returns the summed duration and the number of samples, and resets. */
+ * cn_get_kernel_timing returns the summed duration and the number of dt the samples cover (one
+ * launch of the interleaved kernel integrates a whole window of steps), and resets. */
 int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samples);
 int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
 /* Layout facts for DESIGN/bench, info8 = { n_class, n_group (all), shared-memory bytes per warp and

@@ -102,6 +102,8 @@ struct HTable {
   // host layout tables
   std::vector<int64_t> pp_first;
   std::vector<int32_t> pp_slot;
+  std::vector<uint32_t> pp_wslot;  // window mode: element in one step's block of win_rows
+  uint32_t *d_pp_wslot = nullptr;
   std::vector<int32_t> cls_cnt, cls_nodeoff;
   std::vector<int64_t> grp_instbase;
   // per-cell CSR of distributed instances sorted by local node
@@ -125,6 +127,8 @@ struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh
   std::vector<uint8_t> has_pp;               // per local node
   std::vector<std::vector<int32_t>> tab_row; // [table][local node]: first row of its block or -1
   std::vector<int32_t> cai_row, ica_row, pp_row, vcopy_row;  // per local node or -1
+  std::vector<int32_t> pp_ord;               // ordinal of a node among the class's has_pp nodes
+  int n_pp = 0;
   int n_rows = 0, prog_off = 0;
   int n_srow = 0;                            // rows of the shared-memory system (the rest: TMEM)
   double sim_makespan = 0.0, sim_work = 0.0; // schedule quality (cn_debug_tasks)
@@ -170,12 +174,17 @@ struct cn_model {
   std::vector<TapeGroup> tgrp;
   std::vector<uint8_t> cell_tape;   // per caller cell
   int64_t n_tape = 0;               // doubles
+  int64_t win_stride = 0, win_ninst = 0;  // window mode: doubles per step in win_rows / win_deliv
   int tape_prog_cap = 0, tape_sys_cap = 0;
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
   bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
   bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
   int tape_need_CH = 0;             // longest record that did not fit a chunk (build_layout retries)
   int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
+  bool window = false;              // window mode: one launch of the interleaved kernel per
+  int win_steps = 0;                //   up to win_steps steps (cn_tape.cuh)
+  int64_t win_idx = 0;
+  std::vector<int> ktime_steps;     // steps covered by each kernel-timing sample
   bool state_pending = false;       // nrn_state of the last step has not been applied yet
   int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
   std::vector<double> cai0;         // initial cai per caller node (when any table needs it)
@@ -725,6 +734,11 @@ static int build_tape_program(cn_model *m, HClass &K) {
   }
   // ---- 4. tape rows: each warp's records get consecutive rows, padded so that no record wraps
   // around the warp's ring; system rows in the same order ----------------------------------------
+  P.pp_ord.assign(n, -1);
+  P.n_pp = 0;
+  for (int x = 0; x < n; ++x)
+    if (P.has_pp[x]) P.pp_ord[x] = P.n_pp++;
+  if (P.n_pp > 1023) return give_up();
   P.order.clear();
   P.pos_of.assign(n, 0);
   P.row.assign(n, 0);
@@ -902,7 +916,8 @@ static int build_tape_program(cn_model *m, HClass &K) {
         // the parent's row is written (contribution) or read (v) only if it collects contributions
         // (RF_HAS_ACC); such a row is always in shared memory
         const uint32_t ez =
-            r.srow | (uint32_t)(x && (erec(par[x]).flags & RF_HAS_ACC) ? erec(par[x]).srow : 0) << 10;
+            r.srow | (uint32_t)(x && (erec(par[x]).flags & RF_HAS_ACC) ? erec(par[x]).srow : 0) << 10 |
+            (uint32_t)(P.has_pp[x] ? P.pp_ord[x] : 0) << 21;
         const uint32_t ew = r.row | (uint32_t)(node_mask[x] ? P.vcopy_row[x] : 0) << 16;
         P.prog.push_back(make_uint4(r.ring, ey, ez, ew));
       }
@@ -1436,6 +1451,8 @@ static int build_layout(cn_model *m) {
       tg.tape_base = tape_base;
       tg.cell_base = cell_base;
       tg.ncell = (int32_t)std::min<int64_t>(32, K.tp.n_cells - (int64_t)gq * 32);
+      tg.pp_base = m->win_stride;
+      m->win_stride += (int64_t)K.tp.n_pp * 64;
       const int gidx = ngc + (int)m->tgrp.size();
       for (int c = 0; c < tg.ncell; ++c) {
         const int32_t cell = K.cells[(int64_t)gq * 32 + c];
@@ -1469,6 +1486,7 @@ static int build_layout(cn_model *m) {
       for (int g = 0; g < ng; ++g) T.pp_first[g + 1] += T.pp_first[g];
       std::vector<int64_t> fill(T.pp_first.begin(), T.pp_first.end() - 1);
       T.pp_slot.assign((size_t)T.n, 0);
+      T.pp_wslot.assign((size_t)T.n, 0);
       for (int64_t i = 0; i < T.n; ++i) {
         const int32_t cell = cell_of[T.node[i]];
         const int g = m->cell_grp[cell];
@@ -1483,6 +1501,8 @@ static int build_layout(cn_model *m) {
           const int64_t el = tg.tape_base + (int64_t)m->cls[tg.cls].tp.pp_row[local] * 32 +
                              m->cell_slot[cell];
           T.pp_slot[pos] = (int32_t)(uint32_t)el;
+          T.pp_wslot[pos] = (uint32_t)(tg.pp_base + (int64_t)m->cls[tg.cls].tp.pp_ord[local] * 64 +
+                                       m->cell_slot[cell]);
         }
       }
       T.pp_tape_begin = T.pp_first[ngc];
@@ -1796,8 +1816,10 @@ static int finalize(cn_model *m, double dt) {
     for (int j = 0; j < T.ti.n_dev_param; ++j) { UP(par[j], T.d_param[j]); D.param[j] = T.d_param[j]; }
     for (int j = 0; j < T.ti.n_state; ++j) { UP(st[j], T.d_state[j]); D.state[j] = T.d_state[j]; }
     if (T.ti.point) {
-      UP(T.pp_first, T.d_pp_first); UP(T.pp_slot, T.d_pp_slot);
-      D.pp_first = T.d_pp_first; D.pp_slot = T.d_pp_slot;
+      UP(T.pp_first, T.d_pp_first); UP(T.pp_slot, T.d_pp_slot); UP(T.pp_wslot, T.d_pp_wslot);
+      D.pp_first = T.d_pp_first; D.pp_slot = T.d_pp_slot; D.pp_wslot = T.d_pp_wslot;
+      D.pp_goff = m->win_ninst;
+      m->win_ninst += T.n;
     } else {
       UP(T.cls_cnt, T.d_cls_cnt); UP(T.cls_nodeoff, T.d_cls_nodeoff);
       UP(T.grp_instbase, T.d_grp_instbase);
@@ -1894,6 +1916,31 @@ static int finalize(cn_model *m, double dt) {
     UP(ss, p64); H.stim_step = p64;
     H.n_stim = ns;
   }
+  // window mode: every cell on the interleaved kernel, no point process whose current depends on
+  // v (AMPA+NMDA), no per-step probes; a window is at most the smallest delay long
+  {
+    bool ok = m->hm.n_tgroup > 0 && m->grp.empty() && m->probe.empty();
+    for (const HTable &T : m->tab)
+      if (T.type == CN_AMPANMDA && T.n > 0) ok = false;
+    if (const char *e = std::getenv("CN_TAPE_WINDOW")) ok = ok && std::atoi(e) != 0;
+    int64_t wn = m->n_netcon > 0 ? std::min<int64_t>(H.mind, 64) : 32;
+    if (wn < 2 || (H.maxd + wn - 1) / wn + 2 > 60) ok = false;
+    if (ok && (m->win_stride + m->win_ninst) * wn * 8 > ((int64_t)4 << 30)) ok = false;
+    m->window = ok;
+    m->win_steps = (int)wn;
+    H.win_stride = m->win_stride;
+    H.win_ninst = m->win_ninst;
+    if (ok) {
+      rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_stride * wn, 1), &H.win_rows);
+      if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_ninst * wn, 1), &H.win_deliv);
+      if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)m->hm.n_tgroup, &H.win_done); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, 1, &H.win_ticket); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, 64, &H.win_mark_step); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, 64, &H.win_mark_nsp); if (rc != CN_OK) return rc;
+    }
+  }
   // spikes
   rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_gid, false); if (rc) return rc;
   rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_step, false); if (rc) return rc;
@@ -1946,7 +1993,7 @@ static size_t tape_smem_bytes(const cn_model *m, int pbuf) {
 
 // Persistent CTAs: as many as fit the device at once (shared memory decides), each looping over
 // the groups blockIdx.x, blockIdx.x + gridDim.x, ...
-static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
+static cudaError_t launch_tape(cn_model *m, int64_t k, int mode, int nsteps = 1) {
   auto kern = m->tape_W <= 8 ? tape_step_kernel<256> : tape_step_kernel<512>;
   if (m->tape_ctas == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1980,7 +2027,8 @@ static cudaError_t launch_tape(cn_model *m, int64_t k, int mode) {
               32 * m->tape_W, per_sm);
     m->tape_ctas = std::min(m->hm.n_tgroup, sms * per_sm);
   }
-  kern<<<m->tape_ctas, 32 * m->tape_W, tape_smem_bytes(m, m->hm.tape_pbuf), m->stream>>>(m->hm, k, mode);
+  kern<<<m->tape_ctas, 32 * m->tape_W, tape_smem_bytes(m, m->hm.tape_pbuf), m->stream>>>(
+      m->hm, k, mode, nsteps);
   return cudaGetLastError();
 }
 
@@ -1993,6 +2041,47 @@ static int run_steps(cn_model *m, int64_t K) {
     if (T.ti.point) pp_tape = std::max(pp_tape, T.n - T.pp_tape_begin);
   const int pp_blocks = (int)std::min<int64_t>((pp_tape + 255) / 256, 148 * 8);
   CU(cudaEventRecord(m->ev0, m->stream));
+  if (m->window) {
+    // one launch of the interleaved kernel per window of up to win_steps steps; the events and
+    // point processes of the whole window are prepared by two small kernels in front of it
+    int64_t pp_all = 0;
+    for (const HTable &T : m->tab)
+      if (T.ti.point) pp_all = std::max(pp_all, T.n);
+    const int ppb = (int)std::max<int64_t>(1, std::min<int64_t>((pp_all + 255) / 256, 148 * 8));
+    for (int64_t s = 0; s < K;) {
+      const int n = (int)std::min<int64_t>(m->win_steps, K - s);
+      const int64_t k = m->k + s;
+      if (m->win_stride > 0)
+        CU(cudaMemsetAsync(m->hm.win_rows, 0, (size_t)m->win_stride * n * sizeof(double), m->stream));
+      CU(cudaMemsetAsync(m->hm.win_done, 0, (size_t)ntg * sizeof(int32_t), m->stream));
+      CU(cudaMemsetAsync(m->hm.win_ticket, 0, sizeof(uint32_t), m->stream));
+      if (m->n_netcon > 0) {
+        deliver_window_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->hm, k, n, m->win_idx);
+        m->launches++;
+      }
+      if (pp_all > 0) {
+        pp_window_kernel<<<ppb, 256, 0, m->stream>>>(m->hm, k, n);
+        m->launches++;
+      }
+      const bool timeit = m->ktime_every > 0 && m->ktime_used < m->ktime_ev.size();
+      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
+      cudaError_t e = launch_tape(m, k, (m->state_pending ? TM_ADVANCE : 0) | TM_WINDOW, n);
+      if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
+      if (timeit) {
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+        m->ktime_steps.push_back(n);
+      }
+      m->state_pending = true;
+      m->launches++;
+      m->win_idx++;
+      s += n;
+    }
+    CU(cudaEventRecord(m->ev1, m->stream));
+    CU(cudaGetLastError());
+    m->k += K;
+    m->timed = true;
+    return CN_OK;
+  }
   for (int64_t s = 0; s < K; ++s) {
     const int64_t k = m->k + s;
     if (m->n_netcon > 0) {
@@ -2016,7 +2105,10 @@ static int run_steps(cn_model *m, int64_t K) {
         default: e = launch_step<1>(m, k); break;
       }
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "step launch failed: %s", cudaGetErrorString(e));
-      if (timeit && !time_tape) cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+      if (timeit && !time_tape) {
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+        m->ktime_steps.push_back(1);
+      }
       m->launches++;
     }
     if (ntg > 0) {
@@ -2024,7 +2116,10 @@ static int run_steps(cn_model *m, int64_t K) {
       cudaError_t e = launch_tape(m, k, m->state_pending ? TM_ADVANCE : 0);
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
       m->state_pending = true;
-      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+      if (timeit) {
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+        m->ktime_steps.push_back(1);
+      }
       m->launches++;
     }
     if (!m->probe.empty() && m->probe_rows < m->probe_cap) {
@@ -2231,6 +2326,7 @@ extern "C" int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samp
   for (auto &pr : m->ktime_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   m->ktime_ev.clear();
   m->ktime_used = 0;
+  m->ktime_steps.clear();
   m->ktime_every = every;
   if (every > 0)
     for (int i = 0; i < max_samples; ++i) {
@@ -2252,8 +2348,11 @@ extern "C" int cn_get_kernel_timing(cn_model *m, double *sum_ms, int64_t *count)
     tot += f;
   }
   *sum_ms = tot;
-  *count = (int64_t)m->ktime_used;
+  int64_t steps = 0;  // a sample of the window mode covers several dt
+  for (size_t i = 0; i < m->ktime_used && i < m->ktime_steps.size(); ++i) steps += m->ktime_steps[i];
+  *count = steps;
   m->ktime_used = 0;
+  m->ktime_steps.clear();
   return CN_OK;
 }
 

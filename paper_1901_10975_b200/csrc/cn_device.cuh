@@ -35,6 +35,9 @@ struct DTable {
   double *param[CN_MAX_PARAM];   // permuted SoA, incl. derived per-instance constants (see host)
   double *state[CN_MAX_STATE];
   double glob[CN_MAX_GLOBAL];
+  const uint32_t *pp_wslot;      // point tables, window mode: element of the node's conductance row
+                                 // in one step's block of win_rows
+  int64_t pp_goff;               // point tables, window mode: first column of the table in win_deliv
   const int64_t *pp_first;       // point tables: [n_group+1] instance range of each group
   const int32_t *pp_slot;        // point tables: [n] shared-memory slot (node*G + cell) in its group
   const int32_t *cls_cnt;        // distributed: [n_class] instances per cell
@@ -59,7 +62,7 @@ struct ClassInfo {
 struct TapeGroup {
   int64_t tape_base;     // first element of the group's tape (multiple of 32 doubles)
   int32_t cls, cell_base, ncell, pad0;
-  int64_t pad1;
+  int64_t pp_base;       // window mode: first element of the group's rows in a step's block of win_rows
 };
 
 struct TapeClass {
@@ -149,6 +152,14 @@ struct DModel {
   int64_t n_stim;
   const int32_t *stim_gid;      // sorted by step
   const int64_t *stim_step;
+  // window mode (interleaved kernel only): one launch integrates up to `mind` steps
+  double *win_rows;             // [steps][win_stride]: point-process conductance / current rows
+  double *win_deliv;            // [steps][win_ninst]: summed weights delivered to every instance
+  int64_t win_stride, win_ninst;
+  int32_t *win_done;            // [n_tgroup]: steps of the window completed for the group
+  uint32_t *win_ticket;         // next (step, group) work item
+  int64_t *win_mark_step;       // ring [64]: first step of the recent windows
+  int64_t *win_mark_nsp;        //            and the length of the spike list at their start
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
 };
@@ -688,6 +699,129 @@ __global__ void __launch_bounds__(128) deliver_kernel(const __grid_constant__ DM
     }
     for (int64_t i = a + warp; i < M.n_stim && M.stim_step[i] <= s_hi; i += nwarp)
       deliver_source(M, M.stim_gid[i], (int32_t)(k - M.stim_step[i]), lane);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// window mode: everything the events and point processes contribute to the next `nsteps` steps
+// (nsteps <= smallest delay, so every event delivered in the window stems from a spike recorded
+// before it).  deliver_window_kernel sums the weights per (step, instance); pp_window_kernel then
+// advances every point process through the window and leaves its conductance / current of every
+// step in win_rows, where the interleaved kernel picks them up.  Same arithmetic per step as
+// deliver_kernel + pp_tape_kernel (types whose current depends on v cannot run in this mode).
+// ------------------------------------------------------------------------------------------
+
+__global__ void __launch_bounds__(128) deliver_window_kernel(const __grid_constant__ DModel M,
+                                                             int64_t k0, int nsteps, int64_t widx) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  unsigned long long ns = *M.n_sp;
+  if ((int64_t)ns > M.sp_cap) ns = (unsigned long long)M.sp_cap;
+  // spikes that can matter carry steps >= k0 - maxd: they were recorded in the windows that end
+  // at or after that step (the spike list is ordered by window, not by step)
+  int64_t i_lo = (int64_t)ns;
+  int64_t end_step = k0;  // first step after window j
+  for (int64_t j = widx - 1; j >= 0 && j > widx - 63; --j) {
+    if (end_step < k0 - M.maxd) break;
+    i_lo = M.win_mark_nsp[j & 63];
+    end_step = M.win_mark_step[j & 63];
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    M.win_mark_step[widx & 63] = k0;
+    M.win_mark_nsp[widx & 63] = (int64_t)ns;
+  }
+  auto deliver = [&](int32_t gid, int64_t step) {
+    const int64_t lo = M.src_first[gid], hi = M.src_first[gid + 1];
+    // delays d with k0 <= step + d < k0 + nsteps, in the delay-sorted list of this source
+    const int64_t d_lo = k0 - step, d_hi = k0 + nsteps - 1 - step;
+    int64_t a = lo, b = hi;
+    while (a < b) {
+      const int64_t mid = (a + b) >> 1;
+      if (M.nc_d[mid] < d_lo) a = mid + 1; else b = mid;
+    }
+    for (int64_t nc = a + lane; nc < hi; nc += 32) {
+      const int64_t d = M.nc_d[nc];
+      if (d > d_hi) break;
+      const DTable &T = M.tab[M.nc_tab[nc]];
+      atomicAdd(&M.win_deliv[(step + d - k0) * M.win_ninst + T.pp_goff + M.nc_inst[nc]],
+                M.nc_w[nc]);
+    }
+  };
+  for (int64_t i = i_lo + warp; i < (int64_t)ns; i += nwarp) deliver(M.sp_gid[i], M.sp_step[i]);
+  for (int64_t i = warp; i < M.n_stim; i += nwarp) {
+    const int64_t st = M.stim_step[i];
+    if (st + M.maxd >= k0 && st + M.mind < k0 + nsteps) deliver(M.stim_gid[i], st);
+  }
+}
+
+__global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ DModel M,
+                                                        int64_t k0, int nsteps) {
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t nth = (int64_t)gridDim.x * blockDim.x;
+  const double dt = M.dt;
+  for (int t = 0; t < M.n_table; ++t) {
+    const DTable &T = M.tab[t];
+    if (!T.is_point) continue;
+    const uint32_t *__restrict__ ws = T.pp_wslot;
+    for (int64_t q = tid; q < T.pp_tape_end; q += nth) {
+      double *rows = M.win_rows + ws[q];
+      double *dl = M.win_deliv + T.pp_goff + q;
+      switch (T.type) {
+        case T_EXPSYN: {
+          double g = T.state[0][q];
+          for (int s = 0; s < nsteps; ++s, rows += M.win_stride, dl += M.win_ninst) {
+            const double w = *dl;
+            if (w != 0.0) {
+              g += w;
+              *dl = 0.0;
+            }
+            if (g != 0.0) {
+              const double gs = g * T.param[2][q];
+              atomicAdd(rows, gs);
+              atomicAdd(rows + 32, gs * T.param[1][q]);
+              g = cnexp(g, 0.0, T.param[0][q], dt);
+            }
+          }
+          T.state[0][q] = g;
+          break;
+        }
+        case T_EXP2SYN: {
+          double A = T.state[0][q], B = T.state[1][q];
+          for (int s = 0; s < nsteps; ++s, rows += M.win_stride, dl += M.win_ninst) {
+            const double w = *dl;
+            if (w != 0.0) {
+              const double wf = w * T.param[4][q];
+              A += wf;
+              B += wf;
+              *dl = 0.0;
+            }
+            if (A != 0.0 || B != 0.0) {
+              const double gs = (B - A) * T.param[3][q];
+              if (gs != 0.0) {
+                atomicAdd(rows, gs);
+                atomicAdd(rows + 32, gs * T.param[2][q]);
+              }
+              A = cnexp(A, 0.0, T.param[0][q], dt);
+              B = cnexp(B, 0.0, T.param[1][q], dt);
+            }
+          }
+          T.state[0][q] = A;
+          T.state[1][q] = B;
+          break;
+        }
+        case T_ICLAMP: {
+          const double del = T.param[0][q], dur = T.param[1][q];
+          for (int s = 0; s < nsteps; ++s, rows += M.win_stride) {
+            const double t_mid = ((double)(k0 + s) + 0.5) * dt;
+            if (t_mid >= del && t_mid < del + dur)
+              atomicAdd(rows + 32, T.param[2][q] * T.param[3][q]);
+          }
+          break;
+        }
+        default: break;
+      }
+    }
   }
 }
 

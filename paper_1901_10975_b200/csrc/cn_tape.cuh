@@ -141,7 +141,10 @@ __device__ __forceinline__ void hh_advance(double v, double q10dt, double &m, do
   n += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - n);
 }
 
-enum { TM_ADVANCE = 1, TM_FLUSH = 2 };
+// kernel modes: TM_ADVANCE: the states on the tape still wait for nrn_state of the previous step;
+// TM_FLUSH: apply that update and nothing else; TM_WINDOW: one launch integrates `nsteps` steps,
+// work items (step, group) are handed out by a ticket counter (see the kernel)
+enum { TM_ADVANCE = 1, TM_FLUSH = 2, TM_WINDOW = 4 };
 
 // One mechanism record: nrn_state of the previous step (if `mode & TM_ADVANCE`: the states on the
 // tape are still those the previous nrn_cur used) followed by nrn_cur of this step with the
@@ -276,7 +279,7 @@ __device__ long long g_trace[148 * 16 * 8 * 8];
 #endif
 template <int MAXT>
 __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __grid_constant__ DModel M,
-                                                          int64_t k, int mode) {
+                                                          int64_t k, int mode, int nsteps) {
   extern __shared__ __align__(128) unsigned char sm_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int W = M.tape_W, S = M.tape_S, CH = M.tape_CH;
@@ -349,26 +352,71 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
              pbar_s + 8 * buf);
   };
 
-  int g = blockIdx.x;
-  TapeGroup tg = M.tgrp[g];
+  // Work items.  Per-step mode: item = group, CTA b takes b, b + gridDim.x, ...  Window mode: item
+  // i = step * ngrp + group, handed out by a global ticket counter (any CTA, any order of
+  // arrival); item (s, g) may start once (s - 1, g) is complete (win_done[g] >= s), which its
+  // owner -- usually another SM -- publishes with release semantics after all its global writes.
+  const bool window = mode & TM_WINDOW;
+  const uint32_t n_items = (uint32_t)ngrp * (uint32_t)(window ? nsteps : 1);
+  uint32_t *item_s = tm_base_s + 1;  // two shared slots for the tickets drawn by thread 0
+  auto item_ready = [&](uint32_t item) -> bool {  // one lane
+    const uint32_t s = item / (uint32_t)ngrp;
+    if (!window || s == 0) return true;
+    int32_t d;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];"
+                 : "=r"(d)
+                 : "l"(M.win_done + item % (uint32_t)ngrp)
+                 : "memory");
+    return d >= (int32_t)s;
+  };
+  auto wait_item = [&](uint32_t item, bool block) -> bool {  // whole warp; true when ready
+    bool ok;
+    do {
+      ok = lane == 0 ? item_ready(item) : true;
+      ok = __shfl_sync(0xffffffffu, ok, 0);
+    } while (!ok && block);
+    if (ok && window) asm volatile("fence.proxy.async;" ::: "memory");  // bulk copies read what
+    return ok;                                                        // another SM just wrote
+  };
+  uint32_t cur, nxt;
+  if (window) {
+    if (threadIdx.x == 0) {
+      item_s[0] = atomicAdd(M.win_ticket, 1u);
+      item_s[1] = atomicAdd(M.win_ticket, 1u);
+    }
+    __syncthreads();
+    cur = item_s[0];
+    nxt = item_s[1];
+  } else {
+    cur = blockIdx.x;
+    nxt = cur + gridDim.x;
+  }
+  if (cur < n_items) {
+  TapeGroup tg = M.tgrp[cur % (uint32_t)ngrp];
   TapeClass tc = M.tcls[tg.cls];
   TapeTask tk = M.ttask[(size_t)tg.cls * W + warp];
   if (threadIdx.x == 0) load_program(tc, 0);
+  wait_item(cur, true);
   start_segment(tg, tk);
 
-  for (uint32_t it = 0; g < ngrp; g += gridDim.x, ++it) {
+  for (uint32_t it = 0; cur < n_items; ++it) {
     const uint32_t base = (it + 1) << 13;  // progress counters never run backwards
-    const int gn = g + gridDim.x;
-    const bool has_next = gn < ngrp;
+    const int g = (int)(cur % (uint32_t)ngrp);
+    const int step_in = (int)(cur / (uint32_t)ngrp);  // step of the window
+    const int64_t kk = k + step_in;
+    const int smode = (mode & ~TM_ADVANCE) | ((mode & TM_ADVANCE) || step_in > 0 ? TM_ADVANCE : 0);
+    const bool has_next = nxt < n_items;
+    bool next_started = false;
     TapeGroup tgn = tg;
     TapeClass tcn = tc;
     TapeTask tkn = tk;
     if (has_next) {
-      tgn = M.tgrp[gn];
+      tgn = M.tgrp[nxt % (uint32_t)ngrp];
       tcn = M.tcls[tgn.cls];
       tkn = M.ttask[(size_t)tgn.cls * W + warp];
       if (PB == 2 && threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
     }
+    if (window && threadIdx.x == 0) item_s[it & 1] = atomicAdd(M.win_ticket, 1u);  // the one after
     CN_TR(0);
     const uint32_t pb = PB == 2 ? (it & 1u) : 0u;
     mbar_wait(pbar_s + 8 * pb, (PB == 2 ? it >> 1 : it) & 1u);
@@ -458,14 +506,21 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           D += srow[0];
           R += srow[32];
         }
-        if (fl & RF_HAS_PP) {  // conductance / current of the point processes (pp_tape_kernel)
-          const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
-          D += pd;
-          R += pr;
-          if (pd != 0.0 || pr != 0.0) {
-            double *trec = tape_l + (e.w & 0xFFFFu) * 32u;
-            trec[5 * 32] = 0.0;
-            trec[6 * 32] = 0.0;
+        if (fl & RF_HAS_PP) {  // conductance / current of the point processes
+          if (window) {  // (pp_window_kernel: this step's block of win_rows; z bits 21..30 = the
+            const double *wr = M.win_rows + (size_t)step_in * M.win_stride + tg.pp_base +
+                               ((e.z >> 21) & 1023u) * 64u + lane;  // node's ordinal in the class)
+            D += wr[0];
+            R += wr[32];
+          } else {  // (pp_tape_kernel: the two dynamic rows of the record, cleared after use)
+            const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
+            D += pd;
+            R += pr;
+            if (pd != 0.0 || pr != 0.0) {
+              double *trec = tape_l + (e.w & 0xFFFFu) * 32u;
+              trec[5 * 32] = 0.0;
+              trec[6 * 32] = 0.0;
+            }
           }
         }
         const double rinv = rcp_fast(D);
@@ -497,7 +552,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         }
       } else {  // RT_MECH
         double gD, gR;
-        mech_record(M, rb, tape_l + (e.y >> 16) * 32u, fl, e.w, mode, dt, q10dt, gD, gR);
+        mech_record(M, rb, tape_l + (e.y >> 16) * 32u, fl, e.w, smode, dt, q10dt, gD, gR);
         if (!flush) {
           srow[0] = gD;
           srow[32] = gR;
@@ -512,7 +567,10 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     CN_TR(2);
     // this warp's ring is idle until the next group: start loading it now
     __syncwarp();
-    if (has_next) start_segment(tgn, tkn);
+    if (has_next && wait_item(nxt, false)) {
+      start_segment(tgn, tkn);
+      next_started = true;
+    }
 
     // ========================================================================================
     // backward: back-substitution (L66), v to the tape, threshold at the root (L68)
@@ -585,8 +643,8 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           const int pc = tg.cell_base + lane;
           if (lane < tg.ncell) {
             const bool above = v > M.thr[pc];
-            fire = above && !M.flag[pc];
-            M.flag[pc] = (unsigned char)above;
+            fire = above && !__ldcg(M.flag + pc);  // (another SM may have written it last step)
+            __stcg(M.flag + pc, (unsigned char)above);
           }
           const unsigned ball = __ballot_sync(0xffffffffu, fire);
           if (ball) {
@@ -598,7 +656,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
               const unsigned long long pos = sbase + __popc(ball & ((1u << lane) - 1u));
               if ((int64_t)pos < M.sp_cap) {
                 M.sp_gid[pos] = M.gid_of_pcell[pc];
-                M.sp_step[pos] = k + 1;
+                M.sp_step[pos] = kk + 1;
               } else {
                 *M.overflow = 1;
               }
@@ -609,11 +667,26 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     }
     CN_TR(4);
     __syncthreads();  // the system rows and counters of this group are dead from here on
+    if (window) {
+      if (threadIdx.x == 0) {  // every global write of the CTA for (step, group) is visible first
+        __threadfence();
+        asm volatile("fence.proxy.async;" ::: "memory");
+        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(M.win_done + g), "r"(step_in + 1)
+                     : "memory");
+      }
+    }
     if (PB == 1 && has_next && threadIdx.x == 0) load_program(tcn, 0);
+    if (has_next && !next_started) {  // the next item was not ready when the forward sweep ended
+      wait_item(nxt, true);
+      start_segment(tgn, tkn);
+    }
     CN_TR(5);
+    cur = nxt;
+    nxt = window ? item_s[it & 1] : nxt + gridDim.x;
     tg = tgn;
     tc = tcn;
     tk = tkn;
+  }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();

@@ -295,3 +295,36 @@ def test_config4_full_size_sampled_rings(cn):
     # whole-model invariants at full size: every ring carries the same wave, one spike per cell so far
     per_ring = np.bincount(gg[gg < 32768] // 64, minlength=512)
     assert per_ring.min() > 0 and per_ring.max() <= 64 * 2
+
+
+@pytest.mark.parametrize("which", ["config1", "config4", "config3", "unique"])
+def test_window_mode_matches_oracle(cn, which, monkeypatch):
+    """Without per-step probes a model whose cells all sit on the interleaved kernel runs in
+    WINDOW mode: one launch integrates up to min-delay steps, (step, group) work items are handed
+    out by a ticket counter, events and point processes of the window are prepared up front.
+    Final voltages, states and the whole spike list must still match the oracle."""
+    from oracle import OracleModel
+    monkeypatch.setenv("CN_TAPE", "1")
+    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+    desc, tstop = {
+        "config1": (W.config1(), 60.0),
+        "config4": (W.config4(n_cell=256, n_types=8), 50.0),
+        "config3": (W.config3(n_cell=140, syn_per_cell=60), 40.0),
+        "unique": (W.random_tree_cells(13, 5, 120, stream="gpu-u", weight=0.2, amp=2.0), 40.0),
+    }[which]
+    o = OracleModel(desc)
+    o.run(tstop, DT)
+    g = cn.Model(desc)
+    for t in (0.3 * tstop, 0.3 * tstop + DT, tstop):      # windows of different lengths
+        g.run(t, DT)
+    nsteps = int(round(tstop / DT))
+    assert g.steps_done == nsteps and g.launch_count < nsteps      # not one launch per step
+    err = np.max(np.abs(o.get_v() - g.get_v()))
+    assert err <= TOL, err
+    og, os_ = o.get_spikes()
+    gg, gs = g.get_spikes()
+    assert len(og) >= 5 and list(og) == list(gg) and list(os_) == list(gs)
+    assert o.min_margin > 1e3 * max(err, 1e-12)
+    for t, m in enumerate(desc["mechs"]):
+        if m["type"] in ("hh", "expsyn", "exp2syn", "sk"):
+            assert np.max(np.abs(o.get_state(t, 0) - g.get_state(t, 0))) < 1e-9, m["type"]
