@@ -261,7 +261,7 @@ def main():
     n_tape_launches = max(1, launches // 3) if launches < total_dt_for_launches(args) else None
     achieved = alg_bytes / (kern_ms * 1e-3) / 1e9 if k_n else None
     traffic = None
-    tf = ROOT / "profiles" / "tape_step_kernel_traffic.json"
+    tf = ROOT / "profiles" / "tape_step_kernel_traffic.txt"
     if tf.exists():
         try:
             traffic = json.loads(tf.read_text()).get("dram_bytes_per_dt")

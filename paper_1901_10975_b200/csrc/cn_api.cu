@@ -131,6 +131,7 @@ struct HTape {  // per class: the program of the interleaved kernel (cn_tape.cuh
   int n_pp = 0;
   int n_rows = 0, prog_off = 0;
   int n_srow = 0;                            // rows of the shared-memory system (the rest: TMEM)
+  int n_bar = 0;                             // signal mbarriers (one per signalling record)
   double sim_makespan = 0.0, sim_work = 0.0; // schedule quality (cn_debug_tasks)
 };
 
@@ -175,7 +176,7 @@ struct cn_model {
   std::vector<uint8_t> cell_tape;   // per caller cell
   int64_t n_tape = 0;               // doubles
   int64_t win_stride = 0, win_ninst = 0;  // window mode: doubles per step in win_rows / win_deliv
-  int tape_prog_cap = 0, tape_sys_cap = 0;
+  int tape_prog_cap = 0, tape_sys_cap = 0, tape_bar_cap = 0;
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
   bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
   bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
@@ -655,6 +656,28 @@ static int build_tape_program(cn_model *m, HClass &K) {
   }
   P.sim_work = sw[0];
   for (int x = 0; x < n; ++x) P.sim_work += mcost[x];
+  // Which list runs on which warp is free.  Warps w and w + 4 share a quarter of the tensor
+  // memory (64 row slots): pair the longest list with the shortest, and so on, so that as few
+  // private rows as possible overflow into shared memory.
+  if (W > 4 && W <= 8) {
+    std::vector<int> rank(W);
+    std::iota(rank.begin(), rank.end(), 0);
+    std::stable_sort(rank.begin(), rank.end(),
+                     [&](int a, int b) { return elist[a].size() > elist[b].size(); });
+    std::vector<int> slot(W);
+    for (int r = 0; r < W; ++r) slot[rank[r]] = r < 4 ? r : 4 + (W - 1 - r);
+    std::vector<std::vector<int32_t>> e2(W), m2(W);
+    for (int w = 0; w < W; ++w) {
+      e2[slot[w]].swap(elist[w]);
+      m2[slot[w]].swap(mlist[w]);
+    }
+    elist.swap(e2);
+    mlist.swap(m2);
+    for (int x = 0; x < n; ++x) {
+      e_warp[x] = slot[e_warp[x]];
+      if (m_warp[x] >= 0) m_warp[x] = slot[m_warp[x]];
+    }
+  }
 
   // ---- 3. records, hand-over kinds, dependencies ----------------------------------------------
   struct Rec {
@@ -668,6 +691,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
     uint32_t srow = 0;                      // row of the shared-memory system, or TMEM slot
     bool tm = false;
     int unit = -1;                          // backward unit (RUN or single ELIM record) of the node
+    int sig = 0;                            // mbarrier the record arrives on (RF_SIG_F)
   };
   std::vector<std::vector<Rec>> recs(W);
   std::vector<int> e_pre(n, -1), m_pre(n, -1);  // pre-index of a node's records in its warp's list
@@ -883,14 +907,18 @@ static int build_tape_program(cn_model *m, HClass &K) {
     Tk.head = 0;
     for (uint32_t c = 0; c < 4 && c < chunks[w].size(); ++c) Tk.head |= chunks[w][c].second << (8 * c);
   }
+  // every signalling record arrives on an mbarrier of its own (once per group)
+  P.n_bar = 0;
+  for (int w = 0; w < W; ++w)
+    for (Rec &r : recs[w])
+      if (r.flags & RF_SIG_F) r.sig = P.n_bar++;
   // encoding (layout of the records: cn_device.cuh)
   for (int w = 0; w < W; ++w) {
     HTask &Tk = P.task[w];
     Tk.p0 = (int)P.prog.size();
     for (const Fin &F : fin[w]) {
       if (F.type == 2) {
-        const int pos = recs[F.w2][F.pre2].fidx + 1;
-        P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)F.w2 | (uint32_t)pos << 16, 0u));
+        P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)recs[F.w2][F.pre2].sig, 0u));
         continue;
       }
       if (F.type == 4) {  // chunk c starts: chunk c-1 is consumed, its stage takes chunk c-1+S
@@ -910,9 +938,10 @@ static int build_tape_program(cn_model *m, HClass &K) {
                                         ((r.flags & RF_FWD_IN) ? 1u << 24 : 0u),
                                     (uint32_t)RT_RUN, r.srow | (r.tm ? 1u << 20 : 0u), r.row));
       } else if (r.type == 1) {
-        P.prog.push_back(make_uint4(r.ring, r.flags | r.row << 16, r.srow, node_mask[x]));
+        P.prog.push_back(make_uint4(r.ring, r.flags | r.row << 16, r.srow | (uint32_t)r.sig << 16,
+                                    node_mask[x]));
       } else {
-        const uint32_t ey = r.flags | (r.tm ? (uint32_t)RF_TMEM : 0u);
+        const uint32_t ey = r.flags | (r.tm ? (uint32_t)RF_TMEM : 0u) | (uint32_t)r.sig << 16;
         // the parent's row is written (contribution) or read (v) only if it collects contributions
         // (RF_HAS_ACC); such a row is always in shared memory
         const uint32_t ez =
@@ -1007,7 +1036,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
     }
     // positions in the backward lists (a run whose parent sits on another warp is preceded by a
     // WAIT record; a single record carries its wait itself), signals, waits, encoding
-    std::vector<int> idxb(nu, 0);
+    std::vector<int> idxb(nu, 0), sigid_b(nu, -1);
     std::vector<uint8_t> sig_b(nu, 0);
     for (int w = 0; w < W; ++w) {
       int pos = 0;
@@ -1019,12 +1048,19 @@ static int build_tape_program(cn_model *m, HClass &K) {
         idxb[u] = pos++;
       }
     }
+    for (int u = 0; u < nu; ++u)
+      if (sig_b[u]) sigid_b[u] = P.n_bar++;
+    if (P.n_bar > 255) return give_up();
     for (int w = 0; w < W; ++w) {
       HTask &Tk = P.task[w];
       Tk.b0 = (int)P.prog.size();
       std::vector<int> seen(W, -1);
       for (int u : blist[w]) {
         uint4 e = P.prog[Tk.p0 + units[u].fin_idx];
+        if (!((e.y & RT_MASK) == RT_RUN)) {
+          e.y &= 0xFFFFu & ~(uint32_t)RF_SIG_F;  // the forward signal is not part of the backward copy
+          e.x = 0;
+        }
         const bool is_run = (e.y & RT_MASK) == RT_RUN;
         const int pu = punit[u];
         if (pu >= 0 && units[pu].w != w) {
@@ -1032,9 +1068,9 @@ static int build_tape_program(cn_model *m, HClass &K) {
           const int posb = (P.task[wp].p1 - P.task[wp].p0) + idxb[pu] + 1;
           if (posb > 4095) return give_up();
           if (is_run) {
-            P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)wp | (uint32_t)posb << 16, 0u));
+            P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)sigid_b[pu], 0u));
           } else if (seen[wp] < posb) {
-            e.y |= RF_WAIT_B | (uint32_t)posb << 16 | (uint32_t)wp << 28;
+            e.y |= RF_WAIT_B | (uint32_t)sigid_b[pu] << 16;
           }
           seen[wp] = std::max(seen[wp], posb);
         }
@@ -1048,6 +1084,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
         if (sig_b[u]) {
           if (is_run) return fail(CN_ERR_TOPOLOGY, "internal: tape program (a run cannot signal)");
           e.y |= RF_SIG_B;
+          e.x = (uint32_t)sigid_b[u];
         }
         if ((int)P.prog.size() - Tk.b0 != idxb[u])
           return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward positions)");
@@ -1071,7 +1108,8 @@ static int build_tape_program(cn_model *m, HClass &K) {
           node_of_srow[r.srow] = r.node;
         }
       }
-    std::vector<int> pc(W), ctrv(W, 0), acc(n, 0);
+    std::vector<int> pc(W), acc(n, 0);
+    std::vector<uint8_t> bar_done((size_t)P.n_bar + 1, 0);
     std::vector<uint8_t> done_e(n, 0), done_m(n, 0);
     for (int w = 0; w < W; ++w) pc[w] = P.task[w].p0;
     bool progress = true;
@@ -1083,7 +1121,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
           const uint32_t fl = e.y & 0xFFFFu;
           if ((fl & RT_MASK) == RT_CHUNK) {
           } else if ((fl & RT_MASK) == RT_WAIT) {
-            if (ctrv[e.z & 0xFFFFu] < (int)(e.z >> 16)) break;
+            if (!bar_done[e.z & 0xFFFFu]) break;
           } else if ((fl & RT_MASK) == RT_RUN) {
             for (uint32_t i = 0; i < ((e.x >> 16) & 255u); ++i) {
               const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + i]
@@ -1117,7 +1155,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
             }
             done_e[x] = 1;
           }
-          if (fl & RF_SIG_F) ctrv[w] = pc[w] - P.task[w].p0 + 1;
+          if (fl & RF_SIG_F) bar_done[(fl & RT_MASK) == RT_MECH ? e.z >> 16 : e.y >> 16] = 1;
           ++pc[w];
           progress = true;
         }
@@ -1128,7 +1166,6 @@ static int build_tape_program(cn_model *m, HClass &K) {
     // backward
     std::vector<uint8_t> done_b(n, 0), stored_v(n, 0);
     for (int w = 0; w < W; ++w) pc[w] = P.task[w].b0;
-    std::fill(ctrv.begin(), ctrv.end(), 0);
     std::vector<int> lastn(W, -1);  // the node whose v is in the warp's register
     progress = true;
     while (progress) {
@@ -1139,7 +1176,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
           const uint4 e = P.prog[pc[w]];
           const uint32_t fl = e.y & 0xFFFFu;
           if ((fl & RT_MASK) == RT_WAIT) {
-            if (ctrv[e.z & 0xFFFFu] < (int)(e.z >> 16)) break;
+            if (!bar_done[e.z & 0xFFFFu]) break;
           } else if ((fl & RT_MASK) == RT_RUN) {
             for (int i = (int)((e.x >> 16) & 255u) - 1; i >= 0; --i) {
               const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + (uint32_t)i]
@@ -1153,7 +1190,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
               lastn[w] = x;
             }
           } else if ((fl & RT_MASK) == RT_ELIM) {
-            if ((fl & RF_WAIT_B) && ctrv[e.y >> 28] < (int)((e.y >> 16) & 0xFFFu)) break;
+            if ((fl & RF_WAIT_B) && !bar_done[e.y >> 16]) break;
             const int x = (fl & RF_TMEM) ? node_of_slot[w][e.z & 1023u] : node_of_srow[e.z & 1023u];
             if (x) {
               const bool from_row = fl & RF_BW_ROW;
@@ -1165,7 +1202,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
             done_b[x] = 1;
             lastn[w] = x;
             if (fl & RF_HAS_ACC) stored_v[x] = 1;
-            if (fl & RF_SIG_B) ctrv[w] = (Tk.p1 - Tk.p0) + (pc[w] - Tk.b0) + 1;
+            if (fl & RF_SIG_B) bar_done[e.x & 0xFFFFu] = 1;
           } else {
             return fail(CN_ERR_TOPOLOGY, "internal: tape program (backward record type)");
           }
@@ -1342,7 +1379,8 @@ static int build_layout(cn_model *m) {
     const size_t sys_cap = (size_t)std::max(m->tape_sys_cap, K.tp.n_srow);
     const size_t prog_cap = std::max((size_t)m->tape_prog_cap, K.tp.prog.size());
     const size_t need = (size_t)m->tape_W * m->tape_S * m->tape_CH * 256 + sys_cap * 512 +
-                        prog_cap * 16 + 64 + ((size_t)m->tape_W * m->tape_S + 2) * 8 + 16;
+                        prog_cap * 16 +
+                        ((size_t)m->tape_W * m->tape_S + 2 + std::max(m->tape_bar_cap, K.tp.n_bar)) * 8 + 16;
     if (need > 227 * 1024) {
       K.tp.n_groups = 0;
       K.tp.n_cells = 0;
@@ -1353,6 +1391,7 @@ static int build_layout(cn_model *m) {
     prog_total += (int)K.tp.prog.size();
     m->tape_prog_cap = std::max(m->tape_prog_cap, (int)K.tp.prog.size());
     m->tape_sys_cap = std::max(m->tape_sys_cap, K.tp.n_srow);
+    m->tape_bar_cap = std::max(m->tape_bar_cap, K.tp.n_bar);
   }
 
   // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
@@ -1837,7 +1876,7 @@ static int finalize(cn_model *m, double dt) {
     for (size_t kc = 0; kc < m->cls.size(); ++kc) {
       const HClass &K = m->cls[kc];
       const HTape &P = K.tp;
-      tcls[kc] = TapeClass{K.n, P.prog_off, (int32_t)P.prog.size(), P.n_rows};
+      tcls[kc] = TapeClass{K.n, P.prog_off, (int32_t)P.prog.size(), P.n_bar};
       if (P.n_groups == 0) continue;
       if ((int)prog.size() != P.prog_off) return fail(CN_ERR_ARG, "internal: program offsets");
       prog.insert(prog.end(), P.prog.begin(), P.prog.end());
@@ -1856,6 +1895,7 @@ static int finalize(cn_model *m, double dt) {
     H.tape_CH = m->tape_CH;
     H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
     H.tape_sys_cap = std::max(m->tape_sys_cap, 1);
+    H.tape_bar_cap = m->tape_bar_cap;
     for (int t = 0; t < nt; ++t) {
       H.tab[t].pp_tape_begin = m->tab[t].pp_tape_begin;
       H.tab[t].pp_tape_end = m->tab[t].ti.point ? m->tab[t].n : 0;
@@ -1988,7 +2028,7 @@ static cudaError_t launch_step(cn_model *m, int64_t k) {
 static size_t tape_smem_bytes(const cn_model *m, int pbuf) {
   const size_t W = (size_t)m->tape_W;
   return W * m->tape_S * m->tape_CH * 256 + (size_t)m->hm.tape_sys_cap * 512 +
-         (size_t)pbuf * m->hm.tape_prog_cap * 16 + 64 + (W * m->tape_S + 2) * 8 + 16;
+         (size_t)pbuf * m->hm.tape_prog_cap * 16 + (W * m->tape_S + 2 + m->tape_bar_cap) * 8 + 16;
 }
 
 // Persistent CTAs: as many as fit the device at once (shared memory decides), each looping over

@@ -66,7 +66,7 @@ struct TapeGroup {
 };
 
 struct TapeClass {
-  int32_t n, prog_off, prog_len, n_rows;
+  int32_t n, prog_off, prog_len, n_bar;  // n_bar: signal mbarriers the class's program uses
 };
 
 // the part of a class's program that one warp runs: forward records [p0, p1), backward records
@@ -88,18 +88,20 @@ struct TapeTask {
 //         y = RT_RUN     z = system row of the first node (10), or, with bit 20 set, its slot in
 //             the warp's share of tensor memory     w = first tape row of the first node's record
 //   ELIM  x = ring byte offset (16)
-//         y = flags (16) | backward copy: wait position (12) and warp (4)
+//         y = flags (16) | forward: mbarrier the record arrives on (RF_SIG_F); backward copy:
+//             mbarrier to wait for (RF_WAIT_B); the backward copy arrives on mbarrier x (RF_SIG_B)
 //         z = own system row (10) | parent's system row (10)
 //         w = first tape row of the record (16) | tape row of the v copy in the node's mechanism
 //             record (16)
 //   MECH  x = ring byte offset (16)
 //         y = flags (16) | first tape row of the record (16)
-//         z = system row of the node     w = mask of the distributed tables on the node
+//         z = system row of the node (10) | mbarrier the record arrives on (16, RF_SIG_F)
+//         w = mask of the distributed tables on the node
 //   CHUNK the records that follow sit in the next chunk: the stage of the chunk before it is free
 //         x = first row (relative to the warp's segment) of the chunk to request into that stage
 //             (16) | its rows (8; 0: nothing left to request)
 //         y = RT_CHUNK   z = stage to fill (16) | stage to wait for (16)
-//   WAIT  y = RT_WAIT    z = warp (16) | position (16)
+//   WAIT  y = RT_WAIT    z = mbarrier to wait for
 enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
        RF_FWD_IN = 4,     // the previous record of this warp handed its contribution in registers
        RF_HAS_ACC = 8,    // contributions (mechanisms, children) wait in the node's own system row
@@ -117,7 +119,7 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
   int32_t n_tgroup, tape_prog_cap, tape_sys_cap, tape_W;
-  int32_t tape_S, tape_CH, tape_pbuf, pad_t2;  // ring of a warp: S stages of CH rows; program buffers
+  int32_t tape_S, tape_CH, tape_pbuf, tape_bar_cap;  // ring of a warp: S stages of CH rows; program buffers
   const TapeGroup *tgrp;
   const TapeClass *tcls;
   const TapeTask *ttask;        // [n_class][tape_W]

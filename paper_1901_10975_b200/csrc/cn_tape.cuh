@@ -13,7 +13,7 @@
 //   * The tree is compiled by the host into W record lists (a static schedule of the elimination
 //     over W warps, children before parents, L196).  A chain hands its contribution to the parent
 //     in REGISTERS; at a branch point the contributions meet in the parent's system row.  Warps
-//     synchronise only through per-warp progress counters in shared memory (WAIT records).
+//     synchronise only through mbarriers in shared memory (WAIT records / signal flags).
 //   * Each warp streams its own segment of the tape through a shared-memory ring with 1-D TMA bulk
 //     copies (cp.async.bulk.shared.global + mbarrier complete_tx), S chunks of CH rows in flight,
 //     issued by one lane; the ring of a warp that has finished its part of a group already loads
@@ -59,18 +59,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}" ::"r"(bar), "r"(parity)
       : "memory");
 }
-// Per-warp progress counters in shared memory.  Producer: all lanes write their system rows
-// (shared memory), __syncwarp, then one lane stores the counter with release semantics; consumer:
-// every lane polls the counter with acquire semantics, then reads the rows.  (Plain volatile
-// accesses are NOT enough: measured, the rows can be read before they are written.)
-__device__ __forceinline__ void ctr_publish(uint32_t addr, uint32_t val) {
-  asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(val) : "memory");
-}
-__device__ __forceinline__ void ctr_wait(uint32_t addr, uint32_t target) {
-  uint32_t x;
-  do {
-    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(x) : "r"(addr) : "memory");
-  } while ((int32_t)(x - target) < 0);
+// Signals between the warps of a CTA: every record that another warp waits for arrives on an
+// mbarrier of its own after its shared-memory writes (release; all lanes write, __syncwarp, one
+// lane arrives); the waiting warp sleeps in mbarrier.try_wait (acquire) instead of spinning on a
+// flag, which would take issue slots from the warps that work.  (Plain volatile flags are NOT
+// enough either: measured, the rows can then be read before they are written.)
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
 // Reciprocal to ~1 ulp without the special-case handling of an IEEE division: MUFU.RCP64H seed
@@ -249,7 +244,7 @@ __device__ __forceinline__ void mech_record(const DModel &M, const unsigned char
 // One CTA = W warps = one group of 32 cells at a time (persistent over groups).  See the header
 // of this file and the record layout in cn_device.cuh.
 // Shared memory: W rings of S stages x CH rows | system: tape_sys_cap x (32 + 32) doubles | one
-// or two program buffers of tape_prog_cap records | 16 progress counters | W*S + 2 mbarriers | TMEM base.
+// or two program buffers of tape_prog_cap records | W*S + 2 + tape_bar_cap mbarriers | TMEM base.
 // Tensor memory as a per-lane scratchpad (Blackwell: 512 columns x 128 lanes x 32 bit per SM; a
 // warp addresses the 32 lanes of its quarter, thread i <-> lane i): (multiplier, reduced rhs) of a
 // plain chain node = 4 columns.  SASS: STTM / LDTM.
@@ -290,12 +285,12 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
   uint4 *progbuf = reinterpret_cast<uint4 *>(sm_raw + (size_t)W * RB +
                                              (size_t)M.tape_sys_cap * 512);
   const int PB = M.tape_pbuf;  // program buffers: 2 (the next program loads during the group) or 1
-  uint32_t *ctr = reinterpret_cast<uint32_t *>(progbuf + (size_t)PB * M.tape_prog_cap);
-  uint64_t *mbar_all = reinterpret_cast<uint64_t *>(ctr + 16);
+  uint64_t *mbar_all = reinterpret_cast<uint64_t *>(progbuf + (size_t)PB * M.tape_prog_cap);
   const uint32_t ring_s = smem_u32(sm_raw + (size_t)warp * RB);
   const uint32_t bar_s = smem_u32(mbar_all + (size_t)warp * S);  // S ring barriers of this warp
   const uint32_t pbar_s = smem_u32(mbar_all + (size_t)W * S);    // 2 program barriers
-  const uint32_t ctr_s = smem_u32(ctr);
+  const int NB = M.tape_bar_cap;  // signal mbarriers: one per signalling record of a program
+  const uint32_t sbar_s = smem_u32(mbar_all + (size_t)W * S + 2);
   const double dt = M.dt;
   const double q10dt = M.q10 * dt;
   const bool flush = mode & TM_FLUSH;
@@ -304,13 +299,12 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
 #define CN_RD(base, i) (*reinterpret_cast<const double *>((base) + (uint32_t)(i) * 256u))
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < W * S + 2; ++s) mbar_init(smem_u32(mbar_all + s), 1);
-    for (int w = 0; w < 16; ++w) ctr[w] = 0;
+    for (int s = 0; s < W * S + 2 + NB; ++s) mbar_init(smem_u32(mbar_all + s), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   if (blockIdx.x >= ngrp) return;
-  uint32_t *tm_base_s = reinterpret_cast<uint32_t *>(mbar_all + (size_t)W * S + 2);
+  uint32_t *tm_base_s = reinterpret_cast<uint32_t *>(mbar_all + (size_t)W * S + 2 + NB);
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
                      smem_u32(tm_base_s)),
@@ -400,7 +394,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
   start_segment(tg, tk);
 
   for (uint32_t it = 0; cur < n_items; ++it) {
-    const uint32_t base = (it + 1) << 13;  // progress counters never run backwards
+    const uint32_t sphase = it & 1u;  // every signal mbarrier completes once per group
     const int g = (int)(cur % (uint32_t)ngrp);
     const int step_in = (int)(cur / (uint32_t)ngrp);  // step of the window
     const int64_t kk = k + step_in;
@@ -488,7 +482,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         continue;
       }
       if (ty == RT_WAIT) {
-        if (!flush) ctr_wait(ctr_s + 4 * (e.z & 0xFFFFu), base + (e.z >> 16));
+        if (!flush) mbar_wait(sbar_s + 8 * e.z, sphase);
         continue;
       }
       const uint32_t fl = e.y & 0xFFFFu;
@@ -558,9 +552,9 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           srow[32] = gR;
         }
       }
-      if (fl & RF_SIG_F) {
+      if ((fl & RF_SIG_F) && !flush) {
         __syncwarp();
-        if (lane == 0) ctr_publish(ctr_s + 4 * warp, base + (uint32_t)(j - p0) + 1u);
+        if (lane == 0) mbar_arrive(sbar_s + 8 * (ty == RT_MECH ? e.z >> 16 : e.y >> 16));
       }
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
@@ -576,7 +570,6 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     // backward: back-substitution (L66), v to the tape, threshold at the root (L68)
     // ========================================================================================
     if (!flush) {
-      const uint32_t nrec = (uint32_t)(tk.p1 - tk.p0);
       double v_prev = 0.0;
       for (int j = tk.b0; j < tk.b1; ++j) {
         const uint4 e = prog[j];
@@ -610,13 +603,13 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           continue;
         }
         if (ty == RT_WAIT) {
-          ctr_wait(ctr_s + 4 * (e.z & 0xFFFFu), base + (e.z >> 16));
+          mbar_wait(sbar_s + 8 * e.z, sphase);
           CN_TR(3);
           continue;
         }
         const uint32_t fl = e.y & 0xFFFFu;
         if (fl & RF_WAIT_B) {
-          ctr_wait(ctr_s + 4 * (e.y >> 28), base + ((e.y >> 16) & 0xFFFu));
+          mbar_wait(sbar_s + 8 * (e.y >> 16), sphase);
           CN_TR(3);
         }
         double *srow = sys_l + (e.z & 1023u) * 64u;
@@ -636,7 +629,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         if (fl & RF_MECHV) tape_l[(e.w >> 16) * 32u] = v;
         if (fl & RF_SIG_B) {
           __syncwarp();
-          if (lane == 0) ctr_publish(ctr_s + 4 * warp, base + nrec + (uint32_t)(j - tk.b0) + 1u);
+          if (lane == 0) mbar_arrive(sbar_s + 8 * (e.x & 0xFFFFu));
         }
         if ((fl & RK_KIND) == RK_ROOT) {  // warp-ballot threshold detection, one atomic per warp
           bool fire = false;
@@ -666,7 +659,10 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
       }
     }
     CN_TR(4);
-    __syncthreads();  // the system rows and counters of this group are dead from here on
+    __syncthreads();  // the system rows of this group are dead from here on
+    // the signal mbarriers this program did not use complete their phase too
+    for (int b = (flush ? 0 : tc.n_bar) + (int)threadIdx.x; b < NB; b += (int)blockDim.x)
+      mbar_arrive(sbar_s + 8 * b);
     if (window) {
       if (threadIdx.x == 0) {  // every global write of the CTA for (step, group) is visible first
         __threadfence();
