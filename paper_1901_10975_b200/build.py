@@ -12,7 +12,7 @@ DEPS = SRCS + [HERE / "csrc" / "cn_device.cuh", HERE / "csrc" / "cn_tape.cuh",
                HERE.parent / "include" / "cn.h"]
 
 NVCC_FLAGS = (["-DCN_TRACE"] if os.environ.get("CN_TRACE") else []) + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared"]
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:

@@ -5,6 +5,7 @@
 #include "cn_tape.cuh"
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -13,6 +14,7 @@
 #include <new>
 #include <numeric>
 #include <string>
+#include <thread>
 #include <unordered_map>
 #include <vector>
 
@@ -180,7 +182,6 @@ struct cn_model {
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
   bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
   bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
-  int tape_need_CH = 0;             // longest record that did not fit a chunk (build_layout retries)
   int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
   bool window = false;              // window mode: one launch of the interleaved kernel per
   int win_steps = 0;                //   up to win_steps steps (cn_tape.cuh)
@@ -298,6 +299,21 @@ static bool finite_all(const double *x, int64_t n) {
   for (int64_t i = 0; i < n; ++i)
     if (!std::isfinite(x[i])) return false;
   return true;
+}
+
+// body(begin, end) over [0, n_items) on all host cores (create / first-run set-up only)
+template <class F>
+static void par_for(int64_t n_items, int64_t grain, F &&body) {
+  const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+  const unsigned nth = (unsigned)std::min<int64_t>(hw, std::max<int64_t>(1, n_items / grain));
+  if (nth <= 1) {
+    body((int64_t)0, n_items);
+    return;
+  }
+  std::vector<std::thread> pool;
+  for (unsigned t = 0; t < nth; ++t)
+    pool.emplace_back([&body, n_items, nth, t] { body(n_items * t / nth, n_items * (t + 1) / nth); });
+  for (auto &th : pool) th.join();
 }
 
 static int build_layout(cn_model *m);
@@ -834,10 +850,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
       } else {
         ln = 5 + (P.has_pp[x] ? 2 : 0);
       }
-      if (ln > CH) {  // a record must fit a chunk
-        m->tape_need_CH = std::max(m->tape_need_CH, (int)ln);
-        return give_up();
-      }
+      if (ln > CH) return give_up();  // a record must fit a chunk (build_layout sizes CH for it)
       r.row = row;
       r.len = ln;
       row += ln;
@@ -1221,6 +1234,15 @@ static int build_tape_program(cn_model *m, HClass &K) {
 }
 
 static int build_layout(cn_model *m) {
+  const bool dbg = std::getenv("CN_DEBUG") != nullptr;
+  auto t_prev = std::chrono::steady_clock::now();
+  auto lap = [&](const char *what) {
+    if (!dbg) return;
+    const auto t = std::chrono::steady_clock::now();
+    fprintf(stderr, "[cn] build_layout %-28s %7.1f ms\n", what,
+            std::chrono::duration<double, std::milli>(t - t_prev).count());
+    t_prev = t;
+  };
   const int32_t nc = m->n_cell;
   const int64_t N = m->N;
   const int nt = (int)m->tab.size();
@@ -1247,9 +1269,11 @@ static int build_layout(cn_model *m) {
           return fail(CN_ERR_MECH, "table %d: two instances on node %d", t, T.node[*it]);
     }
   }
+  lap("node -> cell, instance CSR");
   // shape signature per cell: topology + placement of every distributed table
   std::vector<uint64_t> sig(nc);
-  for (int32_t c = 0; c < nc; ++c) {
+  par_for(nc, 4096, [&](int64_t c0, int64_t c1) {
+  for (int32_t c = (int32_t)c0; c < (int32_t)c1; ++c) {
     const int64_t f = m->cell_first[c], l = m->cell_first[c + 1];
     uint64_t h = mix64(0x1234567ull, (uint64_t)(l - f));
     for (int64_t i = f + 1; i < l; ++i) h = mix64(h, (uint64_t)(m->parent[i] - f));
@@ -1262,6 +1286,8 @@ static int build_layout(cn_model *m) {
     }
     sig[c] = h;
   }
+  });
+  lap("signatures");
   auto same_shape = [&](int32_t x, int32_t y) {
     const int64_t fx = m->cell_first[x], fy = m->cell_first[y];
     const int64_t n = m->cell_first[x + 1] - fx;
@@ -1358,22 +1384,58 @@ static int build_layout(cn_model *m) {
       if (P.n_groups > 0) P.has_pp[T.node[i] - m->cell_first[c]] = 1;
     }
   }
+  lap("classes");
   // chunk size: the default suits plain nodes (three 5-row records); a model whose mechanism
   // records are longer gets chunks of that length (a dry pass over the classes finds out)
   if (!std::getenv("CN_TAPE_CH")) {
-    for (HClass &K : m->cls) {
+    int need = 0;
+    for (const HClass &K : m->cls) {
       if (K.tp.n_groups == 0) continue;
-      HClass probe = K;
-      int rc = build_tape_program(m, probe);
-      if (rc != CN_OK) return rc;
+      // rows of the longest mechanism record of the class: v copy, [cai], [ica], table rows
+      std::vector<int> rows(K.n, 0);
+      std::vector<uint8_t> cai(K.n, 0), ica(K.n, 0);
+      const int64_t f = m->cell_first[K.rep_cell];
+      for (int t = 0; t < nt; ++t) {
+        const HTable &T = m->tab[t];
+        if (T.ti.point || T.type == CN_PAS) continue;
+        for (int64_t q = T.cell_first[K.rep_cell]; q < T.cell_first[K.rep_cell + 1]; ++q) {
+          const int x = (int)(T.node[T.cell_inst[q]] - f);
+          rows[x] += tape_rows_of(T.ti, T.type);
+          if (T.type == CN_CADYN) cai[x] = ica[x] = 1;
+          if (T.type == CN_SK) cai[x] = 1;
+        }
+      }
+      for (int x = 0; x < K.n; ++x)
+        if (rows[x] || cai[x]) need = std::max(need, 1 + cai[x] + ica[x] + rows[x]);
     }
-    if (m->tape_need_CH > m->tape_CH && m->tape_need_CH <= 63) m->tape_CH = m->tape_need_CH;
+    if (need > m->tape_CH && need <= 63) m->tape_CH = need;
+  }
+  lap("chunk-length pass");
+  {  // the classes are independent: compile their programs on all host cores
+    std::vector<int> todo;
+    for (int kc = 0; kc < (int)m->cls.size(); ++kc)
+      if (m->cls[kc].tp.n_groups > 0) todo.push_back(kc);
+    const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+    const unsigned nth = (unsigned)std::min<size_t>(hw, std::max<size_t>(1, todo.size() / 8));
+    std::vector<int> rcs(nth, CN_OK);
+    auto work = [&](unsigned tix) {
+      for (size_t j = tix; j < todo.size(); j += nth) {
+        const int rc = build_tape_program(m, m->cls[todo[j]]);
+        if (rc != CN_OK) rcs[tix] = rc;
+      }
+    };
+    if (nth <= 1) {
+      work(0);
+    } else {
+      std::vector<std::thread> pool;
+      for (unsigned tix = 0; tix < nth; ++tix) pool.emplace_back(work, tix);
+      for (auto &th : pool) th.join();
+    }
+    for (int rc : rcs)
+      if (rc != CN_OK) return fail(rc, "internal: compiling a tape program failed");
   }
   int prog_total = 0;
   for (HClass &K : m->cls) {
-    if (K.tp.n_groups == 0) continue;
-    int rc = build_tape_program(m, K);
-    if (rc != CN_OK) return rc;
     if (K.tp.n_groups == 0) continue;
     // the CTA must fit: rings + system + two program buffers + counters and barriers
     const size_t sys_cap = (size_t)std::max(m->tape_sys_cap, K.tp.n_srow);
@@ -1394,6 +1456,7 @@ static int build_layout(cn_model *m) {
     m->tape_bar_cap = std::max(m->tape_bar_cap, K.tp.n_bar);
   }
 
+  lap("tape programs");
   // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
   int force_g = 0;
   if (const char *e = std::getenv("CN_FORCE_G")) force_g = std::atoi(e);
@@ -1601,6 +1664,7 @@ static int build_layout(cn_model *m) {
   if (const char *e = std::getenv("CN_WPB")) wpb = std::max(1, std::atoi(e));
   while (wpb > 1 && wbytes * wpb > 110 * 1024) wpb /= 2;
   m->wpb = wpb;
+  lap("groups, instance layout");
   return CN_OK;
 }
 
@@ -1610,6 +1674,15 @@ static int build_layout(cn_model *m) {
 // ---------------------------------------------------------------------------------------------
 
 static int finalize(cn_model *m, double dt) {
+  const bool dbg = std::getenv("CN_DEBUG") != nullptr;
+  auto t_prev = std::chrono::steady_clock::now();
+  auto lap = [&](const char *what) {
+    if (!dbg) return;
+    const auto t = std::chrono::steady_clock::now();
+    fprintf(stderr, "[cn] finalize %-32s %7.1f ms\n", what,
+            std::chrono::duration<double, std::milli>(t - t_prev).count());
+    t_prev = t;
+  };
   const int64_t N = m->N;
   const int nt = (int)m->tab.size();
   const int ng = (int)m->grp.size();
@@ -1638,46 +1711,55 @@ static int finalize(cn_model *m, double dt) {
   double *tape = v0.data() + m->n_ab;
   std::vector<double> dsum((size_t)N), rsum((size_t)N, 0.0);
   std::vector<int32_t> cell_of_node((size_t)N);
-  for (int32_t c = 0; c < m->n_cell; ++c)
-    for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of_node[i] = c;
-  for (int64_t i = 0; i < N; ++i) {
-    const double c = 1e-3 * m->cm[i] / dt;
-    invc[i] = 1.0 / c;
-    dsum[i] = c;
-  }
-  for (int64_t i = 0; i < N; ++i) {
-    const int32_t p = m->parent[i];
-    if (p >= 0) {
-      const double b = -100.0 / (m->ri[i] * m->area[i]);
-      const double a = -100.0 / (m->ri[i] * m->area[p]);
-      dsum[i] -= b;
-      dsum[p] -= a;
-      bn[i] = b * invc[i];
-      an[i] = a * invc[p];
+  // cells are independent (a parent sits in the same cell): all host cores
+  par_for(m->n_cell, 256, [&](int64_t c0, int64_t c1) {
+    const int64_t i0 = m->cell_first[c0], i1 = m->cell_first[c1];
+    for (int64_t c = c0; c < c1; ++c)
+      for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of_node[i] = (int32_t)c;
+    for (int64_t i = i0; i < i1; ++i) {
+      const double c = 1e-3 * m->cm[i] / dt;
+      invc[i] = 1.0 / c;
+      dsum[i] = c;
     }
-  }
-  for (const HTable &T : m->tab)
-    if (T.type == CN_PAS)
-      for (int64_t i = 0; i < T.n; ++i) {
-        const double g = T.param[i], e = T.param[T.n + i];
-        dsum[T.node[i]] += g;
-        rsum[T.node[i]] += g * e;
+    for (int64_t i = i0; i < i1; ++i) {
+      const int32_t p = m->parent[i];
+      if (p >= 0) {
+        const double b = -100.0 / (m->ri[i] * m->area[i]);
+        const double a = -100.0 / (m->ri[i] * m->area[p]);
+        dsum[i] -= b;
+        dsum[p] -= a;
+        bn[i] = b * invc[i];
+        an[i] = a * invc[p];
       }
-  for (int64_t i = 0; i < N; ++i) {
-    const int64_t q = m->node_pos[i];
-    if (m->cell_tape[cell_of_node[i]]) {  // q is the node's v element; a, b, d, r precede it
-      double *rec = v0.data() + q;
-      rec[-4 * 32] = an[i];
-      rec[-3 * 32] = bn[i];
-      rec[-2 * 32] = dsum[i] * invc[i];
-      rec[-1 * 32] = rsum[i] * invc[i];
-      rec[0] = m->v_init;
-    } else {
-      dstat[q] = dsum[i] * invc[i];
-      rstat[q] = rsum[i] * invc[i];
-      v0[q] = m->v_init;
     }
-  }
+  });
+  for (const HTable &T : m->tab)
+    if (T.type == CN_PAS)  // (at most one instance of a table per node: no two threads meet)
+      par_for(T.n, 65536, [&](int64_t q0, int64_t q1) {
+        for (int64_t i = q0; i < q1; ++i) {
+          const double g = T.param[i], e = T.param[T.n + i];
+          dsum[T.node[i]] += g;
+          rsum[T.node[i]] += g * e;
+        }
+      });
+  par_for(N, 65536, [&](int64_t i0, int64_t i1) {
+    for (int64_t i = i0; i < i1; ++i) {
+      const int64_t q = m->node_pos[i];
+      if (m->cell_tape[cell_of_node[i]]) {  // q is the node's v element; a, b, d, r precede it
+        double *rec = v0.data() + q;
+        rec[-4 * 32] = an[i];
+        rec[-3 * 32] = bn[i];
+        rec[-2 * 32] = dsum[i] * invc[i];
+        rec[-1 * 32] = rsum[i] * invc[i];
+        rec[0] = m->v_init;
+      } else {
+        dstat[q] = dsum[i] * invc[i];
+        rstat[q] = rsum[i] * invc[i];
+        v0[q] = m->v_init;
+      }
+    }
+  });
+  lap("static rows");
   // idle lanes of a ragged tape group: unit diagonal, everything else zero; cai rows
   for (const TapeGroup &tg : m->tgrp) {
     const HTape &P = m->cls[tg.cls].tp;
@@ -1701,6 +1783,7 @@ static int finalize(cn_model *m, double dt) {
         if (P.cai_row[i] >= 0)
           tape[tg.tape_base + (int64_t)P.cai_row[i] * 32 + m->cell_slot[c]] = m->cai0[f + i];
     }
+  lap("idle lanes, v copies, cai");
   // schedule-ordered off-diagonals
   std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
   std::vector<uint32_t> sched_all;
@@ -1737,6 +1820,7 @@ static int finalize(cn_model *m, double dt) {
         }
     }
   }
+  lap("coop schedule arrays");
   // thresholds, flags, gids per permuted cell
   std::vector<double> thr((size_t)m->n_pcell, 0.0);
   std::vector<unsigned char> flag((size_t)m->n_pcell, 0);
@@ -1782,6 +1866,7 @@ static int finalize(cn_model *m, double dt) {
     unsigned char *pf; UP(flag, pf); H.flag = pf;
     int32_t *pg; UP(gid_of, pg); H.gid_of_pcell = pg;
   }
+  lap("small uploads");
   // mechanism tables
   for (int t = 0; t < nt; ++t) {
     HTable &T = m->tab[t];
@@ -1865,6 +1950,7 @@ static int finalize(cn_model *m, double dt) {
       D.cls_cnt = T.d_cls_cnt; D.cls_nodeoff = T.d_cls_nodeoff; D.grp_instbase = T.d_grp_instbase;
     }
   }
+  lap("mechanism tables");
   // the arena (filled above, including the mechanism rows of the tapes) and the programs
   {
     UP(v0, m->d_v);
@@ -1911,6 +1997,7 @@ static int finalize(cn_model *m, double dt) {
     H.tab[t].cls_cnt = T.d_cls_cnt; H.tab[t].cls_nodeoff = T.d_cls_nodeoff;
     H.tab[t].grp_instbase = T.d_grp_instbase;
   }
+  lap("arena + programs upload");
   // NetCons: CSR by source gid, sorted by delay steps (stable in caller order)
   {
     std::vector<int64_t> order((size_t)m->n_netcon);
@@ -1956,6 +2043,7 @@ static int finalize(cn_model *m, double dt) {
     UP(ss, p64); H.stim_step = p64;
     H.n_stim = ns;
   }
+  lap("netcons");
   // window mode: every cell on the interleaved kernel, no point process whose current depends on
   // v (AMPA+NMDA), no per-step probes; a window is at most the smallest delay long
   {
@@ -1988,6 +2076,7 @@ static int finalize(cn_model *m, double dt) {
   rc = dev_alloc(m, 1, &m->d_overflow); if (rc) return rc;
   H.sp_gid = m->d_sp_gid; H.sp_step = m->d_sp_step; H.n_sp = m->d_nsp; H.sp_cap = m->sp_cap;
   H.overflow = m->d_overflow;
+  lap("window buffers, spikes");
   // caller-order lookup for cn_get_v, probes
   UP(m->node_pos, m->d_node_pos);
   rc = dev_alloc(m, (size_t)std::max<int64_t>(N, 1), &m->d_gather, false); if (rc) return rc;
