@@ -1970,7 +1970,7 @@ static int finalize(cn_model *m, double dt) {
         const HTask &Tk = P.task[w];
         // program positions are relative to the class's program (as it sits in shared memory)
         ttask[kc * (size_t)m->tape_W + w] =
-            TapeTask{Tk.p0, Tk.p1, Tk.b0, Tk.b1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.head};
+            TapeTask{Tk.p0, Tk.p1, Tk.b0, Tk.b1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.head, Tk.nrows, 0};
       }
     }
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
@@ -1982,6 +1982,8 @@ static int finalize(cn_model *m, double dt) {
     H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
     H.tape_sys_cap = std::max(m->tape_sys_cap, 1);
     H.tape_bar_cap = m->tape_bar_cap;
+    H.tape_pf = 0;  // measured on config 4: prefetching ahead of the ring only costs (0: off)
+    if (const char *e = std::getenv("CN_TAPE_PF")) H.tape_pf = std::max(0, std::min(4096, std::atoi(e)));
     for (int t = 0; t < nt; ++t) {
       H.tab[t].pp_tape_begin = m->tab[t].pp_tape_begin;
       H.tab[t].pp_tape_end = m->tab[t].ti.point ? m->tab[t].n : 0;

@@ -77,6 +77,7 @@ struct TapeTask {
   int32_t p0, p1, b0, b1;
   int32_t nchunk, tm_base;  // tm_base: first tensor-memory slot of the warp
   uint32_t row0, head;
+  uint32_t nrows, pad0;     // rows of the segment
 };
 
 // Program record (uint4) of the interleaved kernel: one per run of plain chain nodes (RUN), per
@@ -119,6 +120,7 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
   int32_t n_tgroup, tape_prog_cap, tape_sys_cap, tape_W;
+  int32_t tape_pf, pad_pf;      // rows a warp's L2 prefetch runs ahead of its ring
   int32_t tape_S, tape_CH, tape_pbuf, tape_bar_cap;  // ring of a warp: S stages of CH rows; program buffers
   const TapeGroup *tgrp;
   const TapeClass *tcls;

@@ -328,8 +328,20 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     bulk_g2s(ring_s + stage * (uint32_t)(CH * 256), seg + (size_t)row * 32, bytes,
              bar_s + 8 * stage);
   };
+  // rows [r0, r1) of the segment towards L2, so that the bulk copy that follows PF rows later
+  // finds them there (the ring holds two chunks per warp: its refills are latency-bound)
+  uint32_t seg_rows = 0;
+  const uint32_t PF = (uint32_t)M.tape_pf;
+  auto prefetch = [&](uint32_t r0, uint32_t r1) {  // one lane
+    r1 = min(r1, seg_rows);
+    if (r0 < r1)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(seg + (size_t)r0 * 32),
+                   "r"((r1 - r0) * 256u)
+                   : "memory");
+  };
   auto start_segment = [&](const TapeGroup &g, const TapeTask &t) {
     seg = M.tape + g.tape_base + (size_t)t.row0 * 32;
+    seg_rows = t.nrows;
     if (lane == 0) {
       uint32_t row = 0;
       for (int c = 0; c < S && c < t.nchunk; ++c) {
@@ -337,6 +349,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         issue((uint32_t)c, row, rows);
         row += rows;
       }
+      if (PF) prefetch(row, row + PF);
     }
   };
   auto load_program = [&](const TapeClass &c, int buf) {  // one thread
@@ -474,7 +487,10 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         const uint32_t rows = (e.x >> 16) & 255u;
         if (rows) {
           __syncwarp();
-          if (lane == 0) issue(e.z & 0xFFFFu, e.x & 0xFFFFu, rows);
+          if (lane == 0) {
+            issue(e.z & 0xFFFFu, e.x & 0xFFFFu, rows);
+            if (PF) prefetch((e.x & 0xFFFFu) + PF, (e.x & 0xFFFFu) + rows + PF);
+          }
         }
         const uint32_t s = e.z >> 16;
         mbar_wait(bar_s + 8 * s, (phase >> s) & 1u);
