@@ -185,13 +185,16 @@ class Model:
             self.set_stream(stream)
 
     def __del__(self):
-        self.destroy()
+        try:
+            self.destroy()
+        except Exception:  # interpreter shutdown: the module globals may be gone already
+            pass
 
     def destroy(self):
         h = getattr(self, "_h", None)
         if h:
-            lib().cn_model_destroy(h)
             self._h = None
+            lib().cn_model_destroy(h)
 
     def set_stream(self, cuda_stream_handle: int):
         _check(lib().cn_set_stream(self._h, C.c_void_p(int(cuda_stream_handle))))

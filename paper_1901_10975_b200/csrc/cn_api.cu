@@ -482,7 +482,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
   const int n = K.n;
   const int nt = (int)m->tab.size();
   const int W = m->tape_W;
-  const uint32_t CH = (uint32_t)m->tape_CH, R = (uint32_t)(m->tape_S * m->tape_CH);
+  const uint32_t CH = (uint32_t)m->tape_CH;
   const int64_t f = m->cell_first[K.rep_cell];
   auto give_up = [&]() {  // this class stays on the cooperative kernel
     P.n_groups = 0;
@@ -1880,6 +1880,7 @@ static int finalize(cn_model *m, double dt) {
     if (T.type == CN_AMPANMDA) {
       D.glob[7] = h_exp2_factor(T.glob[0], T.glob[1]);
       D.glob[8] = h_exp2_factor(T.glob[2], T.glob[3]);
+      for (int c = 0; c < 4; ++c) D.glob[9 + c] = 1.0 - std::exp(-dt / T.glob[c]);  // cnexp factors
     }
     if (T.type == CN_PAS) continue;  // folded
     const int64_t nd = T.n_dev;
@@ -1906,10 +1907,15 @@ static int finalize(cn_model *m, double dt) {
           S[2] = al / (al + be);
           break;
         }
-        case CN_EXPSYN: P[2] = scale; break;
+        case CN_EXPSYN:  // tau -> the cnexp factor 1 - exp(-dt/tau) (the device never needs tau)
+          P[2] = scale;
+          P[0] = 1.0 - std::exp(-dt / P[0]);
+          break;
         case CN_EXP2SYN:
           P[3] = scale;
           P[4] = h_exp2_factor(P[0], P[1]);
+          P[0] = 1.0 - std::exp(-dt / P[0]);
+          P[1] = 1.0 - std::exp(-dt / P[1]);
           break;
         case CN_ICLAMP: P[3] = scale; break;
         case CN_HHFORM:
@@ -2149,6 +2155,7 @@ static cudaError_t launch_tape(cn_model *m, int64_t k, int mode, int nsteps = 1)
     if (m->tape_W <= 8 && 2 * (tape_smem_bytes(m, 2) + 1024) > (size_t)smem_sm &&
         2 * (tape_smem_bytes(m, 1) + 1024) <= (size_t)smem_sm)
       m->hm.tape_pbuf = 1;
+    if (tape_smem_bytes(m, 2) > 227 * 1024) m->hm.tape_pbuf = 1;  // (build_layout fitted one buffer)
     if (const char *s = std::getenv("CN_TAPE_PBUF")) m->hm.tape_pbuf = std::atoi(s) == 1 ? 1 : 2;
     const size_t smem = tape_smem_bytes(m, m->hm.tape_pbuf);
     per_sm = (m->tape_W <= 8 && 2 * (smem + 1024) <= (size_t)smem_sm) ? 2 : 1;

@@ -182,6 +182,10 @@ __device__ __forceinline__ double cnexp(double y, double yinf, double tau, doubl
   return y + (1.0 - exp(-dt / tau)) * (yinf - y);
 }
 
+// cnexp towards 0 with the factor c = 1 - exp(-dt/tau) precomputed by the host (per instance for
+// ExpSyn / Exp2Syn, per table for AMPA+NMDA): the same expression as cnexp(y, 0, tau, dt)
+__device__ __forceinline__ double decay(double y, double c) { return y + c * (0.0 - y); }
+
 __device__ __forceinline__ void hh_rates(double v, double q10, double &minf, double &mtau,
                                          double &hinf, double &htau, double &ninf,
                                          double &ntau) {
@@ -290,28 +294,48 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
   }
 }
 
-// Point-process table: instances of this group, arbitrary nodes -> shared-memory atomics.
+// Point-process table: instances of this group, arbitrary nodes -> shared-memory atomics.  The
+// states of these types do not depend on v, so their nrn_state (decay over dt) is applied in the
+// same pass, right after the current is taken (one read and one write of every state per dt);
+// four instances per lane are in flight at a time.
 __device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i1, double *D,
                                           double *R, const GroupView &gv, const double *v_g,
                                           int lane, double t_mid) {
   switch (T.type) {
     case T_EXPSYN:
       for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double g = T.state[0][q] * T.param[2][q];  // param[2] = 100/area/c
-        if (g != 0.0) {
+        const double s0 = T.state[0][q];
+        if (s0 != 0.0) {
+          const double g = s0 * T.param[2][q];  // param[2] = 100/area/c
           const int slot = T.pp_slot[q];
           atomicAdd(&D[slot], g);
           atomicAdd(&R[slot], g * T.param[1][q]);
+          T.state[0][q] = decay(s0, T.param[0][q]);
         }
       }
       break;
     case T_EXP2SYN:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double g = (T.state[1][q] - T.state[0][q]) * T.param[3][q];
-        if (g != 0.0) {
-          const int slot = T.pp_slot[q];
-          atomicAdd(&D[slot], g);
-          atomicAdd(&R[slot], g * T.param[2][q]);
+      for (int64_t q0 = i0 + lane; q0 < i1; q0 += 128) {
+        double A[4], B[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int64_t q = q0 + 32 * j;
+          A[j] = q < i1 ? T.state[0][q] : 0.0;
+          B[j] = q < i1 ? T.state[1][q] : 0.0;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int64_t q = q0 + 32 * j;
+          if (A[j] != 0.0 || B[j] != 0.0) {
+            const double g = (B[j] - A[j]) * T.param[3][q];
+            if (g != 0.0) {
+              const int slot = T.pp_slot[q];
+              atomicAdd(&D[slot], g);
+              atomicAdd(&R[slot], g * T.param[2][q]);
+            }
+            T.state[0][q] = decay(A[j], T.param[0][q]);
+            T.state[1][q] = decay(B[j], T.param[1][q]);
+          }
         }
       }
       break;
@@ -323,15 +347,30 @@ __device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i
       }
       break;
     case T_AMPANMDA:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double gA = T.state[1][q] - T.state[0][q];
-        const double gN = T.state[3][q] - T.state[2][q];
-        if (gA != 0.0 || gN != 0.0) {
-          const int slot = T.pp_slot[q];
-          const double g =
-              (gA + T.glob[4] * gN * mgblock(v_g[gv.gpos(slot)], T.glob[5])) * T.param[0][q];
-          atomicAdd(&D[slot], g);
-          atomicAdd(&R[slot], g * T.glob[6]);
+      for (int64_t q0 = i0 + lane; q0 < i1; q0 += 128) {
+        double a[4][4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int64_t q = q0 + 32 * j;
+#pragma unroll
+          for (int c = 0; c < 4; ++c) a[j][c] = q < i1 ? T.state[c][q] : 0.0;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int64_t q = q0 + 32 * j;
+          if (a[j][0] != 0.0 || a[j][1] != 0.0 || a[j][2] != 0.0 || a[j][3] != 0.0) {
+            const double gA = a[j][1] - a[j][0];
+            const double gN = a[j][3] - a[j][2];
+            if (gA != 0.0 || gN != 0.0) {
+              const int slot = T.pp_slot[q];
+              const double g =
+                  (gA + T.glob[4] * gN * mgblock(v_g[gv.gpos(slot)], T.glob[5])) * T.param[0][q];
+              atomicAdd(&D[slot], g);
+              atomicAdd(&R[slot], g * T.glob[6]);
+            }
+#pragma unroll
+            for (int c = 0; c < 4; ++c) T.state[c][q] = decay(a[j][c], T.glob[9 + c]);
+          }
         }
       }
       break;
@@ -402,40 +441,6 @@ __device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, i
       }
       break;
     }
-    default: break;
-  }
-}
-
-__device__ __forceinline__ void state_point(const DTable &T, int64_t i0, int64_t i1, int lane,
-                                            double dt) {
-  switch (T.type) {
-    case T_EXPSYN:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double g = T.state[0][q];
-        if (g != 0.0) T.state[0][q] = cnexp(g, 0.0, T.param[0][q], dt);
-      }
-      break;
-    case T_EXP2SYN:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double A = T.state[0][q], B = T.state[1][q];
-        if (A != 0.0 || B != 0.0) {
-          T.state[0][q] = cnexp(A, 0.0, T.param[0][q], dt);
-          T.state[1][q] = cnexp(B, 0.0, T.param[1][q], dt);
-        }
-      }
-      break;
-    case T_AMPANMDA:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double a0 = T.state[0][q], a1 = T.state[1][q], a2 = T.state[2][q],
-                     a3 = T.state[3][q];
-        if (a0 != 0.0 || a1 != 0.0 || a2 != 0.0 || a3 != 0.0) {
-          T.state[0][q] = cnexp(a0, 0.0, T.glob[0], dt);
-          T.state[1][q] = cnexp(a1, 0.0, T.glob[1], dt);
-          T.state[2][q] = cnexp(a2, 0.0, T.glob[2], dt);
-          T.state[3][q] = cnexp(a3, 0.0, T.glob[3], dt);
-        }
-      }
-      break;
     default: break;
   }
 }
@@ -592,7 +597,8 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
     if (T.n_state == 0 && T.type != T_CADYN) continue;
     if (T.is_point) {
       const int64_t i0 = T.pp_first[g], i1 = T.pp_first[g + 1];
-      if (i1 > i0) state_point(T, i0, i1, lane, dt);
+      (void)i0;  // (point processes were advanced together with their currents, cur_point)
+      (void)i1;
     } else {
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
@@ -784,7 +790,7 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
               const double gs = g * T.param[2][q];
               atomicAdd(rows, gs);
               atomicAdd(rows + 32, gs * T.param[1][q]);
-              g = cnexp(g, 0.0, T.param[0][q], dt);
+              g = decay(g, T.param[0][q]);
             }
           }
           T.state[0][q] = g;
@@ -806,8 +812,8 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
                 atomicAdd(rows, gs);
                 atomicAdd(rows + 32, gs * T.param[2][q]);
               }
-              A = cnexp(A, 0.0, T.param[0][q], dt);
-              B = cnexp(B, 0.0, T.param[1][q], dt);
+              A = decay(A, T.param[0][q]);
+              B = decay(B, T.param[1][q]);
             }
           }
           T.state[0][q] = A;

@@ -733,7 +733,7 @@ __global__ void __launch_bounds__(256) pp_tape_kernel(const __grid_constant__ DM
             const double gs = g * T.param[2][q];
             atomicAdd(&tape[tgt[q]], gs);
             atomicAdd(&tape[tgt[q] + 32], gs * T.param[1][q]);
-            T.state[0][q] = cnexp(g, 0.0, T.param[0][q], dt);
+            T.state[0][q] = decay(g, T.param[0][q]);
           }
         }
         break;
@@ -746,8 +746,8 @@ __global__ void __launch_bounds__(256) pp_tape_kernel(const __grid_constant__ DM
               atomicAdd(&tape[tgt[q]], gs);
               atomicAdd(&tape[tgt[q] + 32], gs * T.param[2][q]);
             }
-            T.state[0][q] = cnexp(A, 0.0, T.param[0][q], dt);
-            T.state[1][q] = cnexp(B, 0.0, T.param[1][q], dt);
+            T.state[0][q] = decay(A, T.param[0][q]);
+            T.state[1][q] = decay(B, T.param[1][q]);
           }
         }
         break;
@@ -768,10 +768,10 @@ __global__ void __launch_bounds__(256) pp_tape_kernel(const __grid_constant__ DM
                 ((a1 - a0) + T.glob[4] * (a3 - a2) * mgblock(v, T.glob[5])) * T.param[0][q];
             atomicAdd(&tape[tgt[q]], gs);
             atomicAdd(&tape[tgt[q] + 32], gs * T.glob[6]);
-            T.state[0][q] = cnexp(a0, 0.0, T.glob[0], dt);
-            T.state[1][q] = cnexp(a1, 0.0, T.glob[1], dt);
-            T.state[2][q] = cnexp(a2, 0.0, T.glob[2], dt);
-            T.state[3][q] = cnexp(a3, 0.0, T.glob[3], dt);
+            T.state[0][q] = decay(a0, T.glob[9]);
+            T.state[1][q] = decay(a1, T.glob[10]);
+            T.state[2][q] = decay(a2, T.glob[11]);
+            T.state[3][q] = decay(a3, T.glob[12]);
           }
         }
         break;
