@@ -68,74 +68,6 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
-// Reciprocal to ~1 ulp without the special-case handling of an IEEE division: MUFU.RCP64H seed
-// plus two Newton steps.  Every argument here is a positive, finite, O(1)..O(1e3) quantity
-// (pivots of a diagonally dominant row-normalised matrix, sums of rate constants).
-__device__ __forceinline__ double rcp_fast(double x) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  return fma(r, e, r);
-}
-
-// exp(x) for |x| < 700 to ~1 ulp without the special-case handling of the library routine:
-// x = n ln2 + r with |r| <= ln2/2 (two-part ln2), Taylor polynomial of degree 13 (truncation
-// 4e-18), scaling by 2^n through the exponent field.  Every argument here is a bounded rate
-// exponent (|x| < 50 for |v| < 500 mV).
-__device__ __forceinline__ double exp_lean(double x) {
-  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);  // round to nearest integer
-  const double nf = t - 6755399441055744.0;
-  double r = fma(nf, -6.93147180369123816490e-01, x);
-  r = fma(nf, -1.90821492927058770002e-10, r);
-  double p = 1.6059043836821613e-10;            // 1/13!
-  p = fma(p, r, 2.08767569878681e-09);          // 1/12!
-  p = fma(p, r, 2.505210838544172e-08);         // 1/11!
-  p = fma(p, r, 2.755731922398589e-07);         // 1/10!
-  p = fma(p, r, 2.7557319223985893e-06);        // 1/9!
-  p = fma(p, r, 2.48015873015873e-05);          // 1/8!
-  p = fma(p, r, 1.984126984126984e-04);         // 1/7!
-  p = fma(p, r, 1.3888888888888889e-03);        // 1/6!
-  p = fma(p, r, 8.333333333333333e-03);         // 1/5!
-  p = fma(p, r, 4.1666666666666664e-02);        // 1/4!
-  p = fma(p, r, 1.6666666666666666e-01);        // 1/3!
-  p = fma(p, r, 0.5);
-  p = fma(p, r, 1.0);
-  p = fma(p, r, 1.0);
-  const int n = __double2loint(t);
-  return p * __hiloint2double((n + 1023) << 20, 0);
-}
-
-// HH gates advanced over dt with cnexp at the new v: y += (1 - exp(-dt*q10*(a+b))) * (a/(a+b) - y).
-// Same formulas as hh_rates() + cnexp(); divisions by constants are multiplications by their
-// reciprocals, 1/tau is never formed, and the three exponentials in v/10 share one evaluation
-// (exp(-(v+40)/10) = exp(-(v+35)/10) e^-0.5, exp(-(v+55)/10) = exp(-(v+35)/10) e^-2): differences
-// of a few ulp in the rates.
-__device__ __forceinline__ void hh_advance(double v, double q10dt, double &m, double &h,
-                                           double &n) {
-  const double x65 = v + 65.0;
-  const double e10 = exp_lean(-(v + 35.0) * 0.1);
-  double al, be, s, u;
-  // m: alpha = 0.1 vtrap(-(v+40), 10), removable singularity as in vtrap()
-  u = -(v + 40.0) * 0.1;
-  al = fabs(u) < 1e-6 ? 1.0 - 0.5 * u : u * rcp_fast(e10 * 0.60653065971263342 - 1.0);
-  be = 4.0 * exp_lean(x65 * (-1.0 / 18.0));
-  s = al + be;
-  m += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - m);
-  // h
-  al = 0.07 * exp_lean(x65 * -0.05);
-  be = rcp_fast(e10 + 1.0);
-  s = al + be;
-  h += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - h);
-  // n: alpha = 0.01 vtrap(-(v+55), 10)
-  u = -(v + 55.0) * 0.1;
-  al = fabs(u) < 1e-6 ? 0.1 * (1.0 - 0.5 * u) : 0.1 * u * rcp_fast(e10 * 0.1353352832366127 - 1.0);
-  be = 0.125 * exp_lean(x65 * -0.0125);
-  s = al + be;
-  n += (1.0 - exp_lean(-q10dt * s)) * (al * rcp_fast(s) - n);
-}
-
 // kernel modes: TM_ADVANCE: the states on the tape still wait for nrn_state of the previous step;
 // TM_FLUSH: apply that update and nothing else; TM_WINDOW: one launch integrates `nsteps` steps,
 // work items (step, group) are handed out by a ticket counter (see the kernel)
