@@ -50,6 +50,18 @@ def workload_config(n_cell):
                     "per dt)"}
 
 
+def aggregate(ms_local, n_node, total_dt, world, dist=None, device="cuda"):
+    """Replicas-only multi-GPU: every rank integrates its own replica of the
+    workload, there is no data-path collective.  The job's time is the MAX over ranks of the
+    device time, the job's throughput the units all ranks processed / that time."""
+    import torch
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if dist is not None and world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    return world * n_node * total_dt / (ms_max * 1e-3), ms_max
+
+
 def m_window_hint(args):
     """Window mode (one launch per <= 40 dt) is what the library picks for this workload unless
     CN_TAPE_WINDOW=0; in per-step mode every 7th launch is sampled instead of every launch."""
@@ -236,12 +248,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     k_ms, k_n = m.get_kernel_timing()
     launches = m.launch_count - launches0
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
     total_dt = DT_PER_STEP * args.steps
-    value = world * n_node * total_dt / (ms_max * 1e-3)
+    value, ms_max = aggregate(ms, n_node, total_dt, world, dist)
     n_spikes = len(m.get_spikes()[0])
     info = m.layout_info()
     m.destroy()
