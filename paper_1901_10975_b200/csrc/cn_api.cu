@@ -180,6 +180,9 @@ struct cn_model {
   int64_t win_stride = 0, win_ninst = 0;  // window mode: doubles per step in win_rows / win_deliv
   int tape_prog_cap = 0, tape_sys_cap = 0, tape_bar_cap = 0;
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
+  double tape_gran = 4.0;  // whole subtrees are cut to at most 1 / (tape_gran * W) of a cell's work
+  double tape_mcost_scale = 0.5, tape_bcost = 1.0;  // cost model of the schedule (units: chain nodes;
+                                                    // swept on config 4, see profiles/r01_README.md)
   bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
   bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
   int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
@@ -511,11 +514,14 @@ static int build_tape_program(cn_model *m, HClass &K) {
       node_mask[x] |= 1u << t;
       if (T.type == CN_CADYN) has_cai[x] = need_ica[x] = 1;
       if (T.type == CN_SK) has_cai[x] = 1;
-      mcost[x] += T.type == CN_HH ? 12.0 : T.type == CN_HHFORM ? 8.0 : T.type == CN_SK ? 6.0 : 1.0;
+      mcost[x] += (T.type == CN_HH ? 12.0 : T.type == CN_HHFORM ? 8.0 : T.type == CN_SK ? 6.0 : 1.0) *
+                  m->tape_mcost_scale;
     }
   }
   for (int x = 0; x < n; ++x)
     if (P.has_pp[x]) ecost[x] += 0.3;
+  for (int x = 0; x < n; ++x)  // a node where contributions meet costs more than a chain node
+    if (ch[x].size() > 1 || node_mask[x]) ecost[x] += m->tape_bcost;
   std::vector<double> sw(ecost), bl(n, 0.0);
   for (int x = n - 1; x >= 1; --x) sw[par[x]] += sw[x];
   for (int x = 0; x < n; ++x) bl[x] = ecost[x] + (x ? bl[par[x]] : 0.0);
@@ -528,7 +534,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
   };
   std::vector<Task> tasks;
   std::vector<int32_t> task_of(n, -1);
-  const double gran = W > 1 ? sw[0] / (4.0 * W) : 1e300;
+  const double gran = W > 1 ? sw[0] / (m->tape_gran * W) : 1e300;
   for (int x = 0; x < n; ++x) {
     if (sw[x] > gran) {  // upper node: a task of its own
       task_of[x] = (int)tasks.size();
@@ -1363,6 +1369,9 @@ static int build_layout(cn_model *m) {
   if (const char *e = std::getenv("CN_TAPE_CH")) m->tape_CH = std::min(63, std::max(7, std::atoi(e)));
   if (const char *e = std::getenv("CN_TAPE_TMEM")) m->tape_tmem = std::atoi(e) != 0;
   if (const char *e = std::getenv("CN_TAPE_LEAF_FIRST")) m->tape_leaf_first = std::atoi(e) != 0;
+  if (const char *e = std::getenv("CN_TAPE_GRAN")) m->tape_gran = std::max(1.0, std::atof(e));
+  if (const char *e = std::getenv("CN_TAPE_MCOST")) m->tape_mcost_scale = std::atof(e);
+  if (const char *e = std::getenv("CN_TAPE_BCOST")) m->tape_bcost = std::atof(e);
   m->cell_tape.assign(nc, 0);
   for (HClass &K : m->cls) {
     K.count = (int64_t)K.cells.size();
