@@ -180,6 +180,7 @@ struct cn_model {
   int64_t win_stride = 0, win_ninst = 0;  // window mode: doubles per step in win_rows / win_deliv
   int tape_prog_cap = 0, tape_sys_cap = 0, tape_bar_cap = 0;
   int tape_W = 8, tape_S = 4, tape_CH = 8;  // warps per group, ring stages, rows per chunk
+  double tape_hcost = 0.0;  // hand-over between warps, in chain nodes
   double tape_gran = 4.0;  // whole subtrees are cut to at most 1 / (tape_gran * W) of a cell's work
   double tape_mcost_scale = 0.5, tape_bcost = 1.0;  // cost model of the schedule (units: chain nodes;
                                                     // swept on config 4, see profiles/r01_README.md)
@@ -530,7 +531,8 @@ static int build_tape_program(cn_model *m, HClass &K) {
   struct Task {
     std::vector<int32_t> nodes;  // in visiting order, top node last
     int ptask = -1, pending = 0, warp = -1;
-    double cost = 0.0, ready = 0.0, prio = 0.0, t0 = 0.0;
+    double cost = 0.0, ready = 0.0, prio = 0.0, t0 = 0.0, t1 = 0.0;
+    std::vector<int> kids;
   };
   std::vector<Task> tasks;
   std::vector<int32_t> task_of(n, -1);
@@ -569,6 +571,16 @@ static int build_tape_program(cn_model *m, HClass &K) {
     T.prio = bl[top];
     T.ptask = top ? task_of[par[top]] : -1;
   }
+  for (int id = 0; id < ntask; ++id)
+    if (tasks[id].ptask >= 0) tasks[tasks[id].ptask].kids.push_back(id);
+  // when a task may start on warp w: all children done, plus a hand-over cost for every child
+  // that ran on another warp (signal, wake-up, contribution through shared memory)
+  const double hcost = m->tape_hcost;
+  auto ready_on = [&](const Task &T, int w) {
+    double r = 0.0;
+    for (int c : T.kids) r = std::max(r, tasks[c].t1 + (tasks[c].warp == w ? 0.0 : hcost));
+    return r;
+  };
   // ---- list scheduling (two passes: the second one knows the mechanism load of each warp) ----
   std::vector<double> mload(W, 0.0), t_end(n, 0.0), mt_end(n, 0.0);
   std::vector<int> e_warp(n, 0), m_warp(n, -1);
@@ -584,7 +596,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
     auto place = [&](int id, int w) {
       Task &T = tasks[id];
       T.warp = w;
-      T.t0 = std::max(wt[w], T.ready);
+      T.t0 = std::max(wt[w], ready_on(T, w));
       double t = T.t0;
       for (int32_t x : T.nodes) {
         t += ecost[x];
@@ -593,6 +605,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
         elist[w].push_back(x);
       }
       wt[w] = t;
+      T.t1 = t;
       last[w] = id;
       if (T.ptask >= 0) {
         tasks[T.ptask].pending--;
@@ -620,7 +633,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
         if (last[w] < 0) return -1;
         const int pt = tasks[last[w]].ptask;
         if (pt >= 0 && tasks[pt].warp < 0 && tasks[pt].pending == 0 &&
-            tasks[pt].ready <= wt[w] + 1e-9)
+            ready_on(tasks[pt], w) <= wt[w] + 1e-9)
           return pt;
         return -1;
       };
@@ -1369,6 +1382,7 @@ static int build_layout(cn_model *m) {
   if (const char *e = std::getenv("CN_TAPE_CH")) m->tape_CH = std::min(63, std::max(7, std::atoi(e)));
   if (const char *e = std::getenv("CN_TAPE_TMEM")) m->tape_tmem = std::atoi(e) != 0;
   if (const char *e = std::getenv("CN_TAPE_LEAF_FIRST")) m->tape_leaf_first = std::atoi(e) != 0;
+  if (const char *e = std::getenv("CN_TAPE_HCOST")) m->tape_hcost = std::atof(e);
   if (const char *e = std::getenv("CN_TAPE_GRAN")) m->tape_gran = std::max(1.0, std::atof(e));
   if (const char *e = std::getenv("CN_TAPE_MCOST")) m->tape_mcost_scale = std::atof(e);
   if (const char *e = std::getenv("CN_TAPE_BCOST")) m->tape_bcost = std::atof(e);
@@ -1396,6 +1410,7 @@ static int build_layout(cn_model *m) {
   lap("classes");
   // chunk size: the default suits plain nodes (three 5-row records); a model whose mechanism
   // records are longer gets chunks of that length (a dry pass over the classes finds out)
+  int min_ch = 7;  // the longest record of any class (a chunk holds whole records)
   if (!std::getenv("CN_TAPE_CH")) {
     int need = 0;
     for (const HClass &K : m->cls) {
@@ -1418,9 +1433,12 @@ static int build_layout(cn_model *m) {
         if (rows[x] || cai[x]) need = std::max(need, 1 + cai[x] + ica[x] + rows[x]);
     }
     if (need > m->tape_CH && need <= 63) m->tape_CH = need;
+    min_ch = std::max(need, 7);
   }
   lap("chunk-length pass");
-  {  // the classes are independent: compile their programs on all host cores
+  std::vector<std::pair<int, int64_t>> saved_groups;
+  for (const HClass &K : m->cls) saved_groups.emplace_back(K.tp.n_groups, K.tp.n_cells);
+  for (;;) {  // the classes are independent: compile their programs on all host cores
     std::vector<int> todo;
     for (int kc = 0; kc < (int)m->cls.size(); ++kc)
       if (m->cls[kc].tp.n_groups > 0) todo.push_back(kc);
@@ -1442,6 +1460,28 @@ static int build_layout(cn_model *m) {
     }
     for (int rc : rcs)
       if (rc != CN_OK) return fail(rc, "internal: compiling a tape program failed");
+    // Two CTAs per SM need 2 x (shared memory + 1 KB) <= 228 KB: if the rings are what is in the
+    // way, shorter chunks (12, 10 rows = 2 plain nodes) cost less than the second CTA is worth.
+    size_t sys_cap = 1, prog_cap = 1, bar_cap = 0;
+    for (const HClass &K : m->cls) {
+      if (K.tp.n_groups == 0) continue;
+      sys_cap = std::max(sys_cap, (size_t)K.tp.n_srow);
+      prog_cap = std::max(prog_cap, K.tp.prog.size());
+      bar_cap = std::max(bar_cap, (size_t)K.tp.n_bar);
+    }
+    const size_t smem = (size_t)m->tape_W * m->tape_S * m->tape_CH * 256 + sys_cap * 512 +
+                        prog_cap * 16 + ((size_t)m->tape_W * m->tape_S + 2 + bar_cap) * 8 + 16;
+    int next_ch = 0;
+    for (int c : {12, 10})
+      if (c < m->tape_CH && c >= min_ch && next_ch == 0) next_ch = c;
+    if (m->tape_W > 8 || std::getenv("CN_TAPE_CH") || 2 * (smem + 1024) <= 233472 || next_ch == 0 ||
+        2 * (smem - (size_t)m->tape_W * m->tape_S * (m->tape_CH - 10) * 256 + 1024) > 233472)
+      break;
+    m->tape_CH = next_ch;
+    for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+      m->cls[kc].tp.n_groups = saved_groups[kc].first;
+      m->cls[kc].tp.n_cells = saved_groups[kc].second;
+    }
   }
   int prog_total = 0;
   for (HClass &K : m->cls) {
