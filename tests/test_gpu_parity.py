@@ -153,6 +153,18 @@ def test_config2_one_ring_of_64(cn, strategy):
     check(o, g, min_spikes=3)
 
 
+def test_config2_full_size(cn):
+    """All four rings of config 2 (256 cells x 601 compartments, HH on every compartment) for
+    30 ms; default strategy for this size (warp-cooperative kernel: a cell with a mechanism on
+    every node keeps its whole system in shared memory)."""
+    desc = W.config2()
+    assert len(desc["parent"]) == 153856
+    o, g = run_both(cn, desc, 30.0)
+    check(o, g, min_spikes=40)
+    for s in (0, 1, 2):
+        assert np.max(np.abs(o.get_state(0, s) - g.get_state(0, s))) < 1e-9
+
+
 def test_config4_small_full_length(cn, strategy):
     desc = W.config4(n_cell=256, n_types=8)
     o, g = run_both(cn, desc, 50.0)
