@@ -115,7 +115,7 @@ struct HTable {
 
 struct HTask {
   int p0 = 0, p1 = 0, b0 = 0, b1 = 0;  // forward / backward records in the class's program
-  int nchunk = 0, tm_base = 0;
+  int nchunk = 0, tm_base = 0, pp0 = 0;  // pp0: ordinal of the warp's first point-process node
   uint32_t row0 = 0, nrows = 0, head = 0;
 };
 
@@ -793,11 +793,6 @@ static int build_tape_program(cn_model *m, HClass &K) {
   }
   // ---- 4. tape rows: each warp's records get consecutive rows, padded so that no record wraps
   // around the warp's ring; system rows in the same order ----------------------------------------
-  P.pp_ord.assign(n, -1);
-  P.n_pp = 0;
-  for (int x = 0; x < n; ++x)
-    if (P.has_pp[x]) P.pp_ord[x] = P.n_pp++;
-  if (P.n_pp > 1023) return give_up();
   P.order.clear();
   P.pos_of.assign(n, 0);
   P.row.assign(n, 0);
@@ -807,11 +802,19 @@ static int build_tape_program(cn_model *m, HClass &K) {
   P.vcopy_row.assign(n, -1);
   P.task.assign(W, HTask());
   P.prog.clear();
-  for (int w = 0; w < W; ++w)
+  // point-process nodes are numbered in the order the warps meet them (window mode prefetches
+  // the rows of the next one while it works on the current one)
+  P.pp_ord.assign(n, -1);
+  P.n_pp = 0;
+  for (int w = 0; w < W; ++w) {
+    P.task[w].pp0 = P.n_pp;
     for (int32_t x : elist[w]) {
       P.pos_of[x] = (int32_t)P.order.size();
       P.order.push_back(x);
+      if (P.has_pp[x]) P.pp_ord[x] = P.n_pp++;
     }
+  }
+  if (P.n_pp > 1023) return give_up();
   // Where (multiplier, reduced rhs) of a node wait for the back-substitution: a node without
   // contributions from mechanisms or from children that do not hand over in registers (its row
   // is written and read by its own warp only) gets a slot of the warp's share of tensor
@@ -1371,7 +1374,12 @@ static int build_layout(cn_model *m) {
   if (const char *e = std::getenv("CN_TAPE_MIN_CELLS")) tape_min_cells = std::atoll(e);
   int tape_min_group = 16;  // a ragged last group needs at least this many cells
   if (const char *e = std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = std::max(1, std::atoi(e));
-  const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells);
+  // A smaller model goes to the interleaved kernel too if ALL of it fits there (then it runs in
+  // window mode: one launch per min-delay window instead of three per dt) and its groups fill at
+  // least a quarter of their lanes; decided after the programs are compiled (below).
+  const bool auto_small = tape_mode == -1 && nc < tape_min_cells && nc > 0;
+  if (auto_small && !std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = 1;
+  const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells) || auto_small;
   // W warps per group (CTA), each with a ring of S chunks x CH rows; the whole CTA must fit the
   // 227 KB of shared memory next to the group's system (512 B per node)
   m->tape_W = 8;
@@ -1503,6 +1511,25 @@ static int build_layout(cn_model *m) {
     m->tape_prog_cap = std::max(m->tape_prog_cap, (int)K.tp.prog.size());
     m->tape_sys_cap = std::max(m->tape_sys_cap, K.tp.n_srow);
     m->tape_bar_cap = std::max(m->tape_bar_cap, K.tp.n_bar);
+  }
+  if (auto_small) {
+    int64_t cells = 0, groups = 0;
+    bool all = true;
+    for (const HClass &K : m->cls) {
+      cells += K.tp.n_cells;
+      groups += K.tp.n_groups;
+      if (K.tp.n_cells < K.count) all = false;
+    }
+    for (const HTable &T : m->tab)
+      if (T.type == CN_AMPANMDA && T.n > 0) all = false;  // (no window mode with these)
+    if (!all || cells * 4 < groups * 32) {  // back to the warp-cooperative kernel, all of it
+      for (HClass &K : m->cls) {
+        K.tp.n_groups = 0;
+        K.tp.n_cells = 0;
+      }
+      std::fill(m->cell_tape.begin(), m->cell_tape.end(), 0);
+      m->tape_prog_cap = m->tape_sys_cap = m->tape_bar_cap = 0;
+    }
   }
 
   lap("tape programs");
@@ -2025,7 +2052,8 @@ static int finalize(cn_model *m, double dt) {
         const HTask &Tk = P.task[w];
         // program positions are relative to the class's program (as it sits in shared memory)
         ttask[kc * (size_t)m->tape_W + w] =
-            TapeTask{Tk.p0, Tk.p1, Tk.b0, Tk.b1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.head, Tk.nrows, 0};
+            TapeTask{Tk.p0, Tk.p1, Tk.b0, Tk.b1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.head, Tk.nrows,
+                     (uint32_t)Tk.pp0};
       }
     }
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
@@ -2116,7 +2144,7 @@ static int finalize(cn_model *m, double dt) {
     H.win_stride = m->win_stride;
     H.win_ninst = m->win_ninst;
     if (ok) {
-      rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_stride * wn, 1), &H.win_rows);
+      rc = dev_alloc(m, (size_t)(m->win_stride * wn + 128), &H.win_rows);  // (+ prefetch overrun)
       if (rc != CN_OK) return rc;
       rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_ninst * wn, 1), &H.win_deliv);
       if (rc != CN_OK) return rc;

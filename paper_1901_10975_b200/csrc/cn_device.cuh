@@ -77,7 +77,7 @@ struct TapeTask {
   int32_t p0, p1, b0, b1;
   int32_t nchunk, tm_base;  // tm_base: first tensor-memory slot of the warp
   uint32_t row0, head;
-  uint32_t nrows, pad0;     // rows of the segment
+  uint32_t nrows, pp0;      // rows of the segment; ordinal of the warp's first point-process node
 };
 
 // Program record (uint4) of the interleaved kernel: one per run of plain chain nodes (RUN), per

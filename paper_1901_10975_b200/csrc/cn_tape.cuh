@@ -369,6 +369,15 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     // triangularisation, children before parents
     // ========================================================================================
     double accD = 0.0, accR = 0.0;
+    // window mode: conductance / current rows of the warp's next point-process node, requested one
+    // such node ahead (they sit in an L2-resident buffer, not on the tape)
+    const double *wrow = M.win_rows + (size_t)step_in * M.win_stride + tg.pp_base +
+                         (size_t)tk.pp0 * 64u + lane;
+    double ppd = 0.0, ppr = 0.0;
+    if (window && !flush) {
+      ppd = __ldcg(wrow);
+      ppr = __ldcg(wrow + 32);
+    }
     for (int j = p0; j < p1; ++j) {
       const uint4 e = prog[j];
       const uint32_t ty = e.y & RT_MASK;
@@ -449,11 +458,12 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           R += srow[32];
         }
         if (fl & RF_HAS_PP) {  // conductance / current of the point processes
-          if (window) {  // (pp_window_kernel: this step's block of win_rows; z bits 21..30 = the
-            const double *wr = M.win_rows + (size_t)step_in * M.win_stride + tg.pp_base +
-                               ((e.z >> 21) & 1023u) * 64u + lane;  // node's ordinal in the class)
-            D += wr[0];
-            R += wr[32];
+          if (window) {  // (pp_window_kernel: this step's block of win_rows, prefetched)
+            D += ppd;
+            R += ppr;
+            wrow += 64;
+            ppd = __ldcg(wrow);
+            ppr = __ldcg(wrow + 32);
           } else {  // (pp_tape_kernel: the two dynamic rows of the record, cleared after use)
             const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
             D += pd;

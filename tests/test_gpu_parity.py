@@ -128,11 +128,19 @@ def test_config3_shape(cn, strategy):
 
 def test_config3_full_size_first_wave(cn):
     """All 3,560 cells / 465,740 compartments / 1.1 M Exp2Syn for 12 ms (the first population
-    wave); default strategy for this size (warp-cooperative kernel)."""
+    wave), default strategy (every cell on the interleaved kernel): once with per-step probes
+    (one launch per dt), once without (window mode, final state only)."""
+    from oracle import OracleModel
     desc = W.config3()
     assert len(desc["parent"]) == 465740 and len(desc["netcons"]["src"]) == 1100040
     o, g = run_both(cn, desc, 12.0)
+    assert g.layout_info()["n_tape_group"] == g.layout_info()["n_group"] > 100
     check(o, g, min_spikes=1000)
+    w = cn.Model(desc)
+    w.run(12.0, DT)
+    assert w.launch_count < 100
+    assert np.max(np.abs(o.get_v() - w.get_v())) <= TOL
+    assert [list(x) for x in w.get_spikes()] == [list(x) for x in o.get_spikes()]
 
 
 def test_config5_shape(cn, strategy):
@@ -268,6 +276,7 @@ def test_node_renumbering_invariance(cn, strategy):
 
 @pytest.mark.parametrize("force_g", ["1", "2", "8"])
 def test_lanes_per_cell_variants(cn, force_g, monkeypatch):
+    monkeypatch.setenv("CN_TAPE", "0")       # the warp-cooperative kernel, G cells per warp
     monkeypatch.setenv("CN_FORCE_G", force_g)
     desc = W.config4(n_cell=64, n_types=2)
     o, g = run_both(cn, desc, 30.0)
