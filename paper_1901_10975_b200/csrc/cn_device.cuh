@@ -212,12 +212,6 @@ __device__ __forceinline__ double exp_lean(double x) {
 }
 
 
-__device__ __forceinline__ double vtrap(double x, double y) {
-  double u = x / y;
-  if (fabs(u) < 1e-6) return y * (1.0 - u / 2.0);
-  return x / (exp(u) - 1.0);
-}
-
 __device__ __forceinline__ double cnexp(double y, double yinf, double tau, double dt) {
   return y + (1.0 - exp_lean(-dt * rcp_fast(tau))) * (yinf - y);
 }
@@ -226,29 +220,8 @@ __device__ __forceinline__ double cnexp(double y, double yinf, double tau, doubl
 // ExpSyn / Exp2Syn, per table for AMPA+NMDA): the same expression as cnexp(y, 0, tau, dt)
 __device__ __forceinline__ double decay(double y, double c) { return y + c * (0.0 - y); }
 
-__device__ __forceinline__ void hh_rates(double v, double q10, double &minf, double &mtau,
-                                         double &hinf, double &htau, double &ninf,
-                                         double &ntau) {
-  double al, be, s;
-  al = 0.1 * vtrap(-(v + 40.0), 10.0);
-  be = 4.0 * exp(-(v + 65.0) / 18.0);
-  s = al + be;
-  minf = al / s;
-  mtau = 1.0 / (q10 * s);
-  al = 0.07 * exp(-(v + 65.0) / 20.0);
-  be = 1.0 / (exp(-(v + 35.0) / 10.0) + 1.0);
-  s = al + be;
-  hinf = al / s;
-  htau = 1.0 / (q10 * s);
-  al = 0.01 * vtrap(-(v + 55.0), 10.0);
-  be = 0.125 * exp(-(v + 65.0) / 80.0);
-  s = al + be;
-  ninf = al / s;
-  ntau = 1.0 / (q10 * s);
-}
-
 // HH gates advanced over dt with cnexp at the new v: y += (1 - exp(-dt*q10*(a+b))) * (a/(a+b) - y).
-// Same formulas as hh_rates() + cnexp(); divisions by constants are multiplications by their
+// The textbook rate functions + cnexp; divisions by constants are multiplications by their
 // reciprocals, 1/tau is never formed, and the three exponentials in v/10 share one evaluation
 // (exp(-(v+40)/10) = exp(-(v+35)/10) e^-0.5, exp(-(v+55)/10) = exp(-(v+35)/10) e^-2): differences
 // of a few ulp in the rates.
@@ -257,7 +230,8 @@ __device__ __forceinline__ void hh_advance(double v, double q10dt, double &m, do
   const double x65 = v + 65.0;
   const double e10 = exp_lean(-(v + 35.0) * 0.1);
   double al, be, s, u;
-  // m: alpha = 0.1 vtrap(-(v+40), 10), removable singularity as in vtrap()
+  // m: alpha = 0.1 vtrap(-(v+40), 10) with vtrap(x, y) = x / (exp(x/y) - 1); removable
+  // singularity: y (1 - x/(2y)) for |x/y| < 1e-6
   u = -(v + 40.0) * 0.1;
   al = fabs(u) < 1e-6 ? 1.0 - 0.5 * u : u * rcp_fast(e10 * 0.60653065971263342 - 1.0);
   be = 4.0 * exp_lean(x65 * (-1.0 / 18.0));

@@ -35,7 +35,7 @@ def test_create_and_initial_v_without_device():
     g, s = m.get_spikes()
     assert len(g) == 0
     info = m.layout_info()
-    assert info["n_class"] == 1 and info["n_group"] >= 2
+    assert info["n_class"] == 1 and info["n_group"] >= 1
 
 
 def test_shape_classes_found_in_shuffled_cells():
