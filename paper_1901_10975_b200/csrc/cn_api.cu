@@ -1673,7 +1673,11 @@ static int build_layout(cn_model *m) {
         const int32_t local = (int32_t)(T.node[i] - m->cell_first[cell]);
         if (g < ngc) {
           const int G = m->cls[m->grp[g].cls].G;
-          T.pp_slot[pos] = (int32_t)(local * G + m->cell_slot[cell]);
+          // element of the node's row pair in ppdr (schedule order, rows of 32 + 32)
+          const int64_t sp = m->grp[g].ab_base + m->cls[m->grp[g].cls].node_off[local] +
+                             m->cell_slot[cell];
+          (void)G;
+          T.pp_slot[pos] = (int32_t)(uint32_t)((sp >> 5) * 64 + (sp & 31));
         } else {
           const TapeGroup &tg = m->tgrp[g - ngc];
           const int64_t el = tg.tape_base + (int64_t)m->cls[tg.cls].tp.pp_row[local] * 32 +
@@ -1933,7 +1937,25 @@ static int finalize(cn_model *m, double dt) {
     H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
     int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
     double *p;
+    // nodes of warp-cooperative cells that carry point processes: negative static diagonal
+    for (const HTable &T : m->tab)
+      if (T.ti.point)
+        for (int64_t i = 0; i < T.n; ++i)
+          if (!m->cell_tape[cell_of_node[T.node[i]]]) {
+            double &d = dstat[m->node_pos[T.node[i]]];
+            d = -std::fabs(d);
+          }
     UP(dstat, p); H.dstat = p;
+    H.ppdr = nullptr;
+    {  // point processes on warp-cooperative groups: their conductance / current rows
+      bool any = false;
+      for (const HTable &T : m->tab)
+        if (T.ti.point && T.pp_tape_begin > 0) any = true;
+      if (any) {
+        rc = dev_alloc(m, (size_t)(2 * m->n_pnode + 64), &H.ppdr);
+        if (rc != CN_OK) return rc;
+      }
+    }
     UP(rstat, p); H.rstat = p;
     UP(a_s, p); H.a_s = p;
     UP(b_s, p); H.b_s = p;
@@ -2255,6 +2277,10 @@ static int run_steps(cn_model *m, int64_t K) {
   for (const HTable &T : m->tab)
     if (T.ti.point) pp_tape = std::max(pp_tape, T.n - T.pp_tape_begin);
   const int pp_blocks = (int)std::min<int64_t>((pp_tape + 255) / 256, 148 * 8);
+  int64_t pp_coop = 0;
+  for (const HTable &T : m->tab)
+    if (T.ti.point) pp_coop = std::max(pp_coop, T.pp_tape_begin);
+  const int ppc_blocks = (int)std::min<int64_t>((pp_coop + 255) / 256, 148 * 16);
   CU(cudaEventRecord(m->ev0, m->stream));
   if (m->window) {
     // one launch of the interleaved kernel per window of up to win_steps steps; the events and
@@ -2304,7 +2330,11 @@ static int run_steps(cn_model *m, int64_t K) {
       m->launches++;
     }
     if (ntg > 0 && pp_tape > 0) {
-      pp_tape_kernel<<<pp_blocks, 256, 0, m->stream>>>(m->hm, k);
+      pp_step_kernel<false><<<pp_blocks, 256, 0, m->stream>>>(m->hm, k);
+      m->launches++;
+    }
+    if (ng > 0 && pp_coop > 0) {
+      pp_step_kernel<true><<<ppc_blocks, 256, 0, m->stream>>>(m->hm, k);
       m->launches++;
     }
     const bool timeit = m->ktime_every > 0 && (k % m->ktime_every) == 0 &&

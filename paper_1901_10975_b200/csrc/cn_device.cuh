@@ -134,6 +134,8 @@ struct DModel {
   const int32_t *node_off;      // per class: slot offset (round*32 + p*G) of every local node
   double *v;                    // [n_slot] schedule order, padded
   const double *dstat, *rstat;  // static diagonal / rhs parts (row-normalised), schedule order
+  double *ppdr;                 // point-process conductance / current of this dt, schedule order,
+                                // rows of 32 + 32 doubles: slot s -> (s/32)*64 + s%32 (+32: current)
   const double *a_s, *b_s;      // off-diagonals, schedule order
   double *cai;                  // per node (only when a table needs it) else null
   const double *thr;            // [n_pcell]
@@ -339,90 +341,6 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
   }
 }
 
-// Point-process table: instances of this group, arbitrary nodes -> shared-memory atomics.  The
-// states of these types do not depend on v, so their nrn_state (decay over dt) is applied in the
-// same pass, right after the current is taken (one read and one write of every state per dt);
-// four instances per lane are in flight at a time.
-__device__ __forceinline__ void cur_point(const DTable &T, int64_t i0, int64_t i1, double *D,
-                                          double *R, const GroupView &gv, const double *v_g,
-                                          int lane, double t_mid) {
-  switch (T.type) {
-    case T_EXPSYN:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double s0 = T.state[0][q];
-        if (s0 != 0.0) {
-          const double g = s0 * T.param[2][q];  // param[2] = 100/area/c
-          const int slot = T.pp_slot[q];
-          atomicAdd(&D[slot], g);
-          atomicAdd(&R[slot], g * T.param[1][q]);
-          T.state[0][q] = decay(s0, T.param[0][q]);
-        }
-      }
-      break;
-    case T_EXP2SYN:
-      for (int64_t q0 = i0 + lane; q0 < i1; q0 += 128) {
-        double A[4], B[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int64_t q = q0 + 32 * j;
-          A[j] = q < i1 ? T.state[0][q] : 0.0;
-          B[j] = q < i1 ? T.state[1][q] : 0.0;
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int64_t q = q0 + 32 * j;
-          if (A[j] != 0.0 || B[j] != 0.0) {
-            const double g = (B[j] - A[j]) * T.param[3][q];
-            if (g != 0.0) {
-              const int slot = T.pp_slot[q];
-              atomicAdd(&D[slot], g);
-              atomicAdd(&R[slot], g * T.param[2][q]);
-            }
-            T.state[0][q] = decay(A[j], T.param[0][q]);
-            T.state[1][q] = decay(B[j], T.param[1][q]);
-          }
-        }
-      }
-      break;
-    case T_ICLAMP:
-      for (int64_t q = i0 + lane; q < i1; q += 32) {
-        const double del = T.param[0][q];
-        if (t_mid >= del && t_mid < del + T.param[1][q])
-          atomicAdd(&R[T.pp_slot[q]], T.param[2][q] * T.param[3][q]);
-      }
-      break;
-    case T_AMPANMDA:
-      for (int64_t q0 = i0 + lane; q0 < i1; q0 += 128) {
-        double a[4][4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int64_t q = q0 + 32 * j;
-#pragma unroll
-          for (int c = 0; c < 4; ++c) a[j][c] = q < i1 ? T.state[c][q] : 0.0;
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int64_t q = q0 + 32 * j;
-          if (a[j][0] != 0.0 || a[j][1] != 0.0 || a[j][2] != 0.0 || a[j][3] != 0.0) {
-            const double gA = a[j][1] - a[j][0];
-            const double gN = a[j][3] - a[j][2];
-            if (gA != 0.0 || gN != 0.0) {
-              const int slot = T.pp_slot[q];
-              const double g =
-                  (gA + T.glob[4] * gN * mgblock(v_g[gv.gpos(slot)], T.glob[5])) * T.param[0][q];
-              atomicAdd(&D[slot], g);
-              atomicAdd(&R[slot], g * T.glob[6]);
-            }
-#pragma unroll
-            for (int c = 0; c < 4; ++c) T.state[c][q] = decay(a[j][c], T.glob[9 + c]);
-          }
-        }
-      }
-      break;
-    default: break;
-  }
-}
-
 // ------------------------------------------------------------------------------------------
 // nrn_state with the new v (in R)
 // ------------------------------------------------------------------------------------------
@@ -512,7 +430,6 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   double *I = R + nG;  // only valid when ci.needs_ica
   const int64_t ab = gi.ab_base;
   const double dt = M.dt;
-  const double t_mid = ((double)k + 0.5) * dt;
   const int c = lane & (G - 1), p = lane >> lgG;
   const int P = 32 >> lgG;
   const int rounds = ci.rounds;
@@ -529,6 +446,20 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   const double *__restrict__ dss = M.dstat + ab + lane;
   const double *__restrict__ rss = M.rstat + ab + lane;
   double *__restrict__ vs = M.v + ab + lane;
+  double *__restrict__ pps = M.ppdr + 2 * ab + lane;  // point processes: pp_coop_kernel put the
+  const bool has_pp = M.ppdr != nullptr;              // conductance / current of this dt here
+  // (a node that carries point processes is marked by a NEGATIVE static diagonal, which is > 0)
+  auto take_pp = [&](int r, double &d, double &rr) {  // add them to (d, r) of round r and clear
+    if (!has_pp || d > 0.0) return;
+    d = -d;
+    const double pd = pps[(size_t)r * 64], pr = pps[(size_t)r * 64 + 32];
+    if (pd != 0.0 || pr != 0.0) {
+      d += pd;
+      rr += pr;
+      pps[(size_t)r * 64] = 0.0;
+      pps[(size_t)r * 64 + 32] = 0.0;
+    }
+  };
 
   // issue the first CN_PF rounds of loads and the root's terms before anything else
   uint32_t e_[CN_PF];
@@ -544,6 +475,7 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
         b_[u] = bs[(size_t)u * 32];
         d_[u] = dss[(size_t)u * 32];
         r_[u] = vs[(size_t)u * 32] + rss[(size_t)u * 32];
+        take_pp(u, d_[u], r_[u]);
       }
     }
   }
@@ -551,6 +483,7 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   if (p == 0) {
     d_root = dss[(size_t)rounds * 32];
     r_root = vs[(size_t)rounds * 32] + rss[(size_t)rounds * 32];
+    take_pp(rounds, d_root, r_root);
   }
 
   // ---- zero the system -------------------------------------------------------------------
@@ -565,13 +498,7 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   // ---- nrn_cur -------------------------------------------------------------------------
   for (int t = 0; t < M.n_table; ++t) {
     const DTable &T = M.tab[t];
-    if (T.is_point) {
-      const int64_t i0 = T.pp_first[g], i1 = T.pp_first[g + 1];
-      if (i1 > i0) {
-        cur_point(T, i0, i1, D, R, gv, M.v, lane, t_mid);
-        __syncwarp();
-      }
-    } else {
+    if (!T.is_point) {  // (point processes: pp_coop_kernel, one thread per instance)
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
         cur_distributed(T, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls], D,
@@ -608,6 +535,7 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
             b_[u] = bs[(size_t)rn * 32];
             d_[u] = dss[(size_t)rn * 32];
             r_[u] = vs[(size_t)rn * 32] + rss[(size_t)rn * 32];
+            take_pp(rn, d_[u], r_[u]);
           }
         }
       }
@@ -640,11 +568,7 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   for (int t = 0; t < M.n_table; ++t) {
     const DTable &T = M.tab[t];
     if (T.n_state == 0 && T.type != T_CADYN) continue;
-    if (T.is_point) {
-      const int64_t i0 = T.pp_first[g], i1 = T.pp_first[g + 1];
-      (void)i0;  // (point processes were advanced together with their currents, cur_point)
-      (void)i1;
-    } else {
+    if (!T.is_point) {
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
         state_distributed(T, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls],
@@ -763,7 +687,7 @@ __global__ void __launch_bounds__(128) deliver_kernel(const __grid_constant__ DM
 // before it).  deliver_window_kernel sums the weights per (step, instance); pp_window_kernel then
 // advances every point process through the window and leaves its conductance / current of every
 // step in win_rows, where the interleaved kernel picks them up.  Same arithmetic per step as
-// deliver_kernel + pp_tape_kernel (types whose current depends on v cannot run in this mode).
+// deliver_kernel + pp_step_kernel (types whose current depends on v cannot run in this mode).
 // ------------------------------------------------------------------------------------------
 
 __global__ void __launch_bounds__(128) deliver_window_kernel(const __grid_constant__ DModel M,

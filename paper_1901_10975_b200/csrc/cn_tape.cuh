@@ -23,7 +23,7 @@
 //     and the old states), but the states are read and written once per step and the
 //     back-substitution carries no mechanism work.  cn_get_state runs the pending update first.
 //   * Control is uniform across a warp; lanes never diverge.
-// Point processes of these cells are evaluated by pp_tape_kernel (one thread per instance) which
+// Point processes of these cells are evaluated by pp_step_kernel (one thread per instance) which
 // adds conductance and current into the two dynamic rows of the node (L60, L65).
 #pragma once
 #include "cn_device.cuh"
@@ -464,7 +464,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
             wrow += 64;
             ppd = __ldcg(wrow);
             ppr = __ldcg(wrow + 32);
-          } else {  // (pp_tape_kernel: the two dynamic rows of the record, cleared after use)
+          } else {  // (pp_step_kernel: the two dynamic rows of the record, cleared after use)
             const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
             D += pd;
             R += pr;
@@ -652,24 +652,27 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
 }
 
 // ------------------------------------------------------------------------------------------------
-// point processes on tape cells: current + conductance into the node's dynamic rows, then the
-// state decay (independent of v for these types, so cur and state fuse exactly; L65, L67)
+// point processes, one thread per instance: current + conductance into the node's dynamic rows,
+// then the state decay (independent of v for these types, so cur and state fuse exactly; L65, L67)
 // ------------------------------------------------------------------------------------------------
 
-__global__ void __launch_bounds__(256) pp_tape_kernel(const __grid_constant__ DModel M,
+template <bool COOP>
+__global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DModel M,
                                                       int64_t k) {
   const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t nth = (int64_t)gridDim.x * blockDim.x;
   const double dt = M.dt;
   const double t_mid = ((double)k + 0.5) * dt;
-  double *__restrict__ tape = M.tape;
+  // targets: the node's conductance row on its group's tape (current row: + 32), or, for the
+  // warp-cooperative groups (COOP, instances [0, pp_tape_begin)), its row pair in M.ppdr
+  double *__restrict__ tape = COOP ? M.ppdr : M.tape;
   for (int t = 0; t < M.n_table; ++t) {
     const DTable &T = M.tab[t];
     if (!T.is_point) continue;
     const uint32_t *__restrict__ tgt = reinterpret_cast<const uint32_t *>(T.pp_slot);
     switch (T.type) {
       case T_EXPSYN:
-        for (int64_t q = T.pp_tape_begin + tid; q < T.pp_tape_end; q += nth) {
+        for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
           const double g = T.state[0][q];
           if (g != 0.0) {
             const double gs = g * T.param[2][q];
@@ -680,7 +683,7 @@ __global__ void __launch_bounds__(256) pp_tape_kernel(const __grid_constant__ DM
         }
         break;
       case T_EXP2SYN:
-        for (int64_t q = T.pp_tape_begin + tid; q < T.pp_tape_end; q += nth) {
+        for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
           const double A = T.state[0][q], B = T.state[1][q];
           if (A != 0.0 || B != 0.0) {
             const double gs = (B - A) * T.param[3][q];
@@ -694,18 +697,19 @@ __global__ void __launch_bounds__(256) pp_tape_kernel(const __grid_constant__ DM
         }
         break;
       case T_ICLAMP:
-        for (int64_t q = T.pp_tape_begin + tid; q < T.pp_tape_end; q += nth) {
+        for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
           const double del = T.param[0][q];
           if (t_mid >= del && t_mid < del + T.param[1][q])
             atomicAdd(&tape[tgt[q] + 32], T.param[2][q] * T.param[3][q]);
         }
         break;
       case T_AMPANMDA:
-        for (int64_t q = T.pp_tape_begin + tid; q < T.pp_tape_end; q += nth) {
+        for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
           const double a0 = T.state[0][q], a1 = T.state[1][q], a2 = T.state[2][q],
                        a3 = T.state[3][q];
           if (a0 != 0.0 || a1 != 0.0 || a2 != 0.0 || a3 != 0.0) {
-            const double v = tape[tgt[q] - 32];  // the v row precedes the two dynamic rows
+            // v of the node: on the tape the v row precedes the two dynamic rows
+            const double v = COOP ? M.v[(size_t)(tgt[q] >> 6) * 32 + (tgt[q] & 31u)] : tape[tgt[q] - 32];
             const double gs =
                 ((a1 - a0) + T.glob[4] * (a3 - a2) * mgblock(v, T.glob[5])) * T.param[0][q];
             atomicAdd(&tape[tgt[q]], gs);
