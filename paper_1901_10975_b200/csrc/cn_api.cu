@@ -223,8 +223,24 @@ struct cn_model {
   int64_t *d_sp_step = nullptr;
 };
 
+// std::vector that does not value-initialise (large set-up arrays are filled by all host cores)
 template <class T>
-static int dev_upload(cn_model *m, const std::vector<T> &h, T **out, size_t min_elems = 1) {
+struct NoInitAlloc {
+  using value_type = T;
+  NoInitAlloc() = default;
+  template <class U> NoInitAlloc(const NoInitAlloc<U> &) {}
+  T *allocate(size_t n) { return static_cast<T *>(::operator new(n * sizeof(T))); }
+  void deallocate(T *p, size_t) { ::operator delete(p); }
+  template <class U, class... A> void construct(U *p, A &&...a) {
+    if constexpr (sizeof...(A) == 0) ::new ((void *)p) U; else ::new ((void *)p) U(std::forward<A>(a)...);
+  }
+  template <class U> bool operator==(const NoInitAlloc<U> &) const { return true; }
+  template <class U> bool operator!=(const NoInitAlloc<U> &) const { return false; }
+};
+template <class T> using uvec = std::vector<T, NoInitAlloc<T>>;
+
+template <class T, class A>
+static int dev_upload(cn_model *m, const std::vector<T, A> &h, T **out, size_t min_elems = 1) {
   size_t n = std::max(h.size(), min_elems);
   void *p = nullptr;
   CU(cudaMalloc(&p, n * sizeof(T)));
@@ -1784,13 +1800,21 @@ static int finalize(cn_model *m, double dt) {
   if (m->n_netcon == 0) mind = 1;
   // row-normalised static arrays:  c_i = 1e-3 cm_i/dt,  b' = b/c_i,  a' = a/c_parent,
   // dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
-  std::vector<double> invc((size_t)N), bn((size_t)N, 0.0), an((size_t)N, 0.0);
+  uvec<double> invc((size_t)N), bn((size_t)N), an((size_t)N);
   std::vector<double> dstat((size_t)m->n_pnode, 1.0), rstat((size_t)m->n_pnode, 0.0);
   // one arena: [schedule-ordered v of the cooperative groups | tapes of the interleaved groups]
-  std::vector<double> v0((size_t)(m->n_ab + m->n_tape), 0.0);
+  uvec<double> v0((size_t)(m->n_ab + m->n_tape));
   double *tape = v0.data() + m->n_ab;
-  std::vector<double> dsum((size_t)N), rsum((size_t)N, 0.0);
-  std::vector<int32_t> cell_of_node((size_t)N);
+  uvec<double> dsum((size_t)N), rsum((size_t)N);
+  uvec<int32_t> cell_of_node((size_t)N);
+  par_for((int64_t)v0.size(), 1 << 20, [&](int64_t i0, int64_t i1) {
+    std::fill(v0.begin() + i0, v0.begin() + i1, 0.0);
+  });
+  par_for(N, 1 << 20, [&](int64_t i0, int64_t i1) {
+    std::fill(bn.begin() + i0, bn.begin() + i1, 0.0);
+    std::fill(an.begin() + i0, an.begin() + i1, 0.0);
+    std::fill(rsum.begin() + i0, rsum.begin() + i1, 0.0);
+  });
   // cells are independent (a parent sits in the same cell): all host cores
   par_for(m->n_cell, 256, [&](int64_t c0, int64_t c1) {
     const int64_t i0 = m->cell_first[c0], i1 = m->cell_first[c1];
