@@ -9,6 +9,7 @@ HERE = Path(__file__).resolve().parent
 SO = HERE / "libcn.so"
 SRCS = [HERE / "csrc" / "cn_api.cu"]
 DEPS = SRCS + [HERE / "csrc" / "cn_device.cuh", HERE / "csrc" / "cn_tape.cuh",
+               HERE / "csrc" / "cn_tape_program.hpp",
                HERE.parent / "include" / "cn.h"]
 
 NVCC_FLAGS = (["-DCN_TRACE"] if os.environ.get("CN_TRACE") else []) + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
