@@ -1394,7 +1394,7 @@ static int finalize(cn_model *m, double dt) {
       if (T.type == CN_AMPANMDA && T.n > 0) ok = false;
     if (const char *e = std::getenv("CN_TAPE_WINDOW")) ok = ok && std::atoi(e) != 0;
     int64_t wn = m->n_netcon > 0 ? std::min<int64_t>(H.mind, 64) : 32;
-    if (wn < 2 || (H.maxd + wn - 1) / wn + 2 > 60) ok = false;
+    if (wn < 2) ok = false;
     if (ok && (m->win_stride + m->win_ninst) * wn * 8 > ((int64_t)4 << 30)) ok = false;
     m->window = ok;
     m->win_steps = (int)wn;
@@ -1407,8 +1407,9 @@ static int finalize(cn_model *m, double dt) {
       if (rc != CN_OK) return rc;
       rc = dev_alloc(m, (size_t)m->hm.n_tgroup, &H.win_done); if (rc != CN_OK) return rc;
       rc = dev_alloc(m, 1, &H.win_ticket); if (rc != CN_OK) return rc;
-      rc = dev_alloc(m, 64, &H.win_mark_step); if (rc != CN_OK) return rc;
-      rc = dev_alloc(m, 64, &H.win_mark_nsp); if (rc != CN_OK) return rc;
+      H.win_mark_cap = H.maxd + 64;
+      rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_step); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_nsp); if (rc != CN_OK) return rc;
     }
   }
   // spikes

@@ -164,7 +164,8 @@ struct DModel {
   int64_t win_stride, win_ninst;
   int32_t *win_done;            // [n_tgroup]: steps of the window completed for the group
   uint32_t *win_ticket;         // next (step, group) work item
-  int64_t *win_mark_step;       // ring [64]: first step of the recent windows
+  int64_t win_mark_cap;         // length of the two rings below
+  int64_t *win_mark_step;       // ring: first step of the recent windows
   int64_t *win_mark_nsp;        //            and the length of the spike list at their start
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
@@ -701,14 +702,15 @@ __global__ void __launch_bounds__(128) deliver_window_kernel(const __grid_consta
   // at or after that step (the spike list is ordered by window, not by step)
   int64_t i_lo = (int64_t)ns;
   int64_t end_step = k0;  // first step after window j
-  for (int64_t j = widx - 1; j >= 0 && j > widx - 63; --j) {
+  // (the ring of window marks holds maxd + 64 windows: enough even if every window is one step)
+  for (int64_t j = widx - 1; j >= 0 && j > widx - M.win_mark_cap + 1; --j) {
     if (end_step < k0 - M.maxd) break;
-    i_lo = M.win_mark_nsp[j & 63];
-    end_step = M.win_mark_step[j & 63];
+    i_lo = M.win_mark_nsp[j % M.win_mark_cap];
+    end_step = M.win_mark_step[j % M.win_mark_cap];
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
-    M.win_mark_step[widx & 63] = k0;
-    M.win_mark_nsp[widx & 63] = (int64_t)ns;
+    M.win_mark_step[widx % M.win_mark_cap] = k0;
+    M.win_mark_nsp[widx % M.win_mark_cap] = (int64_t)ns;
   }
   auto deliver = [&](int32_t gid, int64_t step) {
     const int64_t lo = M.src_first[gid], hi = M.src_first[gid + 1];

@@ -349,3 +349,23 @@ def test_window_mode_matches_oracle(cn, which, monkeypatch):
     for t, m in enumerate(desc["mechs"]):
         if m["type"] in ("hh", "expsyn", "exp2syn", "sk"):
             assert np.max(np.abs(o.get_state(t, 0) - g.get_state(t, 0))) < 1e-9, m["type"]
+
+
+def test_window_mode_one_step_per_call(cn, monkeypatch):
+    """cn_run called once per dt for 300 steps with delays of up to 200 steps: every window is one
+    step long, the events of spikes recorded 200 windows ago must still be found."""
+    from oracle import OracleModel
+    monkeypatch.setenv("CN_TAPE", "1")
+    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+    desc = W.config3(n_cell=28, syn_per_cell=40)
+    assert np.round(desc["netcons"]["delay"].max() / DT) == 200
+    o = OracleModel(desc)
+    g = cn.Model(desc)
+    for k in range(1, 701):
+        g.run(k * DT, DT)
+    o.run(700 * DT, DT)
+    assert g.launch_count <= 3 * 700 + 8
+    assert np.max(np.abs(o.get_v() - g.get_v())) <= TOL
+    og, os_ = o.get_spikes()
+    gg, gs = g.get_spikes()
+    assert len(og) >= 20 and list(og) == list(gg) and list(os_) == list(gs)
