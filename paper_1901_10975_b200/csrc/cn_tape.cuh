@@ -6,10 +6,13 @@
 //     static rhs, v (+ two dynamic rows for point processes); per node with distributed
 //     mechanisms a second record with a copy of v and the parameter / state rows.  The kernel
 //     never computes an address from the tree: it reads the tape front to back.
-//   * One CTA (W warps) owns one group at a time and loops over groups (persistent).  The linear
-//     system of the group lives in SHARED MEMORY for the whole step: triangularisation (L66)
-//     leaves (multiplier, reduced rhs) of every node there, back-substitution reads them back.
-//     Nothing but the tape is read from HBM and nothing but v and the states is written.
+//   * One CTA (W = 8 warps) owns one group at a time and takes groups until none is left
+//     (persistent).  The linear system of the group stays ON CHIP for the whole step:
+//     triangularisation (L66) leaves (multiplier, reduced rhs) of every node there,
+//     back-substitution reads them back.  Rows that only their own warp touches live in TENSOR
+//     MEMORY (tcgen05.st / tcgen05.ld, a per-lane scratchpad), rows where several warps meet in
+//     shared memory; that leaves room for two CTAs per SM.  Nothing but the tape is read from HBM
+//     and nothing but v and the states is written.
 //   * The tree is compiled by the host into W record lists (a static schedule of the elimination
 //     over W warps, children before parents, L196).  A chain hands its contribution to the parent
 //     in REGISTERS; at a branch point the contributions meet in the parent's system row.  Warps
@@ -22,9 +25,14 @@
 //     just before nrn_cur (L65) needs the states: same arithmetic on the same values (the new v
 //     and the old states), but the states are read and written once per step and the
 //     back-substitution carries no mechanism work.  cn_get_state runs the pending update first.
+//   * One launch integrates a WINDOW of up to min-delay steps (L62): (step, group) work items are
+//     handed out by a ticket counter, a group's next step may run on another SM once the previous
+//     one is published (release / acquire through L2).  Events and point processes of the window
+//     are prepared by deliver_window_kernel / pp_window_kernel (cn_device.cuh); with per-step
+//     probes or cells on the other kernel: one launch per dt, pp_step_kernel in front.
 //   * Control is uniform across a warp; lanes never diverge.
-// Point processes of these cells are evaluated by pp_step_kernel (one thread per instance) which
-// adds conductance and current into the two dynamic rows of the node (L60, L65).
+// Host side: cn_tape_program.hpp compiles the per-class programs; DESIGN.md 5.1 has the rationale
+// and profiles/r01_README.md the measurements behind every choice.
 #pragma once
 #include "cn_device.cuh"
 
