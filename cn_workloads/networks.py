@@ -307,3 +307,57 @@ def config5(scale: float = 1.0, n_types: int = 55, syn_per_cell=None, w_scale: f
             "thr": _const(n_cell, -20.0),
             "stim": {"gid": np.zeros(0, np.int32), "t": np.zeros(0)},
             "_type_of": type_of}
+
+
+# ------------------------------------------------------------------------------------------
+# node-ordering study (Fig. 5F): multiple-ring model, every cell 83 nodes,
+# 40 dendrites with a random branching pattern per type, 1..32 identical cells per type
+# ------------------------------------------------------------------------------------------
+
+def fig5f(n_cell: int = 131072, per_type: int = 32, ring_size: int = 64, weight: float = 0.02):
+    """Seeded stand-in for the paper's node-ordering workload (its model files are not here):
+    soma + 40 dendrites (82 compartments, 1..4 per dendrite), each dendrite attached to the soma or
+    to the last compartment of a random earlier dendrite; HH soma, passive dendrites, ExpSyn ring
+    NetCons with 1 ms delay, one scripted source per ring.  Cell g has type g // per_type."""
+    from .configs import _assemble_uniform, _ring_netcons
+    tag = "f5"
+    n_types = n_cell // per_type
+    assert n_types * per_type == n_cell and n_cell % ring_size == 0
+    n = 83
+    pl_t = np.empty((n_types, n), dtype=np.int64)
+    draws = rng.bits((tag, "attach"), n_types * 40).reshape(n_types, 40)
+    for t in range(n_types):
+        ncomp = _composition(82, 40, 1, 4, (tag, "comp", t))
+        bp = np.full(40, -1, dtype=np.int64)
+        for j in range(1, 40):
+            k = int(draws[t, j] % np.uint64(j + 1))      # 0 = soma, else dendrite k - 1
+            bp[j] = k - 1
+        pl_t[t], _, _, _ = expand_branches(bp, ncomp)
+    type_of = np.arange(n_cell) // per_type
+    pl_c = pl_t[type_of]
+    jl = rng.uniform((tag, "jl"), n_cell, 0.9, 1.1)
+    Lc = np.empty((n_cell, n))
+    dm = np.empty((n_cell, n))
+    Lc[:, :] = 20.0 * jl[:, None]
+    dm[:, :] = 1.0
+    Lc[:, 0] = 20.0
+    dm[:, 0] = 20.0
+    cell_first, parent, area, ri = _assemble_uniform(pl_c, Lc, dm, 100.0)
+    N = n_cell * n
+    roots = cell_first[:-1]
+    dend = np.setdiff1d(np.arange(N), roots, assume_unique=True)
+    mechs = [
+        _mech("hh", roots, {k: _const(n_cell, v) for k, v in HH_SQUID.items()}, HH_GLOBALS),
+        _mech("pas", dend, {"g": _const(len(dend), 0.001), "e": _const(len(dend), -65.0)}),
+        _mech("expsyn", roots, {"tau": _const(n_cell, 2.0), "e": _const(n_cell, 0.0)}),
+    ]
+    nc = _ring_netcons(n_cell, ring_size, 2, weight, 1.0)
+    nr = n_cell // ring_size
+    s_src = n_cell + np.arange(nr)
+    nc = {k: np.concatenate([nc[k], v]) for k, v in
+          _netcons(s_src, np.full(nr, 2), np.arange(nr) * ring_size, _const(nr, 2.5 * weight),
+                   _const(nr, 1.0)).items()}
+    return {"cell_first": cell_first, "parent": parent, "area": area, "ri": ri,
+            "cm": _const(N, 1.0), "v_init": -65.0, "celsius": 6.3, "mechs": mechs, "netcons": nc,
+            "thr": _const(n_cell, -20.0),
+            "stim": {"gid": s_src.astype(np.int32), "t": np.zeros(nr)}, "_type_of": type_of}

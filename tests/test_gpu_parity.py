@@ -369,3 +369,15 @@ def test_window_mode_one_step_per_call(cn, monkeypatch):
     og, os_ = o.get_spikes()
     gg, gs = g.get_spikes()
     assert len(og) >= 20 and list(og) == list(gg) and list(os_) == list(gs)
+
+
+@pytest.mark.parametrize("per_type", [32, 4])
+def test_fig5f_node_ordering_workload(cn, per_type):
+    """The paper's node-ordering workload (83-node cells, random branching of 40 dendrites,
+    PAPER.md L204) at 2,048 cells... the library picks the interleaved kernel for 32 identical
+    cells per type and the warp-cooperative one for 4; both must match the oracle."""
+    desc = W.fig5f(n_cell=8192, per_type=per_type)
+    o, g = run_both(cn, desc, 8.0, probes=np.asarray(desc["cell_first"][:64], dtype=np.int32))
+    info = g.layout_info()
+    assert (info["n_tape_group"] > 0) == (per_type == 32)
+    check(o, g, min_spikes=300)

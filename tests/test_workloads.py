@@ -83,3 +83,16 @@ def test_config4_headline_sizes_small_copy():
     assert np.all(np.diff(d["cell_first"]) == 291)
     assert len(d["netcons"]["src"]) == 2048 + 2048 // 64          # ring NetCons + one source per ring
     _forest_ok(d)
+
+
+def test_fig5f_node_ordering_workload_shape():
+    d = W.fig5f(n_cell=4096, per_type=4)
+    assert np.all(np.diff(d["cell_first"]) == 83)              # 83 nodes per cell
+    assert 131072 * 83 == 10878976                             # ... 10,878,976 nodes at full size
+    _forest_ok(d)
+    par = d["parent"].astype(np.int64)
+    # cells of one type share the branching pattern, different types differ
+    loc = (par.reshape(4096, 83) - d["cell_first"][:-1, None])[:, 1:]
+    assert np.array_equal(loc[0], loc[3]) and not np.array_equal(loc[0], loc[4])
+    assert len(np.unique(loc, axis=0)) == 1024
+    assert len(d["netcons"]["src"]) == 4096 + 64
