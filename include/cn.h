@@ -154,6 +154,18 @@ int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
  * tape bytes, shared-memory bytes per CTA of the interleaved kernel (after the first cn_run),
  * warps per CTA | persistent CTAs << 8 | shared-memory system rows << 24 }. */
 int cn_get_layout_info(const cn_model *m, int64_t *info8);
+/* Checkpoint / restore.  A checkpoint holds the complete dynamic state after
+ * the last step: voltages, mechanism and synapse states, threshold flags, and the spikes recorded
+ * so far.  No event queue is saved: the events still in flight are regenerated from the spikes
+ * and the NetCon delays (L156: in-flight events collapse to their originating spikes).  It is a
+ * dump in the library's internal layout: load it into a model created from the SAME description
+ * with the same library build and settings (checked: CN_ERR_ARG otherwise), before or after that
+ * model's first cn_run; the run continues from the saved step with the saved dt.  Per-step
+ * traces (cn_set_probes) are not part of it.  buf: caller-owned HOST memory. */
+int cn_checkpoint_size(const cn_model *m, int64_t *bytes_out);
+int cn_checkpoint_save(const cn_model *m, void *buf, int64_t bytes);
+int cn_checkpoint_load(cn_model *m, const void *buf, int64_t bytes);
+
 /* Spike buffer capacity (default 16*n_cell + 65536); before the first cn_run only. */
 int cn_set_spike_capacity(cn_model *m, int64_t cap);
 

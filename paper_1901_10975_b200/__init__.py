@@ -38,6 +38,7 @@ MECH = {
 EXPORTS = ("cn_model_create", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
            "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_steps_done",
            "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_get_kernel_timing", "cn_get_layout_info", "cn_set_spike_capacity",
+           "cn_checkpoint_size", "cn_checkpoint_save", "cn_checkpoint_load",
            "cn_model_destroy", "cn_last_error")
 
 
@@ -95,6 +96,9 @@ def lib():
         L.cn_get_kernel_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cn_get_layout_info.argtypes = [vp, vp]
         L.cn_set_spike_capacity.argtypes = [vp, C.c_int64]
+        L.cn_checkpoint_size.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.cn_checkpoint_save.argtypes = [vp, vp, C.c_int64]
+        L.cn_checkpoint_load.argtypes = [vp, vp, C.c_int64]
         L.cn_model_destroy.restype = None
         L.cn_model_destroy.argtypes = [vp]
         L.cn_last_error.restype = C.c_char_p
@@ -269,6 +273,18 @@ class Model:
                 "max_rounds": int(a[3]), "n_tape_group": int(a[4]), "tape_bytes": int(a[5]),
                 "tape_smem_bytes": int(a[6]), "tape_warps": int(a[7]) & 255,
                 "tape_ctas": (int(a[7]) >> 8) & 0xFFFF, "tape_sys_rows": int(a[7]) >> 24}
+
+    def checkpoint(self) -> np.ndarray:
+        """cn_checkpoint_size + cn_checkpoint_save into a fresh uint8 array."""
+        n = C.c_int64()
+        _check(lib().cn_checkpoint_size(self._h, C.byref(n)))
+        buf = np.empty(n.value, dtype=np.uint8)
+        _check(lib().cn_checkpoint_save(self._h, _ptr(buf), n.value))
+        return buf
+
+    def restore(self, buf: np.ndarray):
+        buf = np.ascontiguousarray(buf, dtype=np.uint8)
+        _check(lib().cn_checkpoint_load(self._h, _ptr(buf), buf.size))
 
     def set_spike_capacity(self, cap):
         _check(lib().cn_set_spike_capacity(self._h, int(cap)))

@@ -1795,6 +1795,142 @@ extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
   return CN_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// checkpoint / restore (L134-156)
+// ---------------------------------------------------------------------------------------------
+
+struct CkHeader {
+  uint64_t magic;
+  int64_t k, n_sp, win_idx, n_blob;
+  double dt;
+  int32_t state_pending, window;
+  uint64_t layout;  // hash of everything the raw dump depends on
+};
+
+static uint64_t ck_layout_hash(const cn_model *m) {
+  uint64_t h = mix64(0xC0FFEEull, (uint64_t)m->N);
+  h = mix64(h, (uint64_t)m->n_cell);
+  h = mix64(h, (uint64_t)m->n_ab);
+  h = mix64(h, (uint64_t)m->n_tape);
+  h = mix64(h, (uint64_t)m->n_pcell);
+  h = mix64(h, (uint64_t)m->tape_W * 1000003u + (uint64_t)m->tape_CH * 1009u + (uint64_t)m->tape_S);
+  h = mix64(h, (uint64_t)m->cls.size());
+  for (const HTable &T : m->tab) h = mix64(h, (uint64_t)T.n_dev * 31u + (uint64_t)T.type);
+  for (const TapeGroup &tg : m->tgrp) h = mix64(h, (uint64_t)tg.tape_base + (uint64_t)tg.cls);
+  return h;
+}
+
+// every device array that changes during cn_run and is live at a step boundary
+static std::vector<std::pair<void *, size_t>> ck_blobs(const cn_model *m, int64_t n_sp) {
+  std::vector<std::pair<void *, size_t>> b;
+  const DModel &H = m->hm;
+  b.emplace_back(m->d_v, (size_t)(m->n_ab + m->n_tape) * sizeof(double));
+  for (const HTable &T : m->tab)
+    for (int j = 0; j < T.ti.n_state; ++j)
+      if (T.d_state[j]) b.emplace_back(T.d_state[j], (size_t)std::max<int64_t>(T.n_dev, 1) * sizeof(double));
+  if (m->d_cai) b.emplace_back(m->d_cai, (size_t)m->n_pnode * sizeof(double));
+  b.emplace_back(H.flag, (size_t)m->n_pcell);
+  b.emplace_back(m->d_sp_gid, (size_t)n_sp * sizeof(int32_t));
+  b.emplace_back(m->d_sp_step, (size_t)n_sp * sizeof(int64_t));
+  b.emplace_back(m->d_nsp, sizeof(unsigned long long));
+  b.emplace_back(H.sp_end, (size_t)H.wr * sizeof(int64_t));
+  if (m->window) {
+    b.emplace_back(H.win_mark_step, (size_t)H.win_mark_cap * sizeof(int64_t));
+    b.emplace_back(H.win_mark_nsp, (size_t)H.win_mark_cap * sizeof(int64_t));
+  }
+  return b;
+}
+
+static int ck_spike_count(const cn_model *m, int64_t *n_sp) {
+  unsigned long long ns = 0;
+  CU(cudaStreamSynchronize(m->stream));
+  CU(cudaMemcpy(&ns, m->d_nsp, sizeof(ns), cudaMemcpyDeviceToHost));
+  *n_sp = (int64_t)std::min<unsigned long long>(ns, (unsigned long long)m->sp_cap);
+  return CN_OK;
+}
+
+extern "C" int cn_checkpoint_size(const cn_model *m, int64_t *bytes_out) {
+  if (!m || !bytes_out) return fail(CN_ERR_ARG, "NULL argument");
+  if (!m->uploaded) return fail(CN_ERR_ARG, "nothing to checkpoint before the first cn_run");
+  int64_t n_sp = 0;
+  int rc = ck_spike_count(m, &n_sp);
+  if (rc != CN_OK) return rc;
+  size_t tot = sizeof(CkHeader);
+  for (auto &b : ck_blobs(m, n_sp)) tot += sizeof(uint64_t) + ((b.second + 7) & ~(size_t)7);
+  *bytes_out = (int64_t)tot;
+  return CN_OK;
+}
+
+extern "C" int cn_checkpoint_save(const cn_model *m, void *buf, int64_t bytes) {
+  if (!m || !buf) return fail(CN_ERR_ARG, "NULL argument");
+  if (!m->uploaded) return fail(CN_ERR_ARG, "nothing to checkpoint before the first cn_run");
+  int64_t n_sp = 0;
+  int rc = ck_spike_count(m, &n_sp);
+  if (rc != CN_OK) return rc;
+  const auto blobs = ck_blobs(m, n_sp);
+  size_t tot = sizeof(CkHeader);
+  for (auto &b : blobs) tot += sizeof(uint64_t) + ((b.second + 7) & ~(size_t)7);
+  if ((size_t)bytes < tot) return fail(CN_ERR_ARG, "checkpoint buffer too small (%zu needed)", tot);
+  char *p = static_cast<char *>(buf);
+  CkHeader h{};
+  h.magic = 0x434E434B50543031ull;  // "CNCKPT01"
+  h.k = m->k;
+  h.n_sp = n_sp;
+  h.win_idx = m->win_idx;
+  h.n_blob = (int64_t)blobs.size();
+  h.dt = m->dt;
+  h.state_pending = m->state_pending ? 1 : 0;
+  h.window = m->window ? 1 : 0;
+  h.layout = ck_layout_hash(m);
+  memcpy(p, &h, sizeof(h));
+  p += sizeof(h);
+  for (auto &b : blobs) {
+    const uint64_t sz = b.second;
+    memcpy(p, &sz, sizeof(sz));
+    p += sizeof(sz);
+    if (sz) CU(cudaMemcpy(p, b.first, sz, cudaMemcpyDeviceToHost));
+    p += (sz + 7) & ~(size_t)7;
+  }
+  return CN_OK;
+}
+
+extern "C" int cn_checkpoint_load(cn_model *m, const void *buf, int64_t bytes) {
+  if (!m || !buf) return fail(CN_ERR_ARG, "NULL argument");
+  if ((size_t)bytes < sizeof(CkHeader)) return fail(CN_ERR_ARG, "not a checkpoint");
+  const char *p = static_cast<const char *>(buf);
+  CkHeader h;
+  memcpy(&h, p, sizeof(h));
+  p += sizeof(h);
+  if (h.magic != 0x434E434B50543031ull) return fail(CN_ERR_ARG, "not a checkpoint");
+  if (!m->uploaded) {
+    int rc = finalize(m, h.dt);
+    if (rc != CN_OK) return rc;
+  } else if (h.dt != m->dt) {
+    return fail(CN_ERR_DT, "checkpoint was taken with dt = %.17g, the model runs with %.17g", h.dt, m->dt);
+  }
+  if (h.layout != ck_layout_hash(m) || (h.window != 0) != m->window)
+    return fail(CN_ERR_ARG, "checkpoint of a different model, library build or launch mode");
+  if (h.n_sp > m->sp_cap) return fail(CN_ERR_OVERFLOW, "checkpoint holds more spikes than the buffer");
+  const auto blobs = ck_blobs(m, h.n_sp);
+  if ((int64_t)blobs.size() != h.n_blob) return fail(CN_ERR_ARG, "checkpoint layout mismatch");
+  CU(cudaStreamSynchronize(m->stream));
+  const char *end = static_cast<const char *>(buf) + bytes;
+  for (auto &b : blobs) {
+    uint64_t sz;
+    if (p + sizeof(sz) > end) return fail(CN_ERR_ARG, "checkpoint truncated");
+    memcpy(&sz, p, sizeof(sz));
+    p += sizeof(sz);
+    if (sz != b.second || p + sz > end) return fail(CN_ERR_ARG, "checkpoint layout mismatch");
+    if (sz) CU(cudaMemcpy(b.first, p, sz, cudaMemcpyHostToDevice));
+    p += (sz + 7) & ~(size_t)7;
+  }
+  m->k = h.k;
+  m->win_idx = h.win_idx;
+  m->state_pending = h.state_pending != 0;
+  m->probe_rows = 0;
+  return CN_OK;
+}
+
 extern "C" int cn_set_spike_capacity(cn_model *m, int64_t cap) {
   if (!m || cap < 1) return fail(CN_ERR_ARG, "bad capacity");
   if (m->uploaded) return fail(CN_ERR_ARG, "capacity must be set before the first cn_run");
