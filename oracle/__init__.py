@@ -33,10 +33,11 @@ MECH = {
     "sk": (7, ("gbar",), ("E", "Kd", "n", "tau_z")),
     "cadyn": (8, (), ("gamma", "depth", "tau_d", "cai_min")),
     "ampanmda": (9, (), ("tau_r_A", "tau_d_A", "tau_r_N", "tau_d_N", "r_nmda", "mg", "e")),
+    "gap": (10, ("g", "peer"), ()),
 }
 STATES = {
     "pas": (), "hh": ("m", "h", "n"), "expsyn": ("g",), "exp2syn": ("A", "B"), "iclamp": (),
-    "hhform": ("m", "h"), "sk": ("z",), "cadyn": (), "ampanmda": ("A_A", "B_A", "A_N", "B_N"),
+    "hhform": ("m", "h"), "sk": ("z",), "cadyn": (), "ampanmda": ("A_A", "B_A", "A_N", "B_N"), "gap": (),
 }
 
 

@@ -36,6 +36,7 @@ int orc_n_state(int32_t type) {
     case ORC_SK: return 1;      /* z */
     case ORC_CADYN: return 0;   /* cai lives in the per-node ion array */
     case ORC_AMPANMDA: return 4; /* A_ampa B_ampa A_nmda B_nmda */
+    case ORC_GAP: return 0;
   }
   return -1;
 }
@@ -51,6 +52,7 @@ int orc_n_param(int32_t type) {
     case ORC_SK: return 1;
     case ORC_CADYN: return 0;
     case ORC_AMPANMDA: return 0;
+    case ORC_GAP: return 2;
   }
   return -1;
 }
@@ -66,12 +68,14 @@ static int n_global_of(int32_t type) {
     case ORC_SK: return 4;
     case ORC_CADYN: return 4;
     case ORC_AMPANMDA: return 7;
+    case ORC_GAP: return 0;
   }
   return -1;
 }
 
 static int is_point(int32_t type) {
-  return type == ORC_EXPSYN || type == ORC_EXP2SYN || type == ORC_ICLAMP || type == ORC_AMPANMDA;
+  return type == ORC_EXPSYN || type == ORC_EXP2SYN || type == ORC_ICLAMP || type == ORC_AMPANMDA ||
+         type == ORC_GAP;
 }
 
 /* x / (exp(x/y) - 1) with the removable singularity at x = 0 */
@@ -416,6 +420,11 @@ orc_model *orc_create(const orc_desc *de) {
     if (mt->n_param != orc_n_param(mt->type) || mt->n_global != n_global_of(mt->type)) return NULL;
     for (i = 0; i < mt->n; ++i)
       if (mt->node[i] < 0 || mt->node[i] >= N) return NULL;
+    if (mt->type == ORC_GAP) /* the peer is a node of the model, given as an integral double */
+      for (i = 0; i < mt->n; ++i) {
+        double pr = mt->param[(int64_t)1 * mt->n + i];
+        if (!(pr >= 0.0 && pr < (double)N) || pr != (double)(int64_t)pr) return NULL;
+      }
   }
   for (i = 0; i < de->n_netcon; ++i) {
     int32_t tm = de->nc_tgt_mech[i];
@@ -636,6 +645,11 @@ static void one_step(orc_model *m) {
       for (j = 0; j < mt->n_param; ++j) P[j] = mt->param[(int64_t)j * mt->n + i];
       for (j = 0; j < mt->n_state; ++j) S[j] = mt->state[(int64_t)j * mt->n + i];
       orc_mech_cur(mt->type, mt->global, P, S, m->v[nd], m->cai[nd], t_mid, &cur, &g, &ica);
+      if (mt->type == ORC_GAP) { /* L160, L228: the peer's voltage of the start of the step; all
+                                    of v is still v^k here (O8 comes later) */
+        cur = P[0] * (m->v[nd] - m->v[(int64_t)P[1]]);
+        g = P[0];
+      }
       if (point) { /* nA, uS -> mA/cm2, S/cm2 (L60) */
         m->rhs[nd] -= 100.0 * cur / m->area[nd];
         m->d[nd] += 100.0 * g / m->area[nd];

@@ -33,7 +33,11 @@ enum {
   ORC_HHFORM = 6,   /* param: gbar ; global: p,q,E,to_ica, m(vh,k,t0,t1,vt,s), h(..)*/
   ORC_SK = 7,       /* param: gbar ; global: E, Kd, n, tau_z ; state z             */
   ORC_CADYN = 8,    /* no param ; global: gamma, depth, tau_d, cai_min ; state cai */
-  ORC_AMPANMDA = 9  /* no param ; global: tau_r_A,tau_d_A,tau_r_N,tau_d_N,r_nmda,mg,e */
+  ORC_AMPANMDA = 9, /* no param ; global: tau_r_A,tau_d_A,tau_r_N,tau_d_N,r_nmda,mg,e */
+  ORC_GAP = 10      /* param: g (uS), peer (global node index, as a double) ; no state.
+                       Gap junction of the fixed-step method: point current
+                       i = g (v - v_peer) with v_peer the peer's voltage at the START of the step
+                       (the voltages are exchanged once per step), conductance g              */
 };
 
 enum { ORC_OK = 0, ORC_ERR = -1 };

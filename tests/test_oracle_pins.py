@@ -549,6 +549,115 @@ def test_p10_iclamp_active_steps_40_to_79():
 
 
 # ---------------------------------------------------------------------------------------------
+# P10b: gap junctions (L160, L228): explicit peer voltage, exchanged once per step
+# ---------------------------------------------------------------------------------------------
+
+def _gap_cells(g, pairs, n_cell=3, amp=0.5, cm=1.0, decoy_e=0.0):
+    """n_cell one-compartment cells without membrane conductance (pure capacitors), cell 1 a
+    decoy with a leak to decoy_e; `pairs` = (node, peer) list of gap junctions; cell 0 gets a
+    current pulse on steps 40..79."""
+    area = math.pi * 20.0 * 20.0
+    N = n_cell
+    nd = np.array([p[0] for p in pairs], np.int32)
+    pr = np.array([p[1] for p in pairs], np.float64)
+    return {
+        "cell_first": np.arange(N + 1, dtype=np.int64), "parent": np.full(N, -1, np.int32),
+        "area": np.full(N, area), "ri": np.ones(N), "cm": np.full(N, cm), "v_init": -65.0,
+        "celsius": 6.3,
+        "mechs": [
+            {"type": "pas", "node": np.array([1], np.int32),
+             "params": {"g": np.array([0.001]), "e": np.array([decoy_e])}, "globals": {}},
+            {"type": "iclamp", "node": np.array([0], np.int32),
+             "params": {"del": np.array([1.0]), "dur": np.array([1.0]), "amp": np.array([amp])},
+             "globals": {}},
+            {"type": "gap", "node": nd, "params": {"g": np.full(len(pairs), g), "peer": pr},
+             "globals": {}}],
+        "netcons": {"src": np.zeros(0, np.int32), "tgt_mech": np.zeros(0, np.int32),
+                    "tgt_inst": np.zeros(0, np.int64), "weight": np.zeros(0),
+                    "delay": np.zeros(0)},
+        "thr": np.full(N, 1e9), "stim": {"gid": np.zeros(0, np.int32), "t": np.zeros(0)}}, area
+
+
+def test_p10b_gap_pair_closed_form():
+    g, amp = 0.004, 0.5
+    desc, area = _gap_cells(g, [(0, 2), (2, 0)])
+    m = OracleModel(desc)
+    m.set_probes([0, 1, 2])
+    m.run(6.0, DT)
+    tr = np.vstack([[-65.0] * 3, m.get_trace()])
+    c = 1e-3 / DT
+    gs = 100.0 * g / area
+    v0, v2 = tr[:, 0], tr[:, 2]
+    ssum, d = v0 + v2, v0 - v2
+    # the pair exchanges charge only: the sum moves only while the electrode is on (steps 40..79),
+    # by Is / (c + gs) per step (the junction conductance sits on the diagonal of both rows)
+    inc = np.diff(ssum)
+    assert np.max(np.abs(inc[:40])) == 0.0 and np.max(np.abs(inc[80:])) < 1e-12
+    assert np.allclose(inc[40:80], (100.0 * amp / area) / (c + gs), rtol=1e-11)
+    # after the pulse the difference decays by (c - gs)/(c + gs) per step: the peer voltage is the
+    # one of the START of the step (an implicit peer would give c/(c + 2 gs))
+    r = d[81:] / d[80:-1]
+    assert abs(d[80]) > 1.0
+    assert np.allclose(r, (c - gs) / (c + gs), rtol=1e-10)
+    assert not np.allclose(r, c / (c + 2 * gs), rtol=1e-4)
+    # the decoy (same start voltage, leak to 0 mV) is neither read nor written by the junctions
+    alone, _ = _gap_cells(g, [])
+    ma = OracleModel(alone)
+    ma.set_probes([1])
+    ma.run(6.0, DT)
+    assert np.array_equal(ma.get_trace()[:, 0], tr[1:, 1])
+    assert abs(tr[-1, 1] - tr[-1, 2]) > 5.0
+
+
+def test_p10b_gap_difference_mode_converges_to_continuous_decay():
+    g = 0.002
+    errs = []
+    for dt in (DT, DT / 2):
+        desc, area = _gap_cells(g, [(0, 2), (2, 0)])
+        m = OracleModel(desc)
+        m.set_probes([0, 2])
+        m.run(8.0, dt)
+        tr = m.get_trace()
+        k0 = int(round(2.0 / dt)) + 1            # first row after the pulse
+        d = tr[k0:, 0] - tr[k0:, 1]
+        t = np.arange(len(d)) * dt
+        cont = d[0] * np.exp(-2.0 * (100.0 * g / area) * t / 1e-3)   # C dv/dt = -g (v - v_peer)
+        errs.append(np.max(np.abs(d - cont)))
+    # (1 - x)/(1 + x), x = gs dt / C, is the (1,1) Pade approximant of exp(-2x): for this mode
+    # "own voltage implicit, peer explicit" is the trapezoidal rule, hence SECOND order
+    assert errs[0] < 1e-4 * abs(d[0]) and 3.6 < errs[0] / errs[1] < 4.4
+
+
+def test_p10b_gap_one_way_and_sign():
+    # a junction on cell 0 only, towards the decoy: cell 0 is pulled TOWARDS the decoy's voltage,
+    # the decoy does not feel it (one half of a junction is one point process)
+    desc, area = _gap_cells(0.01, [(0, 1)], amp=0.0)
+    m = OracleModel(desc)
+    m.set_probes([0, 1, 2])
+    m.run(10.0, DT)
+    tr = m.get_trace()
+    assert np.all(np.diff(tr[:, 0]) > 0) and tr[-1, 0] > -60.0      # decoy rises towards 0 mV
+    assert np.all(tr[:, 0] < tr[:, 1])
+    assert np.all(tr[:, 2] == -65.0)
+    alone, _ = _gap_cells(0.01, [], amp=0.0)
+    ma = OracleModel(alone)
+    ma.set_probes([1])
+    ma.run(10.0, DT)
+    assert np.array_equal(ma.get_trace()[:, 0], tr[:, 1])
+    # one step by hand: v0' = v0 - gs (v0 - v1) / (c + gs) with v1 of the start of the step
+    c, gs = 1e-3 / DT, 100.0 * 0.01 / area
+    k = 100
+    assert abs(tr[k + 1, 0] - (tr[k, 0] - gs * (tr[k, 0] - tr[k, 1]) / (c + gs))) < 1e-13
+
+
+def test_p10b_gap_peer_validated():
+    for bad in (3.0, -1.0, 0.5):
+        desc, _ = _gap_cells(0.01, [(0, bad)])
+        with pytest.raises(Exception):
+            OracleModel(desc)
+
+
+# ---------------------------------------------------------------------------------------------
 # P11: threshold semantics (R5)
 # ---------------------------------------------------------------------------------------------
 
