@@ -475,6 +475,46 @@ def extract_cells(desc: dict, gids) -> dict:
             "mechs": mechs, "netcons": new_nc, "thr": desc["thr"][gids], "stim": stim}
 
 
+def concat_models(descs) -> dict:
+    """Several descriptions side by side as one model: cells, nodes and instances renumbered, no
+    connection between the parts.  The parts must have the same list of mechanism tables (type and
+    globals) and no scripted sources."""
+    d0 = descs[0]
+    node_off = np.concatenate([[0], np.cumsum([int(d["cell_first"][-1]) for d in descs])])
+    cell_off = np.concatenate([[0], np.cumsum([len(d["cell_first"]) - 1 for d in descs])])
+    for d in descs:
+        assert len(d["stim"]["gid"]) == 0 and len(d["mechs"]) == len(d0["mechs"])
+        assert d["v_init"] == d0["v_init"] and d["celsius"] == d0["celsius"]
+    mechs = []
+    inst_off = []
+    for t, m0 in enumerate(d0["mechs"]):
+        parts = [d["mechs"][t] for d in descs]
+        assert all(p["type"] == m0["type"] and p["globals"] == m0["globals"] for p in parts)
+        inst_off.append(np.concatenate([[0], np.cumsum([len(p["node"]) for p in parts])]))
+        mechs.append(_mech(m0["type"],
+                           np.concatenate([p["node"].astype(np.int64) + node_off[j]
+                                           for j, p in enumerate(parts)]),
+                           {k: np.concatenate([p["params"][k] for p in parts])
+                            for k in m0["params"]}, m0["globals"]))
+    cat = lambda key, sub=None: np.concatenate(  # noqa: E731
+        [(d[key] if sub is None else d[key][sub]) for d in descs])
+    nc = _netcons(
+        np.concatenate([d["netcons"]["src"].astype(np.int64) + cell_off[j]
+                        for j, d in enumerate(descs)]),
+        cat("netcons", "tgt_mech"),
+        np.concatenate([d["netcons"]["tgt_inst"].astype(np.int64) +
+                        np.array([inst_off[t][j] for t in d["netcons"]["tgt_mech"]], np.int64)
+                        for j, d in enumerate(descs)]),
+        cat("netcons", "weight"), cat("netcons", "delay"))
+    par = np.concatenate([np.where(d["parent"] < 0, -1, d["parent"].astype(np.int64) + node_off[j])
+                          for j, d in enumerate(descs)])
+    cf = np.concatenate([[0]] + [d["cell_first"][1:] + node_off[j] for j, d in enumerate(descs)])
+    return {"cell_first": cf.astype(np.int64), "parent": par.astype(np.int32),
+            "area": cat("area"), "ri": cat("ri"), "cm": cat("cm"), "v_init": d0["v_init"],
+            "celsius": d0["celsius"], "mechs": mechs, "netcons": nc, "thr": cat("thr"),
+            "stim": _no_stim()}
+
+
 def renumber_nodes(desc: dict, stream="renum") -> dict:
     """Seeded random parent-before-child renumbering inside every cell (roots stay first)."""
     cf = desc["cell_first"]

@@ -361,3 +361,34 @@ def fig5f(n_cell: int = 131072, per_type: int = 32, ring_size: int = 64, weight:
             "cm": _const(N, 1.0), "v_init": -65.0, "celsius": 6.3, "mechs": mechs, "netcons": nc,
             "thr": _const(n_cell, -20.0),
             "stim": {"gid": s_src.astype(np.int32), "t": np.zeros(nr)}, "_type_of": type_of}
+
+
+# ------------------------------------------------------------------------------------------
+# gap junctions: electrical coupling between cells
+# ------------------------------------------------------------------------------------------
+
+def with_gap_junctions(desc: dict, n_junction: int, g: float = 0.002, tag="gap",
+                       neighbours_only: bool = True) -> dict:
+    """`desc` plus n_junction symmetric gap junctions (two `gap` instances each, conductance g uS
+    +- 50 % seeded).  The two ends are seeded nodes of different cells; with neighbours_only the
+    cells are gid neighbours (c, c+1), the way electrically coupled interneurons sit side by
+    side, otherwise any two cells."""
+    cf = desc["cell_first"]
+    n_cell = len(cf) - 1
+    assert n_cell >= 2
+    bits = rng.bits((tag, "ends"), 4 * n_junction)
+    ca = (bits[0::4] % np.uint64(n_cell)).astype(np.int64)
+    if neighbours_only:
+        cb = (ca + 1) % n_cell
+    else:
+        cb = (ca + 1 + (bits[1::4] % np.uint64(n_cell - 1)).astype(np.int64)) % n_cell
+    sz = cf[1:] - cf[:-1]
+    na = cf[ca] + (bits[2::4] % sz[ca].astype(np.uint64)).astype(np.int64)
+    nb = cf[cb] + (bits[3::4] % sz[cb].astype(np.uint64)).astype(np.int64)
+    gj = g * rng.uniform((tag, "g"), n_junction, 0.5, 1.5)
+    node = np.concatenate([na, nb])
+    peer = np.concatenate([nb, na]).astype(np.float64)
+    out = dict(desc)
+    out["mechs"] = list(desc["mechs"]) + [_mech("gap", node, {"g": np.concatenate([gj, gj]),
+                                                            "peer": peer})]
+    return out

@@ -60,8 +60,13 @@ enum {
                       global: E, Kd, n, tau_z                                                 */
   CN_CADYN = 8,    /* cai' = -(1e4 gamma/(2 F depth)) ica - (cai-cai_min)/tau_d  (derivimplicit)
                       no param ; global: gamma, depth, tau_d, cai_min                         */
-  CN_AMPANMDA = 9  /* point: AMPA + NMDA double exponentials with Mg block
+  CN_AMPANMDA = 9, /* point: AMPA + NMDA double exponentials with Mg block
                       no param ; global: tau_r_A, tau_d_A, tau_r_N, tau_d_N, r_nmda, mg, e    */
+  CN_GAP = 10      /* point: one half of a gap junction, i = g (v - v_peer)
+                      param: g (uS), peer (global node index in caller order, an integral double)
+                      v_peer is the peer's voltage at the START of the step (exchanged once per
+                      dt); g enters the node's diagonal.  A symmetric junction is two instances.
+                      Models with gap junctions run one launch sequence per dt (no window).    */
 };
 
 /* One mechanism type = one instance table, structure of arrays (L178, Fig. 3D). */

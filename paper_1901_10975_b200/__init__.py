@@ -33,6 +33,7 @@ MECH = {
     "sk": (7, ("gbar",), ("E", "Kd", "n", "tau_z")),
     "cadyn": (8, (), ("gamma", "depth", "tau_d", "cai_min")),
     "ampanmda": (9, (), ("tau_r_A", "tau_d_A", "tau_r_N", "tau_d_N", "r_nmda", "mg", "e")),
+    "gap": (10, ("g", "peer"), ()),
 }
 
 EXPORTS = ("cn_model_create", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",

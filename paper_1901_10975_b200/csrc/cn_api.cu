@@ -62,6 +62,7 @@ static bool type_info(int type, TypeInfo &ti) {
     case CN_SK: ti = {1, 1, 4, 0, 2}; return true;        // + invc
     case CN_CADYN: ti = {0, 0, 4, 0, 0}; return true;
     case CN_AMPANMDA: ti = {0, 4, 7, 1, 1}; return true;  // scale
+    case CN_GAP: ti = {2, 0, 0, 1, 2}; return true;       // g * scale, peer's position
   }
   return false;
 }
@@ -395,6 +396,13 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
     if (mt.type == CN_EXPSYN)
       for (int64_t i = 0; i < mt.n; ++i)
         if (!(mt.param[i] > 0.0)) return fail(CN_ERR_MECH, "table %d: ExpSyn needs tau > 0", t);
+    if (mt.type == CN_GAP)
+      for (int64_t i = 0; i < mt.n; ++i) {
+        const double pr = mt.param[mt.n + i];
+        if (!(pr >= 0.0 && pr < (double)N) || pr != (double)(int64_t)pr)
+          return fail(CN_ERR_MECH, "table %d: gap junction %lld has no such peer node", t,
+                      (long long)i);
+      }
   }
   if (de->n_netcon < 0 || de->n_stim < 0) return fail(CN_ERR_NETCON, "negative count");
   int32_t n_src = de->n_cell;
@@ -748,7 +756,8 @@ static int build_layout(cn_model *m) {
       if (K.tp.n_cells < K.count) all = false;
     }
     for (const HTable &T : m->tab)
-      if (T.type == CN_AMPANMDA && T.n > 0) all = false;  // (no window mode with these)
+      if ((T.type == CN_AMPANMDA || T.type == CN_GAP) && T.n > 0)
+        all = false;  // (no window mode with these)
     if (!all || cells * 4 < groups * 32) {  // back to the warp-cooperative kernel, all of it
       for (HClass &K : m->cls) {
         K.tp.n_groups = 0;
@@ -1264,6 +1273,10 @@ static int finalize(cn_model *m, double dt) {
           break;
         }
         case CN_AMPANMDA: P[0] = scale; break;
+        case CN_GAP:  // positions in the voltage arena (exact in a double: < 2^53)
+          P[0] *= scale;
+          P[1] = (double)m->node_pos[(int64_t)P[1]];
+          break;
         default: break;
       }
       if (!T.ti.point && T.tape_loc[i] >= 0) {  // the instance lives on a tape
@@ -1387,11 +1400,11 @@ static int finalize(cn_model *m, double dt) {
   }
   lap("netcons");
   // window mode: every cell on the interleaved kernel, no point process whose current depends on
-  // v (AMPA+NMDA), no per-step probes; a window is at most the smallest delay long
+  // v (AMPA+NMDA, gap junctions), no per-step probes; a window is at most the smallest delay long
   {
     bool ok = m->hm.n_tgroup > 0 && m->grp.empty() && m->probe.empty();
     for (const HTable &T : m->tab)
-      if (T.type == CN_AMPANMDA && T.n > 0) ok = false;
+      if ((T.type == CN_AMPANMDA || T.type == CN_GAP) && T.n > 0) ok = false;
     if (const char *e = std::getenv("CN_TAPE_WINDOW")) ok = ok && std::atoi(e) != 0;
     int64_t wn = m->n_netcon > 0 ? std::min<int64_t>(H.mind, 64) : 32;
     if (wn < 2) ok = false;

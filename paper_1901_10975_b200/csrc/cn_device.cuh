@@ -27,7 +27,7 @@
 namespace cn {
 
 enum { T_PAS = 1, T_HH = 2, T_EXPSYN = 3, T_EXP2SYN = 4, T_ICLAMP = 5, T_HHFORM = 6, T_SK = 7,
-       T_CADYN = 8, T_AMPANMDA = 9 };
+       T_CADYN = 8, T_AMPANMDA = 9, T_GAP = 10 };
 
 struct DTable {
   int type, is_point, n_param, n_state;

@@ -729,6 +729,14 @@ __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DM
           }
         }
         break;
+      case T_GAP:  // L228: the peer's voltage as the previous step left it (this kernel runs
+                   // before any voltage of step k is written)
+        for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
+          const double gs = T.param[0][q];
+          atomicAdd(&tape[tgt[q]], gs);
+          atomicAdd(&tape[tgt[q] + 32], gs * M.v[(int64_t)T.param[1][q]]);
+        }
+        break;
       default: break;
     }
   }

@@ -381,3 +381,43 @@ def test_fig5f_node_ordering_workload(cn, per_type):
     info = g.layout_info()
     assert (info["n_tape_group"] > 0) == (per_type == 32)
     check(o, g, min_spikes=300)
+
+
+# ---------------------------------------------------------------------------------------------
+# gap junctions
+# ---------------------------------------------------------------------------------------------
+
+def test_gap_junctions_between_ring_cells(cn, strategy):
+    """HH ring cells with 60 symmetric gap junctions between neighbours (any node to any node):
+    the peer voltages are the ones of the start of the step.  The coupling is strong enough to
+    move the spike times (checked on the oracle), so a dropped or mis-addressed junction fails."""
+    from oracle import OracleModel
+    base = W.config2(n_cell=64, ring_size=32, depth=2, ncomp_branch=10, weight=0.05)
+    desc = W.with_gap_junctions(base, 60, g=0.02)
+    o, g = run_both(cn, desc, 30.0)
+    check(o, g, min_spikes=20)
+    ob = OracleModel(base)
+    ob.run(30.0, DT)
+    assert [list(x) for x in ob.get_spikes()] != [list(x) for x in o.get_spikes()]
+    # without probes the model would qualify for window mode but for the junctions (their current
+    # depends on the voltages of the step before): one launch sequence per dt, same results
+    g2 = cn.Model(desc)
+    g2.run(30.0, DT)
+    assert g2.launch_count >= 1200
+    assert np.max(np.abs(o.get_v() - g2.get_v())) <= TOL
+    assert [list(x) for x in g2.get_spikes()] == [list(x) for x in o.get_spikes()]
+
+
+def test_gap_junctions_across_kernels(cn, monkeypatch):
+    """Junctions between cells on the interleaved kernel (groups of >= 16 identical cells) and
+    cells on the warp-cooperative kernel (unique topologies): the peer position addresses the
+    one voltage arena both kernels write."""
+    monkeypatch.setenv("CN_TAPE", "1")
+    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "16")
+    a = W.random_tree_cells(24, 40, 40, stream="gap-a", identical=True, weight=0.2, amp=2.0)
+    b = W.random_tree_cells(9, 20, 90, stream="gap-b", weight=0.2, amp=2.0)
+    desc = W.with_gap_junctions(W.concat_models([a, b]), 50, g=0.01, neighbours_only=False)
+    o, g = run_both(cn, desc, 30.0)
+    info = g.layout_info()
+    assert info["n_tape_group"] >= 1 and info["n_group"] > info["n_tape_group"]
+    check(o, g, min_spikes=5)

@@ -96,3 +96,38 @@ def test_fig5f_node_ordering_workload_shape():
     assert np.array_equal(loc[0], loc[3]) and not np.array_equal(loc[0], loc[4])
     assert len(np.unique(loc, axis=0)) == 1024
     assert len(d["netcons"]["src"]) == 4096 + 64
+
+
+def test_concat_models_is_block_diagonal():
+    from oracle import OracleModel
+    a = W.random_tree_cells(5, 10, 10, stream="cat-a", identical=True, weight=0.2, amp=2.0)
+    b = W.random_tree_cells(4, 8, 30, stream="cat-b", weight=0.2, amp=2.0)
+    ab = W.concat_models([a, b])
+    oa, ob, oab = OracleModel(a), OracleModel(b), OracleModel(ab)
+    for o in (oa, ob, oab):
+        o.run(20.0, 0.025)
+    assert np.array_equal(np.concatenate([oa.get_v(), ob.get_v()]), oab.get_v())
+    ga, sa = oa.get_spikes()
+    gb, sb = ob.get_spikes()
+    gab, sab = oab.get_spikes()
+    assert len(ga) > 2 and len(gb) > 2
+    assert sorted(zip(sab, gab)) == sorted(list(zip(sa, ga)) + list(zip(sb, gb + 5)))
+
+
+def test_gap_junction_generator():
+    base = W.config2(n_cell=16, ring_size=8, depth=2, ncomp_branch=4)
+    d = W.with_gap_junctions(base, 25, g=0.01)
+    gj = d["mechs"][-1]
+    assert gj["type"] == "gap" and len(gj["node"]) == 50
+    node, peer = gj["node"].astype(np.int64), gj["params"]["peer"].astype(np.int64)
+    assert np.array_equal(node[:25], peer[25:]) and np.array_equal(node[25:], peer[:25])
+    assert np.array_equal(gj["params"]["g"][:25], gj["params"]["g"][25:])
+    cf = d["cell_first"]
+    ca = np.searchsorted(cf, node, side="right") - 1
+    cb = np.searchsorted(cf, peer, side="right") - 1
+    assert np.all((cb[:25] - ca[:25]) % 16 == 1)          # gid neighbours
+    d2 = W.with_gap_junctions(base, 25, g=0.01, neighbours_only=False)
+    p2 = d2["mechs"][-1]["params"]["peer"].astype(np.int64)
+    n2 = d2["mechs"][-1]["node"].astype(np.int64)
+    assert np.all(np.searchsorted(cf, n2, side="right") != np.searchsorted(cf, p2, side="right"))
+    assert len(base["mechs"]) + 1 == len(d["mechs"])      # the input is left alone
