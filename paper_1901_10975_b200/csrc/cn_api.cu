@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <numeric>
 #include <string>
@@ -78,6 +79,113 @@ static double h_exp2_factor(double t1, double t2) {
   return 1.0 / (std::exp(-tp / t2) - std::exp(-tp / t1));
 }
 
+// std::vector that does not value-initialise (large set-up arrays are filled by all host cores)
+template <class T>
+struct NoInitAlloc {
+  using value_type = T;
+  NoInitAlloc() = default;
+  template <class U> NoInitAlloc(const NoInitAlloc<U> &) {}
+  T *allocate(size_t n) { return static_cast<T *>(::operator new(n * sizeof(T))); }
+  void deallocate(T *p, size_t) { ::operator delete(p); }
+  template <class U, class... A> void construct(U *p, A &&...a) {
+    if constexpr (sizeof...(A) == 0) ::new ((void *)p) U; else ::new ((void *)p) U(std::forward<A>(a)...);
+  }
+  template <class U> bool operator==(const NoInitAlloc<U> &) const { return true; }
+  template <class U> bool operator!=(const NoInitAlloc<U> &) const { return false; }
+};
+template <class T> using uvec = std::vector<T, NoInitAlloc<T>>;
+
+// body(begin, end) over [0, n_items) on all host cores (create / first-run set-up only)
+template <class F>
+static void par_for(int64_t n_items, int64_t grain, F &&body) {
+  const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+  const unsigned nth = (unsigned)std::min<int64_t>(hw, std::max<int64_t>(1, n_items / grain));
+  if (nth <= 1) {
+    body((int64_t)0, n_items);
+    return;
+  }
+  std::vector<std::thread> pool;
+  for (unsigned t = 0; t < nth; ++t)
+    pool.emplace_back([&body, n_items, nth, t] { body(n_items * t / nth, n_items * (t + 1) / nth); });
+  for (auto &th : pool) th.join();
+}
+
+static unsigned par_threads(int64_t n_items, int64_t grain) {
+  const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+  return (unsigned)std::min<int64_t>(hw, std::max<int64_t>(1, n_items / grain));
+}
+
+// body(t) for t in [0, P) on P threads
+template <class F>
+static void par_run(unsigned P, F &&body) {
+  if (P <= 1) {
+    body(0u);
+    return;
+  }
+  std::vector<std::thread> pool;
+  for (unsigned t = 0; t < P; ++t) pool.emplace_back([&body, t] { body(t); });
+  for (auto &th : pool) th.join();
+}
+
+// Stable counting sort of the items [0, n) by key(i) in [0, nb) on all cores: first[b] = number
+// of items with a smaller key, rank[i] = position of item i in the sorted order.
+template <class KeyF>
+static void par_bucket(int64_t n, int64_t nb, KeyF &&key, std::vector<int64_t> &first,
+                       uvec<int64_t> &rank) {
+  unsigned P = par_threads(n, 1 << 16);
+  while (P > 1 && (int64_t)P * nb > ((int64_t)32 << 20)) P /= 2;
+  std::vector<std::vector<int64_t>> cnt(P);
+  par_run(P, [&](unsigned t) {
+    cnt[t].assign((size_t)nb, 0);
+    for (int64_t i = n * t / P, e = n * (t + 1) / P; i < e; ++i) cnt[t][key(i)]++;
+  });
+  first.assign((size_t)nb + 1, 0);
+  int64_t run = 0;
+  for (int64_t b = 0; b < nb; ++b) {
+    first[b] = run;
+    for (unsigned t = 0; t < P; ++t) {
+      const int64_t c = cnt[t][b];
+      cnt[t][b] = run;
+      run += c;
+    }
+  }
+  first[nb] = run;
+  rank.resize((size_t)n);
+  par_run(P, [&](unsigned t) {
+    for (int64_t i = n * t / P, e = n * (t + 1) / P; i < e; ++i) rank[i] = cnt[t][key(i)]++;
+  });
+}
+
+// dst = src[0, n) copied by all cores (first touch of the fresh pages included)
+template <class T>
+static void par_assign(uvec<T> &dst, const T *src, int64_t n) {
+  dst.resize((size_t)n);
+  par_for(n, 1 << 18, [&](int64_t i0, int64_t i1) {
+    if (i1 > i0) memcpy(dst.data() + i0, src + i0, (size_t)(i1 - i0) * sizeof(T));
+  });
+}
+
+// validation passes run on all cores; the failure with the smallest index is the one reported
+struct FirstErr {
+  std::mutex mu;
+  int64_t key = INT64_MAX;
+  int code = CN_OK;
+  char msg[256] = "";
+  void set(int64_t k, int c, const char *fmt, ...) {
+    char buf[256];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    std::lock_guard<std::mutex> lk(mu);
+    if (k < key) {
+      key = k;
+      code = c;
+      memcpy(msg, buf, sizeof(msg));
+    }
+  }
+};
+
 // ---------------------------------------------------------------------------------------------
 // model
 // ---------------------------------------------------------------------------------------------
@@ -86,13 +194,13 @@ struct HTable {
   int type = 0;
   TypeInfo ti{};
   int64_t n = 0;
-  std::vector<int32_t> node;
-  std::vector<double> param;  // [n_param][n]
+  uvec<int32_t> node;
+  uvec<double> param;  // [n_param][n]
   std::vector<double> glob;
   // layout
   int64_t n_dev = 0;               // padded device instance count
-  std::vector<int64_t> inst_pos;   // caller instance -> device instance (table arrays)
-  std::vector<int64_t> tape_loc;   // distributed: tape element of the first PARAMETER row of an
+  uvec<int64_t> inst_pos;   // caller instance -> device instance (table arrays)
+  uvec<int64_t> tape_loc;   // distributed: tape element of the first PARAMETER row of an
                                    // instance on a tape cell, else -1
   int64_t pp_tape_begin = 0;       // point: instances [pp_tape_begin, n) sit on tape cells
   // device
@@ -104,14 +212,14 @@ struct HTable {
   int64_t *d_grp_instbase = nullptr;
   // host layout tables
   std::vector<int64_t> pp_first;
-  std::vector<int32_t> pp_slot;
-  std::vector<uint32_t> pp_wslot;  // window mode: element in one step's block of win_rows
+  uvec<int32_t> pp_slot;
+  uvec<uint32_t> pp_wslot;  // window mode: element in one step's block of win_rows
   uint32_t *d_pp_wslot = nullptr;
   std::vector<int32_t> cls_cnt, cls_nodeoff;
   std::vector<int64_t> grp_instbase;
   // per-cell CSR of distributed instances sorted by local node
   std::vector<int64_t> cell_first;
-  std::vector<int64_t> cell_inst;
+  uvec<int64_t> cell_inst;
 };
 
 struct HTask {
@@ -155,14 +263,15 @@ struct cn_model {
   int32_t n_cell = 0;
   int64_t N = 0;
   std::vector<int64_t> cell_first;
-  std::vector<int32_t> parent;
-  std::vector<double> area, ri, cm, thr;
+  uvec<int32_t> parent;
+  uvec<double> area, ri, cm;
+  std::vector<double> thr;
   double v_init = -65.0, celsius = 6.3;
   std::vector<HTable> tab;
   int64_t n_netcon = 0;
-  std::vector<int32_t> nc_src, nc_tgt_mech;
-  std::vector<int64_t> nc_tgt_inst;
-  std::vector<double> nc_w, nc_delay;
+  uvec<int32_t> nc_src, nc_tgt_mech;
+  uvec<int64_t> nc_tgt_inst;
+  uvec<double> nc_w, nc_delay;
   std::vector<int32_t> stim_gid;
   std::vector<double> stim_t;
   int32_t n_src = 0;
@@ -170,7 +279,7 @@ struct cn_model {
   std::vector<HClass> cls;
   std::vector<GroupInfo> grp;
   std::vector<int32_t> cell_cls, cell_grp, cell_slot;
-  std::vector<int64_t> node_pos;  // caller node -> device node
+  uvec<int64_t> node_pos;  // caller node -> device node
   std::vector<int32_t> dist_nodes;  // per class and distributed table: local node lists
   int64_t n_pnode = 0, n_ab = 0;
   int32_t n_pcell = 0;
@@ -224,21 +333,6 @@ struct cn_model {
   int64_t *d_sp_step = nullptr;
 };
 
-// std::vector that does not value-initialise (large set-up arrays are filled by all host cores)
-template <class T>
-struct NoInitAlloc {
-  using value_type = T;
-  NoInitAlloc() = default;
-  template <class U> NoInitAlloc(const NoInitAlloc<U> &) {}
-  T *allocate(size_t n) { return static_cast<T *>(::operator new(n * sizeof(T))); }
-  void deallocate(T *p, size_t) { ::operator delete(p); }
-  template <class U, class... A> void construct(U *p, A &&...a) {
-    if constexpr (sizeof...(A) == 0) ::new ((void *)p) U; else ::new ((void *)p) U(std::forward<A>(a)...);
-  }
-  template <class U> bool operator==(const NoInitAlloc<U> &) const { return true; }
-  template <class U> bool operator!=(const NoInitAlloc<U> &) const { return false; }
-};
-template <class T> using uvec = std::vector<T, NoInitAlloc<T>>;
 
 template <class T, class A>
 static int dev_upload(cn_model *m, const std::vector<T, A> &h, T **out, size_t min_elems = 1) {
@@ -322,21 +416,6 @@ static bool finite_all(const double *x, int64_t n) {
   return true;
 }
 
-// body(begin, end) over [0, n_items) on all host cores (create / first-run set-up only)
-template <class F>
-static void par_for(int64_t n_items, int64_t grain, F &&body) {
-  const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
-  const unsigned nth = (unsigned)std::min<int64_t>(hw, std::max<int64_t>(1, n_items / grain));
-  if (nth <= 1) {
-    body((int64_t)0, n_items);
-    return;
-  }
-  std::vector<std::thread> pool;
-  for (unsigned t = 0; t < nth; ++t)
-    pool.emplace_back([&body, n_items, nth, t] { body(n_items * t / nth, n_items * (t + 1) / nth); });
-  for (auto &th : pool) th.join();
-}
-
 static int build_layout(cn_model *m);
 
 extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
@@ -354,25 +433,49 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
   if (de->n_cell > 0 && (de->cell_first[0] != 0 || de->cell_first[de->n_cell] != N))
     return fail(CN_ERR_TOPOLOGY, "cell_first must start at 0 and end at n_node");
   if (de->n_cell == 0 && N != 0) return fail(CN_ERR_TOPOLOGY, "nodes without cells");
-  for (int32_t c = 0; c < de->n_cell; ++c) {
-    const int64_t f = de->cell_first[c], l = de->cell_first[c + 1];
-    if (l <= f) return fail(CN_ERR_TOPOLOGY, "cell %d is empty", c);
-    if (l - f > 65534) return fail(CN_ERR_UNSUPPORTED, "cell %d has more than 65534 nodes", c);
-    if (de->parent[f] != -1) return fail(CN_ERR_TOPOLOGY, "root of cell %d has a parent", c);
-    for (int64_t i = f + 1; i < l; ++i)
-      if (de->parent[i] < f || de->parent[i] >= i)
-        return fail(CN_ERR_TOPOLOGY, "parent[%lld] = %d violates parent < child inside cell %d",
-                    (long long)i, de->parent[i], c);
+  {  // cells: monotone cell_first first (the parallel pass below reads ranges from it)
+    FirstErr fe;
+    par_for(de->n_cell, 4096, [&](int64_t c0, int64_t c1) {
+      for (int64_t c = c0; c < c1; ++c) {
+        const int64_t f = de->cell_first[c], l = de->cell_first[c + 1];
+        if (f < 0 || l > N || l <= f) return fe.set(c, CN_ERR_TOPOLOGY, "cell %lld is empty", (long long)c);
+        if (l - f > 65534)
+          return fe.set(c, CN_ERR_UNSUPPORTED, "cell %lld has more than 65534 nodes", (long long)c);
+      }
+    });
+    if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
+    par_for(de->n_cell, 256, [&](int64_t c0, int64_t c1) {
+      for (int64_t c = c0; c < c1; ++c) {
+        const int64_t f = de->cell_first[c], l = de->cell_first[c + 1];
+        if (de->parent[f] != -1)
+          return fe.set(f, CN_ERR_TOPOLOGY, "root of cell %lld has a parent", (long long)c);
+        for (int64_t i = f + 1; i < l; ++i)
+          if (de->parent[i] < f || de->parent[i] >= i)
+            return fe.set(i, CN_ERR_TOPOLOGY,
+                          "parent[%lld] = %d violates parent < child inside cell %lld",
+                          (long long)i, de->parent[i], (long long)c);
+      }
+    });
+    if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
   }
-  if (!finite_all(de->area_um2, N) || !finite_all(de->ri_MOhm, N) ||
-      !finite_all(de->cm_uF_cm2, N) || !finite_all(de->thr_mV, de->n_cell) ||
-      !std::isfinite(de->v_init_mV) || !std::isfinite(de->celsius))
+  if (!finite_all(de->thr_mV, de->n_cell) || !std::isfinite(de->v_init_mV) ||
+      !std::isfinite(de->celsius))
     return fail(CN_ERR_ARG, "non-finite value in a node / cell array");
-  for (int64_t i = 0; i < N; ++i) {
-    if (!(de->area_um2[i] > 0.0) || !(de->cm_uF_cm2[i] > 0.0))
-      return fail(CN_ERR_ARG, "area and cm must be > 0 (node %lld)", (long long)i);
-    if (de->parent[i] >= 0 && !(de->ri_MOhm[i] > 0.0))
-      return fail(CN_ERR_ARG, "ri must be > 0 (node %lld)", (long long)i);
+  {
+    FirstErr fe;
+    par_for(N, 1 << 16, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i) {
+        const double ar = de->area_um2[i], r = de->ri_MOhm[i], c = de->cm_uF_cm2[i];
+        if (!std::isfinite(ar) || !std::isfinite(r) || !std::isfinite(c))
+          return fe.set(i, CN_ERR_ARG, "non-finite value in a node / cell array (node %lld)",
+                        (long long)i);
+        if (!(ar > 0.0) || !(c > 0.0))
+          return fe.set(i, CN_ERR_ARG, "area and cm must be > 0 (node %lld)", (long long)i);
+        if (de->parent[i] >= 0 && !(r > 0.0))
+          return fe.set(i, CN_ERR_ARG, "ri must be > 0 (node %lld)", (long long)i);
+      }
+    });
+    if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
   }
   for (int32_t t = 0; t < de->n_mech; ++t) {
     const cn_mech_table &mt = de->mech[t];
@@ -384,41 +487,59 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
     if (mt.n > 0 && (!mt.node || (ti.n_param > 0 && !mt.param)))
       return fail(CN_ERR_MECH, "table %d: NULL array", t);
     if (ti.n_global > 0 && !mt.global) return fail(CN_ERR_MECH, "table %d: NULL globals", t);
-    for (int64_t i = 0; i < mt.n; ++i)
-      if (mt.node[i] < 0 || mt.node[i] >= N)
-        return fail(CN_ERR_MECH, "table %d: node of instance %lld out of range", t, (long long)i);
-    if (!finite_all(mt.param, mt.n * ti.n_param) || !finite_all(mt.global, ti.n_global))
+    if (!finite_all(mt.global, ti.n_global))
       return fail(CN_ERR_MECH, "table %d: non-finite parameter", t);
-    if (mt.type == CN_EXP2SYN)
-      for (int64_t i = 0; i < mt.n; ++i)
-        if (!(mt.param[i] > 0.0) || !(mt.param[mt.n + i] > mt.param[i]))
-          return fail(CN_ERR_MECH, "table %d: Exp2Syn needs 0 < tau1 < tau2", t);
-    if (mt.type == CN_EXPSYN)
-      for (int64_t i = 0; i < mt.n; ++i)
-        if (!(mt.param[i] > 0.0)) return fail(CN_ERR_MECH, "table %d: ExpSyn needs tau > 0", t);
-    if (mt.type == CN_GAP)
-      for (int64_t i = 0; i < mt.n; ++i) {
-        const double pr = mt.param[mt.n + i];
-        if (!(pr >= 0.0 && pr < (double)N) || pr != (double)(int64_t)pr)
-          return fail(CN_ERR_MECH, "table %d: gap junction %lld has no such peer node", t,
-                      (long long)i);
+    FirstErr fe;
+    par_for(mt.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i) {
+        if (mt.node[i] < 0 || mt.node[i] >= N)
+          return fe.set(i, CN_ERR_MECH, "table %d: node of instance %lld out of range", t,
+                        (long long)i);
+        for (int j = 0; j < ti.n_param; ++j)
+          if (!std::isfinite(mt.param[(int64_t)j * mt.n + i]))
+            return fe.set(i, CN_ERR_MECH, "table %d: non-finite parameter", t);
+        if (mt.type == CN_EXP2SYN && (!(mt.param[i] > 0.0) || !(mt.param[mt.n + i] > mt.param[i])))
+          return fe.set(i, CN_ERR_MECH, "table %d: Exp2Syn needs 0 < tau1 < tau2", t);
+        if (mt.type == CN_EXPSYN && !(mt.param[i] > 0.0))
+          return fe.set(i, CN_ERR_MECH, "table %d: ExpSyn needs tau > 0", t);
+        if (mt.type == CN_GAP) {
+          const double pr = mt.param[mt.n + i];
+          if (!(pr >= 0.0 && pr < (double)N) || pr != (double)(int64_t)pr)
+            return fe.set(i, CN_ERR_MECH, "table %d: gap junction %lld has no such peer node", t,
+                          (long long)i);
+        }
       }
+    });
+    if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
   }
   if (de->n_netcon < 0 || de->n_stim < 0) return fail(CN_ERR_NETCON, "negative count");
   int32_t n_src = de->n_cell;
-  for (int64_t i = 0; i < de->n_netcon; ++i) {
-    const int32_t tm = de->nc_tgt_mech[i];
-    if (tm < 0 || tm >= de->n_mech) return fail(CN_ERR_NETCON, "netcon %lld: bad table", (long long)i);
-    const int ty = de->mech[tm].type;
-    if (ty != CN_EXPSYN && ty != CN_EXP2SYN && ty != CN_AMPANMDA)
-      return fail(CN_ERR_NETCON, "netcon %lld: target type %d receives no events", (long long)i, ty);
-    if (de->nc_tgt_inst[i] < 0 || de->nc_tgt_inst[i] >= de->mech[tm].n)
-      return fail(CN_ERR_NETCON, "netcon %lld: target instance out of range", (long long)i);
-    if (de->nc_src_gid[i] < 0) return fail(CN_ERR_NETCON, "netcon %lld: negative source", (long long)i);
-    if (!std::isfinite(de->nc_weight_uS[i]) || !std::isfinite(de->nc_delay_ms[i]) ||
-        !(de->nc_delay_ms[i] > 0.0))
-      return fail(CN_ERR_NETCON, "netcon %lld: weight / delay invalid", (long long)i);
-    n_src = std::max(n_src, de->nc_src_gid[i] + 1);
+  {
+    FirstErr fe;
+    std::mutex mu;
+    par_for(de->n_netcon, 1 << 16, [&](int64_t i0, int64_t i1) {
+      int32_t hi = 0;
+      for (int64_t i = i0; i < i1; ++i) {
+        const int32_t tm = de->nc_tgt_mech[i];
+        if (tm < 0 || tm >= de->n_mech)
+          return fe.set(i, CN_ERR_NETCON, "netcon %lld: bad table", (long long)i);
+        const int ty = de->mech[tm].type;
+        if (ty != CN_EXPSYN && ty != CN_EXP2SYN && ty != CN_AMPANMDA)
+          return fe.set(i, CN_ERR_NETCON, "netcon %lld: target type %d receives no events",
+                        (long long)i, ty);
+        if (de->nc_tgt_inst[i] < 0 || de->nc_tgt_inst[i] >= de->mech[tm].n)
+          return fe.set(i, CN_ERR_NETCON, "netcon %lld: target instance out of range", (long long)i);
+        if (de->nc_src_gid[i] < 0)
+          return fe.set(i, CN_ERR_NETCON, "netcon %lld: negative source", (long long)i);
+        if (!std::isfinite(de->nc_weight_uS[i]) || !std::isfinite(de->nc_delay_ms[i]) ||
+            !(de->nc_delay_ms[i] > 0.0))
+          return fe.set(i, CN_ERR_NETCON, "netcon %lld: weight / delay invalid", (long long)i);
+        hi = std::max(hi, de->nc_src_gid[i] + 1);
+      }
+      std::lock_guard<std::mutex> lk(mu);
+      n_src = std::max(n_src, hi);
+    });
+    if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
   }
   for (int64_t i = 0; i < de->n_stim; ++i) {
     if (de->stim_gid[i] < de->n_cell)
@@ -435,10 +556,10 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
     m->N = N;
     m->cell_first.assign(de->cell_first, de->cell_first + (de->n_cell ? de->n_cell + 1 : 0));
     if (de->n_cell == 0) m->cell_first.assign(1, 0);
-    m->parent.assign(de->parent, de->parent + N);
-    m->area.assign(de->area_um2, de->area_um2 + N);
-    m->ri.assign(de->ri_MOhm, de->ri_MOhm + N);
-    m->cm.assign(de->cm_uF_cm2, de->cm_uF_cm2 + N);
+    par_assign(m->parent, de->parent, N);
+    par_assign(m->area, de->area_um2, N);
+    par_assign(m->ri, de->ri_MOhm, N);
+    par_assign(m->cm, de->cm_uF_cm2, N);
     m->thr.assign(de->thr_mV, de->thr_mV + de->n_cell);
     m->v_init = de->v_init_mV;
     m->celsius = de->celsius;
@@ -449,16 +570,16 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
       T.type = mt.type;
       type_info(mt.type, T.ti);
       T.n = mt.n;
-      T.node.assign(mt.node, mt.node + mt.n);
-      T.param.assign(mt.param, mt.param + mt.n * T.ti.n_param);
+      par_assign(T.node, mt.node, mt.n);
+      par_assign(T.param, mt.param, mt.n * T.ti.n_param);
       T.glob.assign(mt.global, mt.global + T.ti.n_global);
     }
     m->n_netcon = de->n_netcon;
-    m->nc_src.assign(de->nc_src_gid, de->nc_src_gid + de->n_netcon);
-    m->nc_tgt_mech.assign(de->nc_tgt_mech, de->nc_tgt_mech + de->n_netcon);
-    m->nc_tgt_inst.assign(de->nc_tgt_inst, de->nc_tgt_inst + de->n_netcon);
-    m->nc_w.assign(de->nc_weight_uS, de->nc_weight_uS + de->n_netcon);
-    m->nc_delay.assign(de->nc_delay_ms, de->nc_delay_ms + de->n_netcon);
+    par_assign(m->nc_src, de->nc_src_gid, de->n_netcon);
+    par_assign(m->nc_tgt_mech, de->nc_tgt_mech, de->n_netcon);
+    par_assign(m->nc_tgt_inst, de->nc_tgt_inst, de->n_netcon);
+    par_assign(m->nc_w, de->nc_weight_uS, de->n_netcon);
+    par_assign(m->nc_delay, de->nc_delay_ms, de->n_netcon);
     m->stim_gid.assign(de->stim_gid, de->stim_gid + de->n_stim);
     m->stim_t.assign(de->stim_t_ms, de->stim_t_ms + de->n_stim);
     m->n_src = n_src;
@@ -504,27 +625,34 @@ static int build_layout(cn_model *m) {
   const int64_t N = m->N;
   const int nt = (int)m->tab.size();
   // node -> cell
-  std::vector<int32_t> cell_of(N);
-  for (int32_t c = 0; c < nc; ++c)
-    for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of[i] = c;
+  uvec<int32_t> cell_of((size_t)N);
+  par_for(nc, 256, [&](int64_t c0, int64_t c1) {
+    for (int64_t c = c0; c < c1; ++c)
+      for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of[i] = (int32_t)c;
+  });
   // per distributed table: CSR of instances per cell, sorted by local node
   for (int t = 0; t < nt; ++t) {
     HTable &T = m->tab[t];
     if (T.ti.point) continue;
-    T.cell_first.assign((size_t)nc + 1, 0);
-    for (int64_t i = 0; i < T.n; ++i) T.cell_first[cell_of[T.node[i]] + 1]++;
-    for (int32_t c = 0; c < nc; ++c) T.cell_first[c + 1] += T.cell_first[c];
+    uvec<int64_t> rank;
+    par_bucket(T.n, nc, [&](int64_t i) { return cell_of[T.node[i]]; }, T.cell_first, rank);
     T.cell_inst.resize((size_t)T.n);
-    std::vector<int64_t> fill(T.cell_first.begin(), T.cell_first.end() - 1);
-    for (int64_t i = 0; i < T.n; ++i) T.cell_inst[fill[cell_of[T.node[i]]]++] = i;
-    for (int32_t c = 0; c < nc; ++c) {
-      auto b = T.cell_inst.begin() + T.cell_first[c], e = T.cell_inst.begin() + T.cell_first[c + 1];
-      if (!std::is_sorted(b, e, [&](int64_t x, int64_t y) { return T.node[x] < T.node[y]; }))
-        std::sort(b, e, [&](int64_t x, int64_t y) { return T.node[x] < T.node[y]; });
-      for (auto it = b; it != e && it + 1 != e; ++it)
-        if (T.node[*it] == T.node[*(it + 1)])
-          return fail(CN_ERR_MECH, "table %d: two instances on node %d", t, T.node[*it]);
-    }
+    par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i) T.cell_inst[rank[i]] = i;
+    });
+    FirstErr fe;
+    par_for(nc, 256, [&](int64_t c0, int64_t c1) {
+      for (int64_t c = c0; c < c1; ++c) {
+        auto b = T.cell_inst.begin() + T.cell_first[c], e = T.cell_inst.begin() + T.cell_first[c + 1];
+        if (!std::is_sorted(b, e, [&](int64_t x, int64_t y) { return T.node[x] < T.node[y]; }))
+          std::sort(b, e, [&](int64_t x, int64_t y) { return T.node[x] < T.node[y]; });
+        for (auto it = b; it != e && it + 1 != e; ++it)
+          if (T.node[*it] == T.node[*(it + 1)])
+            return fe.set(T.node[*it], CN_ERR_MECH, "table %d: two instances on node %d", t,
+                          T.node[*it]);
+      }
+    });
+    if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
   }
   lap("node -> cell, instance CSR");
   // shape signature per cell: topology + placement of every distributed table
@@ -826,7 +954,7 @@ static int build_layout(cn_model *m) {
   // groups: cooperative groups first, then tape groups
   m->cell_grp.assign(nc, -1);
   m->cell_slot.assign(nc, 0);
-  m->node_pos.assign((size_t)N, -1);
+  m->node_pos.resize((size_t)N);
   int64_t node_base = 0, ab_base = 0;
   int32_t cell_base = 0;
   for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
@@ -843,8 +971,6 @@ static int build_layout(cn_model *m) {
         const int32_t cell = K.cells[q + c];
         m->cell_grp[cell] = gidx;
         m->cell_slot[cell] = c;
-        const int64_t f = m->cell_first[cell];
-        for (int i = 0; i < K.n; ++i) m->node_pos[f + i] = ab_base + K.node_off[i] + c;
       }
       m->grp.push_back(gi);
       node_base += (int64_t)K.n * K.G;
@@ -872,10 +998,6 @@ static int build_layout(cn_model *m) {
         const int32_t cell = K.cells[(int64_t)gq * 32 + c];
         m->cell_grp[cell] = gidx;
         m->cell_slot[cell] = c;
-        const int64_t f = m->cell_first[cell];
-        for (int i = 0; i < K.n; ++i)
-          m->node_pos[f + i] =
-              m->n_ab + tape_base + ((int64_t)K.tp.row[K.tp.pos_of[i]] + 4) * 32 + c;
       }
       m->tgrp.push_back(tg);
       tape_base += (int64_t)K.tp.n_rows * 32;
@@ -887,46 +1009,71 @@ static int build_layout(cn_model *m) {
     return fail(CN_ERR_UNSUPPORTED, "tape larger than 2^32 doubles");
   m->n_pcell = cell_base;
   const int ng = ngc + (int)m->tgrp.size();
+  // caller node -> element of the voltage arena
+  par_for(nc, 256, [&](int64_t c0, int64_t c1) {
+    for (int64_t cell = c0; cell < c1; ++cell) {
+      const int g = m->cell_grp[cell];
+      const int c = m->cell_slot[cell];
+      const int64_t f = m->cell_first[cell];
+      if (g < ngc) {
+        const GroupInfo &gi = m->grp[g];
+        const HClass &K = m->cls[gi.cls];
+        for (int i = 0; i < K.n; ++i) m->node_pos[f + i] = gi.ab_base + K.node_off[i] + c;
+      } else {
+        const TapeGroup &tg = m->tgrp[g - ngc];
+        const HClass &K = m->cls[tg.cls];
+        for (int i = 0; i < K.n; ++i)
+          m->node_pos[f + i] =
+              m->n_ab + tg.tape_base + ((int64_t)K.tp.row[K.tp.pos_of[i]] + 4) * 32 + c;
+      }
+    }
+  });
   // per-table instance layout
   std::vector<int32_t> dist_nodes;
   for (int t = 0; t < nt; ++t) {
     HTable &T = m->tab[t];
-    T.inst_pos.assign((size_t)T.n, -1);
+    T.inst_pos.resize((size_t)T.n);
+    par_for(T.n, 1 << 18, [&](int64_t i0, int64_t i1) {
+      std::fill(T.inst_pos.begin() + i0, T.inst_pos.begin() + i1, (int64_t)-1);
+    });
     if (T.ti.point) {
       // instances ordered by group (stable); cooperative groups: slot = local node * G + cell
       // slot in shared memory; tape groups: element of the node's conductance row on the tape
-      T.pp_first.assign((size_t)ng + 1, 0);
-      for (int64_t i = 0; i < T.n; ++i) T.pp_first[m->cell_grp[cell_of[T.node[i]]] + 1]++;
-      for (int g = 0; g < ng; ++g) T.pp_first[g + 1] += T.pp_first[g];
-      std::vector<int64_t> fill(T.pp_first.begin(), T.pp_first.end() - 1);
-      T.pp_slot.assign((size_t)T.n, 0);
-      T.pp_wslot.assign((size_t)T.n, 0);
-      for (int64_t i = 0; i < T.n; ++i) {
-        const int32_t cell = cell_of[T.node[i]];
-        const int g = m->cell_grp[cell];
-        const int64_t pos = fill[g]++;
-        T.inst_pos[i] = pos;
-        const int32_t local = (int32_t)(T.node[i] - m->cell_first[cell]);
-        if (g < ngc) {
-          const int G = m->cls[m->grp[g].cls].G;
-          // element of the node's row pair in ppdr (schedule order, rows of 32 + 32)
-          const int64_t sp = m->grp[g].ab_base + m->cls[m->grp[g].cls].node_off[local] +
-                             m->cell_slot[cell];
-          (void)G;
-          T.pp_slot[pos] = (int32_t)(uint32_t)((sp >> 5) * 64 + (sp & 31));
-        } else {
-          const TapeGroup &tg = m->tgrp[g - ngc];
-          const int64_t el = tg.tape_base + (int64_t)m->cls[tg.cls].tp.pp_row[local] * 32 +
-                             m->cell_slot[cell];
-          T.pp_slot[pos] = (int32_t)(uint32_t)el;
-          T.pp_wslot[pos] = (uint32_t)(tg.pp_base + (int64_t)m->cls[tg.cls].tp.pp_ord[local] * 64 +
-                                       m->cell_slot[cell]);
+      uvec<int64_t> rank;
+      par_bucket(T.n, ng, [&](int64_t i) { return m->cell_grp[cell_of[T.node[i]]]; }, T.pp_first,
+                 rank);
+      T.pp_slot.resize((size_t)T.n);
+      T.pp_wslot.resize((size_t)T.n);
+      par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+        for (int64_t i = i0; i < i1; ++i) {
+          const int32_t cell = cell_of[T.node[i]];
+          const int g = m->cell_grp[cell];
+          const int64_t pos = rank[i];
+          T.inst_pos[i] = pos;
+          const int32_t local = (int32_t)(T.node[i] - m->cell_first[cell]);
+          if (g < ngc) {
+            // element of the node's row pair in ppdr (schedule order, rows of 32 + 32)
+            const int64_t sp = m->grp[g].ab_base + m->cls[m->grp[g].cls].node_off[local] +
+                               m->cell_slot[cell];
+            T.pp_slot[pos] = (int32_t)(uint32_t)((sp >> 5) * 64 + (sp & 31));
+            T.pp_wslot[pos] = 0;
+          } else {
+            const TapeGroup &tg = m->tgrp[g - ngc];
+            const int64_t el = tg.tape_base + (int64_t)m->cls[tg.cls].tp.pp_row[local] * 32 +
+                               m->cell_slot[cell];
+            T.pp_slot[pos] = (int32_t)(uint32_t)el;
+            T.pp_wslot[pos] = (uint32_t)(tg.pp_base + (int64_t)m->cls[tg.cls].tp.pp_ord[local] * 64 +
+                                         m->cell_slot[cell]);
+          }
         }
-      }
+      });
       T.pp_tape_begin = T.pp_first[ngc];
       T.n_dev = T.n;
     } else {
-      T.tape_loc.assign((size_t)T.n, -1);
+      T.tape_loc.resize((size_t)T.n);
+      par_for(T.n, 1 << 18, [&](int64_t i0, int64_t i1) {
+        std::fill(T.tape_loc.begin() + i0, T.tape_loc.begin() + i1, (int64_t)-1);
+      });
       T.cls_cnt.assign(m->cls.size(), 0);
       T.cls_nodeoff.assign(m->cls.size(), 0);
       for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
@@ -947,7 +1094,8 @@ static int build_layout(cn_model *m) {
         base += (int64_t)cnt * K.G;
       }
       T.n_dev = base;
-      for (int32_t c = 0; c < nc; ++c) {
+      par_for(nc, 256, [&](int64_t cc0, int64_t cc1) {
+       for (int64_t c = cc0; c < cc1; ++c) {
         const int g = m->cell_grp[c];
         if (g < ngc) {
           const int G = m->cls[m->grp[g].cls].G;
@@ -964,7 +1112,8 @@ static int build_layout(cn_model *m) {
             T.tape_loc[i] = tg.tape_base + (int64_t)P.tab_row[t][local] * 32 + m->cell_slot[c];
           }
         }
-      }
+       }
+      });
     }
   }
   m->dist_nodes = std::move(dist_nodes);
