@@ -693,22 +693,47 @@ static int build_layout(cn_model *m) {
   };
   m->cell_cls.assign(nc, -1);
   {
-    std::unordered_map<uint64_t, std::vector<int>> by_sig;
-    by_sig.reserve((size_t)nc / 8 + 16);
+    // buckets of equal signature (cheap, in cell order), then the exact comparison inside every
+    // bucket on all cores; classes are numbered in the order of their first cell
+    std::unordered_map<uint64_t, int> bucket_of;
+    bucket_of.reserve((size_t)nc / 8 + 16);
+    std::vector<std::vector<int32_t>> bcells;
     for (int32_t c = 0; c < nc; ++c) {
-      auto &cands = by_sig[sig[c]];
-      int found = -1;
-      for (int k : cands)
-        if (same_shape(m->cls[k].rep_cell, c)) { found = k; break; }
-      if (found < 0) {
-        found = (int)m->cls.size();
-        m->cls.emplace_back();
-        m->cls.back().rep_cell = c;
-        m->cls.back().n = (int)(m->cell_first[c + 1] - m->cell_first[c]);
-        cands.push_back(found);
+      auto it = bucket_of.find(sig[c]);
+      if (it == bucket_of.end()) {
+        it = bucket_of.emplace(sig[c], (int)bcells.size()).first;
+        bcells.emplace_back();
       }
-      m->cls[found].cells.push_back(c);
-      m->cell_cls[c] = found;
+      bcells[it->second].push_back(c);
+    }
+    std::vector<std::vector<std::vector<int32_t>>> bcls(bcells.size());
+    par_for((int64_t)bcells.size(), 4, [&](int64_t b0, int64_t b1) {
+      for (int64_t b = b0; b < b1; ++b)
+        for (int32_t c : bcells[b]) {
+          std::vector<int32_t> *hit = nullptr;
+          for (auto &k : bcls[b])
+            if (same_shape(k[0], c)) { hit = &k; break; }
+          if (!hit) {
+            bcls[b].emplace_back();
+            hit = &bcls[b].back();
+          }
+          hit->push_back(c);
+        }
+    });
+    std::vector<std::vector<int32_t> *> all;
+    for (auto &b : bcls)
+      for (auto &k : b) all.push_back(&k);
+    std::sort(all.begin(), all.end(),
+              [](const std::vector<int32_t> *x, const std::vector<int32_t> *y) { return (*x)[0] < (*y)[0]; });
+    m->cls.reserve(all.size());
+    for (auto *k : all) {
+      const int id = (int)m->cls.size();
+      m->cls.emplace_back();
+      HClass &K = m->cls.back();
+      K.rep_cell = (*k)[0];
+      K.n = (int)(m->cell_first[K.rep_cell + 1] - m->cell_first[K.rep_cell]);
+      K.cells.assign(k->begin(), k->end());
+      for (int32_t c : *k) m->cell_cls[c] = id;
     }
   }
   // which tables need ica / cai
@@ -1215,23 +1240,44 @@ static int finalize(cn_model *m, double dt) {
           rsum[T.node[i]] += g * e;
         }
       });
-  par_for(N, 65536, [&](int64_t i0, int64_t i1) {
-    for (int64_t i = i0; i < i1; ++i) {
-      const int64_t q = m->node_pos[i];
-      if (m->cell_tape[cell_of_node[i]]) {  // q is the node's v element; a, b, d, r precede it
-        double *rec = v0.data() + q;
-        rec[-4 * 32] = an[i];
-        rec[-3 * 32] = bn[i];
-        rec[-2 * 32] = dsum[i] * invc[i];
-        rec[-1 * 32] = rsum[i] * invc[i];
-        rec[0] = m->v_init;
-      } else {
+  // inverse map: (group, slot) -> caller cell
+  std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
+  for (int32_t c = 0; c < m->n_cell; ++c) {
+    const int g = m->cell_grp[c];
+    const int32_t cb = g < m->n_cgroup ? m->grp[g].cell_base : m->tgrp[g - m->n_cgroup].cell_base;
+    cell_of_pcell[cb + m->cell_slot[c]] = c;
+  }
+  // interleaved groups: whole rows of 32 lanes at a time (contiguous writes; the 32 cells are
+  // read as 32 sequential streams); a, b, d, r precede the node's v row
+  par_for((int64_t)m->tgrp.size(), 1, [&](int64_t g0, int64_t g1) {
+    for (int64_t g = g0; g < g1; ++g) {
+      const TapeGroup &tg = m->tgrp[g];
+      const HClass &K = m->cls[tg.cls];
+      int64_t f[32];
+      for (int l = 0; l < tg.ncell; ++l) f[l] = m->cell_first[cell_of_pcell[tg.cell_base + l]];
+      for (int j = 0; j < K.n; ++j) {
+        double *rec = tape + tg.tape_base + ((int64_t)K.tp.row[K.tp.pos_of[j]] + 4) * 32;
+        for (int l = 0; l < tg.ncell; ++l) {
+          const int64_t i = f[l] + j;
+          rec[-4 * 32 + l] = an[i];
+          rec[-3 * 32 + l] = bn[i];
+          rec[-2 * 32 + l] = dsum[i] * invc[i];
+          rec[-1 * 32 + l] = rsum[i] * invc[i];
+          rec[l] = m->v_init;
+        }
+      }
+    }
+  });
+  if (m->n_cgroup > 0)
+    par_for(N, 65536, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i) {
+        if (m->cell_tape[cell_of_node[i]]) continue;
+        const int64_t q = m->node_pos[i];
         dstat[q] = dsum[i] * invc[i];
         rstat[q] = rsum[i] * invc[i];
         v0[q] = m->v_init;
       }
-    }
-  });
+    });
   lap("static rows");
   // idle lanes of a ragged tape group: unit diagonal, everything else zero; cai rows
   for (const TapeGroup &tg : m->tgrp) {
@@ -1267,13 +1313,6 @@ static int finalize(cn_model *m, double dt) {
     cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, K.nodeoff_off, 0};
     sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
     nodeoff_all.insert(nodeoff_all.end(), K.node_off.begin(), K.node_off.end());
-  }
-  // inverse map: (group, slot) -> caller cell
-  std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
-  for (int32_t c = 0; c < m->n_cell; ++c) {
-    const int g = m->cell_grp[c];
-    const int32_t cb = g < m->n_cgroup ? m->grp[g].cell_base : m->tgrp[g - m->n_cgroup].cell_base;
-    cell_of_pcell[cb + m->cell_slot[c]] = c;
   }
   for (int g = 0; g < ng; ++g) {
     const GroupInfo &gi = m->grp[g];
@@ -1375,12 +1414,18 @@ static int finalize(cn_model *m, double dt) {
     }
     if (T.type == CN_PAS) continue;  // folded
     const int64_t nd = T.n_dev;
-    std::vector<std::vector<double>> par(T.ti.n_dev_param, std::vector<double>((size_t)nd, 0.0));
-    std::vector<std::vector<double>> st(T.ti.n_state, std::vector<double>((size_t)nd, 0.0));
-    // benign padding for distributed tables
-    if (!T.ti.point && T.ti.n_dev_param > 0)
-      std::fill(par[T.ti.n_dev_param - 1].begin(), par[T.ti.n_dev_param - 1].end(), 1.0);
-    for (int64_t i = 0; i < T.n; ++i) {
+    std::vector<uvec<double>> par(T.ti.n_dev_param), st(T.ti.n_state);
+    for (auto &x : par) x.resize((size_t)nd);
+    for (auto &x : st) x.resize((size_t)nd);
+    par_for(nd, 1 << 18, [&](int64_t i0, int64_t i1) {
+      for (int j = 0; j < T.ti.n_dev_param; ++j)  // benign padding for distributed tables
+        std::fill(par[j].begin() + i0, par[j].begin() + i1,
+                  !T.ti.point && j == T.ti.n_dev_param - 1 ? 1.0 : 0.0);
+      for (auto &x : st) std::fill(x.begin() + i0, x.begin() + i1, 0.0);
+    });
+    // instances are independent (each writes its own elements): all host cores
+    par_for(T.n, 4096, [&](int64_t ii0, int64_t ii1) {
+     for (int64_t i = ii0; i < ii1; ++i) {
       const int32_t nd_i = T.node[i];
       double P[CN_MAX_PARAM] = {0.0}, S[CN_MAX_STATE] = {0.0};
       for (int j = 0; j < T.ti.n_param; ++j) P[j] = T.param[(size_t)j * T.n + i];
@@ -1437,7 +1482,8 @@ static int finalize(cn_model *m, double dt) {
         for (int j = 0; j < T.ti.n_dev_param; ++j) par[j][q] = P[j];
         for (int j = 0; j < T.ti.n_state; ++j) st[j][q] = S[j];
       }
-    }
+     }
+    });
     for (int j = 0; j < T.ti.n_dev_param; ++j) { UP(par[j], T.d_param[j]); D.param[j] = T.d_param[j]; }
     for (int j = 0; j < T.ti.n_state; ++j) { UP(st[j], T.d_state[j]); D.state[j] = T.d_state[j]; }
     if (T.ti.point) {
