@@ -83,6 +83,34 @@ def test_validation_errors():
     pas = dict(d["mechs"][1]); pas["node"] = pas["node"].copy(); pas["node"][1] = pas["node"][0]
     d["mechs"][1] = pas
     _expect(d, -3)
+    # gap junction without a peer node
+    for bad in (488.0, -1.0, 2.5):
+        d = dict(base)
+        d["mechs"] = list(base["mechs"]) + [
+            {"type": "gap", "node": np.array([3], np.int32),
+             "params": {"g": np.array([0.01]), "peer": np.array([bad])}, "globals": {}}]
+        _expect(d, -3)
+
+
+def test_validation_on_all_cores_reports_the_first_failure():
+    """The validation passes run on all host cores over a model large enough to be split; the
+    failure with the smallest index is the one reported, whatever thread found it."""
+    base = W.config4(n_cell=2048, n_types=8)
+    n = len(base["parent"])
+    assert n > 8 * 65536                       # several ranges per pass
+    d = dict(base); d["area"] = base["area"].copy()
+    for i in (n - 5, n // 2, 70001):
+        d["area"][i] = -1.0
+    with pytest.raises(cn.CnError) as e:
+        cn.Model(d)
+    assert e.value.code == -1 and "node 70001)" in str(e.value)
+    d = dict(base); d["parent"] = base["parent"].copy()
+    cf = base["cell_first"]
+    for c in (1900, 700):
+        d["parent"][cf[c] + 4] = cf[c] + 9
+    with pytest.raises(cn.CnError) as e:
+        cn.Model(d)
+    assert e.value.code == -2 and "cell 700" in str(e.value)
 
 
 def test_no_cpu_fallback():
