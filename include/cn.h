@@ -112,8 +112,8 @@ int cn_model_create(const cn_model_desc *desc, cn_model **out);
  * (K <= 0 is a no-op).  dt is fixed by the first call.  Runs on `stream` set by cn_set_stream
  * (default: the legacy default stream) and synchronises it before returning.
  * Launch granularity is an internal matter with identical results: one set of launches per dt,
- * or -- when every cell runs on the interleaved kernel, no point process depends on v within a
- * step and no per-step probe is set -- one launch per window of up to min-delay steps (L62
+ * or -- when every cell runs on the interleaved kernel and no point process depends on v within
+ * a step (AMPA+NMDA, gap junctions do) -- one launch per window of up to min-delay steps (L62
  * "every minimum spike delay interval"). */
 int cn_run(cn_model *m, double tstop_ms, double dt_ms);
 
@@ -131,8 +131,9 @@ int cn_get_v(const cn_model *m, double *v_out, int64_t n);
  * step k+1.  Pass cap = 0 to query *n_out only. */
 int cn_get_spikes(const cn_model *m, int32_t *gid, int64_t *step, int64_t cap, int64_t *n_out);
 
-/* Record v of the given nodes after every step (before the first cn_run only).  Probes make
- * cn_run launch once per dt (a probe kernel follows every step). */
+/* Record v of the given nodes after every step (before the first cn_run only): by a probe
+ * kernel after every step, or, in window mode, by the interleaved kernel itself when a group
+ * completes a step. */
 int cn_set_probes(cn_model *m, const int32_t *node, int64_t n, int64_t max_steps);
 /* trace_out[s*n_probe + j] = v(node j) after step s; *n_steps_out = steps recorded. */
 int cn_get_trace(const cn_model *m, double *trace_out, int64_t cap_steps, int64_t *n_steps_out);

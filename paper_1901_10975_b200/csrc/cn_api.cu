@@ -1595,9 +1595,10 @@ static int finalize(cn_model *m, double dt) {
   }
   lap("netcons");
   // window mode: every cell on the interleaved kernel, no point process whose current depends on
-  // v (AMPA+NMDA, gap junctions), no per-step probes; a window is at most the smallest delay long
+  // v (AMPA+NMDA, gap junctions); a window is at most the smallest delay long (probes are
+  // recorded by the kernel itself then)
   {
-    bool ok = m->hm.n_tgroup > 0 && m->grp.empty() && m->probe.empty();
+    bool ok = m->hm.n_tgroup > 0 && m->grp.empty();
     for (const HTable &T : m->tab)
       if ((T.type == CN_AMPANMDA || T.type == CN_GAP) && T.n > 0) ok = false;
     if (const char *e = std::getenv("CN_TAPE_WINDOW")) ok = ok && std::atoi(e) != 0;
@@ -1637,6 +1638,33 @@ static int finalize(cn_model *m, double dt) {
     UP(pp, m->d_probe_pos);
     rc = dev_alloc(m, (size_t)(m->probe_cap * (int64_t)m->probe.size()), &m->d_trace, false);
     if (rc) return rc;
+    if (m->window) {  // the probes of every group: the interleaved kernel records them per step
+      const int ntg = (int)m->tgrp.size();
+      std::vector<int32_t> first((size_t)ntg + 1, 0), col(m->probe.size());
+      std::vector<int64_t> pos(m->probe.size());
+      std::vector<int32_t> grp_of(m->probe.size());
+      for (size_t j = 0; j < m->probe.size(); ++j) {
+        const int64_t nd = m->probe[j];
+        const int32_t c = (int32_t)(std::upper_bound(m->cell_first.begin(), m->cell_first.end(), nd) -
+                                    m->cell_first.begin()) - 1;
+        grp_of[j] = m->cell_grp[c] - m->n_cgroup;
+        first[grp_of[j] + 1]++;
+      }
+      for (int g = 0; g < ntg; ++g) first[g + 1] += first[g];
+      std::vector<int32_t> fill(first.begin(), first.end() - 1);
+      for (size_t j = 0; j < m->probe.size(); ++j) {
+        const int32_t q = fill[grp_of[j]]++;
+        pos[q] = pp[j];
+        col[q] = (int32_t)j;
+      }
+      int32_t *df, *dc;
+      int64_t *dp;
+      UP(first, df); UP(pos, dp); UP(col, dc);
+      H.wp_first = df; H.wp_pos = dp; H.wp_col = dc;
+      H.trace = m->d_trace;
+      H.trace_cap = m->probe_cap;
+      H.n_probe = (int32_t)m->probe.size();
+    }
   }
 #undef UP
   CU(cudaEventCreate(&m->ev0));
@@ -1750,6 +1778,8 @@ static int run_steps(cn_model *m, int64_t K) {
       }
       const bool timeit = m->ktime_every > 0 && m->ktime_used < m->ktime_ev.size();
       if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
+      m->hm.trace_row0 = m->probe_rows;
+      if (!m->probe.empty()) m->probe_rows = std::min(m->probe_cap, m->probe_rows + n);
       cudaError_t e = launch_tape(m, k, (m->state_pending ? TM_ADVANCE : 0) | TM_WINDOW, n);
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
       if (timeit) {

@@ -167,6 +167,14 @@ struct DModel {
   int64_t win_mark_cap;         // length of the two rings below
   int64_t *win_mark_step;       // ring: first step of the recent windows
   int64_t *win_mark_nsp;        //            and the length of the spike list at their start
+  // probes recorded by the interleaved kernel itself in window mode (null otherwise): per group
+  // the probed nodes (element of the voltage arena) and their column of the trace
+  const int32_t *wp_first;      // [n_tgroup + 1]
+  const int64_t *wp_pos;
+  const int32_t *wp_col;
+  double *trace;                // [trace_cap][n_probe]
+  int64_t trace_row0, trace_cap;  // row of the first step of this launch
+  int32_t n_probe, pad3;
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
 };

@@ -28,8 +28,9 @@
 //   * One launch integrates a WINDOW of up to min-delay steps (L62): (step, group) work items are
 //     handed out by a ticket counter, a group's next step may run on another SM once the previous
 //     one is published (release / acquire through L2).  Events and point processes of the window
-//     are prepared by deliver_window_kernel / pp_window_kernel (cn_device.cuh); with per-step
-//     probes or cells on the other kernel: one launch per dt, pp_step_kernel in front.
+//     are prepared by deliver_window_kernel / pp_window_kernel (cn_device.cuh), probed voltages
+//     are recorded at the end of every (step, group) item; with cells on the other kernel or
+//     point processes that depend on v: one launch per dt, pp_step_kernel in front.
 //   * Control is uniform across a warp; lanes never diverge.
 // Host side: cn_tape_program.hpp compiles the per-class programs; DESIGN.md 5.1 has the rationale
 // and profiles/r01_README.md the measurements behind every choice.
@@ -626,6 +627,13 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     }
     CN_TR(4);
     __syncthreads();  // the system rows of this group are dead from here on
+    if (M.wp_first && !flush) {  // window mode: the probed voltages of this (step, group)
+      const int64_t row = M.trace_row0 + step_in;
+      if (row < M.trace_cap)
+        for (int p = M.wp_first[g] + (int)threadIdx.x; p < M.wp_first[g + 1]; p += (int)blockDim.x)
+          M.trace[row * M.n_probe + M.wp_col[p]] =
+              *reinterpret_cast<const volatile double *>(M.v + M.wp_pos[p]);  // (never from L1)
+    }
     // the signal mbarriers this program did not use complete their phase too
     for (int b = (flush ? 0 : tc.n_bar) + (int)threadIdx.x; b < NB; b += (int)blockDim.x)
       mbar_arrive(sbar_s + 8 * b);

@@ -26,14 +26,18 @@ def cn():
     return cn
 
 
-@pytest.fixture(params=["coop", "tape", "tape-w1", "tape-w4"])
+@pytest.fixture(params=["coop", "tape", "tape-step", "tape-w1", "tape-w4"])
 def strategy(request, monkeypatch):
     """Both kernels on the same inputs: warp-cooperative groups, or every cell on the interleaved
-    (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1), with 2 (default), 1 or 4 warps
-    (subtree tasks) per group of 32 cells."""
+    (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1), with 8 (default), 1 or 4 warps
+    (subtree tasks) per group of 32 cells.  The interleaved kernel runs in window mode where the
+    model allows it (the probes are then recorded by the kernel itself); "tape-step" forces one
+    launch sequence per dt."""
     if request.param.startswith("tape"):
         monkeypatch.setenv("CN_TAPE", "1")
         monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+        if request.param == "tape-step":
+            monkeypatch.setenv("CN_TAPE_WINDOW", "0")
         if "-w" in request.param:
             monkeypatch.setenv("CN_TAPE_W", request.param[-1])
     else:
@@ -126,19 +130,21 @@ def test_config3_shape(cn, strategy):
         assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9, (t, s)
 
 
-def test_config3_full_size_first_wave(cn):
+def test_config3_full_size_first_wave(cn, monkeypatch):
     """All 3,560 cells / 465,740 compartments / 1.1 M Exp2Syn for 12 ms (the first population
-    wave), default strategy (every cell on the interleaved kernel): once with per-step probes
-    (one launch per dt), once without (window mode, final state only)."""
+    wave), default strategy (every cell on the interleaved kernel): once in window mode with
+    the soma voltages probed every step, once with one launch sequence per dt."""
     from oracle import OracleModel
     desc = W.config3()
     assert len(desc["parent"]) == 465740 and len(desc["netcons"]["src"]) == 1100040
     o, g = run_both(cn, desc, 12.0)
     assert g.layout_info()["n_tape_group"] == g.layout_info()["n_group"] > 100
+    assert g.launch_count < 100
     check(o, g, min_spikes=1000)
+    monkeypatch.setenv("CN_TAPE_WINDOW", "0")
     w = cn.Model(desc)
     w.run(12.0, DT)
-    assert w.launch_count < 100
+    assert w.launch_count >= 480
     assert np.max(np.abs(o.get_v() - w.get_v())) <= TOL
     assert [list(x) for x in w.get_spikes()] == [list(x) for x in o.get_spikes()]
 
