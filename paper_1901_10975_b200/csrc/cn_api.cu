@@ -932,6 +932,8 @@ static int build_layout(cn_model *m) {
   const int64_t hard_cap = 200 * 1024;
   int sched_total = 0, nodeoff_total = 0;
   m->warp_smem_doubles = 0;
+  int64_t coop_cells = 0;
+  for (const HClass &K : m->cls) coop_cells += K.count - K.tp.n_cells;
   for (HClass &K : m->cls) {
     K.needs_ica = m->any_ica ? 1 : 0;
     const int64_t ccount = K.count - K.tp.n_cells;  // cells left for the cooperative kernel
@@ -949,8 +951,12 @@ static int build_layout(cn_model *m) {
       return fail(CN_ERR_UNSUPPORTED,
                   "a cell with %d nodes does not fit the on-chip solve (limit %lld nodes)", K.n,
                   (long long)(hard_cap / (arrays * 8)));
+    // several cells per warp only while that still leaves every SM its 8 warps: below that, more
+    // lanes per cell (fewer rounds, fewer mechanism passes per warp) beat more cells per warp
+    // (config 2, 256 cells x 601 nodes: 94.9 us per dt with G = 1, 110.7 with G = 2)
     int G = 1;
-    while (G * 2 <= max_g && G * 2 <= ccount && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap)
+    while (G * 2 <= max_g && G * 2 <= ccount && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap &&
+           coop_cells / (G * 2) >= 148 * 8)
       G *= 2;
     if (force_g > 0) {
       G = 1;

@@ -92,13 +92,18 @@ def test_unique_topologies_one_cell_per_warp(cn, strategy):
     check(o, g, min_spikes=5)
 
 
-def test_identical_random_cells_grouped(cn, strategy):
+def test_identical_random_cells_grouped(cn, strategy, monkeypatch):
     desc = W.random_tree_cells(11, 77, 77, stream="gpu-i", identical=True, weight=0.2, amp=2.0)
+    if strategy == "coop":      # (a model this small gets one cell per warp unless told otherwise)
+        monkeypatch.setenv("CN_FORCE_G", "4")
     o, g = run_both(cn, desc, 40.0)
     info = g.layout_info()
     # coop: 4 + 4 + 3 (ragged tail group); tape: one ragged group of 11 lanes
     assert info["n_class"] == 1 and info["n_group"] == (3 if strategy == "coop" else 1)
     check(o, g, min_spikes=5)
+    if strategy == "coop":
+        monkeypatch.delenv("CN_FORCE_G")
+        assert cn.Model(desc).layout_info()["n_group"] == 11
 
 
 def test_hh_everywhere_config2_shape(cn, strategy):
@@ -190,6 +195,7 @@ def test_config4_small_full_length(cn, strategy):
 def test_mixed_strategies_in_one_model(cn, monkeypatch):
     """Classes of 40 cells: 32 go to one tape group, the ragged 8 to warp-cooperative groups."""
     monkeypatch.setenv("CN_TAPE", "1")
+    monkeypatch.setenv("CN_FORCE_G", "4")
     desc = W.config4(n_cell=320, n_types=8, ring_size=64)
     o, g = run_both(cn, desc, 30.0)
     info = g.layout_info()
