@@ -457,11 +457,13 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   double *__restrict__ vs = M.v + ab + lane;
   double *__restrict__ pps = M.ppdr + 2 * ab + lane;  // point processes: pp_coop_kernel put the
   const bool has_pp = M.ppdr != nullptr;              // conductance / current of this dt here
-  // (a node that carries point processes is marked by a NEGATIVE static diagonal, which is > 0)
-  auto take_pp = [&](int r, double &d, double &rr) {  // add them to (d, r) of round r and clear
+  // (a node that carries point processes is marked by a NEGATIVE static diagonal, which is > 0).
+  // Their conductance / current rows are requested together with the node's other streams and
+  // looked at only when the round is worked on: nothing here may depend on a load just issued,
+  // or the prefetch distance is lost (one L2 round trip per round).
+  auto take_pp = [&](int r, double &d, double &rr, double pd, double pr) {
     if (!has_pp || d > 0.0) return;
     d = -d;
-    const double pd = pps[(size_t)r * 64], pr = pps[(size_t)r * 64 + 32];
     if (pd != 0.0 || pr != 0.0) {
       d += pd;
       rr += pr;
@@ -472,27 +474,32 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
 
   // issue the first CN_PF rounds of loads and the root's terms before anything else
   uint32_t e_[CN_PF];
-  double a_[CN_PF], b_[CN_PF], d_[CN_PF], r_[CN_PF];
+  double a_[CN_PF], b_[CN_PF], d_[CN_PF], r_[CN_PF], v_[CN_PF], pd_[CN_PF], pr_[CN_PF];
 #pragma unroll
   for (int u = 0; u < CN_PF; ++u) {
     e_[u] = CN_IDLE;
-    a_[u] = b_[u] = d_[u] = r_[u] = 0.0;
+    a_[u] = b_[u] = d_[u] = r_[u] = v_[u] = pd_[u] = pr_[u] = 0.0;
     if (u < rounds) {
       e_[u] = sched[u * P];
-      if ((e_[u] & 0xFFFFu) != CN_IDLE) {
-        a_[u] = as[(size_t)u * 32];
-        b_[u] = bs[(size_t)u * 32];
-        d_[u] = dss[(size_t)u * 32];
-        r_[u] = vs[(size_t)u * 32] + rss[(size_t)u * 32];
-        take_pp(u, d_[u], r_[u]);
+      a_[u] = as[(size_t)u * 32];
+      b_[u] = bs[(size_t)u * 32];
+      d_[u] = dss[(size_t)u * 32];
+      r_[u] = rss[(size_t)u * 32];
+      v_[u] = vs[(size_t)u * 32];
+      if (has_pp) {
+        pd_[u] = pps[(size_t)u * 64];
+        pr_[u] = pps[(size_t)u * 64 + 32];
       }
     }
   }
-  double d_root = 1.0, r_root = 0.0;
+  double d_root = 1.0, r_root = 0.0, pd_root = 0.0, pr_root = 0.0;
   if (p == 0) {
     d_root = dss[(size_t)rounds * 32];
     r_root = vs[(size_t)rounds * 32] + rss[(size_t)rounds * 32];
-    take_pp(rounds, d_root, r_root);
+    if (has_pp) {
+      pd_root = pps[(size_t)rounds * 64];
+      pr_root = pps[(size_t)rounds * 64 + 32];
+    }
   }
 
   // ---- zero the system -------------------------------------------------------------------
@@ -526,8 +533,10 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
         const uint32_t e = e_[u];
         if ((e & 0xFFFFu) != CN_IDLE) {
           const int si = ((e & 0xFFFFu) << lgG) + c, sp = ((e >> 16) << lgG) + c;
-          const double di = D[si] + d_[u], ri = R[si] + r_[u];
-          const double rinv = 1.0 / di;
+          double ds = d_[u], rs = v_[u] + r_[u];
+          take_pp(r, ds, rs, pd_[u], pr_[u]);
+          const double di = D[si] + ds, ri = R[si] + rs;
+          const double rinv = rcp_fast(di);  // (pivots of a diagonally dominant matrix: > 0, O(1))
           const double f = a_[u] * rinv;
           D[sp] -= f * b_[u];
           R[sp] -= f * ri;
@@ -537,14 +546,16 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
         __syncwarp();
         const int rn = r + CN_PF;  // refill this ring slot
         e_[u] = CN_IDLE;
-        if (rn < rounds) {
+        if (rn < rounds) {  // (idle slots hold benign padding: loaded like any other)
           e_[u] = sched[rn * P];
-          if ((e_[u] & 0xFFFFu) != CN_IDLE) {
-            a_[u] = as[(size_t)rn * 32];
-            b_[u] = bs[(size_t)rn * 32];
-            d_[u] = dss[(size_t)rn * 32];
-            r_[u] = vs[(size_t)rn * 32] + rss[(size_t)rn * 32];
-            take_pp(rn, d_[u], r_[u]);
+          a_[u] = as[(size_t)rn * 32];
+          b_[u] = bs[(size_t)rn * 32];
+          d_[u] = dss[(size_t)rn * 32];
+          r_[u] = rss[(size_t)rn * 32];
+          v_[u] = vs[(size_t)rn * 32];
+          if (has_pp) {
+            pd_[u] = pps[(size_t)rn * 64];
+            pr_[u] = pps[(size_t)rn * 64 + 32];
           }
         }
       }
@@ -552,7 +563,8 @@ __global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ 
   }
   // root: local node 0, stored in the extra round
   if (p == 0) {
-    const double u0 = (R[c] + r_root) / (D[c] + d_root);
+    take_pp(rounds, d_root, r_root, pd_root, pr_root);
+    const double u0 = (R[c] + r_root) * rcp_fast(D[c] + d_root);
     R[c] = u0;
     vs[(size_t)rounds * 32] = u0;
   }
