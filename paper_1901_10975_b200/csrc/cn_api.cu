@@ -1156,7 +1156,7 @@ static int build_layout(cn_model *m) {
   static_assert(sizeof(TapeGroup) == 32, "TapeGroup layout");
   // CTA shape of the cooperative kernel: as many warps per block as fit ~100 KB, at most 8
   const int64_t wbytes = std::max<int64_t>((int64_t)m->warp_smem_doubles * 8, 8);
-  int wpb = 8;
+  int wpb = 4;  // (4 warps x 3 CTAs per SM: 170 registers per thread, no spills)
   if (const char *e = std::getenv("CN_WPB")) wpb = std::max(1, std::atoi(e));
   while (wpb > 1 && wbytes * wpb > 110 * 1024) wpb /= 2;
   m->wpb = wpb;

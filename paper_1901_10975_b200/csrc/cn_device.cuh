@@ -424,7 +424,10 @@ __device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, i
 #define CN_PF 4  // rounds of prefetch distance for the schedule-ordered streams
 
 template <int WPB>
-__global__ void __launch_bounds__(WPB * 32) step_kernel(const __grid_constant__ DModel M,
+// (registers: the prefetched streams must stay in registers -- a spill store waits for its load
+// and the prefetch distance is gone -- so the bound asks for 12 warps per SM, not 16)
+__global__ void __launch_bounds__(WPB * 32, WPB >= 8 ? 1 : 12 / WPB)
+    step_kernel(const __grid_constant__ DModel M,
                                                         int64_t k) {
   extern __shared__ double smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
