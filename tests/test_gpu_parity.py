@@ -433,3 +433,27 @@ def test_gap_junctions_across_kernels(cn, monkeypatch):
     info = g.layout_info()
     assert info["n_tape_group"] >= 1 and info["n_group"] > info["n_tape_group"]
     check(o, g, min_spikes=5)
+
+
+def test_probe_capacity_and_interior_nodes(cn, strategy):
+    """Probes on interior nodes of several cells (two of them in the same group), a trace capacity
+    shorter than the run, cn_run in uneven pieces: the first `cap` rows must be the oracle's, the
+    rest is dropped -- whether a probe kernel follows every step or the interleaved kernel records
+    the voltages itself (window mode)."""
+    desc = W.config4(n_cell=128, n_types=2)
+    cf = desc["cell_first"]
+    probes = np.array([cf[0], cf[0] + 17, cf[1] + 290, cf[70] + 5, cf[127] + 100, cf[64]], np.int32)
+    cap, nsteps = 150, 400
+    from oracle import OracleModel
+    o = OracleModel(desc)
+    o.set_probes(probes)
+    o.run(nsteps * DT, DT)
+    g = cn.Model(desc)
+    g.set_probes(probes, cap)
+    for k in (3, 44, 149, 151, 290, nsteps):
+        g.run(k * DT, DT)
+    tr = g.get_trace()
+    assert tr.shape == (cap, len(probes))
+    assert np.max(np.abs(tr - o.get_trace()[:cap])) <= TOL
+    assert np.max(np.abs(g.get_v() - o.get_v())) <= TOL
+    assert [list(x) for x in g.get_spikes()] == [list(x) for x in o.get_spikes()]
