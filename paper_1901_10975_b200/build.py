@@ -9,6 +9,8 @@ HERE = Path(__file__).resolve().parent
 SO = HERE / "libcn.so"
 SRCS = [HERE / "csrc" / "cn_api.cu"]
 DEPS = SRCS + [HERE / "csrc" / "cn_device.cuh", HERE / "csrc" / "cn_tape.cuh",
+               HERE / "csrc" / "cn_host.hpp", HERE / "csrc" / "cn_layout.hpp",
+               HERE / "csrc" / "cn_finalize.hpp",
                HERE / "csrc" / "cn_tape_program.hpp",
                HERE.parent / "include" / "cn.h"]
 

@@ -1,0 +1,520 @@
+// cn_finalize.hpp -- finalize(): the part of the set-up that needs dt (first cn_run): row-normalised
+// static rows, tapes, mechanism tables, NetCon tables, window buffers, uploads.  Included by
+// cn_api.cu only.
+#pragma once
+
+// ---------------------------------------------------------------------------------------------
+// first cn_run: dt-dependent constants (row-normalised system), initial states, upload
+// ---------------------------------------------------------------------------------------------
+
+static int finalize(cn_model *m, double dt) {
+  const bool dbg = std::getenv("CN_DEBUG") != nullptr;
+  auto t_prev = std::chrono::steady_clock::now();
+  auto lap = [&](const char *what) {
+    if (!dbg) return;
+    const auto t = std::chrono::steady_clock::now();
+    fprintf(stderr, "[cn] finalize %-32s %7.1f ms\n", what,
+            std::chrono::duration<double, std::milli>(t - t_prev).count());
+    t_prev = t;
+  };
+  const int64_t N = m->N;
+  const int nt = (int)m->tab.size();
+  const int ng = (int)m->grp.size();
+  int dev_count = 0;
+  if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
+    return fail(CN_ERR_CUDA, "no CUDA device: libcn has no CPU fallback");
+  // delays
+  std::vector<int32_t> dsteps((size_t)m->n_netcon);
+  int64_t mind = INT32_MAX, maxd = 1;
+  for (int64_t i = 0; i < m->n_netcon; ++i) {
+    const long long ds = llround(m->nc_delay[i] / dt);
+    if (ds < 1) return fail(CN_ERR_NETCON, "netcon %lld: delay %.6g ms is < 1 step of %.6g ms",
+                            (long long)i, m->nc_delay[i], dt);
+    if (ds > 1000000) return fail(CN_ERR_NETCON, "netcon %lld: delay too long", (long long)i);
+    dsteps[i] = (int32_t)ds;
+    mind = std::min<int64_t>(mind, ds);
+    maxd = std::max<int64_t>(maxd, ds);
+  }
+  if (m->n_netcon == 0) mind = 1;
+  // row-normalised static arrays:  c_i = 1e-3 cm_i/dt,  b' = b/c_i,  a' = a/c_parent,
+  // dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
+  uvec<double> invc((size_t)N), bn((size_t)N), an((size_t)N);
+  std::vector<double> dstat((size_t)m->n_pnode, 1.0), rstat((size_t)m->n_pnode, 0.0);
+  // one arena: [schedule-ordered v of the cooperative groups | tapes of the interleaved groups]
+  uvec<double> v0((size_t)(m->n_ab + m->n_tape));
+  double *tape = v0.data() + m->n_ab;
+  uvec<double> dsum((size_t)N), rsum((size_t)N);
+  uvec<int32_t> cell_of_node((size_t)N);
+  par_for((int64_t)v0.size(), 1 << 20, [&](int64_t i0, int64_t i1) {
+    std::fill(v0.begin() + i0, v0.begin() + i1, 0.0);
+  });
+  par_for(N, 1 << 20, [&](int64_t i0, int64_t i1) {
+    std::fill(bn.begin() + i0, bn.begin() + i1, 0.0);
+    std::fill(an.begin() + i0, an.begin() + i1, 0.0);
+    std::fill(rsum.begin() + i0, rsum.begin() + i1, 0.0);
+  });
+  // cells are independent (a parent sits in the same cell): all host cores
+  par_for(m->n_cell, 256, [&](int64_t c0, int64_t c1) {
+    const int64_t i0 = m->cell_first[c0], i1 = m->cell_first[c1];
+    for (int64_t c = c0; c < c1; ++c)
+      for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of_node[i] = (int32_t)c;
+    for (int64_t i = i0; i < i1; ++i) {
+      const double c = 1e-3 * m->cm[i] / dt;
+      invc[i] = 1.0 / c;
+      dsum[i] = c;
+    }
+    for (int64_t i = i0; i < i1; ++i) {
+      const int32_t p = m->parent[i];
+      if (p >= 0) {
+        const double b = -100.0 / (m->ri[i] * m->area[i]);
+        const double a = -100.0 / (m->ri[i] * m->area[p]);
+        dsum[i] -= b;
+        dsum[p] -= a;
+        bn[i] = b * invc[i];
+        an[i] = a * invc[p];
+      }
+    }
+  });
+  for (const HTable &T : m->tab)
+    if (T.type == CN_PAS)  // (at most one instance of a table per node: no two threads meet)
+      par_for(T.n, 65536, [&](int64_t q0, int64_t q1) {
+        for (int64_t i = q0; i < q1; ++i) {
+          const double g = T.param[i], e = T.param[T.n + i];
+          dsum[T.node[i]] += g;
+          rsum[T.node[i]] += g * e;
+        }
+      });
+  // inverse map: (group, slot) -> caller cell
+  std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
+  for (int32_t c = 0; c < m->n_cell; ++c) {
+    const int g = m->cell_grp[c];
+    const int32_t cb = g < m->n_cgroup ? m->grp[g].cell_base : m->tgrp[g - m->n_cgroup].cell_base;
+    cell_of_pcell[cb + m->cell_slot[c]] = c;
+  }
+  // interleaved groups: whole rows of 32 lanes at a time (contiguous writes; the 32 cells are
+  // read as 32 sequential streams); a, b, d, r precede the node's v row
+  par_for((int64_t)m->tgrp.size(), 1, [&](int64_t g0, int64_t g1) {
+    for (int64_t g = g0; g < g1; ++g) {
+      const TapeGroup &tg = m->tgrp[g];
+      const HClass &K = m->cls[tg.cls];
+      int64_t f[32];
+      for (int l = 0; l < tg.ncell; ++l) f[l] = m->cell_first[cell_of_pcell[tg.cell_base + l]];
+      for (int j = 0; j < K.n; ++j) {
+        double *rec = tape + tg.tape_base + ((int64_t)K.tp.row[K.tp.pos_of[j]] + 4) * 32;
+        for (int l = 0; l < tg.ncell; ++l) {
+          const int64_t i = f[l] + j;
+          rec[-4 * 32 + l] = an[i];
+          rec[-3 * 32 + l] = bn[i];
+          rec[-2 * 32 + l] = dsum[i] * invc[i];
+          rec[-1 * 32 + l] = rsum[i] * invc[i];
+          rec[l] = m->v_init;
+        }
+      }
+    }
+  });
+  if (m->n_cgroup > 0)
+    par_for(N, 65536, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i) {
+        if (m->cell_tape[cell_of_node[i]]) continue;
+        const int64_t q = m->node_pos[i];
+        dstat[q] = dsum[i] * invc[i];
+        rstat[q] = rsum[i] * invc[i];
+        v0[q] = m->v_init;
+      }
+    });
+  lap("static rows");
+  // idle lanes of a ragged tape group: unit diagonal, everything else zero; cai rows
+  for (const TapeGroup &tg : m->tgrp) {
+    const HTape &P = m->cls[tg.cls].tp;
+    for (int j = 0; j < m->cls[tg.cls].n; ++j)
+      for (int l = tg.ncell; l < 32; ++l) tape[tg.tape_base + ((int64_t)P.row[j] + 2) * 32 + l] = 1.0;
+  }
+  for (const TapeGroup &tg : m->tgrp) {  // the copy of v at the head of every mechanism record
+    const HTape &P = m->cls[tg.cls].tp;
+    for (int i = 0; i < m->cls[tg.cls].n; ++i)
+      if (P.vcopy_row[i] >= 0)
+        for (int l = 0; l < 32; ++l)
+          tape[tg.tape_base + (int64_t)P.vcopy_row[i] * 32 + l] = m->v_init;
+  }
+  if (m->any_cai)
+    for (int32_t c = 0; c < m->n_cell; ++c) {
+      if (!m->cell_tape[c]) continue;
+      const TapeGroup &tg = m->tgrp[m->cell_grp[c] - m->n_cgroup];
+      const HTape &P = m->cls[tg.cls].tp;
+      const int64_t f = m->cell_first[c];
+      for (int i = 0; i < m->cls[tg.cls].n; ++i)
+        if (P.cai_row[i] >= 0)
+          tape[tg.tape_base + (int64_t)P.cai_row[i] * 32 + m->cell_slot[c]] = m->cai0[f + i];
+    }
+  lap("idle lanes, v copies, cai");
+  // schedule-ordered off-diagonals
+  std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
+  std::vector<uint32_t> sched_all;
+  std::vector<int32_t> nodeoff_all;
+  std::vector<ClassInfo> cinfo(m->cls.size());
+  for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+    const HClass &K = m->cls[kc];
+    cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, K.nodeoff_off, 0};
+    sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
+    nodeoff_all.insert(nodeoff_all.end(), K.node_off.begin(), K.node_off.end());
+  }
+  for (int g = 0; g < ng; ++g) {
+    const GroupInfo &gi = m->grp[g];
+    const HClass &K = m->cls[gi.cls];
+    const int P = 32 / K.G;
+    for (int c = 0; c < gi.ncell; ++c) {
+      const int32_t cell = cell_of_pcell[gi.cell_base + c];
+      const int64_t f = m->cell_first[cell];
+      for (int r = 0; r < K.rounds; ++r)
+        for (int p = 0; p < P; ++p) {
+          const uint32_t e = K.sched[(size_t)r * P + p];
+          if ((e & 0xFFFFu) == CN_IDLE) continue;
+          const int64_t i = f + (e & 0xFFFFu);
+          const int64_t pos = gi.ab_base + (int64_t)r * 32 + p * K.G + c;
+          a_s[pos] = an[i];
+          b_s[pos] = bn[i];
+        }
+    }
+  }
+  lap("coop schedule arrays");
+  // thresholds, flags, gids per permuted cell
+  std::vector<double> thr((size_t)m->n_pcell, 0.0);
+  std::vector<unsigned char> flag((size_t)m->n_pcell, 0);
+  std::vector<int32_t> gid_of((size_t)m->n_pcell, -1);
+  for (int32_t pc = 0; pc < m->n_pcell; ++pc) {
+    const int32_t c = cell_of_pcell[pc];
+    if (c < 0) continue;
+    thr[pc] = m->thr[c];
+    flag[pc] = m->v_init > m->thr[c];
+    gid_of[pc] = c;
+  }
+  // cai per node of the cooperative groups
+  std::vector<double> cai;
+  if (m->any_cai) {
+    cai.assign((size_t)m->n_pnode, 1e-4);
+    for (int64_t i = 0; i < N; ++i)
+      if (!m->cell_tape[cell_of_node[i]]) cai[m->node_pos[i]] = m->cai0[i];
+  }
+
+  DModel &H = m->hm;
+  H.warp_smem_doubles = m->warp_smem_doubles;
+  H.dt = dt;
+  H.celsius = m->celsius;
+  H.q10 = std::pow(3.0, (m->celsius - 6.3) / 10.0);
+  int rc;
+#define UP(vec, ptr)                                            \
+  do {                                                          \
+    rc = dev_upload(m, vec, &ptr);                              \
+    if (rc != CN_OK) return rc;                                 \
+  } while (0)
+  {
+    GroupInfo *dg; ClassInfo *dc; uint32_t *ds; int32_t *dn;
+    UP(m->grp, dg); UP(cinfo, dc); UP(sched_all, ds); UP(m->dist_nodes, dn);
+    H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
+    int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
+    double *p;
+    // nodes of warp-cooperative cells that carry point processes: negative static diagonal
+    for (const HTable &T : m->tab)
+      if (T.ti.point)
+        for (int64_t i = 0; i < T.n; ++i)
+          if (!m->cell_tape[cell_of_node[T.node[i]]]) {
+            double &d = dstat[m->node_pos[T.node[i]]];
+            d = -std::fabs(d);
+          }
+    UP(dstat, p); H.dstat = p;
+    H.ppdr = nullptr;
+    {  // point processes on warp-cooperative groups: their conductance / current rows
+      bool any = false;
+      for (const HTable &T : m->tab)
+        if (T.ti.point && T.pp_tape_begin > 0) any = true;
+      if (any) {
+        rc = dev_alloc(m, (size_t)(2 * m->n_pnode + 64), &H.ppdr);
+        if (rc != CN_OK) return rc;
+      }
+    }
+    UP(rstat, p); H.rstat = p;
+    UP(a_s, p); H.a_s = p;
+    UP(b_s, p); H.b_s = p;
+    if (m->any_cai) { UP(cai, m->d_cai); H.cai = m->d_cai; } else H.cai = nullptr;
+    UP(thr, p); H.thr = p;
+    unsigned char *pf; UP(flag, pf); H.flag = pf;
+    int32_t *pg; UP(gid_of, pg); H.gid_of_pcell = pg;
+  }
+  lap("small uploads");
+  // mechanism tables
+  for (int t = 0; t < nt; ++t) {
+    HTable &T = m->tab[t];
+    DTable &D = H.tab[t];
+    memset(&D, 0, sizeof(D));
+    D.type = T.type;
+    D.is_point = T.ti.point;
+    D.n_param = T.ti.n_dev_param;
+    D.n_state = T.ti.n_state;
+    for (size_t j = 0; j < T.glob.size(); ++j) D.glob[j] = T.glob[j];
+    if (T.type == CN_AMPANMDA) {
+      D.glob[7] = h_exp2_factor(T.glob[0], T.glob[1]);
+      D.glob[8] = h_exp2_factor(T.glob[2], T.glob[3]);
+      for (int c = 0; c < 4; ++c) D.glob[9 + c] = 1.0 - std::exp(-dt / T.glob[c]);  // cnexp factors
+    }
+    if (T.type == CN_PAS) continue;  // folded
+    const int64_t nd = T.n_dev;
+    std::vector<uvec<double>> par(T.ti.n_dev_param), st(T.ti.n_state);
+    for (auto &x : par) x.resize((size_t)nd);
+    for (auto &x : st) x.resize((size_t)nd);
+    par_for(nd, 1 << 18, [&](int64_t i0, int64_t i1) {
+      for (int j = 0; j < T.ti.n_dev_param; ++j)  // benign padding for distributed tables
+        std::fill(par[j].begin() + i0, par[j].begin() + i1,
+                  !T.ti.point && j == T.ti.n_dev_param - 1 ? 1.0 : 0.0);
+      for (auto &x : st) std::fill(x.begin() + i0, x.begin() + i1, 0.0);
+    });
+    // instances are independent (each writes its own elements): all host cores
+    par_for(T.n, 4096, [&](int64_t ii0, int64_t ii1) {
+     for (int64_t i = ii0; i < ii1; ++i) {
+      const int32_t nd_i = T.node[i];
+      double P[CN_MAX_PARAM] = {0.0}, S[CN_MAX_STATE] = {0.0};
+      for (int j = 0; j < T.ti.n_param; ++j) P[j] = T.param[(size_t)j * T.n + i];
+      const double scale = 100.0 / m->area[nd_i] * invc[nd_i];
+      const double v = m->v_init;
+      switch (T.type) {
+        case CN_HH: {
+          P[4] = invc[nd_i];
+          double al, be;
+          al = 0.1 * h_vtrap(-(v + 40.0), 10.0); be = 4.0 * std::exp(-(v + 65.0) / 18.0);
+          S[0] = al / (al + be);
+          al = 0.07 * std::exp(-(v + 65.0) / 20.0); be = 1.0 / (std::exp(-(v + 35.0) / 10.0) + 1.0);
+          S[1] = al / (al + be);
+          al = 0.01 * h_vtrap(-(v + 55.0), 10.0); be = 0.125 * std::exp(-(v + 65.0) / 80.0);
+          S[2] = al / (al + be);
+          break;
+        }
+        case CN_EXPSYN:  // tau -> the cnexp factor 1 - exp(-dt/tau) (the device never needs tau)
+          P[2] = scale;
+          P[0] = 1.0 - std::exp(-dt / P[0]);
+          break;
+        case CN_EXP2SYN:
+          P[3] = scale;
+          P[4] = h_exp2_factor(P[0], P[1]);
+          P[0] = 1.0 - std::exp(-dt / P[0]);
+          P[1] = 1.0 - std::exp(-dt / P[1]);
+          break;
+        case CN_ICLAMP: P[3] = scale; break;
+        case CN_HHFORM:
+          P[1] = invc[nd_i];
+          S[0] = 1.0 / (1.0 + std::exp((T.glob[4] - v) / T.glob[5]));
+          S[1] = 1.0 / (1.0 + std::exp((T.glob[10] - v) / T.glob[11]));
+          break;
+        case CN_SK: {
+          P[1] = invc[nd_i];
+          double ca = m->any_cai ? m->cai0[nd_i] : 1e-4;
+          if (ca < 1e-9) ca = 1e-9;
+          S[0] = 1.0 / (1.0 + std::pow(T.glob[1] / ca, T.glob[2]));
+          break;
+        }
+        case CN_AMPANMDA: P[0] = scale; break;
+        case CN_GAP:  // positions in the voltage arena (exact in a double: < 2^53)
+          P[0] *= scale;
+          P[1] = (double)m->node_pos[(int64_t)P[1]];
+          break;
+        default: break;
+      }
+      if (!T.ti.point && T.tape_loc[i] >= 0) {  // the instance lives on a tape
+        double *rec = tape + T.tape_loc[i];
+        for (int j = 0; j < T.ti.n_dev_param; ++j) rec[(size_t)j * 32] = P[j];
+        for (int j = 0; j < T.ti.n_state; ++j) rec[(size_t)(T.ti.n_dev_param + j) * 32] = S[j];
+      } else if (T.inst_pos[i] >= 0) {
+        const int64_t q = T.inst_pos[i];
+        for (int j = 0; j < T.ti.n_dev_param; ++j) par[j][q] = P[j];
+        for (int j = 0; j < T.ti.n_state; ++j) st[j][q] = S[j];
+      }
+     }
+    });
+    for (int j = 0; j < T.ti.n_dev_param; ++j) { UP(par[j], T.d_param[j]); D.param[j] = T.d_param[j]; }
+    for (int j = 0; j < T.ti.n_state; ++j) { UP(st[j], T.d_state[j]); D.state[j] = T.d_state[j]; }
+    if (T.ti.point) {
+      UP(T.pp_first, T.d_pp_first); UP(T.pp_slot, T.d_pp_slot); UP(T.pp_wslot, T.d_pp_wslot);
+      D.pp_first = T.d_pp_first; D.pp_slot = T.d_pp_slot; D.pp_wslot = T.d_pp_wslot;
+      D.pp_goff = m->win_ninst;
+      m->win_ninst += T.n;
+    } else {
+      UP(T.cls_cnt, T.d_cls_cnt); UP(T.cls_nodeoff, T.d_cls_nodeoff);
+      UP(T.grp_instbase, T.d_grp_instbase);
+      D.cls_cnt = T.d_cls_cnt; D.cls_nodeoff = T.d_cls_nodeoff; D.grp_instbase = T.d_grp_instbase;
+    }
+  }
+  lap("mechanism tables");
+  // the arena (filled above, including the mechanism rows of the tapes) and the programs
+  {
+    UP(v0, m->d_v);
+    H.v = m->d_v;
+    H.tape = m->d_v + m->n_ab;
+    std::vector<TapeClass> tcls(m->cls.size());
+    std::vector<TapeTask> ttask(m->cls.size() * (size_t)m->tape_W);
+    std::vector<uint4> prog;
+    for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+      const HClass &K = m->cls[kc];
+      const HTape &P = K.tp;
+      tcls[kc] = TapeClass{K.n, P.prog_off, (int32_t)P.prog.size(), P.n_bar};
+      if (P.n_groups == 0) continue;
+      if ((int)prog.size() != P.prog_off) return fail(CN_ERR_ARG, "internal: program offsets");
+      prog.insert(prog.end(), P.prog.begin(), P.prog.end());
+      for (int w = 0; w < m->tape_W; ++w) {
+        const HTask &Tk = P.task[w];
+        // program positions are relative to the class's program (as it sits in shared memory)
+        ttask[kc * (size_t)m->tape_W + w] =
+            TapeTask{Tk.p0, Tk.p1, Tk.b0, Tk.b1, Tk.nchunk, Tk.tm_base, Tk.row0, Tk.head, Tk.nrows,
+                     (uint32_t)Tk.pp0};
+      }
+    }
+    TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
+    UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg); UP(ttask, dtt);
+    H.tgrp = dtg; H.tcls = dtc; H.prog = dpg; H.ttask = dtt;
+    H.tape_W = m->tape_W;
+    H.tape_S = m->tape_S;
+    H.tape_CH = m->tape_CH;
+    H.tape_prog_cap = std::max(m->tape_prog_cap, 1);
+    H.tape_sys_cap = std::max(m->tape_sys_cap, 1);
+    H.tape_bar_cap = m->tape_bar_cap;
+    H.tape_pf = 0;  // measured on config 4: prefetching ahead of the ring only costs (0: off)
+    if (const char *e = std::getenv("CN_TAPE_PF")) H.tape_pf = std::max(0, std::min(4096, std::atoi(e)));
+    for (int t = 0; t < nt; ++t) {
+      H.tab[t].pp_tape_begin = m->tab[t].pp_tape_begin;
+      H.tab[t].pp_tape_end = m->tab[t].ti.point ? m->tab[t].n : 0;
+    }
+  }
+  // PAS tables still need (empty) layout pointers so the kernel's table loop can skip them
+  for (int t = 0; t < nt; ++t) {
+    HTable &T = m->tab[t];
+    if (T.type != CN_PAS) continue;
+    std::vector<int32_t> zc(m->cls.size(), 0);
+    std::vector<int64_t> zg((size_t)ng, 0);
+    UP(zc, T.d_cls_cnt); UP(zc, T.d_cls_nodeoff); UP(zg, T.d_grp_instbase);
+    H.tab[t].cls_cnt = T.d_cls_cnt; H.tab[t].cls_nodeoff = T.d_cls_nodeoff;
+    H.tab[t].grp_instbase = T.d_grp_instbase;
+  }
+  lap("arena + programs upload");
+  // NetCons: CSR by source gid, sorted by delay steps (stable in caller order)
+  {
+    std::vector<int64_t> order((size_t)m->n_netcon);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) {
+      if (m->nc_src[x] != m->nc_src[y]) return m->nc_src[x] < m->nc_src[y];
+      return dsteps[x] < dsteps[y];
+    });
+    std::vector<int64_t> src_first((size_t)m->n_src + 1, 0);
+    for (int64_t i = 0; i < m->n_netcon; ++i) src_first[m->nc_src[i] + 1]++;
+    for (int32_t s = 0; s < m->n_src; ++s) src_first[s + 1] += src_first[s];
+    std::vector<int32_t> nd((size_t)m->n_netcon), ntab((size_t)m->n_netcon);
+    std::vector<int64_t> ninst((size_t)m->n_netcon);
+    std::vector<double> nw((size_t)m->n_netcon);
+    for (int64_t j = 0; j < m->n_netcon; ++j) {
+      const int64_t i = order[j];
+      nd[j] = dsteps[i];
+      ntab[j] = m->nc_tgt_mech[i];
+      ninst[j] = m->tab[m->nc_tgt_mech[i]].inst_pos[m->nc_tgt_inst[i]];
+      nw[j] = m->nc_w[i];
+    }
+    int64_t *p64; int32_t *p32; double *pd;
+    UP(src_first, p64); H.src_first = p64;
+    UP(nd, p32); H.nc_d = p32;
+    UP(ntab, p32); H.nc_tab = p32;
+    UP(ninst, p64); H.nc_inst = p64;
+    UP(nw, pd); H.nc_w = pd;
+    H.mind = (int32_t)mind;
+    H.maxd = (int32_t)maxd;
+    H.wr = (int32_t)(maxd + 2);
+    rc = dev_alloc(m, (size_t)H.wr, &H.sp_end);
+    if (rc != CN_OK) return rc;
+    // scripted sources sorted by step
+    const int64_t ns = (int64_t)m->stim_gid.size();
+    std::vector<int64_t> sstep((size_t)ns), so((size_t)ns);
+    for (int64_t i = 0; i < ns; ++i) sstep[i] = llround(m->stim_t[i] / dt);
+    std::iota(so.begin(), so.end(), 0);
+    std::stable_sort(so.begin(), so.end(), [&](int64_t x, int64_t y) { return sstep[x] < sstep[y]; });
+    std::vector<int32_t> sg((size_t)ns);
+    std::vector<int64_t> ss((size_t)ns);
+    for (int64_t j = 0; j < ns; ++j) { sg[j] = m->stim_gid[so[j]]; ss[j] = sstep[so[j]]; }
+    UP(sg, p32); H.stim_gid = p32;
+    UP(ss, p64); H.stim_step = p64;
+    H.n_stim = ns;
+  }
+  lap("netcons");
+  // window mode: every cell on the interleaved kernel, no point process whose current depends on
+  // v (AMPA+NMDA, gap junctions); a window is at most the smallest delay long (probes are
+  // recorded by the kernel itself then)
+  {
+    bool ok = m->hm.n_tgroup > 0 && m->grp.empty();
+    for (const HTable &T : m->tab)
+      if ((T.type == CN_AMPANMDA || T.type == CN_GAP) && T.n > 0) ok = false;
+    if (const char *e = std::getenv("CN_TAPE_WINDOW")) ok = ok && std::atoi(e) != 0;
+    int64_t wn = m->n_netcon > 0 ? std::min<int64_t>(H.mind, 64) : 32;
+    if (wn < 2) ok = false;
+    if (ok && (m->win_stride + m->win_ninst) * wn * 8 > ((int64_t)4 << 30)) ok = false;
+    m->window = ok;
+    m->win_steps = (int)wn;
+    H.win_stride = m->win_stride;
+    H.win_ninst = m->win_ninst;
+    if (ok) {
+      rc = dev_alloc(m, (size_t)(m->win_stride * wn + 128), &H.win_rows);  // (+ prefetch overrun)
+      if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_ninst * wn, 1), &H.win_deliv);
+      if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)m->hm.n_tgroup, &H.win_done); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, 1, &H.win_ticket); if (rc != CN_OK) return rc;
+      H.win_mark_cap = H.maxd + 64;
+      rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_step); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_nsp); if (rc != CN_OK) return rc;
+    }
+  }
+  // spikes
+  rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_gid, false); if (rc) return rc;
+  rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_step, false); if (rc) return rc;
+  rc = dev_alloc(m, 1, &m->d_nsp); if (rc) return rc;
+  rc = dev_alloc(m, 1, &m->d_overflow); if (rc) return rc;
+  H.sp_gid = m->d_sp_gid; H.sp_step = m->d_sp_step; H.n_sp = m->d_nsp; H.sp_cap = m->sp_cap;
+  H.overflow = m->d_overflow;
+  lap("window buffers, spikes");
+  // caller-order lookup for cn_get_v, probes
+  UP(m->node_pos, m->d_node_pos);
+  rc = dev_alloc(m, (size_t)std::max<int64_t>(N, 1), &m->d_gather, false); if (rc) return rc;
+  if (!m->probe.empty()) {
+    std::vector<int64_t> pp(m->probe.size());
+    for (size_t j = 0; j < pp.size(); ++j) pp[j] = m->node_pos[m->probe[j]];
+    UP(pp, m->d_probe_pos);
+    rc = dev_alloc(m, (size_t)(m->probe_cap * (int64_t)m->probe.size()), &m->d_trace, false);
+    if (rc) return rc;
+    if (m->window) {  // the probes of every group: the interleaved kernel records them per step
+      const int ntg = (int)m->tgrp.size();
+      std::vector<int32_t> first((size_t)ntg + 1, 0), col(m->probe.size());
+      std::vector<int64_t> pos(m->probe.size());
+      std::vector<int32_t> grp_of(m->probe.size());
+      for (size_t j = 0; j < m->probe.size(); ++j) {
+        const int64_t nd = m->probe[j];
+        const int32_t c = (int32_t)(std::upper_bound(m->cell_first.begin(), m->cell_first.end(), nd) -
+                                    m->cell_first.begin()) - 1;
+        grp_of[j] = m->cell_grp[c] - m->n_cgroup;
+        first[grp_of[j] + 1]++;
+      }
+      for (int g = 0; g < ntg; ++g) first[g + 1] += first[g];
+      std::vector<int32_t> fill(first.begin(), first.end() - 1);
+      for (size_t j = 0; j < m->probe.size(); ++j) {
+        const int32_t q = fill[grp_of[j]]++;
+        pos[q] = pp[j];
+        col[q] = (int32_t)j;
+      }
+      int32_t *df, *dc;
+      int64_t *dp;
+      UP(first, df); UP(pos, dp); UP(col, dc);
+      H.wp_first = df; H.wp_pos = dp; H.wp_col = dc;
+      H.trace = m->d_trace;
+      H.trace_cap = m->probe_cap;
+      H.n_probe = (int32_t)m->probe.size();
+    }
+  }
+#undef UP
+  CU(cudaEventCreate(&m->ev0));
+  CU(cudaEventCreate(&m->ev1));
+  m->dt = dt;
+  m->uploaded = true;
+  return CN_OK;
+}
+

@@ -1,6 +1,6 @@
 // cn_tape_program.hpp -- host side of the interleaved kernel (cn_tape.cuh): compiles the tree of one
 // shape class into the W record lists the kernel interprets (static schedule, hand-over kinds,
-// dependencies, tape rows, chunks, backward program) and dry-runs them.  Included by cn_api.cu
+// dependencies, tape rows, chunks, backward program) and dry-runs them.  Included by cn_layout.hpp
 // after the host model structures (cn_model, HClass, HTape, HTask); not a stand-alone unit.
 #pragma once
 
