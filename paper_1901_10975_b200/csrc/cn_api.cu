@@ -708,6 +708,7 @@ extern "C" int cn_checkpoint_load(cn_model *m, const void *buf, int64_t bytes) {
     if (sz) CU(cudaMemcpy(b.first, p, sz, cudaMemcpyHostToDevice));
     p += (sz + 7) & ~(size_t)7;
   }
+  CU(cudaDeviceSynchronize());  // (the model's stream may not wait for the legacy default stream)
   m->k = h.k;
   m->win_idx = h.win_idx;
   m->state_pending = h.state_pending != 0;

@@ -92,9 +92,11 @@ static int finalize(cn_model *m, double dt) {
     cell_of_pcell[cb + m->cell_slot[c]] = c;
   }
   // interleaved groups: whole rows of 32 lanes at a time (contiguous writes; the 32 cells are
-  // read as 32 sequential streams); a, b, d, r precede the node's v row
-  par_for((int64_t)m->tgrp.size(), 1, [&](int64_t g0, int64_t g1) {
-    for (int64_t g = g0; g < g1; ++g) {
+  // read as 32 sequential streams); a, b, d, r precede the node's v row.  Run chunk by chunk at
+  // the very end, each chunk's upload overlapping the next chunk's rows (see the arena upload).
+  auto static_rows_of_groups = [&](int64_t ga, int64_t gb) {
+   par_for(gb - ga, 1, [&](int64_t g0, int64_t g1) {
+    for (int64_t g = ga + g0; g < ga + g1; ++g) {
       const TapeGroup &tg = m->tgrp[g];
       const HClass &K = m->cls[tg.cls];
       int64_t f[32];
@@ -111,7 +113,8 @@ static int finalize(cn_model *m, double dt) {
         }
       }
     }
-  });
+   });
+  };
   if (m->n_cgroup > 0)
     par_for(N, 65536, [&](int64_t i0, int64_t i1) {
       for (int64_t i = i0; i < i1; ++i) {
@@ -344,7 +347,39 @@ static int finalize(cn_model *m, double dt) {
   lap("mechanism tables");
   // the arena (filled above, including the mechanism rows of the tapes) and the programs
   {
-    UP(v0, m->d_v);
+    {
+      void *p = nullptr;
+      CU(cudaMalloc(&p, std::max<size_t>(v0.size(), 1) * sizeof(double)));
+      m->dev_allocs.push_back(p);
+      m->d_v = static_cast<double *>(p);
+      if (m->n_ab > 0)
+        CU(cudaMemcpy(m->d_v, v0.data(), (size_t)m->n_ab * sizeof(double), cudaMemcpyHostToDevice));
+      // the tapes: static rows of a chunk of groups on all cores, then its upload on a thread of
+      // its own while the cores fill the next chunk (a pageable copy moves ~13 GB/s)
+      const int64_t ntg = (int64_t)m->tgrp.size();
+      const int64_t nch = ntg >= 64 ? 8 : 1;
+      int dev = 0;
+      CU(cudaGetDevice(&dev));
+      std::thread up;
+      cudaError_t up_err = cudaSuccess;
+      for (int64_t c = 0; c < nch && ntg > 0; ++c) {
+        const int64_t ga = ntg * c / nch, gb = ntg * (c + 1) / nch;
+        static_rows_of_groups(ga, gb);
+        if (up.joinable()) up.join();
+        const int64_t e0 = m->tgrp[ga].tape_base, e1 = gb < ntg ? m->tgrp[gb].tape_base : m->n_tape;
+        double *dst = m->d_v + m->n_ab + e0;
+        const double *src = tape + e0;
+        up = std::thread([dev, dst, src, e0, e1, &up_err] {
+          cudaSetDevice(dev);
+          const cudaError_t e =
+              cudaMemcpy(dst, src, (size_t)(e1 - e0) * sizeof(double), cudaMemcpyHostToDevice);
+          if (e != cudaSuccess) up_err = e;
+        });
+      }
+      if (up.joinable()) up.join();
+      if (up_err != cudaSuccess)
+        return fail(CN_ERR_CUDA, "upload of the tapes failed: %s", cudaGetErrorString(up_err));
+    }
     H.v = m->d_v;
     H.tape = m->d_v + m->n_ab;
     std::vector<TapeClass> tcls(m->cls.size());
@@ -511,6 +546,9 @@ static int finalize(cn_model *m, double dt) {
     }
   }
 #undef UP
+  // The uploads and memsets above ran on the legacy default stream; the model's stream may be a
+  // non-blocking one (torch's are) that does not wait for it: everything lands before the first launch.
+  CU(cudaDeviceSynchronize());
   CU(cudaEventCreate(&m->ev0));
   CU(cudaEventCreate(&m->ev1));
   m->dt = dt;
