@@ -173,7 +173,7 @@ def run_reference(args):
            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": workload_config(32768),
+           "config": dict(workload_config(32768), sample_desc_sha256=W.desc_hash(desc)),
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
                             "sample": sample},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0,
@@ -320,7 +320,8 @@ def main():
 
     if rank == 0:
         cfg = workload_config(args.n_cell)
-        cfg.update({"replicas": world, "layout": info, "spikes_in_run": n_spikes})
+        cfg.update({"replicas": world, "layout": info, "spikes_in_run": n_spikes,
+                    "desc_sha256": W.desc_hash(desc)})   # the input's hash with every result
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps,
                "us_per_dt": 1e3 * ms_max / total_dt,
