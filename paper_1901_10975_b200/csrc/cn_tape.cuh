@@ -634,6 +634,9 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           M.trace[row * M.n_probe + M.wp_col[p]] =
               *reinterpret_cast<const volatile double *>(M.v + M.wp_pos[p]);  // (never from L1)
     }
+    // one program buffer: the next group's program is requested first, so that its latency runs
+    // beside the fence and the release below
+    if (PB == 1 && has_next && threadIdx.x == 0) load_program(tcn, 0);
     // the signal mbarriers this program did not use complete their phase too
     for (int b = (flush ? 0 : tc.n_bar) + (int)threadIdx.x; b < NB; b += (int)blockDim.x)
       mbar_arrive(sbar_s + 8 * b);
@@ -645,7 +648,6 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
                      : "memory");
       }
     }
-    if (PB == 1 && has_next && threadIdx.x == 0) load_program(tcn, 0);
     if (has_next && !next_started) {  // the next item was not ready when the forward sweep ended
       wait_item(nxt, true);
       start_segment(tgn, tkn);
