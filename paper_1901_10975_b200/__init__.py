@@ -2,7 +2,8 @@
 
 Argument marshalling only: every step of the path (event delivery, nrn_cur, Hines solve, voltage
 update, nrn_state, threshold detection) runs in the CUDA kernels of
-csrc/cn_device.cuh.  There is no CPU fallback; without the built library or a CUDA device the
+csrc/cn_tape.cuh (interleaved kernel) and csrc/cn_device.cuh (warp-cooperative kernel, event
+delivery, point processes).  There is no CPU fallback; without the built library or a CUDA device the
 calls raise.  This package never imports the oracle.
 """
 from __future__ import annotations
