@@ -12,8 +12,11 @@
  *
  * Parity pins (tests/test_oracle_pins.py, P1..P16 of SURVEY.md 8(c)) check it
  * against closed forms, Thomas / dense LU solves, RK4 and exact ring timing.
- * "parity unpinned": the synthetic channel constants / network densities of
- * configs 3 and 5 have no external truth (self-consistency pins P7/P9 only).
+ * The model-level plumbing ica -> cai -> SK of one_step (per-step zeroing of ica, accumulation
+ * over several Ca channels, the order of cai dynamics and SK in nrn_state, the cai floor of
+ * z_inf) is pinned by P9b.
+ * "parity unpinned": the VALUES of the synthetic channel constants / network densities of
+ * configs 3 and 5 have no external truth (every formula they enter is pinned: P7/P8/P9/P9b).
  */
 #ifndef CN_ORACLE_H
 #define CN_ORACLE_H

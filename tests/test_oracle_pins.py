@@ -501,6 +501,147 @@ def test_p9_cadyn_newton_equals_closed_form():
 
 
 # ---------------------------------------------------------------------------------------------
+# P9b: model-level plumbing ica -> cai -> SK inside one_step (O2/O3/O9)
+# ---------------------------------------------------------------------------------------------
+
+def _ca_cell(order=("cadyn", "sk"), v_init=-30.0, second_source=True):
+    """One compartment: pas + Ca_HVA (+ Ca_LVA) as Ca sources, cai dynamics and SK in the given
+    table order, and an IClamp so that v (and with it the Ca current) changes from step to step."""
+    ms = [("pas", {"g": 3e-5, "e": -75.0}, {}),
+          ("hhform", {"gbar": 1e-3}, _hhform_globals("CaHVA"))]
+    if second_source:
+        ms.append(("hhform", {"gbar": 4e-4}, _hhform_globals("CaLVA")))
+    tail = {"cadyn": ("cadyn", {}, dict(gamma=0.05, depth=0.1, tau_d=80.0, cai_min=1e-4)),
+            "sk": ("sk", {"gbar": 2e-4}, dict(E=-85.0, Kd=4.3e-4, n=4.8, tau_z=1.0))}
+    ms += [tail[o] for o in order]
+    ms.append(("iclamp", {"del": 0.0, "dur": 10.0, "amp": 0.3}, {}))
+    return W.single_compartment(ms, v_init=v_init)
+
+
+def _gate_inf_tau(g6, v):
+    vh, k, t0, t1, vt, s = g6
+    return 1 / (1 + math.exp((vh - v) / k)), t0 + t1 / (2 * math.cosh((v - vt) / s))
+
+
+def _ca_current(name, gbar, S, v):
+    p, q, E, _, _ = HHFORM_TABLE[name]
+    return gbar * S[0] ** p * S[1] ** q * (v - E)
+
+
+def _be_cai(cai, ica, dt=DT, gamma=0.05, depth=0.1, tau_d=80.0, cai_min=1e-4):
+    kappa = 1e4 * gamma / (2 * 96485.33212 * depth)
+    return (cai + dt * (-kappa * ica + cai_min / tau_d)) / (1 + dt / tau_d)
+
+
+def test_p9b_ica_feeds_cai_per_step_and_is_zeroed():
+    """cai after step 1 is the closed-form backward-Euler update with the Ca current of step 1
+    (sum over BOTH Ca channels, evaluated at the OLD v with the OLD gates, mA/cm2 -> mM through
+    kappa = 1e4 gamma / (2 F depth)); after step 2 with the current of step 2 ONLY (the per-step
+    zeroing of ica), evaluated with the gates advanced at the end of step 1 and v after step 1.
+    The gate values used here come from the gate formulas, not from the oracle."""
+    v0 = -30.0
+    desc = _ca_cell(v_init=v0)
+    m = OracleModel(desc)
+    m.set_probes([0])
+    # step 1: gates at steady state of v_init
+    S = {}
+    for name in ("CaHVA", "CaLVA"):
+        _, _, _, mg, hg = HHFORM_TABLE[name]
+        S[name] = [_gate_inf_tau(mg, v0)[0], _gate_inf_tau(hg, v0)[0]]
+    ica0 = _ca_current("CaHVA", 1e-3, S["CaHVA"], v0) + _ca_current("CaLVA", 4e-4, S["CaLVA"], v0)
+    assert ica0 < -1e-3                       # an inward current large enough to move cai by %
+    m.run(DT, DT)
+    cai1 = _be_cai(1e-4, ica0)
+    assert abs(cai1 - 1e-4) > 1e-6
+    assert abs(m.get_cai()[0] - cai1) < 1e-16
+    # a single-source reading (accumulation "=" instead of "+=") is visibly different
+    assert abs(_be_cai(1e-4, _ca_current("CaLVA", 4e-4, S["CaLVA"], v0)) - cai1) > 1e-8
+    # step 2: gates were advanced by cnexp at v1 (the new v of step 1)
+    v1 = m.get_trace()[0, 0]
+    assert abs(v1 - v0) > 1e-3
+    for name in ("CaHVA", "CaLVA"):
+        _, _, _, mg, hg = HHFORM_TABLE[name]
+        for j, g6 in enumerate((mg, hg)):
+            inf, tau = _gate_inf_tau(g6, v1)
+            S[name][j] = S[name][j] + (1 - math.exp(-DT / tau)) * (inf - S[name][j])
+    ica1 = _ca_current("CaHVA", 1e-3, S["CaHVA"], v1) + _ca_current("CaLVA", 4e-4, S["CaLVA"], v1)
+    m.run(2 * DT, DT)
+    cai2 = _be_cai(cai1, ica1)
+    assert abs(m.get_cai()[0] - cai2) < 1e-16
+    # without the per-step zeroing step 2 would see ica0 + ica1
+    assert abs(_be_cai(cai1, ica0 + ica1) - cai2) > 1e-7
+    # the oracle's own gates agree with the formulas used above
+    assert abs(m.get_state(1, 0)[0] - _advance(S["CaHVA"][0], HHFORM_TABLE["CaHVA"][3],
+                                               m.get_trace()[1, 0])) < 1e-15
+
+
+def _advance(x, g6, v):
+    inf, tau = _gate_inf_tau(g6, v)
+    return x + (1 - math.exp(-DT / tau)) * (inf - x)
+
+
+def test_p9b_state_order_cadyn_before_or_after_sk():
+    """O9 runs the tables in description order: with cai dynamics BEFORE SK the gate relaxes
+    towards z_inf(cai after this step), with SK first towards z_inf(cai before it).  Initial
+    z = z_inf(cai_min), so in the second case step 1 leaves z exactly where it was."""
+    Kd, n, tau_z = 4.3e-4, 4.8, 1.0
+    zinf = lambda c: 1 / (1 + (Kd / c) ** n)
+    z0 = zinf(1e-4)
+    a = OracleModel(_ca_cell(("cadyn", "sk")))
+    b = OracleModel(_ca_cell(("sk", "cadyn")))
+    a.run(DT, DT)
+    b.run(DT, DT)
+    cai1 = a.get_cai()[0]
+    assert cai1 == b.get_cai()[0]             # cai itself does not depend on the order
+    za = a.get_state(4, 0)[0]                 # tables: pas, CaHVA, CaLVA, cadyn, sk
+    zb = b.get_state(3, 0)[0]                 # tables: pas, CaHVA, CaLVA, sk, cadyn
+    assert abs(za - (z0 + (1 - math.exp(-DT / tau_z)) * (zinf(cai1) - z0))) < 1e-18
+    assert zb == z0
+    assert abs(za - zb) > 1e-3 * z0
+    # SK's current reaches the voltage: a model without SK conductance ends elsewhere
+    a.run(40 * DT, DT)
+    c = _ca_cell(("cadyn", "sk"))
+    c["mechs"][4]["params"]["gbar"] = np.zeros(1)
+    cm_ = OracleModel(c)
+    cm_.run(40 * DT, DT)
+    assert abs(a.get_v()[0] - cm_.get_v()[0]) > 1e-9
+
+
+def test_p9b_cai_fixed_point_with_a_real_channel_current():
+    """Voltage-clamp-like check of the units of kappa with a real channel current: a huge membrane
+    capacitance pins v, the Ca gates sit at their steady state for that v, and cai must converge to
+    cai_min - kappa * ica * tau_d with ica = gbar m_inf^2 h_inf (v - E_Ca) from the formulas."""
+    v0 = -25.0
+    desc = _ca_cell(v_init=v0, second_source=False)
+    desc["cm"] = np.array([1e12])
+    desc["mechs"] = [x for x in desc["mechs"] if x["type"] not in ("iclamp", "sk")]
+    m = OracleModel(desc)
+    m.run(3000.0, 0.5)
+    _, _, _, mg, hg = HHFORM_TABLE["CaHVA"]
+    S = [_gate_inf_tau(mg, v0)[0], _gate_inf_tau(hg, v0)[0]]
+    ica = _ca_current("CaHVA", 1e-3, S, v0)
+    kappa = 1e4 * 0.05 / (2 * 96485.33212 * 0.1)
+    star = 1e-4 - kappa * ica * 80.0
+    assert abs(m.get_v()[0] - v0) < 1e-7
+    assert star > 5e-3 and abs(m.get_cai()[0] - star) < 1e-8 * star
+
+
+def test_p9b_sk_cai_floor():
+    """z_inf floors cai at 1e-9 mM: cai = 0, 1e-12 and negative values give the
+    1e-9 value, which is 1 / (1 + (Kd/1e-9)^n); just above the floor the value moves again.
+    (z starts at 0 so that the tiny z_inf is not absorbed by rounding.)"""
+    G = {"E": -85.0, "Kd": 4.3e-4, "n": 4.8, "tau_z": 1.0}
+    ref, _ = oracle.mech_state("sk", {"gbar": 1e-3}, G, [0.0], -60.0, DT, cai=1e-9)
+    for cai in (0.0, 1e-12, -1e-5):
+        S, _ = oracle.mech_state("sk", {"gbar": 1e-3}, G, [0.0], -60.0, DT, cai=cai)
+        assert S[0] == ref[0]
+    zinf = 1 / (1 + (4.3e-4 / 1e-9) ** 4.8)
+    assert ref[0] > 0 and abs(ref[0] / ((1 - math.exp(-DT)) * zinf) - 1) < 1e-13
+    above, _ = oracle.mech_state("sk", {"gbar": 1e-3}, G, [0.0], -60.0, DT, cai=2e-9)
+    assert abs(above[0] / ref[0] - 2 ** 4.8) < 1e-9 * 2 ** 4.8
+
+
+# ---------------------------------------------------------------------------------------------
 # P10: event and clamp timing on the integer step grid (R4, R10)
 # ---------------------------------------------------------------------------------------------
 
@@ -804,6 +945,9 @@ def test_p13_permuting_cells_permutes_results_bitwise():
 # ---------------------------------------------------------------------------------------------
 
 def test_p14_node_renumbering():
+    # (weight 0.4 / amp 4.0: with the generator's defaults -- 0.08 uS, 0.5 nA -- these small cells
+    # never reach threshold, so the pin would compare sub-threshold voltages only; with the stronger
+    # drive 12 spikes travel round the ring and the spike list is part of the comparison)
     desc = W.random_tree_cells(3, 30, 60, stream="p14", weight=0.4, amp=4.0)
     ren = W.renumber_nodes(desc)
     m, mr = OracleModel(desc), OracleModel(ren)
@@ -812,6 +956,7 @@ def test_p14_node_renumbering():
     v, vr = m.get_v(), mr.get_v()
     assert not np.array_equal(ren["parent"], desc["parent"])
     assert np.max(np.abs(vr[ren["_new_of_old"]] - v)) < 1e-10
+    assert len(m.get_spikes()[0]) >= 10
     assert [list(x) for x in m.get_spikes()] == [list(x) for x in mr.get_spikes()]
 
 
