@@ -108,6 +108,35 @@ typedef struct {
 /* Validate, find shape classes, choose the permutation, upload.  *out is NULL on failure. */
 int cn_model_create(const cn_model_desc *desc, cn_model **out);
 
+/* The same with options: "key=value;key=value" (';', ',' or white space between pairs; values are
+ * numbers; NULL or "" = defaults; an unknown key or a malformed pair -> CN_ERR_ARG).  Options are
+ * fixed for the life of the model.  The library reads NO environment variable and has no global
+ * flag: these are the only knobs, and every one of them leaves the results unchanged (within the
+ * parity tolerance) -- they choose between launch strategies:
+ *   tape             -1 auto / 0 / 1   which kernel: 1 every class with enough cells on the
+ *                                      interleaved kernel, 0 all cells on the warp-cooperative one
+ *   tape_min_cells   8192              auto: models at least this large use the interleaved kernel
+ *   tape_min_group   16 (1 for small   smallest ragged group of a class kept on the interleaved
+ *                    models)           kernel
+ *   tape_w           8                 warps per CTA of the interleaved kernel (1..16)
+ *   tape_s, tape_ch  2, 16 (auto)      TMA ring of a warp: stages x rows per chunk
+ *   tape_tmem        1                 0: all system rows in shared memory, none in tensor memory
+ *   tape_window      1                 0: one launch sequence per dt even where a min-delay window
+ *                                      per launch is possible
+ *   tape_pbuf, tape_ctas_per_sm        program buffers (1/2) and CTAs per SM (1/2), default auto
+ *   tape_pf          0                 rows of L2 prefetch ahead of the ring
+ *   tape_leaf_first, tape_hcost, tape_gran, tape_mcost, tape_bcost
+ *                                      cost model of the static schedule
+ *   force_g, max_g, warp_smem, wpb     warp-cooperative kernel: cells per warp, shared-memory cap
+ *                                      per warp, warps per block
+ *   graph            1                 0: per-dt launch sequences are issued one by one instead of
+ *                                      being replayed from a CUDA graph
+ *   onchip           -1 auto / 0 / 1   on-chip window mode: a model that fits the
+ *                                      shared memory of the device is integrated a whole min-delay
+ *                                      window per launch without touching HBM in between
+ *   debug            0                 1: set-up timings on stderr */
+int cn_model_create_opts(const cn_model_desc *desc, const char *options, cn_model **out);
+
 /* Advance to ABSOLUTE time tstop with fixed step dt: K = llround(tstop/dt) - steps_done steps
  * (K <= 0 is a no-op).  dt is fixed by the first call.  Runs on `stream` set by cn_set_stream
  * (default: the legacy default stream) and synchronises it before returning.
@@ -160,14 +189,19 @@ int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
  * tape bytes, shared-memory bytes per CTA of the interleaved kernel (after the first cn_run),
  * warps per CTA | persistent CTAs << 8 | shared-memory system rows << 24 }. */
 int cn_get_layout_info(const cn_model *m, int64_t *info8);
-/* Checkpoint / restore.  A checkpoint holds the complete dynamic state after
- * the last step: voltages, mechanism and synapse states, threshold flags, and the spikes recorded
- * so far.  No event queue is saved: the events still in flight are regenerated from the spikes
- * and the NetCon delays (L156: in-flight events collapse to their originating spikes).  It is a
- * dump in the library's internal layout: load it into a model created from the SAME description
- * with the same library build and settings (checked: CN_ERR_ARG otherwise), before or after that
- * model's first cn_run; the run continues from the saved step with the saved dt.  Per-step
- * traces (cn_set_probes) are not part of it.  buf: caller-owned HOST memory. */
+/* Checkpoint / restore.  A checkpoint holds the dynamic state after the last
+ * step and nothing else, in the CALLER'S order: voltages, mechanism and synapse states, cai,
+ * threshold flags, and the spikes recorded so far (state-sized: 8 B per node and per state).  No
+ * event queue is saved: the events still in flight are regenerated from the spikes and the NetCon
+ * delays (L156: in-flight events collapse to their originating spikes).  No parameter and nothing
+ * of the internal layout is in it, so it loads into ANY model with the same structure -- cells,
+ * topology, mechanism tables and their nodes (hashed; CN_ERR_ARG otherwise) -- whatever that
+ * model's parameters, stimuli (IClamp tables, scripted sources), NetCon weights, options or launch
+ * mode: "launch multiple simulations with different stimuli" (L156).  The restored model continues
+ * from the saved step with the saved dt (CN_ERR_DT if it already runs with another dt), with ITS
+ * OWN parameters and NetCons.  Load before or after the model's first cn_run.  Every check is done
+ * before the model is touched: a rejected buffer leaves the model as it was.  Per-step traces
+ * (cn_set_probes) are not part of it.  buf: caller-owned HOST memory. */
 int cn_checkpoint_size(const cn_model *m, int64_t *bytes_out);
 int cn_checkpoint_save(const cn_model *m, void *buf, int64_t bytes);
 int cn_checkpoint_load(cn_model *m, const void *buf, int64_t bytes);

@@ -37,7 +37,7 @@ MECH = {
     "gap": (10, ("g", "peer"), ()),
 }
 
-EXPORTS = ("cn_model_create", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
+EXPORTS = ("cn_model_create", "cn_model_create_opts", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
            "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_steps_done",
            "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_get_kernel_timing", "cn_get_layout_info", "cn_set_spike_capacity",
            "cn_checkpoint_size", "cn_checkpoint_save", "cn_checkpoint_load",
@@ -80,6 +80,7 @@ def lib():
         L = C.CDLL(str(_SO))
         vp = C.c_void_p
         L.cn_model_create.argtypes = [C.POINTER(_Desc), C.POINTER(vp)]
+        L.cn_model_create_opts.argtypes = [C.POINTER(_Desc), C.c_char_p, C.POINTER(vp)]
         L.cn_run.argtypes = [vp, C.c_double, C.c_double]
         L.cn_run_async.argtypes = [vp, C.c_double, C.c_double]
         L.cn_sync.argtypes = [vp]
@@ -176,15 +177,21 @@ def marshal(desc: dict):
 class Model:
     """cn_model_create / cn_run / cn_get_v / cn_get_spikes with the same names as the C ABI."""
 
-    def __init__(self, desc: dict, marshalled=None, stream=None):
+    def __init__(self, desc: dict, marshalled=None, stream=None, options=None):
+        """options: dict or "key=value;..." string for cn_model_create_opts (include/cn.h)."""
         L = lib()
+        if isinstance(options, dict):
+            options = ";".join(f"{k}={v}" for k, v in options.items())
         d, keep, self.desc_bytes = marshalled if marshalled is not None else marshal(desc)
         self.n_node = int(d.n_node)
         self.n_cell = int(d.n_cell)
         self.mech_n = [int(len(m["node"])) for m in desc["mechs"]] if desc is not None else []
         h = C.c_void_p()
         self._h = None
-        _check(L.cn_model_create(C.byref(d), C.byref(h)))
+        if options:
+            _check(L.cn_model_create_opts(C.byref(d), options.encode(), C.byref(h)))
+        else:
+            _check(L.cn_model_create(C.byref(d), C.byref(h)))
         self._h = h
         self._n_probe = 0
         if stream is not None:

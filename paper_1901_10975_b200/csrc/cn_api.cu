@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cctype>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -39,13 +40,20 @@ static bool finite_all(const double *x, int64_t n) {
 static int build_layout(cn_model *m);
 
 extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
+  return cn_model_create_opts(de, nullptr, out);
+}
+
+extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options, cn_model **out) {
   if (out) *out = nullptr;
   if (!de || !out) return fail(CN_ERR_ARG, "cn_model_create: NULL argument");
+  Options parsed;
+  if (int rc = parsed.parse(options)) return rc;
   if (de->n_cell < 0 || de->n_node < 0) return fail(CN_ERR_ARG, "negative sizes");
   if (de->n_node >= (int64_t)1 << 31) return fail(CN_ERR_ARG, "n_node must be < 2^31");
   if (de->n_mech < 0 || de->n_mech > CN_MAX_TABLES)
     return fail(CN_ERR_MECH, "n_mech must be in [0, %d]", CN_MAX_TABLES);
   const int64_t N = de->n_node;
+  if (de->n_mech > 0 && !de->mech) return fail(CN_ERR_MECH, "NULL mechanism table array");
   if (de->n_cell > 0 &&
       (!de->cell_first || !de->parent || !de->area_um2 || !de->ri_MOhm || !de->cm_uF_cm2 ||
        !de->thr_mV))
@@ -133,6 +141,11 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
     if (fe.code != CN_OK) return fail(fe.code, "%s", fe.msg);
   }
   if (de->n_netcon < 0 || de->n_stim < 0) return fail(CN_ERR_NETCON, "negative count");
+  if (de->n_netcon > 0 && (!de->nc_src_gid || !de->nc_tgt_mech || !de->nc_tgt_inst ||
+                           !de->nc_weight_uS || !de->nc_delay_ms))
+    return fail(CN_ERR_NETCON, "NULL NetCon array with n_netcon > 0");
+  if (de->n_stim > 0 && (!de->stim_gid || !de->stim_t_ms))
+    return fail(CN_ERR_NETCON, "NULL scripted-source array with n_stim > 0");
   int32_t n_src = de->n_cell;
   {
     FirstErr fe;
@@ -172,6 +185,7 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
   cn_model *m = new (std::nothrow) cn_model();
   if (!m) return fail(CN_ERR_NOMEM, "out of host memory");
   try {
+    m->options = parsed;
     m->n_cell = de->n_cell;
     m->N = N;
     m->cell_first.assign(de->cell_first, de->cell_first + (de->n_cell ? de->n_cell + 1 : 0));
@@ -225,17 +239,17 @@ extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
 // ---------------------------------------------------------------------------------------------
 
 template <int WPB>
-static cudaError_t launch_step(cn_model *m, int64_t k) {
+static cudaError_t launch_step(cn_model *m, int64_t k, cudaStream_t st) {
   const int ng = m->hm.n_group;
   const size_t smem = (size_t)WPB * m->warp_smem_doubles * sizeof(double);
-  static bool attr_set[16] = {};
+  bool *attr_set = m->step_attr_set;  // (per model: cudaFuncSetAttribute is per device)
   if (!attr_set[WPB]) {
     cudaError_t e = cudaFuncSetAttribute(step_kernel<WPB>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     attr_set[WPB] = true;
   }
-  step_kernel<WPB><<<(ng + WPB - 1) / WPB, WPB * 32, smem, m->stream>>>(m->hm, k);
+  step_kernel<WPB><<<(ng + WPB - 1) / WPB, WPB * 32, smem, st>>>(m->hm, k);
   return cudaGetLastError();
 }
 
@@ -247,7 +261,9 @@ static size_t tape_smem_bytes(const cn_model *m, int pbuf) {
 
 // Persistent CTAs: as many as fit the device at once (shared memory decides), each looping over
 // the groups blockIdx.x, blockIdx.x + gridDim.x, ...
-static cudaError_t launch_tape(cn_model *m, int64_t k, int mode, int nsteps = 1) {
+static cudaError_t launch_tape(cn_model *m, int64_t k, int mode, int nsteps = 1,
+                               cudaStream_t st = nullptr) {
+  if (!st) st = m->stream;
   auto kern = m->tape_W <= 8 ? tape_step_kernel<256> : tape_step_kernel<512>;
   if (m->tape_ctas == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -273,16 +289,16 @@ static cudaError_t launch_tape(cn_model *m, int64_t k, int mode, int nsteps = 1)
         2 * (tape_smem_bytes(m, 1) + 1024) <= (size_t)smem_sm)
       m->hm.tape_pbuf = 1;
     if (tape_smem_bytes(m, 2) > 227 * 1024) m->hm.tape_pbuf = 1;  // (build_layout fitted one buffer)
-    if (const char *s = std::getenv("CN_TAPE_PBUF")) m->hm.tape_pbuf = std::atoi(s) == 1 ? 1 : 2;
+    if (const char *s = m->opt("tape_pbuf")) m->hm.tape_pbuf = std::atoi(s) == 1 ? 1 : 2;
     const size_t smem = tape_smem_bytes(m, m->hm.tape_pbuf);
     per_sm = (m->tape_W <= 8 && 2 * (smem + 1024) <= (size_t)smem_sm) ? 2 : 1;
-    if (const char *s = std::getenv("CN_TAPE_CTAS_PER_SM")) per_sm = std::max(1, std::min(2, std::atoi(s)));
-    if (std::getenv("CN_DEBUG"))
+    if (const char *s = m->opt("tape_ctas_per_sm")) per_sm = std::max(1, std::min(2, std::atoi(s)));
+    if (m->opt("debug") && std::atoi(m->opt("debug")) != 0)
       fprintf(stderr, "[cn] tape kernel: %zu B smem, %d threads, %d CTAs/SM\n", smem,
               32 * m->tape_W, per_sm);
     m->tape_ctas = std::min(m->hm.n_tgroup, sms * per_sm);
   }
-  kern<<<m->tape_ctas, 32 * m->tape_W, tape_smem_bytes(m, m->hm.tape_pbuf), m->stream>>>(
+  kern<<<m->tape_ctas, 32 * m->tape_W, tape_smem_bytes(m, m->hm.tape_pbuf), st>>>(
       m->hm, k, mode, nsteps);
   return cudaGetLastError();
 }
@@ -343,57 +359,100 @@ static int run_steps(cn_model *m, int64_t K) {
     m->timed = true;
     return CN_OK;
   }
-  for (int64_t s = 0; s < K; ++s) {
-    const int64_t k = m->k + s;
+  // ---- one launch sequence per dt: deliver -> point processes -> step kernels (-> probes) --------
+  // k_arg >= 0: the step itself; k_arg = -(1 + s): step = device counter + s (replayed CUDA graph).
+  auto issue_step = [&](int64_t k_arg, int64_t row_arg, cudaStream_t st, bool timeit) -> int {
     if (m->n_netcon > 0) {
-      deliver_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->hm, k);
+      deliver_kernel<<<deliver_blocks, 128, 0, st>>>(m->hm, k_arg);
       m->launches++;
     }
     if (ntg > 0 && pp_tape > 0) {
-      pp_step_kernel<false><<<pp_blocks, 256, 0, m->stream>>>(m->hm, k);
+      pp_step_kernel<false><<<pp_blocks, 256, 0, st>>>(m->hm, k_arg);
       m->launches++;
     }
     if (ng > 0 && pp_coop > 0) {
-      pp_step_kernel<true><<<ppc_blocks, 256, 0, m->stream>>>(m->hm, k);
+      pp_step_kernel<true><<<ppc_blocks, 256, 0, st>>>(m->hm, k_arg);
       m->launches++;
     }
-    const bool timeit = m->ktime_every > 0 && (k % m->ktime_every) == 0 &&
-                        m->ktime_used < m->ktime_ev.size();
     const bool time_tape = ntg > 0;  // the dominant kernel is the tape kernel when it runs
     if (ng > 0) {
       cudaError_t e;
-      if (timeit && !time_tape) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
+      if (timeit && !time_tape) cudaEventRecord(m->ktime_ev[m->ktime_used].first, st);
       switch (m->wpb) {
-        case 8: e = launch_step<8>(m, k); break;
-        case 4: e = launch_step<4>(m, k); break;
-        case 2: e = launch_step<2>(m, k); break;
-        default: e = launch_step<1>(m, k); break;
+        case 8: e = launch_step<8>(m, k_arg, st); break;
+        case 4: e = launch_step<4>(m, k_arg, st); break;
+        case 2: e = launch_step<2>(m, k_arg, st); break;
+        default: e = launch_step<1>(m, k_arg, st); break;
       }
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "step launch failed: %s", cudaGetErrorString(e));
       if (timeit && !time_tape) {
-        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, st);
         m->ktime_steps.push_back(1);
       }
       m->launches++;
     }
     if (ntg > 0) {
-      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
-      cudaError_t e = launch_tape(m, k, m->state_pending ? TM_ADVANCE : 0);
+      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, st);
+      cudaError_t e = launch_tape(m, k_arg, m->state_pending ? TM_ADVANCE : 0, 1, st);
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
       m->state_pending = true;
       if (timeit) {
-        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, st);
         m->ktime_steps.push_back(1);
       }
       m->launches++;
     }
-    if (!m->probe.empty() && m->probe_rows < m->probe_cap) {
+    if (!m->probe.empty() && (row_arg < 0 || row_arg < m->probe_cap)) {
       const int np = (int)m->probe.size();
-      probe_kernel<<<(np + 127) / 128, 128, 0, m->stream>>>(m->d_v, m->d_probe_pos, np,
-                                                              m->d_trace, m->probe_rows);
-      m->probe_rows++;
+      probe_kernel<<<(np + 127) / 128, 128, 0, st>>>(m->d_v, m->d_probe_pos, np, m->d_trace, row_arg,
+                                                      m->hm.step_ctr, m->probe_cap);
       m->launches++;
     }
+    return CN_OK;
+  };
+  // The sequence of CN_GRAPH_STEPS consecutive steps is captured once into a CUDA graph (on a
+  // stream of the model's own: the caller's may be the legacy default stream, which cannot
+  // capture) and replayed; the kernels of the graph take their step from a device counter that a
+  // one-thread kernel sets in front of every replay.  The first step of a model, runs shorter
+  // than a graph, the remainder of a run and runs with per-launch event timing are issued directly.
+  const bool use_graph = m->graph_on && m->ktime_every == 0;
+  int64_t s = 0;
+  while (s < K) {
+    const int64_t k = m->k + s;
+    const bool warm = m->direct_steps > 0 && (ntg == 0 || m->state_pending);
+    if (use_graph && warm && K - s >= CN_GRAPH_STEPS) {
+      if (!m->graph_exec) {
+        const int64_t l0 = m->launches;
+        if (!m->cap_stream) CU(cudaStreamCreateWithFlags(&m->cap_stream, cudaStreamNonBlocking));
+        CU(cudaStreamBeginCapture(m->cap_stream, cudaStreamCaptureModeThreadLocal));
+        int rc = CN_OK;
+        for (int j = 0; j < CN_GRAPH_STEPS && rc == CN_OK; ++j)
+          rc = issue_step(-(1 + (int64_t)j), -(1 + (int64_t)j), m->cap_stream, false);
+        cudaGraph_t g = nullptr;
+        cudaError_t e = cudaStreamEndCapture(m->cap_stream, &g);
+        m->graph_kernels = m->launches - l0;
+        m->launches = l0;
+        if (rc != CN_OK) { if (g) cudaGraphDestroy(g); return rc; }
+        if (e != cudaSuccess) return fail(CN_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
+        e = cudaGraphInstantiate(&m->graph_exec, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) return fail(CN_ERR_CUDA, "graph instantiation failed: %s", cudaGetErrorString(e));
+      }
+      set_ctr_kernel<<<1, 1, 0, m->stream>>>(m->hm.step_ctr, k, m->probe_rows);
+      CU(cudaGraphLaunch(m->graph_exec, m->stream));
+      m->launches += 1 + m->graph_kernels;
+      m->graph_replays++;
+      if (!m->probe.empty()) m->probe_rows = std::min(m->probe_cap, m->probe_rows + CN_GRAPH_STEPS);
+      s += CN_GRAPH_STEPS;
+      continue;
+    }
+    const bool timeit = m->ktime_every > 0 && (k % m->ktime_every) == 0 &&
+                        m->ktime_used < m->ktime_ev.size();
+    int rc = issue_step(k, m->probe_rows, m->stream, timeit);
+    if (rc != CN_OK) return rc;
+    if (!m->probe.empty() && m->probe_rows < m->probe_cap) m->probe_rows++;
+    m->direct_steps++;
+    ++s;
   }
   CU(cudaEventRecord(m->ev1, m->stream));
   CU(cudaGetLastError());
@@ -511,46 +570,6 @@ extern "C" int cn_get_trace(const cn_model *cm, double *out, int64_t cap_steps, 
   return CN_OK;
 }
 
-extern "C" int cn_get_state(const cn_model *cm, int32_t t, int32_t s, double *out, int64_t n) {
-  cn_model *m = const_cast<cn_model *>(cm);
-  if (!m || !out) return fail(CN_ERR_ARG, "NULL argument");
-  if (t < 0 || t >= (int)m->tab.size()) return fail(CN_ERR_MECH, "table out of range");
-  HTable &T = m->tab[t];
-  if (s < 0 || s >= T.ti.n_state || n != T.n) return fail(CN_ERR_MECH, "state / size mismatch");
-  if (!m->uploaded) return fail(CN_ERR_ARG, "states exist after the first cn_run");
-  if (n == 0) return CN_OK;
-  if (m->state_pending && !T.ti.point && m->hm.n_tgroup > 0) {
-    // the interleaved kernel applies nrn_state of a step at the start of the next one: do it now
-    cudaError_t e = launch_tape(m, m->k, TM_ADVANCE | TM_FLUSH);
-    if (e != cudaSuccess) return fail(CN_ERR_CUDA, "state flush failed: %s", cudaGetErrorString(e));
-    m->launches++;
-    m->state_pending = false;
-  }
-  // instances live in the table arrays (cooperative groups) or on a tape (interleaved groups)
-  std::vector<int64_t> loc((size_t)n);
-  for (int64_t i = 0; i < n; ++i) {
-    const bool on_tape = !T.ti.point && T.tape_loc[i] >= 0;
-    loc[i] = on_tape ? -(T.tape_loc[i] + (int64_t)T.ti.n_dev_param * 32 + 1) : T.inst_pos[i];
-  }
-  int64_t *d_loc = nullptr;
-  double *d_out = nullptr;
-  CU(cudaMalloc(&d_loc, (size_t)n * sizeof(int64_t)));
-  if (cudaMalloc(&d_out, (size_t)n * sizeof(double)) != cudaSuccess) {
-    cudaFree(d_loc);
-    return fail(CN_ERR_NOMEM, "out of device memory");
-  }
-  cudaMemcpyAsync(d_loc, loc.data(), (size_t)n * sizeof(int64_t), cudaMemcpyHostToDevice, m->stream);
-  gather_state_kernel<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(
-      m->hm.tape, T.d_state[s], d_loc, n, s, d_out);
-  m->launches++;
-  cudaMemcpyAsync(out, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, m->stream);
-  cudaError_t e = cudaStreamSynchronize(m->stream);
-  cudaFree(d_loc);
-  cudaFree(d_out);
-  if (e != cudaSuccess) return fail(CN_ERR_CUDA, "cn_get_state: %s", cudaGetErrorString(e));
-  return CN_OK;
-}
-
 extern "C" int64_t cn_steps_done(const cn_model *m) { return m ? m->k : 0; }
 extern "C" int64_t cn_launch_count(const cn_model *m) { return m ? m->launches : 0; }
 
@@ -579,142 +598,7 @@ extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
   return CN_OK;
 }
 
-// ---------------------------------------------------------------------------------------------
-// checkpoint / restore (L134-156)
-// ---------------------------------------------------------------------------------------------
-
-struct CkHeader {
-  uint64_t magic;
-  int64_t k, n_sp, win_idx, n_blob;
-  double dt;
-  int32_t state_pending, window;
-  uint64_t layout;  // hash of everything the raw dump depends on
-};
-
-static uint64_t ck_layout_hash(const cn_model *m) {
-  uint64_t h = mix64(0xC0FFEEull, (uint64_t)m->N);
-  h = mix64(h, (uint64_t)m->n_cell);
-  h = mix64(h, (uint64_t)m->n_ab);
-  h = mix64(h, (uint64_t)m->n_tape);
-  h = mix64(h, (uint64_t)m->n_pcell);
-  h = mix64(h, (uint64_t)m->tape_W * 1000003u + (uint64_t)m->tape_CH * 1009u + (uint64_t)m->tape_S);
-  h = mix64(h, (uint64_t)m->cls.size());
-  for (const HTable &T : m->tab) h = mix64(h, (uint64_t)T.n_dev * 31u + (uint64_t)T.type);
-  for (const TapeGroup &tg : m->tgrp) h = mix64(h, (uint64_t)tg.tape_base + (uint64_t)tg.cls);
-  return h;
-}
-
-// every device array that changes during cn_run and is live at a step boundary
-static std::vector<std::pair<void *, size_t>> ck_blobs(const cn_model *m, int64_t n_sp) {
-  std::vector<std::pair<void *, size_t>> b;
-  const DModel &H = m->hm;
-  b.emplace_back(m->d_v, (size_t)(m->n_ab + m->n_tape) * sizeof(double));
-  for (const HTable &T : m->tab)
-    for (int j = 0; j < T.ti.n_state; ++j)
-      if (T.d_state[j]) b.emplace_back(T.d_state[j], (size_t)std::max<int64_t>(T.n_dev, 1) * sizeof(double));
-  if (m->d_cai) b.emplace_back(m->d_cai, (size_t)m->n_pnode * sizeof(double));
-  b.emplace_back(H.flag, (size_t)m->n_pcell);
-  b.emplace_back(m->d_sp_gid, (size_t)n_sp * sizeof(int32_t));
-  b.emplace_back(m->d_sp_step, (size_t)n_sp * sizeof(int64_t));
-  b.emplace_back(m->d_nsp, sizeof(unsigned long long));
-  b.emplace_back(H.sp_end, (size_t)H.wr * sizeof(int64_t));
-  if (m->window) {
-    b.emplace_back(H.win_mark_step, (size_t)H.win_mark_cap * sizeof(int64_t));
-    b.emplace_back(H.win_mark_nsp, (size_t)H.win_mark_cap * sizeof(int64_t));
-  }
-  return b;
-}
-
-static int ck_spike_count(const cn_model *m, int64_t *n_sp) {
-  unsigned long long ns = 0;
-  CU(cudaStreamSynchronize(m->stream));
-  CU(cudaMemcpy(&ns, m->d_nsp, sizeof(ns), cudaMemcpyDeviceToHost));
-  *n_sp = (int64_t)std::min<unsigned long long>(ns, (unsigned long long)m->sp_cap);
-  return CN_OK;
-}
-
-extern "C" int cn_checkpoint_size(const cn_model *m, int64_t *bytes_out) {
-  if (!m || !bytes_out) return fail(CN_ERR_ARG, "NULL argument");
-  if (!m->uploaded) return fail(CN_ERR_ARG, "nothing to checkpoint before the first cn_run");
-  int64_t n_sp = 0;
-  int rc = ck_spike_count(m, &n_sp);
-  if (rc != CN_OK) return rc;
-  size_t tot = sizeof(CkHeader);
-  for (auto &b : ck_blobs(m, n_sp)) tot += sizeof(uint64_t) + ((b.second + 7) & ~(size_t)7);
-  *bytes_out = (int64_t)tot;
-  return CN_OK;
-}
-
-extern "C" int cn_checkpoint_save(const cn_model *m, void *buf, int64_t bytes) {
-  if (!m || !buf) return fail(CN_ERR_ARG, "NULL argument");
-  if (!m->uploaded) return fail(CN_ERR_ARG, "nothing to checkpoint before the first cn_run");
-  int64_t n_sp = 0;
-  int rc = ck_spike_count(m, &n_sp);
-  if (rc != CN_OK) return rc;
-  const auto blobs = ck_blobs(m, n_sp);
-  size_t tot = sizeof(CkHeader);
-  for (auto &b : blobs) tot += sizeof(uint64_t) + ((b.second + 7) & ~(size_t)7);
-  if ((size_t)bytes < tot) return fail(CN_ERR_ARG, "checkpoint buffer too small (%zu needed)", tot);
-  char *p = static_cast<char *>(buf);
-  CkHeader h{};
-  h.magic = 0x434E434B50543031ull;  // "CNCKPT01"
-  h.k = m->k;
-  h.n_sp = n_sp;
-  h.win_idx = m->win_idx;
-  h.n_blob = (int64_t)blobs.size();
-  h.dt = m->dt;
-  h.state_pending = m->state_pending ? 1 : 0;
-  h.window = m->window ? 1 : 0;
-  h.layout = ck_layout_hash(m);
-  memcpy(p, &h, sizeof(h));
-  p += sizeof(h);
-  for (auto &b : blobs) {
-    const uint64_t sz = b.second;
-    memcpy(p, &sz, sizeof(sz));
-    p += sizeof(sz);
-    if (sz) CU(cudaMemcpy(p, b.first, sz, cudaMemcpyDeviceToHost));
-    p += (sz + 7) & ~(size_t)7;
-  }
-  return CN_OK;
-}
-
-extern "C" int cn_checkpoint_load(cn_model *m, const void *buf, int64_t bytes) {
-  if (!m || !buf) return fail(CN_ERR_ARG, "NULL argument");
-  if ((size_t)bytes < sizeof(CkHeader)) return fail(CN_ERR_ARG, "not a checkpoint");
-  const char *p = static_cast<const char *>(buf);
-  CkHeader h;
-  memcpy(&h, p, sizeof(h));
-  p += sizeof(h);
-  if (h.magic != 0x434E434B50543031ull) return fail(CN_ERR_ARG, "not a checkpoint");
-  if (!m->uploaded) {
-    int rc = finalize(m, h.dt);
-    if (rc != CN_OK) return rc;
-  } else if (h.dt != m->dt) {
-    return fail(CN_ERR_DT, "checkpoint was taken with dt = %.17g, the model runs with %.17g", h.dt, m->dt);
-  }
-  if (h.layout != ck_layout_hash(m) || (h.window != 0) != m->window)
-    return fail(CN_ERR_ARG, "checkpoint of a different model, library build or launch mode");
-  if (h.n_sp > m->sp_cap) return fail(CN_ERR_OVERFLOW, "checkpoint holds more spikes than the buffer");
-  const auto blobs = ck_blobs(m, h.n_sp);
-  if ((int64_t)blobs.size() != h.n_blob) return fail(CN_ERR_ARG, "checkpoint layout mismatch");
-  CU(cudaStreamSynchronize(m->stream));
-  const char *end = static_cast<const char *>(buf) + bytes;
-  for (auto &b : blobs) {
-    uint64_t sz;
-    if (p + sizeof(sz) > end) return fail(CN_ERR_ARG, "checkpoint truncated");
-    memcpy(&sz, p, sizeof(sz));
-    p += sizeof(sz);
-    if (sz != b.second || p + sz > end) return fail(CN_ERR_ARG, "checkpoint layout mismatch");
-    if (sz) CU(cudaMemcpy(b.first, p, sz, cudaMemcpyHostToDevice));
-    p += (sz + 7) & ~(size_t)7;
-  }
-  CU(cudaDeviceSynchronize());  // (the model's stream may not wait for the legacy default stream)
-  m->k = h.k;
-  m->win_idx = h.win_idx;
-  m->state_pending = h.state_pending != 0;
-  m->probe_rows = 0;
-  return CN_OK;
-}
+#include "cn_checkpoint.hpp"
 
 extern "C" int cn_set_spike_capacity(cn_model *m, int64_t cap) {
   if (!m || cap < 1) return fail(CN_ERR_ARG, "bad capacity");
@@ -763,12 +647,16 @@ extern "C" void cn_model_destroy(cn_model *m) {
   if (m->uploaded) cudaStreamSynchronize(m->stream);
   for (auto &pr : m->ktime_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   for (void *p : m->dev_allocs) cudaFree(p);
+  if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);
+  if (m->graph_exec) cudaGraphExecDestroy(m->graph_exec);
+  if (m->cap_stream) cudaStreamDestroy(m->cap_stream);
   delete m;
 }
 
-// debugging aid for DESIGN/bench: positions per task of the first tape class
+#ifdef CN_TRACE
+// development builds only (CN_TRACE=1): positions per task of the first tape class, phase clocks
 extern "C" int cn_debug_tasks(const cn_model *m, int32_t *out, int32_t cap) {
   for (const HClass &K : m->cls) {
     if (K.tp.n_groups == 0) continue;
@@ -785,7 +673,6 @@ extern "C" int cn_debug_tasks(const cn_model *m, int32_t *out, int32_t cap) {
   return 0;
 }
 
-#ifdef CN_TRACE
 extern "C" int cn_debug_trace(long long *out) {
   return (int)cudaMemcpyFromSymbol(out, cn::g_trace, sizeof(long long) * 148 * 16 * 8 * 8);
 }

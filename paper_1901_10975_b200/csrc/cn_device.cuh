@@ -175,6 +175,7 @@ struct DModel {
   double *trace;                // [trace_cap][n_probe]
   int64_t trace_row0, trace_cap;  // row of the first step of this launch
   int32_t n_probe, pad3;
+  int64_t *step_ctr;            // [0] step, [1] trace row that a replayed CUDA graph starts from
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
 };
@@ -430,6 +431,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 8 ? 1 : 12 / WPB)
     step_kernel(const __grid_constant__ DModel M,
                                                         int64_t k) {
   extern __shared__ double smem[];
+  if (k < 0) k = M.step_ctr[0] - k - 1;  // replayed graph: the device counter + offset
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = blockIdx.x * WPB + warp;
   if (g >= M.n_group) return;
@@ -680,6 +682,7 @@ __device__ __forceinline__ void deliver_source(const DModel &M, int32_t gid, int
 
 __global__ void __launch_bounds__(128) deliver_kernel(const __grid_constant__ DModel M,
                                                       int64_t k) {
+  if (k < 0) k = M.step_ctr[0] - k - 1;  // replayed graph: the device counter + offset
   const int lane = threadIdx.x & 31;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
@@ -830,15 +833,29 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
 }
 
 __global__ void probe_kernel(const double *__restrict__ v, const int64_t *__restrict__ pos,
-                             int n_probe, double *__restrict__ trace, int64_t row) {
+                             int n_probe, double *__restrict__ trace, int64_t row,
+                             const int64_t *__restrict__ ctr, int64_t cap) {
+  if (row < 0) row = ctr[1] - row - 1;  // replayed graph: the device counter + offset
+  if (row >= cap) return;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j < n_probe) trace[row * n_probe + j] = v[pos[j]];
+}
+
+__global__ void set_ctr_kernel(int64_t *ctr, int64_t k, int64_t row) {
+  ctr[0] = k;
+  ctr[1] = row;
 }
 
 __global__ void gather_kernel(const double *__restrict__ src, const int64_t *__restrict__ pos,
                               int64_t n, double *__restrict__ out) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = src[pos[i]];
+}
+
+__global__ void scatter_kernel(double *__restrict__ dst, const int64_t *__restrict__ pos,
+                               int64_t n, const double *__restrict__ src) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[pos[i]] = src[i];
 }
 
 }  // namespace cn

@@ -8,7 +8,7 @@
 // ---------------------------------------------------------------------------------------------
 
 static int finalize(cn_model *m, double dt) {
-  const bool dbg = std::getenv("CN_DEBUG") != nullptr;
+  const bool dbg = m->opt("debug") && std::atoi(m->opt("debug")) != 0;
   auto t_prev = std::chrono::steady_clock::now();
   auto lap = [&](const char *what) {
     if (!dbg) return;
@@ -410,7 +410,7 @@ static int finalize(cn_model *m, double dt) {
     H.tape_sys_cap = std::max(m->tape_sys_cap, 1);
     H.tape_bar_cap = m->tape_bar_cap;
     H.tape_pf = 0;  // measured on config 4: prefetching ahead of the ring only costs (0: off)
-    if (const char *e = std::getenv("CN_TAPE_PF")) H.tape_pf = std::max(0, std::min(4096, std::atoi(e)));
+    if (const char *e = m->opt("tape_pf")) H.tape_pf = std::max(0, std::min(4096, std::atoi(e)));
     for (int t = 0; t < nt; ++t) {
       H.tab[t].pp_tape_begin = m->tab[t].pp_tape_begin;
       H.tab[t].pp_tape_end = m->tab[t].ti.point ? m->tab[t].n : 0;
@@ -480,7 +480,7 @@ static int finalize(cn_model *m, double dt) {
     bool ok = m->hm.n_tgroup > 0 && m->grp.empty();
     for (const HTable &T : m->tab)
       if ((T.type == CN_AMPANMDA || T.type == CN_GAP) && T.n > 0) ok = false;
-    if (const char *e = std::getenv("CN_TAPE_WINDOW")) ok = ok && std::atoi(e) != 0;
+    if (const char *e = m->opt("tape_window")) ok = ok && std::atoi(e) != 0;
     int64_t wn = m->n_netcon > 0 ? std::min<int64_t>(H.mind, 64) : 32;
     if (wn < 2) ok = false;
     if (ok && (m->win_stride + m->win_ninst) * wn * 8 > ((int64_t)4 << 30)) ok = false;
@@ -500,6 +500,8 @@ static int finalize(cn_model *m, double dt) {
       rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_nsp); if (rc != CN_OK) return rc;
     }
   }
+  rc = dev_alloc(m, 2, &H.step_ctr); if (rc != CN_OK) return rc;
+  if (const char *e = m->opt("graph")) m->graph_on = std::atoi(e) != 0;
   // spikes
   rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_gid, false); if (rc) return rc;
   rc = dev_alloc(m, (size_t)m->sp_cap, &m->d_sp_step, false); if (rc) return rc;

@@ -7,6 +7,8 @@
 // errors
 // ---------------------------------------------------------------------------------------------
 
+#define CN_GRAPH_STEPS 20  // per-dt launch sequences per CUDA graph
+
 static thread_local char g_err[512] = "";
 
 static int fail(int code, const char *fmt, ...) {
@@ -239,7 +241,53 @@ struct HClass {
   int nodeoff_off = 0;
 };
 
+// Options of one model, fixed at cn_model_create_opts ("key=value;key=value"; include/cn.h lists
+// them).  The library reads no environment variable and has no global flag.
+static const char *const kOptionKeys[] = {
+    "tape", "tape_min_cells", "tape_min_group", "tape_w", "tape_s", "tape_ch", "tape_tmem",
+    "tape_leaf_first", "tape_hcost", "tape_gran", "tape_mcost", "tape_bcost", "tape_pf",
+    "tape_window", "tape_pbuf", "tape_ctas_per_sm", "force_g", "max_g", "warp_smem", "wpb",
+    "graph", "onchip", "debug"};
+
+struct Options {
+  std::vector<std::pair<std::string, std::string>> kv;
+  const char *get(const char *key) const {
+    for (const auto &p : kv)
+      if (p.first == key) return p.second.c_str();
+    return nullptr;
+  }
+  // "k=v;k=v" (';', ',' or white space between the pairs); CN_OK or CN_ERR_ARG with a message
+  int parse(const char *str) {
+    kv.clear();
+    if (!str) return CN_OK;
+    std::string s(str);
+    size_t i = 0;
+    while (i < s.size()) {
+      while (i < s.size() && (s[i] == ';' || s[i] == ',' || std::isspace((unsigned char)s[i]))) ++i;
+      size_t j = i;
+      while (j < s.size() && s[j] != ';' && s[j] != ',' && !std::isspace((unsigned char)s[j])) ++j;
+      if (j == i) break;
+      const std::string item = s.substr(i, j - i);
+      i = j;
+      const size_t eq = item.find('=');
+      if (eq == std::string::npos || eq == 0 || eq + 1 == item.size())
+        return fail(CN_ERR_ARG, "option '%s' is not key=value", item.c_str());
+      const std::string key = item.substr(0, eq), val = item.substr(eq + 1);
+      bool known = false;
+      for (const char *k : kOptionKeys) known = known || key == k;
+      if (!known) return fail(CN_ERR_ARG, "unknown option '%s'", key.c_str());
+      char *end = nullptr;
+      (void)std::strtod(val.c_str(), &end);
+      if (!end || *end != '\0') return fail(CN_ERR_ARG, "option '%s': '%s' is not a number", key.c_str(), val.c_str());
+      kv.emplace_back(key, val);
+    }
+    return CN_OK;
+  }
+};
+
 struct cn_model {
+  Options options;
+  const char *opt(const char *key) const { return options.get(key); }
   // description (deep copy)
   int32_t n_cell = 0;
   int64_t N = 0;
@@ -286,6 +334,7 @@ struct cn_model {
   int n_cgroup = 0;                 // warp-cooperative groups come first in the group numbering
   std::vector<double> cai0;         // initial cai per caller node (when any table needs it)
   int warp_smem_doubles = 0, wpb = 4;
+  bool step_attr_set[16] = {};      // shared-memory opt-in of step_kernel<WPB> done on this model's device
   bool any_ica = false, any_cai = false;
   // run state
   double dt = 0.0;
@@ -299,6 +348,16 @@ struct cn_model {
   int ktime_every = 0;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ktime_ev;
   size_t ktime_used = 0;
+  // CUDA graph of CN_GRAPH_STEPS per-dt launch sequences (cn_api.cu run_steps)
+  bool graph_on = true;
+  cudaGraphExec_t graph_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;
+  int64_t graph_kernels = 0, graph_replays = 0, direct_steps = 0;
+  // checkpoints / state read-back
+  uint64_t ck_hash = 0;
+  bool ck_hash_done = false;
+  void *d_scratch = nullptr;
+  size_t scratch_bytes = 0;
   // probes
   std::vector<int32_t> probe;
   int64_t probe_cap = 0, probe_rows = 0;

@@ -18,7 +18,7 @@ static int tape_rows_of(const TypeInfo &ti, int type) {
 #include "cn_tape_program.hpp"
 
 static int build_layout(cn_model *m) {
-  const bool dbg = std::getenv("CN_DEBUG") != nullptr;
+  const bool dbg = m->opt("debug") && std::atoi(m->opt("debug")) != 0;
   auto t_prev = std::chrono::steady_clock::now();
   auto lap = [&](const char *what) {
     if (!dbg) return;
@@ -163,31 +163,31 @@ static int build_layout(cn_model *m) {
   // the model is large enough to fill the GPU that way; everything else (small classes, small
   // models, the ragged remainder of a class) goes to the warp-cooperative kernel.
   int tape_mode = -1;  // -1 auto, 0 off, 1 on
-  if (const char *e = std::getenv("CN_TAPE")) tape_mode = std::atoi(e);
+  if (const char *e = m->opt("tape")) tape_mode = std::atoi(e);
   int64_t tape_min_cells = 8192;
-  if (const char *e = std::getenv("CN_TAPE_MIN_CELLS")) tape_min_cells = std::atoll(e);
+  if (const char *e = m->opt("tape_min_cells")) tape_min_cells = std::atoll(e);
   int tape_min_group = 16;  // a ragged last group needs at least this many cells
-  if (const char *e = std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = std::max(1, std::atoi(e));
+  if (const char *e = m->opt("tape_min_group")) tape_min_group = std::max(1, std::atoi(e));
   // A smaller model goes to the interleaved kernel too if ALL of it fits there (then it runs in
   // window mode: one launch per min-delay window instead of three per dt) and its groups fill at
   // least a quarter of their lanes; decided after the programs are compiled (below).
   const bool auto_small = tape_mode == -1 && nc < tape_min_cells && nc > 0;
-  if (auto_small && !std::getenv("CN_TAPE_MIN_GROUP")) tape_min_group = 1;
+  if (auto_small && !m->opt("tape_min_group")) tape_min_group = 1;
   const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells) || auto_small;
   // W warps per group (CTA), each with a ring of S chunks x CH rows; the whole CTA must fit the
   // 227 KB of shared memory next to the group's system (512 B per node)
   m->tape_W = 8;
-  if (const char *e = std::getenv("CN_TAPE_W")) m->tape_W = std::min(16, std::max(1, std::atoi(e)));
+  if (const char *e = m->opt("tape_w")) m->tape_W = std::min(16, std::max(1, std::atoi(e)));
   m->tape_S = 2;
   m->tape_CH = 16;
-  if (const char *e = std::getenv("CN_TAPE_S")) m->tape_S = std::min(4, std::max(2, std::atoi(e)));
-  if (const char *e = std::getenv("CN_TAPE_CH")) m->tape_CH = std::min(63, std::max(7, std::atoi(e)));
-  if (const char *e = std::getenv("CN_TAPE_TMEM")) m->tape_tmem = std::atoi(e) != 0;
-  if (const char *e = std::getenv("CN_TAPE_LEAF_FIRST")) m->tape_leaf_first = std::atoi(e) != 0;
-  if (const char *e = std::getenv("CN_TAPE_HCOST")) m->tape_hcost = std::atof(e);
-  if (const char *e = std::getenv("CN_TAPE_GRAN")) m->tape_gran = std::max(1.0, std::atof(e));
-  if (const char *e = std::getenv("CN_TAPE_MCOST")) m->tape_mcost_scale = std::atof(e);
-  if (const char *e = std::getenv("CN_TAPE_BCOST")) m->tape_bcost = std::atof(e);
+  if (const char *e = m->opt("tape_s")) m->tape_S = std::min(4, std::max(2, std::atoi(e)));
+  if (const char *e = m->opt("tape_ch")) m->tape_CH = std::min(63, std::max(7, std::atoi(e)));
+  if (const char *e = m->opt("tape_tmem")) m->tape_tmem = std::atoi(e) != 0;
+  if (const char *e = m->opt("tape_leaf_first")) m->tape_leaf_first = std::atoi(e) != 0;
+  if (const char *e = m->opt("tape_hcost")) m->tape_hcost = std::atof(e);
+  if (const char *e = m->opt("tape_gran")) m->tape_gran = std::max(1.0, std::atof(e));
+  if (const char *e = m->opt("tape_mcost")) m->tape_mcost_scale = std::atof(e);
+  if (const char *e = m->opt("tape_bcost")) m->tape_bcost = std::atof(e);
   m->cell_tape.assign(nc, 0);
   for (HClass &K : m->cls) {
     K.count = (int64_t)K.cells.size();
@@ -213,7 +213,7 @@ static int build_layout(cn_model *m) {
   // chunk size: the default suits plain nodes (three 5-row records); a model whose mechanism
   // records are longer gets chunks of that length (a dry pass over the classes finds out)
   int min_ch = 7;  // the longest record of any class (a chunk holds whole records)
-  if (!std::getenv("CN_TAPE_CH")) {
+  if (!m->opt("tape_ch")) {
     int need = 0;
     for (const HClass &K : m->cls) {
       if (K.tp.n_groups == 0) continue;
@@ -276,7 +276,7 @@ static int build_layout(cn_model *m) {
     int next_ch = 0;
     for (int c : {12, 10})
       if (c < m->tape_CH && c >= min_ch && next_ch == 0) next_ch = c;
-    if (m->tape_W > 8 || std::getenv("CN_TAPE_CH") || 2 * (smem + 1024) <= 233472 || next_ch == 0 ||
+    if (m->tape_W > 8 || m->opt("tape_ch") || 2 * (smem + 1024) <= 233472 || next_ch == 0 ||
         2 * (smem - (size_t)m->tape_W * m->tape_S * (m->tape_CH - 10) * 256 + 1024) > 233472)
       break;
     m->tape_CH = next_ch;
@@ -330,11 +330,11 @@ static int build_layout(cn_model *m) {
   lap("tape programs");
   // ---- warp-cooperative groups: choose G per class and schedule ------------------------------
   int force_g = 0;
-  if (const char *e = std::getenv("CN_FORCE_G")) force_g = std::atoi(e);
+  if (const char *e = m->opt("force_g")) force_g = std::atoi(e);
   int max_g = 4;
-  if (const char *e = std::getenv("CN_MAX_G")) max_g = std::max(1, std::atoi(e));
+  if (const char *e = m->opt("max_g")) max_g = std::max(1, std::atoi(e));
   int64_t smem_cap = 24 * 1024;
-  if (const char *e = std::getenv("CN_WARP_SMEM")) smem_cap = std::atoll(e);
+  if (const char *e = m->opt("warp_smem")) smem_cap = std::atoll(e);
   const int64_t hard_cap = 200 * 1024;
   int sched_total = 0, nodeoff_total = 0;
   m->warp_smem_doubles = 0;
@@ -563,7 +563,7 @@ static int build_layout(cn_model *m) {
   // CTA shape of the cooperative kernel: as many warps per block as fit ~100 KB, at most 8
   const int64_t wbytes = std::max<int64_t>((int64_t)m->warp_smem_doubles * 8, 8);
   int wpb = 4;  // (4 warps x 3 CTAs per SM: 170 registers per thread, no spills)
-  if (const char *e = std::getenv("CN_WPB")) wpb = std::max(1, std::atoi(e));
+  if (const char *e = m->opt("wpb")) wpb = std::max(1, std::atoi(e));
   while (wpb > 1 && wbytes * wpb > 110 * 1024) wpb /= 2;
   m->wpb = wpb;
   lap("groups, instance layout");

@@ -217,6 +217,7 @@ template <int MAXT>
 __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __grid_constant__ DModel M,
                                                           int64_t k, int mode, int nsteps) {
   extern __shared__ __align__(128) unsigned char sm_raw[];
+  if (k < 0) k = M.step_ctr[0] - k - 1;  // replayed graph: the device counter + offset
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int W = M.tape_W, S = M.tape_S, CH = M.tape_CH;
   const uint32_t RB = (uint32_t)(S * CH) * 256u;  // ring bytes per warp
@@ -306,7 +307,12 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
   // owner -- usually another SM -- publishes with release semantics after all its global writes.
   const bool window = mode & TM_WINDOW;
   const uint32_t n_items = (uint32_t)ngrp * (uint32_t)(window ? nsteps : 1);
-  uint32_t *item_s = tm_base_s + 1;  // two shared slots for the tickets drawn by thread 0
+  // three shared slots for the tickets drawn by thread 0: the ticket drawn at the start of
+  // iteration `it` goes to slot (it + 2) % 3 and is read after the barrier at the end of that
+  // iteration; the slot is written again three iterations (three barriers) later, so no warp can
+  // still be reading it (two slots were not enough: thread 0 overwrote slot 0 at it = 0 while a
+  // delayed warp could still be reading its first ticket from it)
+  uint32_t *item_s = tm_base_s + 1;
   auto item_ready = [&](uint32_t item) -> bool {  // one lane
     const uint32_t s = item / (uint32_t)ngrp;
     if (!window || s == 0) return true;
@@ -364,7 +370,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
       tkn = M.ttask[(size_t)tgn.cls * W + warp];
       if (PB == 2 && threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
     }
-    if (window && threadIdx.x == 0) item_s[it & 1] = atomicAdd(M.win_ticket, 1u);  // the one after
+    if (window && threadIdx.x == 0) item_s[(it + 2) % 3] = atomicAdd(M.win_ticket, 1u);  // the one after
     CN_TR(0);
     const uint32_t pb = PB == 2 ? (it & 1u) : 0u;
     mbar_wait(pbar_s + 8 * pb, (PB == 2 ? it >> 1 : it) & 1u);
@@ -654,7 +660,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     }
     CN_TR(5);
     cur = nxt;
-    nxt = window ? item_s[it & 1] : nxt + gridDim.x;
+    nxt = window ? item_s[(it + 2) % 3] : nxt + gridDim.x;
     tg = tgn;
     tc = tcn;
     tk = tkn;
@@ -677,6 +683,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
 template <bool COOP>
 __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DModel M,
                                                       int64_t k) {
+  if (k < 0) k = M.step_ctr[0] - k - 1;  // replayed graph: the device counter + offset
   const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t nth = (int64_t)gridDim.x * blockDim.x;
   const double dt = M.dt;
@@ -761,6 +768,16 @@ __global__ void gather_state_kernel(const double *__restrict__ tape,
   if (i >= n) return;
   const int64_t l = loc[i];
   out[i] = l >= 0 ? st[l] : tape[-(l + 1) + (int64_t)s * 32];
+}
+
+// the inverse (checkpoint load): loc already includes the state's row offset
+__global__ void scatter_state_kernel(double *__restrict__ tape, double *__restrict__ st,
+                                     const int64_t *__restrict__ loc, int64_t n,
+                                     const double *__restrict__ src) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t l = loc[i];
+  if (l >= 0) st[l] = src[i]; else tape[-(l + 1)] = src[i];
 }
 
 }  // namespace cn

@@ -26,6 +26,50 @@ def test_exports_every_declared_symbol():
     for name in declared:
         assert hasattr(L, name), name
     assert declared == set(cn.EXPORTS)
+    # ... and nothing else: every cn_* symbol the shared library exports is declared in the header
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", str(ROOT / "paper_1901_10975_b200" / "libcn.so")],
+                         capture_output=True, text=True, check=True).stdout
+    exported = {ln.split()[-1] for ln in out.splitlines() if ln.split() and ln.split()[-2] in "TW"}
+    exported = {x for x in exported if re.fullmatch(r"cn_[a-z_0-9]+", x)}
+    assert exported == declared, exported ^ declared
+
+
+def test_options_are_per_model_and_validated(monkeypatch):
+    """cn_model_create_opts: the only knobs; unknown keys and malformed pairs are rejected, the
+    environment is not consulted."""
+    d = W.config4(n_cell=64, n_types=2)
+    assert cn.Model(d, options={"tape": 1}).layout_info()["n_tape_group"] == 2
+    assert cn.Model(d, options="tape=0; force_g=4").layout_info()["n_tape_group"] == 0
+    assert cn.Model(d, options="tape=1,tape_w=4").layout_info()["tape_warps"] == 4
+    before = cn.Model(d).layout_info()
+    monkeypatch.setenv("CN_TAPE", "0")          # ambient state steers nothing
+    monkeypatch.setenv("CN_TAPE_W", "4")
+    info = cn.Model(d).layout_info()
+    assert info == before and info["n_tape_group"] == 2 and info["tape_warps"] == 8
+    for bad in ("bogus=1", "tape", "tape=", "tape=yes", "=1"):
+        with pytest.raises(cn.CnError) as e:
+            cn.Model(d, options=bad)
+        assert e.value.code == -1, bad
+    src = "".join(f.read_text() for f in (ROOT / "paper_1901_10975_b200" / "csrc").iterdir())
+    assert "getenv" not in src
+
+
+def test_null_arrays_with_nonzero_counts_are_rejected():
+    """A description whose counts promise arrays that are NULL returns an error, never a crash."""
+    import ctypes as C
+    d, keep, _ = cn.marshal(W.config1())
+    L = cn.lib()
+    h = C.c_void_p()
+    for field, code in (("nc_weight", -4), ("nc_src", -4), ("mech", -3), ("parent", -1)):
+        saved = getattr(d, field)
+        setattr(d, field, None)
+        assert L.cn_model_create(C.byref(d), C.byref(h)) == code, field
+        assert not h.value
+        setattr(d, field, saved)
+    d.n_stim = 3
+    d.stim_gid = None
+    assert L.cn_model_create(C.byref(d), C.byref(h)) == -4
 
 
 def test_create_and_initial_v_without_device():

@@ -15,33 +15,27 @@ DT = 0.025
 TOL = 1e-6
 
 
-@pytest.fixture(scope="module")
-def cn():
-    import torch
-    if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
-    from paper_1901_10975_b200.build import build
-    build()
-    import paper_1901_10975_b200 as cn
-    return cn
+@pytest.fixture(autouse=True)
+def _gpu(need_gpu):
+    pass
 
 
 @pytest.fixture(params=["coop", "tape", "tape-step", "tape-w1", "tape-w4"])
-def strategy(request, monkeypatch):
+def strategy(request, opts):
     """Both kernels on the same inputs: warp-cooperative groups, or every cell on the interleaved
     (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1), with 8 (default), 1 or 4 warps
     (subtree tasks) per group of 32 cells.  The interleaved kernel runs in window mode where the
     model allows it (the probes are then recorded by the kernel itself); "tape-step" forces one
     launch sequence per dt."""
     if request.param.startswith("tape"):
-        monkeypatch.setenv("CN_TAPE", "1")
-        monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+        opts["tape"] = 1
+        opts["tape_min_group"] = 1
         if request.param == "tape-step":
-            monkeypatch.setenv("CN_TAPE_WINDOW", "0")
+            opts["tape_window"] = 0
         if "-w" in request.param:
-            monkeypatch.setenv("CN_TAPE_W", request.param[-1])
+            opts["tape_w"] = int(request.param[-1])
     else:
-        monkeypatch.setenv("CN_TAPE", "0")
+        opts["tape"] = 0
     return "tape" if request.param.startswith("tape") else "coop"
 
 
@@ -92,17 +86,17 @@ def test_unique_topologies_one_cell_per_warp(cn, strategy):
     check(o, g, min_spikes=5)
 
 
-def test_identical_random_cells_grouped(cn, strategy, monkeypatch):
+def test_identical_random_cells_grouped(cn, strategy, opts):
     desc = W.random_tree_cells(11, 77, 77, stream="gpu-i", identical=True, weight=0.2, amp=2.0)
     if strategy == "coop":      # (a model this small gets one cell per warp unless told otherwise)
-        monkeypatch.setenv("CN_FORCE_G", "4")
+        opts["force_g"] = 4
     o, g = run_both(cn, desc, 40.0)
     info = g.layout_info()
     # coop: 4 + 4 + 3 (ragged tail group); tape: one ragged group of 11 lanes
     assert info["n_class"] == 1 and info["n_group"] == (3 if strategy == "coop" else 1)
     check(o, g, min_spikes=5)
     if strategy == "coop":
-        monkeypatch.delenv("CN_FORCE_G")
+        opts.pop("force_g", None)
         assert cn.Model(desc).layout_info()["n_group"] == 11
 
 
@@ -135,7 +129,7 @@ def test_config3_shape(cn, strategy):
         assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9, (t, s)
 
 
-def test_config3_full_size_first_wave(cn, monkeypatch):
+def test_config3_full_size_first_wave(cn, opts):
     """All 3,560 cells / 465,740 compartments / 1.1 M Exp2Syn for 12 ms (the first population
     wave), default strategy (every cell on the interleaved kernel): once in window mode with
     the soma voltages probed every step, once with one launch sequence per dt."""
@@ -146,7 +140,7 @@ def test_config3_full_size_first_wave(cn, monkeypatch):
     assert g.layout_info()["n_tape_group"] == g.layout_info()["n_group"] > 100
     assert g.launch_count < 100
     check(o, g, min_spikes=1000)
-    monkeypatch.setenv("CN_TAPE_WINDOW", "0")
+    opts["tape_window"] = 0
     w = cn.Model(desc)
     w.run(12.0, DT)
     assert w.launch_count >= 480
@@ -192,10 +186,10 @@ def test_config4_small_full_length(cn, strategy):
     check(o, g, min_spikes=100)
 
 
-def test_mixed_strategies_in_one_model(cn, monkeypatch):
+def test_mixed_strategies_in_one_model(cn, opts):
     """Classes of 40 cells: 32 go to one tape group, the ragged 8 to warp-cooperative groups."""
-    monkeypatch.setenv("CN_TAPE", "1")
-    monkeypatch.setenv("CN_FORCE_G", "4")
+    opts["tape"] = 1
+    opts["force_g"] = 4
     desc = W.config4(n_cell=320, n_types=8, ring_size=64)
     o, g = run_both(cn, desc, 30.0)
     info = g.layout_info()
@@ -287,9 +281,9 @@ def test_node_renumbering_invariance(cn, strategy):
 
 
 @pytest.mark.parametrize("force_g", ["1", "2", "8"])
-def test_lanes_per_cell_variants(cn, force_g, monkeypatch):
-    monkeypatch.setenv("CN_TAPE", "0")       # the warp-cooperative kernel, G cells per warp
-    monkeypatch.setenv("CN_FORCE_G", force_g)
+def test_lanes_per_cell_variants(cn, force_g, opts):
+    opts["tape"] = 0       # the warp-cooperative kernel, G cells per warp
+    opts["force_g"] = int(force_g)
     desc = W.config4(n_cell=64, n_types=2)
     o, g = run_both(cn, desc, 30.0)
     check(o, g, min_spikes=10)
@@ -331,14 +325,14 @@ def test_config4_full_size_sampled_rings(cn):
 
 
 @pytest.mark.parametrize("which", ["config1", "config4", "config3", "unique"])
-def test_window_mode_matches_oracle(cn, which, monkeypatch):
+def test_window_mode_matches_oracle(cn, which, opts):
     """Without per-step probes a model whose cells all sit on the interleaved kernel runs in
     WINDOW mode: one launch integrates up to min-delay steps, (step, group) work items are handed
     out by a ticket counter, events and point processes of the window are prepared up front.
     Final voltages, states and the whole spike list must still match the oracle."""
     from oracle import OracleModel
-    monkeypatch.setenv("CN_TAPE", "1")
-    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+    opts["tape"] = 1
+    opts["tape_min_group"] = 1
     desc, tstop = {
         "config1": (W.config1(), 60.0),
         "config4": (W.config4(n_cell=256, n_types=8), 50.0),
@@ -363,12 +357,12 @@ def test_window_mode_matches_oracle(cn, which, monkeypatch):
             assert np.max(np.abs(o.get_state(t, 0) - g.get_state(t, 0))) < 1e-9, m["type"]
 
 
-def test_window_mode_one_step_per_call(cn, monkeypatch):
+def test_window_mode_one_step_per_call(cn, opts):
     """cn_run called once per dt for 300 steps with delays of up to 200 steps: every window is one
     step long, the events of spikes recorded 200 windows ago must still be found."""
     from oracle import OracleModel
-    monkeypatch.setenv("CN_TAPE", "1")
-    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
+    opts["tape"] = 1
+    opts["tape_min_group"] = 1
     desc = W.config3(n_cell=28, syn_per_cell=40)
     assert np.round(desc["netcons"]["delay"].max() / DT) == 200
     o = OracleModel(desc)
@@ -420,12 +414,12 @@ def test_gap_junctions_between_ring_cells(cn, strategy):
     assert [list(x) for x in g2.get_spikes()] == [list(x) for x in o.get_spikes()]
 
 
-def test_gap_junctions_across_kernels(cn, monkeypatch):
+def test_gap_junctions_across_kernels(cn, opts):
     """Junctions between cells on the interleaved kernel (groups of >= 16 identical cells) and
     cells on the warp-cooperative kernel (unique topologies): the peer position addresses the
     one voltage arena both kernels write."""
-    monkeypatch.setenv("CN_TAPE", "1")
-    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "16")
+    opts["tape"] = 1
+    opts["tape_min_group"] = 16
     a = W.random_tree_cells(24, 40, 40, stream="gap-a", identical=True, weight=0.2, amp=2.0)
     b = W.random_tree_cells(9, 20, 90, stream="gap-b", weight=0.2, amp=2.0)
     desc = W.with_gap_junctions(W.concat_models([a, b]), 50, g=0.01, neighbours_only=False)

@@ -12,66 +12,52 @@ import pytest
 import cn_workloads as W
 
 
-@pytest.fixture(scope="module")
-def cn():
-    from paper_1901_10975_b200.build import build
-    build()
-    import paper_1901_10975_b200 as cn
-    return cn
-
-
-def _model(cn, desc, monkeypatch, **env):
-    monkeypatch.setenv("CN_TAPE", "1")
-    monkeypatch.setenv("CN_TAPE_MIN_GROUP", "1")
-    for k, v in env.items():
-        monkeypatch.setenv(k, str(v))
-    m = cn.Model(desc)
+def _model(cn, desc, **options):
+    m = cn.Model(desc, options=dict({"tape": 1, "tape_min_group": 1}, **options))
     info = m.layout_info()
     m.destroy()
     return info
 
 
 @pytest.mark.parametrize("warps", [1, 2, 3, 5, 8, 16])
-def test_compiles_for_every_warp_count(cn, warps, monkeypatch):
+def test_compiles_for_every_warp_count(cn, warps):
     desc = W.config4(n_cell=128, n_types=4)
-    info = _model(cn, desc, monkeypatch, CN_TAPE_W=warps, CN_TAPE_CH=10 if warps > 8 else 15)
+    info = _model(cn, desc, tape_w=warps, tape_ch=10 if warps > 8 else 15)
     assert info["n_class"] == 4 and info["n_tape_group"] == 4 and info["tape_warps"] == warps
 
 
 @pytest.mark.parametrize("s,ch", [(2, 9), (2, 15), (3, 10), (4, 9), (2, 40)])
-def test_ring_geometries(cn, s, ch, monkeypatch):
+def test_ring_geometries(cn, s, ch):
     desc = W.config4(n_cell=64, n_types=2)
-    info = _model(cn, desc, monkeypatch, CN_TAPE_S=s, CN_TAPE_CH=ch)
+    info = _model(cn, desc, tape_s=s, tape_ch=ch)
     assert info["n_tape_group"] == 2
 
 
-def test_random_trees_of_every_size(cn, monkeypatch):
+def test_random_trees_of_every_size(cn):
     # 40 unique topologies from single nodes to 300 nodes, up to 3 children per node
     desc = W.random_tree_cells(40, 1, 300, stream="prog-a", weight=0.2, amp=2.0)
-    info = _model(cn, desc, monkeypatch)
+    info = _model(cn, desc)
     assert info["n_class"] == 40 and info["n_tape_group"] == 40
 
 
-def test_mechanism_heavy_shapes(cn, monkeypatch):
+def test_mechanism_heavy_shapes(cn):
     # every node with HH (all system rows in shared memory), and config 3's four tables per node
-    info = _model(cn, W.config2(n_cell=32, ring_size=32, depth=2, ncomp_branch=10), monkeypatch)
+    info = _model(cn, W.config2(n_cell=32, ring_size=32, depth=2, ncomp_branch=10))
     assert info["n_tape_group"] == 1 and info["tape_sys_rows"] == 61      # no private rows at all
-    info = _model(cn, W.config3(n_cell=28, syn_per_cell=20), monkeypatch)
+    info = _model(cn, W.config3(n_cell=28, syn_per_cell=20))
     assert info["n_class"] == 14 and info["n_tape_group"] == 14
 
 
-def test_shapes_that_do_not_fit_fall_back(cn, monkeypatch):
+def test_shapes_that_do_not_fit_fall_back(cn):
     # config 2's 601-node cells with a mechanism on every node: 601 shared-memory rows > 227 KB
-    info = _model(cn, W.config2(n_cell=8, ring_size=4), monkeypatch)
+    info = _model(cn, W.config2(n_cell=8, ring_size=4))
     assert info["n_tape_group"] == 0 and info["n_group"] > 0
     # config 5's 30-row mechanism records and 330..580-node cells
-    info = _model(cn, W.config5(n_cell=55, syn_per_cell=8), monkeypatch)
+    info = _model(cn, W.config5(n_cell=55, syn_per_cell=8))
     assert info["n_tape_group"] == 0
 
 
-def test_auto_strategy_for_small_models(cn, monkeypatch):
-    monkeypatch.delenv("CN_TAPE", raising=False)
-    monkeypatch.delenv("CN_TAPE_MIN_GROUP", raising=False)
+def test_auto_strategy_for_small_models(cn):
     for desc, on_tape in ((W.config1(), True), (W.config3(n_cell=140, syn_per_cell=20), True),
                           (W.config2(n_cell=8, ring_size=4), False),
                           (W.random_tree_cells(13, 5, 120, stream="gpu-u"), False)):
