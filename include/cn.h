@@ -189,6 +189,11 @@ int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
  * tape bytes, shared-memory bytes per CTA of the interleaved kernel (after the first cn_run),
  * warps per CTA | persistent CTAs << 8 | shared-memory system rows << 24 }. */
 int cn_get_layout_info(const cn_model *m, int64_t *info8);
+/* How the model runs (after the first cn_run), info4 = { launch mode: 0 one launch sequence per
+ * dt, 1 window mode of the interleaved kernel, 2 on-chip window mode (one CTA keeps one cell on
+ * chip for a min-delay window), -1 not yet known; CUDA-graph replays so far; steps per window;
+ * persistent CTAs of the window kernel }. */
+int cn_get_run_info(const cn_model *m, int64_t *info4);
 /* Checkpoint / restore.  A checkpoint holds the dynamic state after the last
  * step and nothing else, in the CALLER'S order: voltages, mechanism and synapse states, cai,
  * threshold flags, and the spikes recorded so far (state-sized: 8 B per node and per state).  No

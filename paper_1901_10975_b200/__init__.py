@@ -39,7 +39,7 @@ MECH = {
 
 EXPORTS = ("cn_model_create", "cn_model_create_opts", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
            "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_steps_done",
-           "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_get_kernel_timing", "cn_get_layout_info", "cn_set_spike_capacity",
+           "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_get_kernel_timing", "cn_get_layout_info", "cn_get_run_info", "cn_set_spike_capacity",
            "cn_checkpoint_size", "cn_checkpoint_save", "cn_checkpoint_load",
            "cn_model_destroy", "cn_last_error")
 
@@ -98,6 +98,7 @@ def lib():
         L.cn_set_kernel_timing.argtypes = [vp, C.c_int32, C.c_int32]
         L.cn_get_kernel_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cn_get_layout_info.argtypes = [vp, vp]
+        L.cn_get_run_info.argtypes = [vp, vp]
         L.cn_set_spike_capacity.argtypes = [vp, C.c_int64]
         L.cn_checkpoint_size.argtypes = [vp, C.POINTER(C.c_int64)]
         L.cn_checkpoint_save.argtypes = [vp, vp, C.c_int64]
@@ -282,6 +283,12 @@ class Model:
                 "max_rounds": int(a[3]), "n_tape_group": int(a[4]), "tape_bytes": int(a[5]),
                 "tape_smem_bytes": int(a[6]), "tape_warps": int(a[7]) & 255,
                 "tape_ctas": (int(a[7]) >> 8) & 0xFFFF, "tape_sys_rows": int(a[7]) >> 24}
+
+    def run_info(self):
+        a = np.zeros(4, dtype=np.int64)
+        _check(lib().cn_get_run_info(self._h, _ptr(a)))
+        return {"mode": {-1: "unknown", 0: "per-step", 1: "window", 2: "onchip-window"}[int(a[0])],
+                "graph_replays": int(a[1]), "window_steps": int(a[2]), "window_ctas": int(a[3])}
 
     def checkpoint(self) -> np.ndarray:
         """cn_checkpoint_size + cn_checkpoint_save into a fresh uint8 array."""

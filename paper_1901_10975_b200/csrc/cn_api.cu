@@ -5,6 +5,7 @@
 #include "../../include/cn.h"
 #include "cn_device.cuh"
 #include "cn_tape.cuh"
+#include "cn_cell.cuh"
 
 #include <algorithm>
 #include <chrono>
@@ -316,6 +317,35 @@ static int run_steps(cn_model *m, int64_t K) {
     if (T.ti.point) pp_coop = std::max(pp_coop, T.pp_tape_begin);
   const int ppc_blocks = (int)std::min<int64_t>((pp_coop + 255) / 256, 148 * 16);
   CU(cudaEventRecord(m->ev0, m->stream));
+  if (m->cwindow) {
+    // cell-window mode: the events of a window of up to win_steps steps are summed per (step,
+    // synapse), then one launch keeps every cell on chip for the whole window (cn_cell.cuh)
+    for (int64_t s = 0; s < K;) {
+      const int n = (int)std::min<int64_t>(m->win_steps, K - s);
+      const int64_t k = m->k + s;
+      if (m->n_netcon > 0) {
+        deliver_window_kernel<<<deliver_blocks, 128, 0, m->stream>>>(m->hm, k, n, m->win_idx);
+        m->launches++;
+      }
+      const bool timeit = m->ktime_every > 0 && m->ktime_used < m->ktime_ev.size();
+      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
+      cell_window_kernel<<<m->cwin_grid, CN_CELL_THREADS, m->cwin_smem, m->stream>>>(m->hm, k, n,
+                                                                                    m->probe_rows);
+      if (timeit) {
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
+        m->ktime_steps.push_back(n);
+      }
+      if (!m->probe.empty()) m->probe_rows = std::min(m->probe_cap, m->probe_rows + n);
+      m->launches++;
+      m->win_idx++;
+      s += n;
+    }
+    CU(cudaEventRecord(m->ev1, m->stream));
+    CU(cudaGetLastError());
+    m->k += K;
+    m->timed = true;
+    return CN_OK;
+  }
   if (m->window) {
     // one launch of the interleaved kernel per window of up to win_steps steps; the events and
     // point processes of the whole window are prepared by two small kernels in front of it
@@ -580,6 +610,15 @@ extern "C" int cn_last_run_ms(const cn_model *m, double *ms) {
   CU(cudaEventSynchronize(m->ev1));
   CU(cudaEventElapsedTime(&f, m->ev0, m->ev1));
   *ms = f;
+  return CN_OK;
+}
+
+extern "C" int cn_get_run_info(const cn_model *m, int64_t *info) {
+  if (!m || !info) return fail(CN_ERR_ARG, "NULL argument");
+  info[0] = !m->uploaded ? -1 : m->cwindow ? 2 : m->window ? 1 : 0;
+  info[1] = m->graph_replays;
+  info[2] = (m->window || m->cwindow) ? m->win_steps : 1;
+  info[3] = m->cwindow ? m->cwin_grid : m->tape_ctas;
   return CN_OK;
 }
 

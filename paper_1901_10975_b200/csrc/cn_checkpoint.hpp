@@ -365,7 +365,7 @@ extern "C" int cn_checkpoint_load(cn_model *m, const void *buf, int64_t bytes) {
       ring[(size_t)(s % H.wr)] = std::upper_bound(pstep, pstep + h.n_sp, s) - pstep;
     CU(cudaMemcpy(H.sp_end, ring.data(), (size_t)H.wr * 8, cudaMemcpyHostToDevice));
     m->win_idx = 0;
-    if (m->window) {
+    if (m->window || m->cwindow) {
       // window delivery: one mark that stands for all the windows before the restart -- every spike
       // that can still deliver (step >= k - maxd) lies behind it
       const int64_t lo_step = std::max<int64_t>(0, h.k - H.maxd);

@@ -40,6 +40,7 @@ struct DTable {
   int64_t pp_goff;               // point tables, window mode: first column of the table in win_deliv
   const int64_t *pp_first;       // point tables: [n_group+1] instance range of each group
   const int32_t *pp_slot;        // point tables: [n] shared-memory slot (node*G + cell) in its group
+  const int32_t *pp_local;       // point tables, cell-window mode: [n] local node of the instance
   const int32_t *cls_cnt;        // distributed: [n_class] instances per cell
   const int32_t *cls_nodeoff;    // distributed: [n_class] offset into dist_nodes
   const int64_t *grp_instbase;   // distributed: [n_group] first instance of the group
@@ -117,6 +118,13 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
        RT_ELIM = 0, RT_MECH = 1 << 13, RT_WAIT = 2 << 13, RT_RUN = 3 << 13, RT_CHUNK = 4 << 13,
        RT_MASK = 7 << 13 };
 
+// cell-window mode (cn_cell.cuh): where the copies of a class's mechanism tables sit in the CTA's
+// shared memory (doubles from the start of the mechanism block), and the size of the whole block
+struct CellClass {
+  int32_t mech_off[CN_MAX_TABLES];
+  int32_t mech_doubles, pad;
+};
+
 struct DModel {
   int32_t n_group, n_class, n_table, warp_smem_doubles;
   int32_t n_tgroup, tape_prog_cap, tape_sys_cap, tape_W;
@@ -176,6 +184,7 @@ struct DModel {
   int64_t trace_row0, trace_cap;  // row of the first step of this launch
   int32_t n_probe, pad3;
   int64_t *step_ctr;            // [0] step, [1] trace row that a replayed CUDA graph starts from
+  const struct CellClass *ccls; // cell-window mode (cn_cell.cuh): shared-memory layout per class
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
 };
@@ -290,33 +299,38 @@ struct GroupView {
   int64_t ab;             // first slot of the group
   const int32_t *noff;    // class table: node -> round*32 + p*G
   int G, lgG;
+  bool direct;            // per-node arrays are indexed by slot itself (cn_cell.cuh: arrays in
+                          // shared memory, by local node)
   __device__ __forceinline__ int64_t gpos(int slot) const {
-    return ab + noff[slot >> lgG] + (slot & (G - 1));
+    return direct ? (int64_t)slot : ab + noff[slot >> lgG] + (slot & (G - 1));
   }
 };
 
 // Distributed table, lockstep over the group's cells: instance j = k*G + c sits on node
 // nodes[k] of cell c.  At most one instance per node and table, so plain read-modify-write.
-__device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int cnt,
+// par / st: the table's parameter and state arrays (T.param / T.state in HBM, or their copies in
+// shared memory); the `stride` threads lane, lane + stride, ... share the instances.
+__device__ __forceinline__ void cur_distributed(const DTable &T, double *const *par,
+                                                double *const *st, int64_t ib, int cnt,
                                                 const GroupView &gv, const int32_t *nodes,
                                                 double *D, double *R, double *I,
-                                                const double *v_g, int lane) {
+                                                const double *v_g, int lane, int stride = 32) {
   const int G = gv.G, lgG = gv.lgG;
   const int tot = cnt << lgG;
   switch (T.type) {
     case T_HH: {
       const double ena = T.glob[0], ek = T.glob[1];
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
-        const double m = T.state[0][q], h = T.state[1][q], n = T.state[2][q];
-        const double invc = T.param[4][q];
-        const double gna = T.param[0][q] * m * m * m * h;
+        const double m = st[0][q], h = st[1][q], n = st[2][q];
+        const double invc = par[4][q];
+        const double gna = par[0][q] * m * m * m * h;
         const double n2 = n * n;
-        const double gk = T.param[1][q] * n2 * n2;
-        const double gl = T.param[2][q];
+        const double gk = par[1][q] * n2 * n2;
+        const double gl = par[2][q];
         D[slot] += (gna + gk + gl) * invc;
-        R[slot] += (gna * ena + gk * ek + gl * T.param[3][q]) * invc;
+        R[slot] += (gna * ena + gk * ek + gl * par[3][q]) * invc;
       }
       break;
     }
@@ -324,11 +338,11 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
       const int p = (int)T.glob[0], qq = (int)T.glob[1];
       const double E = T.glob[2];
       const bool to_ica = T.glob[3] != 0.0;
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
-        const double g = T.param[0][q] * ipow(T.state[0][q], p) * ipow(T.state[1][q], qq);
-        const double invc = T.param[1][q];
+        const double g = par[0][q] * ipow(st[0][q], p) * ipow(st[1][q], qq);
+        const double invc = par[1][q];
         D[slot] += g * invc;
         R[slot] += g * E * invc;
         if (to_ica) I[slot] += g * (v_g[gv.gpos(slot)] - E);  // ica uses v_old (still in HBM)
@@ -337,11 +351,11 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
     }
     case T_SK: {
       const double E = T.glob[0];
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
-        const double g = T.param[0][q] * T.state[0][q];
-        const double invc = T.param[1][q];
+        const double g = par[0][q] * st[0][q];
+        const double invc = par[1][q];
         D[slot] += g * invc;
         R[slot] += g * E * invc;
       }
@@ -355,58 +369,60 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, int64_t ib, int
 // nrn_state with the new v (in R)
 // ------------------------------------------------------------------------------------------
 
-__device__ __forceinline__ void state_distributed(const DTable &T, int64_t ib, int cnt,
+__device__ __forceinline__ void state_distributed(const DTable &T, double *const *par,
+                                                  double *const *st, int64_t ib, int cnt,
                                                   const GroupView &gv, const int32_t *nodes,
                                                   const double *R, double *cai_g,
                                                   const double *I, int lane, double dt,
-                                                  double q10) {
+                                                  double q10, int stride = 32) {
+  (void)par;
   const int G = gv.G, lgG = gv.lgG;
   const int tot = cnt << lgG;
   switch (T.type) {
     case T_HH:
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
-        double sm = T.state[0][q], sh = T.state[1][q], sn = T.state[2][q];
+        double sm = st[0][q], sh = st[1][q], sn = st[2][q];
         hh_advance(R[slot], q10 * dt, sm, sh, sn);
-        T.state[0][q] = sm;
-        T.state[1][q] = sh;
-        T.state[2][q] = sn;
+        st[0][q] = sm;
+        st[1][q] = sh;
+        st[2][q] = sn;
       }
       break;
     case T_HHFORM: {
       const int p = (int)T.glob[0], qq = (int)T.glob[1];
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
         const double v = R[slot];
         double xinf, xtau;
         if (p > 0) {
           hhform_gate(v, T.glob + 4, xinf, xtau);
-          T.state[0][q] = cnexp(T.state[0][q], xinf, xtau, dt);
+          st[0][q] = cnexp(st[0][q], xinf, xtau, dt);
         }
         if (qq > 0) {
           hhform_gate(v, T.glob + 10, xinf, xtau);
-          T.state[1][q] = cnexp(T.state[1][q], xinf, xtau, dt);
+          st[1][q] = cnexp(st[1][q], xinf, xtau, dt);
         }
       }
       break;
     }
     case T_SK:
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
         double cai = cai_g[gv.gpos(slot)];
         if (cai < 1e-9) cai = 1e-9;
         const double zinf = 1.0 / (1.0 + pow(T.glob[1] / cai, T.glob[2]));
-        T.state[0][q] = cnexp(T.state[0][q], zinf, T.glob[3], dt);
+        st[0][q] = cnexp(st[0][q], zinf, T.glob[3], dt);
       }
       break;
     case T_CADYN: {
       // derivimplicit on a linear ODE: one Newton step of backward Euler is exact (L278)
       const double kappa = 1e4 * T.glob[0] / (2.0 * 96485.33212 * T.glob[1]);
       const double taud = T.glob[2], cmin = T.glob[3];
-      for (int j = lane; j < tot; j += 32) {
+      for (int j = lane; j < tot; j += stride) {
         const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
         const int64_t gp = gv.gpos(slot);
         const double y0 = cai_g[gp];
@@ -452,6 +468,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 8 ? 1 : 12 / WPB)
   gv.noff = M.node_off + ci.nodeoff_off;
   gv.G = G;
   gv.lgG = lgG;
+  gv.direct = false;
 
   // schedule-ordered streams of this lane: slot (round r, lane) = ab + r*32 + lane
   const uint32_t *__restrict__ sched = M.sched + ci.sched_off + p;
@@ -522,7 +539,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 8 ? 1 : 12 / WPB)
     if (!T.is_point) {  // (point processes: pp_coop_kernel, one thread per instance)
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
-        cur_distributed(T, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls], D,
+        cur_distributed(T, T.param, T.state, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls], D,
                         R, I, M.v, lane);
         __syncwarp();
       }
@@ -597,7 +614,7 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 8 ? 1 : 12 / WPB)
     if (!T.is_point) {
       const int cnt = T.cls_cnt[gi.cls];
       if (cnt > 0) {
-        state_distributed(T, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls],
+        state_distributed(T, T.param, T.state, T.grp_instbase[g], cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls],
                           R, M.cai, I, lane, dt, M.q10);
         __syncwarp();
       }

@@ -500,6 +500,73 @@ static int finalize(cn_model *m, double dt) {
       rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_nsp); if (rc != CN_OK) return rc;
     }
   }
+  // cell-window mode (cn_cell.cuh): every cell on the warp-cooperative layout with one
+  // cell per warp, no gap junctions, the largest cell fits the shared memory of a CTA; chosen
+  // automatically when the whole model is resident on the device at once, or forced by onchip=1
+  {
+    int onchip = -1;
+    if (const char *e = m->opt("onchip")) onchip = std::atoi(e);
+    bool ok = onchip != 0 && m->hm.n_tgroup == 0 && !m->grp.empty();
+    for (const HClass &K : m->cls)
+      if (K.count - K.tp.n_cells > 0 && K.G != 1) ok = false;
+    for (const HTable &T : m->tab)
+      if (T.type == CN_GAP && T.n > 0) ok = false;
+    const int64_t wn = m->n_netcon > 0 ? std::min<int64_t>(H.mind, 64) : 32;
+    if (wn < 2 && onchip != 1) ok = false;
+    if (ok && m->win_ninst * wn * 8 > ((int64_t)4 << 30)) ok = false;
+    std::vector<CellClass> ccls(m->cls.size());
+    size_t max_bytes = 0;
+    if (ok) {
+      for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+        const HClass &K = m->cls[kc];
+        int off = 0;
+        for (int t = 0; t < nt; ++t) {
+          const HTable &T = m->tab[t];
+          ccls[kc].mech_off[t] = off;
+          if (T.ti.point || T.type == CN_PAS) continue;
+          off += (T.ti.n_dev_param + T.ti.n_state) * T.cls_cnt[kc];
+        }
+        ccls[kc].mech_doubles = off;
+        if (K.count - K.tp.n_cells > 0)
+          max_bytes = std::max(max_bytes, ((size_t)K.n * (7 + (K.needs_ica ? 1 : 0) + (m->any_cai ? 1 : 0)) + off) * 8);
+      }
+      if (max_bytes > 220 * 1024) ok = false;
+    }
+    if (ok) {
+      int dev = 0, sms = 0;
+      CU(cudaGetDevice(&dev));
+      CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+      const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (227 * 1024) / (max_bytes + 1024)));
+      if (onchip == -1 && ng > sms * per_sm) ok = false;  // auto: only when everything is resident at once
+      m->cwin_grid = std::min(ng, sms * per_sm);
+      m->cwin_smem = max_bytes;
+    }
+    m->cwindow = ok;
+    if (ok) {
+      m->win_steps = (int)std::max<int64_t>(wn, 1);
+      H.win_stride = 0;
+      H.win_ninst = m->win_ninst;
+      if (m->n_netcon > 0) {
+        rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_ninst * m->win_steps, 1), &H.win_deliv);
+        if (rc != CN_OK) return rc;
+      }
+      H.win_mark_cap = H.maxd + 64;
+      rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_step); if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)H.win_mark_cap, &H.win_mark_nsp); if (rc != CN_OK) return rc;
+      CellClass *dcc;
+      rc = dev_upload(m, ccls, &dcc); if (rc != CN_OK) return rc;
+      H.ccls = dcc;
+      for (int t = 0; t < nt; ++t) {
+        HTable &T = m->tab[t];
+        if (!T.ti.point) continue;
+        rc = dev_upload(m, T.pp_local, &T.d_pp_local); if (rc != CN_OK) return rc;
+        H.tab[t].pp_local = T.d_pp_local;
+      }
+      if (max_bytes > 48 * 1024)
+        CU(cudaFuncSetAttribute(cell_window_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)max_bytes));
+    }
+  }
   rc = dev_alloc(m, 2, &H.step_ctr); if (rc != CN_OK) return rc;
   if (const char *e = m->opt("graph")) m->graph_on = std::atoi(e) != 0;
   // spikes
@@ -519,6 +586,34 @@ static int finalize(cn_model *m, double dt) {
     UP(pp, m->d_probe_pos);
     rc = dev_alloc(m, (size_t)(m->probe_cap * (int64_t)m->probe.size()), &m->d_trace, false);
     if (rc) return rc;
+    if (m->cwindow) {  // the probes of every cell: the cell-window kernel records them per step
+      std::vector<int32_t> first((size_t)ng + 1, 0), col(m->probe.size());
+      std::vector<int64_t> pos(m->probe.size());
+      std::vector<int32_t> grp_of(m->probe.size());
+      for (size_t j = 0; j < m->probe.size(); ++j) {
+        const int64_t nd = m->probe[j];
+        const int32_t c = (int32_t)(std::upper_bound(m->cell_first.begin(), m->cell_first.end(), nd) -
+                                    m->cell_first.begin()) - 1;
+        grp_of[j] = m->cell_grp[c];
+        first[grp_of[j] + 1]++;
+      }
+      for (int g = 0; g < ng; ++g) first[g + 1] += first[g];
+      std::vector<int32_t> fill(first.begin(), first.end() - 1);
+      for (size_t j = 0; j < m->probe.size(); ++j) {
+        const int32_t q = fill[grp_of[j]]++;
+        const int32_t c = (int32_t)(std::upper_bound(m->cell_first.begin(), m->cell_first.end(),
+                                                     (int64_t)m->probe[j]) - m->cell_first.begin()) - 1;
+        pos[q] = m->probe[j] - m->cell_first[c];  // local node
+        col[q] = (int32_t)j;
+      }
+      int32_t *df, *dc;
+      int64_t *dp;
+      UP(first, df); UP(pos, dp); UP(col, dc);
+      H.wp_first = df; H.wp_pos = dp; H.wp_col = dc;
+      H.trace = m->d_trace;
+      H.trace_cap = m->probe_cap;
+      H.n_probe = (int32_t)m->probe.size();
+    }
     if (m->window) {  // the probes of every group: the interleaved kernel records them per step
       const int ntg = (int)m->tgrp.size();
       std::vector<int32_t> first((size_t)ntg + 1, 0), col(m->probe.size());

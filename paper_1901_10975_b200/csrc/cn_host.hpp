@@ -197,6 +197,8 @@ struct HTable {
   std::vector<int64_t> pp_first;
   uvec<int32_t> pp_slot;
   uvec<uint32_t> pp_wslot;  // window mode: element in one step's block of win_rows
+  uvec<int32_t> pp_local;   // local node of the instance in its cell (cell-window mode)
+  int32_t *d_pp_local = nullptr;
   uint32_t *d_pp_wslot = nullptr;
   std::vector<int32_t> cls_cnt, cls_nodeoff;
   std::vector<int64_t> grp_instbase;
@@ -326,6 +328,9 @@ struct cn_model {
   bool tape_leaf_first = false;     // scheduling variant: all whole subtrees before any upper node
   bool tape_tmem = true;            // plain chain nodes keep their system rows in tensor memory
   int tape_ctas = 0;                // persistent CTAs of the interleaved kernel (0: not yet known)
+  bool cwindow = false;             // cell-window mode (cn_cell.cuh): one CTA keeps one cell on chip
+  int cwin_grid = 0;                //   for a window of up to win_steps steps
+  size_t cwin_smem = 0;
   bool window = false;              // window mode: one launch of the interleaved kernel per
   int win_steps = 0;                //   up to win_steps steps (cn_tape.cuh)
   int64_t win_idx = 0;

@@ -481,6 +481,7 @@ static int build_layout(cn_model *m) {
                  rank);
       T.pp_slot.resize((size_t)T.n);
       T.pp_wslot.resize((size_t)T.n);
+      T.pp_local.resize((size_t)T.n);
       par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
         for (int64_t i = i0; i < i1; ++i) {
           const int32_t cell = cell_of[T.node[i]];
@@ -488,6 +489,7 @@ static int build_layout(cn_model *m) {
           const int64_t pos = rank[i];
           T.inst_pos[i] = pos;
           const int32_t local = (int32_t)(T.node[i] - m->cell_first[cell]);
+          T.pp_local[pos] = local;
           if (g < ngc) {
             // element of the node's row pair in ppdr (schedule order, rows of 32 + 32)
             const int64_t sp = m->grp[g].ab_base + m->cls[m->grp[g].cls].node_off[local] +

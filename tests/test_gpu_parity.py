@@ -20,7 +20,7 @@ def _gpu(need_gpu):
     pass
 
 
-@pytest.fixture(params=["coop", "tape", "tape-step", "tape-w1", "tape-w4"])
+@pytest.fixture(params=["coop", "cell", "tape", "tape-step", "tape-w1", "tape-w4"])
 def strategy(request, opts):
     """Both kernels on the same inputs: warp-cooperative groups, or every cell on the interleaved
     (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1), with 8 (default), 1 or 4 warps
@@ -35,7 +35,10 @@ def strategy(request, opts):
         if "-w" in request.param:
             opts["tape_w"] = int(request.param[-1])
     else:
+        # the warp-cooperative layout: one launch sequence per dt (replayed from a CUDA graph), or
+        # "cell": the on-chip window kernel, one CTA per cell for a whole min-delay window
         opts["tape"] = 0
+        opts["onchip"] = 1 if request.param == "cell" else 0
     return "tape" if request.param.startswith("tape") else "coop"
 
 
@@ -167,15 +170,107 @@ def test_config2_one_ring_of_64(cn, strategy):
 
 
 def test_config2_full_size(cn):
-    """All four rings of config 2 (256 cells x 601 compartments, HH on every compartment) for
-    30 ms; default strategy for this size (warp-cooperative kernel: a cell with a mechanism on
-    every node keeps its whole system in shared memory)."""
+    """All four rings of config 2 (256 cells x 601 compartments, HH on every compartment) for its
+    full 200 ms, soma voltages compared at every step; default strategy for this size: the
+    warp-cooperative layout run by the on-chip window kernel (the 19 MB model is resident in the
+    shared memory of the device; one launch per 40-step window)."""
     desc = W.config2()
     assert len(desc["parent"]) == 153856
-    o, g = run_both(cn, desc, 30.0)
-    check(o, g, min_spikes=40)
+    o, g = run_both(cn, desc, 200.0)
+    info = g.run_info()
+    assert info["mode"] == "onchip-window" and info["window_steps"] == 40
+    assert g.launch_count <= 2 * 200 + 8
+    check(o, g, min_spikes=400)
     for s in (0, 1, 2):
         assert np.max(np.abs(o.get_state(0, s) - g.get_state(0, s))) < 1e-9
+
+
+def test_config2_full_size_per_step_graph(cn, opts):
+    """The same model with one launch sequence per dt (onchip=0), replayed from a CUDA graph."""
+    opts["onchip"] = 0
+    desc = W.config2()
+    o, g = run_both(cn, desc, 30.0)
+    info = g.run_info()
+    assert info["mode"] == "per-step" and info["graph_replays"] >= 1200 // 20 - 2
+    check(o, g, min_spikes=40)
+
+
+@pytest.mark.parametrize("which", ["config1", "config2", "config3", "config5", "unique"])
+def test_onchip_window_matches_oracle(cn, which, opts):
+    """On-chip window mode: one CTA keeps one cell in shared memory for a window of
+    up to min-delay steps.  Windows of different lengths (cn_run in uneven pieces), probes inside
+    the windows, every mechanism type, AMPA+NMDA synapses (their current depends on v: evaluated in
+    the kernel from the cell's own voltage), delays from 4 steps."""
+    from oracle import OracleModel
+    opts.update({"tape": 0, "onchip": 1})
+    desc, tstop = {
+        "config1": (W.config1(), 60.0),
+        "config2": (W.config2(n_cell=8, ring_size=4, weight=0.05), 30.0),
+        "config3": (W.config3(n_cell=140, syn_per_cell=60), 40.0),
+        "config5": (W.config5(n_cell=110, syn_per_cell=40), 20.0),
+        "unique": (W.random_tree_cells(13, 5, 120, stream="gpu-u", weight=0.2, amp=2.0), 40.0),
+    }[which]
+    nsteps = int(round(tstop / DT))
+    cf = desc["cell_first"]
+    probes = np.concatenate([cf[:-1], [cf[1] - 1, cf[2] - 3]]).astype(np.int32)
+    o = OracleModel(desc)
+    o.set_probes(probes)
+    o.run(tstop, DT)
+    g = cn.Model(desc)
+    g.set_probes(probes, nsteps)
+    for t in (0.3 * tstop, 0.3 * tstop + DT, 0.3 * tstop + 8 * DT, tstop):
+        g.run(t, DT)
+    info = g.run_info()
+    assert info["mode"] == "onchip-window"
+    assert info["window_steps"] == (4 if which == "config5" else 40)
+    assert g.steps_done == nsteps and g.launch_count <= 2 * (nsteps // info["window_steps"] + 4) + 4
+    check(o, g, min_spikes=5)
+    for t, m in enumerate(desc["mechs"]):
+        for st in range({"hh": 3, "hhform": 2, "sk": 1, "expsyn": 1, "exp2syn": 2, "ampanmda": 4}.get(m["type"], 0)):
+            assert np.max(np.abs(o.get_state(t, st) - g.get_state(t, st))) < 1e-9, (m["type"], st)
+
+
+def test_onchip_window_one_step_per_call_and_checkpoint(cn, opts):
+    """cn_run once per dt (every window one step long) with delays of up to 200 steps, a checkpoint
+    in the middle that is continued by the per-step kernel."""
+    from oracle import OracleModel
+    opts.update({"tape": 0, "onchip": 1})
+    desc = W.config3(n_cell=28, syn_per_cell=40)
+    o = OracleModel(desc)
+    g = cn.Model(desc)
+    for k in range(1, 501):
+        g.run(k * DT, DT)
+    assert g.run_info()["mode"] == "onchip-window"
+    h = cn.Model(desc, options={"onchip": 0})
+    h.restore(g.checkpoint())
+    h.run(700 * DT, DT)
+    g.run(700 * DT, DT)
+    o.run(700 * DT, DT)
+    for x in (g, h):
+        assert np.max(np.abs(o.get_v() - x.get_v())) <= TOL
+        assert [list(a) for a in x.get_spikes()] == [list(a) for a in o.get_spikes()]
+    assert len(o.get_spikes()[0]) >= 20
+
+
+def test_graph_replay_equals_direct_launches(cn, opts):
+    """Per-dt launch sequences replayed from a CUDA graph (20 steps per graph, a device-side step
+    counter) against the same launches issued one by one: bit-identical, on both kernels, with
+    probes, in uneven pieces."""
+    for base in ({"tape": 0, "onchip": 0}, {"tape": 1, "tape_window": 0, "tape_min_group": 1}):
+        desc = W.config4(n_cell=128, n_types=4)
+        probes = np.asarray(desc["cell_first"][:8], np.int32)
+        res = []
+        for graph in (1, 0):
+            m = cn.Model(desc, options=dict(base, graph=graph))
+            m.set_probes(probes, 700)
+            for k in (7, 48, 49, 300, 641, 800):
+                m.run(k * DT, DT)
+            assert (m.run_info()["graph_replays"] > 25) == (graph == 1)
+            res.append((m.get_v(), m.get_spikes(), m.get_trace()))
+        assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][2], res[1][2])
+        assert res[0][2].shape == (700, 8)
+        assert [list(x) for x in res[0][1]] == [list(x) for x in res[1][1]]
+        assert len(res[0][1][0]) > 20
 
 
 def test_config4_small_full_length(cn, strategy):
