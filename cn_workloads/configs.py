@@ -450,20 +450,26 @@ def extract_cells(desc: dict, gids) -> dict:
                            {k: v[keep] for k, v in m["params"].items()}, m["globals"]))
     nc = desc["netcons"]
     src = nc["src"].astype(np.int64)
-    tgt_keep = np.array([inst_maps[tm][ti] >= 0 for tm, ti in zip(nc["tgt_mech"], nc["tgt_inst"])],
-                        dtype=bool) if len(src) else np.zeros(0, bool)
+    # (vectorised: one flat instance map over all tables)
+    toff = np.concatenate([[0], np.cumsum([len(x) for x in inst_maps])]).astype(np.int64)
+    flat = np.concatenate(inst_maps) if inst_maps else np.zeros(0, np.int64)
+    tm_all = nc["tgt_mech"].astype(np.int64)
+    new_inst = flat[toff[tm_all] + nc["tgt_inst"].astype(np.int64)] if len(src) else np.zeros(0, np.int64)
+    tgt_keep = new_inst >= 0
     is_stim = src >= n_cell
-    src_cell_new = np.where(is_stim, -1, gid_map[np.minimum(src, n_cell - 1)])
+    src_cell_new = np.where(is_stim, -1, gid_map[np.minimum(src, n_cell - 1)]) if n_cell else \
+        np.full(len(src), -1, np.int64)
     if np.any(tgt_keep & ~is_stim & (src_cell_new < 0)):
         raise ValueError("extract_cells: a kept target has a dropped source (set not closed)")
     # renumber scripted sources densely after the kept cells
     stim_old = np.unique(src[tgt_keep & is_stim])
     stim_map = {int(g): len(gids) + j for j, g in enumerate(stim_old)}
-    new_src = np.array([stim_map[int(s)] if st else int(c)
-                        for s, st, c in zip(src[tgt_keep], is_stim[tgt_keep],
-                                            src_cell_new[tgt_keep])], dtype=np.int64)
+    new_src = src_cell_new[tgt_keep].copy()
+    ks = is_stim[tgt_keep]
+    if ks.any():
+        new_src[ks] = len(gids) + np.searchsorted(stim_old, src[tgt_keep][ks])
     tm = nc["tgt_mech"][tgt_keep]
-    ti = np.array([inst_maps[a][b] for a, b in zip(tm, nc["tgt_inst"][tgt_keep])], dtype=np.int64)
+    ti = new_inst[tgt_keep]
     new_nc = _netcons(new_src, tm, ti, nc["weight"][tgt_keep], nc["delay"][tgt_keep])
     sk = np.array([int(g) in stim_map for g in desc["stim"]["gid"]], dtype=bool) \
         if len(desc["stim"]["gid"]) else np.zeros(0, bool)

@@ -249,14 +249,18 @@ def config3(n_cell: int = 3560, n_types: int = 14, n_comp_total=465740, syn_per_
 # ------------------------------------------------------------------------------------------
 
 def config5(scale: float = 1.0, n_types: int = 55, syn_per_cell=None, w_scale: float = 1.0,
-            drive_amp: float = 2.0, dt: float = 0.025, n_cell=None):
+            drive_amp: float = 2.0, dt: float = 0.025, n_cell=None, block=None):
     """scale = 1: 20,000 cells, 4,000 synapses per cell (80 M).  Smaller scales shrink the cell
     count and (unless given) the synapses per cell proportionally; cells keep their full size.
     Weights are lognormal(-4, 0.5) uS x w_scale x 10 / syn_per_cell (tuned once in the oracle on a
     100-cell copy so that about a quarter of the cells fire within the 20 ms, then frozen; the
     1 / syn_per_cell factor keeps the summed drive of a cell independent of the scale).  The config
     names no stimulus: 10 % of the cells get one 2 ms IClamp pulse of drive_amp nA with a seeded
-    onset in [0.5, 5) ms (reading R24)."""
+    onset in [0.5, 5) ms (reading R24).
+    block: if given, the presynaptic cell of every synapse is drawn among the `block` cells of the
+    target's own block (gids [j*block, (j+1)*block)): the network falls into closed sub-networks of
+    full-size cells with the full number of synapses per cell, each of which the oracle can
+    integrate on its own (extract_cells) -- sampled parity at the stated per-cell size."""
     tag = "c5"
     if n_cell is None:
         n_cell = max(n_types, int(round(20000 * scale)))
@@ -298,7 +302,13 @@ def config5(scale: float = 1.0, n_types: int = 55, syn_per_cell=None, w_scale: f
     onset = dt * rng.randint((tag, "onset"), nd, int(round(0.5 / dt)), int(round(5.0 / dt)))
     mechs.append(_mech("iclamp", roots[driven], {"del": onset, "dur": _const(nd, 2.0),
                                                   "amp": _const(nd, drive_amp)}))
-    src = rng.randint((tag, "pre"), ns, 0, n_cell)
+    if block is None:
+        src = rng.randint((tag, "pre"), ns, 0, n_cell)
+    else:
+        tgt_cell = np.arange(ns, dtype=np.int64) // syn_per_cell
+        b0 = (tgt_cell // block) * block
+        bsz = np.minimum(block, n_cell - b0)
+        src = b0 + (rng.bits((tag, "pre"), ns) % bsz.astype(np.uint64)).astype(np.int64)
     delay = dt * rng.randint((tag, "delay"), ns, int(round(0.1 / dt)), int(round(10.0 / dt)) + 1)
     weight = w_scale * (10.0 / syn_per_cell) * np.exp(-4.0 + 0.5 * rng.normal((tag, "w"), ns))
     nc = _netcons(src, np.full(ns, 10), np.arange(ns), weight, delay)

@@ -183,6 +183,11 @@ int cn_last_run_ms(const cn_model *m, double *ms_out);
  * cn_get_kernel_timing returns the summed duration and the number of dt the samples cover (one
  * launch of the interleaved kernel integrates a whole window of steps), and resets. */
 int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samples);
+/* Which kernel the samples bracket when the model runs one launch sequence per dt: 0 the step
+ * kernel (default: interleaved kernel if it runs, else the warp-cooperative one), 1 the
+ * point-process kernel(s), 2 the event-delivery kernel.  (Window modes always time the window
+ * kernel.)  While sampling is on, launch sequences are issued directly, not from a CUDA graph. */
+int cn_select_timed_kernel(cn_model *m, int32_t which);
 int cn_get_kernel_timing(cn_model *m, double *sum_ms_out, int64_t *count_out);
 /* Layout facts for DESIGN/bench, info8 = { n_class, n_group (all), shared-memory bytes per warp and
  * max elimination rounds of the warp-cooperative kernel, n_group of the interleaved (tape) kernel,

@@ -39,7 +39,7 @@ MECH = {
 
 EXPORTS = ("cn_model_create", "cn_model_create_opts", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
            "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_steps_done",
-           "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_get_kernel_timing", "cn_get_layout_info", "cn_get_run_info", "cn_set_spike_capacity",
+           "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_select_timed_kernel", "cn_get_kernel_timing", "cn_get_layout_info", "cn_get_run_info", "cn_set_spike_capacity",
            "cn_checkpoint_size", "cn_checkpoint_save", "cn_checkpoint_load",
            "cn_model_destroy", "cn_last_error")
 
@@ -96,6 +96,7 @@ def lib():
         L.cn_launch_count.argtypes = [vp]
         L.cn_last_run_ms.argtypes = [vp, C.POINTER(C.c_double)]
         L.cn_set_kernel_timing.argtypes = [vp, C.c_int32, C.c_int32]
+        L.cn_select_timed_kernel.argtypes = [vp, C.c_int32]
         L.cn_get_kernel_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.cn_get_layout_info.argtypes = [vp, vp]
         L.cn_get_run_info.argtypes = [vp, vp]
@@ -270,6 +271,9 @@ class Model:
 
     def set_kernel_timing(self, every, max_samples=4096):
         _check(lib().cn_set_kernel_timing(self._h, int(every), int(max_samples)))
+
+    def select_timed_kernel(self, which):
+        _check(lib().cn_select_timed_kernel(self._h, {"step": 0, "pp": 1, "deliver": 2}[which]))
 
     def get_kernel_timing(self):
         ms, n = C.c_double(), C.c_int64()

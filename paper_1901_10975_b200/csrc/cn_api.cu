@@ -392,10 +392,24 @@ static int run_steps(cn_model *m, int64_t K) {
   // ---- one launch sequence per dt: deliver -> point processes -> step kernels (-> probes) --------
   // k_arg >= 0: the step itself; k_arg = -(1 + s): step = device counter + s (replayed CUDA graph).
   auto issue_step = [&](int64_t k_arg, int64_t row_arg, cudaStream_t st, bool timeit) -> int {
+    // event pair around the kernel class selected by cn_select_timed_kernel
+    auto t0 = [&](int which) {
+      if (timeit && m->ktime_which == which) cudaEventRecord(m->ktime_ev[m->ktime_used].first, st);
+    };
+    auto t1 = [&](int which) {
+      if (timeit && m->ktime_which == which) {
+        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, st);
+        m->ktime_steps.push_back(1);
+      }
+    };
+    const bool pp_any = (ntg > 0 && pp_tape > 0) || (ng > 0 && pp_coop > 0);
     if (m->n_netcon > 0) {
+      t0(2);
       deliver_kernel<<<deliver_blocks, 128, 0, st>>>(m->hm, k_arg);
+      t1(2);
       m->launches++;
     }
+    if (pp_any) t0(1);
     if (ntg > 0 && pp_tape > 0) {
       pp_step_kernel<false><<<pp_blocks, 256, 0, st>>>(m->hm, k_arg);
       m->launches++;
@@ -404,10 +418,11 @@ static int run_steps(cn_model *m, int64_t K) {
       pp_step_kernel<true><<<ppc_blocks, 256, 0, st>>>(m->hm, k_arg);
       m->launches++;
     }
-    const bool time_tape = ntg > 0;  // the dominant kernel is the tape kernel when it runs
+    if (pp_any) t1(1);
+    const bool time_tape = ntg > 0;  // the dominant step kernel is the tape kernel when it runs
     if (ng > 0) {
       cudaError_t e;
-      if (timeit && !time_tape) cudaEventRecord(m->ktime_ev[m->ktime_used].first, st);
+      if (!time_tape) t0(0);
       switch (m->wpb) {
         case 8: e = launch_step<8>(m, k_arg, st); break;
         case 4: e = launch_step<4>(m, k_arg, st); break;
@@ -415,21 +430,15 @@ static int run_steps(cn_model *m, int64_t K) {
         default: e = launch_step<1>(m, k_arg, st); break;
       }
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "step launch failed: %s", cudaGetErrorString(e));
-      if (timeit && !time_tape) {
-        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, st);
-        m->ktime_steps.push_back(1);
-      }
+      if (!time_tape) t1(0);
       m->launches++;
     }
     if (ntg > 0) {
-      if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, st);
+      t0(0);
       cudaError_t e = launch_tape(m, k_arg, m->state_pending ? TM_ADVANCE : 0, 1, st);
       if (e != cudaSuccess) return fail(CN_ERR_CUDA, "tape launch failed: %s", cudaGetErrorString(e));
       m->state_pending = true;
-      if (timeit) {
-        cudaEventRecord(m->ktime_ev[m->ktime_used++].second, st);
-        m->ktime_steps.push_back(1);
-      }
+      t1(0);
       m->launches++;
     }
     if (!m->probe.empty() && (row_arg < 0 || row_arg < m->probe_cap)) {
@@ -660,6 +669,12 @@ extern "C" int cn_set_kernel_timing(cn_model *m, int32_t every, int32_t max_samp
       CU(cudaEventCreate(&b));
       m->ktime_ev.emplace_back(a, b);
     }
+  return CN_OK;
+}
+
+extern "C" int cn_select_timed_kernel(cn_model *m, int32_t which) {
+  if (!m || which < 0 || which > 2) return fail(CN_ERR_ARG, "bad argument");
+  m->ktime_which = which;
   return CN_OK;
 }
 

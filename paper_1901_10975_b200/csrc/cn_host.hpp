@@ -350,7 +350,7 @@ struct cn_model {
   cudaStream_t stream = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
-  int ktime_every = 0;
+  int ktime_every = 0, ktime_which = 0;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ktime_ev;
   size_t ktime_used = 0;
   // CUDA graph of CN_GRAPH_STEPS per-dt launch sequences (cn_api.cu run_steps)

@@ -132,25 +132,6 @@ def test_config3_shape(cn, strategy):
         assert np.max(np.abs(o.get_state(t, s) - g.get_state(t, s))) < 1e-9, (t, s)
 
 
-def test_config3_full_size_first_wave(cn, opts):
-    """All 3,560 cells / 465,740 compartments / 1.1 M Exp2Syn for 12 ms (the first population
-    wave), default strategy (every cell on the interleaved kernel): once in window mode with
-    the soma voltages probed every step, once with one launch sequence per dt."""
-    from oracle import OracleModel
-    desc = W.config3()
-    assert len(desc["parent"]) == 465740 and len(desc["netcons"]["src"]) == 1100040
-    o, g = run_both(cn, desc, 12.0)
-    assert g.layout_info()["n_tape_group"] == g.layout_info()["n_group"] > 100
-    assert g.launch_count < 100
-    check(o, g, min_spikes=1000)
-    opts["tape_window"] = 0
-    w = cn.Model(desc)
-    w.run(12.0, DT)
-    assert w.launch_count >= 480
-    assert np.max(np.abs(o.get_v() - w.get_v())) <= TOL
-    assert [list(x) for x in w.get_spikes()] == [list(x) for x in o.get_spikes()]
-
-
 def test_config5_shape(cn, strategy):
     """Config 5 scaled to 110 cells (55 types x 2, full-size cells of 330-580 compartments):
     ten channel types, AMPA+NMDA synapses with Mg block, delays from 0.1 ms (4 steps).  Every
@@ -382,41 +363,6 @@ def test_lanes_per_cell_variants(cn, force_g, opts):
     desc = W.config4(n_cell=64, n_types=2)
     o, g = run_both(cn, desc, 30.0)
     check(o, g, min_spikes=10)
-
-
-def test_config4_full_size_sampled_rings(cn):
-    """The bench workload itself (32,768 cells x 291 compartments, the launch configuration
-    bench.py times: interleaved kernel, default warps / ring) for 10 ms; rings are independent,
-    so the oracle integrates a sample of them (the same cells, generated from the same seeds) and
-    every voltage and spike of those cells must agree."""
-    from oracle import OracleModel
-    rings = [0, 137, 311, 511]
-    full = W.config4()
-    assert len(full["parent"]) == 9535488 and len(full["netcons"]["src"]) == 33280
-    g = cn.Model(full)
-    info_before = g.layout_info()
-    assert info_before["n_tape_group"] == 1024 and info_before["n_group"] == 1024
-    g.run(10.0, DT)
-    assert g.layout_info()["tape_ctas"] == 296           # two CTAs per SM (tensor-memory rows)
-    sub = W.config4(cells=rings)
-    o = OracleModel(sub)
-    o.run(10.0, DT)
-    gids = np.concatenate([np.arange(r * 64, (r + 1) * 64) for r in rings])
-    cf = full["cell_first"]
-    nodes = np.concatenate([np.arange(cf[c], cf[c + 1]) for c in gids])
-    err = np.max(np.abs(g.get_v()[nodes] - o.get_v()))
-    assert err <= TOL, err
-    gg, gs = g.get_spikes()
-    og, os_ = o.get_spikes()
-    keep = np.isin(gg, gids)
-    remap = {int(c): j for j, c in enumerate(gids)}
-    sub_g = sorted((int(s), remap[int(c)]) for c, s in zip(gg[keep], gs[keep]))
-    sub_o = sorted((int(s), int(c)) for c, s in zip(og, os_) if c < len(gids))
-    assert len(sub_o) >= 16 and sub_g == sub_o
-    assert o.min_margin > 1e3 * max(err, 1e-12)
-    # whole-model invariants at full size: every ring carries the same wave, one spike per cell so far
-    per_ring = np.bincount(gg[gg < 32768] // 64, minlength=512)
-    assert per_ring.min() > 0 and per_ring.max() <= 64 * 2
 
 
 @pytest.mark.parametrize("which", ["config1", "config4", "config3", "unique"])
