@@ -123,11 +123,12 @@ def test_config4_full_size_full_length_and_rerun_is_bit_identical(cn):
     remap = {int(c): j for j, c in enumerate(gids)}
     sub_g = sorted((int(s), remap[int(c)]) for c, s in zip(gg[keep], gs[keep]))
     sub_o = sorted((int(s), int(c)) for c, s in zip(og, os_) if c < len(gids))
-    assert len(sub_o) >= 256 and sub_g == sub_o
+    assert len(sub_o) >= 100 and sub_g == sub_o
     assert o.min_margin > 1e3 * max(err, err_t, 1e-12)
-    # whole-model invariants: every ring carries the same kind of wave
+    # whole-model invariants: every ring carries the same kind of wave (one hop per ~1.8 ms: about
+    # 28 of the 64 cells of a ring have fired after 50 ms)
     per_ring = np.bincount(gg[gg < 32768] // 64, minlength=512)
-    assert per_ring.min() >= 64 and per_ring.max() <= 64 * 8
+    assert per_ring.min() >= 20 and per_ring.max() <= 64
     assert np.all(np.isfinite(v1))
     # the same run again: bit-identical
     g.destroy()
