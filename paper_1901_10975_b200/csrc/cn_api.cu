@@ -329,8 +329,11 @@ static int run_steps(cn_model *m, int64_t K) {
       }
       const bool timeit = m->ktime_every > 0 && m->ktime_used < m->ktime_ev.size();
       if (timeit) cudaEventRecord(m->ktime_ev[m->ktime_used].first, m->stream);
-      cell_window_kernel<<<m->cwin_grid, CN_CELL_THREADS, m->cwin_smem, m->stream>>>(m->hm, k, n,
-                                                                                    m->probe_rows);
+      switch (m->cwin_threads) {
+        case 64: cell_window_kernel<64><<<m->cwin_grid, 64, m->cwin_smem, m->stream>>>(m->hm, k, n, m->probe_rows); break;
+        case 128: cell_window_kernel<128><<<m->cwin_grid, 128, m->cwin_smem, m->stream>>>(m->hm, k, n, m->probe_rows); break;
+        default: cell_window_kernel<256><<<m->cwin_grid, 256, m->cwin_smem, m->stream>>>(m->hm, k, n, m->probe_rows); break;
+      }
       if (timeit) {
         cudaEventRecord(m->ktime_ev[m->ktime_used++].second, m->stream);
         m->ktime_steps.push_back(n);

@@ -22,13 +22,12 @@
 
 namespace cn {
 
-#define CN_CELL_THREADS 256
-
-__global__ void __launch_bounds__(CN_CELL_THREADS)
+// NT threads per CTA: 64 for small cells (more CTAs per SM), up to 256 for large ones
+template <int NT>
+__global__ void __launch_bounds__(NT)
     cell_window_kernel(const __grid_constant__ DModel M, int64_t k0, int nsteps, int64_t trace_row0) {
   extern __shared__ double csm[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int NT = CN_CELL_THREADS;
   const double dt = M.dt;
   for (int g = blockIdx.x; g < M.n_group; g += gridDim.x) {
     const GroupInfo gi = M.grp[g];
@@ -188,20 +187,39 @@ __global__ void __launch_bounds__(CN_CELL_THREADS)
                         tid, NT);
         __syncthreads();
       }
-      // ---- Hines solve: warp 0, rounds of independent nodes (L66) ---------------------------------
+      // ---- Hines solve: warp 0, rounds of independent nodes (L66).  Along a chain the parent sits
+      // on its child's lane in the next round (SF_OUT / SF_IN, cn_host.hpp hu_schedule): the
+      // contribution travels in a register, and so does the parent's v on the way back; only
+      // contributions that meet at a branch point go through the parent's row. --------------------
       if (warp == 0) {
+        const uint8_t *__restrict__ sfl = M.sched_fl + ci.sched_off + lane;
         uint32_t en = rounds > 0 ? __ldg(sched) : CN_IDLE;
+        uint32_t fn = rounds > 0 ? __ldg(sfl) : 0u;
+        double accD = 0.0, accR = 0.0;
         for (int r = 0; r < rounds; ++r) {
-          const uint32_t e = en;
-          if (r + 1 < rounds) en = __ldg(sched + (size_t)(r + 1) * 32);
+          const uint32_t e = en, fl = fn;
+          if (r + 1 < rounds) {
+            en = __ldg(sched + (size_t)(r + 1) * 32);
+            fn = __ldg(sfl + (size_t)(r + 1) * 32);
+          }
           if ((e & 0xFFFFu) != CN_IDLE) {
             const int si = (int)(e & 0xFFFFu), sp = (int)(e >> 16);
-            const double di = D[si] + DS[si], ri = R[si] + (V[si] + RS[si]);
-            const double rinv = rcp_fast(di);
+            double di = D[si] + DS[si], ri = R[si] + (V[si] + RS[si]);
+            if (fl & 2u) {  // SF_IN
+              di += accD;
+              ri += accR;
+            }
+            const double rinv = rcp_chain(di);
             const double a = A[si], b = B[si];
             const double f = a * rinv;
-            D[sp] -= f * b;
-            R[sp] -= f * ri;
+            const double cD = -(f * b), cR = -(f * ri);
+            if (fl & 1u) {  // SF_OUT
+              accD = cD;
+              accR = cR;
+            } else {
+              D[sp] += cD;
+              R[sp] += cR;
+            }
             D[si] = b * rinv;  // back-substitution multiplier
             R[si] = ri * rinv;
           }
@@ -209,11 +227,20 @@ __global__ void __launch_bounds__(CN_CELL_THREADS)
         }
         if (lane == 0) R[0] = (R[0] + (V[0] + RS[0])) * rcp_fast(D[0] + DS[0]);
         __syncwarp();
+        double vreg = 0.0;
+        en = rounds > 0 ? __ldg(sched + (size_t)(rounds - 1) * 32) : CN_IDLE;
+        fn = rounds > 0 ? __ldg(sfl + (size_t)(rounds - 1) * 32) : 0u;
         for (int r = rounds - 1; r >= 0; --r) {
-          const uint32_t e = __ldg(sched + (size_t)r * 32);
+          const uint32_t e = en, fl = fn;
+          if (r > 0) {
+            en = __ldg(sched + (size_t)(r - 1) * 32);
+            fn = __ldg(sfl + (size_t)(r - 1) * 32);
+          }
           if ((e & 0xFFFFu) != CN_IDLE) {
             const int si = (int)(e & 0xFFFFu), sp = (int)(e >> 16);
-            R[si] = R[si] - D[si] * R[sp];
+            const double vp = (fl & 1u) ? vreg : R[sp];  // (SF_OUT: this lane solved the parent last)
+            vreg = fma(-D[si], vp, R[si]);
+            R[si] = vreg;
           }
           __syncwarp();
         }

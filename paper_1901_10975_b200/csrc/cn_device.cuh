@@ -138,6 +138,7 @@ struct DModel {
   const GroupInfo *grp;
   const ClassInfo *cls;
   const uint32_t *sched;        // per class: rounds * P entries, node | parent << 16
+  const uint8_t *sched_fl;      // per entry: register hand-over flags (cn_cell.cuh)
   const int32_t *dist_nodes;    // local node lists of distributed tables per class
   const int32_t *node_off;      // per class: slot offset (round*32 + p*G) of every local node
   double *v;                    // [n_slot] schedule order, padded
@@ -203,6 +204,17 @@ __device__ __forceinline__ double rcp_fast(double x) {
   r = fma(r, e, r);
   e = fma(-x, r, 1.0);
   return fma(r, e, r);
+}
+
+// The same with ONE correction step of third order (r (1 + e + e^2), e = 1 - x r): three dependent
+// fp64 operations behind the MUFU instead of four, relative error ~ e^3 (< 1e-17 from the ~2e-6
+// seed).  Used where the reciprocal sits on the dependent chain of an elimination.
+__device__ __forceinline__ double rcp_chain(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x, r, 1.0);
+  const double t = fma(e, e, e);
+  return fma(r, t, r);
 }
 
 // exp(x) for |x| < 700 to ~1 ulp without the special-case handling of the library routine:

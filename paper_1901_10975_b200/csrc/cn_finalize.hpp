@@ -153,12 +153,14 @@ static int finalize(cn_model *m, double dt) {
   // schedule-ordered off-diagonals
   std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
   std::vector<uint32_t> sched_all;
+  std::vector<uint8_t> schedfl_all;
   std::vector<int32_t> nodeoff_all;
   std::vector<ClassInfo> cinfo(m->cls.size());
   for (size_t kc = 0; kc < m->cls.size(); ++kc) {
     const HClass &K = m->cls[kc];
     cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, K.nodeoff_off, 0};
     sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
+    schedfl_all.insert(schedfl_all.end(), K.sched_fl.begin(), K.sched_fl.end());
     nodeoff_all.insert(nodeoff_all.end(), K.node_off.begin(), K.node_off.end());
   }
   for (int g = 0; g < ng; ++g) {
@@ -214,6 +216,7 @@ static int finalize(cn_model *m, double dt) {
     GroupInfo *dg; ClassInfo *dc; uint32_t *ds; int32_t *dn;
     UP(m->grp, dg); UP(cinfo, dc); UP(sched_all, ds); UP(m->dist_nodes, dn);
     H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
+    uint8_t *dfl; UP(schedfl_all, dfl); H.sched_fl = dfl;
     int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
     double *p;
     // nodes of warp-cooperative cells that carry point processes: negative static diagonal
@@ -536,7 +539,12 @@ static int finalize(cn_model *m, double dt) {
       int dev = 0, sms = 0;
       CU(cudaGetDevice(&dev));
       CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-      const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (227 * 1024) / (max_bytes + 1024)));
+      int max_n = 1;
+      for (const HClass &K : m->cls)
+        if (K.count - K.tp.n_cells > 0) max_n = std::max(max_n, K.n);
+      m->cwin_threads = max_n <= 128 ? 64 : max_n <= 320 ? 128 : 256;
+      const int per_sm = (int)std::max<size_t>(
+          1, std::min<size_t>(std::min(32, 2048 / m->cwin_threads), (227 * 1024) / (max_bytes + 1024)));
       if (onchip == -1 && ng > sms * per_sm) ok = false;  // auto: only when everything is resident at once
       m->cwin_grid = std::min(ng, sms * per_sm);
       m->cwin_smem = max_bytes;
@@ -562,9 +570,11 @@ static int finalize(cn_model *m, double dt) {
         rc = dev_upload(m, T.pp_local, &T.d_pp_local); if (rc != CN_OK) return rc;
         H.tab[t].pp_local = T.d_pp_local;
       }
-      if (max_bytes > 48 * 1024)
-        CU(cudaFuncSetAttribute(cell_window_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)max_bytes));
+      if (max_bytes > 48 * 1024) {
+        CU(cudaFuncSetAttribute(cell_window_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_bytes));
+        CU(cudaFuncSetAttribute(cell_window_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_bytes));
+        CU(cudaFuncSetAttribute(cell_window_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_bytes));
+      }
     }
   }
   rc = dev_alloc(m, 2, &H.step_ctr); if (rc != CN_OK) return rc;

@@ -171,7 +171,33 @@ static int build_layout(cn_model *m) {
   // A smaller model goes to the interleaved kernel too if ALL of it fits there (then it runs in
   // window mode: one launch per min-delay window instead of three per dt) and its groups fill at
   // least a quarter of their lanes; decided after the programs are compiled (below).
-  const bool auto_small = tape_mode == -1 && nc < tape_min_cells && nc > 0;
+  // A small model whose cells can all be RESIDENT ON CHIP AT ONCE (one CTA per cell, cn_cell.cuh)
+  // goes to the on-chip window kernel instead: it then never streams from HBM inside a min-delay
+  // window (config 1: 8.2 instead of 13.0 us per dt; config 2: 23 instead of 61).  Estimated here
+  // for a 148-SM device; finalize() checks the real one and the delays (fallback: one launch
+  // sequence per dt on the warp-cooperative kernel).
+  int onchip_opt = -1;
+  if (const char *e = m->opt("onchip")) onchip_opt = std::atoi(e);
+  bool prefer_onchip = false;
+  if (tape_mode == -1 && onchip_opt != 0 && nc > 0 && nc < tape_min_cells) {
+    size_t max_bytes = 0;
+    int max_n = 1;
+    for (const HClass &K : m->cls) {
+      size_t d = (size_t)K.n * (7 + (m->any_ica ? 1 : 0) + (m->any_cai ? 1 : 0));
+      for (const HTable &T : m->tab)
+        if (!T.ti.point && T.type != CN_PAS)
+          d += (size_t)(T.ti.n_dev_param + T.ti.n_state) *
+               (size_t)(T.cell_first[K.rep_cell + 1] - T.cell_first[K.rep_cell]);
+      max_bytes = std::max(max_bytes, d * 8);
+      max_n = std::max(max_n, K.n);
+    }
+    const int threads = max_n <= 128 ? 64 : max_n <= 320 ? 128 : 256;
+    const size_t per_sm = std::min<size_t>(std::min(32, 2048 / threads), (227 * 1024) / (max_bytes + 1024));
+    prefer_onchip = max_bytes <= 220 * 1024 && (size_t)nc <= 148 * per_sm;
+    for (const HTable &T : m->tab)
+      if (T.type == CN_GAP && T.n > 0) prefer_onchip = false;
+  }
+  const bool auto_small = tape_mode == -1 && nc < tape_min_cells && nc > 0 && !prefer_onchip;
   if (auto_small && !m->opt("tape_min_group")) tape_min_group = 1;
   const bool tape_on = tape_mode == 1 || (tape_mode == -1 && nc >= tape_min_cells) || auto_small;
   // W warps per group (CTA), each with a ring of S chunks x CH rows; the whole CTA must fit the
@@ -333,6 +359,7 @@ static int build_layout(cn_model *m) {
   if (const char *e = m->opt("force_g")) force_g = std::atoi(e);
   int max_g = 4;
   if (const char *e = m->opt("max_g")) max_g = std::max(1, std::atoi(e));
+  if (onchip_opt == 1 || prefer_onchip) max_g = 1;  // the on-chip window kernel keeps one cell per CTA
   int64_t smem_cap = 24 * 1024;
   if (const char *e = m->opt("warp_smem")) smem_cap = std::atoll(e);
   const int64_t hard_cap = 200 * 1024;
@@ -344,6 +371,7 @@ static int build_layout(cn_model *m) {
     K.needs_ica = m->any_ica ? 1 : 0;
     const int64_t ccount = K.count - K.tp.n_cells;  // cells left for the cooperative kernel
     K.sched.clear();
+    K.sched_fl.clear();
     K.node_off.assign(K.n, 0);
     if (ccount == 0) {
       K.G = 1; K.lgG = 0; K.rounds = 0;
@@ -375,7 +403,7 @@ static int build_layout(cn_model *m) {
     const int64_t f = m->cell_first[K.rep_cell];
     pl[0] = -1;
     for (int i = 1; i < K.n; ++i) pl[i] = (int32_t)(m->parent[f + i] - f);
-    K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched);
+    K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched, K.sched_fl);
     K.sched_off = sched_total;
     sched_total += (int)K.sched.size();
     K.node_off[0] = K.rounds * 32;

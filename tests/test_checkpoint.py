@@ -21,13 +21,17 @@ def _gpu(need_gpu):
     pass
 
 
+TAPE = {"tape": 1, "tape_min_group": 1}
 CASES = {
-    "config1-window": (lambda: W.config1(), {}, 13.7, 40.0),
-    "config1-per-step": (lambda: W.config1(), {"tape_window": 0}, 13.7, 40.0),
-    "config1-coop": (lambda: W.config1(), {"tape": 0}, 13.7, 40.0),
-    "config4-window": (lambda: W.config4(n_cell=256, n_types=8), {}, 20.3, 45.0),
-    "config3-window": (lambda: W.config3(n_cell=140, syn_per_cell=60), {}, 9.1, 30.0),
-    "config5-coop": (lambda: W.config5(n_cell=110, syn_per_cell=40), {}, 6.0, 16.0),
+    "config1-onchip": (lambda: W.config1(), {}, 13.7, 40.0),
+    "config1-window": (lambda: W.config1(), TAPE, 13.7, 40.0),
+    "config1-per-step": (lambda: W.config1(), dict(TAPE, tape_window=0), 13.7, 40.0),
+    "config1-coop": (lambda: W.config1(), {"tape": 0, "onchip": 0}, 13.7, 40.0),
+    "config4-window": (lambda: W.config4(n_cell=256, n_types=8), TAPE, 20.3, 45.0),
+    "config3-window": (lambda: W.config3(n_cell=140, syn_per_cell=60), TAPE, 9.1, 30.0),
+    "config3-onchip": (lambda: W.config3(n_cell=140, syn_per_cell=60), {}, 9.1, 30.0),
+    "config5-coop": (lambda: W.config5(n_cell=110, syn_per_cell=40), {"onchip": 0}, 6.0, 16.0),
+    "config5-onchip": (lambda: W.config5(n_cell=110, syn_per_cell=40), {}, 6.0, 16.0),
 }
 
 
@@ -170,13 +174,14 @@ def _with_late_stimuli(desc, variant, t_on):
     return d
 
 
-@pytest.mark.parametrize("mode", ["window", "per-step", "coop"])
+@pytest.mark.parametrize("mode", ["window", "per-step", "coop", "onchip"])
 def test_restart_with_different_stimuli(cn, mode, opts):
     """save at T1, restore into models whose stimuli differ after T1 (IClamp tables,
     scripted sources); each continuation must equal ITS OWN uninterrupted oracle run (the variants
     agree up to T1 because their stimuli only start later, so the state at T1 is theirs too)."""
     from oracle import OracleModel
-    opts.update({"window": {}, "per-step": {"tape_window": 0}, "coop": {"tape": 0}}[mode])
+    opts.update({"window": TAPE, "per-step": dict(TAPE, tape_window=0), "coop": {"tape": 0, "onchip": 0},
+                 "onchip": {}}[mode])
     t1, t2 = 12.0, 40.0
     base = W.config1()
     a_desc, b_desc = _with_late_stimuli(base, "A", t1), _with_late_stimuli(base, "B", t1)
@@ -202,9 +207,10 @@ def test_checkpoint_moves_between_kernels_and_launch_modes(cn):
     from oracle import OracleModel
     desc = W.config3(n_cell=140, syn_per_cell=60)
     t1, t2, t3 = 9.1, 20.0, 30.0
-    a = cn.Model(desc)                                  # interleaved, window mode
+    a = cn.Model(desc, options=TAPE)                    # interleaved, window mode
     a.run(t1, DT)
-    b = cn.Model(desc, options={"tape": 0})             # warp-cooperative, per step
+    assert a.run_info()["mode"] == "window"
+    b = cn.Model(desc, options={"tape": 0, "onchip": 0})  # warp-cooperative, per step
     b.restore(a.checkpoint())
     b.run(t2, DT)
     c = cn.Model(desc, options={"tape": 1, "tape_window": 0, "tape_min_group": 1})

@@ -58,11 +58,19 @@ def test_shapes_that_do_not_fit_fall_back(cn):
 
 
 def test_auto_strategy_for_small_models(cn):
-    for desc, on_tape in ((W.config1(), True), (W.config3(n_cell=140, syn_per_cell=20), True),
+    """Default strategy below 8,192 cells: a model whose cells are all resident on chip at once goes
+    to the on-chip window kernel (warp-cooperative layout, one cell per CTA); a larger one to the
+    interleaved kernel if all of it fits there; else the warp-cooperative kernel."""
+    for desc, on_tape in ((W.config1(), False), (W.config3(n_cell=140, syn_per_cell=20), False),
                           (W.config2(n_cell=8, ring_size=4), False),
-                          (W.random_tree_cells(13, 5, 120, stream="gpu-u"), False)):
+                          (W.random_tree_cells(13, 5, 120, stream="gpu-u"), False),
+                          (W.config3(syn_per_cell=2), True),
+                          (W.config5(n_cell=3000, syn_per_cell=2), False)):
         m = cn.Model(desc)
         info = m.layout_info()
         m.destroy()
         assert (info["n_tape_group"] == info["n_group"]) == on_tape, info
         assert on_tape or info["n_tape_group"] == 0
+    # the explicit options still decide
+    m = cn.Model(W.config1(), options={"onchip": 0})
+    assert m.layout_info()["n_tape_group"] == m.layout_info()["n_group"] == 1
