@@ -11,8 +11,8 @@
 // and writes voltages and states back once.  Between the load and the store nothing but the few
 // synapse states of the cell, the delivered weights and the spike list touches L2 / HBM: the step
 // is bound by the fp64 pipe and by the dependent chain of the elimination, not by memory.
-// All W warps share the mechanism work (one thread per instance); warp 0 runs the elimination in
-// the list-scheduled rounds of the warp-cooperative kernel (cn_device.cuh, same arithmetic).
+// All warps share the mechanism work (one thread per instance) and the elimination (one thread per
+// unbranched chain of the tree, the chains of one level side by side).
 // Used for models whose cells all sit on the warp-cooperative layout with one cell per warp and
 // fit the device at once (configs 1 and 2; option onchip=1 forces it for any model whose largest
 // cell fits the shared memory of a CTA).  Gap junctions need the peer's voltage of every step and
@@ -27,18 +27,19 @@ template <int NT>
 __global__ void __launch_bounds__(NT)
     cell_window_kernel(const __grid_constant__ DModel M, int64_t k0, int nsteps, int64_t trace_row0) {
   extern __shared__ double csm[];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x;
   const double dt = M.dt;
   for (int g = blockIdx.x; g < M.n_group; g += gridDim.x) {
     const GroupInfo gi = M.grp[g];
     const ClassInfo ci = M.cls[gi.cls];
     const CellClass &cc = M.ccls[gi.cls];
-    const int n = ci.n, rounds = ci.rounds;
+    const int n = ci.n;
     const int64_t ab = gi.ab_base;
     const int32_t *__restrict__ noff = M.node_off + ci.nodeoff_off;
-    // shared memory: A B DS RS V D R [I] [CAI] by local node, then the mechanism block
+    // shared memory: A B DS RS V D R CD CR [I] [CAI] by local node, then the mechanism block
     double *A = csm, *B = A + n, *DS = B + n, *RS = DS + n, *V = RS + n, *D = V + n, *R = D + n;
-    double *nx = R + n;
+    double *CD = R + n, *CR = CD + n;  // contribution of the last node of a chain to its parent
+    double *nx = CR + n;
     double *I = nullptr, *CAI = nullptr;
     if (ci.needs_ica) { I = nx; nx += n; }
     if (M.cai) { CAI = nx; nx += n; }
@@ -79,7 +80,6 @@ __global__ void __launch_bounds__(NT)
     gv.G = 1;
     gv.lgG = 0;
     gv.direct = true;
-    const uint32_t *__restrict__ sched = M.sched + ci.sched_off + lane;
     __syncthreads();
 
     for (int s = 0; s < nsteps; ++s) {
@@ -187,65 +187,69 @@ __global__ void __launch_bounds__(NT)
                         tid, NT);
         __syncthreads();
       }
-      // ---- Hines solve: warp 0, rounds of independent nodes (L66).  Along a chain the parent sits
-      // on its child's lane in the next round (SF_OUT / SF_IN, cn_host.hpp hu_schedule): the
-      // contribution travels in a register, and so does the parent's v on the way back; only
-      // contributions that meet at a branch point go through the parent's row. --------------------
-      if (warp == 0) {
-        const uint8_t *__restrict__ sfl = M.sched_fl + ci.sched_off + lane;
-        uint32_t en = rounds > 0 ? __ldg(sched) : CN_IDLE;
-        uint32_t fn = rounds > 0 ? __ldg(sfl) : 0u;
-        double accD = 0.0, accR = 0.0;
-        for (int r = 0; r < rounds; ++r) {
-          const uint32_t e = en, fl = fn;
-          if (r + 1 < rounds) {
-            en = __ldg(sched + (size_t)(r + 1) * 32);
-            fn = __ldg(sfl + (size_t)(r + 1) * 32);
-          }
-          if ((e & 0xFFFFu) != CN_IDLE) {
-            const int si = (int)(e & 0xFFFFu), sp = (int)(e >> 16);
-            double di = D[si] + DS[si], ri = R[si] + (V[si] + RS[si]);
-            if (fl & 2u) {  // SF_IN
-              di += accD;
-              ri += accR;
+      // ---- Hines solve (L66): one thread per unbranched chain, one barrier per level of the tree
+      // of chains (cn_finalize.hpp build_cell_segments).  Along a chain the contribution to the
+      // parent, and on the way back the parent's v, travel in registers; where chains meet, the
+      // parent's chain sums the contributions of its children in a fixed order. ----------------------
+      {
+        const CellSeg *__restrict__ segs = M.cseg + cc.seg_off;
+        const int32_t *__restrict__ lvl = M.cseg_lvl + cc.lvl_off;
+        for (int L = 0; L < cc.n_lev; ++L) {
+          const int s1 = lvl[L + 1];
+          for (int sg = lvl[L] + tid; sg < s1; sg += NT) {
+            const CellSeg S = segs[sg];
+            const uint16_t *__restrict__ nd = M.cseg_nodes + S.node_off;
+            const uint16_t *__restrict__ chn = M.cseg_child + S.child_off;
+            double accD = 0.0, accR = 0.0;
+            for (int c = 0; c < (int)S.nchild; ++c) {
+              accD += CD[chn[c]];
+              accR += CR[chn[c]];
             }
-            const double rinv = rcp_chain(di);
-            const double a = A[si], b = B[si];
-            const double f = a * rinv;
-            const double cD = -(f * b), cR = -(f * ri);
-            if (fl & 1u) {  // SF_OUT
-              accD = cD;
-              accR = cR;
-            } else {
-              D[sp] += cD;
-              R[sp] += cR;
+            int x = nd[0];
+            for (int j = 0; j < (int)S.len; ++j) {
+              const int xn = j + 1 < (int)S.len ? nd[j + 1] : x;
+              const double di = (D[x] + DS[x]) + accD, ri = (R[x] + (V[x] + RS[x])) + accR;
+              const double a = A[x], b = B[x];
+              const double rinv = rcp_chain(di);
+              const double f = a * rinv;
+              D[x] = b * rinv;  // back-substitution multiplier
+              R[x] = ri * rinv;
+              accD = -(f * b);
+              accR = -(f * ri);
+              if (j + 1 == (int)S.len) {
+                CD[x] = accD;
+                CR[x] = accR;
+              }
+              x = xn;
             }
-            D[si] = b * rinv;  // back-substitution multiplier
-            R[si] = ri * rinv;
           }
-          __syncwarp();
+          __syncthreads();
         }
-        if (lane == 0) R[0] = (R[0] + (V[0] + RS[0])) * rcp_fast(D[0] + DS[0]);
-        __syncwarp();
-        double vreg = 0.0;
-        en = rounds > 0 ? __ldg(sched + (size_t)(rounds - 1) * 32) : CN_IDLE;
-        fn = rounds > 0 ? __ldg(sfl + (size_t)(rounds - 1) * 32) : 0u;
-        for (int r = rounds - 1; r >= 0; --r) {
-          const uint32_t e = en, fl = fn;
-          if (r > 0) {
-            en = __ldg(sched + (size_t)(r - 1) * 32);
-            fn = __ldg(sfl + (size_t)(r - 1) * 32);
+        if (tid == 0) {
+          const uint16_t *__restrict__ chn = M.cseg_child + cc.root_child_off;
+          double accD = 0.0, accR = 0.0;
+          for (int c = 0; c < cc.root_nchild; ++c) {
+            accD += CD[chn[c]];
+            accR += CR[chn[c]];
           }
-          if ((e & 0xFFFFu) != CN_IDLE) {
-            const int si = (int)(e & 0xFFFFu), sp = (int)(e >> 16);
-            const double vp = (fl & 1u) ? vreg : R[sp];  // (SF_OUT: this lane solved the parent last)
-            vreg = fma(-D[si], vp, R[si]);
-            R[si] = vreg;
+          R[0] = ((R[0] + (V[0] + RS[0])) + accR) * rcp_fast((D[0] + DS[0]) + accD);
+        }
+        __syncthreads();
+        for (int L = cc.n_lev - 1; L >= 0; --L) {
+          const int s1 = lvl[L + 1];
+          for (int sg = lvl[L] + tid; sg < s1; sg += NT) {
+            const CellSeg S = segs[sg];
+            const uint16_t *__restrict__ nd = M.cseg_nodes + S.node_off;
+            double vp = R[S.par];
+            for (int j = (int)S.len - 1; j >= 0; --j) {
+              const int x = nd[j];
+              vp = fma(-D[x], vp, R[x]);
+              R[x] = vp;
+            }
           }
-          __syncwarp();
+          __syncthreads();
         }
       }
-      __syncthreads();
       // ---- voltage update, threshold at the root (L66, L68), probes -------------------------------
       for (int i = tid; i < n; i += NT) V[i] = R[i];
       if (tid == 0) {

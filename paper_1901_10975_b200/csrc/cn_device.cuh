@@ -122,7 +122,20 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
 // shared memory (doubles from the start of the mechanism block), and the size of the whole block
 struct CellClass {
   int32_t mech_off[CN_MAX_TABLES];
-  int32_t mech_doubles, pad;
+  int32_t mech_doubles;
+  // elimination plan (cn_finalize.hpp build_cell_segments): segments [seg_off, ...) sorted by
+  // level, lvl[lvl_off + L] = first segment of level L (relative to seg_off), n_lev + 1 entries;
+  // the children of the root
+  int32_t seg_off, n_lev, lvl_off, root_child_off, root_nchild;
+};
+
+// one unbranched chain of a cell: nodes[node_off .. node_off + len) in elimination order (distal
+// to proximal), the children of its first node (each the last node of an earlier segment), and
+// the parent of its last node
+struct CellSeg {
+  uint32_t node_off, child_off;
+  uint16_t len, nchild;
+  uint32_t par;
 };
 
 struct DModel {
@@ -138,7 +151,6 @@ struct DModel {
   const GroupInfo *grp;
   const ClassInfo *cls;
   const uint32_t *sched;        // per class: rounds * P entries, node | parent << 16
-  const uint8_t *sched_fl;      // per entry: register hand-over flags (cn_cell.cuh)
   const int32_t *dist_nodes;    // local node lists of distributed tables per class
   const int32_t *node_off;      // per class: slot offset (round*32 + p*G) of every local node
   double *v;                    // [n_slot] schedule order, padded
@@ -186,6 +198,9 @@ struct DModel {
   int32_t n_probe, pad3;
   int64_t *step_ctr;            // [0] step, [1] trace row that a replayed CUDA graph starts from
   const struct CellClass *ccls; // cell-window mode (cn_cell.cuh): shared-memory layout per class
+  const struct CellSeg *cseg;   //   and elimination plan
+  const uint16_t *cseg_nodes, *cseg_child;
+  const int32_t *cseg_lvl;
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
 };

@@ -7,6 +7,73 @@
 // first cn_run: dt-dependent constants (row-normalised system), initial states, upload
 // ---------------------------------------------------------------------------------------------
 
+// Elimination plan of the on-chip window kernel (cn_cell.cuh) for one class: the tree is cut into
+// SEGMENTS, maximal unbranched chains x0 -> parent(x0) -> ... -> xk (x0 a leaf or a branch point,
+// every later node with exactly one child); one thread eliminates a whole segment with the
+// contribution travelling in registers.  A segment may start once all segments that end at the
+// children of x0 are done: its LEVEL.  All segments of a level run side by side on the threads of
+// the CTA, one barrier per level; sibling contributions are summed by the parent's segment in a
+// fixed order (no atomics: runs are bit-reproducible).
+static void build_cell_segments(const cn_model *m, const HClass &K, CellClass &cc,
+                                std::vector<CellSeg> &segs, std::vector<uint16_t> &nodes,
+                                std::vector<uint16_t> &child, std::vector<int32_t> &lvl) {
+  const int n = K.n;
+  const int64_t f = m->cell_first[K.rep_cell];
+  std::vector<int32_t> par(n, -1), nch(n, 0);
+  std::vector<std::vector<uint16_t>> ch(n);
+  for (int i = 1; i < n; ++i) {
+    par[i] = (int32_t)(m->parent[f + i] - f);
+    ch[par[i]].push_back((uint16_t)i);
+  }
+  struct Tmp { std::vector<uint16_t> nd; int level; int par; int x0; };
+  std::vector<Tmp> tmp;
+  std::vector<int> end_level(n, -1);  // level of the segment that ends at this node
+  for (int x = n - 1; x >= 1; --x) {
+    if (ch[x].size() == 1) continue;  // interior of a segment
+    Tmp t;
+    t.x0 = x;
+    t.level = 0;
+    for (uint16_t c : ch[x]) t.level = std::max(t.level, end_level[c] + 1);
+    int cur = x;
+    t.nd.push_back((uint16_t)cur);
+    while (par[cur] != 0 && ch[par[cur]].size() == 1) {
+      cur = par[cur];
+      t.nd.push_back((uint16_t)cur);
+    }
+    t.par = par[cur];
+    end_level[cur] = t.level;
+    tmp.push_back(std::move(t));
+  }
+  std::stable_sort(tmp.begin(), tmp.end(), [](const Tmp &a, const Tmp &b) {
+    if (a.level != b.level) return a.level < b.level;
+    return a.nd.size() > b.nd.size();
+  });
+  int nlev = 0;
+  for (const Tmp &t : tmp) nlev = std::max(nlev, t.level + 1);
+  cc.seg_off = (int32_t)segs.size();
+  cc.n_lev = nlev;
+  cc.lvl_off = (int32_t)lvl.size();
+  int li = 0;
+  for (int L = 0; L <= nlev; ++L) {
+    while (li < (int)tmp.size() && tmp[li].level < L) ++li;
+    lvl.push_back(li);
+  }
+  for (const Tmp &t : tmp) {
+    CellSeg sg;
+    sg.node_off = (uint32_t)nodes.size();
+    sg.child_off = (uint32_t)child.size();
+    sg.len = (uint16_t)t.nd.size();
+    sg.nchild = (uint16_t)ch[t.x0].size();
+    sg.par = (uint32_t)t.par;
+    nodes.insert(nodes.end(), t.nd.begin(), t.nd.end());
+    child.insert(child.end(), ch[t.x0].begin(), ch[t.x0].end());
+    segs.push_back(sg);
+  }
+  cc.root_child_off = (int32_t)child.size();
+  cc.root_nchild = (int32_t)ch[0].size();
+  child.insert(child.end(), ch[0].begin(), ch[0].end());
+}
+
 static int finalize(cn_model *m, double dt) {
   const bool dbg = m->opt("debug") && std::atoi(m->opt("debug")) != 0;
   auto t_prev = std::chrono::steady_clock::now();
@@ -153,14 +220,12 @@ static int finalize(cn_model *m, double dt) {
   // schedule-ordered off-diagonals
   std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
   std::vector<uint32_t> sched_all;
-  std::vector<uint8_t> schedfl_all;
   std::vector<int32_t> nodeoff_all;
   std::vector<ClassInfo> cinfo(m->cls.size());
   for (size_t kc = 0; kc < m->cls.size(); ++kc) {
     const HClass &K = m->cls[kc];
     cinfo[kc] = ClassInfo{K.n, K.G, K.lgG, K.rounds, K.sched_off, K.needs_ica, K.nodeoff_off, 0};
     sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
-    schedfl_all.insert(schedfl_all.end(), K.sched_fl.begin(), K.sched_fl.end());
     nodeoff_all.insert(nodeoff_all.end(), K.node_off.begin(), K.node_off.end());
   }
   for (int g = 0; g < ng; ++g) {
@@ -216,7 +281,6 @@ static int finalize(cn_model *m, double dt) {
     GroupInfo *dg; ClassInfo *dc; uint32_t *ds; int32_t *dn;
     UP(m->grp, dg); UP(cinfo, dc); UP(sched_all, ds); UP(m->dist_nodes, dn);
     H.grp = dg; H.cls = dc; H.sched = ds; H.dist_nodes = dn;
-    uint8_t *dfl; UP(schedfl_all, dfl); H.sched_fl = dfl;
     int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
     double *p;
     // nodes of warp-cooperative cells that carry point processes: negative static diagonal
@@ -518,6 +582,9 @@ static int finalize(cn_model *m, double dt) {
     if (wn < 2 && onchip != 1) ok = false;
     if (ok && m->win_ninst * wn * 8 > ((int64_t)4 << 30)) ok = false;
     std::vector<CellClass> ccls(m->cls.size());
+    std::vector<CellSeg> segs;
+    std::vector<uint16_t> seg_nodes, seg_child;
+    std::vector<int32_t> seg_lvl;
     size_t max_bytes = 0;
     if (ok) {
       for (size_t kc = 0; kc < m->cls.size(); ++kc) {
@@ -530,8 +597,10 @@ static int finalize(cn_model *m, double dt) {
           off += (T.ti.n_dev_param + T.ti.n_state) * T.cls_cnt[kc];
         }
         ccls[kc].mech_doubles = off;
-        if (K.count - K.tp.n_cells > 0)
-          max_bytes = std::max(max_bytes, ((size_t)K.n * (7 + (K.needs_ica ? 1 : 0) + (m->any_cai ? 1 : 0)) + off) * 8);
+        if (K.count - K.tp.n_cells > 0) {
+          max_bytes = std::max(max_bytes, ((size_t)K.n * (9 + (K.needs_ica ? 1 : 0) + (m->any_cai ? 1 : 0)) + off) * 8);
+          build_cell_segments(m, K, ccls[kc], segs, seg_nodes, seg_child, seg_lvl);
+        }
       }
       if (max_bytes > 220 * 1024) ok = false;
     }
@@ -564,6 +633,12 @@ static int finalize(cn_model *m, double dt) {
       CellClass *dcc;
       rc = dev_upload(m, ccls, &dcc); if (rc != CN_OK) return rc;
       H.ccls = dcc;
+      CellSeg *dsg; uint16_t *dsn, *dsc; int32_t *dsl;
+      rc = dev_upload(m, segs, &dsg); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, seg_nodes, &dsn); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, seg_child, &dsc); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, seg_lvl, &dsl); if (rc != CN_OK) return rc;
+      H.cseg = dsg; H.cseg_nodes = dsn; H.cseg_child = dsc; H.cseg_lvl = dsl;
       for (int t = 0; t < nt; ++t) {
         HTable &T = m->tab[t];
         if (!T.ti.point) continue;

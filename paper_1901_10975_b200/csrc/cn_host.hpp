@@ -239,7 +239,6 @@ struct HClass {
   int sched_off = 0;
   std::vector<int32_t> cells;
   std::vector<uint32_t> sched;
-  std::vector<uint8_t> sched_fl;  // SF_* per schedule entry
   std::vector<int32_t> node_off;  // local node -> slot offset round*32 + p*G (root: rounds*32)
   int nodeoff_off = 0;
 };
@@ -409,16 +408,8 @@ static int dev_alloc(cn_model *m, size_t n, T **out, bool zero = true) {
 // at most one child of a parent per round so that the parent updates never collide)
 // ---------------------------------------------------------------------------------------------
 
-// flags (one byte per schedule entry, used by the on-chip window kernel): a node whose parent is
-// eliminated in the NEXT round is moved to... rather, the parent is moved to the child's lane, so
-// that the child hands its contribution over in a register (SF_OUT) and the parent takes it from
-// there (SF_IN); in the back-substitution the child then finds its parent's v in the same register.
-enum { SF_OUT = 1, SF_IN = 2 };
-
-static int hu_schedule(int n, const int32_t *par, int P, std::vector<uint32_t> &out,
-                       std::vector<uint8_t> &flags) {
+static int hu_schedule(int n, const int32_t *par, int P, std::vector<uint32_t> &out) {
   out.clear();
-  flags.clear();
   if (n <= 1) return 0;
   std::vector<int> depth(n, 0), left(n, 0), used(n, -1);
   int maxd = 0;
@@ -456,45 +447,6 @@ static int hu_schedule(int n, const int32_t *par, int P, std::vector<uint32_t> &
     }
     for (int j = (int)picked.size(); j < P; ++j) out.push_back(CN_IDLE | (CN_IDLE << 16));
     ++round;
-  }
-  // lane-stable chains: within round r + 1, put the parent of lane l's node of round r on lane l
-  // (at most one child of a parent per round, so the wishes of a round never collide)
-  flags.assign(out.size(), 0);
-  std::vector<uint32_t> tmp(P);
-  std::vector<int> lane_of(n, -1);
-  for (int r = 0; r + 1 < round; ++r) {
-    uint32_t *cur = out.data() + (size_t)r * P, *nxt = out.data() + (size_t)(r + 1) * P;
-    for (int l = 0; l < P; ++l)
-      if ((nxt[l] & 0xFFFFu) != CN_IDLE) lane_of[nxt[l] & 0xFFFFu] = l;
-    std::vector<int> want(P, -1);  // lane -> entry of nxt that should sit there
-    std::vector<uint8_t> taken(P, 0);
-    for (int l = 0; l < P; ++l) {
-      if ((cur[l] & 0xFFFFu) == CN_IDLE) continue;
-      const int p = (int)(cur[l] >> 16);
-      if (p != 0 && lane_of[p] >= 0) {
-        want[l] = lane_of[p];
-        taken[lane_of[p]] = 1;
-      }
-    }
-    int free_src = 0;
-    for (int l = 0; l < P; ++l) {
-      if (want[l] >= 0) {
-        tmp[l] = nxt[want[l]];
-      } else {
-        while (free_src < P && taken[free_src]) ++free_src;
-        tmp[l] = nxt[free_src++];
-      }
-    }
-    for (int l = 0; l < P; ++l) {
-      if ((nxt[l] & 0xFFFFu) != CN_IDLE) lane_of[nxt[l] & 0xFFFFu] = -1;
-    }
-    for (int l = 0; l < P; ++l) {
-      nxt[l] = tmp[l];
-      if (want[l] >= 0) {
-        flags[(size_t)r * P + l] |= SF_OUT;
-        flags[(size_t)(r + 1) * P + l] |= SF_IN;
-      }
-    }
   }
   return round;
 }

@@ -183,7 +183,7 @@ static int build_layout(cn_model *m) {
     size_t max_bytes = 0;
     int max_n = 1;
     for (const HClass &K : m->cls) {
-      size_t d = (size_t)K.n * (7 + (m->any_ica ? 1 : 0) + (m->any_cai ? 1 : 0));
+      size_t d = (size_t)K.n * (9 + (m->any_ica ? 1 : 0) + (m->any_cai ? 1 : 0));
       for (const HTable &T : m->tab)
         if (!T.ti.point && T.type != CN_PAS)
           d += (size_t)(T.ti.n_dev_param + T.ti.n_state) *
@@ -371,7 +371,6 @@ static int build_layout(cn_model *m) {
     K.needs_ica = m->any_ica ? 1 : 0;
     const int64_t ccount = K.count - K.tp.n_cells;  // cells left for the cooperative kernel
     K.sched.clear();
-    K.sched_fl.clear();
     K.node_off.assign(K.n, 0);
     if (ccount == 0) {
       K.G = 1; K.lgG = 0; K.rounds = 0;
@@ -403,7 +402,7 @@ static int build_layout(cn_model *m) {
     const int64_t f = m->cell_first[K.rep_cell];
     pl[0] = -1;
     for (int i = 1; i < K.n; ++i) pl[i] = (int32_t)(m->parent[f + i] - f);
-    K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched, K.sched_fl);
+    K.rounds = hu_schedule(K.n, pl.data(), 32 / G, K.sched);
     K.sched_off = sched_total;
     sched_total += (int)K.sched.size();
     K.node_off[0] = K.rounds * 32;
