@@ -730,6 +730,15 @@ extern "C" int cn_debug_tasks(const cn_model *m, int32_t *out, int32_t cap) {
   return 0;
 }
 
+extern "C" int cn_debug_cell_trace(long long *out, int reset) {
+  int rc = (int)cudaMemcpyFromSymbol(out, cn::g_cell_trace, sizeof(long long) * 16);
+  if (reset) {
+    long long z[16] = {};
+    cudaMemcpyToSymbol(cn::g_cell_trace, z, sizeof(z));
+  }
+  return rc;
+}
+
 extern "C" int cn_debug_trace(long long *out) {
   return (int)cudaMemcpyFromSymbol(out, cn::g_trace, sizeof(long long) * 148 * 16 * 8 * 8);
 }

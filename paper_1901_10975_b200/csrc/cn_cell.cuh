@@ -5,22 +5,191 @@
 // for `nsteps` <= min-delay steps a cell depends on nothing but itself and on events whose spikes
 // were recorded before the window (summed per (step, synapse) by deliver_window_kernel).  The CTA
 // loads the cell once -- tree coefficients, voltages, parameters and states of every distributed
-// mechanism, cai -- into shared memory, runs the whole hot path nsteps times there:
+// mechanism, cai, and the cell's elimination plan -- into shared memory, runs the whole hot path
+// nsteps times there:
 //     point processes (events of the step, conductances; L64, L65) -> nrn_cur of the distributed
 //     mechanisms (L65) -> Hines solve (L66) -> voltage update -> nrn_state (L67) -> threshold (L68)
 // and writes voltages and states back once.  Between the load and the store nothing but the few
 // synapse states of the cell, the delivered weights and the spike list touches L2 / HBM: the step
 // is bound by the fp64 pipe and by the dependent chain of the elimination, not by memory.
-// All warps share the mechanism work (one thread per instance) and the elimination (one thread per
-// unbranched chain of the tree, the chains of one level side by side).
+//
+// Elimination: the tree is cut into unbranched CHAINS (cn_finalize.hpp build_cell_plan); one
+// thread eliminates a whole chain with the contribution to the parent travelling in registers
+// (and the parent's v on the way back); the chains of one level of the tree of chains run side by
+// side on the lanes of one warp, one barrier per level; where chains meet, the parent's chain
+// sums its children's contributions in a fixed order (no atomics: runs are bit-reproducible).
+// Every per-node array in shared memory is in PLAN ORDER -- the nodes of a chain side by side --
+// so the chain loops address shared memory by a running index: no index loads on the chain.
+//
 // Used for models whose cells all sit on the warp-cooperative layout with one cell per warp and
-// fit the device at once (configs 1 and 2; option onchip=1 forces it for any model whose largest
-// cell fits the shared memory of a CTA).  Gap junctions need the peer's voltage of every step and
-// exclude this mode.
+// fit the device at once (configs 1 and 2 by default; option onchip=1 forces it for any model
+// whose largest cell fits the shared memory of a CTA).  Gap junctions need the peer's voltage of
+// every step and exclude this mode.
 #pragma once
 #include "cn_device.cuh"
 
 namespace cn {
+
+#ifdef CN_TRACE
+__device__ long long g_cell_trace[16];
+#define CN_CT(i) do { if (tid == 0 && blockIdx.x == 0) { const long long t_ = clock64(); g_cell_trace[i] += t_ - tprev; tprev = t_; } } while (0)
+#else
+#define CN_CT(i)
+#endif
+
+// the point processes of one cell for one step: events delivered at this step, conductance and
+// current into the node's row (several instances may sit on one node: shared-memory atomics; the
+// order of the additions is the only run-to-run freedom, as in pp_step_kernel), state decay
+template <int NT>
+__device__ __forceinline__ void cell_point_processes(const DModel &M, const long long *ppq, int s,
+                                                     int64_t k, double *D, double *R,
+                                                     const double *V, int tid) {
+  const double t_mid = ((double)k + 0.5) * M.dt;
+  for (int t = 0; t < M.n_table; ++t) {
+    const DTable &T = M.tab[t];
+    if (!T.is_point) continue;
+    const int64_t q0 = ppq[2 * t], q1 = ppq[2 * t + 1];
+    double *dl0 = M.win_deliv ? M.win_deliv + (size_t)s * M.win_ninst + T.pp_goff : nullptr;
+    for (int64_t q = q0 + tid; q < q1; q += NT) {
+      const int nd = T.pp_local[q];
+      double w = 0.0;
+      if (dl0 && T.type != T_ICLAMP) {
+        w = dl0[q];
+        if (w != 0.0) dl0[q] = 0.0;
+      }
+      switch (T.type) {
+        case T_EXPSYN: {
+          double gg = T.state[0][q];
+          if (w != 0.0) gg += w;
+          if (gg != 0.0) {
+            const double gs = gg * T.param[2][q];
+            atomicAdd(&D[nd], gs);
+            atomicAdd(&R[nd], gs * T.param[1][q]);
+            T.state[0][q] = decay(gg, T.param[0][q]);
+          }
+          break;
+        }
+        case T_EXP2SYN: {
+          double a = T.state[0][q], b = T.state[1][q];
+          if (w != 0.0) {
+            const double wf = w * T.param[4][q];
+            a += wf;
+            b += wf;
+          }
+          if (a != 0.0 || b != 0.0) {
+            const double gs = (b - a) * T.param[3][q];
+            if (gs != 0.0) {
+              atomicAdd(&D[nd], gs);
+              atomicAdd(&R[nd], gs * T.param[2][q]);
+            }
+            T.state[0][q] = decay(a, T.param[0][q]);
+            T.state[1][q] = decay(b, T.param[1][q]);
+          }
+          break;
+        }
+        case T_ICLAMP: {
+          const double del = T.param[0][q];
+          if (t_mid >= del && t_mid < del + T.param[1][q])
+            atomicAdd(&R[nd], T.param[2][q] * T.param[3][q]);
+          break;
+        }
+        case T_AMPANMDA: {
+          double a0 = T.state[0][q], a1 = T.state[1][q], a2 = T.state[2][q], a3 = T.state[3][q];
+          if (w != 0.0) {
+            const double wa = w * T.glob[7], wn = w * T.glob[8];
+            a0 += wa;
+            a1 += wa;
+            a2 += wn;
+            a3 += wn;
+          }
+          if (a0 != 0.0 || a1 != 0.0 || a2 != 0.0 || a3 != 0.0) {
+            const double gs =
+                ((a1 - a0) + T.glob[4] * (a3 - a2) * mgblock(V[nd], T.glob[5])) * T.param[0][q];
+            atomicAdd(&D[nd], gs);
+            atomicAdd(&R[nd], gs * T.glob[6]);
+            T.state[0][q] = decay(a0, T.glob[9]);
+            T.state[1][q] = decay(a1, T.glob[10]);
+            T.state[2][q] = decay(a2, T.glob[11]);
+            T.state[3][q] = decay(a3, T.glob[12]);
+          }
+          break;
+        }
+        default: break;
+      }
+    }
+  }
+}
+
+// Hines solve of one cell in shared memory (L66).  D / R come in as the assembled diagonal / right
+// side and leave as back-substitution multipliers / the new voltages.  `st`: this thread's index
+// among the SW solving threads (>= SW: not solving).
+template <int NT>
+__device__ __forceinline__ void cell_solve(const CellClass &cc, const CellSeg *segs,
+                                           const int32_t *lvl, const uint16_t *child,
+                                           const double *A, const double *B, double *D, double *R,
+                                           double *CD, double *CR, int n, int st, int SW, int tid) {
+  for (int L = 0; L < cc.n_lev; ++L) {
+    const int s1 = lvl[L + 1];
+    if (st < SW)
+      for (int sg = lvl[L] + st; sg < s1; sg += SW) {
+        const CellSeg S = segs[sg];
+        const uint16_t *chn = child + S.child_off;
+        double accD = 0.0, accR = 0.0;
+        for (int c = 0; c < (int)S.nchild; ++c) {
+          accD += CD[chn[c]];
+          accR += CR[chn[c]];
+        }
+        // operands of the next node are fetched while the current one is on the dependent chain:
+        // pivot -> reciprocal -> contribution (one DADD, MUFU + 3 DFMA, one DMUL)
+        const int x0 = S.first, len = S.len;
+        double d0 = D[x0], r0 = R[x0], a0 = A[x0], b0 = B[x0];
+        for (int j = 0; j < len; ++j) {
+          const int x = x0 + j, xn = j + 1 < len ? x + 1 : x;
+          const double d1 = D[xn], r1 = R[xn], a1 = A[xn], b1 = B[xn];
+          const double di = d0 + accD, ri = r0 + accR;
+          const double ab = a0 * b0, ar = a0 * ri;
+          const double rinv = rcp_chain(di);
+          accD = -(ab * rinv);
+          accR = -(ar * rinv);
+          D[x] = b0 * rinv;  // back-substitution multiplier
+          R[x] = ri * rinv;
+          d0 = d1; r0 = r1; a0 = a1; b0 = b1;
+        }
+        CD[x0 + len - 1] = accD;
+        CR[x0 + len - 1] = accR;
+      }
+    __syncthreads();
+  }
+  if (tid == 0) {  // the root is the last node of the plan
+    const uint16_t *chn = child + cc.root_child_off;
+    double accD = 0.0, accR = 0.0;
+    for (int c = 0; c < cc.root_nchild; ++c) {
+      accD += CD[chn[c]];
+      accR += CR[chn[c]];
+    }
+    R[n - 1] = (R[n - 1] + accR) * rcp_fast(D[n - 1] + accD);
+  }
+  __syncthreads();
+  for (int L = cc.n_lev - 1; L >= 0; --L) {
+    const int s1 = lvl[L + 1];
+    if (st < SW)
+      for (int sg = lvl[L] + st; sg < s1; sg += SW) {
+        const CellSeg S = segs[sg];
+        double vp = R[S.par];
+        const int x0 = S.first, len = S.len;
+        int x = x0 + len - 1;
+        double m0 = D[x], r0 = R[x];
+        for (int j = len - 1; j >= 0; --j, --x) {
+          const int xn = j > 0 ? x - 1 : x;
+          const double m1 = D[xn], r1 = R[xn];
+          vp = fma(-m0, vp, r0);
+          R[x] = vp;
+          m0 = m1; r0 = r1;
+        }
+      }
+    __syncthreads();
+  }
+}
 
 // NT threads per CTA: 64 for small cells (more CTAs per SM), up to 256 for large ones
 template <int NT>
@@ -29,14 +198,28 @@ __global__ void __launch_bounds__(NT)
   extern __shared__ double csm[];
   const int tid = threadIdx.x;
   const double dt = M.dt;
+  // which warp of this CTA runs the elimination: CTAs that arrive on the same SM take turns, so
+  // that their solving warps sit on different quarters (schedulers, fp64 pipes) of the SM
+  __shared__ int swarp_s;
+  __shared__ int cnt_s[CN_MAX_TABLES];          // instances per table of this cell
+  __shared__ long long ppq_s[2 * CN_MAX_TABLES];  // point-process instance range per table
+  if (tid == 0) {
+    uint32_t smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    swarp_s = (int)(atomicAdd(M.cwin_smctr + (smid & 255u), 1u) % (uint32_t)(NT / 32));
+  }
+  __syncthreads();
+  // the solving threads: the 32 lanes of warp `swarp` first, then those of the next warp
+  const int st = (tid - swarp_s * 32 + NT) % NT;
+  const int SW = NT < 64 ? NT : 64;
   for (int g = blockIdx.x; g < M.n_group; g += gridDim.x) {
     const GroupInfo gi = M.grp[g];
     const ClassInfo ci = M.cls[gi.cls];
     const CellClass &cc = M.ccls[gi.cls];
     const int n = ci.n;
     const int64_t ab = gi.ab_base;
-    const int32_t *__restrict__ noff = M.node_off + ci.nodeoff_off;
-    // shared memory: A B DS RS V D R CD CR [I] [CAI] by local node, then the mechanism block
+    // shared memory, per node in plan order: A B DS RS V D R CD CR [I] [CAI]; then the
+    // mechanism block; then the plan: chains, levels, child positions, node positions per table
     double *A = csm, *B = A + n, *DS = B + n, *RS = DS + n, *V = RS + n, *D = V + n, *R = D + n;
     double *CD = R + n, *CR = CD + n;  // contribution of the last node of a chain to its parent
     double *nx = CR + n;
@@ -44,22 +227,39 @@ __global__ void __launch_bounds__(NT)
     if (ci.needs_ica) { I = nx; nx += n; }
     if (M.cai) { CAI = nx; nx += n; }
     double *MB = nx;
+    CellSeg *segs = reinterpret_cast<CellSeg *>(MB + cc.mech_doubles);
+    int32_t *lvl = reinterpret_cast<int32_t *>(segs + cc.n_seg);
+    uint16_t *child = reinterpret_cast<uint16_t *>(lvl + cc.n_lev + 1);
+    uint16_t *dist = child + cc.n_child;
     __syncthreads();  // (the previous cell's stores are done with shared memory)
     // ---- load the cell ---------------------------------------------------------------------------
-    for (int i = tid; i < n; i += NT) {
-      const int64_t q = ab + noff[i];
-      A[i] = M.a_s[q];
-      B[i] = M.b_s[q];
-      DS[i] = fabs(M.dstat[q]);  // (a negative static diagonal marks nodes with point processes)
-      RS[i] = M.rstat[q];
-      V[i] = M.v[q];
-      if (CAI) CAI[i] = M.cai[q];
+    {
+      const int32_t *__restrict__ pno = M.cplan_noff + cc.noff_off;
+      for (int i = tid; i < n; i += NT) {
+        const int64_t q = ab + pno[i];
+        A[i] = M.a_s[q];
+        B[i] = M.b_s[q];
+        DS[i] = fabs(M.dstat[q]);  // (a negative static diagonal marks nodes with point processes)
+        RS[i] = M.rstat[q];
+        V[i] = M.v[q];
+        if (CAI) CAI[i] = M.cai[q];
+      }
+      for (int i = tid; i < cc.n_seg; i += NT) segs[i] = M.cseg[cc.seg_off + i];
+      for (int i = tid; i <= cc.n_lev; i += NT) lvl[i] = M.cseg_lvl[cc.lvl_off + i];
+      for (int i = tid; i < cc.n_child; i += NT) child[i] = M.cseg_child[cc.child_off + i];
+      for (int i = tid; i < cc.n_dist; i += NT) dist[i] = M.cdist[cc.dist_base + i];
+      for (int t = tid; t < M.n_table; t += NT) {
+        const DTable &T = M.tab[t];
+        cnt_s[t] = T.is_point || T.type == T_PAS ? 0 : T.cls_cnt[gi.cls];
+        ppq_s[2 * t] = T.is_point ? T.pp_first[g] : 0;
+        ppq_s[2 * t + 1] = T.is_point ? T.pp_first[g + 1] : 0;
+      }
     }
+    __syncthreads();
     for (int t = 0; t < M.n_table; ++t) {
       const DTable &T = M.tab[t];
-      if (T.is_point || T.type == T_PAS) continue;
-      const int cnt = T.cls_cnt[gi.cls];
-      if (cnt == 0) continue;
+      const int cnt = cnt_s[t];
+      if (cnt == 0 || T.type == T_CADYN) continue;
       const int64_t ib = T.grp_instbase[g];
       double *dst = MB + cc.mech_off[t];
       for (int j = 0; j < T.n_param; ++j, dst += cnt)
@@ -81,179 +281,43 @@ __global__ void __launch_bounds__(NT)
     gv.lgG = 0;
     gv.direct = true;
     __syncthreads();
-
+#ifdef CN_TRACE
+    long long tprev = clock64();
+#endif
     for (int s = 0; s < nsteps; ++s) {
       const int64_t k = k0 + s;
-      // ---- zero the system --------------------------------------------------------------------
+      // ---- the system starts from the static terms: D = static diagonal, R = v + static rhs -------
       for (int i = tid; i < n; i += NT) {
-        D[i] = 0.0;
-        R[i] = 0.0;
+        D[i] = DS[i];
+        R[i] = V[i] + RS[i];
         if (I) I[i] = 0.0;
       }
       __syncthreads();
-      // ---- point processes of the cell: events of this step, conductance / current, decay --------
-      // (several instances may sit on one node: shared-memory atomics)
-      {
-        const double t_mid = ((double)k + 0.5) * dt;
-        for (int t = 0; t < M.n_table; ++t) {
-          const DTable &T = M.tab[t];
-          if (!T.is_point) continue;
-          const int64_t q0 = T.pp_first[g], q1 = T.pp_first[g + 1];
-          double *dl0 = M.win_deliv ? M.win_deliv + (size_t)s * M.win_ninst + T.pp_goff : nullptr;
-          for (int64_t q = q0 + tid; q < q1; q += NT) {
-            const int nd = T.pp_local[q];
-            double w = 0.0;
-            if (dl0 && T.type != T_ICLAMP) {
-              w = dl0[q];
-              if (w != 0.0) dl0[q] = 0.0;
-            }
-            switch (T.type) {
-              case T_EXPSYN: {
-                double gg = T.state[0][q];
-                if (w != 0.0) gg += w;
-                if (gg != 0.0) {
-                  const double gs = gg * T.param[2][q];
-                  atomicAdd(&D[nd], gs);
-                  atomicAdd(&R[nd], gs * T.param[1][q]);
-                  T.state[0][q] = decay(gg, T.param[0][q]);
-                }
-                break;
-              }
-              case T_EXP2SYN: {
-                double a = T.state[0][q], b = T.state[1][q];
-                if (w != 0.0) {
-                  const double wf = w * T.param[4][q];
-                  a += wf;
-                  b += wf;
-                }
-                if (a != 0.0 || b != 0.0) {
-                  const double gs = (b - a) * T.param[3][q];
-                  if (gs != 0.0) {
-                    atomicAdd(&D[nd], gs);
-                    atomicAdd(&R[nd], gs * T.param[2][q]);
-                  }
-                  T.state[0][q] = decay(a, T.param[0][q]);
-                  T.state[1][q] = decay(b, T.param[1][q]);
-                }
-                break;
-              }
-              case T_ICLAMP: {
-                const double del = T.param[0][q];
-                if (t_mid >= del && t_mid < del + T.param[1][q])
-                  atomicAdd(&R[nd], T.param[2][q] * T.param[3][q]);
-                break;
-              }
-              case T_AMPANMDA: {
-                double a0 = T.state[0][q], a1 = T.state[1][q], a2 = T.state[2][q],
-                       a3 = T.state[3][q];
-                if (w != 0.0) {
-                  const double wa = w * T.glob[7], wn = w * T.glob[8];
-                  a0 += wa;
-                  a1 += wa;
-                  a2 += wn;
-                  a3 += wn;
-                }
-                if (a0 != 0.0 || a1 != 0.0 || a2 != 0.0 || a3 != 0.0) {
-                  const double gs =
-                      ((a1 - a0) + T.glob[4] * (a3 - a2) * mgblock(V[nd], T.glob[5])) * T.param[0][q];
-                  atomicAdd(&D[nd], gs);
-                  atomicAdd(&R[nd], gs * T.glob[6]);
-                  T.state[0][q] = decay(a0, T.glob[9]);
-                  T.state[1][q] = decay(a1, T.glob[10]);
-                  T.state[2][q] = decay(a2, T.glob[11]);
-                  T.state[3][q] = decay(a3, T.glob[12]);
-                }
-                break;
-              }
-              default: break;
-            }
-          }
-        }
-      }
+      CN_CT(0);
+      cell_point_processes<NT>(M, ppq_s, s, k, D, R, V, tid);
       __syncthreads();
+      CN_CT(1);
       // ---- nrn_cur of the distributed mechanisms (one instance per node and table) ----------------
       for (int t = 0; t < M.n_table; ++t) {
         const DTable &T = M.tab[t];
-        if (T.is_point || T.type == T_PAS || T.type == T_CADYN) continue;
-        const int cnt = T.cls_cnt[gi.cls];
-        if (cnt == 0) continue;
-        double *par[CN_MAX_PARAM], *st[CN_MAX_STATE];
+        const int cnt = cnt_s[t];
+        if (cnt == 0 || T.type == T_CADYN) continue;
+        double *par[CN_MAX_PARAM], *sta[CN_MAX_STATE];
         double *p = MB + cc.mech_off[t];
 #pragma unroll
         for (int j = 0; j < CN_MAX_PARAM; ++j) par[j] = p + (j < T.n_param ? j : 0) * cnt;
 #pragma unroll
-        for (int j = 0; j < CN_MAX_STATE; ++j) st[j] = p + (T.n_param + (j < T.n_state ? j : 0)) * cnt;
-        cur_distributed(T, par, st, 0, cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls], D, R, I, V,
-                        tid, NT);
+        for (int j = 0; j < CN_MAX_STATE; ++j) sta[j] = p + (T.n_param + (j < T.n_state ? j : 0)) * cnt;
+        cur_distributed(T, par, sta, 0, cnt, gv, dist + cc.dist_off[t], D, R, I, V, tid, NT);
         __syncthreads();
       }
-      // ---- Hines solve (L66): one thread per unbranched chain, one barrier per level of the tree
-      // of chains (cn_finalize.hpp build_cell_segments).  Along a chain the contribution to the
-      // parent, and on the way back the parent's v, travel in registers; where chains meet, the
-      // parent's chain sums the contributions of its children in a fixed order. ----------------------
-      {
-        const CellSeg *__restrict__ segs = M.cseg + cc.seg_off;
-        const int32_t *__restrict__ lvl = M.cseg_lvl + cc.lvl_off;
-        for (int L = 0; L < cc.n_lev; ++L) {
-          const int s1 = lvl[L + 1];
-          for (int sg = lvl[L] + tid; sg < s1; sg += NT) {
-            const CellSeg S = segs[sg];
-            const uint16_t *__restrict__ nd = M.cseg_nodes + S.node_off;
-            const uint16_t *__restrict__ chn = M.cseg_child + S.child_off;
-            double accD = 0.0, accR = 0.0;
-            for (int c = 0; c < (int)S.nchild; ++c) {
-              accD += CD[chn[c]];
-              accR += CR[chn[c]];
-            }
-            int x = nd[0];
-            for (int j = 0; j < (int)S.len; ++j) {
-              const int xn = j + 1 < (int)S.len ? nd[j + 1] : x;
-              const double di = (D[x] + DS[x]) + accD, ri = (R[x] + (V[x] + RS[x])) + accR;
-              const double a = A[x], b = B[x];
-              const double rinv = rcp_chain(di);
-              const double f = a * rinv;
-              D[x] = b * rinv;  // back-substitution multiplier
-              R[x] = ri * rinv;
-              accD = -(f * b);
-              accR = -(f * ri);
-              if (j + 1 == (int)S.len) {
-                CD[x] = accD;
-                CR[x] = accR;
-              }
-              x = xn;
-            }
-          }
-          __syncthreads();
-        }
-        if (tid == 0) {
-          const uint16_t *__restrict__ chn = M.cseg_child + cc.root_child_off;
-          double accD = 0.0, accR = 0.0;
-          for (int c = 0; c < cc.root_nchild; ++c) {
-            accD += CD[chn[c]];
-            accR += CR[chn[c]];
-          }
-          R[0] = ((R[0] + (V[0] + RS[0])) + accR) * rcp_fast((D[0] + DS[0]) + accD);
-        }
-        __syncthreads();
-        for (int L = cc.n_lev - 1; L >= 0; --L) {
-          const int s1 = lvl[L + 1];
-          for (int sg = lvl[L] + tid; sg < s1; sg += NT) {
-            const CellSeg S = segs[sg];
-            const uint16_t *__restrict__ nd = M.cseg_nodes + S.node_off;
-            double vp = R[S.par];
-            for (int j = (int)S.len - 1; j >= 0; --j) {
-              const int x = nd[j];
-              vp = fma(-D[x], vp, R[x]);
-              R[x] = vp;
-            }
-          }
-          __syncthreads();
-        }
-      }
+      CN_CT(2);
+      cell_solve<NT>(cc, segs, lvl, child, A, B, D, R, CD, CR, n, st, SW, tid);
+      CN_CT(3);
       // ---- voltage update, threshold at the root (L66, L68), probes -------------------------------
       for (int i = tid; i < n; i += NT) V[i] = R[i];
       if (tid == 0) {
-        const bool above = R[0] > thr;
+        const bool above = R[n - 1] > thr;
         if (above && !flag) {
           const unsigned long long pos = atomicAdd(M.n_sp, 1ull);
           if ((int64_t)pos < M.sp_cap) {
@@ -271,36 +335,38 @@ __global__ void __launch_bounds__(NT)
           for (int p = M.wp_first[g] + tid; p < M.wp_first[g + 1]; p += NT)
             M.trace[row * M.n_probe + M.wp_col[p]] = R[M.wp_pos[p]];
       }
+      CN_CT(4);
       // ---- nrn_state with the new v (L67), tables in description order -----------------------------
       for (int t = 0; t < M.n_table; ++t) {
         const DTable &T = M.tab[t];
-        if (T.is_point || (T.n_state == 0 && T.type != T_CADYN)) continue;
-        const int cnt = T.cls_cnt[gi.cls];
-        if (cnt == 0) continue;
-        double *par[CN_MAX_PARAM], *st[CN_MAX_STATE];
+        const int cnt = cnt_s[t];
+        if (cnt == 0 || (T.n_state == 0 && T.type != T_CADYN)) continue;
+        double *par[CN_MAX_PARAM], *sta[CN_MAX_STATE];
         double *p = MB + cc.mech_off[t];
 #pragma unroll
         for (int j = 0; j < CN_MAX_PARAM; ++j) par[j] = p + (j < T.n_param ? j : 0) * cnt;
 #pragma unroll
-        for (int j = 0; j < CN_MAX_STATE; ++j) st[j] = p + (T.n_param + (j < T.n_state ? j : 0)) * cnt;
-        state_distributed(T, par, st, 0, cnt, gv, M.dist_nodes + T.cls_nodeoff[gi.cls], R, CAI, I,
-                          tid, dt, M.q10, NT);
+        for (int j = 0; j < CN_MAX_STATE; ++j) sta[j] = p + (T.n_param + (j < T.n_state ? j : 0)) * cnt;
+        state_distributed(T, par, sta, 0, cnt, gv, dist + cc.dist_off[t], R, CAI, I, tid, dt, M.q10, NT);
         __syncthreads();  // (SK reads the cai that the cai dynamics of an earlier table wrote)
       }
       __syncthreads();
+      CN_CT(5);
     }
 
     // ---- store the cell -----------------------------------------------------------------------------
-    for (int i = tid; i < n; i += NT) {
-      const int64_t q = ab + noff[i];
-      M.v[q] = V[i];
-      if (CAI) M.cai[q] = CAI[i];
+    {
+      const int32_t *__restrict__ pno = M.cplan_noff + cc.noff_off;
+      for (int i = tid; i < n; i += NT) {
+        const int64_t q = ab + pno[i];
+        M.v[q] = V[i];
+        if (CAI) M.cai[q] = CAI[i];
+      }
     }
     for (int t = 0; t < M.n_table; ++t) {
       const DTable &T = M.tab[t];
-      if (T.is_point || T.n_state == 0) continue;
-      const int cnt = T.cls_cnt[gi.cls];
-      if (cnt == 0) continue;
+      const int cnt = cnt_s[t];
+      if (cnt == 0 || T.n_state == 0) continue;
       const int64_t ib = T.grp_instbase[g];
       const double *src = MB + cc.mech_off[t] + (size_t)T.n_param * cnt;
       for (int j = 0; j < T.n_state; ++j, src += cnt)

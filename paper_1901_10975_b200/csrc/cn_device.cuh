@@ -121,21 +121,26 @@ enum { RK_ROOT = 0, RK_FWD = 1, RK_STORE = 2, RK_ADD = 3, RK_KIND = 3,
 // cell-window mode (cn_cell.cuh): where the copies of a class's mechanism tables sit in the CTA's
 // shared memory (doubles from the start of the mechanism block), and the size of the whole block
 struct CellClass {
-  int32_t mech_off[CN_MAX_TABLES];
+  int32_t mech_off[CN_MAX_TABLES];  // doubles from the start of the mechanism block
+  int32_t dist_off[CN_MAX_TABLES];  // first entry of the table's node positions in the plan's dist list
   int32_t mech_doubles;
-  // elimination plan (cn_finalize.hpp build_cell_segments): segments [seg_off, ...) sorted by
-  // level, lvl[lvl_off + L] = first segment of level L (relative to seg_off), n_lev + 1 entries;
-  // the children of the root
-  int32_t seg_off, n_lev, lvl_off, root_child_off, root_nchild;
+  // Elimination plan (cn_finalize.hpp build_cell_plan).  Every per-node array in shared memory is
+  // in PLAN ORDER: the nodes of a chain side by side in elimination order, chains sorted by level,
+  // the root last.  plan_noff[noff_off + p] = where node p lives in the schedule-ordered arrays
+  // in HBM.  Segments [seg_off, seg_off + n_seg); lvl[lvl_off + L] = first segment of level L
+  // (n_lev + 1 entries, relative); child positions from child_off (n_child entries, the root's
+  // children last: root_child_off relative to child_off); dist positions from dist_base (n_dist).
+  int32_t seg_off, n_seg, n_lev, lvl_off, child_off, n_child, root_child_off, root_nchild;
+  int32_t noff_off, dist_base, n_dist, pad;
 };
 
-// one unbranched chain of a cell: nodes[node_off .. node_off + len) in elimination order (distal
-// to proximal), the children of its first node (each the last node of an earlier segment), and
-// the parent of its last node
+// one unbranched chain of a cell in plan order: nodes first .. first + len - 1 (distal to
+// proximal), the positions of the children of its first node (each the last node of an earlier
+// chain; child_off relative to the class's child list), and the position of the parent of its
+// last node
 struct CellSeg {
-  uint32_t node_off, child_off;
-  uint16_t len, nchild;
-  uint32_t par;
+  uint16_t first, len, nchild, par;
+  uint32_t child_off, pad;
 };
 
 struct DModel {
@@ -199,8 +204,9 @@ struct DModel {
   int64_t *step_ctr;            // [0] step, [1] trace row that a replayed CUDA graph starts from
   const struct CellClass *ccls; // cell-window mode (cn_cell.cuh): shared-memory layout per class
   const struct CellSeg *cseg;   //   and elimination plan
-  const uint16_t *cseg_nodes, *cseg_child;
-  const int32_t *cseg_lvl;
+  const uint16_t *cseg_child, *cdist;
+  const int32_t *cseg_lvl, *cplan_noff;
+  uint32_t *cwin_smctr;         // [256] per-SM arrival counter (which warp of a CTA solves)
   double q10, dt, celsius;
   DTable tab[CN_MAX_TABLES];
 };
@@ -337,9 +343,10 @@ struct GroupView {
 // nodes[k] of cell c.  At most one instance per node and table, so plain read-modify-write.
 // par / st: the table's parameter and state arrays (T.param / T.state in HBM, or their copies in
 // shared memory); the `stride` threads lane, lane + stride, ... share the instances.
+template <class NodeT>
 __device__ __forceinline__ void cur_distributed(const DTable &T, double *const *par,
                                                 double *const *st, int64_t ib, int cnt,
-                                                const GroupView &gv, const int32_t *nodes,
+                                                const GroupView &gv, const NodeT *nodes,
                                                 double *D, double *R, double *I,
                                                 const double *v_g, int lane, int stride = 32) {
   const int G = gv.G, lgG = gv.lgG;
@@ -349,7 +356,7 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, double *const *
       const double ena = T.glob[0], ek = T.glob[1];
       for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         const double m = st[0][q], h = st[1][q], n = st[2][q];
         const double invc = par[4][q];
         const double gna = par[0][q] * m * m * m * h;
@@ -367,7 +374,7 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, double *const *
       const bool to_ica = T.glob[3] != 0.0;
       for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         const double g = par[0][q] * ipow(st[0][q], p) * ipow(st[1][q], qq);
         const double invc = par[1][q];
         D[slot] += g * invc;
@@ -380,7 +387,7 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, double *const *
       const double E = T.glob[0];
       for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         const double g = par[0][q] * st[0][q];
         const double invc = par[1][q];
         D[slot] += g * invc;
@@ -396,9 +403,10 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, double *const *
 // nrn_state with the new v (in R)
 // ------------------------------------------------------------------------------------------
 
+template <class NodeT>
 __device__ __forceinline__ void state_distributed(const DTable &T, double *const *par,
                                                   double *const *st, int64_t ib, int cnt,
-                                                  const GroupView &gv, const int32_t *nodes,
+                                                  const GroupView &gv, const NodeT *nodes,
                                                   const double *R, double *cai_g,
                                                   const double *I, int lane, double dt,
                                                   double q10, int stride = 32) {
@@ -409,7 +417,7 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
     case T_HH:
       for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         double sm = st[0][q], sh = st[1][q], sn = st[2][q];
         hh_advance(R[slot], q10 * dt, sm, sh, sn);
         st[0][q] = sm;
@@ -421,7 +429,7 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
       const int p = (int)T.glob[0], qq = (int)T.glob[1];
       for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         const double v = R[slot];
         double xinf, xtau;
         if (p > 0) {
@@ -438,7 +446,7 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
     case T_SK:
       for (int j = lane; j < tot; j += stride) {
         const int64_t q = ib + j;
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         double cai = cai_g[gv.gpos(slot)];
         if (cai < 1e-9) cai = 1e-9;
         const double zinf = 1.0 / (1.0 + pow(T.glob[1] / cai, T.glob[2]));
@@ -450,7 +458,7 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
       const double kappa = 1e4 * T.glob[0] / (2.0 * 96485.33212 * T.glob[1]);
       const double taud = T.glob[2], cmin = T.glob[3];
       for (int j = lane; j < tot; j += stride) {
-        const int slot = (nodes[j >> lgG] << lgG) + (j & (G - 1));
+        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
         const int64_t gp = gv.gpos(slot);
         const double y0 = cai_g[gp];
         cai_g[gp] = (y0 + dt * (-kappa * I[slot] + cmin / taud)) / (1.0 + dt / taud);

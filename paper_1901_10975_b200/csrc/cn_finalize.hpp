@@ -8,37 +8,43 @@
 // ---------------------------------------------------------------------------------------------
 
 // Elimination plan of the on-chip window kernel (cn_cell.cuh) for one class: the tree is cut into
-// SEGMENTS, maximal unbranched chains x0 -> parent(x0) -> ... -> xk (x0 a leaf or a branch point,
-// every later node with exactly one child); one thread eliminates a whole segment with the
-// contribution travelling in registers.  A segment may start once all segments that end at the
-// children of x0 are done: its LEVEL.  All segments of a level run side by side on the threads of
-// the CTA, one barrier per level; sibling contributions are summed by the parent's segment in a
-// fixed order (no atomics: runs are bit-reproducible).
-static void build_cell_segments(const cn_model *m, const HClass &K, CellClass &cc,
-                                std::vector<CellSeg> &segs, std::vector<uint16_t> &nodes,
-                                std::vector<uint16_t> &child, std::vector<int32_t> &lvl) {
+// CHAINS, maximal unbranched paths x0 -> parent(x0) -> ... -> xk (x0 a leaf or a branch point,
+// every later node with exactly one child); one thread eliminates a whole chain with the
+// contribution travelling in registers.  A chain may start once all chains that end at the
+// children of x0 are done: its LEVEL.  The chains of a level run side by side, one barrier per
+// level; sibling contributions are summed by the parent's chain in a fixed order.  PLAN ORDER:
+// chains sorted by level (longest first), the nodes of a chain side by side in elimination
+// order, the root last; `perm` maps a local node to its position.
+struct CellPlan {
+  std::vector<CellSeg> segs;
+  std::vector<uint16_t> child, dist;
+  std::vector<int32_t> lvl, noff;
+};
+
+static void build_cell_plan(const cn_model *m, const HClass &K, int kc, CellClass &cc, CellPlan &P,
+                            std::vector<uint16_t> &perm) {
   const int n = K.n;
   const int64_t f = m->cell_first[K.rep_cell];
-  std::vector<int32_t> par(n, -1), nch(n, 0);
-  std::vector<std::vector<uint16_t>> ch(n);
+  std::vector<int32_t> par(n, -1);
+  std::vector<std::vector<int>> ch(n);
   for (int i = 1; i < n; ++i) {
     par[i] = (int32_t)(m->parent[f + i] - f);
-    ch[par[i]].push_back((uint16_t)i);
+    ch[par[i]].push_back(i);
   }
-  struct Tmp { std::vector<uint16_t> nd; int level; int par; int x0; };
+  struct Tmp { std::vector<int> nd; int level, par, x0; };
   std::vector<Tmp> tmp;
-  std::vector<int> end_level(n, -1);  // level of the segment that ends at this node
-  for (int x = n - 1; x >= 1; --x) {
-    if (ch[x].size() == 1) continue;  // interior of a segment
+  std::vector<int> end_level(n, -1);  // level of the chain that ends at this node
+  for (int x = n - 1; x >= 1; --x) {  // (children carry larger indices than their parents)
+    if (ch[x].size() == 1) continue;  // interior of a chain
     Tmp t;
     t.x0 = x;
     t.level = 0;
-    for (uint16_t c : ch[x]) t.level = std::max(t.level, end_level[c] + 1);
+    for (int c : ch[x]) t.level = std::max(t.level, end_level[c] + 1);
     int cur = x;
-    t.nd.push_back((uint16_t)cur);
+    t.nd.push_back(cur);
     while (par[cur] != 0 && ch[par[cur]].size() == 1) {
       cur = par[cur];
-      t.nd.push_back((uint16_t)cur);
+      t.nd.push_back(cur);
     }
     t.par = par[cur];
     end_level[cur] = t.level;
@@ -48,30 +54,51 @@ static void build_cell_segments(const cn_model *m, const HClass &K, CellClass &c
     if (a.level != b.level) return a.level < b.level;
     return a.nd.size() > b.nd.size();
   });
+  perm.assign(n, 0);
+  int pos = 0;
+  for (const Tmp &t : tmp)
+    for (int x : t.nd) perm[x] = (uint16_t)pos++;
+  perm[0] = (uint16_t)(n - 1);
   int nlev = 0;
   for (const Tmp &t : tmp) nlev = std::max(nlev, t.level + 1);
-  cc.seg_off = (int32_t)segs.size();
+  cc.seg_off = (int32_t)P.segs.size();
+  cc.n_seg = (int32_t)tmp.size();
   cc.n_lev = nlev;
-  cc.lvl_off = (int32_t)lvl.size();
-  int li = 0;
+  cc.lvl_off = (int32_t)P.lvl.size();
+  cc.child_off = (int32_t)P.child.size();
+  size_t li = 0;
   for (int L = 0; L <= nlev; ++L) {
-    while (li < (int)tmp.size() && tmp[li].level < L) ++li;
-    lvl.push_back(li);
+    while (li < tmp.size() && tmp[li].level < L) ++li;
+    P.lvl.push_back((int32_t)li);
   }
   for (const Tmp &t : tmp) {
-    CellSeg sg;
-    sg.node_off = (uint32_t)nodes.size();
-    sg.child_off = (uint32_t)child.size();
+    CellSeg sg{};
+    sg.first = perm[t.nd[0]];
     sg.len = (uint16_t)t.nd.size();
     sg.nchild = (uint16_t)ch[t.x0].size();
-    sg.par = (uint32_t)t.par;
-    nodes.insert(nodes.end(), t.nd.begin(), t.nd.end());
-    child.insert(child.end(), ch[t.x0].begin(), ch[t.x0].end());
-    segs.push_back(sg);
+    sg.par = perm[t.par];
+    sg.child_off = (uint32_t)(P.child.size() - (size_t)cc.child_off);
+    for (int c : ch[t.x0]) P.child.push_back(perm[c]);
+    P.segs.push_back(sg);
   }
-  cc.root_child_off = (int32_t)child.size();
+  cc.root_child_off = (int32_t)(P.child.size() - (size_t)cc.child_off);
   cc.root_nchild = (int32_t)ch[0].size();
-  child.insert(child.end(), ch[0].begin(), ch[0].end());
+  for (int c : ch[0]) P.child.push_back(perm[c]);
+  cc.n_child = (int32_t)(P.child.size() - (size_t)cc.child_off);
+  // where a position lives in the schedule-ordered arrays in HBM
+  cc.noff_off = (int32_t)P.noff.size();
+  P.noff.resize(P.noff.size() + (size_t)n);
+  for (int x = 0; x < n; ++x) P.noff[(size_t)cc.noff_off + perm[x]] = K.node_off[x];
+  // node positions of the instances of every distributed table (instance order of the class)
+  cc.dist_base = (int32_t)P.dist.size();
+  for (size_t t = 0; t < m->tab.size(); ++t) {
+    const HTable &T = m->tab[t];
+    cc.dist_off[t] = (int32_t)(P.dist.size() - (size_t)cc.dist_base);
+    if (T.ti.point || T.type == CN_PAS) continue;
+    const int32_t *nodes = m->dist_nodes.data() + T.cls_nodeoff[kc];
+    for (int j = 0; j < T.cls_cnt[kc]; ++j) P.dist.push_back(perm[nodes[j]]);
+  }
+  cc.n_dist = (int32_t)(P.dist.size() - (size_t)cc.dist_base);
 }
 
 static int finalize(cn_model *m, double dt) {
@@ -582,9 +609,8 @@ static int finalize(cn_model *m, double dt) {
     if (wn < 2 && onchip != 1) ok = false;
     if (ok && m->win_ninst * wn * 8 > ((int64_t)4 << 30)) ok = false;
     std::vector<CellClass> ccls(m->cls.size());
-    std::vector<CellSeg> segs;
-    std::vector<uint16_t> seg_nodes, seg_child;
-    std::vector<int32_t> seg_lvl;
+    CellPlan plan;
+    std::vector<std::vector<uint16_t>> perm(m->cls.size());  // local node -> plan position
     size_t max_bytes = 0;
     if (ok) {
       for (size_t kc = 0; kc < m->cls.size(); ++kc) {
@@ -598,8 +624,11 @@ static int finalize(cn_model *m, double dt) {
         }
         ccls[kc].mech_doubles = off;
         if (K.count - K.tp.n_cells > 0) {
-          max_bytes = std::max(max_bytes, ((size_t)K.n * (9 + (K.needs_ica ? 1 : 0) + (m->any_cai ? 1 : 0)) + off) * 8);
-          build_cell_segments(m, K, ccls[kc], segs, seg_nodes, seg_child, seg_lvl);
+          CellClass &cc = ccls[kc];
+          build_cell_plan(m, K, (int)kc, cc, plan, perm[kc]);
+          const size_t plan_bytes = (size_t)cc.n_seg * sizeof(CellSeg) + (size_t)(cc.n_lev + 1) * 4 +
+                                    (size_t)(cc.n_child + cc.n_dist) * 2 + 16;
+          max_bytes = std::max(max_bytes, ((size_t)K.n * (9 + (K.needs_ica ? 1 : 0) + (m->any_cai ? 1 : 0)) + off) * 8 + plan_bytes);
         }
       }
       if (max_bytes > 220 * 1024) ok = false;
@@ -633,16 +662,27 @@ static int finalize(cn_model *m, double dt) {
       CellClass *dcc;
       rc = dev_upload(m, ccls, &dcc); if (rc != CN_OK) return rc;
       H.ccls = dcc;
-      CellSeg *dsg; uint16_t *dsn, *dsc; int32_t *dsl;
-      rc = dev_upload(m, segs, &dsg); if (rc != CN_OK) return rc;
-      rc = dev_upload(m, seg_nodes, &dsn); if (rc != CN_OK) return rc;
-      rc = dev_upload(m, seg_child, &dsc); if (rc != CN_OK) return rc;
-      rc = dev_upload(m, seg_lvl, &dsl); if (rc != CN_OK) return rc;
-      H.cseg = dsg; H.cseg_nodes = dsn; H.cseg_child = dsc; H.cseg_lvl = dsl;
+      CellSeg *dsg; uint16_t *dsc, *dsd; int32_t *dsl, *dno;
+      rc = dev_upload(m, plan.segs, &dsg); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, plan.child, &dsc); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, plan.dist, &dsd); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, plan.lvl, &dsl); if (rc != CN_OK) return rc;
+      rc = dev_upload(m, plan.noff, &dno); if (rc != CN_OK) return rc;
+      H.cseg = dsg; H.cseg_child = dsc; H.cdist = dsd; H.cseg_lvl = dsl; H.cplan_noff = dno;
+      m->cwin_perm = perm;
+      rc = dev_alloc(m, 256, &H.cwin_smctr); if (rc != CN_OK) return rc;
       for (int t = 0; t < nt; ++t) {
         HTable &T = m->tab[t];
         if (!T.ti.point) continue;
-        rc = dev_upload(m, T.pp_local, &T.d_pp_local); if (rc != CN_OK) return rc;
+        // the node of every instance as a plan position of its cell's class
+        uvec<int32_t> ppos((size_t)T.n);
+        par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+          for (int64_t i = i0; i < i1; ++i) {
+            const int32_t c = cell_of_node[T.node[i]];
+            ppos[T.inst_pos[i]] = perm[m->cell_cls[c]][T.node[i] - m->cell_first[c]];
+          }
+        });
+        rc = dev_upload(m, ppos, &T.d_pp_local); if (rc != CN_OK) return rc;
         H.tab[t].pp_local = T.d_pp_local;
       }
       if (max_bytes > 48 * 1024) {
@@ -688,7 +728,7 @@ static int finalize(cn_model *m, double dt) {
         const int32_t q = fill[grp_of[j]]++;
         const int32_t c = (int32_t)(std::upper_bound(m->cell_first.begin(), m->cell_first.end(),
                                                      (int64_t)m->probe[j]) - m->cell_first.begin()) - 1;
-        pos[q] = m->probe[j] - m->cell_first[c];  // local node
+        pos[q] = m->cwin_perm[m->cell_cls[c]][m->probe[j] - m->cell_first[c]];  // plan position
         col[q] = (int32_t)j;
       }
       int32_t *df, *dc;

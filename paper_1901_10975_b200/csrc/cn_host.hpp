@@ -331,6 +331,7 @@ struct cn_model {
   bool cwindow = false;             // cell-window mode (cn_cell.cuh): one CTA keeps one cell on chip
   int cwin_grid = 0, cwin_threads = 256;  //   for a window of up to win_steps steps
   size_t cwin_smem = 0;
+  std::vector<std::vector<uint16_t>> cwin_perm;  // per class: local node -> plan position
   bool window = false;              // window mode: one launch of the interleaved kernel per
   int win_steps = 0;                //   up to win_steps steps (cn_tape.cuh)
   int64_t win_idx = 0;

@@ -188,7 +188,7 @@ static int build_layout(cn_model *m) {
         if (!T.ti.point && T.type != CN_PAS)
           d += (size_t)(T.ti.n_dev_param + T.ti.n_state) *
                (size_t)(T.cell_first[K.rep_cell + 1] - T.cell_first[K.rep_cell]);
-      max_bytes = std::max(max_bytes, d * 8);
+      max_bytes = std::max(max_bytes, d * 8 + (size_t)K.n * 24);  // (+ the elimination plan)
       max_n = std::max(max_n, K.n);
     }
     const int threads = max_n <= 128 ? 64 : max_n <= 320 ? 128 : 256;
