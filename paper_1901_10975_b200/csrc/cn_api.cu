@@ -524,6 +524,9 @@ extern "C" int cn_sync(cn_model *m) {
   CU(cudaStreamSynchronize(m->stream));
   int32_t ov = 0;
   CU(cudaMemcpy(&ov, m->d_overflow, sizeof(ov), cudaMemcpyDeviceToHost));
+  if (ov == 2)
+    return fail(CN_ERR_OVERFLOW, "a point-process conductance / current or event weight left the "
+                                 "range of the fixed-point sums (2^18 row-normalised units)");
   if (ov) return fail(CN_ERR_OVERFLOW, "spike buffer overflow (capacity %lld)", (long long)m->sp_cap);
   return CN_OK;
 }

@@ -38,11 +38,11 @@ __device__ long long g_cell_trace[16];
 #endif
 
 // the point processes of one cell for one step: events delivered at this step, conductance and
-// current into the node's row (several instances may sit on one node: shared-memory atomics; the
-// order of the additions is the only run-to-run freedom, as in pp_step_kernel), state decay
+// current into the node's fixed-point accumulators PD / PR (several instances may sit on one node:
+// shared-memory integer atomics, the sum does not depend on their order), state decay
 template <int NT>
 __device__ __forceinline__ void cell_point_processes(const DModel &M, const long long *ppq, int s,
-                                                     int64_t k, double *D, double *R,
+                                                     int64_t k, double *PD, double *PR,
                                                      const double *V, int tid) {
   const double t_mid = ((double)k + 0.5) * M.dt;
   for (int t = 0; t < M.n_table; ++t) {
@@ -54,8 +54,11 @@ __device__ __forceinline__ void cell_point_processes(const DModel &M, const long
       const int nd = T.pp_local[q];
       double w = 0.0;
       if (dl0 && T.type != T_ICLAMP) {
-        w = dl0[q];
-        if (w != 0.0) dl0[q] = 0.0;
+        const double raw = dl0[q];
+        if (fx_nonzero(raw)) {
+          w = fxw_get(raw, M.fxw_inv);
+          dl0[q] = 0.0;
+        }
       }
       switch (T.type) {
         case T_EXPSYN: {
@@ -63,8 +66,8 @@ __device__ __forceinline__ void cell_point_processes(const DModel &M, const long
           if (w != 0.0) gg += w;
           if (gg != 0.0) {
             const double gs = gg * T.param[2][q];
-            atomicAdd(&D[nd], gs);
-            atomicAdd(&R[nd], gs * T.param[1][q]);
+            fx_add(&PD[nd], gs, M.overflow);
+            fx_add(&PR[nd], gs * T.param[1][q], M.overflow);
             T.state[0][q] = decay(gg, T.param[0][q]);
           }
           break;
@@ -79,8 +82,8 @@ __device__ __forceinline__ void cell_point_processes(const DModel &M, const long
           if (a != 0.0 || b != 0.0) {
             const double gs = (b - a) * T.param[3][q];
             if (gs != 0.0) {
-              atomicAdd(&D[nd], gs);
-              atomicAdd(&R[nd], gs * T.param[2][q]);
+              fx_add(&PD[nd], gs, M.overflow);
+              fx_add(&PR[nd], gs * T.param[2][q], M.overflow);
             }
             T.state[0][q] = decay(a, T.param[0][q]);
             T.state[1][q] = decay(b, T.param[1][q]);
@@ -90,7 +93,7 @@ __device__ __forceinline__ void cell_point_processes(const DModel &M, const long
         case T_ICLAMP: {
           const double del = T.param[0][q];
           if (t_mid >= del && t_mid < del + T.param[1][q])
-            atomicAdd(&R[nd], T.param[2][q] * T.param[3][q]);
+            fx_add(&PR[nd], T.param[2][q] * T.param[3][q], M.overflow);
           break;
         }
         case T_AMPANMDA: {
@@ -105,8 +108,8 @@ __device__ __forceinline__ void cell_point_processes(const DModel &M, const long
           if (a0 != 0.0 || a1 != 0.0 || a2 != 0.0 || a3 != 0.0) {
             const double gs =
                 ((a1 - a0) + T.glob[4] * (a3 - a2) * mgblock(V[nd], T.glob[5])) * T.param[0][q];
-            atomicAdd(&D[nd], gs);
-            atomicAdd(&R[nd], gs * T.glob[6]);
+            fx_add(&PD[nd], gs, M.overflow);
+            fx_add(&PR[nd], gs * T.glob[6], M.overflow);
             T.state[0][q] = decay(a0, T.glob[9]);
             T.state[1][q] = decay(a1, T.glob[10]);
             T.state[2][q] = decay(a2, T.glob[11]);
@@ -274,6 +277,8 @@ __global__ void __launch_bounds__(NT)
       flag = M.flag[pc] != 0;
       thr = M.thr[pc];
     }
+    bool any_pp = false;
+    for (int t = 0; t < M.n_table; ++t) any_pp = any_pp || ppq_s[2 * t + 1] > ppq_s[2 * t];
     GroupView gv;
     gv.ab = 0;
     gv.noff = nullptr;
@@ -290,12 +295,21 @@ __global__ void __launch_bounds__(NT)
       for (int i = tid; i < n; i += NT) {
         D[i] = DS[i];
         R[i] = V[i] + RS[i];
+        CD[i] = 0.0;  // (the chains' contribution rows double as the point processes' accumulators)
+        CR[i] = 0.0;
         if (I) I[i] = 0.0;
       }
       __syncthreads();
       CN_CT(0);
-      cell_point_processes<NT>(M, ppq_s, s, k, D, R, V, tid);
-      __syncthreads();
+      if (any_pp) {
+        cell_point_processes<NT>(M, ppq_s, s, k, CD, CR, V, tid);
+        __syncthreads();
+        for (int i = tid; i < n; i += NT) {
+          D[i] += fx_get(CD[i]);
+          R[i] += fx_get(CR[i]);
+        }
+        __syncthreads();
+      }
       CN_CT(1);
       // ---- nrn_cur of the distributed mechanisms (one instance per node and table) ----------------
       for (int t = 0; t < M.n_table; ++t) {

@@ -208,6 +208,7 @@ struct DModel {
   const int32_t *cseg_lvl, *cplan_noff;
   uint32_t *cwin_smctr;         // [256] per-SM arrival counter (which warp of a CTA solves)
   double q10, dt, celsius;
+  double fxw_scale, fxw_inv;    // fixed-point scale of the per-step event-weight sums (window modes)
   DTable tab[CN_MAX_TABLES];
 };
 
@@ -236,6 +237,34 @@ __device__ __forceinline__ double rcp_chain(double x) {
   const double e = fma(-x, r, 1.0);
   const double t = fma(e, e, e);
   return fma(r, t, r);
+}
+
+// Sums that several threads add to in no fixed order -- conductance / current of the point
+// processes of a node, weights of the events that reach a synapse in one step -- are accumulated
+// as 64-bit FIXED-POINT integers (resolution 2^-44 = 5.7e-14 of the row-normalised unit, range
+// +-2^19): integer addition is associative, so the sum does not depend on the order in which the
+// atomics land and a run is bit-reproducible (SURVEY.md 7 "accumulation of point-process
+// currents"; PAPER.md L196 contention).  The slot is a double-sized word holding the integer; an
+// addend beyond +-2^18 raises the overflow flag (cn_sync: CN_ERR_OVERFLOW).
+#define CN_FX 17592186044416.0            // 2^44
+#define CN_FX_INV 5.684341886080802e-14   // 2^-44
+__device__ __forceinline__ void fx_add(double *slot, double val, int32_t *overflow) {
+  if (!(fabs(val) < 262144.0)) *overflow = 2;
+  atomicAdd(reinterpret_cast<unsigned long long *>(slot),
+            (unsigned long long)__double2ll_rn(val * CN_FX));
+}
+__device__ __forceinline__ double fx_get(double raw) {
+  return (double)__double_as_longlong(raw) * CN_FX_INV;
+}
+__device__ __forceinline__ bool fx_nonzero(double raw) { return __double_as_longlong(raw) != 0; }
+// The same for the event weights that reach a synapse in one step (window modes), with a scale the
+// host derives from the model: the largest sum of |weights| that can meet on one synapse fits 62
+// bits, so the sum cannot overflow and keeps every bit a double could hold for such weights.
+__device__ __forceinline__ void fxw_add(double *slot, double w, double scale) {
+  atomicAdd(reinterpret_cast<unsigned long long *>(slot), (unsigned long long)__double2ll_rn(w * scale));
+}
+__device__ __forceinline__ double fxw_get(double raw, double inv) {
+  return (double)__double_as_longlong(raw) * inv;
 }
 
 // exp(x) for |x| < 700 to ~1 ulp without the special-case handling of the library routine:
@@ -521,9 +550,9 @@ __global__ void __launch_bounds__(WPB * 32, WPB >= 8 ? 1 : 12 / WPB)
   auto take_pp = [&](int r, double &d, double &rr, double pd, double pr) {
     if (!has_pp || d > 0.0) return;
     d = -d;
-    if (pd != 0.0 || pr != 0.0) {
-      d += pd;
-      rr += pr;
+    if (fx_nonzero(pd) || fx_nonzero(pr)) {
+      d += fx_get(pd);
+      rr += fx_get(pr);
       pps[(size_t)r * 64] = 0.0;
       pps[(size_t)r * 64 + 32] = 0.0;
     }
@@ -803,8 +832,8 @@ __global__ void __launch_bounds__(128) deliver_window_kernel(const __grid_consta
       const int64_t d = M.nc_d[nc];
       if (d > d_hi) break;
       const DTable &T = M.tab[M.nc_tab[nc]];
-      atomicAdd(&M.win_deliv[(step + d - k0) * M.win_ninst + T.pp_goff + M.nc_inst[nc]],
-                M.nc_w[nc]);
+      fxw_add(&M.win_deliv[(step + d - k0) * M.win_ninst + T.pp_goff + M.nc_inst[nc]], M.nc_w[nc],
+              M.fxw_scale);
     }
   };
   for (int64_t i = i_lo + warp; i < (int64_t)ns; i += nwarp) deliver(M.sp_gid[i], M.sp_step[i]);
@@ -830,15 +859,15 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
         case T_EXPSYN: {
           double g = T.state[0][q];
           for (int s = 0; s < nsteps; ++s, rows += M.win_stride, dl += M.win_ninst) {
-            const double w = *dl;
+            const double w = fxw_get(*dl, M.fxw_inv);
             if (w != 0.0) {
               g += w;
               *dl = 0.0;
             }
             if (g != 0.0) {
               const double gs = g * T.param[2][q];
-              atomicAdd(rows, gs);
-              atomicAdd(rows + 32, gs * T.param[1][q]);
+              fx_add(rows, gs, M.overflow);
+              fx_add(rows + 32, gs * T.param[1][q], M.overflow);
               g = decay(g, T.param[0][q]);
             }
           }
@@ -848,7 +877,7 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
         case T_EXP2SYN: {
           double A = T.state[0][q], B = T.state[1][q];
           for (int s = 0; s < nsteps; ++s, rows += M.win_stride, dl += M.win_ninst) {
-            const double w = *dl;
+            const double w = fxw_get(*dl, M.fxw_inv);
             if (w != 0.0) {
               const double wf = w * T.param[4][q];
               A += wf;
@@ -858,8 +887,8 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
             if (A != 0.0 || B != 0.0) {
               const double gs = (B - A) * T.param[3][q];
               if (gs != 0.0) {
-                atomicAdd(rows, gs);
-                atomicAdd(rows + 32, gs * T.param[2][q]);
+                fx_add(rows, gs, M.overflow);
+                fx_add(rows + 32, gs * T.param[2][q], M.overflow);
               }
               A = decay(A, T.param[0][q]);
               B = decay(B, T.param[1][q]);
@@ -874,7 +903,7 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
           for (int s = 0; s < nsteps; ++s, rows += M.win_stride) {
             const double t_mid = ((double)(k0 + s) + 0.5) * dt;
             if (t_mid >= del && t_mid < del + dur)
-              atomicAdd(rows + 32, T.param[2][q] * T.param[3][q]);
+              fx_add(rows + 32, T.param[2][q] * T.param[3][q], M.overflow);
           }
           break;
         }

@@ -542,6 +542,20 @@ static int finalize(cn_model *m, double dt) {
       ninst[j] = m->tab[m->nc_tgt_mech[i]].inst_pos[m->nc_tgt_inst[i]];
       nw[j] = m->nc_w[i];
     }
+    {  // fixed-point scale of the event-weight sums: the largest sum of |w| on one synapse < 2^62
+      std::vector<int64_t> toff(m->tab.size() + 1, 0);
+      for (size_t t = 0; t < m->tab.size(); ++t) toff[t + 1] = toff[t] + m->tab[t].n;
+      std::vector<double> wsum((size_t)toff.back(), 0.0);
+      for (int64_t i = 0; i < m->n_netcon; ++i)
+        wsum[(size_t)(toff[m->nc_tgt_mech[i]] + m->nc_tgt_inst[i])] += std::fabs(m->nc_w[i]);
+      double wmax = 1e-300;
+      for (double x : wsum) wmax = std::max(wmax, x);
+      int ex = 0;
+      std::frexp(wmax, &ex);  // wmax < 2^ex
+      ex = std::max(-400, std::min(400, ex));
+      H.fxw_scale = std::ldexp(1.0, 62 - ex);
+      H.fxw_inv = std::ldexp(1.0, ex - 62);
+    }
     int64_t *p64; int32_t *p32; double *pd;
     UP(src_first, p64); H.src_first = p64;
     UP(nd, p32); H.nc_d = p32;

@@ -406,34 +406,42 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         }
         if (e.z & (1u << 20)) {  // (multiplier, reduced rhs) to the warp's tensor-memory slots
           uint32_t ta = tm_warp + ((uint32_t)tk.tm_base + (e.z & 1023u)) * 4u;
+          // (the operands of the next node are fetched while the current one is on the dependent
+          // chain: pivot -> reciprocal -> contribution = one DADD, MUFU + 3 DFMA, one DMUL)
+          double a = CN_RD(rb, 0), b = CN_RD(rb, 1), d = CN_RD(rb, 2), vr = CN_RD(rb, 4) + CN_RD(rb, 3);
 #pragma unroll 1
           for (int q = (int)((e.x >> 16) & 255u); q; --q) {
-            const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
-            const double D = CN_RD(rb, 2) + accD;
-            const double R = (CN_RD(rb, 4) + CN_RD(rb, 3)) + accR;
-            const double rinv = rcp_fast(D);
-            const double f = a * rinv;
+            const unsigned char *rn = rb + (q > 1 ? 5 * 256 : 0);
+            const double a1 = CN_RD(rn, 0), b1 = CN_RD(rn, 1), d1 = CN_RD(rn, 2),
+                         vr1 = CN_RD(rn, 4) + CN_RD(rn, 3);
+            const double D = d + accD, R = vr + accR;
+            const double ab = a * b, aR = a * R;
+            const double rinv = rcp_chain(D);
             tm_store2(ta, b * rinv, R * rinv);
-            accD = -(f * b);
-            accR = -(f * R);
-            rb += 5 * 256;
+            accD = -(ab * rinv);
+            accR = -(aR * rinv);
+            rb = rn;
+            a = a1; b = b1; d = d1; vr = vr1;
             ta += 4;
           }
           continue;
         }
         double *srow = sys_l + (e.z & 1023u) * 64u;
+        double a = CN_RD(rb, 0), b = CN_RD(rb, 1), d = CN_RD(rb, 2), vr = CN_RD(rb, 4) + CN_RD(rb, 3);
 #pragma unroll 1
         for (int q = (int)((e.x >> 16) & 255u); q; --q) {
-          const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
-          const double D = CN_RD(rb, 2) + accD;
-          const double R = (CN_RD(rb, 4) + CN_RD(rb, 3)) + accR;
-          const double rinv = rcp_fast(D);
-          const double f = a * rinv;
+          const unsigned char *rn = rb + (q > 1 ? 5 * 256 : 0);
+          const double a1 = CN_RD(rn, 0), b1 = CN_RD(rn, 1), d1 = CN_RD(rn, 2),
+                       vr1 = CN_RD(rn, 4) + CN_RD(rn, 3);
+          const double D = d + accD, R = vr + accR;
+          const double ab = a * b, aR = a * R;
+          const double rinv = rcp_chain(D);
           srow[0] = b * rinv;
           srow[32] = R * rinv;
-          accD = -(f * b);
-          accR = -(f * R);
-          rb += 5 * 256;
+          accD = -(ab * rinv);
+          accR = -(aR * rinv);
+          rb = rn;
+          a = a1; b = b1; d = d1; vr = vr1;
           srow += 64;
         }
         continue;
@@ -474,28 +482,28 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         }
         if (fl & RF_HAS_PP) {  // conductance / current of the point processes
           if (window) {  // (pp_window_kernel: this step's block of win_rows, prefetched)
-            D += ppd;
-            R += ppr;
+            D += fx_get(ppd);
+            R += fx_get(ppr);
             wrow += 64;
             ppd = __ldcg(wrow);
             ppr = __ldcg(wrow + 32);
           } else {  // (pp_step_kernel: the two dynamic rows of the record, cleared after use)
-            const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);
-            D += pd;
-            R += pr;
-            if (pd != 0.0 || pr != 0.0) {
+            const double pd = CN_RD(rb, 5), pr = CN_RD(rb, 6);  // (fixed-point sums)
+            D += fx_get(pd);
+            R += fx_get(pr);
+            if (fx_nonzero(pd) || fx_nonzero(pr)) {
               double *trec = tape_l + (e.w & 0xFFFFu) * 32u;
               trec[5 * 32] = 0.0;
               trec[6 * 32] = 0.0;
             }
           }
         }
-        const double rinv = rcp_fast(D);
+        const double ab = a * b, aR = a * R;
+        const double rinv = rcp_chain(D);
         const uint32_t kind = fl & RK_KIND;
         double mult = 0.0;
         if (kind != RK_ROOT) {
-          const double f = a * rinv;
-          const double cD = -(f * b), cR = -(f * R);
+          const double cD = -(ab * rinv), cR = -(aR * rinv);
           mult = b * rinv;  // back-substitution multiplier
           if (kind == RK_FWD) {
             accD = cD;
@@ -701,8 +709,8 @@ __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DM
           const double g = T.state[0][q];
           if (g != 0.0) {
             const double gs = g * T.param[2][q];
-            atomicAdd(&tape[tgt[q]], gs);
-            atomicAdd(&tape[tgt[q] + 32], gs * T.param[1][q]);
+            fx_add(&tape[tgt[q]], gs, M.overflow);
+            fx_add(&tape[tgt[q] + 32], gs * T.param[1][q], M.overflow);
             T.state[0][q] = decay(g, T.param[0][q]);
           }
         }
@@ -713,8 +721,8 @@ __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DM
           if (A != 0.0 || B != 0.0) {
             const double gs = (B - A) * T.param[3][q];
             if (gs != 0.0) {
-              atomicAdd(&tape[tgt[q]], gs);
-              atomicAdd(&tape[tgt[q] + 32], gs * T.param[2][q]);
+              fx_add(&tape[tgt[q]], gs, M.overflow);
+              fx_add(&tape[tgt[q] + 32], gs * T.param[2][q], M.overflow);
             }
             T.state[0][q] = decay(A, T.param[0][q]);
             T.state[1][q] = decay(B, T.param[1][q]);
@@ -725,7 +733,7 @@ __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DM
         for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
           const double del = T.param[0][q];
           if (t_mid >= del && t_mid < del + T.param[1][q])
-            atomicAdd(&tape[tgt[q] + 32], T.param[2][q] * T.param[3][q]);
+            fx_add(&tape[tgt[q] + 32], T.param[2][q] * T.param[3][q], M.overflow);
         }
         break;
       case T_AMPANMDA:
@@ -737,8 +745,8 @@ __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DM
             const double v = COOP ? M.v[(size_t)(tgt[q] >> 6) * 32 + (tgt[q] & 31u)] : tape[tgt[q] - 32];
             const double gs =
                 ((a1 - a0) + T.glob[4] * (a3 - a2) * mgblock(v, T.glob[5])) * T.param[0][q];
-            atomicAdd(&tape[tgt[q]], gs);
-            atomicAdd(&tape[tgt[q] + 32], gs * T.glob[6]);
+            fx_add(&tape[tgt[q]], gs, M.overflow);
+            fx_add(&tape[tgt[q] + 32], gs * T.glob[6], M.overflow);
             T.state[0][q] = decay(a0, T.glob[9]);
             T.state[1][q] = decay(a1, T.glob[10]);
             T.state[2][q] = decay(a2, T.glob[11]);
@@ -750,8 +758,8 @@ __global__ void __launch_bounds__(256) pp_step_kernel(const __grid_constant__ DM
                    // before any voltage of step k is written)
         for (int64_t q = (COOP ? 0 : T.pp_tape_begin) + tid; q < (COOP ? T.pp_tape_begin : T.pp_tape_end); q += nth) {
           const double gs = T.param[0][q];
-          atomicAdd(&tape[tgt[q]], gs);
-          atomicAdd(&tape[tgt[q] + 32], gs * M.v[(int64_t)T.param[1][q]]);
+          fx_add(&tape[tgt[q]], gs, M.overflow);
+          fx_add(&tape[tgt[q] + 32], gs * M.v[(int64_t)T.param[1][q]], M.overflow);
         }
         break;
       default: break;

@@ -285,6 +285,24 @@ def test_chunked_run_equals_one_shot(cn, strategy):
     assert [list(x) for x in a.get_spikes()] == [list(x) for x in b.get_spikes()]
 
 
+@pytest.mark.parametrize("which", ["config3", "config5"])
+def test_runs_with_many_synapses_per_node_are_bit_reproducible(cn, strategy, which):
+    """Several synapses per node and several events per step: the conductance / current of a
+    node's point processes is summed in fixed point, so the order in which the atomics land
+    cannot change a bit."""
+    desc = W.config3(n_cell=140, syn_per_cell=300) if which == "config3" else \
+        W.config5(n_cell=110, syn_per_cell=400)
+    r = []
+    for _ in range(3):
+        m = cn.Model(desc)
+        m.run(15.0, DT)
+        r.append((m.get_v(), m.get_spikes(), m.get_state(len(desc["mechs"]) - 2, 1)))
+    for x in r[1:]:
+        assert np.array_equal(r[0][0], x[0]) and np.array_equal(r[0][2], x[2])
+        assert [list(a) for a in r[0][1]] == [list(a) for a in x[1]]
+    assert len(r[0][1][0]) >= 5
+
+
 def test_run_is_deterministic(cn, strategy):
     desc = W.config4(n_cell=128, n_types=4)
     r = []
