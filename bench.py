@@ -163,7 +163,8 @@ def write_traffic(csv_path):
     hdr = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
     names, units = rows[hdr], rows[hdr + 1]
     col = {n: j for j, n in enumerate(names)}
-    scale = {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    scale = {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12,
+             "ns": 1, "us": 1e3, "ms": 1e6, "s": 1e9}
 
     def val(r, name):
         return float(r[col[name]].replace(",", "")) * scale[units[col[name]]]
@@ -172,19 +173,20 @@ def write_traffic(csv_path):
     for r in rows[hdr + 2:]:
         if len(r) <= col["dram__bytes_read.sum"] or not r[col["Kernel Name"]]:
             continue
-        k = r[col["Kernel Name"]].split("(")[0].replace("cn::", "").split("<")[0]
+        k = r[col["Kernel Name"]].split("(")[0].replace("cn::", "").replace("void ", "").split("<")[0]
         e = out.setdefault(k, {"launches": 0, "dram_bytes": 0.0, "duration_ns": 0.0})
         e["launches"] += 1
         e["dram_bytes"] += val(r, "dram__bytes_read.sum") + val(r, "dram__bytes_write.sum")
         if "gpu__time_duration.sum" in col:
-            e["duration_ns"] += float(r[col["gpu__time_duration.sum"]].replace(",", ""))
+            e["duration_ns"] += val(r, "gpu__time_duration.sum")
     for e in out.values():
         e["dram_bytes_per_launch"] = e.pop("dram_bytes") / e["launches"]
         e["duration_ns_per_launch"] = e.pop("duration_ns") / e["launches"]
     prev = json.loads(TRAFFIC_FILE.read_text()) if TRAFFIC_FILE.exists() else {}
-    prev[Path(csv_path).stem] = {"source_sha": source_sha(), "kernels": out}
+    key = Path(csv_path).stem.replace("_full", "")      # config4_full.csv -> "config4"
+    prev[key] = {"source_sha": source_sha(), "from": Path(csv_path).name, "kernels": out}
     TRAFFIC_FILE.write_text(json.dumps(prev, indent=1, sort_keys=True) + "\n")
-    print(json.dumps(prev[Path(csv_path).stem]))
+    print(json.dumps(prev[key]))
 
 
 def measured_traffic(key, kernel):

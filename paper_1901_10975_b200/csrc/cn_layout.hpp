@@ -387,8 +387,17 @@ static int build_layout(cn_model *m) {
     // several cells per warp only while that still leaves every SM its 8 warps: below that, more
     // lanes per cell (fewer rounds, fewer mechanism passes per warp) beat more cells per warp
     // (config 2, 256 cells x 601 nodes: 94.9 us per dt with G = 1, 110.7 with G = 2)
+    // ... and never for cells that carry distributed mechanisms on most of their nodes (config 5:
+    // Ih on every dendritic node): their mechanism loops want all 32 lanes and the occupancy that
+    // the smaller system leaves (config 5 at quarter scale: step kernel 288 us per dt with one cell
+    // per warp, 362 with two)
+    int64_t mech_inst = 0;
+    for (const HTable &T : m->tab)
+      if (!T.ti.point && T.type != CN_PAS)
+        mech_inst += T.cell_first[K.rep_cell + 1] - T.cell_first[K.rep_cell];
+    const int class_max_g = mech_inst >= K.n ? 1 : max_g;
     int G = 1;
-    while (G * 2 <= max_g && G * 2 <= ccount && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap &&
+    while (G * 2 <= class_max_g && G * 2 <= ccount && (int64_t)K.n * arrays * 8 * G * 2 <= smem_cap &&
            coop_cells / (G * 2) >= 148 * 8)
       G *= 2;
     if (force_g > 0) {
