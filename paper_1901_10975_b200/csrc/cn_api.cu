@@ -359,8 +359,7 @@ static int run_steps(cn_model *m, int64_t K) {
     for (int64_t s = 0; s < K;) {
       const int n = (int)std::min<int64_t>(m->win_steps, K - s);
       const int64_t k = m->k + s;
-      if (m->win_stride > 0)
-        CU(cudaMemsetAsync(m->hm.win_rows, 0, (size_t)m->win_stride * n * sizeof(double), m->stream));
+      // (win_rows needs no clearing: the interleaved kernel zeroes every row it consumes)
       CU(cudaMemsetAsync(m->hm.win_done, 0, (size_t)ntg * sizeof(int32_t), m->stream));
       CU(cudaMemsetAsync(m->hm.win_ticket, 0, sizeof(uint32_t), m->stream));
       if (m->n_netcon > 0) {

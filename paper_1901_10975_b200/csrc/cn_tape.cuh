@@ -484,6 +484,10 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           if (window) {  // (pp_window_kernel: this step's block of win_rows, prefetched)
             D += fx_get(ppd);
             R += fx_get(ppr);
+            if (fx_nonzero(ppd) || fx_nonzero(ppr)) {  // consumed: the row is zero for the next window
+              __stcg(const_cast<double *>(wrow), 0.0);  // (no memset of the whole buffer per window)
+              __stcg(const_cast<double *>(wrow) + 32, 0.0);
+            }
             wrow += 64;
             ppd = __ldcg(wrow);
             ppr = __ldcg(wrow + 32);
