@@ -183,7 +183,7 @@ def write_traffic(csv_path):
         e["dram_bytes_per_launch"] = e.pop("dram_bytes") / e["launches"]
         e["duration_ns_per_launch"] = e.pop("duration_ns") / e["launches"]
     prev = json.loads(TRAFFIC_FILE.read_text()) if TRAFFIC_FILE.exists() else {}
-    key = Path(csv_path).stem.replace("_full", "")      # config4_full.csv -> "config4"
+    key = Path(csv_path).stem.replace("_full", "").replace("r02_", "")   # r02_config4_full.csv -> "config4"
     prev[key] = {"source_sha": source_sha(), "from": Path(csv_path).name, "kernels": out}
     TRAFFIC_FILE.write_text(json.dumps(prev, indent=1, sort_keys=True) + "\n")
     print(json.dumps(prev[key]))
