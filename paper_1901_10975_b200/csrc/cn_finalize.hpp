@@ -543,8 +543,9 @@ static int finalize(cn_model *m, double dt) {
       nw[j] = m->nc_w[i];
     }
     {  // fixed-point scale of the event-weight sums: the largest sum of |w| on one synapse < 2^62
-      std::vector<int64_t> toff(m->tab.size() + 1, 0);
-      for (size_t t = 0; t < m->tab.size(); ++t) toff[t + 1] = toff[t] + m->tab[t].n;
+      std::vector<int64_t> toff(m->tab.size() + 1, 0);  // (point tables only: the others get no events)
+      for (size_t t = 0; t < m->tab.size(); ++t)
+        toff[t + 1] = toff[t] + (m->tab[t].ti.point ? m->tab[t].n : 0);
       std::vector<double> wsum((size_t)toff.back(), 0.0);
       for (int64_t i = 0; i < m->n_netcon; ++i)
         wsum[(size_t)(toff[m->nc_tgt_mech[i]] + m->nc_tgt_inst[i])] += std::fabs(m->nc_w[i]);
