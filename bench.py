@@ -150,8 +150,11 @@ def flops_per_dt(desc):
 
 
 def source_sha():
+    """Hash of what decides the kernels' DRAM traffic: the device code and the layout / program
+    compilers (not the host-side set-up and ABI code)."""
     h = hashlib.sha256()
-    for f in sorted((ROOT / "paper_1901_10975_b200" / "csrc").iterdir()):
+    csrc = ROOT / "paper_1901_10975_b200" / "csrc"
+    for f in sorted(list(csrc.glob("*.cuh")) + [csrc / "cn_layout.hpp", csrc / "cn_tape_program.hpp"]):
         h.update(f.name.encode())
         h.update(f.read_bytes())
     return h.hexdigest()[:16]
