@@ -46,7 +46,7 @@ def test_options_are_per_model_and_validated(monkeypatch):
     monkeypatch.setenv("CN_TAPE", "0")          # ambient state steers nothing
     monkeypatch.setenv("CN_TAPE_W", "4")
     info = cn.Model(d).layout_info()
-    assert info == before and info["tape_warps"] == 8
+    assert info == before and info["tape_warps"] == 12    # (small model: 12 warps per group)
     for bad in ("bogus=1", "tape", "tape=", "tape=yes", "=1"):
         with pytest.raises(cn.CnError) as e:
             cn.Model(d, options=bad)

@@ -20,10 +20,10 @@ def _gpu(need_gpu):
     pass
 
 
-@pytest.fixture(params=["coop", "cell", "tape", "tape-step", "tape-w1", "tape-w4"])
+@pytest.fixture(params=["coop", "cell", "tape", "tape-step", "tape-w1", "tape-w4", "tape-w8"])
 def strategy(request, opts):
     """Both kernels on the same inputs: warp-cooperative groups, or every cell on the interleaved
-    (tape) kernel, ragged groups included (CN_TAPE_MIN_GROUP=1), with 8 (default), 1 or 4 warps
+    (tape) kernel, ragged groups included (tape_min_group=1), with 12 (default for small models), 8, 1 or 4 warps
     (subtree tasks) per group of 32 cells.  The interleaved kernel runs in window mode where the
     model allows it (the probes are then recorded by the kernel itself); "tape-step" forces one
     launch sequence per dt."""
@@ -33,7 +33,7 @@ def strategy(request, opts):
         if request.param == "tape-step":
             opts["tape_window"] = 0
         if "-w" in request.param:
-            opts["tape_w"] = int(request.param[-1])
+            opts["tape_w"] = int(request.param.split("-w")[1])
     else:
         # the warp-cooperative layout: one launch sequence per dt (replayed from a CUDA graph), or
         # "cell": the on-chip window kernel, one CTA per cell for a whole min-delay window

@@ -29,7 +29,7 @@ def test_compiles_for_every_warp_count(cn, warps):
 @pytest.mark.parametrize("s,ch", [(2, 9), (2, 15), (3, 10), (4, 9), (2, 40)])
 def test_ring_geometries(cn, s, ch):
     desc = W.config4(n_cell=64, n_types=2)
-    info = _model(cn, desc, tape_s=s, tape_ch=ch)
+    info = _model(cn, desc, tape_s=s, tape_ch=ch, tape_w=8)
     assert info["n_tape_group"] == 2
 
 
