@@ -89,6 +89,24 @@ def test_unique_topologies_one_cell_per_warp(cn, strategy):
     check(o, g, min_spikes=5)
 
 
+@pytest.mark.parametrize("mech", ["pas", "hh"])
+def test_random_trees_of_every_size(cn, strategy, mech):
+    """Fuzz of the tree handling of every kernel: 48 unique random topologies from single nodes to
+    330 nodes (up to 3 children per node: stars, long unbranched chains, a root with one child),
+    passive dendrites or HH on every node, plus degenerate hand-made shapes (a pure chain of 300
+    nodes, a star of 60 leaves on the soma)."""
+    a = W.random_tree_cells(48, 1, 330, stream="fuzz-" + mech, mech=mech, weight=0.3, amp=3.0)
+    chain = W.random_tree_cells(2, 300, 300, stream="fuzz-chain", mech=mech, identical=True, weight=0.3, amp=3.0)
+    chain["parent"] = np.concatenate([np.arange(-1, 299), 300 + np.arange(-1, 299)]).astype(np.int32)
+    chain["parent"][300] = -1
+    star = W.random_tree_cells(2, 61, 61, stream="fuzz-star", mech=mech, identical=True, weight=0.3, amp=3.0)
+    star["parent"] = np.concatenate([[-1], np.zeros(60), [-1], np.full(60, 61)]).astype(np.int32)
+    desc = W.concat_models([a, chain, star])
+    o, g = run_both(cn, desc, 25.0)
+    assert g.layout_info()["n_class"] == 50
+    check(o, g, min_spikes=20)
+
+
 def test_identical_random_cells_grouped(cn, strategy, opts):
     desc = W.random_tree_cells(11, 77, 77, stream="gpu-i", identical=True, weight=0.2, amp=2.0)
     if strategy == "coop":      # (a model this small gets one cell per warp unless told otherwise)
