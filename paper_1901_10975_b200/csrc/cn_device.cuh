@@ -401,14 +401,32 @@ __device__ __forceinline__ void cur_distributed(const DTable &T, double *const *
       const int p = (int)T.glob[0], qq = (int)T.glob[1];
       const double E = T.glob[2];
       const bool to_ica = T.glob[3] != 0.0;
-      for (int j = lane; j < tot; j += stride) {
-        const int64_t q = ib + j;
-        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
-        const double g = par[0][q] * ipow(st[0][q], p) * ipow(st[1][q], qq);
-        const double invc = par[1][q];
-        D[slot] += g * invc;
-        R[slot] += g * E * invc;
-        if (to_ica) I[slot] += g * (v_g[gv.gpos(slot)] - E);  // ica uses v_old (still in HBM)
+      // four instances per lane and pass with every load issued before the first use (clamped
+      // indices, no branches around the loads): when parameters and states stream from HBM the
+      // loop is bound by the latency of these loads (config 5)
+      for (int j0 = lane; j0 < tot; j0 += 4 * stride) {
+        double gb[4], sm[4], sh[4], ic[4];
+        int sl[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int j = min(j0 + u * stride, tot - 1);
+          const int64_t q = ib + j;
+          gb[u] = par[0][q];
+          sm[u] = st[0][q];
+          sh[u] = st[1][q];
+          ic[u] = par[1][q];
+          sl[u] = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (j0 + u * stride < tot) {
+            const int slot = sl[u];
+            const double g = gb[u] * ipow(sm[u], p) * ipow(sh[u], qq);
+            D[slot] += g * ic[u];
+            R[slot] += g * E * ic[u];
+            if (to_ica) I[slot] += g * (v_g[gv.gpos(slot)] - E);  // ica uses v_old (still in HBM)
+          }
+        }
       }
       break;
     }
@@ -456,18 +474,31 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
       break;
     case T_HHFORM: {
       const int p = (int)T.glob[0], qq = (int)T.glob[1];
-      for (int j = lane; j < tot; j += stride) {
-        const int64_t q = ib + j;
-        const int slot = ((int)nodes[j >> lgG] << lgG) + (j & (G - 1));
-        const double v = R[slot];
-        double xinf, xtau;
-        if (p > 0) {
-          hhform_gate(v, T.glob + 4, xinf, xtau);
-          st[0][q] = cnexp(st[0][q], xinf, xtau, dt);
+      for (int j0 = lane; j0 < tot; j0 += 2 * stride) {  // (two instances per pass: loads first)
+        double sm[2], sh[2], vv[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int j = min(j0 + u * stride, tot - 1);
+          const int64_t q = ib + j;
+          sm[u] = st[0][q];
+          sh[u] = st[1][q];
+          vv[u] = R[((int)nodes[j >> lgG] << lgG) + (j & (G - 1))];
         }
-        if (qq > 0) {
-          hhform_gate(v, T.glob + 10, xinf, xtau);
-          st[1][q] = cnexp(st[1][q], xinf, xtau, dt);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int j = j0 + u * stride;
+          if (j < tot) {
+            const int64_t q = ib + j;
+            double xinf, xtau;
+            if (p > 0) {
+              hhform_gate(vv[u], T.glob + 4, xinf, xtau);
+              st[0][q] = cnexp(sm[u], xinf, xtau, dt);
+            }
+            if (qq > 0) {
+              hhform_gate(vv[u], T.glob + 10, xinf, xtau);
+              st[1][q] = cnexp(sh[u], xinf, xtau, dt);
+            }
+          }
         }
       }
       break;
