@@ -474,10 +474,10 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
       break;
     case T_HHFORM: {
       const int p = (int)T.glob[0], qq = (int)T.glob[1];
-      for (int j0 = lane; j0 < tot; j0 += 2 * stride) {  // (two instances per pass: loads first)
-        double sm[2], sh[2], vv[2];
+      for (int j0 = lane; j0 < tot; j0 += 4 * stride) {  // (four instances per pass: loads first)
+        double sm[4], sh[4], vv[4];
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < 4; ++u) {
           const int j = min(j0 + u * stride, tot - 1);
           const int64_t q = ib + j;
           sm[u] = st[0][q];
@@ -485,7 +485,7 @@ __device__ __forceinline__ void state_distributed(const DTable &T, double *const
           vv[u] = R[((int)nodes[j >> lgG] << lgG) + (j & (G - 1))];
         }
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < 4; ++u) {
           const int j = j0 + u * stride;
           if (j < tot) {
             const int64_t q = ib + j;
