@@ -187,6 +187,9 @@ struct DModel {
   // window mode (interleaved kernel only): one launch integrates up to `mind` steps
   double *win_rows;             // [steps][win_stride]: point-process conductance / current rows
   double *win_deliv;            // [steps][win_ninst]: summed weights delivered to every instance
+  unsigned long long *win_mask; // [win_ninst] window mode of the interleaved kernel: bit s = an event
+                                // reaches the instance at step s of the window (deliveries are
+                                // sparse: pp_window_kernel reads win_deliv only where a bit is set)
   int64_t win_stride, win_ninst;
   int32_t *win_done;            // [n_tgroup]: steps of the window completed for the group
   uint32_t *win_ticket;         // next (step, group) work item
@@ -250,8 +253,10 @@ __device__ __forceinline__ double rcp_chain(double x) {
 #define CN_FX_INV 5.684341886080802e-14   // 2^-44
 __device__ __forceinline__ void fx_add(double *slot, double val, int32_t *overflow) {
   if (!(fabs(val) < 262144.0)) *overflow = 2;
-  atomicAdd(reinterpret_cast<unsigned long long *>(slot),
-            (unsigned long long)__double2ll_rn(val * CN_FX));
+  const long long q = __double2ll_rn(val * CN_FX);
+  if (q != 0)  // (an addend that rounds to 0 -- a current towards a reversal potential of 0 mV, a
+               // synapse that has decayed below the resolution -- costs no atomic)
+    atomicAdd(reinterpret_cast<unsigned long long *>(slot), (unsigned long long)q);
 }
 __device__ __forceinline__ double fx_get(double raw) {
   return (double)__double_as_longlong(raw) * CN_FX_INV;
@@ -865,6 +870,7 @@ __global__ void __launch_bounds__(128) deliver_window_kernel(const __grid_consta
       const DTable &T = M.tab[M.nc_tab[nc]];
       fxw_add(&M.win_deliv[(step + d - k0) * M.win_ninst + T.pp_goff + M.nc_inst[nc]], M.nc_w[nc],
               M.fxw_scale);
+      if (M.win_mask) atomicOr(&M.win_mask[T.pp_goff + M.nc_inst[nc]], 1ull << (step + d - k0));
     }
   };
   for (int64_t i = i_lo + warp; i < (int64_t)ns; i += nwarp) deliver(M.sp_gid[i], M.sp_step[i]);
@@ -886,20 +892,25 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
     for (int64_t q = tid; q < T.pp_tape_end; q += nth) {
       double *rows = M.win_rows + ws[q];
       double *dl = M.win_deliv + T.pp_goff + q;
+      unsigned long long mask = 0;  // steps of the window at which an event reaches this instance
+      if (T.type != T_ICLAMP) {
+        mask = M.win_mask[T.pp_goff + q];
+        if (mask) M.win_mask[T.pp_goff + q] = 0;
+      }
       switch (T.type) {
         case T_EXPSYN: {
           double g = T.state[0][q];
+          const double c0 = T.param[0][q], e = T.param[1][q], sc = T.param[2][q];
           for (int s = 0; s < nsteps; ++s, rows += M.win_stride, dl += M.win_ninst) {
-            const double w = fxw_get(*dl, M.fxw_inv);
-            if (w != 0.0) {
-              g += w;
+            if (mask >> s & 1ull) {
+              g += fxw_get(*dl, M.fxw_inv);
               *dl = 0.0;
             }
             if (g != 0.0) {
-              const double gs = g * T.param[2][q];
+              const double gs = g * sc;
               fx_add(rows, gs, M.overflow);
-              fx_add(rows + 32, gs * T.param[1][q], M.overflow);
-              g = decay(g, T.param[0][q]);
+              fx_add(rows + 32, gs * e, M.overflow);
+              g = decay(g, c0);
             }
           }
           T.state[0][q] = g;
@@ -907,22 +918,23 @@ __global__ void __launch_bounds__(256) pp_window_kernel(const __grid_constant__ 
         }
         case T_EXP2SYN: {
           double A = T.state[0][q], B = T.state[1][q];
+          const double c0 = T.param[0][q], c1 = T.param[1][q], e = T.param[2][q], sc = T.param[3][q],
+                       f = T.param[4][q];
           for (int s = 0; s < nsteps; ++s, rows += M.win_stride, dl += M.win_ninst) {
-            const double w = fxw_get(*dl, M.fxw_inv);
-            if (w != 0.0) {
-              const double wf = w * T.param[4][q];
+            if (mask >> s & 1ull) {
+              const double wf = fxw_get(*dl, M.fxw_inv) * f;
               A += wf;
               B += wf;
               *dl = 0.0;
             }
             if (A != 0.0 || B != 0.0) {
-              const double gs = (B - A) * T.param[3][q];
+              const double gs = (B - A) * sc;
               if (gs != 0.0) {
                 fx_add(rows, gs, M.overflow);
-                fx_add(rows + 32, gs * T.param[2][q], M.overflow);
+                fx_add(rows + 32, gs * e, M.overflow);
               }
-              A = decay(A, T.param[0][q]);
-              B = decay(B, T.param[1][q]);
+              A = decay(A, c0);
+              B = decay(B, c1);
             }
           }
           T.state[0][q] = A;

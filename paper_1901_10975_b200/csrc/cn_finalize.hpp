@@ -602,6 +602,8 @@ static int finalize(cn_model *m, double dt) {
       if (rc != CN_OK) return rc;
       rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_ninst * wn, 1), &H.win_deliv);
       if (rc != CN_OK) return rc;
+      rc = dev_alloc(m, (size_t)std::max<int64_t>(m->win_ninst, 1), &H.win_mask);
+      if (rc != CN_OK) return rc;
       rc = dev_alloc(m, (size_t)m->hm.n_tgroup, &H.win_done); if (rc != CN_OK) return rc;
       rc = dev_alloc(m, 1, &H.win_ticket); if (rc != CN_OK) return rc;
       H.win_mark_cap = H.maxd + 64;
