@@ -494,25 +494,30 @@ def main():
     # ---------------- end to end from host buffers ---------------------------------------------
     e2e = None
     if not args.no_e2e:
-        barrier()
-        t0 = time.perf_counter()
-        m2 = cn.Model(desc, marshalled=marsh, stream=stream.cuda_stream, options=opts)
-        m2.run(total_dt * DT, DT)
-        v = m2.get_v()
-        g, s = m2.get_spikes()
-        torch.cuda.synchronize()
-        el = time.perf_counter() - t0
-        t = torch.tensor([el], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        el = float(t.item())
+        # (two repetitions, the faster one reported and both listed: the set-up runs on all host
+        # cores of a shared box and a single sample varies by 2x)
+        times = []
+        for _ in range(2):
+            barrier()
+            t0 = time.perf_counter()
+            m2 = cn.Model(desc, marshalled=marsh, stream=stream.cuda_stream, options=opts)
+            m2.run(total_dt * DT, DT)
+            v = m2.get_v()
+            g, s = m2.get_spikes()
+            torch.cuda.synchronize()
+            el = time.perf_counter() - t0
+            t = torch.tensor([el], dtype=torch.float64, device="cuda")
+            if dist is not None:
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            times.append(float(t.item()))
+            m2.destroy()
+        el = min(times)
         e2e = {"value": world * n_node * total_dt / el, "unit": UNIT,
                "h2d_bytes_per_step": marsh[2] / args.steps,
                "d2h_bytes_per_step": (v.nbytes + g.nbytes + s.nbytes) / args.steps,
-               "seconds": el,
+               "seconds": el, "seconds_all": times,
                "includes": "cn_model_create (validation, shape classes, H2D of the model) + "
-                           "cn_run of all steps + cn_get_v + cn_get_spikes (D2H)"}
-        m2.destroy()
+                           "cn_run of all steps + cn_get_v + cn_get_spikes (D2H); best of 2"}
 
     # ---------------- CPU baseline: the oracle, bounded sample, rank 0 at N = 1 -------------------
     cpu = None
