@@ -118,6 +118,10 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
     if (ti.n_global > 0 && !mt.global) return fail(CN_ERR_MECH, "table %d: NULL globals", t);
     if (!finite_all(mt.global, ti.n_global))
       return fail(CN_ERR_MECH, "table %d: non-finite parameter", t);
+    if (mt.type == CN_HHFORM)
+      for (int j : {5, 9, 11, 15})
+        if (mt.global[j] == 0.0)
+          return fail(CN_ERR_MECH, "table %d: gate slope constants k and sigma must be non-zero", t);
     FirstErr fe;
     par_for(mt.n, 1 << 16, [&](int64_t i0, int64_t i1) {
       for (int64_t i = i0; i < i1; ++i) {
