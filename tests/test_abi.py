@@ -127,6 +127,15 @@ def test_validation_errors():
     pas = dict(d["mechs"][1]); pas["node"] = pas["node"].copy(); pas["node"][1] = pas["node"][0]
     d["mechs"][1] = pas
     _expect(d, -3)
+    # an HH-form gate with a zero slope constant (its rate functions divide by it)
+    import cn_workloads.networks as NW
+    for key in ("m_k", "h_s"):
+        g = NW.hhform_globals("CaHVA"); g[key] = 0.0
+        d = dict(base)
+        d["mechs"] = list(base["mechs"]) + [
+            {"type": "hhform", "node": np.array([3], np.int32), "params": {"gbar": np.array([1e-4])},
+             "globals": g}]
+        _expect(d, -3)
     # gap junction without a peer node
     for bad in (488.0, -1.0, 2.5):
         d = dict(base)
