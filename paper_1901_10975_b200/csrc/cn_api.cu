@@ -6,8 +6,10 @@
 #include "cn_device.cuh"
 #include "cn_tape.cuh"
 #include "cn_cell.cuh"
+#include "cn_expand.cuh"
 
 #include <algorithm>
+#include <atomic>
 #include <chrono>
 #include <cmath>
 #include <cctype>
@@ -39,6 +41,8 @@ static bool finite_all(const double *x, int64_t n) {
 }
 
 static int build_layout(cn_model *m);
+static void raw_upload(cn_model *m, int dev, int64_t N, const double *cm, const double *ri,
+                       const double *area, const std::vector<RawSrc> &tabs);
 
 extern "C" int cn_model_create(const cn_model_desc *de, cn_model **out) {
   return cn_model_create_opts(de, nullptr, out);
@@ -189,6 +193,32 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
 
   cn_model *m = new (std::nothrow) cn_model();
   if (!m) return fail(CN_ERR_NOMEM, "out of host memory");
+  // A model that is headed for the interleaved kernel: its compact arrays travel to the device on
+  // a thread of their own while the cores below copy the description and compile the layout
+  // (cn_expand.cuh).  Joined before this call returns or fails.
+  std::thread raw_thread;
+  auto raw_join = [&] {
+    if (raw_thread.joinable()) raw_thread.join();
+  };
+  {
+    int tape_mode = -1, dev = 0;
+    int64_t tape_min_cells = 8192;
+    if (const char *e = parsed.get("tape")) tape_mode = std::atoi(e);
+    if (const char *e = parsed.get("tape_min_cells")) tape_min_cells = std::atoll(e);
+    const bool headed = tape_mode == 1 || (tape_mode == -1 && de->n_cell >= tape_min_cells);
+    if (headed && N >= (1 << 16) && de->n_mech <= 20 && cudaGetDevice(&dev) == cudaSuccess) {
+      std::vector<RawSrc> src((size_t)de->n_mech);
+      for (int32_t t = 0; t < de->n_mech; ++t) {
+        const cn_mech_table &mt = de->mech[t];
+        TypeInfo ti;
+        type_info(mt.type, ti);
+        src[t] = RawSrc{mt.node, mt.param, mt.n, ti.n_param, !ti.point && ti.n_param > 0 && mt.n > 0};
+      }
+      m->raw.param.assign((size_t)de->n_mech, nullptr);
+      m->raw.node.assign((size_t)de->n_mech, nullptr);
+      raw_thread = std::thread(raw_upload, m, dev, N, de->cm_uF_cm2, de->ri_MOhm, de->area_um2, src);
+    }
+  }
   try {
     m->options = parsed;
     m->n_cell = de->n_cell;
@@ -224,11 +254,18 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
     m->n_src = n_src;
     m->sp_cap = 16 * (int64_t)de->n_cell + 65536;
     int rc = build_layout(m);
+    if (rc != CN_OK || m->tgrp.empty()) m->raw.cancel.store(true);
+    raw_join();
     if (rc != CN_OK) {
+      m->raw.release();
       delete m;
       return rc;
     }
+    if (m->tgrp.empty()) m->raw.release();
   } catch (const std::bad_alloc &) {
+    m->raw.cancel.store(true);
+    raw_join();
+    m->raw.release();
     delete m;
     return fail(CN_ERR_NOMEM, "out of host memory");
   }
@@ -710,6 +747,7 @@ extern "C" void cn_model_destroy(cn_model *m) {
   if (m->uploaded) cudaStreamSynchronize(m->stream);
   for (auto &pr : m->ktime_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   for (void *p : m->dev_allocs) cudaFree(p);
+  m->raw.release();
   if (m->d_scratch) cudaFree(m->d_scratch);
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);

@@ -101,6 +101,197 @@ static void build_cell_plan(const cn_model *m, const HClass &K, int kc, CellClas
   cc.n_dist = (int32_t)(P.dist.size() - (size_t)cc.dist_base);
 }
 
+// ---------------------------------------------------------------------------------------------
+// interleaved groups: the tapes are expanded on the device (cn_expand.cuh)
+// ---------------------------------------------------------------------------------------------
+
+// the caller's compact arrays -> device; arrays that are there already are left alone.  Runs on a
+// thread of cn_model_create (from the caller's arrays) and, for what is still missing, in
+// finalize() (from the model's copies).  Errors go to RawDev::err (fail() is per thread).
+static void raw_upload(cn_model *m, int dev, int64_t N, const double *cm, const double *ri,
+                       const double *area, const std::vector<RawSrc> &tabs) {
+  RawDev &R = m->raw;
+  if (cudaSetDevice(dev) != cudaSuccess) {
+    R.err = cudaErrorInvalidDevice;
+    return;
+  }
+  auto put = [&R](auto **dst, const auto *src, int64_t n) {
+    if (*dst || R.err != cudaSuccess || R.cancel.load()) return;
+    void *p = nullptr;
+    cudaError_t e = cudaMalloc(&p, (size_t)std::max<int64_t>(n, 1) * sizeof(*src));
+    if (e == cudaSuccess && n > 0)
+      e = cudaMemcpy(p, src, (size_t)n * sizeof(*src), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+      if (p) cudaFree(p);
+      R.err = e;
+      return;
+    }
+    *dst = static_cast<std::remove_reference_t<decltype(*dst)>>(p);
+  };
+  put(&R.cm, cm, N);
+  put(&R.ri, ri, N);
+  put(&R.area, area, N);
+  for (size_t t = 0; t < tabs.size(); ++t) {
+    if (!tabs[t].want) continue;
+    put(&R.node[t], tabs[t].node, tabs[t].n);
+    put(&R.param[t], tabs[t].param, tabs[t].n * tabs[t].n_param);
+  }
+}
+
+// initial states of an instance of a distributed table at v_init (nrn_init: every gate at its
+// steady state)
+static void dist_initial_states(const cn_model *m, const HTable &T, int32_t nd, double *S) {
+  const double v = m->v_init;
+  switch (T.type) {
+    case CN_HH: {
+      double al, be;
+      al = 0.1 * h_vtrap(-(v + 40.0), 10.0); be = 4.0 * std::exp(-(v + 65.0) / 18.0);
+      S[0] = al / (al + be);
+      al = 0.07 * std::exp(-(v + 65.0) / 20.0); be = 1.0 / (std::exp(-(v + 35.0) / 10.0) + 1.0);
+      S[1] = al / (al + be);
+      al = 0.01 * h_vtrap(-(v + 55.0), 10.0); be = 0.125 * std::exp(-(v + 65.0) / 80.0);
+      S[2] = al / (al + be);
+      break;
+    }
+    case CN_HHFORM:
+      S[0] = 1.0 / (1.0 + std::exp((T.glob[4] - v) / T.glob[5]));
+      S[1] = 1.0 / (1.0 + std::exp((T.glob[10] - v) / T.glob[11]));
+      break;
+    case CN_SK: {
+      double ca = m->any_cai ? m->cai0[nd] : 1e-4;
+      if (ca < 1e-9) ca = 1e-9;
+      S[0] = 1.0 / (1.0 + std::pow(T.glob[1] / ca, T.glob[2]));
+      break;
+    }
+    default: break;
+  }
+}
+
+template <class T, class A>
+static int tmp_upload(cn_model *m, const std::vector<T, A> &h, const T **out) {
+  void *p = nullptr;
+  CU(cudaMalloc(&p, std::max<size_t>(h.size(), 1) * sizeof(T)));
+  m->raw.tmp.push_back(p);
+  if (!h.empty()) CU(cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  *out = static_cast<const T *>(p);
+  return CN_OK;
+}
+
+// Fills the tapes (already zeroed) of all interleaved groups; m->hm.tgrp, m->d_node_pos and the
+// arena must be on the device.  Asynchronous on the legacy default stream: finalize() synchronises
+// at its end and releases the temporary arrays.
+static int expand_tapes(cn_model *m, double dt, const std::vector<int32_t> &cell_of_pcell) {
+  const int nt = (int)m->tab.size();
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  RawDev &R = m->raw;
+  if (R.err != cudaSuccess) {  // the early upload failed: once more, from the model's copies
+    R.release();
+    R.err = cudaSuccess;
+  }
+  R.cancel.store(false);
+  if (R.param.empty()) {
+    R.param.assign((size_t)nt, nullptr);
+    R.node.assign((size_t)nt, nullptr);
+  }
+  std::vector<RawSrc> src((size_t)nt);
+  for (int t = 0; t < nt; ++t) {
+    const HTable &T = m->tab[t];
+    src[t] = RawSrc{T.node.data(), T.param.data(), T.n, T.ti.n_param,
+                    !T.ti.point && T.ti.n_param > 0 && T.n > 0};
+  }
+  raw_upload(m, dev, m->N, m->cm.data(), m->ri.data(), m->area.data(), src);
+  if (R.err != cudaSuccess)
+    return fail(R.err == cudaErrorMemoryAllocation ? CN_ERR_NOMEM : CN_ERR_CUDA,
+                "upload of the model arrays failed: %s", cudaGetErrorString(R.err));
+  // per class: tape rows, local parents and children (ascending) of every node
+  std::vector<ExpClass> ec(m->cls.size(), ExpClass{0, 0, 0, 0});
+  std::vector<uint32_t> row;
+  std::vector<int32_t> par, vcopy, cai, chf, ch;
+  for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+    const HClass &K = m->cls[kc];
+    const HTape &P = K.tp;
+    if (P.n_groups == 0) continue;
+    ec[kc] = ExpClass{K.n, (int32_t)row.size(), (int32_t)ch.size(), (int32_t)chf.size()};
+    const int64_t f = m->cell_first[K.rep_cell];
+    std::vector<std::vector<int32_t>> kids((size_t)K.n);
+    for (int j = 0; j < K.n; ++j) {
+      const int32_t p = j ? (int32_t)(m->parent[f + j] - f) : -1;
+      row.push_back(P.row[P.pos_of[j]]);
+      par.push_back(p);
+      if (p >= 0) kids[p].push_back(j);
+      vcopy.push_back((size_t)j < P.vcopy_row.size() ? P.vcopy_row[j] : -1);
+      cai.push_back(m->any_cai && (size_t)j < P.cai_row.size() ? P.cai_row[j] : -1);
+    }
+    int32_t run = 0;
+    for (int j = 0; j < K.n; ++j) {
+      chf.push_back(run);
+      ch.insert(ch.end(), kids[j].begin(), kids[j].end());
+      run += (int32_t)kids[j].size();
+    }
+    chf.push_back(run);
+  }
+  ExpTables E{};
+  int rc;
+#define TUP(vec, ptr)                                  \
+  do {                                                 \
+    rc = tmp_upload(m, vec, &ptr);                     \
+    if (rc != CN_OK) return rc;                        \
+  } while (0)
+  TUP(ec, E.cls); TUP(row, E.row); TUP(par, E.par); TUP(vcopy, E.vcopy); TUP(cai, E.cai);
+  TUP(chf, E.ch_first); TUP(ch, E.ch); TUP(cell_of_pcell, E.cell_of_pcell);
+  TUP(m->cell_first, E.cell_first);
+  E.cai0 = nullptr;
+  if (m->any_cai) TUP(m->cai0, E.cai0);
+  E.tgrp = m->hm.tgrp;
+  E.cm = R.cm; E.ri = R.ri; E.area = R.area;
+  E.tape = m->d_v + m->n_ab;
+  E.dt = dt;
+  E.v_init = m->v_init;
+  const int ntg = (int)m->tgrp.size();
+  expand_static_kernel<<<ntg, 256>>>(E);
+  for (int t = 0; t < nt; ++t) {  // (table after table: the order of the sums is part of the result)
+    const HTable &T = m->tab[t];
+    if (T.type != CN_PAS || T.n == 0) continue;
+    expand_pas_kernel<<<(unsigned)((T.n + 255) / 256), 256>>>(R.node[t], R.param[t], T.n,
+                                                              m->d_node_pos, m->n_ab, m->d_v);
+  }
+  expand_norm_kernel<<<ntg, 256>>>(E);
+  for (int t = 0; t < nt; ++t) {
+    const HTable &T = m->tab[t];
+    if (T.ti.point || T.n == 0 || tape_rows_of(T.ti, T.type) == 0) continue;
+    bool any = false;
+    for (const HClass &K : m->cls)
+      if (K.tp.n_groups > 0 && T.cell_first[K.rep_cell + 1] > T.cell_first[K.rep_cell]) any = true;
+    if (!any) continue;
+    ExpMech X{};
+    X.node = R.node[t];
+    X.param = R.param[t];
+    X.n = T.n;
+    X.n_param = T.ti.n_param;
+    X.n_state = T.ti.n_state;
+    TUP(T.tape_loc, X.tape_loc);
+    X.s_inst = nullptr;
+    if (T.type == CN_SK) {  // the one type whose initial state depends on the node (cai)
+      uvec<double> s((size_t)T.n * T.ti.n_state);
+      par_for(T.n, 1 << 14, [&](int64_t i0, int64_t i1) {
+        for (int64_t i = i0; i < i1; ++i) {
+          double S[CN_MAX_STATE] = {0.0};
+          dist_initial_states(m, T, T.node[i], S);
+          for (int j = 0; j < T.ti.n_state; ++j) s[(size_t)j * T.n + i] = S[j];
+        }
+      });
+      TUP(s, X.s_inst);
+    } else {
+      dist_initial_states(m, T, -1, X.s);
+    }
+    expand_mech_kernel<<<(unsigned)((T.n + 255) / 256), 256>>>(X, R.cm, dt, m->d_v + m->n_ab);
+  }
+#undef TUP
+  CU(cudaGetLastError());
+  return CN_OK;
+}
+
 static int finalize(cn_model *m, double dt) {
   const bool dbg = m->opt("debug") && std::atoi(m->opt("debug")) != 0;
   auto t_prev = std::chrono::steady_clock::now();
@@ -130,25 +321,29 @@ static int finalize(cn_model *m, double dt) {
     maxd = std::max<int64_t>(maxd, ds);
   }
   if (m->n_netcon == 0) mind = 1;
-  // row-normalised static arrays:  c_i = 1e-3 cm_i/dt,  b' = b/c_i,  a' = a/c_parent,
-  // dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
-  uvec<double> invc((size_t)N), bn((size_t)N), an((size_t)N);
+  // Row-normalised static arrays of the WARP-COOPERATIVE groups (the tapes of the interleaved groups
+  // are expanded on the device from the compact arrays, cn_expand.cuh: same operations, same order):
+  //   c_i = 1e-3 cm_i/dt,  b' = b/c_i,  a' = a/c_parent,
+  //   dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
+  const bool host_rows = m->n_cgroup > 0;
+  const int64_t NH = host_rows ? N : 0;
+  auto inv_c = [&](int64_t i) { return 1.0 / (1e-3 * m->cm[i] / dt); };
+  uvec<double> invc((size_t)NH), bn((size_t)NH), an((size_t)NH);
   std::vector<double> dstat((size_t)m->n_pnode, 1.0), rstat((size_t)m->n_pnode, 0.0);
-  // one arena: [schedule-ordered v of the cooperative groups | tapes of the interleaved groups]
-  uvec<double> v0((size_t)(m->n_ab + m->n_tape));
-  double *tape = v0.data() + m->n_ab;
-  uvec<double> dsum((size_t)N), rsum((size_t)N);
-  uvec<int32_t> cell_of_node((size_t)N);
+  uvec<double> v0((size_t)m->n_ab);  // schedule-ordered v of the cooperative groups
+  uvec<double> dsum((size_t)NH), rsum((size_t)NH);
+  uvec<int32_t> cell_of_node((size_t)NH);
   par_for((int64_t)v0.size(), 1 << 20, [&](int64_t i0, int64_t i1) {
     std::fill(v0.begin() + i0, v0.begin() + i1, 0.0);
   });
-  par_for(N, 1 << 20, [&](int64_t i0, int64_t i1) {
+  par_for(NH, 1 << 20, [&](int64_t i0, int64_t i1) {
     std::fill(bn.begin() + i0, bn.begin() + i1, 0.0);
     std::fill(an.begin() + i0, an.begin() + i1, 0.0);
     std::fill(rsum.begin() + i0, rsum.begin() + i1, 0.0);
   });
   // cells are independent (a parent sits in the same cell): all host cores
-  par_for(m->n_cell, 256, [&](int64_t c0, int64_t c1) {
+  if (host_rows)
+   par_for(m->n_cell, 256, [&](int64_t c0, int64_t c1) {
     const int64_t i0 = m->cell_first[c0], i1 = m->cell_first[c1];
     for (int64_t c = c0; c < c1; ++c)
       for (int64_t i = m->cell_first[c]; i < m->cell_first[c + 1]; ++i) cell_of_node[i] = (int32_t)c;
@@ -168,8 +363,9 @@ static int finalize(cn_model *m, double dt) {
         an[i] = a * invc[p];
       }
     }
-  });
-  for (const HTable &T : m->tab)
+   });
+  if (host_rows)
+   for (const HTable &T : m->tab)
     if (T.type == CN_PAS)  // (at most one instance of a table per node: no two threads meet)
       par_for(T.n, 65536, [&](int64_t q0, int64_t q1) {
         for (int64_t i = q0; i < q1; ++i) {
@@ -178,6 +374,8 @@ static int finalize(cn_model *m, double dt) {
           rsum[T.node[i]] += g * e;
         }
       });
+  // a caller node that sits on a tape (node_pos: element of the arena, the tapes come last)
+  auto on_tape = [&](int64_t i) { return m->node_pos[i] >= m->n_ab; };
   // inverse map: (group, slot) -> caller cell
   std::vector<int32_t> cell_of_pcell((size_t)m->n_pcell, -1);
   for (int32_t c = 0; c < m->n_cell; ++c) {
@@ -185,34 +383,10 @@ static int finalize(cn_model *m, double dt) {
     const int32_t cb = g < m->n_cgroup ? m->grp[g].cell_base : m->tgrp[g - m->n_cgroup].cell_base;
     cell_of_pcell[cb + m->cell_slot[c]] = c;
   }
-  // interleaved groups: whole rows of 32 lanes at a time (contiguous writes; the 32 cells are
-  // read as 32 sequential streams); a, b, d, r precede the node's v row.  Run chunk by chunk at
-  // the very end, each chunk's upload overlapping the next chunk's rows (see the arena upload).
-  auto static_rows_of_groups = [&](int64_t ga, int64_t gb) {
-   par_for(gb - ga, 1, [&](int64_t g0, int64_t g1) {
-    for (int64_t g = ga + g0; g < ga + g1; ++g) {
-      const TapeGroup &tg = m->tgrp[g];
-      const HClass &K = m->cls[tg.cls];
-      int64_t f[32];
-      for (int l = 0; l < tg.ncell; ++l) f[l] = m->cell_first[cell_of_pcell[tg.cell_base + l]];
-      for (int j = 0; j < K.n; ++j) {
-        double *rec = tape + tg.tape_base + ((int64_t)K.tp.row[K.tp.pos_of[j]] + 4) * 32;
-        for (int l = 0; l < tg.ncell; ++l) {
-          const int64_t i = f[l] + j;
-          rec[-4 * 32 + l] = an[i];
-          rec[-3 * 32 + l] = bn[i];
-          rec[-2 * 32 + l] = dsum[i] * invc[i];
-          rec[-1 * 32 + l] = rsum[i] * invc[i];
-          rec[l] = m->v_init;
-        }
-      }
-    }
-   });
-  };
-  if (m->n_cgroup > 0)
+  if (host_rows)
     par_for(N, 65536, [&](int64_t i0, int64_t i1) {
       for (int64_t i = i0; i < i1; ++i) {
-        if (m->cell_tape[cell_of_node[i]]) continue;
+        if (on_tape(i)) continue;
         const int64_t q = m->node_pos[i];
         dstat[q] = dsum[i] * invc[i];
         rstat[q] = rsum[i] * invc[i];
@@ -220,30 +394,6 @@ static int finalize(cn_model *m, double dt) {
       }
     });
   lap("static rows");
-  // idle lanes of a ragged tape group: unit diagonal, everything else zero; cai rows
-  for (const TapeGroup &tg : m->tgrp) {
-    const HTape &P = m->cls[tg.cls].tp;
-    for (int j = 0; j < m->cls[tg.cls].n; ++j)
-      for (int l = tg.ncell; l < 32; ++l) tape[tg.tape_base + ((int64_t)P.row[j] + 2) * 32 + l] = 1.0;
-  }
-  for (const TapeGroup &tg : m->tgrp) {  // the copy of v at the head of every mechanism record
-    const HTape &P = m->cls[tg.cls].tp;
-    for (int i = 0; i < m->cls[tg.cls].n; ++i)
-      if (P.vcopy_row[i] >= 0)
-        for (int l = 0; l < 32; ++l)
-          tape[tg.tape_base + (int64_t)P.vcopy_row[i] * 32 + l] = m->v_init;
-  }
-  if (m->any_cai)
-    for (int32_t c = 0; c < m->n_cell; ++c) {
-      if (!m->cell_tape[c]) continue;
-      const TapeGroup &tg = m->tgrp[m->cell_grp[c] - m->n_cgroup];
-      const HTape &P = m->cls[tg.cls].tp;
-      const int64_t f = m->cell_first[c];
-      for (int i = 0; i < m->cls[tg.cls].n; ++i)
-        if (P.cai_row[i] >= 0)
-          tape[tg.tape_base + (int64_t)P.cai_row[i] * 32 + m->cell_slot[c]] = m->cai0[f + i];
-    }
-  lap("idle lanes, v copies, cai");
   // schedule-ordered off-diagonals
   std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
   std::vector<uint32_t> sched_all;
@@ -290,7 +440,7 @@ static int finalize(cn_model *m, double dt) {
   if (m->any_cai) {
     cai.assign((size_t)m->n_pnode, 1e-4);
     for (int64_t i = 0; i < N; ++i)
-      if (!m->cell_tape[cell_of_node[i]]) cai[m->node_pos[i]] = m->cai0[i];
+      if (!on_tape(i)) cai[m->node_pos[i]] = m->cai0[i];
   }
 
   DModel &H = m->hm;
@@ -314,7 +464,7 @@ static int finalize(cn_model *m, double dt) {
     for (const HTable &T : m->tab)
       if (T.ti.point)
         for (int64_t i = 0; i < T.n; ++i)
-          if (!m->cell_tape[cell_of_node[T.node[i]]]) {
+          if (!on_tape(T.node[i])) {
             double &d = dstat[m->node_pos[T.node[i]]];
             d = -std::fabs(d);
           }
@@ -364,26 +514,22 @@ static int finalize(cn_model *m, double dt) {
                   !T.ti.point && j == T.ti.n_dev_param - 1 ? 1.0 : 0.0);
       for (auto &x : st) std::fill(x.begin() + i0, x.begin() + i1, 0.0);
     });
-    // instances are independent (each writes its own elements): all host cores
-    par_for(T.n, 4096, [&](int64_t ii0, int64_t ii1) {
+    // instances are independent (each writes its own elements): all host cores.  (The instances
+    // of a distributed table that live on tapes are written by expand_mech_kernel.)
+    if (T.ti.point || nd > 0)
+     par_for(T.n, 4096, [&](int64_t ii0, int64_t ii1) {
      for (int64_t i = ii0; i < ii1; ++i) {
+      if (T.inst_pos[i] < 0 || (!T.ti.point && T.tape_loc[i] >= 0)) continue;
       const int32_t nd_i = T.node[i];
       double P[CN_MAX_PARAM] = {0.0}, S[CN_MAX_STATE] = {0.0};
       for (int j = 0; j < T.ti.n_param; ++j) P[j] = T.param[(size_t)j * T.n + i];
-      const double scale = 100.0 / m->area[nd_i] * invc[nd_i];
-      const double v = m->v_init;
+      const double ic = inv_c(nd_i);
+      const double scale = 100.0 / m->area[nd_i] * ic;
       switch (T.type) {
-        case CN_HH: {
-          P[4] = invc[nd_i];
-          double al, be;
-          al = 0.1 * h_vtrap(-(v + 40.0), 10.0); be = 4.0 * std::exp(-(v + 65.0) / 18.0);
-          S[0] = al / (al + be);
-          al = 0.07 * std::exp(-(v + 65.0) / 20.0); be = 1.0 / (std::exp(-(v + 35.0) / 10.0) + 1.0);
-          S[1] = al / (al + be);
-          al = 0.01 * h_vtrap(-(v + 55.0), 10.0); be = 0.125 * std::exp(-(v + 65.0) / 80.0);
-          S[2] = al / (al + be);
+        case CN_HH:
+          P[4] = ic;
+          dist_initial_states(m, T, nd_i, S);
           break;
-        }
         case CN_EXPSYN:  // tau -> the cnexp factor 1 - exp(-dt/tau) (the device never needs tau)
           P[2] = scale;
           P[0] = 1.0 - std::exp(-dt / P[0]);
@@ -396,17 +542,10 @@ static int finalize(cn_model *m, double dt) {
           break;
         case CN_ICLAMP: P[3] = scale; break;
         case CN_HHFORM:
-          P[1] = invc[nd_i];
-          S[0] = 1.0 / (1.0 + std::exp((T.glob[4] - v) / T.glob[5]));
-          S[1] = 1.0 / (1.0 + std::exp((T.glob[10] - v) / T.glob[11]));
+        case CN_SK:
+          P[1] = ic;
+          dist_initial_states(m, T, nd_i, S);
           break;
-        case CN_SK: {
-          P[1] = invc[nd_i];
-          double ca = m->any_cai ? m->cai0[nd_i] : 1e-4;
-          if (ca < 1e-9) ca = 1e-9;
-          S[0] = 1.0 / (1.0 + std::pow(T.glob[1] / ca, T.glob[2]));
-          break;
-        }
         case CN_AMPANMDA: P[0] = scale; break;
         case CN_GAP:  // positions in the voltage arena (exact in a double: < 2^53)
           P[0] *= scale;
@@ -414,15 +553,9 @@ static int finalize(cn_model *m, double dt) {
           break;
         default: break;
       }
-      if (!T.ti.point && T.tape_loc[i] >= 0) {  // the instance lives on a tape
-        double *rec = tape + T.tape_loc[i];
-        for (int j = 0; j < T.ti.n_dev_param; ++j) rec[(size_t)j * 32] = P[j];
-        for (int j = 0; j < T.ti.n_state; ++j) rec[(size_t)(T.ti.n_dev_param + j) * 32] = S[j];
-      } else if (T.inst_pos[i] >= 0) {
-        const int64_t q = T.inst_pos[i];
-        for (int j = 0; j < T.ti.n_dev_param; ++j) par[j][q] = P[j];
-        for (int j = 0; j < T.ti.n_state; ++j) st[j][q] = S[j];
-      }
+      const int64_t q = T.inst_pos[i];
+      for (int j = 0; j < T.ti.n_dev_param; ++j) par[j][q] = P[j];
+      for (int j = 0; j < T.ti.n_state; ++j) st[j][q] = S[j];
      }
     });
     for (int j = 0; j < T.ti.n_dev_param; ++j) { UP(par[j], T.d_param[j]); D.param[j] = T.d_param[j]; }
@@ -439,40 +572,18 @@ static int finalize(cn_model *m, double dt) {
     }
   }
   lap("mechanism tables");
-  // the arena (filled above, including the mechanism rows of the tapes) and the programs
+  // the arena [schedule-ordered v of the cooperative groups | tapes of the interleaved groups] and
+  // the programs; the tapes are expanded on the device once the group table is there (below)
   {
     {
       void *p = nullptr;
-      CU(cudaMalloc(&p, std::max<size_t>(v0.size(), 1) * sizeof(double)));
+      CU(cudaMalloc(&p, (size_t)std::max<int64_t>(m->n_ab + m->n_tape, 1) * sizeof(double)));
       m->dev_allocs.push_back(p);
       m->d_v = static_cast<double *>(p);
       if (m->n_ab > 0)
         CU(cudaMemcpy(m->d_v, v0.data(), (size_t)m->n_ab * sizeof(double), cudaMemcpyHostToDevice));
-      // the tapes: static rows of a chunk of groups on all cores, then its upload on a thread of
-      // its own while the cores fill the next chunk (a pageable copy moves ~13 GB/s)
-      const int64_t ntg = (int64_t)m->tgrp.size();
-      const int64_t nch = ntg >= 64 ? 8 : 1;
-      int dev = 0;
-      CU(cudaGetDevice(&dev));
-      std::thread up;
-      cudaError_t up_err = cudaSuccess;
-      for (int64_t c = 0; c < nch && ntg > 0; ++c) {
-        const int64_t ga = ntg * c / nch, gb = ntg * (c + 1) / nch;
-        static_rows_of_groups(ga, gb);
-        if (up.joinable()) up.join();
-        const int64_t e0 = m->tgrp[ga].tape_base, e1 = gb < ntg ? m->tgrp[gb].tape_base : m->n_tape;
-        double *dst = m->d_v + m->n_ab + e0;
-        const double *src = tape + e0;
-        up = std::thread([dev, dst, src, e0, e1, &up_err] {
-          cudaSetDevice(dev);
-          const cudaError_t e =
-              cudaMemcpy(dst, src, (size_t)(e1 - e0) * sizeof(double), cudaMemcpyHostToDevice);
-          if (e != cudaSuccess) up_err = e;
-        });
-      }
-      if (up.joinable()) up.join();
-      if (up_err != cudaSuccess)
-        return fail(CN_ERR_CUDA, "upload of the tapes failed: %s", cudaGetErrorString(up_err));
+      if (m->n_tape > 0)
+        CU(cudaMemsetAsync(m->d_v + m->n_ab, 0, (size_t)m->n_tape * sizeof(double), 0));
     }
     H.v = m->d_v;
     H.tape = m->d_v + m->n_ab;
@@ -497,6 +608,11 @@ static int finalize(cn_model *m, double dt) {
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
     UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg); UP(ttask, dtt);
     H.tgrp = dtg; H.tcls = dtc; H.prog = dpg; H.ttask = dtt;
+    UP(m->node_pos, m->d_node_pos);  // caller-order lookup (cn_get_v, probes, the expansion)
+    if (m->n_tape > 0) {
+      rc = expand_tapes(m, dt, cell_of_pcell);
+      if (rc != CN_OK) return rc;
+    }
     H.tape_W = m->tape_W;
     H.tape_S = m->tape_S;
     H.tape_CH = m->tape_CH;
@@ -520,7 +636,7 @@ static int finalize(cn_model *m, double dt) {
     H.tab[t].cls_cnt = T.d_cls_cnt; H.tab[t].cls_nodeoff = T.d_cls_nodeoff;
     H.tab[t].grp_instbase = T.d_grp_instbase;
   }
-  lap("arena + programs upload");
+  lap("arena, programs, tape expansion");
   // NetCons: CSR by source gid, sorted by delay steps (stable in caller order)
   {
     std::vector<int64_t> order((size_t)m->n_netcon);
@@ -719,8 +835,7 @@ static int finalize(cn_model *m, double dt) {
   H.sp_gid = m->d_sp_gid; H.sp_step = m->d_sp_step; H.n_sp = m->d_nsp; H.sp_cap = m->sp_cap;
   H.overflow = m->d_overflow;
   lap("window buffers, spikes");
-  // caller-order lookup for cn_get_v, probes
-  UP(m->node_pos, m->d_node_pos);
+  // caller-order gather buffer for cn_get_v, probes
   rc = dev_alloc(m, (size_t)std::max<int64_t>(N, 1), &m->d_gather, false); if (rc) return rc;
   if (!m->probe.empty()) {
     std::vector<int64_t> pp(m->probe.size());
@@ -788,6 +903,7 @@ static int finalize(cn_model *m, double dt) {
   // The uploads and memsets above ran on the legacy default stream; the model's stream may be a
   // non-blocking one (torch's are) that does not wait for it: everything lands before the first launch.
   CU(cudaDeviceSynchronize());
+  m->raw.release();
   CU(cudaEventCreate(&m->ev0));
   CU(cudaEventCreate(&m->ev1));
   m->dt = dt;

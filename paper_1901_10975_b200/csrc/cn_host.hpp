@@ -287,8 +287,40 @@ struct Options {
   }
 };
 
+// The caller's compact arrays on the device, from which the tapes of the interleaved groups are
+// expanded (cn_expand.cuh).  A thread of cn_model_create uploads them while the host compiles the
+// layout (joined before create returns: the caller's arrays are not read afterwards); finalize()
+// uploads what is missing from the model's copies and releases everything once the tapes stand.
+struct RawDev {
+  double *cm = nullptr, *ri = nullptr, *area = nullptr;
+  std::vector<double *> param;   // per table: [n_param][n] as given, NULL = not on the device
+  std::vector<int32_t *> node;   // per table
+  std::vector<void *> tmp;       // layout tables of the expansion kernels
+  std::atomic<bool> cancel{false};  // the layout found no use for the rest
+  cudaError_t err = cudaSuccess;
+  void release() {
+    for (double **p : {&cm, &ri, &area})
+      if (*p) { cudaFree(*p); *p = nullptr; }
+    for (double *&p : param)
+      if (p) { cudaFree(p); p = nullptr; }
+    for (int32_t *&p : node)
+      if (p) { cudaFree(p); p = nullptr; }
+    for (void *p : tmp) cudaFree(p);
+    tmp.clear();
+  }
+};
+
+struct RawSrc {  // one table of the description, wherever it lives on the host
+  const int32_t *node;
+  const double *param;
+  int64_t n;
+  int n_param;
+  bool want;  // distributed with parameters (the tables a tape can hold or fold)
+};
+
 struct cn_model {
   Options options;
+  RawDev raw;
   const char *opt(const char *key) const { return options.get(key); }
   // description (deep copy)
   int32_t n_cell = 0;
