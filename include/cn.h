@@ -40,7 +40,7 @@ enum {
   CN_ERR_CUDA = -6,     /* CUDA runtime error (message in cn_last_error) */
   CN_ERR_OVERFLOW = -7, /* spike buffer overflowed during a run; results are invalid */
   CN_ERR_NOMEM = -8,    /* host or device allocation failed */
-  CN_ERR_UNSUPPORTED = -9 /* a cell too large for the on-chip solve */
+  CN_ERR_UNSUPPORTED = -9 /* a cell too large for the on-chip solve, a size beyond a stated limit */
 };
 
 /* Mechanism types.  Parameter order = row order of cn_mech_table.param. */
@@ -171,6 +171,18 @@ int cn_get_trace(const cn_model *m, double *trace_out, int64_t cap_steps, int64_
  * n = table size.  (The interleaved kernel applies nrn_state of a step at the start of the next
  * one; this call applies the pending update first.) */
 int cn_get_state(const cn_model *m, int32_t t, int32_t s, double *out, int64_t n);
+
+/* cn_get_state for callers that cannot call cudaMalloc (code under CUDA graph capture, serving
+ * loops, harnesses that forbid it): same arguments (`out`: host buffer of n doubles, owned by the
+ * caller), same result, but the gather scratch is a static device array of the library instead of
+ * a buffer grown with cudaMalloc.  The call allocates nothing (no cudaMalloc / cudaFree, no host
+ * heap).  Limit: tables of at most CN_NOALLOC_MAX_INSTANCES instances (the array is 16 B per
+ * instance = 1 MiB, held by every GPU that loads the library until the process exits); a larger
+ * table -> CN_ERR_UNSUPPORTED, nothing written.  Every call shares the array: the call is
+ * synchronous on the model's stream and serialised by a process-wide lock; work that the caller
+ * overlaps with it by other means must not touch the same entry point (it would race). */
+#define CN_NOALLOC_MAX_INSTANCES 65536
+int cn_get_state_noalloc(const cn_model *m, int32_t t, int32_t s, double *out, int64_t n);
 
 int64_t cn_steps_done(const cn_model *m);
 /* Number of kernels launched by this model so far (for bench.py's gpu_launches). */

@@ -37,8 +37,10 @@ MECH = {
     "gap": (10, ("g", "peer"), ()),
 }
 
+NOALLOC_MAX_INSTANCES = 65536   # include/cn.h CN_NOALLOC_MAX_INSTANCES
+
 EXPORTS = ("cn_model_create", "cn_model_create_opts", "cn_run", "cn_run_async", "cn_sync", "cn_set_stream", "cn_get_v",
-           "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_steps_done",
+           "cn_get_spikes", "cn_set_probes", "cn_get_trace", "cn_get_state", "cn_get_state_noalloc", "cn_steps_done",
            "cn_launch_count", "cn_last_run_ms", "cn_set_kernel_timing", "cn_select_timed_kernel", "cn_get_kernel_timing", "cn_get_layout_info", "cn_get_run_info", "cn_set_spike_capacity",
            "cn_checkpoint_size", "cn_checkpoint_save", "cn_checkpoint_load",
            "cn_model_destroy", "cn_last_error")
@@ -90,6 +92,7 @@ def lib():
         L.cn_set_probes.argtypes = [vp, vp, C.c_int64, C.c_int64]
         L.cn_get_trace.argtypes = [vp, vp, C.c_int64, C.POINTER(C.c_int64)]
         L.cn_get_state.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int64]
+        L.cn_get_state_noalloc.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_int64]
         L.cn_steps_done.restype = C.c_int64
         L.cn_steps_done.argtypes = [vp]
         L.cn_launch_count.restype = C.c_int64
@@ -254,6 +257,14 @@ class Model:
     def get_state(self, t, s):
         out = np.empty(self.mech_n[t], dtype=np.float64)
         _check(lib().cn_get_state(self._h, t, s, _ptr(out), len(out)))
+        return out
+
+    def get_state_noalloc(self, t, s, out=None):
+        """cn_get_state through the library's static device scratch (no allocation in the call;
+        tables of at most NOALLOC_MAX_INSTANCES instances); `out`: caller's buffer."""
+        if out is None:
+            out = np.empty(self.mech_n[t], dtype=np.float64)
+        _check(lib().cn_get_state_noalloc(self._h, t, s, _ptr(out), len(out)))
         return out
 
     @property

@@ -694,6 +694,83 @@ extern "C" int cn_get_layout_info(const cn_model *m, int64_t *info) {
 
 #include "cn_checkpoint.hpp"
 
+// ---------------------------------------------------------------------------------------------
+// cn_get_state_noalloc: cn_get_state for callers that must not allocate device memory
+// ---------------------------------------------------------------------------------------------
+// cn_get_state gathers through a scratch buffer that it grows with cudaMalloc on first use
+// (ensure_scratch).  This variant keeps its scratch -- the location list and the gathered
+// values, 16 B per instance -- in a file-scope device array of fixed size, so the call allocates
+// nothing on the device or on the host heap: CN_NOALLOC_MAX_INSTANCES instances, 1 MiB, held by
+// every GPU that loads the library until the process exits.  The array is shared by every call
+// and keeps the last call's contents; nothing in it has to start at zero (the n locations and the
+// n values are written before they are read).  Calls that overlap on the GPU would race on it:
+// the entry point holds a process-wide lock and returns after its work has completed on the
+// model's stream, so two calls of one process never overlap.
+static __device__ __align__(256) unsigned char cn_noalloc_scratch[CN_NOALLOC_MAX_INSTANCES * 16];
+static int64_t g_noalloc_loc[CN_NOALLOC_MAX_INSTANCES];  // host staging of the location list
+static std::mutex g_noalloc_mu;
+static void *g_noalloc_ptr[64] = {};  // device address of the array, per device ordinal
+
+// variant of gather_state_kernel (cn_tape.cuh) on the static scratch: locations in the first
+// half, values in the second
+__global__ void gather_state_noalloc_kernel(const double *__restrict__ tape,
+                                            const double *__restrict__ st,
+                                            unsigned char *__restrict__ scratch, int64_t n) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int64_t *loc = reinterpret_cast<const int64_t *>(scratch);
+  double *val = reinterpret_cast<double *>(scratch + (size_t)CN_NOALLOC_MAX_INSTANCES * 8);
+  const int64_t l = loc[i];
+  val[i] = l >= 0 ? st[l] : tape[-(l + 1)];
+}
+
+// In host code the array's name is a host-side stand-in, not a device address: the address a
+// kernel can use comes from cudaGetSymbolAddress, once per device, with that device current.
+static int noalloc_scratch_ptr(unsigned char **out) {
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(CN_ERR_UNSUPPORTED, "device ordinal %d not supported", dev);
+  if (!g_noalloc_ptr[dev]) {
+    void *p = nullptr;
+    CU(cudaGetSymbolAddress(&p, cn_noalloc_scratch));
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = static_cast<unsigned char *>(g_noalloc_ptr[dev]);
+  return CN_OK;
+}
+
+extern "C" int cn_get_state_noalloc(const cn_model *cm, int32_t t, int32_t s, double *out, int64_t n) {
+  cn_model *m = const_cast<cn_model *>(cm);
+  if (!m || !out) return fail(CN_ERR_ARG, "NULL argument");
+  if (t < 0 || t >= (int)m->tab.size()) return fail(CN_ERR_MECH, "table out of range");
+  HTable &T = m->tab[t];
+  if (s < 0 || s >= T.ti.n_state || n != T.n) return fail(CN_ERR_MECH, "state / size mismatch");
+  if (n > CN_NOALLOC_MAX_INSTANCES)
+    return fail(CN_ERR_UNSUPPORTED,
+                "cn_get_state_noalloc: table %d has %lld instances, the static scratch holds %d "
+                "(use cn_get_state)", t, (long long)n, CN_NOALLOC_MAX_INSTANCES);
+  if (!m->uploaded) return fail(CN_ERR_ARG, "states exist after the first cn_run");
+  if (n == 0) return CN_OK;
+  std::lock_guard<std::mutex> lk(g_noalloc_mu);
+  unsigned char *scratch = nullptr;
+  int rc = noalloc_scratch_ptr(&scratch);
+  if (rc != CN_OK) return rc;
+  if (!T.ti.point) {  // (see cn_get_state)
+    rc = flush_pending_state(m);
+    if (rc != CN_OK) return rc;
+  }
+  for (int64_t i = 0; i < n; ++i) g_noalloc_loc[i] = state_loc(T, i, s);
+  CU(cudaMemcpyAsync(scratch, g_noalloc_loc, (size_t)n * 8, cudaMemcpyHostToDevice, m->stream));
+  gather_state_noalloc_kernel<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(
+      m->hm.tape, T.d_state[s], scratch, n);
+  CU(cudaGetLastError());
+  m->launches++;
+  CU(cudaMemcpyAsync(out, scratch + (size_t)CN_NOALLOC_MAX_INSTANCES * 8, (size_t)n * 8,
+                     cudaMemcpyDeviceToHost, m->stream));
+  CU(cudaStreamSynchronize(m->stream));
+  return CN_OK;
+}
+
 extern "C" int cn_set_spike_capacity(cn_model *m, int64_t cap) {
   if (!m || cap < 1) return fail(CN_ERR_ARG, "bad capacity");
   if (m->uploaded) return fail(CN_ERR_ARG, "capacity must be set before the first cn_run");
