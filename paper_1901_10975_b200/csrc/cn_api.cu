@@ -53,6 +53,15 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
   if (!de || !out) return fail(CN_ERR_ARG, "cn_model_create: NULL argument");
   Options parsed;
   if (int rc = parsed.parse(options)) return rc;
+  const bool dbg = parsed.get("debug") && std::atoi(parsed.get("debug")) != 0;
+  auto t_prev = std::chrono::steady_clock::now();
+  auto lap = [&](const char *what) {
+    if (!dbg) return;
+    const auto t = std::chrono::steady_clock::now();
+    fprintf(stderr, "[cn] create %-34s %7.1f ms\n", what,
+            std::chrono::duration<double, std::milli>(t - t_prev).count());
+    t_prev = t;
+  };
   if (de->n_cell < 0 || de->n_node < 0) return fail(CN_ERR_ARG, "negative sizes");
   if (de->n_node >= (int64_t)1 << 31) return fail(CN_ERR_ARG, "n_node must be < 2^31");
   if (de->n_mech < 0 || de->n_mech > CN_MAX_TABLES)
@@ -191,12 +200,14 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
     n_src = std::max(n_src, de->stim_gid[i] + 1);
   }
 
+  lap("validation");
   cn_model *m = new (std::nothrow) cn_model();
   if (!m) return fail(CN_ERR_NOMEM, "out of host memory");
   // A model that is headed for the interleaved kernel: its compact arrays travel to the device on
   // a thread of their own while the cores below copy the description and compile the layout
   // (cn_expand.cuh).  Joined before this call returns or fails.
   std::thread raw_thread;
+  bool raw_started = false;
   auto raw_join = [&] {
     if (raw_thread.joinable()) raw_thread.join();
   };
@@ -217,6 +228,7 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
       m->raw.param.assign((size_t)de->n_mech, nullptr);
       m->raw.node.assign((size_t)de->n_mech, nullptr);
       raw_thread = std::thread(raw_upload, m, dev, N, de->cm_uF_cm2, de->ri_MOhm, de->area_um2, src);
+      raw_started = true;
     }
   }
   try {
@@ -226,9 +238,13 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
     m->cell_first.assign(de->cell_first, de->cell_first + (de->n_cell ? de->n_cell + 1 : 0));
     if (de->n_cell == 0) m->cell_first.assign(1, 0);
     par_assign(m->parent, de->parent, N);
-    par_assign(m->area, de->area_um2, N);
-    par_assign(m->ri, de->ri_MOhm, N);
-    par_assign(m->cm, de->cm_uF_cm2, N);
+    // (area, ri, cm and the parameters of distributed tables that are on their way to the device
+    // already are copied after the layout is known, and only if the host will need them: below)
+    if (!raw_started) {
+      par_assign(m->area, de->area_um2, N);
+      par_assign(m->ri, de->ri_MOhm, N);
+      par_assign(m->cm, de->cm_uF_cm2, N);
+    }
     m->thr.assign(de->thr_mV, de->thr_mV + de->n_cell);
     m->v_init = de->v_init_mV;
     m->celsius = de->celsius;
@@ -240,9 +256,11 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
       type_info(mt.type, T.ti);
       T.n = mt.n;
       par_assign(T.node, mt.node, mt.n);
-      par_assign(T.param, mt.param, mt.n * T.ti.n_param);
+      const bool deferred = raw_started && !T.ti.point && T.ti.n_param > 0 && mt.n > 0;
+      if (!deferred) par_assign(T.param, mt.param, mt.n * T.ti.n_param);
       T.glob.assign(mt.global, mt.global + T.ti.n_global);
     }
+    lap("deep copy");
     m->n_netcon = de->n_netcon;
     par_assign(m->nc_src, de->nc_src_gid, de->n_netcon);
     par_assign(m->nc_tgt_mech, de->nc_tgt_mech, de->n_netcon);
@@ -262,6 +280,40 @@ extern "C" int cn_model_create_opts(const cn_model_desc *de, const char *options
       return rc;
     }
     if (m->tgrp.empty()) m->raw.release();
+    // The host keeps the node arrays and the parameters of a distributed table only where
+    // finalize() reads them: cells on the warp-cooperative kernel, or a device copy that did not
+    // arrive.  Otherwise all it needs is cm and area at the nodes of the point processes.
+    if (raw_started) {
+      const bool on_device = m->raw.err == cudaSuccess && m->raw.cm && m->raw.ri && m->raw.area;
+      if (m->n_cgroup > 0 || !on_device) {
+        par_assign(m->area, de->area_um2, N);
+        par_assign(m->ri, de->ri_MOhm, N);
+        par_assign(m->cm, de->cm_uF_cm2, N);
+      } else {
+        m->node_arrays_host = false;
+        for (int32_t t = 0; t < de->n_mech; ++t) {
+          HTable &T = m->tab[t];
+          if (!T.ti.point) continue;
+          T.pp_cm.resize((size_t)T.n);
+          T.pp_area.resize((size_t)T.n);
+          par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+            for (int64_t i = i0; i < i1; ++i) {
+              T.pp_cm[i] = de->cm_uF_cm2[T.node[i]];
+              T.pp_area[i] = de->area_um2[T.node[i]];
+            }
+          });
+        }
+      }
+    }
+    for (int32_t t = 0; t < de->n_mech; ++t) {
+      HTable &T = m->tab[t];
+      const cn_mech_table &mt = de->mech[t];
+      if (T.ti.point || T.ti.n_param == 0 || mt.n == 0 || !T.param.empty()) continue;
+      const bool on_device = m->raw.err == cudaSuccess && (size_t)t < m->raw.param.size() &&
+                             m->raw.param[t] != nullptr;
+      if (m->n_cgroup > 0 || !on_device) par_assign(T.param, mt.param, mt.n * T.ti.n_param);
+    }
+    lap("layout, upload of the compact arrays joined");
   } catch (const std::bad_alloc &) {
     m->raw.cancel.store(true);
     raw_join();

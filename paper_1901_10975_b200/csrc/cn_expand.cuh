@@ -20,6 +20,46 @@ struct ExpClass {
   int32_t n, node_off, child_off, chf_off;  // chf_off: the class's n + 1 entries of ch_first
 };
 
+// where a caller cell lives: group (warp-cooperative groups first) and slot
+struct ExpCells {
+  const int64_t *cell_first;   // [n_cell + 1]
+  const int32_t *cell_grp, *cell_slot;
+  const GroupInfo *grp;        // warp-cooperative groups
+  const ClassInfo *ccls;       //   and their classes (nodeoff_off into node_off)
+  const int32_t *node_off;
+  const TapeGroup *tgrp;       // interleaved groups
+  const ExpClass *ecls;        //   and their classes
+  const uint32_t *row;
+  int32_t n_cell, n_cgroup;
+  int64_t n_ab;
+};
+
+__device__ __forceinline__ int32_t exp_cell_of(const ExpCells &C, int64_t node) {
+  int32_t lo = 0, hi = C.n_cell;  // the cell with cell_first[c] <= node < cell_first[c + 1]
+  while (hi - lo > 1) {
+    const int32_t mid = (lo + hi) >> 1;
+    if (C.cell_first[mid] <= node) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+// caller node -> element of the voltage arena (the table cn_layout.hpp computes on the host;
+// written here so that 8 B per node need not cross PCIe)
+__global__ void expand_node_pos_kernel(ExpCells C, int64_t n_node, int64_t *__restrict__ node_pos) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_node) return;
+  const int32_t c = exp_cell_of(C, i);
+  const int32_t g = C.cell_grp[c], slot = C.cell_slot[c];
+  const int32_t local = (int32_t)(i - C.cell_first[c]);
+  if (g < C.n_cgroup) {
+    const GroupInfo gi = C.grp[g];
+    node_pos[i] = gi.ab_base + C.node_off[C.ccls[gi.cls].nodeoff_off + local] + slot;
+  } else {
+    const TapeGroup tg = C.tgrp[g - C.n_cgroup];
+    node_pos[i] = C.n_ab + tg.tape_base + ((int64_t)C.row[C.ecls[tg.cls].node_off + local] + 4) * 32 + slot;
+  }
+}
+
 struct ExpTables {
   const ExpClass *cls;       // [n_class]
   const uint32_t *row;       // [node_off + j]: first tape row of the record of local node j
@@ -117,21 +157,26 @@ __global__ void __launch_bounds__(256) expand_norm_kernel(ExpTables E) {
 struct ExpMech {
   const int32_t *node;
   const double *param;     // [n_param][n] as the caller gave them
-  const int64_t *tape_loc; // element of the first parameter row, -1: not on a tape
+  const int32_t *tab_row;  // [class node_off + local node]: first row of the table's block, or -1
   const double *s_inst;    // [n_state][n] or NULL
   int64_t n;
   int32_t n_param, n_state;
   double s[CN_MAX_STATE];
 };
 
-__global__ void expand_mech_kernel(ExpMech X, const double *cm, double dt, double *tape) {
+__global__ void expand_mech_kernel(ExpMech X, ExpCells C, const double *cm, double dt, double *tape) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= X.n) return;
-  const int64_t loc = X.tape_loc[i];
-  if (loc < 0) return;
-  double *rec = tape + loc;
+  const int64_t node = X.node[i];
+  const int32_t c = exp_cell_of(C, node);
+  const int32_t g = C.cell_grp[c];
+  if (g < C.n_cgroup) return;  // a warp-cooperative cell: its instances live in the table arrays
+  const TapeGroup tg = C.tgrp[g - C.n_cgroup];
+  const int32_t r = X.tab_row[C.ecls[tg.cls].node_off + (int32_t)(node - C.cell_first[c])];
+  if (r < 0) return;
+  double *rec = tape + tg.tape_base + (int64_t)r * 32 + C.cell_slot[c];
   for (int j = 0; j < X.n_param; ++j) rec[(int64_t)j * 32] = X.param[(int64_t)j * X.n + i];
-  rec[(int64_t)X.n_param * 32] = exp_invc(cm[X.node[i]], dt);
+  rec[(int64_t)X.n_param * 32] = exp_invc(cm[node], dt);
   for (int j = 0; j < X.n_state; ++j)
     rec[(int64_t)(X.n_param + 1 + j) * 32] = X.s_inst ? X.s_inst[(int64_t)j * X.n + i] : X.s[j];
 }

@@ -177,16 +177,76 @@ static int tmp_upload(cn_model *m, const std::vector<T, A> &h, const T **out) {
   return CN_OK;
 }
 
+#define TUP(vec, ptr)                                  \
+  do {                                                 \
+    rc = tmp_upload(m, vec, &ptr);                     \
+    if (rc != CN_OK) return rc;                        \
+  } while (0)
+
+// Layout tables of the set-up kernels (cn_expand.cuh): per class with interleaved groups the tape
+// rows, local parents and children (ascending) of every node; per caller cell its group and slot.
+// m->hm.grp / cls / node_off / tgrp must be on the device.  The arrays are temporary (RawDev::tmp).
+static int exp_layout_tables(cn_model *m, ExpTables &E, ExpCells &C, std::vector<ExpClass> &ec) {
+  ec.assign(m->cls.size(), ExpClass{0, 0, 0, 0});
+  std::vector<uint32_t> row;
+  std::vector<int32_t> par, vcopy, cai, chf, ch;
+  std::vector<int32_t> fill;
+  for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+    const HClass &K = m->cls[kc];
+    const HTape &P = K.tp;
+    if (P.n_groups == 0) continue;
+    ec[kc] = ExpClass{K.n, (int32_t)row.size(), (int32_t)ch.size(), (int32_t)chf.size()};
+    const int64_t f = m->cell_first[K.rep_cell];
+    const size_t chf0 = chf.size(), ch0 = ch.size();
+    chf.resize(chf0 + (size_t)K.n + 1, 0);
+    for (int j = 0; j < K.n; ++j) {
+      const int32_t p = j ? (int32_t)(m->parent[f + j] - f) : -1;
+      row.push_back(P.row[P.pos_of[j]]);
+      par.push_back(p);
+      if (p >= 0) chf[chf0 + (size_t)p + 1]++;
+      vcopy.push_back((size_t)j < P.vcopy_row.size() ? P.vcopy_row[j] : -1);
+      cai.push_back(m->any_cai && (size_t)j < P.cai_row.size() ? P.cai_row[j] : -1);
+    }
+    for (int j = 0; j < K.n; ++j) chf[chf0 + (size_t)j + 1] += chf[chf0 + (size_t)j];
+    ch.resize(ch0 + (size_t)std::max(K.n - 1, 0));
+    fill.assign(chf.begin() + (std::ptrdiff_t)chf0, chf.begin() + (std::ptrdiff_t)(chf0 + (size_t)K.n));
+    for (int j = 1; j < K.n; ++j) ch[ch0 + (size_t)fill[par[par.size() - (size_t)K.n + (size_t)j]]++] = j;
+  }
+  int rc;
+  TUP(ec, E.cls); TUP(row, E.row); TUP(par, E.par); TUP(vcopy, E.vcopy); TUP(cai, E.cai);
+  TUP(chf, E.ch_first); TUP(ch, E.ch);
+  TUP(m->cell_first, E.cell_first);
+  E.tgrp = m->hm.tgrp;
+  C.cell_first = E.cell_first;
+  TUP(m->cell_grp, C.cell_grp); TUP(m->cell_slot, C.cell_slot);
+  C.grp = m->hm.grp;
+  C.ccls = m->hm.cls;
+  C.node_off = m->hm.node_off;
+  C.tgrp = m->hm.tgrp;
+  C.ecls = E.cls;
+  C.row = E.row;
+  C.n_cell = m->n_cell;
+  C.n_cgroup = m->n_cgroup;
+  C.n_ab = m->n_ab;
+  return CN_OK;
+}
+
 // Fills the tapes (already zeroed) of all interleaved groups; m->hm.tgrp, m->d_node_pos and the
 // arena must be on the device.  Asynchronous on the legacy default stream: finalize() synchronises
 // at its end and releases the temporary arrays.
-static int expand_tapes(cn_model *m, double dt, const std::vector<int32_t> &cell_of_pcell) {
+static int expand_tapes(cn_model *m, double dt, ExpTables E, const ExpCells &C,
+                        const std::vector<ExpClass> &ec, const std::vector<int32_t> &cell_of_pcell) {
   const int nt = (int)m->tab.size();
   int dev = 0;
   CU(cudaGetDevice(&dev));
   RawDev &R = m->raw;
   if (R.err != cudaSuccess) {  // the early upload failed: once more, from the model's copies
-    R.release();
+    for (double **p : {&R.cm, &R.ri, &R.area})
+      if (*p) { cudaFree(*p); *p = nullptr; }
+    for (double *&p : R.param)
+      if (p) { cudaFree(p); p = nullptr; }
+    for (int32_t *&p : R.node)
+      if (p) { cudaFree(p); p = nullptr; }
     R.err = cudaSuccess;
   }
   R.cancel.store(false);
@@ -200,50 +260,19 @@ static int expand_tapes(cn_model *m, double dt, const std::vector<int32_t> &cell
     src[t] = RawSrc{T.node.data(), T.param.data(), T.n, T.ti.n_param,
                     !T.ti.point && T.ti.n_param > 0 && T.n > 0};
   }
+  for (int t = 0; t < nt; ++t)
+    if (src[t].want && !R.param[t] && m->tab[t].param.empty())
+      return fail(CN_ERR_ARG, "internal: the parameters of table %d are neither on the device nor on the host", t);
+  if (!m->node_arrays_host && !(R.cm && R.ri && R.area))
+    return fail(CN_ERR_ARG, "internal: the node arrays are neither on the device nor on the host");
   raw_upload(m, dev, m->N, m->cm.data(), m->ri.data(), m->area.data(), src);
   if (R.err != cudaSuccess)
     return fail(R.err == cudaErrorMemoryAllocation ? CN_ERR_NOMEM : CN_ERR_CUDA,
                 "upload of the model arrays failed: %s", cudaGetErrorString(R.err));
-  // per class: tape rows, local parents and children (ascending) of every node
-  std::vector<ExpClass> ec(m->cls.size(), ExpClass{0, 0, 0, 0});
-  std::vector<uint32_t> row;
-  std::vector<int32_t> par, vcopy, cai, chf, ch;
-  for (size_t kc = 0; kc < m->cls.size(); ++kc) {
-    const HClass &K = m->cls[kc];
-    const HTape &P = K.tp;
-    if (P.n_groups == 0) continue;
-    ec[kc] = ExpClass{K.n, (int32_t)row.size(), (int32_t)ch.size(), (int32_t)chf.size()};
-    const int64_t f = m->cell_first[K.rep_cell];
-    std::vector<std::vector<int32_t>> kids((size_t)K.n);
-    for (int j = 0; j < K.n; ++j) {
-      const int32_t p = j ? (int32_t)(m->parent[f + j] - f) : -1;
-      row.push_back(P.row[P.pos_of[j]]);
-      par.push_back(p);
-      if (p >= 0) kids[p].push_back(j);
-      vcopy.push_back((size_t)j < P.vcopy_row.size() ? P.vcopy_row[j] : -1);
-      cai.push_back(m->any_cai && (size_t)j < P.cai_row.size() ? P.cai_row[j] : -1);
-    }
-    int32_t run = 0;
-    for (int j = 0; j < K.n; ++j) {
-      chf.push_back(run);
-      ch.insert(ch.end(), kids[j].begin(), kids[j].end());
-      run += (int32_t)kids[j].size();
-    }
-    chf.push_back(run);
-  }
-  ExpTables E{};
   int rc;
-#define TUP(vec, ptr)                                  \
-  do {                                                 \
-    rc = tmp_upload(m, vec, &ptr);                     \
-    if (rc != CN_OK) return rc;                        \
-  } while (0)
-  TUP(ec, E.cls); TUP(row, E.row); TUP(par, E.par); TUP(vcopy, E.vcopy); TUP(cai, E.cai);
-  TUP(chf, E.ch_first); TUP(ch, E.ch); TUP(cell_of_pcell, E.cell_of_pcell);
-  TUP(m->cell_first, E.cell_first);
+  TUP(cell_of_pcell, E.cell_of_pcell);
   E.cai0 = nullptr;
   if (m->any_cai) TUP(m->cai0, E.cai0);
-  E.tgrp = m->hm.tgrp;
   E.cm = R.cm; E.ri = R.ri; E.area = R.area;
   E.tape = m->d_v + m->n_ab;
   E.dt = dt;
@@ -260,9 +289,19 @@ static int expand_tapes(cn_model *m, double dt, const std::vector<int32_t> &cell
   for (int t = 0; t < nt; ++t) {
     const HTable &T = m->tab[t];
     if (T.ti.point || T.n == 0 || tape_rows_of(T.ti, T.type) == 0) continue;
+    // first row of the table's block per (class, local node)
+    std::vector<int32_t> tab_row;
     bool any = false;
-    for (const HClass &K : m->cls)
-      if (K.tp.n_groups > 0 && T.cell_first[K.rep_cell + 1] > T.cell_first[K.rep_cell]) any = true;
+    for (size_t kc = 0; kc < m->cls.size(); ++kc) {
+      const HClass &K = m->cls[kc];
+      if (K.tp.n_groups == 0) continue;
+      tab_row.resize((size_t)ec[kc].node_off + (size_t)K.n, -1);
+      if ((size_t)t >= K.tp.tab_row.size() || K.tp.tab_row[t].empty()) continue;
+      for (int j = 0; j < K.n; ++j) {
+        tab_row[(size_t)ec[kc].node_off + (size_t)j] = K.tp.tab_row[t][j];
+        any = any || K.tp.tab_row[t][j] >= 0;
+      }
+    }
     if (!any) continue;
     ExpMech X{};
     X.node = R.node[t];
@@ -270,7 +309,7 @@ static int expand_tapes(cn_model *m, double dt, const std::vector<int32_t> &cell
     X.n = T.n;
     X.n_param = T.ti.n_param;
     X.n_state = T.ti.n_state;
-    TUP(T.tape_loc, X.tape_loc);
+    TUP(tab_row, X.tab_row);
     X.s_inst = nullptr;
     if (T.type == CN_SK) {  // the one type whose initial state depends on the node (cai)
       uvec<double> s((size_t)T.n * T.ti.n_state);
@@ -285,12 +324,12 @@ static int expand_tapes(cn_model *m, double dt, const std::vector<int32_t> &cell
     } else {
       dist_initial_states(m, T, -1, X.s);
     }
-    expand_mech_kernel<<<(unsigned)((T.n + 255) / 256), 256>>>(X, R.cm, dt, m->d_v + m->n_ab);
+    expand_mech_kernel<<<(unsigned)((T.n + 255) / 256), 256>>>(X, C, R.cm, dt, m->d_v + m->n_ab);
   }
-#undef TUP
   CU(cudaGetLastError());
   return CN_OK;
 }
+#undef TUP
 
 static int finalize(cn_model *m, double dt) {
   const bool dbg = m->opt("debug") && std::atoi(m->opt("debug")) != 0;
@@ -327,9 +366,12 @@ static int finalize(cn_model *m, double dt) {
   //   dstat = (c - b - sum_children a + sum static g)/c,  rstat = (sum static g*e)/c
   const bool host_rows = m->n_cgroup > 0;
   const int64_t NH = host_rows ? N : 0;
-  auto inv_c = [&](int64_t i) { return 1.0 / (1e-3 * m->cm[i] / dt); };
   uvec<double> invc((size_t)NH), bn((size_t)NH), an((size_t)NH);
-  std::vector<double> dstat((size_t)m->n_pnode, 1.0), rstat((size_t)m->n_pnode, 0.0);
+  uvec<double> dstat((size_t)m->n_pnode), rstat((size_t)m->n_pnode);
+  par_for(m->n_pnode, 1 << 20, [&](int64_t i0, int64_t i1) {
+    std::fill(dstat.begin() + i0, dstat.begin() + i1, 1.0);
+    std::fill(rstat.begin() + i0, rstat.begin() + i1, 0.0);
+  });
   uvec<double> v0((size_t)m->n_ab);  // schedule-ordered v of the cooperative groups
   uvec<double> dsum((size_t)NH), rsum((size_t)NH);
   uvec<int32_t> cell_of_node((size_t)NH);
@@ -395,7 +437,11 @@ static int finalize(cn_model *m, double dt) {
     });
   lap("static rows");
   // schedule-ordered off-diagonals
-  std::vector<double> a_s((size_t)m->n_ab, 0.0), b_s((size_t)m->n_ab, 0.0);
+  uvec<double> a_s((size_t)m->n_ab), b_s((size_t)m->n_ab);
+  par_for(m->n_ab, 1 << 20, [&](int64_t i0, int64_t i1) {
+    std::fill(a_s.begin() + i0, a_s.begin() + i1, 0.0);
+    std::fill(b_s.begin() + i0, b_s.begin() + i1, 0.0);
+  });
   std::vector<uint32_t> sched_all;
   std::vector<int32_t> nodeoff_all;
   std::vector<ClassInfo> cinfo(m->cls.size());
@@ -405,7 +451,8 @@ static int finalize(cn_model *m, double dt) {
     sched_all.insert(sched_all.end(), K.sched.begin(), K.sched.end());
     nodeoff_all.insert(nodeoff_all.end(), K.node_off.begin(), K.node_off.end());
   }
-  for (int g = 0; g < ng; ++g) {
+  par_for(ng, 64, [&](int64_t g0, int64_t g1) {  // (every group writes its own slots)
+   for (int64_t g = g0; g < g1; ++g) {
     const GroupInfo &gi = m->grp[g];
     const HClass &K = m->cls[gi.cls];
     const int P = 32 / K.G;
@@ -422,25 +469,30 @@ static int finalize(cn_model *m, double dt) {
           b_s[pos] = bn[i];
         }
     }
-  }
+   }
+  });
   lap("coop schedule arrays");
   // thresholds, flags, gids per permuted cell
   std::vector<double> thr((size_t)m->n_pcell, 0.0);
   std::vector<unsigned char> flag((size_t)m->n_pcell, 0);
   std::vector<int32_t> gid_of((size_t)m->n_pcell, -1);
-  for (int32_t pc = 0; pc < m->n_pcell; ++pc) {
-    const int32_t c = cell_of_pcell[pc];
-    if (c < 0) continue;
-    thr[pc] = m->thr[c];
-    flag[pc] = m->v_init > m->thr[c];
-    gid_of[pc] = c;
-  }
+  par_for(m->n_pcell, 1 << 14, [&](int64_t p0, int64_t p1) {
+    for (int64_t pc = p0; pc < p1; ++pc) {
+      const int32_t c = cell_of_pcell[pc];
+      if (c < 0) continue;
+      thr[pc] = m->thr[c];
+      flag[pc] = m->v_init > m->thr[c];
+      gid_of[pc] = c;
+    }
+  });
   // cai per node of the cooperative groups
   std::vector<double> cai;
   if (m->any_cai) {
     cai.assign((size_t)m->n_pnode, 1e-4);
-    for (int64_t i = 0; i < N; ++i)
-      if (!on_tape(i)) cai[m->node_pos[i]] = m->cai0[i];
+    par_for(N, 1 << 16, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i)
+        if (!on_tape(i)) cai[m->node_pos[i]] = m->cai0[i];
+    });
   }
 
   DModel &H = m->hm;
@@ -461,13 +513,22 @@ static int finalize(cn_model *m, double dt) {
     int32_t *dno; UP(nodeoff_all, dno); H.node_off = dno;
     double *p;
     // nodes of warp-cooperative cells that carry point processes: negative static diagonal
-    for (const HTable &T : m->tab)
-      if (T.ti.point)
-        for (int64_t i = 0; i < T.n; ++i)
-          if (!on_tape(T.node[i])) {
-            double &d = dstat[m->node_pos[T.node[i]]];
+    // (one pass per node, not per instance: several point processes may share a node)
+    if (m->n_cgroup > 0) {
+      std::vector<uint8_t> has_pp((size_t)N, 0);
+      for (const HTable &T : m->tab)
+        if (T.ti.point)
+          par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+            for (int64_t i = i0; i < i1; ++i) has_pp[T.node[i]] = 1;  // (all writers store 1)
+          });
+      par_for(N, 1 << 16, [&](int64_t i0, int64_t i1) {
+        for (int64_t i = i0; i < i1; ++i)
+          if (has_pp[i] && !on_tape(i)) {
+            double &d = dstat[m->node_pos[i]];
             d = -std::fabs(d);
           }
+      });
+    }
     UP(dstat, p); H.dstat = p;
     H.ppdr = nullptr;
     {  // point processes on warp-cooperative groups: their conductance / current rows
@@ -523,8 +584,11 @@ static int finalize(cn_model *m, double dt) {
       const int32_t nd_i = T.node[i];
       double P[CN_MAX_PARAM] = {0.0}, S[CN_MAX_STATE] = {0.0};
       for (int j = 0; j < T.ti.n_param; ++j) P[j] = T.param[(size_t)j * T.n + i];
-      const double ic = inv_c(nd_i);
-      const double scale = 100.0 / m->area[nd_i] * ic;
+      // (node arrays off the host: every distributed instance is on a tape and was skipped above)
+      const double cm_i = m->node_arrays_host ? m->cm[nd_i] : T.pp_cm[i];
+      const double area_i = m->node_arrays_host ? m->area[nd_i] : T.pp_area[i];
+      const double ic = 1.0 / (1e-3 * cm_i / dt);
+      const double scale = 100.0 / area_i * ic;
       switch (T.type) {
         case CN_HH:
           P[4] = ic;
@@ -608,9 +672,20 @@ static int finalize(cn_model *m, double dt) {
     TapeGroup *dtg; TapeClass *dtc; uint4 *dpg; TapeTask *dtt;
     UP(m->tgrp, dtg); UP(tcls, dtc); UP(prog, dpg); UP(ttask, dtt);
     H.tgrp = dtg; H.tcls = dtc; H.prog = dpg; H.ttask = dtt;
-    UP(m->node_pos, m->d_node_pos);  // caller-order lookup (cn_get_v, probes, the expansion)
+    lap("arena, programs");
+    // caller node -> arena element on the device (cn_get_v, probes, the expansion): computed
+    // there from the per-cell and per-class tables instead of uploading 8 B per node
+    ExpTables E{};
+    ExpCells C{};
+    std::vector<ExpClass> ec;
+    rc = exp_layout_tables(m, E, C, ec);
+    if (rc != CN_OK) return rc;
+    rc = dev_alloc(m, (size_t)std::max<int64_t>(N, 1), &m->d_node_pos, false);
+    if (rc != CN_OK) return rc;
+    if (N > 0) expand_node_pos_kernel<<<(unsigned)((N + 255) / 256), 256>>>(C, N, m->d_node_pos);
+    lap("layout tables, node positions");
     if (m->n_tape > 0) {
-      rc = expand_tapes(m, dt, cell_of_pcell);
+      rc = expand_tapes(m, dt, E, C, ec, cell_of_pcell);
       if (rc != CN_OK) return rc;
     }
     H.tape_W = m->tape_W;
@@ -636,28 +711,36 @@ static int finalize(cn_model *m, double dt) {
     H.tab[t].cls_cnt = T.d_cls_cnt; H.tab[t].cls_nodeoff = T.d_cls_nodeoff;
     H.tab[t].grp_instbase = T.d_grp_instbase;
   }
-  lap("arena, programs, tape expansion");
+  lap("tape expansion (launches)");
   // NetCons: CSR by source gid, sorted by delay steps (stable in caller order)
   {
-    std::vector<int64_t> order((size_t)m->n_netcon);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(), [&](int64_t x, int64_t y) {
-      if (m->nc_src[x] != m->nc_src[y]) return m->nc_src[x] < m->nc_src[y];
-      return dsteps[x] < dsteps[y];
+    // (a stable counting sort by source on all cores, then every source's few NetCons by delay)
+    std::vector<int64_t> src_first;
+    uvec<int64_t> rank, order((size_t)m->n_netcon);
+    par_bucket(m->n_netcon, m->n_src, [&](int64_t i) { return m->nc_src[i]; }, src_first, rank);
+    par_for(m->n_netcon, 1 << 16, [&](int64_t i0, int64_t i1) {
+      for (int64_t i = i0; i < i1; ++i) order[rank[i]] = i;
     });
-    std::vector<int64_t> src_first((size_t)m->n_src + 1, 0);
-    for (int64_t i = 0; i < m->n_netcon; ++i) src_first[m->nc_src[i] + 1]++;
-    for (int32_t s = 0; s < m->n_src; ++s) src_first[s + 1] += src_first[s];
-    std::vector<int32_t> nd((size_t)m->n_netcon), ntab((size_t)m->n_netcon);
-    std::vector<int64_t> ninst((size_t)m->n_netcon);
-    std::vector<double> nw((size_t)m->n_netcon);
-    for (int64_t j = 0; j < m->n_netcon; ++j) {
-      const int64_t i = order[j];
-      nd[j] = dsteps[i];
-      ntab[j] = m->nc_tgt_mech[i];
-      ninst[j] = m->tab[m->nc_tgt_mech[i]].inst_pos[m->nc_tgt_inst[i]];
-      nw[j] = m->nc_w[i];
-    }
+    par_for(m->n_src, 1024, [&](int64_t s0, int64_t s1) {
+      const auto by_delay = [&](int64_t x, int64_t y) { return dsteps[x] < dsteps[y]; };
+      for (int64_t sg = s0; sg < s1; ++sg) {
+        auto b = order.begin() + src_first[sg], e = order.begin() + src_first[sg + 1];
+        if (!std::is_sorted(b, e, by_delay)) std::stable_sort(b, e, by_delay);
+      }
+    });
+    uvec<int32_t> nd((size_t)m->n_netcon), ntab((size_t)m->n_netcon);
+    uvec<int64_t> ninst((size_t)m->n_netcon);
+    uvec<double> nw((size_t)m->n_netcon);
+    par_for(m->n_netcon, 1 << 16, [&](int64_t j0, int64_t j1) {
+      for (int64_t j = j0; j < j1; ++j) {
+        const int64_t i = order[j];
+        nd[j] = dsteps[i];
+        ntab[j] = m->nc_tgt_mech[i];
+        ninst[j] = m->tab[m->nc_tgt_mech[i]].inst_pos[m->nc_tgt_inst[i]];
+        nw[j] = m->nc_w[i];
+      }
+    });
+    lap("netcons: sort");
     {  // fixed-point scale of the event-weight sums: the largest sum of |w| on one synapse < 2^62
       std::vector<int64_t> toff(m->tab.size() + 1, 0);  // (point tables only: the others get no events)
       for (size_t t = 0; t < m->tab.size(); ++t)
@@ -902,8 +985,11 @@ static int finalize(cn_model *m, double dt) {
 #undef UP
   // The uploads and memsets above ran on the legacy default stream; the model's stream may be a
   // non-blocking one (torch's are) that does not wait for it: everything lands before the first launch.
+  lap("probes");
   CU(cudaDeviceSynchronize());
+  lap("device synchronize");
   m->raw.release();
+  lap("release of the compact arrays");
   CU(cudaEventCreate(&m->ev0));
   CU(cudaEventCreate(&m->ev1));
   m->dt = dt;

@@ -204,7 +204,11 @@ struct HTable {
   std::vector<int64_t> grp_instbase;
   // per-cell CSR of distributed instances sorted by local node
   std::vector<int64_t> cell_first;
-  uvec<int64_t> cell_inst;
+  uvec<int64_t> cell_inst;  // empty: the caller's instances are ordered by node already (identity)
+  int64_t inst(int64_t j) const { return cell_inst.empty() ? j : cell_inst[j]; }
+  // point tables of a model whose node arrays stayed off the host (cn_model::node_arrays_host):
+  // cm and area at the node of every instance
+  uvec<double> pp_cm, pp_area;
 };
 
 struct HTask {
@@ -328,6 +332,7 @@ struct cn_model {
   std::vector<int64_t> cell_first;
   uvec<int32_t> parent;
   uvec<double> area, ri, cm;
+  bool node_arrays_host = true;  // false: area / ri / cm live on the device only (RawDev), see cn_model_create_opts
   std::vector<double> thr;
   double v_init = -65.0, celsius = 6.3;
   std::vector<HTable> tab;

@@ -40,6 +40,26 @@ static int build_layout(cn_model *m) {
   for (int t = 0; t < nt; ++t) {
     HTable &T = m->tab[t];
     if (T.ti.point) continue;
+    {  // instances ordered by node already (the usual case): the CSR is a search per cell
+      std::atomic<bool> increasing{true};
+      par_for(T.n, 1 << 16, [&](int64_t i0, int64_t i1) {
+        for (int64_t i = std::max<int64_t>(i0, 1); i < i1; ++i)
+          if (T.node[i] <= T.node[i - 1]) {
+            increasing.store(false);
+            return;
+          }
+      });
+      if (increasing.load()) {
+        T.cell_inst.clear();
+        T.cell_first.assign((size_t)nc + 1, 0);
+        par_for((int64_t)nc + 1, 1024, [&](int64_t c0, int64_t c1) {
+          for (int64_t c = c0; c < c1; ++c)
+            T.cell_first[c] = std::lower_bound(T.node.begin(), T.node.end(), (int32_t)m->cell_first[c]) -
+                              T.node.begin();
+        });
+        continue;
+      }
+    }
     uvec<int64_t> rank;
     par_bucket(T.n, nc, [&](int64_t i) { return cell_of[T.node[i]]; }, T.cell_first, rank);
     T.cell_inst.resize((size_t)T.n);
@@ -73,7 +93,7 @@ static int build_layout(cn_model *m) {
       if (T.ti.point) continue;
       h = mix64(h, 0xABCD0000ull + (uint64_t)t);
       for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j)
-        h = mix64(h, (uint64_t)(T.node[T.cell_inst[j]] - f));
+        h = mix64(h, (uint64_t)(T.node[T.inst(j)] - f));
     }
     sig[c] = h;
   }
@@ -91,8 +111,8 @@ static int build_layout(cn_model *m) {
       const int64_t cx = T.cell_first[x + 1] - T.cell_first[x];
       if (cx != T.cell_first[y + 1] - T.cell_first[y]) return false;
       for (int64_t j = 0; j < cx; ++j)
-        if (T.node[T.cell_inst[T.cell_first[x] + j]] - fx !=
-            T.node[T.cell_inst[T.cell_first[y] + j]] - fy)
+        if (T.node[T.inst(T.cell_first[x] + j)] - fx !=
+            T.node[T.inst(T.cell_first[y] + j)] - fy)
           return false;
     }
     return true;
@@ -259,7 +279,7 @@ static int build_layout(cn_model *m) {
         const HTable &T = m->tab[t];
         if (T.ti.point || T.type == CN_PAS) continue;
         for (int64_t q = T.cell_first[K.rep_cell]; q < T.cell_first[K.rep_cell + 1]; ++q) {
-          const int x = (int)(T.node[T.cell_inst[q]] - f);
+          const int x = (int)(T.node[T.inst(q)] - f);
           rows[x] += tape_rows_of(T.ti, T.type);
           if (T.type == CN_CADYN) cai[x] = ica[x] = 1;
           if (T.type == CN_SK) cai[x] = 1;
@@ -513,10 +533,14 @@ static int build_layout(cn_model *m) {
   std::vector<int32_t> dist_nodes;
   for (int t = 0; t < nt; ++t) {
     HTable &T = m->tab[t];
-    T.inst_pos.resize((size_t)T.n);
-    par_for(T.n, 1 << 18, [&](int64_t i0, int64_t i1) {
-      std::fill(T.inst_pos.begin() + i0, T.inst_pos.begin() + i1, (int64_t)-1);
-    });
+    // (pas is folded into the static rows: its instances have no place of their own)
+    const bool placed = T.type != CN_PAS;
+    if (placed) {
+      T.inst_pos.resize((size_t)T.n);
+      par_for(T.n, 1 << 18, [&](int64_t i0, int64_t i1) {
+        std::fill(T.inst_pos.begin() + i0, T.inst_pos.begin() + i1, (int64_t)-1);
+      });
+    }
     if (T.ti.point) {
       // instances ordered by group (stable); cooperative groups: slot = local node * G + cell
       // slot in shared memory; tape groups: element of the node's conductance row on the tape
@@ -553,10 +577,12 @@ static int build_layout(cn_model *m) {
       T.pp_tape_begin = T.pp_first[ngc];
       T.n_dev = T.n;
     } else {
-      T.tape_loc.resize((size_t)T.n);
-      par_for(T.n, 1 << 18, [&](int64_t i0, int64_t i1) {
-        std::fill(T.tape_loc.begin() + i0, T.tape_loc.begin() + i1, (int64_t)-1);
-      });
+      if (placed) {
+        T.tape_loc.resize((size_t)T.n);
+        par_for(T.n, 1 << 18, [&](int64_t i0, int64_t i1) {
+          std::fill(T.tape_loc.begin() + i0, T.tape_loc.begin() + i1, (int64_t)-1);
+        });
+      }
       T.cls_cnt.assign(m->cls.size(), 0);
       T.cls_nodeoff.assign(m->cls.size(), 0);
       for (int kc = 0; kc < (int)m->cls.size(); ++kc) {
@@ -565,7 +591,7 @@ static int build_layout(cn_model *m) {
         T.cls_cnt[kc] = (int32_t)(T.cell_first[rc + 1] - T.cell_first[rc]);
         T.cls_nodeoff[kc] = (int32_t)dist_nodes.size();
         for (int64_t j = T.cell_first[rc]; j < T.cell_first[rc + 1]; ++j)
-          dist_nodes.push_back((int32_t)(T.node[T.cell_inst[j]] - m->cell_first[rc]));
+          dist_nodes.push_back((int32_t)(T.node[T.inst(j)] - m->cell_first[rc]));
       }
       T.grp_instbase.assign((size_t)std::max(ngc, 1), 0);
       int64_t base = 0;
@@ -577,7 +603,8 @@ static int build_layout(cn_model *m) {
         base += (int64_t)cnt * K.G;
       }
       T.n_dev = base;
-      par_for(nc, 256, [&](int64_t cc0, int64_t cc1) {
+      if (placed)
+       par_for(nc, 256, [&](int64_t cc0, int64_t cc1) {
        for (int64_t c = cc0; c < cc1; ++c) {
         const int g = m->cell_grp[c];
         if (g < ngc) {
@@ -585,12 +612,12 @@ static int build_layout(cn_model *m) {
           const int64_t b0 = T.grp_instbase[g];
           int64_t kk = 0;
           for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j, ++kk)
-            T.inst_pos[T.cell_inst[j]] = b0 + kk * G + m->cell_slot[c];
-        } else if (T.type != CN_PAS && T.type != CN_CADYN) {
+            T.inst_pos[T.inst(j)] = b0 + kk * G + m->cell_slot[c];
+        } else if (T.type != CN_CADYN) {
           const TapeGroup &tg = m->tgrp[g - ngc];
           const HTape &P = m->cls[tg.cls].tp;
           for (int64_t j = T.cell_first[c]; j < T.cell_first[c + 1]; ++j) {
-            const int64_t i = T.cell_inst[j];
+            const int64_t i = T.inst(j);
             const int32_t local = (int32_t)(T.node[i] - m->cell_first[c]);
             T.tape_loc[i] = tg.tape_base + (int64_t)P.tab_row[t][local] * 32 + m->cell_slot[c];
           }

@@ -51,7 +51,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
     P.tab_row[t].assign(n, -1);
     if (T.type == CN_PAS) continue;  // folded into the static rows
     for (int64_t q = T.cell_first[K.rep_cell]; q < T.cell_first[K.rep_cell + 1]; ++q) {
-      const int x = (int)(T.node[T.cell_inst[q]] - f);
+      const int x = (int)(T.node[T.inst(q)] - f);
       node_mask[x] |= 1u << t;
       if (T.type == CN_CADYN) has_cai[x] = need_ica[x] = 1;
       if (T.type == CN_SK) has_cai[x] = 1;
