@@ -554,3 +554,26 @@ def renumber_nodes(desc: dict, stream="renum") -> dict:
                     for m in desc["mechs"]]
     out["_new_of_old"] = new_of_old
     return out
+
+
+def shuffle_instances(desc: dict, stream="shuf") -> dict:
+    """The same model with the instances of every mechanism table in a seeded random order
+    (NetCon targets follow); `_new_of_old_inst[t]` maps an old instance index to its new one."""
+    out = dict(desc)
+    mechs, maps = [], []
+    for t, m in enumerate(desc["mechs"]):
+        n = len(m["node"])
+        old_of_new = rng.permutation((stream, t), n).astype(np.int64) if n else np.zeros(0, np.int64)
+        new_of_old = np.empty(n, dtype=np.int64)
+        new_of_old[old_of_new] = np.arange(n)
+        mechs.append(_mech(m["type"], m["node"][old_of_new],
+                           {k: v[old_of_new] for k, v in m["params"].items()}, m["globals"]))
+        maps.append(new_of_old)
+    out["mechs"] = mechs
+    nc = dict(desc["netcons"])
+    if len(nc["tgt_inst"]):
+        nc["tgt_inst"] = np.array([maps[tm][ti] for tm, ti in zip(nc["tgt_mech"], nc["tgt_inst"])],
+                                  dtype=np.int64)
+    out["netcons"] = nc
+    out["_new_of_old_inst"] = maps
+    return out

@@ -392,6 +392,31 @@ def test_node_renumbering_invariance(cn, strategy):
     assert [list(x) for x in a.get_spikes()] == [list(x) for x in b.get_spikes()]
 
 
+@pytest.mark.parametrize("which", ["config3", "config5"])
+def test_instance_order_invariance(cn, strategy, which):
+    """The instances of every mechanism table in a random order (tables not ordered by node take
+    the general path of the per-cell instance lists): same voltages, spikes and states, bit for
+    bit -- one distributed instance per node, point-process sums are fixed-point."""
+    desc = W.config3(n_cell=140, syn_per_cell=60) if which == "config3" else \
+        W.config5(n_cell=110, syn_per_cell=40)
+    shuf = W.shuffle_instances(desc)
+    a, b = cn.Model(desc), cn.Model(shuf)
+    a.run(20.0, DT)
+    b.run(20.0, DT)
+    assert len(a.get_spikes()[0]) > 0
+    assert np.array_equal(a.get_v(), b.get_v())
+    assert [list(x) for x in a.get_spikes()] == [list(x) for x in b.get_spikes()]
+    for t, m in enumerate(desc["mechs"]):
+        s = 0
+        while True:
+            try:
+                sa = a.get_state(t, s)
+            except cn.CnError:
+                break
+            assert np.array_equal(sa, b.get_state(t, s)[shuf["_new_of_old_inst"][t]]), (t, s)
+            s += 1
+
+
 @pytest.mark.parametrize("force_g", ["1", "2", "8"])
 def test_lanes_per_cell_variants(cn, force_g, opts):
     opts["tape"] = 0       # the warp-cooperative kernel, G cells per warp
