@@ -912,6 +912,10 @@ extern "C" int cn_debug_cell_trace(long long *out, int reset) {
   return rc;
 }
 
+extern "C" int cn_debug_trace2(long long *out) {
+  return (int)cudaMemcpyFromSymbol(out, cn::g_trace2, sizeof(long long) * 2 * 8 * 16 * 128 * 2);
+}
+
 extern "C" int cn_debug_trace(long long *out) {
   return (int)cudaMemcpyFromSymbol(out, cn::g_trace, sizeof(long long) * 148 * 16 * 8 * 8);
 }

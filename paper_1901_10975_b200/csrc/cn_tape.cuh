@@ -56,6 +56,13 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
       ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
       : "memory");
 }
+__device__ __forceinline__ uint4 lds_u4(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+               : "r"(addr));
+  return v;
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
@@ -210,8 +217,14 @@ constexpr int CN_TMEM_COLS = 256;  // per CTA: two CTAs share the 512 columns of
 #ifdef CN_TRACE
 __device__ long long g_trace[148 * 16 * 8 * 8];
 #define CN_TR(i) if (lane == 0 && it < 8 && blockIdx.x < 148) g_trace[((blockIdx.x * 16 + warp) * 8 + it) * 8 + (i)] = clock64()
+// per record of the backward (B) / forward (F) sweep of item 3 of the first 8 CTAs: clock, record word
+__device__ long long g_trace2[2 * 8 * 16 * 128 * 2];
+#define CN_TR2(dir, j0, j, ey) if (lane == 0 && it == 3 && blockIdx.x < 8 && (j) - (j0) < 128) { \
+    long long *q_ = g_trace2 + ((((dir) * 8 + blockIdx.x) * 16 + warp) * 128 + ((j) - (j0))) * 2; \
+    q_[0] = clock64(); q_[1] = (long long)(ey); }
 #else
 #define CN_TR(i)
+#define CN_TR2(dir, j0, j, ey)
 #endif
 template <int MAXT>
 __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __grid_constant__ DModel M,
@@ -306,6 +319,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
   // arrival); item (s, g) may start once (s - 1, g) is complete (win_done[g] >= s), which its
   // owner -- usually another SM -- publishes with release semantics after all its global writes.
   const bool window = mode & TM_WINDOW;
+  const uint32_t ctl_t = 32u * (uint32_t)((W > 4 && W <= 8) ? 4 : W - 1);
   const uint32_t n_items = (uint32_t)ngrp * (uint32_t)(window ? nsteps : 1);
   // three shared slots for the tickets drawn by thread 0: the ticket drawn at the start of
   // iteration `it` goes to slot (it + 2) % 3 and is read after the barrier at the end of that
@@ -368,9 +382,16 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
       tgn = M.tgrp[nxt % (uint32_t)ngrp];
       tcn = M.tcls[tgn.cls];
       tkn = M.ttask[(size_t)tgn.cls * W + warp];
-      if (PB == 2 && threadIdx.x == 0) load_program(tcn, (it + 1) & 1);
     }
-    if (window && threadIdx.x == 0) item_s[(it + 2) % 3] = atomicAdd(M.win_ticket, 1u);  // the one after
+    // Per-item control duties (ticket, program request, publishing the item) belong to the first
+    // lane of the CONTROL WARP: the warp with the shortest list of the group (ctl_warp: the host
+    // pairs the longest list, warp 0, with the shortest, warp 4, for 5..8 warps).  The
+    // fence + release at the end of an item cost that lane ~2.4 us (measured); warp 0 would
+    // start its -- longest -- forward sweep that much late.  The ticket of the item after the
+    // next is drawn now and stored after the forward sweep, so that nobody waits for the
+    // atomic's return.
+    uint32_t ticket_r = 0;
+    if (window && threadIdx.x == ctl_t) ticket_r = atomicAdd(M.win_ticket, 1u);
     CN_TR(0);
     const uint32_t pb = PB == 2 ? (it & 1u) : 0u;
     mbar_wait(pbar_s + 8 * pb, (PB == 2 ? it >> 1 : it) & 1u);
@@ -393,9 +414,13 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
       ppd = __ldcg(wrow);
       ppr = __ldcg(wrow + 32);
     }
-    for (int j = p0; j < p1; ++j) {
-      const uint4 e = prog[j];
+    // (a running 32-bit shared address: the compiler otherwise rebuilds &prog[j] from constants
+    // in front of every record's load, on the warp's only instruction stream)
+    uint32_t pa = smem_u32(prog + p0);
+    for (int j = p0; j < p1; ++j, pa += 16) {
+      const uint4 e = lds_u4(pa);
       const uint32_t ty = e.y & RT_MASK;
+      CN_TR2(1, p0, j, (uint64_t)e.y | (uint64_t)e.x << 32);
       if (ty == RT_RUN) {
         // a run of plain chain nodes: each hands its contribution to the next in registers
         if (flush) continue;
@@ -544,6 +569,10 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     CN_TR(2);
+    if (threadIdx.x == ctl_t) {
+      if (PB == 2 && has_next) load_program(tcn, (it + 1) & 1);
+      if (window) item_s[(it + 2) % 3] = ticket_r;  // read after the barrier at the end of this iteration
+    }
     // this warp's ring is idle until the next group: start loading it now
     __syncwarp();
     if (has_next && wait_item(nxt, false)) {
@@ -556,9 +585,11 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     // ========================================================================================
     if (!flush) {
       double v_prev = 0.0;
-      for (int j = tk.b0; j < tk.b1; ++j) {
-        const uint4 e = prog[j];
+      uint32_t pab = smem_u32(prog + tk.b0);
+      for (int j = tk.b0; j < tk.b1; ++j, pab += 16) {
+        const uint4 e = lds_u4(pab);
         const uint32_t ty = e.y & RT_MASK;
+        CN_TR2(0, tk.b0, j, (uint64_t)e.y | (uint64_t)e.x << 32);
         if (ty == RT_RUN) {
           // the parent of the run's last node: the node just solved, or a row that keeps its v
           const int q = (int)((e.x >> 16) & 255u);
@@ -654,12 +685,12 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
     }
     // one program buffer: the next group's program is requested first, so that its latency runs
     // beside the fence and the release below
-    if (PB == 1 && has_next && threadIdx.x == 0) load_program(tcn, 0);
+    if (PB == 1 && has_next && threadIdx.x == ctl_t) load_program(tcn, 0);
     // the signal mbarriers this program did not use complete their phase too
     for (int b = (flush ? 0 : tc.n_bar) + (int)threadIdx.x; b < NB; b += (int)blockDim.x)
       mbar_arrive(sbar_s + 8 * b);
     if (window) {
-      if (threadIdx.x == 0) {  // every global write of the CTA for (step, group) is visible first
+      if (threadIdx.x == ctl_t) {  // every global write of the CTA for (step, group) is visible first
         __threadfence();
         asm volatile("fence.proxy.async;" ::: "memory");
         asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(M.win_done + g), "r"(step_in + 1)
