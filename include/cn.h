@@ -12,7 +12,10 @@
  * Conventions
  *   - All pointers in cn_model_desc are HOST pointers; cn_model_create deep-copies, so the
  *     caller may free them on return.  Output pointers are HOST pointers owned by the caller.
- *   - The model owns its device and host memory until cn_model_destroy.
+ *   - The model owns its device and host memory until cn_model_destroy.  Device memory is
+ *     allocated on the CUDA device that is current at cn_model_create (a large model starts
+ *     uploading its arrays there while the layout is compiled) and at the first cn_run: keep
+ *     the same device current for every call on a model.
  *   - Every call returns a status (CN_OK or a negative CN_ERR_*), never throws or aborts;
  *     cn_last_error() gives a thread-local message for the last non-OK return.
  *   - Units (L58-60): mV, ms, uF/cm2, S/cm2 and mA/cm2 for distributed mechanisms; point
@@ -105,7 +108,9 @@ typedef struct {
   const double *stim_t_ms;    /* [n_stim] >= 0; spike step = llround(t/dt) */
 } cn_model_desc;
 
-/* Validate, find shape classes, choose the permutation, upload.  *out is NULL on failure. */
+/* Validate, deep-copy, find shape classes, choose the permutation (no CUDA device is needed for
+ * that; with one, a large model's arrays start travelling to it).  The dt-dependent tables are
+ * built at the first cn_run.  *out is NULL on failure. */
 int cn_model_create(const cn_model_desc *desc, cn_model **out);
 
 /* The same with options: "key=value;key=value" (';', ',' or white space between pairs; values are
