@@ -553,3 +553,33 @@ def test_probe_capacity_and_interior_nodes(cn, strategy):
     assert np.max(np.abs(tr - o.get_trace()[:cap])) <= TOL
     assert np.max(np.abs(g.get_v() - o.get_v())) <= TOL
     assert [list(x) for x in g.get_spikes()] == [list(x) for x in o.get_spikes()]
+
+
+def test_device_memory_returns_after_destroy(cn):
+    """Every device allocation of a model (the arena, tables, the compact arrays that a large
+    model uploads at cn_model_create, scratch) is released by cn_model_destroy -- run or not run,
+    read back or not."""
+    import torch
+    desc = W.config4(n_cell=320, n_types=8, ring_size=64)     # 93,120 nodes: the early upload path
+    def free():
+        torch.cuda.synchronize()
+        return torch.cuda.mem_get_info()[0]
+    cases = (({"tape": 1}, True), ({"tape": 1}, False), ({"tape": 1, "tape_min_group": 32}, True),
+             ({"tape": 0}, True), (None, False))
+
+    def cycle(opts, run):
+        m = cn.Model(desc, options=opts)
+        if run:
+            m.run(2.0, DT)
+            m.get_v()
+            m.get_state(0, 0)
+            m.checkpoint()
+        m.destroy()
+
+    for opts, run in cases:      # first pass: context, lazy loading of every kernel involved
+        cycle(opts, run)
+    base = free()
+    for rep in range(2):
+        for opts, run in cases:
+            cycle(opts, run)
+            assert free() == base, (rep, opts, run, base - free())
