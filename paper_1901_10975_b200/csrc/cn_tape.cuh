@@ -120,7 +120,7 @@ __device__ __forceinline__ void mech_record(const DModel &M, const unsigned char
       case T_HH: {
         double m = CN_RD(mr, 5), h = CN_RD(mr, 6), nn = CN_RD(mr, 7);
         if (adv) {
-          hh_advance(v, q10dt, m, h, nn);
+          hh_advance<false>(v, q10dt, m, h, nn);
           trec[(cur + 5) * 32] = m;
           trec[(cur + 6) * 32] = h;
           trec[(cur + 7) * 32] = nn;
