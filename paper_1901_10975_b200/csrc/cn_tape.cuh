@@ -449,8 +449,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
             a = a1; b = b1; d = d1; vr = vr1;
             ta += 4;
           }
-          continue;
-        }
+        } else {
         double *srow = sys_l + (e.z & 1023u) * 64u;
         double a = CN_RD(rb, 0), b = CN_RD(rb, 1), d = CN_RD(rb, 2), vr = CN_RD(rb, 4) + CN_RD(rb, 3);
 #pragma unroll 1
@@ -468,6 +467,21 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
           rb = rn;
           a = a1; b = b1; d = d1; vr = vr1;
           srow += 64;
+        }
+        }
+        if (e.y & (1u << 26)) {  // the run ends with the top of its chain: contribution to the parent's row
+          double *prow = sys_l + ((e.y >> 16) & 1023u) * 64u;
+          if (e.y & (1u << 27)) {
+            prow[0] += accD;
+            prow[32] += accR;
+          } else {
+            prow[0] = accD;
+            prow[32] = accR;
+          }
+          if (e.w & (1u << 24)) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sbar_s + 8 * ((e.w >> 16) & 255u));
+          }
         }
         continue;
       }

@@ -440,10 +440,17 @@ static int build_tape_program(cn_model *m, HClass &K) {
   // WAIT records go in front of the record that needs them (a wait that an earlier wait of the
   // same warp already covers is dropped: positions on one warp only grow).  Plain chain nodes
   // that follow one another inside a chunk are merged into RUN records.
-  struct Fin { int type; int pre; int cnt; int w2, pre2; };  // type 2 = WAIT, 3 = RUN, 4 = CHUNK
+  // A run may end with the TOP of its chain: a node like the plain ones, except that its contribution
+  // goes to its parent's row (store / add, possibly signalled) instead of to the next record in
+  // registers (Fin::tail): one record less per chain for the interpreter.
+  struct Fin { int type; int pre; int cnt; int w2, pre2; bool tail = false; };  // type 2 = WAIT, 3 = RUN, 4 = CHUNK
   std::vector<std::vector<Fin>> fin(W);
   std::vector<std::vector<std::pair<uint32_t, uint32_t>>> chunks(W);  // (first row in segment, rows)
   const uint32_t S = (uint32_t)m->tape_S;
+  auto x_parent_row_ok = [&](const Rec &r) {  // the parent collects contributions in a shared row
+    const int x = r.node;
+    return x > 0 && (erec(par[x]).flags & RF_HAS_ACC) && !erec(par[x]).tm;
+  };
   for (int w = 0; w < W; ++w) {
     std::vector<int> seen(W, -1);
     uint32_t fill = CH + 1;  // rows used in the current chunk (none open yet)
@@ -466,11 +473,15 @@ static int build_tape_program(cn_model *m, HClass &K) {
         fresh = true;
       }
       const bool plain = r.type == 0 && (r.flags & ~(uint32_t)RF_FWD_IN) == RK_FWD;
-      if (plain && !fresh && fin[w].back().type == 3 && fin[w].back().cnt < 255 &&
-          (r.flags & RF_FWD_IN) && recs[w][i - 1].tm == r.tm &&
+      const uint32_t kind = r.flags & RK_KIND;
+      const bool chain_top = r.type == 0 && (kind == RK_STORE || kind == RK_ADD) &&
+                             (r.flags & ~(uint32_t)(RK_KIND | RF_SIG_F)) == RF_FWD_IN && x_parent_row_ok(r);
+      if ((plain || chain_top) && !fresh && fin[w].back().type == 3 && !fin[w].back().tail &&
+          fin[w].back().cnt < 255 && (r.flags & RF_FWD_IN) && recs[w][i - 1].tm == r.tm &&
           recs[w][i - 1].srow + 1 == r.srow) {
         r.fidx = (int)fin[w].size() - 1;
         fin[w].back().cnt++;
+        fin[w].back().tail = chain_top;
         continue;
       }
       r.fidx = (int)fin[w].size();
@@ -509,9 +520,15 @@ static int build_tape_program(cn_model *m, HClass &K) {
       const Rec &r = recs[w][F.pre];
       const int x = r.node;
       if (F.type == 3) {
+        uint32_t y = (uint32_t)RT_RUN, wv = r.row;
+        if (F.tail) {  // the run's last node stores / adds its contribution to its parent's row
+          const Rec &t = recs[w][F.pre + F.cnt - 1];
+          y |= erec(par[t.node]).srow << 16 | 1u << 26 | ((t.flags & RK_KIND) == RK_ADD ? 1u << 27 : 0u);
+          if (t.flags & RF_SIG_F) wv |= (uint32_t)t.sig << 16 | 1u << 24;
+        }
         P.prog.push_back(make_uint4(r.ring | (uint32_t)F.cnt << 16 |
                                         ((r.flags & RF_FWD_IN) ? 1u << 24 : 0u),
-                                    (uint32_t)RT_RUN, r.srow | (r.tm ? 1u << 20 : 0u), r.row));
+                                    y, r.srow | (r.tm ? 1u << 20 : 0u), wv));
       } else if (r.type == 1) {
         P.prog.push_back(make_uint4(r.ring, r.flags | r.row << 16, r.srow | (uint32_t)r.sig << 16,
                                     node_mask[x]));
@@ -656,7 +673,11 @@ static int build_tape_program(cn_model *m, HClass &K) {
           e.x = 0;
         }
         const bool is_run = (e.y & RT_MASK) == RT_RUN;
-        if (is_run) e.x = (e.x & ~(255u << 16)) | (uint32_t)units[u].cnt << 16;  // (merged runs)
+        if (is_run) {  // (merged runs; the tail fields belong to the forward record only)
+          e.x = (e.x & ~(255u << 16)) | (uint32_t)units[u].cnt << 16;
+          e.y = (uint32_t)RT_RUN;
+          e.w &= 0xFFFFu;
+        }
         const int pu = punit[u];
         if (pu >= 0 && units[pu].w != w) {
           const int wp = units[pu].w;
@@ -718,13 +739,22 @@ static int build_tape_program(cn_model *m, HClass &K) {
           } else if ((fl & RT_MASK) == RT_WAIT) {
             if (!bar_done[e.z & 0xFFFFu]) break;
           } else if ((fl & RT_MASK) == RT_RUN) {
-            for (uint32_t i = 0; i < ((e.x >> 16) & 255u); ++i) {
+            const uint32_t cnt = (e.x >> 16) & 255u;
+            for (uint32_t i = 0; i < cnt; ++i) {
               const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + i]
                                              : node_of_srow[(e.z & 1023u) + i];
-              if (node_mask[x] || acc[x] != 0 || !fwd[x] || ch[x].size() > 1 ||
+              const bool tail = i + 1 == cnt && (e.y >> 26 & 1u);
+              if (node_mask[x] || acc[x] != 0 || (!fwd[x]) != tail || ch[x].size() > 1 ||
                   (ch[x].size() == 1 && (!done_e[ch[x][0]] || !fwd[ch[x][0]])) ||
                   (ch[x].size() == 1) != (i > 0 || (e.x >> 24 & 1u)))
                 return fail(CN_ERR_TOPOLOGY, "internal: tape program (run)");
+              if (tail) {
+                const int p = node_of_srow[(e.y >> 16) & 1023u];
+                if (x == 0 || p != par[x] || ((e.y >> 27 & 1u) == 0) != (acc[p] == 0))
+                  return fail(CN_ERR_TOPOLOGY, "internal: tape program (run tail)");
+                acc[p]++;
+                if (e.w >> 24 & 1u) bar_done[(e.w >> 16) & 255u] = 1;
+              }
               done_e[x] = 1;
             }
           } else if ((fl & RT_MASK) == RT_MECH) {
