@@ -87,12 +87,13 @@ struct TapeTask {
 //   RUN   x = ring byte offset of the first node's record (16) | nodes in the run (8) | first
 //             node takes a contribution in registers (bit 24) | backward: v of the run's parent
 //             comes from the parent's system row, z bits 21..30 (bit 25)
-//         y = RT_RUN | forward: the run's last node is the top of its chain (bit 26) and stores /
+//         y = RT_RUN | backward: wait for mbarrier bits 16..23 first (bit 24) | forward: the run's
+//             last node is the top of its chain (bit 26) and stores /
 //             adds (bit 27) its contribution to its parent's system row (bits 16..25)
 //         z = system row of the first node (10), or, with bit 20 set, its slot in the warp's share
 //             of tensor memory     w = first tape row of the first node's record (16) | forward,
 //             chain top: it arrives on mbarrier bits 16..23 (bit 24)
-//   ELIM  x = ring byte offset (16)
+//   ELIM  x = ring byte offset (16) | forward: wait for mbarrier bits 16..23 first (bit 24)
 //         y = flags (16) | forward: mbarrier the record arrives on (RF_SIG_F); backward copy:
 //             mbarrier to wait for (RF_WAIT_B); the backward copy arrives on mbarrier x (RF_SIG_B)
 //         z = own system row (10) | parent's system row (10)

@@ -509,6 +509,7 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
       double *srow = sys_l + (e.z & 1023u) * 64u;
       if (ty == RT_ELIM) {
         if (flush) continue;
+        if (e.x & (1u << 24)) mbar_wait(sbar_s + 8 * ((e.x >> 16) & 255u), sphase);  // (its own wait)
         const double a = CN_RD(rb, 0), b = CN_RD(rb, 1);
         double D = CN_RD(rb, 2), R = CN_RD(rb, 4) + CN_RD(rb, 3);
         if (fl & RF_FWD_IN) {
@@ -606,6 +607,8 @@ __global__ void __launch_bounds__(MAXT, 512 / MAXT) tape_step_kernel(const __gri
         CN_TR2(0, tk.b0, j, (uint64_t)e.y | (uint64_t)e.x << 32);
         if (ty == RT_RUN) {
           // the parent of the run's last node: the node just solved, or a row that keeps its v
+          // (a parent on another warp: the run waits for it itself)
+          if (e.y & (1u << 24)) mbar_wait(sbar_s + 8 * ((e.y >> 16) & 255u), sphase);
           const int q = (int)((e.x >> 16) & 255u);
           if (e.x & (1u << 25)) v_prev = sys_l[((e.z >> 21) & 1023u) * 64u + 32];
           double *trow = tape_l + ((e.w & 0xFFFFu) + 5u * (uint32_t)q + 4u) * 32u;

@@ -466,11 +466,21 @@ static int build_tape_program(cn_model *m, HClass &K) {
       r.ring = ((uint32_t)((chunks[w].size() - 1) % S) * CH + fill) * 256u;
       fill += r.len;
       chunks[w].back().second = fill;
+      int n_wait = 0;
       for (auto &d : r.deps) {
         if (seen[d.first] >= d.second) continue;
         seen[d.first] = d.second;
         fin[w].push_back(Fin{2, -1, 0, d.first, d.second});
         fresh = true;
+        ++n_wait;
+      }
+      // a single wait in front of an elimination record travels in the record itself (one record
+      // less on the warps that eliminate the upper nodes: the forward critical path)
+      int emb_w = -1, emb_pre = -1;
+      if (n_wait == 1 && r.type == 0 && (r.flags & ~(uint32_t)RF_FWD_IN) != RK_FWD) {
+        emb_w = fin[w].back().w2;
+        emb_pre = fin[w].back().pre2;
+        fin[w].pop_back();
       }
       const bool plain = r.type == 0 && (r.flags & ~(uint32_t)RF_FWD_IN) == RK_FWD;
       const uint32_t kind = r.flags & RK_KIND;
@@ -485,7 +495,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
         continue;
       }
       r.fidx = (int)fin[w].size();
-      fin[w].push_back(Fin{plain ? 3 : r.type, i, 1, -1, -1});
+      fin[w].push_back(Fin{plain ? 3 : r.type, i, 1, emb_w, emb_pre});
     }
     if (fin[w].size() > 2047) return give_up();  // 12-bit backward positions
     HTask &Tk = P.task[w];
@@ -540,7 +550,9 @@ static int build_tape_program(cn_model *m, HClass &K) {
             r.srow | (uint32_t)(x && (erec(par[x]).flags & RF_HAS_ACC) ? erec(par[x]).srow : 0) << 10 |
             (uint32_t)(P.has_pp[x] ? P.pp_ord[x] : 0) << 21;
         const uint32_t ew = r.row | (uint32_t)(node_mask[x] ? P.vcopy_row[x] : 0) << 16;
-        P.prog.push_back(make_uint4(r.ring, ey, ez, ew));
+        uint32_t ex = r.ring;
+        if (F.w2 >= 0) ex |= (uint32_t)recs[F.w2][F.pre2].sig << 16 | 1u << 24;  // forward: wait first
+        P.prog.push_back(make_uint4(ex, ey, ez, ew));
       }
     }
     Tk.p1 = (int)P.prog.size();
@@ -645,8 +657,8 @@ static int build_tape_program(cn_model *m, HClass &K) {
         }
       }
     }
-    // positions in the backward lists (a run whose parent sits on another warp is preceded by a
-    // WAIT record; a single record carries its wait itself), signals, waits, encoding
+    // positions in the backward lists (a unit whose parent sits on another warp carries the wait for
+    // it itself, run or single record), signals, waits, encoding
     std::vector<int> idxb(nu, 0), sigid_b(nu, -1);
     std::vector<uint8_t> sig_b(nu, 0);
     for (int w = 0; w < W; ++w) {
@@ -655,7 +667,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
         const bool remote = punit[u] >= 0 && units[punit[u]].w != w;
         const bool is_run = fin[w][units[u].fin_idx].type == 3;
         if (remote) sig_b[punit[u]] = 1;
-        if (remote && is_run) ++pos;
+        (void)is_run;  // (a run carries the wait for a remote parent itself, like a single record)
         idxb[u] = pos++;
       }
     }
@@ -684,7 +696,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
           const int posb = (P.task[wp].p1 - P.task[wp].p0) + idxb[pu] + 1;
           if (posb > 4095) return give_up();
           if (is_run) {
-            P.prog.push_back(make_uint4(0u, (uint32_t)RT_WAIT, (uint32_t)sigid_b[pu], 0u));
+            if (seen[wp] < posb) e.y |= (uint32_t)sigid_b[pu] << 16 | 1u << 24;
           } else if (seen[wp] < posb) {
             e.y |= RF_WAIT_B | (uint32_t)sigid_b[pu] << 16;
           }
@@ -763,6 +775,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
             acc[x] = 1;
             done_m[x] = 1;
           } else {
+            if ((e.x >> 24 & 1u) && !bar_done[(e.x >> 16) & 255u]) break;  // (its own wait)
             const int x = (fl & RF_TMEM) ? node_of_slot[w][e.z & 1023u] : node_of_srow[e.z & 1023u];
             int want = node_mask[x] ? 1 : 0;
             for (int32_t c : ch[x]) {
@@ -803,6 +816,7 @@ static int build_tape_program(cn_model *m, HClass &K) {
           if ((fl & RT_MASK) == RT_WAIT) {
             if (!bar_done[e.z & 0xFFFFu]) break;
           } else if ((fl & RT_MASK) == RT_RUN) {
+            if ((e.y >> 24 & 1u) && !bar_done[(e.y >> 16) & 255u]) break;  // (its own wait)
             for (int i = (int)((e.x >> 16) & 255u) - 1; i >= 0; --i) {
               const int x = (e.z >> 20 & 1u) ? node_of_slot[w][(e.z & 1023u) + (uint32_t)i]
                                              : node_of_srow[(e.z & 1023u) + (uint32_t)i];
